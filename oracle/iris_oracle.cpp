@@ -1,0 +1,575 @@
+// ORACLE -- TEST INFRASTRUCTURE ONLY.  Not part of the product path.
+//
+// Plain, slow, float64, scalar C++ restatement of the IRIS-SO hot path of arxiv/paper_2607_01338
+// (PAPER.md sections 3-4), written from the paper's equations in the paper's order and notation.
+// It shares no code, header, table or constant generator with the CUDA path
+// (paper_2607_01338_b200/csrc) and neither includes the other.  Only tests/, __graft_entry__.smoke()
+// and bench.py's cpu_baseline / --impl reference legs may call it.
+//
+// Every function cites the passage it follows.  Readings of garbled / silent passages are the ones
+// listed in DESIGN.md ("Readings") and SURVEY.md section 8(c).
+//
+// Pins (tests/test_oracle_pins.py): every function below is pinned by closed forms, limits,
+// invariants or brute force -- none is "parity unpinned".
+//
+// Units: CGS throughout.  Field arrays are float32 [nz][ny][nx] (x fastest, k = 0 far side) and are
+// widened to double on load; every intermediate and every output is double.
+
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <limits>
+#include <vector>
+
+namespace {
+
+// O1 constants: CODATA-2018 exact SI values converted to CGS.
+constexpr double kH = 6.62607015e-27;    // erg s
+constexpr double kK = 1.380649e-16;      // erg / K
+constexpr double kC = 2.99792458e10;     // cm / s
+constexpr double kPi = 3.14159265358979323846;
+
+}  // namespace
+
+extern "C" {
+
+// Parameter record of the oracle (declared here on its own; the CUDA path has its own struct).
+struct orc_config {
+  int32_t nx, ny, nz;
+  double cell_cm;
+  int32_t n_levels;
+  const double *energy_K, *weight, *einstein_A, *coll_down_ref;
+  double coll_T_ref, coll_T_exp;
+  int32_t line_upper, line_lower;
+  double nu0_Hz, mol_mass_g, abundance, microturb_cms, T_bar, T_cmb, T_inf;
+  int32_t dust_on;
+  double kappa_gas_cm2_g, mass_per_H2_g;
+  int32_t nv;
+  double v0_cms, dv_cms;
+  int32_t subtract_continuum, subtract_space, out_unit;
+  double beam_fwhm_px, noise_mu, noise_sigma;
+  int32_t noise_gamma_mode;
+  uint64_t seed;
+};
+
+// Planck function B_nu(T), Eq. 3.2.1 = Eq. 3.6.2 = Eq. 4.9.1.
+// T <= 0 gives 0 (no radiation field; "pure" OT case).
+double orc_planck(double nu, double T) {
+  if (!(T > 0.0)) return 0.0;
+  return 2.0 * kH * nu * nu * nu / (kC * kC) / std::expm1(kH * nu / (kK * T));
+}
+
+// Inverse of Eq. 4.9.1: Planck brightness temperature of an intensity.
+// Reading R7: odd extension for I < 0, T_B(0) = 0.
+double orc_planck_TB(double nu, double I) {
+  if (I == 0.0) return 0.0;
+  double a = std::fabs(I);
+  double T = (kH * nu / kK) / std::log1p(2.0 * kH * nu * nu * nu / (kC * kC * a));
+  return I < 0.0 ? -T : T;
+}
+
+// Eq. 4.9.2: T_RJ = c^2 I / (2 k nu^2).
+double orc_rayleigh_jeans_T(double nu, double I) { return kC * kC * I / (2.0 * kK * nu * nu); }
+
+// ---------------------------------------------------------------------------------------------
+// O3  Level balance, Eq. 3.6.1 - 3.6.3 with Eq. 3.7.1 - 3.7.2.
+// Builds the transition rates R[i*N + j] = C_ij + A_ij + B_ij J_ij   (i -> j, per unit n_i, i != j).
+//   C_ij = K_ij n_H2                                   (Eq. 3.6.3, single partner H2)
+//   K_ul(T) = K_ul(T_ref) (T / T_ref)^p for u > l      (input table)
+//   K_lu = K_ul (g_u / g_l) exp(-(E_u - E_l) / T_gas)  (Eq. 3.7.2, detailed balance)
+//   B_ul = c^2 / (2 h nu^3) A_ul,  B_lu = (g_u / g_l) B_ul   (Eq. 3.7.1)
+//   J_ul = B_nu_ul(T_bar)                              (Eq. 3.6.2, reading G2: the temperature is T_bar)
+void orc_rates(const orc_config *c, double nH2, double Tgas, double *R) {
+  const int N = c->n_levels;
+  for (int i = 0; i < N * N; ++i) R[i] = 0.0;
+  for (int u = 1; u < N; ++u) {
+    for (int l = 0; l < u; ++l) {
+      const double dE = c->energy_K[u] - c->energy_K[l];   // (E_u - E_l) / k, Kelvin
+      const double gr = c->weight[u] / c->weight[l];
+      double down = 0.0, up = 0.0;
+      const double Kul = c->coll_down_ref[u * N + l];
+      if (Kul != 0.0) {
+        const double K = Kul * std::pow(Tgas / c->coll_T_ref, c->coll_T_exp);
+        down += K * nH2;
+        up += K * gr * std::exp(-dE / Tgas) * nH2;
+      }
+      const double A = c->einstein_A[u * N + l];
+      if (A != 0.0) {
+        const double nu = kK * dE / kH;
+        const double Bul = kC * kC / (2.0 * kH * nu * nu * nu) * A;
+        const double Blu = gr * Bul;
+        const double J = orc_planck(nu, c->T_bar);
+        down += A + Bul * J;
+        up += Blu * J;
+      }
+      R[u * N + l] = down;
+      R[l * N + u] = up;
+    }
+  }
+}
+
+// Statistical-equilibrium matrix of Eq. 3.6.1: (M x)_i = sum_{j != i} [x_j R_ji - x_i R_ij].
+// Row 0 is NOT yet replaced here (used by the stationarity pin).
+void orc_balance_matrix(const orc_config *c, double nH2, double Tgas, double *M) {
+  const int N = c->n_levels;
+  std::vector<double> R(N * N);
+  orc_rates(c, nH2, Tgas, R.data());
+  for (int i = 0; i < N; ++i) {
+    double out = 0.0;
+    for (int j = 0; j < N; ++j) {
+      if (j == i) continue;
+      M[i * N + j] = R[j * N + i];
+      out += R[i * N + j];
+    }
+    M[i * N + i] = -out;
+  }
+}
+
+// Dense partial-pivot Gaussian elimination, A x = b, A is n x n row-major (destroyed).
+static void solve_ge(int n, double *A, double *b, double *x) {
+  for (int k = 0; k < n; ++k) {
+    int p = k;
+    double best = std::fabs(A[k * n + k]);
+    for (int r = k + 1; r < n; ++r)
+      if (std::fabs(A[r * n + k]) > best) { best = std::fabs(A[r * n + k]); p = r; }
+    if (p != k) {
+      for (int j = 0; j < n; ++j) { double t = A[k * n + j]; A[k * n + j] = A[p * n + j]; A[p * n + j] = t; }
+      double t = b[k]; b[k] = b[p]; b[p] = t;
+    }
+    for (int r = k + 1; r < n; ++r) {
+      const double f = A[r * n + k] / A[k * n + k];
+      if (f == 0.0) continue;
+      for (int j = k; j < n; ++j) A[r * n + j] -= f * A[k * n + j];
+      b[r] -= f * b[k];
+    }
+  }
+  for (int k = n - 1; k >= 0; --k) {
+    double s = b[k];
+    for (int j = k + 1; j < n; ++j) s -= A[k * n + j] * x[j];
+    x[k] = s / A[k * n + k];
+  }
+}
+
+// Level fractions x_i (sum = 1) of one cell: Eq. 3.6.1 with the ground-state row replaced by the
+// conservation equation, N = 1 (fractions; linearity in abundance).
+void orc_levelpop_cell(const orc_config *c, double nH2, double Tgas, double *x) {
+  const int N = c->n_levels;
+  std::vector<double> M(N * N), b(N, 0.0);
+  orc_balance_matrix(c, nH2, Tgas, M.data());
+  for (int j = 0; j < N; ++j) M[j] = 1.0;
+  b[0] = 1.0;
+  solve_ge(N, M.data(), b.data(), x);
+}
+
+// pop[N][ncell] for arrays of cells.
+void orc_levelpop(const orc_config *c, int64_t ncell, const float *nH2, const float *Tgas, double *pop) {
+  const int N = c->n_levels;
+#pragma omp parallel for schedule(static)
+  for (int64_t i = 0; i < ncell; ++i) {
+    double x[32];
+    orc_levelpop_cell(c, (double)nH2[i], (double)Tgas[i], x);
+    for (int l = 0; l < N; ++l) pop[(int64_t)l * ncell + i] = x[l];
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// O4  Per-cell coefficients.
+//   j^[L]     = (h nu0 / 4 pi) n_u A_ul                       Eq. 3.3.1
+//   alpha^[L] = (h nu0 / 4 pi) (n_l B_lu - n_u B_ul)          Eq. 3.3.2
+//   n_i = X n_H2 x_i                                          Eq. 4.2.1, reading S16
+//   b = sqrt(2 k T / m_a + xi^2)   (Delta nu_D = nu0 b / c)   Eq. 3.3.4, reading S1
+//   alpha^[D] = kappa rho_gas, rho_gas = mass_per_H2 n_H2     Eq. 3.2.2, reading S3
+//   S^[D] = B_nu0(T_dust)                                     Eq. 3.2.1, reading S6
+//   no line above T_inf
+// out5 = {j0, kappa0, b, alpha_d, S_d}
+void orc_cell_coefficients(const orc_config *c, double nH2, double Tgas, double Tdust, const double *x,
+                           double *out5) {
+  const int N = c->n_levels;
+  const int u = c->line_upper, l = c->line_lower;
+  const double nu0 = c->nu0_Hz;
+  const double A = c->einstein_A[u * N + l];
+  const double Bul = kC * kC / (2.0 * kH * nu0 * nu0 * nu0) * A;
+  const double Blu = c->weight[u] / c->weight[l] * Bul;
+  const double ntr = c->abundance * nH2;
+  double j0 = kH * nu0 / (4.0 * kPi) * ntr * x[u] * A;
+  double k0 = kH * nu0 / (4.0 * kPi) * ntr * (x[l] * Blu - x[u] * Bul);
+  if (Tgas > c->T_inf) { j0 = 0.0; k0 = 0.0; }
+  out5[0] = j0;
+  out5[1] = k0;
+  out5[2] = std::sqrt(2.0 * kK * Tgas / c->mol_mass_g + c->microturb_cms * c->microturb_cms);
+  out5[3] = c->dust_on ? c->kappa_gas_cm2_g * c->mass_per_H2_g * nH2 : 0.0;
+  out5[4] = c->dust_on ? orc_planck(nu0, Tdust) : 0.0;
+}
+
+// coef[5][ncell]; pop may be NULL (then solved here) or [N][ncell].
+void orc_coefficients(const orc_config *c, int64_t ncell, const float *nH2, const float *Tgas,
+                      const float *Tdust, const double *pop, double *coef) {
+  const int N = c->n_levels;
+#pragma omp parallel for schedule(static)
+  for (int64_t i = 0; i < ncell; ++i) {
+    double x[32], o[5];
+    if (pop) for (int l = 0; l < N; ++l) x[l] = pop[(int64_t)l * ncell + i];
+    else orc_levelpop_cell(c, (double)nH2[i], (double)Tgas[i], x);
+    orc_cell_coefficients(c, (double)nH2[i], (double)Tgas[i], (double)Tdust[i], x, o);
+    for (int q = 0; q < 5; ++q) coef[(int64_t)q * ncell + i] = o[q];
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// O5  Channel-averaged (integrated) Gaussian profile, Eq. 4.4.1 applied to Eq. 3.3.3
+// (PAPER.md:378), i.e. Eq. 4.6.3 (reading G1: erf difference between channel edges).
+// Worked in velocity space (reading G9): channel k has centre v_k = v0 + k dv and edges v_k -+ dv/2;
+// a cell emits at channel velocity v = v_los.  Delta nu_W = nu0 dv / c.
+//   phibar_k = [erf((v_k + dv/2 - v_los)/b) - erf((v_k - dv/2 - v_los)/b)] / (2 Delta nu_W)   [1/Hz]
+double orc_phibar(const orc_config *c, int k, double vlos, double b) {
+  const double vk = c->v0_cms + k * c->dv_cms;
+  const double dnuW = c->nu0_Hz * c->dv_cms / kC;
+  const double hi = (vk + 0.5 * c->dv_cms - vlos) / b;
+  const double lo = (vk - 0.5 * c->dv_cms - vlos) / b;
+  return (std::erf(hi) - std::erf(lo)) / (2.0 * dnuW);
+}
+
+// Point profile phi(nu) of Eq. 3.3.3 evaluated at the frequency that corresponds to velocity v
+// (used only by the brute-force pin).  Delta nu_D = nu0 b / c (Eq. 3.3.4).
+double orc_phi_point(const orc_config *c, double v, double vlos, double b) {
+  const double dnuD = c->nu0_Hz * b / kC;
+  const double x = (v - vlos) / b;
+  return std::exp(-x * x) / (dnuD * std::sqrt(kPi));
+}
+
+// w(tau) = (1 - e^-tau) / tau, w(0) = 1: the formal step S (1 - e^-tau) written as j h w(tau)
+// (reading S13: identical for alpha != 0, defined for alpha = 0 and alpha < 0).
+static double w_of_tau(double tau) { return tau == 0.0 ? 1.0 : -std::expm1(-tau) / tau; }
+
+// O6  Formal integration step, Eq. 4.8.5 - 4.8.7:
+//   I_{n+1} = I_n e^-tau + S (1 - e^-tau),  S = j / alpha,  tau = h alpha.
+static double formal_step(double I, double j, double alpha, double h) {
+  const double tau = alpha * h;
+  return I * std::exp(-tau) + j * h * w_of_tau(tau);
+}
+
+// March one pixel column (k = 0 far ... nz-1 near; reading S11) for all channels.
+// coef = {j0, kappa0, b, alpha_d, S_d} planes [5][ncell], vlos plane float32.
+// Total: alpha = kappa0 phibar + alpha_d, j = j0 phibar + alpha_d S_d   (Eq. 4.8.6-4.8.7, 4.6.4)
+// Continuum: alpha = alpha_d, j = alpha_d S_d                           (Eq. 3.1.3, 4.4.3-4.4.5)
+// Both start from I_bg = B_nu0(T_cmb).  No ReLU clamp (smooth integrator only).
+void orc_march_column(const orc_config *c, const double *coef, const float *vlos, int64_t pix,
+                      double *I_tot /*[nv]*/, double *I_cont /*[1]*/) {
+  const int64_t plane = (int64_t)c->nx * c->ny, ncell = plane * c->nz;
+  const double h = c->cell_cm;
+  const double Ibg = orc_planck(c->nu0_Hz, c->T_cmb);
+  for (int v = 0; v < c->nv; ++v) I_tot[v] = Ibg;
+  double Ic = Ibg;
+  for (int k = 0; k < c->nz; ++k) {
+    const int64_t cell = (int64_t)k * plane + pix;
+    const double j0 = coef[cell], k0 = coef[ncell + cell], b = coef[2 * ncell + cell];
+    const double ad = coef[3 * ncell + cell], Sd = coef[4 * ncell + cell];
+    const double vl = (double)vlos[cell];
+    for (int v = 0; v < c->nv; ++v) {
+      const double pb = orc_phibar(c, v, vl, b);
+      I_tot[v] = formal_step(I_tot[v], j0 * pb + ad * Sd, k0 * pb + ad, h);
+    }
+    Ic = formal_step(Ic, ad * Sd, ad, h);
+  }
+  *I_cont = Ic;
+}
+
+// Columns pix[0..npix): I_tot[npix][nv], I_cont[npix].
+void orc_march(const orc_config *c, const double *coef, const float *vlos, int64_t npix,
+               const int64_t *pix, double *I_tot, double *I_cont) {
+#pragma omp parallel for schedule(dynamic, 4)
+  for (int64_t p = 0; p < npix; ++p)
+    orc_march_column(c, coef, vlos, pix[p], I_tot + p * c->nv, I_cont + p);
+}
+
+// O7  Continuum subtraction and unit conversion (Eq. 4.9.1-4.9.2).
+//   subtract_space 0: D = I_tot - I_cont (intensity space == RJ space), then converted to out_unit
+//   subtract_space 1: T_B(I_tot) - T_B(I_cont)  (Planck space; result is in Kelvin)
+//   subtract_continuum 0: I_tot converted to out_unit.
+double orc_convert_voxel(const orc_config *c, double It, double Ic) {
+  const double nu = c->nu0_Hz;
+  if (c->subtract_continuum && c->subtract_space == 1) return orc_planck_TB(nu, It) - orc_planck_TB(nu, Ic);
+  const double D = c->subtract_continuum ? It - Ic : It;
+  if (c->out_unit == 0) return D;
+  if (c->out_unit == 1) return orc_rayleigh_jeans_T(nu, D);
+  return orc_planck_TB(nu, D);
+}
+
+void orc_convert(const orc_config *c, int64_t npix, const double *I_tot, const double *I_cont, double *cube) {
+  for (int64_t p = 0; p < npix; ++p)
+    for (int v = 0; v < c->nv; ++v)
+      cube[p * c->nv + v] = orc_convert_voxel(c, I_tot[p * c->nv + v], I_cont[p]);
+}
+
+// ---------------------------------------------------------------------------------------------
+// O8  Gaussian beam, reading S8: sigma = FWHM / (2 sqrt(2 ln 2)), integer-offset
+// samples g(d) ~ exp(-d^2 / 2 sigma^2), |d| <= R = ceil(4 sigma), normalised to sum 1 in 1-D, zero
+// outside the image ("same" convolution).  Direct 2-D sum (not separated) per channel.
+int orc_beam_radius(double fwhm_px) {
+  const double sigma = fwhm_px / (2.0 * std::sqrt(2.0 * std::log(2.0)));
+  return (int)std::ceil(4.0 * sigma);
+}
+
+void orc_beam_weights(double fwhm_px, double *g /*[2R+1]*/) {
+  const double sigma = fwhm_px / (2.0 * std::sqrt(2.0 * std::log(2.0)));
+  const int R = orc_beam_radius(fwhm_px);
+  double s = 0.0;
+  for (int d = -R; d <= R; ++d) { g[d + R] = std::exp(-0.5 * d * d / (sigma * sigma)); s += g[d + R]; }
+  for (int d = 0; d <= 2 * R; ++d) g[d] /= s;
+}
+
+void orc_beam(int ny, int nx, int nv, double fwhm_px, const double *in, double *out) {
+  const int R = orc_beam_radius(fwhm_px);
+  std::vector<double> g(2 * R + 1);
+  orc_beam_weights(fwhm_px, g.data());
+#pragma omp parallel for schedule(static)
+  for (int y = 0; y < ny; ++y)
+    for (int x = 0; x < nx; ++x)
+      for (int v = 0; v < nv; ++v) {
+        double s = 0.0;
+        for (int dy = -R; dy <= R; ++dy) {
+          const int yy = y + dy;
+          if (yy < 0 || yy >= ny) continue;
+          for (int dx = -R; dx <= R; ++dx) {
+            const int xx = x + dx;
+            if (xx < 0 || xx >= nx) continue;
+            s += g[dy + R] * g[dx + R] * in[((int64_t)yy * nx + xx) * nv + v];
+          }
+        }
+        out[((int64_t)y * nx + x) * nv + v] = s;
+      }
+}
+
+// ---------------------------------------------------------------------------------------------
+// O9  Noise, Eq. 4.12.1: T += gamma (mu + sigma z), z ~ N(0,1) independently per voxel.
+// Reading S10: z comes from the counter-based generator Philox4x32-10 (Salmon et al. 2011)
+// with key = (seed lo, seed hi) and counter = (voxel lo, voxel hi, 0, 0); the first two output words
+// give u1 = ((r0 >> 8) + 0.5) 2^-24, u2 = ((r1 >> 8) + 0.5) 2^-24 and Box-Muller
+// z = sqrt(-2 ln u1) cos(2 pi u2).  gamma (reading S9): mode 0 -> 1; mode 1 -> one draw per cube,
+// gamma = (r0 >> 8) 2^-24 of counter (0, 0, 1, 0).
+void orc_philox4x32_10(uint64_t seed, uint64_t ctr_lo, uint64_t ctr_hi, uint32_t out[4]) {
+  uint32_t c0 = (uint32_t)ctr_lo, c1 = (uint32_t)(ctr_lo >> 32), c2 = (uint32_t)ctr_hi, c3 = (uint32_t)(ctr_hi >> 32);
+  uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+  for (int r = 0; r < 10; ++r) {
+    const uint64_t p0 = (uint64_t)0xD2511F53u * c0;
+    const uint64_t p1 = (uint64_t)0xCD9E8D57u * c2;
+    const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0;
+    const uint32_t n1 = (uint32_t)p1;
+    const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1;
+    const uint32_t n3 = (uint32_t)p0;
+    c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+    k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+  }
+  out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+double orc_normal(uint64_t seed, uint64_t voxel) {
+  uint32_t r[4];
+  orc_philox4x32_10(seed, voxel, 0, r);
+  const double u1 = ((double)(r[0] >> 8) + 0.5) / 16777216.0;
+  const double u2 = ((double)(r[1] >> 8) + 0.5) / 16777216.0;
+  return std::sqrt(-2.0 * std::log(u1)) * std::cos(2.0 * kPi * u2);
+}
+
+double orc_noise_gamma(const orc_config *c) {
+  if (c->noise_gamma_mode == 0) return 1.0;
+  uint32_t r[4];
+  orc_philox4x32_10(c->seed, 0, 1, r);
+  return (double)(r[0] >> 8) / 16777216.0;
+}
+
+void orc_noise(const orc_config *c, int64_t nvox, double *cube) {
+  const double gamma = orc_noise_gamma(c);
+  for (int64_t i = 0; i < nvox; ++i)
+    cube[i] += gamma * (c->noise_mu + c->noise_sigma * orc_normal(c->seed, (uint64_t)i));
+}
+
+// ---------------------------------------------------------------------------------------------
+// Whole path (stage list PAPER.md:467): level balance -> coefficients -> transfer (total + continuum)
+// -> continuum subtraction + units -> beam -> noise.  cube[ny][nx][nv].
+// stage_mask bit 0: apply beam (if fwhm > 0); bit 1: apply noise (if configured).
+void orc_observe(const orc_config *c, const float *nH2, const float *Tgas, const float *Tdust,
+                 const float *vlos, int stage_mask, double *cube) {
+  const int64_t plane = (int64_t)c->nx * c->ny, ncell = plane * c->nz;
+  std::vector<double> coef(5 * ncell);
+  orc_coefficients(c, ncell, nH2, Tgas, Tdust, nullptr, coef.data());
+#pragma omp parallel for schedule(dynamic, 4)
+  for (int64_t p = 0; p < plane; ++p) {
+    std::vector<double> It(c->nv);
+    double Ic;
+    orc_march_column(c, coef.data(), vlos, p, It.data(), &Ic);
+    for (int v = 0; v < c->nv; ++v) cube[p * c->nv + v] = orc_convert_voxel(c, It[v], Ic);
+  }
+  if ((stage_mask & 1) && c->beam_fwhm_px > 0.0) {
+    std::vector<double> tmp(cube, cube + plane * c->nv);
+    orc_beam(c->ny, c->nx, c->nv, c->beam_fwhm_px, tmp.data(), cube);
+  }
+  if ((stage_mask & 2) && (c->noise_sigma != 0.0 || c->noise_mu != 0.0)) orc_noise(c, plane * c->nv, cube);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Brute-force pin (SURVEY 8(c) pin 8): monochromatic RTE, Eq. 3.1.2 with the POINT
+// profile Eq. 3.3.3, solved exactly per cell (coefficients constant in a cell) at nsub frequencies
+// per channel (midpoints), then channel-averaged, Eq. 4.4.2.  Not the method: the
+// method applies the channel-AVERAGED profile inside the step (reading R1); the two agree as tau -> 0.
+void orc_brute_column(const orc_config *c, const double *coef, const float *vlos, int64_t pix, int nsub,
+                      double *I_avg /*[nv]*/) {
+  const int64_t plane = (int64_t)c->nx * c->ny, ncell = plane * c->nz;
+  const double h = c->cell_cm;
+  const double Ibg = orc_planck(c->nu0_Hz, c->T_cmb);
+  for (int v = 0; v < c->nv; ++v) {
+    double acc = 0.0;
+    for (int s = 0; s < nsub; ++s) {
+      const double vel = c->v0_cms + (v - 0.5) * c->dv_cms + (s + 0.5) * c->dv_cms / nsub;
+      double I = Ibg;
+      for (int k = 0; k < c->nz; ++k) {
+        const int64_t cell = (int64_t)k * plane + pix;
+        const double phi = orc_phi_point(c, vel, (double)vlos[cell], coef[2 * ncell + cell]);
+        const double ad = coef[3 * ncell + cell];
+        I = formal_step(I, coef[cell] * phi + ad * coef[4 * ncell + cell], coef[ncell + cell] * phi + ad, h);
+      }
+      acc += I;
+    }
+    I_avg[v] = acc / nsub;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// O10  Gradient of L = sum_voxels w * cube(noise-free, beam-convolved) with respect to n_H2.
+//
+// (a) Finite differences (the definition): central differences with relative step eps on the listed
+// cells.  Only the column holding the cell changes and the beam is linear, so L changes by
+// sum_v what[pixel][v] * d(cube_raw[pixel][v]) with what = G^T w (beam adjoint = same symmetric
+// zero-padded convolution, reading S20); `what` is computed by the caller with orc_beam.
+static void raw_column(const orc_config *c, const float *nH2, const float *Tgas, const float *Tdust,
+                       const float *vlos, int64_t pix, int64_t cell_mod, double n_mod, double *out) {
+  const int64_t plane = (int64_t)c->nx * c->ny;
+  const double h = c->cell_cm;
+  const double Ibg = orc_planck(c->nu0_Hz, c->T_cmb);
+  std::vector<double> It(c->nv, Ibg);
+  double Ic = Ibg;
+  for (int k = 0; k < c->nz; ++k) {
+    const int64_t cell = (int64_t)k * plane + pix;
+    const double n = cell == cell_mod ? n_mod : (double)nH2[cell];
+    double x[32], o[5];
+    orc_levelpop_cell(c, n, (double)Tgas[cell], x);
+    orc_cell_coefficients(c, n, (double)Tgas[cell], (double)Tdust[cell], x, o);
+    for (int v = 0; v < c->nv; ++v) {
+      const double pb = orc_phibar(c, v, (double)vlos[cell], o[2]);
+      It[v] = formal_step(It[v], o[0] * pb + o[3] * o[4], o[1] * pb + o[3], h);
+    }
+    Ic = formal_step(Ic, o[3] * o[4], o[3], h);
+  }
+  for (int v = 0; v < c->nv; ++v) out[v] = orc_convert_voxel(c, It[v], Ic);
+}
+
+void orc_grad_fd(const orc_config *c, const float *nH2, const float *Tgas, const float *Tdust,
+                 const float *vlos, const double *what /*[ny][nx][nv]*/, int64_t nprobe,
+                 const int64_t *cells, double eps, double *grad /*[nprobe]*/) {
+  const int64_t plane = (int64_t)c->nx * c->ny;
+#pragma omp parallel for schedule(dynamic, 1)
+  for (int64_t q = 0; q < nprobe; ++q) {
+    const int64_t cell = cells[q], pix = cell % plane;
+    const double n0 = (double)nH2[cell], dn = eps * n0;
+    std::vector<double> a(c->nv), b(c->nv);
+    raw_column(c, nH2, Tgas, Tdust, vlos, pix, cell, n0 + dn, a.data());
+    raw_column(c, nH2, Tgas, Tdust, vlos, pix, cell, n0 - dn, b.data());
+    double s = 0.0;
+    for (int v = 0; v < c->nv; ++v) s += what[pix * c->nv + v] * (a[v] - b[v]);
+    grad[q] = s / (2.0 * dn);
+  }
+}
+
+// (b) Analytic reverse-scan adjoint in float64, for out_unit = T_RJ or I with
+// intensity-space subtraction.  Used to pin (a) against itself on every cell of a small cube and as
+// the dense reference for the GPU adjoint.  grad[ncell].
+//   forward:  I_{k+1} = I_k e^-tau + j h w(tau)
+//   dI_{k+1}/dalpha = h [ -I_k e^-tau + j h w'(tau) ],  w'(tau) = (e^-tau (1 + tau) - 1) / tau^2
+//   dI_{k+1}/dj     = h w(tau)
+//   lambda_k = lambda_{k+1} e^-tau,  lambda_nz = scale * what
+//   chain: dj0/dn = j0/n + (h nu0 / 4 pi) X n A dx_u/dn (same for kappa0), M dx/dn = -M_col x with the
+//   conservation row zeroed on the right-hand side; d alpha_d / dn = kappa mass_per_H2.
+static double wprime_of_tau(double tau) {
+  if (std::fabs(tau) < 1e-4) return -0.5 + tau / 3.0 - tau * tau / 8.0;
+  return (std::exp(-tau) * (1.0 + tau) - 1.0) / (tau * tau);
+}
+
+void orc_grad_adjoint(const orc_config *c, const float *nH2, const float *Tgas, const float *Tdust,
+                      const float *vlos, const double *what, double *grad) {
+  const int64_t plane = (int64_t)c->nx * c->ny;
+  const int N = c->n_levels, nz = c->nz, nv = c->nv;
+  const double h = c->cell_cm;
+  const double Ibg = orc_planck(c->nu0_Hz, c->T_cmb);
+  const double scale = c->out_unit == 1 ? kC * kC / (2.0 * kK * c->nu0_Hz * c->nu0_Hz) : 1.0;
+  const int u = c->line_upper, l = c->line_lower;
+  const double A = c->einstein_A[u * N + l];
+  const double Bul = kC * kC / (2.0 * kH * c->nu0_Hz * c->nu0_Hz * c->nu0_Hz) * A;
+  const double Blu = c->weight[u] / c->weight[l] * Bul;
+  const double pref = kH * c->nu0_Hz / (4.0 * kPi);
+#pragma omp parallel for schedule(dynamic, 4)
+  for (int64_t pix = 0; pix < plane; ++pix) {
+    std::vector<double> co(5 * nz), It((int64_t)(nz + 1) * nv), Ic(nz + 1), lam(nv), xs(nz * N);
+    for (int k = 0; k < nz; ++k) {
+      const int64_t cell = (int64_t)k * plane + pix;
+      orc_levelpop_cell(c, (double)nH2[cell], (double)Tgas[cell], &xs[k * N]);
+      orc_cell_coefficients(c, (double)nH2[cell], (double)Tgas[cell], (double)Tdust[cell], &xs[k * N], &co[5 * k]);
+    }
+    for (int v = 0; v < nv; ++v) It[v] = Ibg;
+    Ic[0] = Ibg;
+    for (int k = 0; k < nz; ++k) {
+      const int64_t cell = (int64_t)k * plane + pix;
+      const double *o = &co[5 * k];
+      for (int v = 0; v < nv; ++v) {
+        const double pb = orc_phibar(c, v, (double)vlos[cell], o[2]);
+        It[(int64_t)(k + 1) * nv + v] = formal_step(It[(int64_t)k * nv + v], o[0] * pb + o[3] * o[4], o[1] * pb + o[3], h);
+      }
+      Ic[k + 1] = formal_step(Ic[k], o[3] * o[4], o[3], h);
+    }
+    double lamC = 0.0;   // adjoint of the continuum: -sum_v lambda (subtraction), if enabled
+    for (int v = 0; v < nv; ++v) { lam[v] = scale * what[pix * nv + v]; if (c->subtract_continuum) lamC -= lam[v]; }
+    for (int k = nz - 1; k >= 0; --k) {
+      const int64_t cell = (int64_t)k * plane + pix;
+      const double *o = &co[5 * k];
+      double g_j0 = 0.0, g_k0 = 0.0, g_ad = 0.0;
+      for (int v = 0; v < nv; ++v) {
+        const double pb = orc_phibar(c, v, (double)vlos[cell], o[2]);
+        const double al = o[1] * pb + o[3], j = o[0] * pb + o[3] * o[4], tau = al * h, e = std::exp(-tau);
+        const double dIda = h * (-It[(int64_t)k * nv + v] * e + j * h * wprime_of_tau(tau));
+        const double dIdj = h * w_of_tau(tau);
+        g_k0 += lam[v] * dIda * pb;
+        g_j0 += lam[v] * dIdj * pb;
+        g_ad += lam[v] * (dIda + o[4] * dIdj);
+        lam[v] *= e;
+      }
+      {  // continuum branch
+        const double tau = o[3] * h, e = std::exp(-tau), j = o[3] * o[4];
+        const double dIda = h * (-Ic[k] * e + j * h * wprime_of_tau(tau));
+        g_ad += lamC * (dIda + o[4] * h * w_of_tau(tau));
+        lamC *= e;
+      }
+      // chain through the level balance: M dx = -(dM/dn) x, conservation row: sum dx = 0
+      const double n = (double)nH2[cell], T = (double)Tgas[cell];
+      std::vector<double> M(N * N), M1(N * N), rhs(N, 0.0), dx(N);
+      orc_balance_matrix(c, n, T, M.data());
+      // dM/dn: the balance matrix is affine in n; difference of two evaluations is exact up to rounding
+      orc_balance_matrix(c, 2.0 * n, T, M1.data());
+      const double *x = &xs[k * N];
+      for (int i = 1; i < N; ++i) {
+        double s = 0.0;
+        for (int jx = 0; jx < N; ++jx) s += (M1[i * N + jx] - M[i * N + jx]) / n * x[jx];
+        rhs[i] = -s;
+      }
+      for (int jx = 0; jx < N; ++jx) M[jx] = 1.0;
+      rhs[0] = 0.0;
+      solve_ge(N, M.data(), rhs.data(), dx.data());
+      const double X = c->abundance;
+      double dj0 = pref * X * A * (x[u] + n * dx[u]);
+      double dk0 = pref * X * ((x[l] + n * dx[l]) * Blu - (x[u] + n * dx[u]) * Bul);
+      if (T > c->T_inf) { dj0 = 0.0; dk0 = 0.0; }
+      const double dad = c->dust_on ? c->kappa_gas_cm2_g * c->mass_per_H2_g : 0.0;
+      grad[cell] = g_j0 * dj0 + g_k0 * dk0 + g_ad * dad;
+    }
+  }
+}
+
+}  // extern "C"

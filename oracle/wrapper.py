@@ -1,0 +1,271 @@
+"""ORACLE -- test infrastructure only.  ctypes marshalling for oracle/iris_oracle.cpp.
+
+The config argument is duck-typed (any object with the attribute names of the parameter record);
+nothing here imports the CUDA package.
+"""
+import ctypes as C
+import os
+import subprocess
+import threading
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "iris_oracle.cpp")
+_LIB = os.path.join(_HERE, "liboracle.so")
+_lock = threading.Lock()
+
+
+def oracle_lib_path():
+    return _LIB
+
+
+def build_oracle(force=False):
+    """Compile the oracle with g++ -O2 (+OpenMP over cells / pixel columns). Returns the .so path."""
+    with _lock:
+        if (not force and os.path.exists(_LIB)
+                and os.path.getmtime(_LIB) >= os.path.getmtime(_SRC)):
+            return _LIB
+        tmp = _LIB + ".tmp%d" % os.getpid()
+        cmd = ["g++", "-O2", "-std=c++17", "-fPIC", "-shared", "-fopenmp", "-ffp-contract=off",
+               "-o", tmp, _SRC]
+        subprocess.run(cmd, check=True)
+        os.replace(tmp, _LIB)
+        return _LIB
+
+
+class _Cfg(C.Structure):
+    _fields_ = [
+        ("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32),
+        ("cell_cm", C.c_double),
+        ("n_levels", C.c_int32),
+        ("energy_K", C.POINTER(C.c_double)), ("weight", C.POINTER(C.c_double)),
+        ("einstein_A", C.POINTER(C.c_double)), ("coll_down_ref", C.POINTER(C.c_double)),
+        ("coll_T_ref", C.c_double), ("coll_T_exp", C.c_double),
+        ("line_upper", C.c_int32), ("line_lower", C.c_int32),
+        ("nu0_Hz", C.c_double), ("mol_mass_g", C.c_double), ("abundance", C.c_double),
+        ("microturb_cms", C.c_double), ("T_bar", C.c_double), ("T_cmb", C.c_double), ("T_inf", C.c_double),
+        ("dust_on", C.c_int32),
+        ("kappa_gas_cm2_g", C.c_double), ("mass_per_H2_g", C.c_double),
+        ("nv", C.c_int32),
+        ("v0_cms", C.c_double), ("dv_cms", C.c_double),
+        ("subtract_continuum", C.c_int32), ("subtract_space", C.c_int32), ("out_unit", C.c_int32),
+        ("beam_fwhm_px", C.c_double), ("noise_mu", C.c_double), ("noise_sigma", C.c_double),
+        ("noise_gamma_mode", C.c_int32),
+        ("seed", C.c_uint64),
+    ]
+
+
+def _dp(a):
+    return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def _fp(a):
+    return a.ctypes.data_as(C.POINTER(C.c_float))
+
+
+def _ip(a):
+    return a.ctypes.data_as(C.POINTER(C.c_int64))
+
+
+def _f32(a):
+    a = np.ascontiguousarray(a, dtype=np.float32)
+    return a
+
+
+class Oracle:
+    """One parameter record bound to the oracle library."""
+
+    def __init__(self, cfg, threads=None):
+        self.lib = C.CDLL(build_oracle())
+        self.cfg = cfg
+        self._keep = [np.ascontiguousarray(np.asarray(getattr(cfg, k), dtype=np.float64))
+                      for k in ("energy_K", "weight", "einstein_A", "coll_down_ref")]
+        s = _Cfg()
+        for name, ctype in _Cfg._fields_:
+            if name in ("energy_K", "weight", "einstein_A", "coll_down_ref"):
+                continue
+            if name == "n_levels":
+                s.n_levels = len(self._keep[0])
+                continue
+            val = getattr(cfg, name)
+            setattr(s, name, float(val) if ctype is C.c_double else int(val))
+        s.energy_K, s.weight, s.einstein_A, s.coll_down_ref = (_dp(a) for a in self._keep)
+        self.s = s
+        self.N = int(s.n_levels)
+        self.threads = threads
+        L = self.lib
+        L.orc_planck.restype = C.c_double
+        L.orc_planck.argtypes = [C.c_double, C.c_double]
+        L.orc_planck_TB.restype = C.c_double
+        L.orc_planck_TB.argtypes = [C.c_double, C.c_double]
+        L.orc_rayleigh_jeans_T.restype = C.c_double
+        L.orc_rayleigh_jeans_T.argtypes = [C.c_double, C.c_double]
+        L.orc_phibar.restype = C.c_double
+        L.orc_phibar.argtypes = [C.c_void_p, C.c_int, C.c_double, C.c_double]
+        L.orc_phi_point.restype = C.c_double
+        L.orc_phi_point.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_double]
+        L.orc_normal.restype = C.c_double
+        L.orc_normal.argtypes = [C.c_uint64, C.c_uint64]
+        L.orc_noise_gamma.restype = C.c_double
+        L.orc_beam_radius.restype = C.c_int
+        L.orc_beam_radius.argtypes = [C.c_double]
+
+    # -- helpers ---------------------------------------------------------------------------------
+    def _p(self):
+        return C.byref(self.s)
+
+    def _omp(self):
+        if self.threads is not None:
+            try:
+                omp = C.CDLL("libgomp.so.1")
+                omp.omp_set_num_threads(int(self.threads))
+            except OSError:
+                pass
+
+    @property
+    def n_cells(self):
+        return int(self.s.nx) * int(self.s.ny) * int(self.s.nz)
+
+    # -- scalar functions ------------------------------------------------------------------------
+    def planck(self, nu, T):
+        return self.lib.orc_planck(float(nu), float(T))
+
+    def planck_TB(self, nu, I):
+        return self.lib.orc_planck_TB(float(nu), float(I))
+
+    def rayleigh_jeans_T(self, nu, I):
+        return self.lib.orc_rayleigh_jeans_T(float(nu), float(I))
+
+    def phibar(self, k, vlos, b):
+        return self.lib.orc_phibar(self._p(), int(k), float(vlos), float(b))
+
+    def phi_point(self, v, vlos, b):
+        return self.lib.orc_phi_point(self._p(), float(v), float(vlos), float(b))
+
+    def normal(self, seed, voxel):
+        return self.lib.orc_normal(int(seed), int(voxel))
+
+    def philox(self, seed, ctr_lo, ctr_hi=0):
+        out = (C.c_uint32 * 4)()
+        self.lib.orc_philox4x32_10(C.c_uint64(seed), C.c_uint64(ctr_lo), C.c_uint64(ctr_hi), out)
+        return [int(v) for v in out]
+
+    def noise_gamma(self):
+        self.lib.orc_noise_gamma.argtypes = [C.c_void_p]
+        return self.lib.orc_noise_gamma(self._p())
+
+    def beam_weights(self, fwhm):
+        R = self.lib.orc_beam_radius(float(fwhm))
+        g = np.zeros(2 * R + 1)
+        self.lib.orc_beam_weights(C.c_double(fwhm), _dp(g))
+        return g
+
+    # -- level balance ---------------------------------------------------------------------------
+    def rates(self, nH2, Tgas):
+        R = np.zeros((self.N, self.N))
+        self.lib.orc_rates(self._p(), C.c_double(nH2), C.c_double(Tgas), _dp(R))
+        return R
+
+    def balance_matrix(self, nH2, Tgas):
+        M = np.zeros((self.N, self.N))
+        self.lib.orc_balance_matrix(self._p(), C.c_double(nH2), C.c_double(Tgas), _dp(M))
+        return M
+
+    def levelpop_cell(self, nH2, Tgas):
+        x = np.zeros(self.N)
+        self.lib.orc_levelpop_cell(self._p(), C.c_double(nH2), C.c_double(Tgas), _dp(x))
+        return x
+
+    def levelpop(self, nH2, Tgas):
+        """pop[N, ncell] (float64) for flat float32 arrays of cells."""
+        self._omp()
+        nH2, Tgas = _f32(nH2).ravel(), _f32(Tgas).ravel()
+        pop = np.zeros((self.N, nH2.size))
+        self.lib.orc_levelpop(self._p(), C.c_int64(nH2.size), _fp(nH2), _fp(Tgas), _dp(pop))
+        return pop
+
+    # -- coefficients ----------------------------------------------------------------------------
+    def coefficients(self, nH2, Tgas, Tdust, pop=None):
+        """coef[5, ncell] = j0, kappa0, b, alpha_d, S_d."""
+        self._omp()
+        nH2, Tgas, Tdust = _f32(nH2).ravel(), _f32(Tgas).ravel(), _f32(Tdust).ravel()
+        coef = np.zeros((5, nH2.size))
+        pp = None
+        if pop is not None:
+            pop = np.ascontiguousarray(pop, dtype=np.float64)
+            pp = _dp(pop)
+        self.lib.orc_coefficients(self._p(), C.c_int64(nH2.size), _fp(nH2), _fp(Tgas), _fp(Tdust), pp, _dp(coef))
+        return coef
+
+    # -- transfer --------------------------------------------------------------------------------
+    def march(self, coef, vlos, pix=None):
+        """I_tot[npix, nv], I_cont[npix] for the listed pixel columns (all if None)."""
+        self._omp()
+        coef = np.ascontiguousarray(coef, dtype=np.float64)
+        vlos = _f32(vlos).ravel()
+        assert coef.shape == (5, self.n_cells) and vlos.size == self.n_cells
+        plane = int(self.s.nx) * int(self.s.ny)
+        pix = np.arange(plane, dtype=np.int64) if pix is None else np.ascontiguousarray(pix, dtype=np.int64)
+        It = np.zeros((pix.size, int(self.s.nv)))
+        Ic = np.zeros(pix.size)
+        self.lib.orc_march(self._p(), _dp(coef), _fp(vlos), C.c_int64(pix.size), _ip(pix), _dp(It), _dp(Ic))
+        return It, Ic
+
+    def brute_column(self, coef, vlos, pix, nsub):
+        coef = np.ascontiguousarray(coef, dtype=np.float64)
+        vlos = _f32(vlos).ravel()
+        out = np.zeros(int(self.s.nv))
+        self.lib.orc_brute_column(self._p(), _dp(coef), _fp(vlos), C.c_int64(pix), C.c_int(nsub), _dp(out))
+        return out
+
+    def convert(self, I_tot, I_cont):
+        I_tot = np.ascontiguousarray(I_tot, dtype=np.float64)
+        I_cont = np.ascontiguousarray(I_cont, dtype=np.float64)
+        cube = np.zeros_like(I_tot)
+        self.lib.orc_convert(self._p(), C.c_int64(I_cont.size), _dp(I_tot), _dp(I_cont), _dp(cube))
+        return cube
+
+    # -- post-processing -------------------------------------------------------------------------
+    def beam(self, cube, fwhm=None):
+        self._omp()
+        cube = np.ascontiguousarray(cube, dtype=np.float64)
+        ny, nx, nv = cube.shape
+        out = np.zeros_like(cube)
+        fwhm = float(self.s.beam_fwhm_px if fwhm is None else fwhm)
+        self.lib.orc_beam(C.c_int(ny), C.c_int(nx), C.c_int(nv), C.c_double(fwhm), _dp(cube), _dp(out))
+        return out
+
+    def noise(self, cube):
+        cube = np.array(cube, dtype=np.float64, order="C", copy=True)
+        self.lib.orc_noise(self._p(), C.c_int64(cube.size), _dp(cube))
+        return cube
+
+    def observe(self, fields, beam=True, noise=True):
+        """Whole path; cube[ny, nx, nv] float64."""
+        self._omp()
+        f = [_f32(fields[k]).ravel() for k in ("nH2", "Tgas", "Tdust", "vlos")]
+        assert all(a.size == self.n_cells for a in f)
+        cube = np.zeros((int(self.s.ny), int(self.s.nx), int(self.s.nv)))
+        mask = (1 if beam else 0) | (2 if noise else 0)
+        self.lib.orc_observe(self._p(), *[_fp(a) for a in f], C.c_int(mask), _dp(cube))
+        return cube
+
+    # -- gradient --------------------------------------------------------------------------------
+    def grad_fd(self, fields, what, cells, eps=1e-4):
+        self._omp()
+        f = [_f32(fields[k]).ravel() for k in ("nH2", "Tgas", "Tdust", "vlos")]
+        what = np.ascontiguousarray(what, dtype=np.float64)
+        cells = np.ascontiguousarray(cells, dtype=np.int64)
+        g = np.zeros(cells.size)
+        self.lib.orc_grad_fd(self._p(), *[_fp(a) for a in f], _dp(what), C.c_int64(cells.size), _ip(cells),
+                             C.c_double(eps), _dp(g))
+        return g
+
+    def grad_adjoint(self, fields, what):
+        self._omp()
+        f = [_f32(fields[k]).ravel() for k in ("nH2", "Tgas", "Tdust", "vlos")]
+        what = np.ascontiguousarray(what, dtype=np.float64)
+        g = np.zeros(self.n_cells)
+        self.lib.orc_grad_adjoint(self._p(), *[_fp(a) for a in f], _dp(what), _dp(g))
+        return g.reshape(int(self.s.nz), int(self.s.ny), int(self.s.nx))
