@@ -1,0 +1,163 @@
+/* iris_so.h -- C ABI of the B200-native (sm_100a) IRIS-SO hot path.
+ *
+ * The library computes, entirely in hand-written CUDA kernels, the synthetic-observation hot path of
+ * arxiv/paper_2607_01338 (IRIS-SO, PAPER.md sections 3-4):
+ *
+ *   per cell   optically-thin level balance  (Eq. 3.6.1-3.6.3, 3.7.1-3.7.2)
+ *   per cell   line + dust coefficients      (Eq. 3.3.1-3.3.4, 3.2.1-3.2.2)
+ *   per ray    formal solution of the transfer equation for every velocity channel with the
+ *              channel-integrated (erf) profile (Eq. 4.8.5-4.8.7, 4.6.3-4.6.4, 4.4.1)
+ *   per voxel  continuum subtraction and unit conversion (section 4.9-4.10)
+ *   per cube   Gaussian beam (section 4.11) and seeded noise (Eq. 4.12.1)
+ *   optional   reverse-scan adjoint d(sum w * cube) / d n_H2 (section 4 intro)
+ *
+ * Conventions
+ *   - Pointers named d_* are CUDA DEVICE pointers, pointers named h_* are HOST pointers; all are owned
+ *     by the caller.  The library never allocates or frees caller buffers.  A context owns only its
+ *     private scratch (per-cell coefficient planes, one cube-sized temporary when the beam is on).
+ *   - All field arrays are float32 [nz][ny][nx] (x fastest); rays march along z and k = 0 is the FAR
+ *     side (the background enters there), k = nz-1 is nearest the observer.
+ *   - All cube arrays are float32 [ny][nx][nv] (velocity channel fastest).
+ *   - Units are CGS.  v_los > 0 means receding gas; a cell emits at channel velocity v = v_los
+ *     (radio convention; velocity-space reading of Eq. 4.3.1).
+ *   - Every d_* call is asynchronous on `cuda_stream` (a cudaStream_t passed as void*; NULL = the
+ *     legacy default stream) and never synchronises the device.  h_* calls synchronise the stream
+ *     before returning.
+ *   - Argument errors return IRIS_SO_EINVAL before any launch; CUDA failures return IRIS_SO_ECUDA /
+ *     IRIS_SO_ENOMEM.  iris_so_last_error() gives the text.  No exception crosses the ABI.
+ *   - There is no CPU fallback: without a CUDA device iris_so_create fails with IRIS_SO_ECUDA.
+ *   - A context is not thread-safe; use one per host thread / stream.
+ */
+#ifndef IRIS_SO_H_
+#define IRIS_SO_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define IRIS_SO_VERSION 100     /* 0.1.0 */
+#define IRIS_SO_MAX_LEVELS 10
+
+typedef struct iris_so_ctx iris_so_ctx; /* opaque */
+
+typedef enum {
+  IRIS_SO_OK = 0,
+  IRIS_SO_EINVAL = 1,        /* bad argument or configuration */
+  IRIS_SO_EUNSUPPORTED = 2,  /* valid but not implemented combination */
+  IRIS_SO_ECUDA = 3,         /* CUDA runtime / launch failure, or no device */
+  IRIS_SO_ENOMEM = 4         /* device or host allocation failed */
+} iris_so_status;
+
+/* transfer_algo */
+#define IRIS_SO_ALGO_AUTO 0     /* = IRIS_SO_ALGO_WINDOW */
+#define IRIS_SO_ALGO_DENSE 1    /* every (cell, channel) update evaluated; register-resident channel blocks */
+#define IRIS_SO_ALGO_WINDOW 2   /* only channels inside each cell's line window are updated; exact in fp32 */
+
+typedef struct {
+  /* grid: Cartesian analogue of the paper's (r, l, b) lattice; rays = z columns */
+  int32_t nx, ny, nz;
+  double cell_cm;               /* step h along the ray (Eq. 4.8.7) */
+  /* molecule (the paper reads these from a LAMDA file); host arrays, copied by create */
+  int32_t n_levels;             /* 2 .. IRIS_SO_MAX_LEVELS */
+  const double *energy_K;       /* [n_levels]  E_i / k, ascending */
+  const double *weight;         /* [n_levels]  statistical weights g_i */
+  const double *einstein_A;     /* [n_levels * n_levels]  A[u*n + l] (1/s) for u > l, else 0 */
+  const double *coll_down_ref;  /* [n_levels * n_levels]  K_ul(T_ref) (cm^3/s) for u > l, else 0 */
+  double coll_T_ref, coll_T_exp;/* K_ul(T) = K_ul(T_ref) (T / T_ref)^coll_T_exp; upward by Eq. 3.7.2 */
+  int32_t line_upper, line_lower;
+  double nu0_Hz;                /* frequency of the observed transition */
+  double mol_mass_g;            /* m_a of Eq. 3.3.4 */
+  double abundance;             /* tracer molecules per H2 (Eq. 4.2.1) */
+  double microturb_cms;         /* xi: b^2 = 2 k T / m_a + xi^2; 0 = thermal only */
+  double T_bar;                 /* level-balance radiation temperature (Eq. 3.6.2); 0 = none */
+  double T_cmb;                 /* transfer background temperature */
+  double T_inf;                 /* no line above this gas temperature; +inf = off */
+  /* dust (Eq. 3.2.1-3.2.2) */
+  int32_t dust_on;
+  double kappa_gas_cm2_g;       /* opacity per gram of GAS (gas-to-dust ratio folded in) */
+  double mass_per_H2_g;         /* rho_gas = mass_per_H2_g * n_H2 */
+  /* channel grid: channel k has centre v0 + k dv and width dv (Eq. 4.4.1) */
+  int32_t nv;
+  double v0_cms, dv_cms;
+  /* post-processing */
+  int32_t subtract_continuum;   /* 1: cube = total - continuum (section 4.10) */
+  int32_t subtract_space;       /* 0: intensity / Rayleigh-Jeans space, 1: Planck brightness-temperature space */
+  int32_t out_unit;             /* 0: intensity (cgs), 1: T_RJ (Eq. 4.9.2), 2: Planck T_B (Eq. 4.9.1) */
+  double beam_fwhm_px;          /* Gaussian beam FWHM in pixels; 0 = off (section 4.11) */
+  double noise_mu, noise_sigma; /* Eq. 4.12.1, in the output unit; both 0 = off */
+  int32_t noise_gamma_mode;     /* 0: gamma = 1; 1: one gamma ~ U[0,1) per cube */
+  uint64_t seed;                /* noise seed (Philox4x32-10 key) */
+  /* implementation choice, does not change the mathematics */
+  int32_t transfer_algo;        /* IRIS_SO_ALGO_* */
+} iris_so_config;
+
+/* Validates and copies the configuration (including the host arrays), selects the current CUDA device.
+ * On failure *out is NULL; the text is available through iris_so_last_error(NULL). */
+iris_so_status iris_so_create(const iris_so_config *cfg, iris_so_ctx **out);
+void iris_so_destroy(iris_so_ctx *ctx);
+
+/* Text of the last error of this context (or of the last failed create if ctx is NULL).
+ * Valid until the next call on the same context. */
+const char *iris_so_last_error(const iris_so_ctx *ctx);
+const char *iris_so_status_string(iris_so_status s);
+int iris_so_version(void);
+
+/* Number of kernels this context has launched so far (for launch accounting in benchmarks). */
+uint64_t iris_so_launch_count(const iris_so_ctx *ctx);
+
+/* Bytes of device scratch the context holds after its first observe / transfer call. */
+uint64_t iris_so_scratch_bytes(const iris_so_ctx *ctx);
+
+/* K1.  Level fractions x_i (sum_i x_i = 1) of every cell: Eq. 3.6.1 with the ground-state row replaced
+ * by the conservation equation, radiation field B_nu(T_bar), collisions with H2 only (Eq. 3.6.3).
+ * d_pop is [n_levels][n_cells] float32, n_cells = nx*ny*nz. */
+iris_so_status iris_so_levelpop(iris_so_ctx *ctx, const float *d_nH2, const float *d_Tgas, float *d_pop,
+                                void *cuda_stream);
+
+/* K2 + K3 + K4.  Coefficients and formal transfer.  d_pop may be NULL (populations solved internally,
+ * never written) or the output of iris_so_levelpop.  Outputs are specific intensities in CGS
+ * (erg s^-1 cm^-2 Hz^-1 sr^-1): d_I_total [ny][nx][nv] is the channel-averaged total intensity
+ * (Eq. 3.1.2), d_I_cont [ny][nx] the continuum baseline (Eq. 3.1.3); either may be NULL. */
+iris_so_status iris_so_transfer(iris_so_ctx *ctx, const float *d_nH2, const float *d_Tgas,
+                                const float *d_Tdust, const float *d_vlos, const float *d_pop,
+                                float *d_I_total, float *d_I_cont, void *cuda_stream);
+
+/* K1 .. K7.  Whole path: cube [ny][nx][nv] in `out_unit`, continuum-subtracted if configured, then beam
+ * and noise if configured (stage order of PAPER.md:467). */
+iris_so_status iris_so_observe(iris_so_ctx *ctx, const float *d_nH2, const float *d_Tgas,
+                               const float *d_Tdust, const float *d_vlos, float *d_cube, void *cuda_stream);
+
+/* Same as iris_so_observe with `stage_mask` overriding the configured post-processing:
+ * bit 0 = apply the beam, bit 1 = apply the noise (each only if configured). */
+iris_so_status iris_so_observe_stages(iris_so_ctx *ctx, const float *d_nH2, const float *d_Tgas,
+                                      const float *d_Tdust, const float *d_vlos, int32_t stage_mask,
+                                      float *d_cube, void *cuda_stream);
+
+/* Whole path with HOST buffers (pinned or pageable): copies the four fields to the device, runs
+ * iris_so_observe, copies the cube back and synchronises.  h_* fields [nz][ny][nx], h_cube [ny][nx][nv]. */
+iris_so_status iris_so_observe_host(iris_so_ctx *ctx, const float *h_nH2, const float *h_Tgas,
+                                    const float *h_Tdust, const float *h_vlos, float *h_cube,
+                                    void *cuda_stream);
+
+/* K8 + K9.  Gradient of L = sum_{y,x,v} w * cube (noise-free cube, beam applied if configured) with
+ * respect to n_H2 of every cell, by a reverse scan along every ray.  Requires subtract_space = 0 and
+ * out_unit 0 or 1.  d_w [ny][nx][nv], d_grad_nH2 [nz][ny][nx]. */
+iris_so_status iris_so_observe_adjoint(iris_so_ctx *ctx, const float *d_nH2, const float *d_Tgas,
+                                       const float *d_Tdust, const float *d_vlos, const float *d_w,
+                                       float *d_grad_nH2, void *cuda_stream);
+
+/* Stand-alone post-processing stages (also used inside iris_so_observe). */
+/* K6: separable Gaussian beam of FWHM beam_fwhm_px on d_in -> d_out (must not alias), zero padding,
+ * radius ceil(4 sigma), weights normalised to sum 1.  d_tmp is a cube-sized temporary or NULL (context
+ * scratch is used). */
+iris_so_status iris_so_beam(iris_so_ctx *ctx, const float *d_in, float *d_out, float *d_tmp,
+                            void *cuda_stream);
+/* K7: d_cube += gamma (mu + sigma z), z = Box-Muller of Philox4x32-10(key = seed, counter = voxel index). */
+iris_so_status iris_so_noise(iris_so_ctx *ctx, float *d_cube, void *cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* IRIS_SO_H_ */

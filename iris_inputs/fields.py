@@ -43,7 +43,11 @@ def gaussian_random_field(shape, seed, index=-11.0 / 3.0, stream=0):
     g = _fft.irfftn(fk, s=(nz, ny, nx), workers=-1).astype(np.float32, copy=False)
     del fk
     g -= g.mean(dtype=np.float64)
-    g /= np.float32(math.sqrt(float(np.mean(np.square(g, dtype=np.float64)))))
+    rms = math.sqrt(float(np.mean(np.square(g, dtype=np.float64))))
+    if rms > 0.0:                      # a single-cell grid has no fluctuating mode: the field is zero
+        g /= np.float32(rms)
+    else:
+        g[...] = 0.0
     return np.ascontiguousarray(g)
 
 

@@ -1,0 +1,255 @@
+"""ctypes binding of include/iris_so.h: argument marshalling only (every step runs in the CUDA kernels)."""
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libiris_so.so")
+_lib = None
+
+ALGO_AUTO, ALGO_DENSE, ALGO_WINDOW = 0, 1, 2
+
+# every entry point include/iris_so.h declares
+DECLARED_SYMBOLS = (
+    "iris_so_create", "iris_so_destroy", "iris_so_last_error", "iris_so_status_string", "iris_so_version",
+    "iris_so_launch_count", "iris_so_scratch_bytes", "iris_so_levelpop", "iris_so_transfer", "iris_so_observe",
+    "iris_so_observe_stages", "iris_so_observe_host", "iris_so_observe_adjoint", "iris_so_beam", "iris_so_noise",
+)
+
+
+class IrisSOError(RuntimeError):
+    def __init__(self, status, text):
+        super().__init__("iris_so status %d: %s" % (status, text))
+        self.status = status
+
+
+class _Config(C.Structure):
+    _fields_ = [
+        ("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32),
+        ("cell_cm", C.c_double),
+        ("n_levels", C.c_int32),
+        ("energy_K", C.POINTER(C.c_double)), ("weight", C.POINTER(C.c_double)),
+        ("einstein_A", C.POINTER(C.c_double)), ("coll_down_ref", C.POINTER(C.c_double)),
+        ("coll_T_ref", C.c_double), ("coll_T_exp", C.c_double),
+        ("line_upper", C.c_int32), ("line_lower", C.c_int32),
+        ("nu0_Hz", C.c_double), ("mol_mass_g", C.c_double), ("abundance", C.c_double),
+        ("microturb_cms", C.c_double), ("T_bar", C.c_double), ("T_cmb", C.c_double), ("T_inf", C.c_double),
+        ("dust_on", C.c_int32),
+        ("kappa_gas_cm2_g", C.c_double), ("mass_per_H2_g", C.c_double),
+        ("nv", C.c_int32),
+        ("v0_cms", C.c_double), ("dv_cms", C.c_double),
+        ("subtract_continuum", C.c_int32), ("subtract_space", C.c_int32), ("out_unit", C.c_int32),
+        ("beam_fwhm_px", C.c_double), ("noise_mu", C.c_double), ("noise_sigma", C.c_double),
+        ("noise_gamma_mode", C.c_int32),
+        ("seed", C.c_uint64),
+        ("transfer_algo", C.c_int32),
+    ]
+
+
+def lib_path():
+    return _LIB_PATH
+
+
+def load_library():
+    """Load libiris_so.so (built in-tree by paper_2607_01338_b200.build). Raises if it is missing."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIB_PATH):
+        raise IrisSOError(-1, "CUDA library %s is missing: run `python -m paper_2607_01338_b200.build` "
+                              "(there is no CPU fallback)" % _LIB_PATH)
+    lib = C.CDLL(_LIB_PATH)
+    vp, fp, st = C.c_void_p, C.c_void_p, C.c_int
+    lib.iris_so_create.restype = st
+    lib.iris_so_create.argtypes = [C.POINTER(_Config), C.POINTER(vp)]
+    lib.iris_so_destroy.restype = None
+    lib.iris_so_destroy.argtypes = [vp]
+    lib.iris_so_last_error.restype = C.c_char_p
+    lib.iris_so_last_error.argtypes = [vp]
+    lib.iris_so_status_string.restype = C.c_char_p
+    lib.iris_so_status_string.argtypes = [st]
+    lib.iris_so_version.restype = C.c_int
+    lib.iris_so_launch_count.restype = C.c_uint64
+    lib.iris_so_launch_count.argtypes = [vp]
+    lib.iris_so_scratch_bytes.restype = C.c_uint64
+    lib.iris_so_scratch_bytes.argtypes = [vp]
+    lib.iris_so_levelpop.restype = st
+    lib.iris_so_levelpop.argtypes = [vp, fp, fp, fp, vp]
+    lib.iris_so_transfer.restype = st
+    lib.iris_so_transfer.argtypes = [vp, fp, fp, fp, fp, fp, fp, fp, vp]
+    lib.iris_so_observe.restype = st
+    lib.iris_so_observe.argtypes = [vp, fp, fp, fp, fp, fp, vp]
+    lib.iris_so_observe_stages.restype = st
+    lib.iris_so_observe_stages.argtypes = [vp, fp, fp, fp, fp, C.c_int32, fp, vp]
+    lib.iris_so_observe_host.restype = st
+    lib.iris_so_observe_host.argtypes = [vp, fp, fp, fp, fp, fp, vp]
+    lib.iris_so_observe_adjoint.restype = st
+    lib.iris_so_observe_adjoint.argtypes = [vp, fp, fp, fp, fp, fp, fp, vp]
+    lib.iris_so_beam.restype = st
+    lib.iris_so_beam.argtypes = [vp, fp, fp, fp, vp]
+    lib.iris_so_noise.restype = st
+    lib.iris_so_noise.argtypes = [vp, fp, vp]
+    _lib = lib
+    return lib
+
+
+def _make_config(cfg, transfer_algo):
+    keep = [np.ascontiguousarray(np.asarray(getattr(cfg, k), dtype=np.float64))
+            for k in ("energy_K", "weight", "einstein_A", "coll_down_ref")]
+    s = _Config()
+    for name, ctype in _Config._fields_:
+        if name in ("energy_K", "weight", "einstein_A", "coll_down_ref"):
+            continue
+        if name == "n_levels":
+            s.n_levels = len(keep[0])
+        elif name == "transfer_algo":
+            s.transfer_algo = int(transfer_algo)
+        else:
+            val = getattr(cfg, name)
+            setattr(s, name, float(val) if ctype is C.c_double else int(val))
+    ptr = lambda a: a.ctypes.data_as(C.POINTER(C.c_double))
+    s.energy_K, s.weight, s.einstein_A, s.coll_down_ref = (ptr(a) for a in keep)
+    return s, keep
+
+
+class IrisSO:
+    """One iris_so_ctx.  Methods mirror the C entry points; tensors are float32 CUDA torch tensors."""
+
+    def __init__(self, cfg, transfer_algo=ALGO_AUTO):
+        self.lib = load_library()
+        self.cfg = cfg
+        s, keep = _make_config(cfg, transfer_algo)
+        h = C.c_void_p()
+        st = self.lib.iris_so_create(C.byref(s), C.byref(h))
+        if st != 0:
+            raise IrisSOError(st, self.lib.iris_so_last_error(None).decode())
+        self._h = h
+        self.n_levels = int(s.n_levels)
+        self.shape_fields = (int(cfg.nz), int(cfg.ny), int(cfg.nx))
+        self.shape_cube = (int(cfg.ny), int(cfg.nx), int(cfg.nv))
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self.lib.iris_so_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- helpers ---------------------------------------------------------------------------------
+    def _check(self, st):
+        if st != 0:
+            raise IrisSOError(st, self.lib.iris_so_last_error(self._h).decode())
+
+    @staticmethod
+    def _stream():
+        import torch
+        return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+    def _dev(self, t, numel, what):
+        import torch
+        if t is None:
+            return None
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()):
+            raise TypeError("%s must be a contiguous float32 CUDA tensor" % what)
+        if t.numel() != numel:
+            raise ValueError("%s has %d elements, expected %d" % (what, t.numel(), numel))
+        return C.c_void_p(t.data_ptr())
+
+    @property
+    def n_cells(self):
+        return self.shape_fields[0] * self.shape_fields[1] * self.shape_fields[2]
+
+    @property
+    def n_vox(self):
+        return self.shape_cube[0] * self.shape_cube[1] * self.shape_cube[2]
+
+    def launch_count(self):
+        return int(self.lib.iris_so_launch_count(self._h))
+
+    def scratch_bytes(self):
+        return int(self.lib.iris_so_scratch_bytes(self._h))
+
+    # -- entry points ----------------------------------------------------------------------------
+    def levelpop(self, nH2, Tgas, pop=None):
+        import torch
+        n = nH2.numel()
+        if n != self.n_cells:
+            raise ValueError("field has %d cells, context expects %d" % (n, self.n_cells))
+        if pop is None:
+            pop = torch.empty((self.n_levels,) + tuple(nH2.shape), dtype=torch.float32, device=nH2.device)
+        self._check(self.lib.iris_so_levelpop(self._h, self._dev(nH2, n, "nH2"), self._dev(Tgas, n, "Tgas"),
+                                              self._dev(pop, n * self.n_levels, "pop"), self._stream()))
+        return pop
+
+    def transfer(self, nH2, Tgas, Tdust, vlos, pop=None, I_total=None, I_cont=None):
+        import torch
+        n = self.n_cells
+        dev = nH2.device
+        if I_total is None:
+            I_total = torch.empty(self.shape_cube, dtype=torch.float32, device=dev)
+        if I_cont is None:
+            I_cont = torch.empty(self.shape_cube[:2], dtype=torch.float32, device=dev)
+        self._check(self.lib.iris_so_transfer(
+            self._h, self._dev(nH2, n, "nH2"), self._dev(Tgas, n, "Tgas"), self._dev(Tdust, n, "Tdust"),
+            self._dev(vlos, n, "vlos"), self._dev(pop, n * self.n_levels, "pop"),
+            self._dev(I_total, self.n_vox, "I_total"), self._dev(I_cont, self.n_vox // self.shape_cube[2], "I_cont"),
+            self._stream()))
+        return I_total, I_cont
+
+    def observe(self, nH2, Tgas, Tdust, vlos, cube=None, beam=True, noise=True):
+        import torch
+        n = self.n_cells
+        if cube is None:
+            cube = torch.empty(self.shape_cube, dtype=torch.float32, device=nH2.device)
+        args = [self._h, self._dev(nH2, n, "nH2"), self._dev(Tgas, n, "Tgas"), self._dev(Tdust, n, "Tdust"),
+                self._dev(vlos, n, "vlos")]
+        if beam and noise:
+            st = self.lib.iris_so_observe(*args, self._dev(cube, self.n_vox, "cube"), self._stream())
+        else:
+            mask = (1 if beam else 0) | (2 if noise else 0)
+            st = self.lib.iris_so_observe_stages(*args, C.c_int32(mask), self._dev(cube, self.n_vox, "cube"), self._stream())
+        self._check(st)
+        return cube
+
+    def observe_host(self, nH2, Tgas, Tdust, vlos, cube):
+        """Host buffers (numpy arrays or CPU torch tensors, ideally pinned); synchronises."""
+        def hp(a, numel, what):
+            if hasattr(a, "data_ptr"):
+                if a.is_cuda or str(a.dtype) != "torch.float32" or not a.is_contiguous() or a.numel() != numel:
+                    raise TypeError("%s must be a contiguous float32 host tensor of %d elements" % (what, numel))
+                return C.c_void_p(a.data_ptr())
+            if a.dtype != np.float32 or not a.flags.c_contiguous or a.size != numel:
+                raise TypeError("%s must be a C-contiguous float32 array of %d elements" % (what, numel))
+            return C.c_void_p(a.ctypes.data)
+        n = self.n_cells
+        self._check(self.lib.iris_so_observe_host(self._h, hp(nH2, n, "nH2"), hp(Tgas, n, "Tgas"), hp(Tdust, n, "Tdust"),
+                                                  hp(vlos, n, "vlos"), hp(cube, self.n_vox, "cube"), self._stream()))
+        return cube
+
+    def observe_adjoint(self, nH2, Tgas, Tdust, vlos, w, grad=None):
+        import torch
+        n = self.n_cells
+        if grad is None:
+            grad = torch.empty(self.shape_fields, dtype=torch.float32, device=nH2.device)
+        self._check(self.lib.iris_so_observe_adjoint(
+            self._h, self._dev(nH2, n, "nH2"), self._dev(Tgas, n, "Tgas"), self._dev(Tdust, n, "Tdust"),
+            self._dev(vlos, n, "vlos"), self._dev(w, self.n_vox, "w"), self._dev(grad, n, "grad"), self._stream()))
+        return grad
+
+    def beam(self, cube_in, cube_out=None, tmp=None):
+        import torch
+        if cube_out is None:
+            cube_out = torch.empty_like(cube_in)
+        self._check(self.lib.iris_so_beam(self._h, self._dev(cube_in, self.n_vox, "cube_in"),
+                                          self._dev(cube_out, self.n_vox, "cube_out"),
+                                          self._dev(tmp, self.n_vox, "tmp"), self._stream()))
+        return cube_out
+
+    def noise(self, cube):
+        self._check(self.lib.iris_so_noise(self._h, self._dev(cube, self.n_vox, "cube"), self._stream()))
+        return cube

@@ -1,0 +1,167 @@
+// K1 (level populations) and K2 (per-cell transfer coefficients), one thread per cell.
+//
+// K1 solves the statistical equilibrium of Eq. 3.6.1 with the rates of
+// Eq. 3.6.2-3.6.3 and 3.7.1-3.7.2 for the level FRACTIONS x_i.  The system is the stationary
+// distribution of a continuous-time Markov chain on the levels; it is solved in registers by the
+// subtraction-free Grassmann-Taksar-Heyman state elimination, which carries component-wise relative
+// accuracy over the ~30 decades the populations span (partial-pivot GE in fp32 does not guarantee it).
+//
+// K2 turns (x_u, x_l, n_H2, T_gas, T_dust, v_los) into the six scaled per-cell coefficients the march
+// consumes (Eq. 3.3.1-3.3.4, 3.2.1-3.2.2, 4.6.3-4.6.4 folded with the step h and the unit conversion):
+//   e_c   = K_RJ (h nu0 / 4 pi) X n x_u A_ul h / (2 dnu_W)            [K per unit erf-difference]
+//   a_c   =      (h nu0 / 4 pi) X n (x_l B_lu - x_u B_ul) h / (2 dnu_W)  [optical depth per unit erf-difference]
+//   c_los = (v_los - v0) / dv + 1/2     line centre in channel-edge index units (edge k <-> index k)
+//   s     = dv / b,  b = sqrt(2 k T / m_a + xi^2)                     [Doppler widths per channel]
+//   tau_d = kappa rho_gas h                                            [dust optical depth of the cell]
+//   S_d   = K_RJ B_nu0(T_dust) = (h nu0 / k) / (exp(h nu0 / k T_dust) - 1)   [K]
+// so that for channel k:  tau_L = a_c * dErf_k,  J_L = e_c * dErf_k,  dErf_k = erf((k+1-c_los) s) - erf((k-c_los) s).
+// Intensities are carried as Rayleigh-Jeans-equivalent Kelvin (I * c^2 / (2 k nu0^2)): CGS intensities
+// (~1e-15) times path lengths (~1e18) would otherwise leave the fp32 range (PAPER.md:268 warns of this).
+#pragma once
+#include "iris_math.cuh"
+
+namespace iris {
+
+constexpr int kMaxLevels = 10;
+constexpr int kMaxPairs = kMaxLevels * (kMaxLevels - 1) / 2;
+
+// pair index of (u > l)
+__host__ __device__ constexpr int pair_index(int u, int l) { return u * (u - 1) / 2 + l; }
+
+struct LevelConsts {
+  float dE_adj[kMaxLevels];     // (E_i - E_{i-1}) / k  [K], i >= 1
+  float rad_down[kMaxPairs];    // A_ul + B_ul J_ul = A_ul (1 + n_gamma)
+  float rad_up[kMaxPairs];      // B_lu J_ul = (g_u / g_l) A_ul n_gamma
+  float coll[kMaxPairs];        // K_ul(T_ref)
+  float coll_gr[kMaxPairs];     // K_ul(T_ref) g_u / g_l
+  float inv_Tref, Texp;
+};
+
+struct CoefConsts {
+  int upper, lower;
+  float gr;          // g_u / g_l of the line
+  float c_e, c_a;    // e_c = c_e n x_u ; a_c = c_a n (x_l gr - x_u)
+  float c_d;         // tau_d = c_d n  (0 if dust off)
+  float hnu_k;       // h nu0 / k  [K]
+  float c_b, xi2;    // b^2 = c_b T + xi2  [(cm/s)^2]
+  float dv, inv_dv, v0;
+  float T_inf;
+  int dust_on;
+};
+
+// Level fractions of one cell.  N is a template parameter so that the rate matrix lives in registers.
+template <int N>
+__device__ __forceinline__ void level_fractions(const LevelConsts& lc, float n, float T, float (&x)[N]) {
+  float R[N][N];   // R[i][j]: rate i -> j (i != j)
+  const float invT = 1.0f / T;
+  // n * (T / T_ref)^p
+  const float kf = n * exp2f(lc.Texp * log2f(T * lc.inv_Tref));
+  float q[N];      // Boltzmann factors of adjacent levels, exp(-(E_i - E_{i-1}) / T)
+#pragma unroll
+  for (int i = 1; i < N; ++i) q[i] = expf(-lc.dE_adj[i] * invT);
+#pragma unroll
+  for (int u = 1; u < N; ++u) {
+    float bz = 1.0f;
+#pragma unroll
+    for (int l = u - 1; l >= 0; --l) {
+      bz *= q[l + 1];                                   // exp(-(E_u - E_l) / T), Eq. 3.7.2
+      const int p = pair_index(u, l);
+      R[u][l] = fmaf(kf, lc.coll[p], lc.rad_down[p]);
+      R[l][u] = fmaf(kf * bz, lc.coll_gr[p], lc.rad_up[p]);
+    }
+  }
+  // GTH elimination of states N-1 .. 1
+#pragma unroll
+  for (int m = N - 1; m >= 1; --m) {
+    float s = 0.0f;
+#pragma unroll
+    for (int j = 0; j < m; ++j) s += R[m][j];
+    const float inv = 1.0f / s;
+#pragma unroll
+    for (int i = 0; i < m; ++i) R[i][m] *= inv;
+#pragma unroll
+    for (int i = 0; i < m; ++i)
+#pragma unroll
+      for (int j = 0; j < m; ++j)
+        if (i != j) R[i][j] = fmaf(R[i][m], R[m][j], R[i][j]);
+  }
+  x[0] = 1.0f;
+  float tot = 1.0f;
+#pragma unroll
+  for (int j = 1; j < N; ++j) {
+    float s = 0.0f;
+#pragma unroll
+    for (int i = 0; i < j; ++i) s = fmaf(x[i], R[i][j], s);
+    x[j] = s;
+    tot += s;
+  }
+  const float inv = 1.0f / tot;
+#pragma unroll
+  for (int j = 0; j < N; ++j) x[j] *= inv;
+}
+
+// Six coefficient planes of one cell from its line-level fractions.
+__device__ __forceinline__ void cell_coefficients(const CoefConsts& cc, float n, float T, float Td, float vlos,
+                                                  float xu, float xl, float (&o)[6]) {
+  float e = cc.c_e * n * xu;
+  float a = cc.c_a * n * fmaf(xl, cc.gr, -xu);
+  if (T > cc.T_inf) { e = 0.0f; a = 0.0f; }
+  o[0] = e;
+  o[1] = a;
+  o[2] = fmaf(vlos - cc.v0, cc.inv_dv, 0.5f);
+  o[3] = cc.dv * rsqrtf(fmaf(cc.c_b, T, cc.xi2));
+  o[4] = cc.c_d * n;
+  o[5] = cc.dust_on ? cc.hnu_k / expm1f(cc.hnu_k / Td) : 0.0f;
+}
+
+// K1: pop[N][ncell]
+template <int N>
+__global__ void __launch_bounds__(128) levelpop_kernel(LevelConsts lc, int64_t ncell, const float* __restrict__ nH2,
+                                                       const float* __restrict__ Tgas, float* __restrict__ pop) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= ncell) return;
+  float x[N];
+  level_fractions<N>(lc, nH2[i], Tgas[i], x);
+#pragma unroll
+  for (int l = 0; l < N; ++l) pop[(int64_t)l * ncell + i] = x[l];
+}
+
+// K1 + K2 fused: coef[6][ncell]; populations never leave registers.
+template <int N>
+__global__ void __launch_bounds__(128) cellcoef_kernel(LevelConsts lc, CoefConsts cc, int64_t ncell,
+                                                       const float* __restrict__ nH2, const float* __restrict__ Tgas,
+                                                       const float* __restrict__ Tdust, const float* __restrict__ vlos,
+                                                       float* __restrict__ coef) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= ncell) return;
+  const float n = nH2[i], T = Tgas[i];
+  float x[N];
+  level_fractions<N>(lc, n, T, x);
+  float xu = 0.0f, xl = 0.0f;
+#pragma unroll
+  for (int l = 0; l < N; ++l) {       // static indexing keeps x[] in registers
+    if (l == cc.upper) xu = x[l];
+    if (l == cc.lower) xl = x[l];
+  }
+  float o[6];
+  cell_coefficients(cc, n, T, Tdust[i], vlos[i], xu, xl, o);
+#pragma unroll
+  for (int q = 0; q < 6; ++q) coef[(int64_t)q * ncell + i] = o[q];
+}
+
+// K2 alone, from caller-supplied populations pop[N][ncell].
+__global__ void __launch_bounds__(256) coef_from_pop_kernel(CoefConsts cc, int64_t ncell, const float* __restrict__ nH2,
+                                                            const float* __restrict__ Tgas,
+                                                            const float* __restrict__ Tdust,
+                                                            const float* __restrict__ vlos,
+                                                            const float* __restrict__ pop, float* __restrict__ coef) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= ncell) return;
+  float o[6];
+  cell_coefficients(cc, nH2[i], Tgas[i], Tdust[i], vlos[i], pop[(int64_t)cc.upper * ncell + i],
+                    pop[(int64_t)cc.lower * ncell + i], o);
+#pragma unroll
+  for (int q = 0; q < 6; ++q) coef[(int64_t)q * ncell + i] = o[q];
+}
+
+}  // namespace iris

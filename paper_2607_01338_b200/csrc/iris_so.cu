@@ -1,0 +1,483 @@
+// Host side of the C ABI declared in include/iris_so.h: configuration, constant folding (in double),
+// scratch management and kernel launches.  Every step of the path runs in the kernels of this directory;
+// there is no CPU fallback.
+#include "../../include/iris_so.h"
+
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "cell_kernels.cuh"
+#include "post_kernels.cuh"
+#include "transfer_dense.cuh"
+#include "transfer_window.cuh"
+#include "adjoint_kernels.cuh"
+
+namespace {
+
+// CODATA-2018 exact SI values in CGS (this translation unit's own copy).
+constexpr double H_PLANCK = 6.62607015e-27;
+constexpr double K_BOLTZ = 1.380649e-16;
+constexpr double C_LIGHT = 2.99792458e10;
+constexpr double PI = 3.14159265358979323846;
+
+thread_local std::string g_create_error;
+
+}  // namespace
+
+struct iris_so_ctx {
+  iris_so_config cfg;
+  std::vector<double> energy, weight, A, Kd;
+  iris::LevelConsts lc;
+  iris::CoefConsts cc;
+  iris::MarchConsts mc;
+  iris::BeamConsts bc;
+  iris::NoiseConsts nc;
+  iris::AdjointConsts ac;
+  int device = 0, sm_count = 0;
+  int64_t ncell = 0, npix = 0, nvox = 0;
+  float* d_coef = nullptr;      // [6][ncell]
+  float* d_tmp = nullptr;       // cube-sized temporary (beam)
+  float* d_stage = nullptr;     // host-path staging: 4 fields + cube
+  float* d_adj = nullptr;       // adjoint scratch
+  size_t adj_bytes = 0;
+  uint64_t scratch_bytes = 0;
+  uint64_t launches = 0;
+  std::string err;
+};
+
+namespace {
+
+iris_so_status fail(iris_so_ctx* ctx, iris_so_status s, const std::string& msg) {
+  if (ctx) ctx->err = msg; else g_create_error = msg;
+  return s;
+}
+
+iris_so_status cuda_fail(iris_so_ctx* ctx, cudaError_t e, const char* what) {
+  char buf[512];
+  snprintf(buf, sizeof buf, "%s: %s", what, cudaGetErrorString(e));
+  return fail(ctx, e == cudaErrorMemoryAllocation ? IRIS_SO_ENOMEM : IRIS_SO_ECUDA, buf);
+}
+
+#define IRIS_CHECK_LAUNCH(ctx, name)                                         \
+  do {                                                                       \
+    (ctx)->launches++;                                                       \
+    cudaError_t e_ = cudaGetLastError();                                     \
+    if (e_ != cudaSuccess) return cuda_fail((ctx), e_, "launch of " name);   \
+  } while (0)
+
+iris_so_status ensure(iris_so_ctx* ctx, float** p, size_t bytes, const char* what) {
+  if (*p) return IRIS_SO_OK;
+  cudaError_t e = cudaMalloc(reinterpret_cast<void**>(p), bytes);
+  if (e != cudaSuccess) { *p = nullptr; cudaGetLastError(); return cuda_fail(ctx, e, what); }
+  ctx->scratch_bytes += bytes;
+  return IRIS_SO_OK;
+}
+
+double planck_krj(double hnu_k, double T) { return T > 0.0 ? hnu_k / std::expm1(hnu_k / T) : 0.0; }
+
+void host_philox(uint64_t seed, uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t out[4]) {
+  uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+  for (int r = 0; r < 10; ++r) {
+    const uint64_t p0 = (uint64_t)0xD2511F53u * c0, p1 = (uint64_t)0xCD9E8D57u * c2;
+    const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0, n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1;
+    c0 = n0; c1 = (uint32_t)p1; c2 = n2; c3 = (uint32_t)p0;
+    k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+  }
+  out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+iris_so_status validate(const iris_so_config* c, std::string& why) {
+  auto bad = [&](const char* m) { why = m; return IRIS_SO_EINVAL; };
+  if (!c) return bad("config is NULL");
+  if (c->nx < 1 || c->ny < 1 || c->nz < 1) return bad("grid dimensions must be >= 1");
+  if ((int64_t)c->nx * c->ny * c->nz > (int64_t)1 << 30) return bad("grid too large (> 2^30 cells)");
+  if (!(c->cell_cm > 0.0)) return bad("cell_cm must be > 0");
+  if (c->n_levels < 2 || c->n_levels > IRIS_SO_MAX_LEVELS) return bad("n_levels must be in [2, 10]");
+  if (!c->energy_K || !c->weight || !c->einstein_A || !c->coll_down_ref) return bad("molecule arrays must not be NULL");
+  const int N = c->n_levels;
+  for (int i = 0; i < N; ++i) {
+    if (!(c->weight[i] > 0.0)) return bad("statistical weights must be > 0");
+    if (i > 0 && !(c->energy_K[i] > c->energy_K[i - 1])) return bad("energy_K must be strictly ascending");
+  }
+  for (int u = 0; u < N; ++u) {
+    double down = 0.0;
+    for (int l = 0; l < N; ++l) {
+      const double a = c->einstein_A[u * N + l], k = c->coll_down_ref[u * N + l];
+      if (l >= u && (a != 0.0 || k != 0.0)) return bad("einstein_A / coll_down_ref must be 0 for u <= l");
+      if (a < 0.0 || k < 0.0 || !std::isfinite(a) || !std::isfinite(k)) return bad("rates must be finite and >= 0");
+      down += a + k;
+    }
+    if (u > 0 && !(down > 0.0)) return bad("every excited level needs a downward rate");
+  }
+  if (!(c->coll_T_ref > 0.0)) return bad("coll_T_ref must be > 0");
+  if (c->line_upper <= c->line_lower || c->line_lower < 0 || c->line_upper >= N) return bad("bad line levels");
+  if (!(c->einstein_A[c->line_upper * N + c->line_lower] > 0.0)) return bad("observed line has no Einstein A");
+  if (!(c->nu0_Hz > 0.0) || !(c->mol_mass_g > 0.0)) return bad("nu0_Hz and mol_mass_g must be > 0");
+  if (!(c->abundance >= 0.0) || !(c->microturb_cms >= 0.0)) return bad("abundance and microturb_cms must be >= 0");
+  if (!(c->T_bar >= 0.0) || !(c->T_cmb >= 0.0)) return bad("T_bar and T_cmb must be >= 0");
+  if (std::isnan(c->T_inf)) return bad("T_inf is NaN");
+  if (c->dust_on && (!(c->kappa_gas_cm2_g >= 0.0) || !(c->mass_per_H2_g > 0.0))) return bad("bad dust parameters");
+  if (c->nv < 1 || c->nv > 65536) return bad("nv must be in [1, 65536]");
+  if (!(c->dv_cms > 0.0) || !std::isfinite(c->v0_cms)) return bad("bad channel grid");
+  if (c->subtract_space < 0 || c->subtract_space > 1 || c->out_unit < 0 || c->out_unit > 2) return bad("bad output mode");
+  if (c->subtract_continuum && c->subtract_space == 1 && c->out_unit != 2)
+    return bad("Planck-space subtraction yields Kelvin: out_unit must be 2");
+  if (!(c->beam_fwhm_px >= 0.0)) return bad("beam_fwhm_px must be >= 0");
+  if (!(c->noise_sigma >= 0.0) || !std::isfinite(c->noise_mu)) return bad("bad noise parameters");
+  if (c->noise_gamma_mode < 0 || c->noise_gamma_mode > 1) return bad("bad noise_gamma_mode");
+  if (c->transfer_algo < 0 || c->transfer_algo > 2) return bad("bad transfer_algo");
+  return IRIS_SO_OK;
+}
+
+int out_mode_of(const iris_so_config& c) {
+  if (c.subtract_continuum) {
+    if (c.subtract_space == 1) return iris::OUT_TB_SUB;
+    return c.out_unit == 1 ? iris::OUT_TRJ_SUB : c.out_unit == 0 ? iris::OUT_I_SUB : iris::OUT_TB_OF_SUB;
+  }
+  return c.out_unit == 1 ? iris::OUT_TRJ_TOT : c.out_unit == 0 ? iris::OUT_I_TOT : iris::OUT_TB_OF_TOT;
+}
+
+void fold_constants(iris_so_ctx* ctx) {
+  const iris_so_config& c = ctx->cfg;
+  const int N = c.n_levels;
+  iris::LevelConsts& lc = ctx->lc;
+  std::memset(&lc, 0, sizeof lc);
+  for (int i = 1; i < N; ++i) lc.dE_adj[i] = (float)(ctx->energy[i] - ctx->energy[i - 1]);
+  for (int u = 1; u < N; ++u)
+    for (int l = 0; l < u; ++l) {
+      const int p = iris::pair_index(u, l);
+      const double A = ctx->A[u * N + l], K = ctx->Kd[u * N + l];
+      const double gr = ctx->weight[u] / ctx->weight[l];
+      double ngam = 0.0;
+      if (A > 0.0 && c.T_bar > 0.0) {
+        const double hnu_k = ctx->energy[u] - ctx->energy[l];   // h nu_ul / k
+        ngam = 1.0 / std::expm1(hnu_k / c.T_bar);               // photon occupation of B_nu(T_bar), Eq. 3.6.2
+      }
+      lc.rad_down[p] = (float)(A * (1.0 + ngam));               // A_ul + B_ul J
+      lc.rad_up[p] = (float)(gr * A * ngam);                    // B_lu J
+      lc.coll[p] = (float)K;
+      lc.coll_gr[p] = (float)(K * gr);
+    }
+  lc.inv_Tref = (float)(1.0 / c.coll_T_ref);
+  lc.Texp = (float)c.coll_T_exp;
+
+  const int u = c.line_upper, l = c.line_lower;
+  const double nu = c.nu0_Hz, A = ctx->A[u * N + l];
+  const double gr = ctx->weight[u] / ctx->weight[l];
+  const double Bul = C_LIGHT * C_LIGHT / (2.0 * H_PLANCK * nu * nu * nu) * A;   // Eq. 3.7.1
+  const double KRJ = C_LIGHT * C_LIGHT / (2.0 * K_BOLTZ * nu * nu);             // Eq. 4.9.2
+  const double dnuW = nu * c.dv_cms / C_LIGHT;                                  // channel width in Hz
+  const double pref = H_PLANCK * nu / (4.0 * PI) * c.abundance * c.cell_cm / (2.0 * dnuW);
+  iris::CoefConsts& cc = ctx->cc;
+  cc.upper = u; cc.lower = l; cc.gr = (float)gr;
+  cc.c_e = (float)(KRJ * pref * A);
+  cc.c_a = (float)(pref * Bul);
+  cc.c_d = c.dust_on ? (float)(c.kappa_gas_cm2_g * c.mass_per_H2_g * c.cell_cm) : 0.0f;
+  cc.hnu_k = (float)(H_PLANCK * nu / K_BOLTZ);
+  cc.c_b = (float)(2.0 * K_BOLTZ / c.mol_mass_g);
+  cc.xi2 = (float)(c.microturb_cms * c.microturb_cms);
+  cc.dv = (float)c.dv_cms; cc.inv_dv = (float)(1.0 / c.dv_cms); cc.v0 = (float)c.v0_cms;
+  cc.T_inf = std::isinf(c.T_inf) ? INFINITY : (float)c.T_inf;
+  cc.dust_on = c.dust_on ? 1 : 0;
+
+  iris::MarchConsts& mc = ctx->mc;
+  mc.hnu_k = cc.hnu_k;
+  mc.T_bg = (float)planck_krj(H_PLANCK * nu / K_BOLTZ, c.T_cmb);
+  mc.inv_KRJ = (float)(1.0 / KRJ);
+  mc.out_mode = out_mode_of(c);
+
+  iris::BeamConsts& bc = ctx->bc;
+  std::memset(&bc, 0, sizeof bc);
+  if (c.beam_fwhm_px > 0.0) {
+    const double sigma = c.beam_fwhm_px / (2.0 * std::sqrt(2.0 * std::log(2.0)));
+    const int R = (int)std::ceil(4.0 * sigma);
+    bc.R = R;
+    double g[2 * iris::kMaxBeamRadius + 1], s = 0.0;
+    for (int d = -R; d <= R; ++d) { g[d + R] = std::exp(-0.5 * d * d / (sigma * sigma)); s += g[d + R]; }
+    for (int d = 0; d <= 2 * R; ++d) bc.g[d] = (float)(g[d] / s);
+  }
+
+  iris::NoiseConsts& nc = ctx->nc;
+  nc.k0 = (uint32_t)c.seed; nc.k1 = (uint32_t)(c.seed >> 32);
+  double gamma = 1.0;
+  if (c.noise_gamma_mode == 1) {
+    uint32_t r[4];
+    host_philox(c.seed, 0u, 0u, 1u, 0u, r);
+    gamma = (double)(r[0] >> 8) / 16777216.0;
+  }
+  nc.mu = (float)(gamma * c.noise_mu);
+  nc.sigma = (float)(gamma * c.noise_sigma);
+  nc.on = (c.noise_sigma != 0.0 || c.noise_mu != 0.0) ? 1 : 0;
+
+  iris::AdjointConsts& ac = ctx->ac;
+  ac.c_e = cc.c_e; ac.c_a = cc.c_a; ac.c_d = cc.c_d; ac.gr = cc.gr; ac.upper = u; ac.lower = l;
+  ac.T_inf = cc.T_inf;
+  ac.scale = c.out_unit == 1 ? 1.0f : mc.inv_KRJ;      // dL/dD in Kelvin space
+  ac.subtract = c.subtract_continuum ? 1 : 0;
+}
+
+template <int N>
+void launch_levelpop(iris_so_ctx* ctx, const float* n, const float* T, float* pop, cudaStream_t st) {
+  const int64_t nc = ctx->ncell;
+  iris::levelpop_kernel<N><<<(unsigned)((nc + 127) / 128), 128, 0, st>>>(ctx->lc, nc, n, T, pop);
+}
+
+template <int N>
+void launch_cellcoef(iris_so_ctx* ctx, const float* n, const float* T, const float* Td, const float* v, float* coef,
+                     cudaStream_t st) {
+  const int64_t nc = ctx->ncell;
+  iris::cellcoef_kernel<N><<<(unsigned)((nc + 127) / 128), 128, 0, st>>>(ctx->lc, ctx->cc, nc, n, T, Td, v, coef);
+}
+
+#define IRIS_DISPATCH_N(N_, CALL)                       \
+  switch (N_) {                                         \
+    case 2: CALL(2); break;  case 3: CALL(3); break;    \
+    case 4: CALL(4); break;  case 5: CALL(5); break;    \
+    case 6: CALL(6); break;  case 7: CALL(7); break;    \
+    case 8: CALL(8); break;  case 9: CALL(9); break;    \
+    default: CALL(10); break;                           \
+  }
+
+// K1+K2 (or K2 from caller populations) into ctx->d_coef
+iris_so_status run_coefficients(iris_so_ctx* ctx, const float* n, const float* T, const float* Td, const float* v,
+                                const float* pop, cudaStream_t st) {
+  iris_so_status s = ensure(ctx, &ctx->d_coef, sizeof(float) * 6 * (size_t)ctx->ncell, "cudaMalloc(coefficient planes)");
+  if (s != IRIS_SO_OK) return s;
+  if (pop) {
+    iris::coef_from_pop_kernel<<<(unsigned)((ctx->ncell + 255) / 256), 256, 0, st>>>(ctx->cc, ctx->ncell, n, T, Td, v, pop,
+                                                                                     ctx->d_coef);
+    IRIS_CHECK_LAUNCH(ctx, "coef_from_pop_kernel");
+  } else {
+#define CALL_(N) launch_cellcoef<N>(ctx, n, T, Td, v, ctx->d_coef, st)
+    IRIS_DISPATCH_N(ctx->cfg.n_levels, CALL_)
+#undef CALL_
+    IRIS_CHECK_LAUNCH(ctx, "cellcoef_kernel");
+  }
+  return IRIS_SO_OK;
+}
+
+// K3 (+K4, K5) from ctx->d_coef
+iris_so_status run_transfer(iris_so_ctx* ctx, const iris::MarchConsts& mc, float* out, float* out_cont, cudaStream_t st) {
+  const bool dust = ctx->cfg.dust_on != 0;
+  const int npix = (int)ctx->npix, nz = ctx->cfg.nz, nv = ctx->cfg.nv;
+  int algo = ctx->cfg.transfer_algo;
+  if (algo == IRIS_SO_ALGO_AUTO) algo = IRIS_SO_ALGO_WINDOW;
+  if (algo == IRIS_SO_ALGO_DENSE) {
+    constexpr int CB = 16, NW = 4;
+    dim3 block(32, NW), grid((npix + 31) / 32, (nv + CB * NW - 1) / (CB * NW));
+    if (dust) iris::transfer_dense_kernel<CB, true><<<grid, block, 0, st>>>(mc, ctx->d_coef, ctx->ncell, npix, nz, nv, out, out_cont);
+    else iris::transfer_dense_kernel<CB, false><<<grid, block, 0, st>>>(mc, ctx->d_coef, ctx->ncell, npix, nz, nv, out, out_cont);
+    IRIS_CHECK_LAUNCH(ctx, "transfer_dense_kernel");
+    return IRIS_SO_OK;
+  }
+  cudaError_t e = iris::launch_transfer_window(mc, ctx->d_coef, ctx->ncell, npix, nz, nv, dust, ctx->sm_count, out, out_cont, st);
+  ctx->launches++;
+  if (e != cudaSuccess) return cuda_fail(ctx, e, "launch of transfer_window_kernel");
+  return IRIS_SO_OK;
+}
+
+iris_so_status run_beam(iris_so_ctx* ctx, const float* in, float* out, float* tmp, bool noise, cudaStream_t st) {
+  const iris_so_config& c = ctx->cfg;
+  if (!tmp) {
+    iris_so_status s = ensure(ctx, &ctx->d_tmp, sizeof(float) * (size_t)ctx->nvox, "cudaMalloc(beam temporary)");
+    if (s != IRIS_SO_OK) return s;
+    tmp = ctx->d_tmp;
+  }
+  iris::NoiseConsts off = ctx->nc; off.on = 0;
+  iris::NoiseConsts nz2 = ctx->nc; nz2.on = noise ? ctx->nc.on : 0;
+  dim3 block(32, 8);
+  // pass 1 along x: a = x (stride nv), b = y (stride nx*nv)
+  dim3 g1((c.nv + 31) / 32, (c.nx + iris::kBeamTA - 1) / iris::kBeamTA, c.ny);
+  iris::beam_pass_kernel<<<g1, block, 0, st>>>(ctx->bc, off, in, tmp, c.nx, c.ny, c.nv, (int64_t)c.nv, (int64_t)c.nx * c.nv);
+  IRIS_CHECK_LAUNCH(ctx, "beam_pass_kernel(x)");
+  // pass 2 along y: a = y (stride nx*nv), b = x (stride nv)
+  dim3 g2((c.nv + 31) / 32, (c.ny + iris::kBeamTA - 1) / iris::kBeamTA, c.nx);
+  iris::beam_pass_kernel<<<g2, block, 0, st>>>(ctx->bc, nz2, tmp, out, c.ny, c.nx, c.nv, (int64_t)c.nx * c.nv, (int64_t)c.nv);
+  IRIS_CHECK_LAUNCH(ctx, "beam_pass_kernel(y)");
+  return IRIS_SO_OK;
+}
+
+iris_so_status run_noise(iris_so_ctx* ctx, float* cube, cudaStream_t st) {
+  iris::noise_kernel<<<(unsigned)((ctx->nvox + 255) / 256), 256, 0, st>>>(ctx->nc, cube, ctx->nvox);
+  IRIS_CHECK_LAUNCH(ctx, "noise_kernel");
+  return IRIS_SO_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int iris_so_version(void) { return IRIS_SO_VERSION; }
+
+const char* iris_so_status_string(iris_so_status s) {
+  switch (s) {
+    case IRIS_SO_OK: return "ok";
+    case IRIS_SO_EINVAL: return "invalid argument";
+    case IRIS_SO_EUNSUPPORTED: return "unsupported";
+    case IRIS_SO_ECUDA: return "CUDA error";
+    case IRIS_SO_ENOMEM: return "out of memory";
+  }
+  return "unknown";
+}
+
+const char* iris_so_last_error(const iris_so_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_error.c_str(); }
+
+uint64_t iris_so_launch_count(const iris_so_ctx* ctx) { return ctx ? ctx->launches : 0; }
+uint64_t iris_so_scratch_bytes(const iris_so_ctx* ctx) { return ctx ? ctx->scratch_bytes : 0; }
+
+iris_so_status iris_so_create(const iris_so_config* cfg, iris_so_ctx** out) {
+  if (!out) return fail(nullptr, IRIS_SO_EINVAL, "out is NULL");
+  *out = nullptr;
+  std::string why;
+  iris_so_status s = validate(cfg, why);
+  if (s != IRIS_SO_OK) return fail(nullptr, s, why);
+  if (cfg->beam_fwhm_px > 0.0) {
+    const double sigma = cfg->beam_fwhm_px / (2.0 * std::sqrt(2.0 * std::log(2.0)));
+    if ((int)std::ceil(4.0 * sigma) > iris::kMaxBeamRadius)
+      return fail(nullptr, IRIS_SO_EUNSUPPORTED, "beam radius ceil(4 sigma) exceeds 32 pixels");
+  }
+  int dev = 0, count = 0;
+  cudaError_t e = cudaGetDeviceCount(&count);
+  if (e != cudaSuccess || count == 0) {
+    cudaGetLastError();
+    return fail(nullptr, IRIS_SO_ECUDA, "no CUDA device: this library has no CPU fallback");
+  }
+  if ((e = cudaGetDevice(&dev)) != cudaSuccess) return cuda_fail(nullptr, e, "cudaGetDevice");
+  iris_so_ctx* ctx = new (std::nothrow) iris_so_ctx;
+  if (!ctx) return fail(nullptr, IRIS_SO_ENOMEM, "host allocation failed");
+  ctx->cfg = *cfg;
+  const int N = cfg->n_levels;
+  ctx->energy.assign(cfg->energy_K, cfg->energy_K + N);
+  ctx->weight.assign(cfg->weight, cfg->weight + N);
+  ctx->A.assign(cfg->einstein_A, cfg->einstein_A + N * N);
+  ctx->Kd.assign(cfg->coll_down_ref, cfg->coll_down_ref + N * N);
+  ctx->cfg.energy_K = ctx->energy.data(); ctx->cfg.weight = ctx->weight.data();
+  ctx->cfg.einstein_A = ctx->A.data(); ctx->cfg.coll_down_ref = ctx->Kd.data();
+  ctx->device = dev;
+  cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, dev);
+  ctx->npix = (int64_t)cfg->nx * cfg->ny;
+  ctx->ncell = ctx->npix * cfg->nz;
+  ctx->nvox = ctx->npix * cfg->nv;
+  fold_constants(ctx);
+  *out = ctx;
+  return IRIS_SO_OK;
+}
+
+void iris_so_destroy(iris_so_ctx* ctx) {
+  if (!ctx) return;
+  cudaFree(ctx->d_coef); cudaFree(ctx->d_tmp); cudaFree(ctx->d_stage); cudaFree(ctx->d_adj);
+  delete ctx;
+}
+
+iris_so_status iris_so_levelpop(iris_so_ctx* ctx, const float* d_nH2, const float* d_Tgas, float* d_pop, void* stream) {
+  if (!ctx) return IRIS_SO_EINVAL;
+  if (!d_nH2 || !d_Tgas || !d_pop) return fail(ctx, IRIS_SO_EINVAL, "iris_so_levelpop: NULL pointer");
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+#define CALL_(N) launch_levelpop<N>(ctx, d_nH2, d_Tgas, d_pop, st)
+  IRIS_DISPATCH_N(ctx->cfg.n_levels, CALL_)
+#undef CALL_
+  IRIS_CHECK_LAUNCH(ctx, "levelpop_kernel");
+  return IRIS_SO_OK;
+}
+
+iris_so_status iris_so_transfer(iris_so_ctx* ctx, const float* d_nH2, const float* d_Tgas, const float* d_Tdust,
+                                const float* d_vlos, const float* d_pop, float* d_I_total, float* d_I_cont, void* stream) {
+  if (!ctx) return IRIS_SO_EINVAL;
+  if (!d_nH2 || !d_Tgas || !d_Tdust || !d_vlos) return fail(ctx, IRIS_SO_EINVAL, "iris_so_transfer: NULL field pointer");
+  if (!d_I_total && !d_I_cont) return fail(ctx, IRIS_SO_EINVAL, "iris_so_transfer: no output requested");
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  iris_so_status s = run_coefficients(ctx, d_nH2, d_Tgas, d_Tdust, d_vlos, d_pop, st);
+  if (s != IRIS_SO_OK) return s;
+  iris::MarchConsts mc = ctx->mc;
+  mc.out_mode = iris::OUT_I_TOT;
+  return run_transfer(ctx, mc, d_I_total, d_I_cont, st);
+}
+
+iris_so_status iris_so_observe_stages(iris_so_ctx* ctx, const float* d_nH2, const float* d_Tgas, const float* d_Tdust,
+                                      const float* d_vlos, int32_t stage_mask, float* d_cube, void* stream) {
+  if (!ctx) return IRIS_SO_EINVAL;
+  if (!d_nH2 || !d_Tgas || !d_Tdust || !d_vlos || !d_cube) return fail(ctx, IRIS_SO_EINVAL, "iris_so_observe: NULL pointer");
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  iris_so_status s = run_coefficients(ctx, d_nH2, d_Tgas, d_Tdust, d_vlos, nullptr, st);
+  if (s != IRIS_SO_OK) return s;
+  if ((s = run_transfer(ctx, ctx->mc, d_cube, nullptr, st)) != IRIS_SO_OK) return s;
+  const bool beam = (stage_mask & 1) && ctx->cfg.beam_fwhm_px > 0.0;
+  const bool noise = (stage_mask & 2) && ctx->nc.on;
+  if (beam) return run_beam(ctx, d_cube, d_cube, nullptr, noise, st);   // x pass: cube -> tmp, y pass: tmp -> cube
+  if (noise) return run_noise(ctx, d_cube, st);
+  return IRIS_SO_OK;
+}
+
+iris_so_status iris_so_observe(iris_so_ctx* ctx, const float* d_nH2, const float* d_Tgas, const float* d_Tdust,
+                               const float* d_vlos, float* d_cube, void* stream) {
+  return iris_so_observe_stages(ctx, d_nH2, d_Tgas, d_Tdust, d_vlos, 3, d_cube, stream);
+}
+
+iris_so_status iris_so_observe_host(iris_so_ctx* ctx, const float* h_nH2, const float* h_Tgas, const float* h_Tdust,
+                                    const float* h_vlos, float* h_cube, void* stream) {
+  if (!ctx) return IRIS_SO_EINVAL;
+  if (!h_nH2 || !h_Tgas || !h_Tdust || !h_vlos || !h_cube) return fail(ctx, IRIS_SO_EINVAL, "iris_so_observe_host: NULL pointer");
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const size_t fb = sizeof(float) * (size_t)ctx->ncell, cb = sizeof(float) * (size_t)ctx->nvox;
+  iris_so_status s = ensure(ctx, &ctx->d_stage, 4 * fb + cb, "cudaMalloc(host-path staging)");
+  if (s != IRIS_SO_OK) return s;
+  float* f[4] = {ctx->d_stage, ctx->d_stage + ctx->ncell, ctx->d_stage + 2 * ctx->ncell, ctx->d_stage + 3 * ctx->ncell};
+  float* d_cube = ctx->d_stage + 4 * ctx->ncell;
+  const float* h[4] = {h_nH2, h_Tgas, h_Tdust, h_vlos};
+  cudaError_t e;
+  for (int i = 0; i < 4; ++i)
+    if ((e = cudaMemcpyAsync(f[i], h[i], fb, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_fail(ctx, e, "H2D copy");
+  if ((s = iris_so_observe(ctx, f[0], f[1], f[2], f[3], d_cube, stream)) != IRIS_SO_OK) return s;
+  if ((e = cudaMemcpyAsync(h_cube, d_cube, cb, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(ctx, e, "D2H copy");
+  if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(ctx, e, "cudaStreamSynchronize");
+  return IRIS_SO_OK;
+}
+
+iris_so_status iris_so_beam(iris_so_ctx* ctx, const float* d_in, float* d_out, float* d_tmp, void* stream) {
+  if (!ctx) return IRIS_SO_EINVAL;
+  if (!d_in || !d_out) return fail(ctx, IRIS_SO_EINVAL, "iris_so_beam: NULL pointer");
+  if (!(ctx->cfg.beam_fwhm_px > 0.0)) return fail(ctx, IRIS_SO_EINVAL, "iris_so_beam: no beam configured");
+  return run_beam(ctx, d_in, d_out, d_tmp, false, static_cast<cudaStream_t>(stream));
+}
+
+iris_so_status iris_so_noise(iris_so_ctx* ctx, float* d_cube, void* stream) {
+  if (!ctx) return IRIS_SO_EINVAL;
+  if (!d_cube) return fail(ctx, IRIS_SO_EINVAL, "iris_so_noise: NULL pointer");
+  if (!ctx->nc.on) return IRIS_SO_OK;
+  return run_noise(ctx, d_cube, static_cast<cudaStream_t>(stream));
+}
+
+iris_so_status iris_so_observe_adjoint(iris_so_ctx* ctx, const float* d_nH2, const float* d_Tgas, const float* d_Tdust,
+                                       const float* d_vlos, const float* d_w, float* d_grad, void* stream) {
+  if (!ctx) return IRIS_SO_EINVAL;
+  if (!d_nH2 || !d_Tgas || !d_Tdust || !d_vlos || !d_w || !d_grad)
+    return fail(ctx, IRIS_SO_EINVAL, "iris_so_observe_adjoint: NULL pointer");
+  const iris_so_config& c = ctx->cfg;
+  if ((c.subtract_continuum && c.subtract_space != 0) || c.out_unit == 2)
+    return fail(ctx, IRIS_SO_EUNSUPPORTED, "adjoint needs intensity-space subtraction and out_unit 0 or 1");
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  iris_so_status s = run_coefficients(ctx, d_nH2, d_Tgas, d_Tdust, d_vlos, nullptr, st);
+  if (s != IRIS_SO_OK) return s;
+  // what = G^T w (the beam is symmetric and zero padded, so its adjoint is the same convolution)
+  const float* what = d_w;
+  if (c.beam_fwhm_px > 0.0) {
+    const size_t need = sizeof(float) * (size_t)ctx->nvox;
+    if (ctx->d_adj && ctx->adj_bytes < need) { cudaFree(ctx->d_adj); ctx->d_adj = nullptr; ctx->scratch_bytes -= ctx->adj_bytes; }
+    if ((s = ensure(ctx, &ctx->d_adj, need, "cudaMalloc(adjoint weights)")) != IRIS_SO_OK) return s;
+    ctx->adj_bytes = need;
+    if ((s = run_beam(ctx, d_w, ctx->d_adj, nullptr, false, st)) != IRIS_SO_OK) return s;
+    what = ctx->d_adj;
+  }
+  cudaError_t e = iris::launch_adjoint(ctx->mc, ctx->ac, ctx->lc, c.n_levels, ctx->d_coef, ctx->ncell, (int)ctx->npix, c.nz,
+                                       c.nv, c.dust_on != 0, d_nH2, d_Tgas, what, d_grad, st, &ctx->launches);
+  if (e != cudaSuccess) return cuda_fail(ctx, e, "launch of adjoint kernels");
+  return IRIS_SO_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,86 @@
+// Shared pieces of the LOS transfer kernels (K3 + fused K4 / K5).
+//
+// The march of Eq. 4.8.5-4.8.7 is carried in the DIFFERENCE form
+//   D_k = I^[T]_k - I^[C]_k     (total minus continuum, Rayleigh-Jeans Kelvin),
+// together with the scalar continuum march C_k = I^[C]_k (Eq. 3.1.3), which is algebraically the same
+// recurrence as marching I^[T] and I^[C] separately and subtracting at the end (section 4.10), but has no
+// cancellation: weak lines on a bright continuum keep their relative accuracy in fp32.
+//
+// One cell, one channel, with  tau_L = a_c dErf,  J_L = e_c dErf,  m = 1 - exp(-tau_L),
+// E_d = exp(-tau_d),  m_d = 1 - E_d,  tau_T = tau_L + tau_d:
+//   D' = E_d [ D - (D + C) m ] + [ J_L (m_d + E_d m) + S_d (tau_d E_d m - tau_L m_d) ] / tau_T
+//   C' = C E_d + S_d m_d
+// and without dust (tau_d = 0, C = I_bg constant):   D' = D + (S_L - C - D) m,  S_L = e_c / a_c.
+#pragma once
+#include "iris_math.cuh"
+
+namespace iris {
+
+// coefficient plane order written by K2
+enum { Q_E = 0, Q_A = 1, Q_CLOS = 2, Q_S = 3, Q_TAUD = 4, Q_SD = 5 };
+
+// output conversion (K5): what to write for a voxel with difference D and continuum C (both in K_RJ)
+enum OutMode {
+  OUT_TRJ_SUB = 0,     // D
+  OUT_TRJ_TOT = 1,     // D + C
+  OUT_I_SUB = 2,       // D / K_RJ
+  OUT_I_TOT = 3,       // (D + C) / K_RJ
+  OUT_TB_OF_SUB = 4,   // T_B(D / K_RJ)              (odd extension for negative values)
+  OUT_TB_OF_TOT = 5,   // T_B((D + C) / K_RJ)
+  OUT_TB_SUB = 6       // T_B(total) - T_B(continuum)  (Planck-space subtraction, section 4.10)
+};
+
+struct MarchConsts {
+  float T_bg;       // K_RJ B_nu0(T_cmb): background in Rayleigh-Jeans Kelvin
+  float hnu_k;      // h nu0 / k
+  float inv_KRJ;    // 2 k nu0^2 / c^2  (Kelvin -> CGS intensity)
+  int out_mode;
+};
+
+// Planck brightness temperature of a Rayleigh-Jeans temperature (Eq. 4.9.1 with I = T_rj / K_RJ):
+// T_B = (h nu / k) / ln(1 + (h nu / k) / T_rj); odd extension, T_B(0) = 0.
+__device__ __forceinline__ float planck_tb_of_trj(float t, float hnu_k) {
+  if (t == 0.0f) return 0.0f;
+  const float tb = hnu_k / log1pf(hnu_k / fabsf(t));
+  return copysignf(tb, t);
+}
+
+__device__ __forceinline__ float convert_out(float D, float C, const MarchConsts& mc) {
+  switch (mc.out_mode) {
+    case OUT_TRJ_SUB: return D;
+    case OUT_TRJ_TOT: return D + C;
+    case OUT_I_SUB: return D * mc.inv_KRJ;
+    case OUT_I_TOT: return (D + C) * mc.inv_KRJ;
+    case OUT_TB_OF_SUB: return planck_tb_of_trj(D, mc.hnu_k);
+    case OUT_TB_OF_TOT: return planck_tb_of_trj(D + C, mc.hnu_k);
+    default: return planck_tb_of_trj(D + C, mc.hnu_k) - planck_tb_of_trj(C, mc.hnu_k);
+  }
+}
+
+// Per-(pixel, cell) scalars of the dust / continuum part.
+struct DustStep {
+  float tau_d, S_d, E_d, m_d, C;   // C = continuum BEFORE the cell
+};
+
+// One heavy update with dust.  dErf = erf difference of the channel in this cell.
+__device__ __forceinline__ float update_dust(float D, float dErf, float e_c, float a_c, const DustStep& d) {
+  const float tau_L = a_c * dErf;
+  const float J_L = e_c * dErf;
+  const float m = one_minus_exp_neg(tau_L);
+  const float tau_T = tau_L + d.tau_d;
+  const float r = rcp_approx(tau_T == 0.0f ? 1.0f : tau_T);
+  const float Em = d.E_d * m;
+  const float t1 = d.m_d + Em;
+  const float t2 = fmaf(d.tau_d, Em, -tau_L * d.m_d);
+  const float num = fmaf(J_L, t1, d.S_d * t2);
+  const float inner = fmaf(-(D + d.C), m, D);
+  return fmaf(d.E_d, inner, r * num);
+}
+
+// One heavy update without dust: sc = S_L - C (per cell), D' = D + (sc - D) m.
+__device__ __forceinline__ float update_nodust(float D, float dErf, float a_c, float sc) {
+  const float m = one_minus_exp_neg(a_c * dErf);
+  return fmaf(sc - D, m, D);
+}
+
+}  // namespace iris

@@ -1,0 +1,290 @@
+"""GPU parity: the CUDA path (through the C ABI) against the float64 oracle, element by element, on the
+same seeded inputs.  Tolerances: tests/parity.py (BASELINE.json north_star)."""
+import math
+
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+
+from iris_inputs import make_fields, make_workload
+from oracle import Oracle
+from parity import assert_pops, assert_spectra, krj
+
+pytestmark = pytest.mark.gpu
+
+ALGOS = {"window": 2, "dense": 1}
+KB_ = 1.380649e-16
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def dev_fields(f):
+    return [dev(f[k]) for k in ("nH2", "Tgas", "Tdust", "vlos")]
+
+
+def iris(cfg, algo=0):
+    from paper_2607_01338_b200 import IrisSO
+    return IrisSO(cfg, transfer_algo=algo)
+
+
+# ------------------------------------------------------------------------------------------------
+# K1 level populations
+@pytest.mark.parametrize("name,n", [("tiny", 32), ("small", 40)])
+def test_levelpop_workload(name, n):
+    cfg, r = make_workload(name, n=n)
+    f = make_fields(cfg, r)
+    pop = iris(cfg).levelpop(dev(f["nH2"]), dev(f["Tgas"])).cpu().numpy().reshape(cfg.n_levels, -1)
+    ref = Oracle(cfg).levelpop(f["nH2"], f["Tgas"])
+    rel = assert_pops(pop, ref)
+    assert np.allclose(pop.sum(axis=0), 1.0, atol=3e-6)
+    print("levelpop %s: max rel err %.3g" % (name, rel))
+
+
+@pytest.mark.parametrize("n_levels", [2, 3, 4, 5, 6, 7, 8, 9, 10])
+@pytest.mark.parametrize("T_bar", [0.0, 2.725])
+def test_levelpop_extremes(n_levels, T_bar):
+    """Density 1e-2 .. 1e9 cm^-3, temperature 5 .. 3000 K: 30+ decades of dynamic range in x."""
+    cfg, _ = make_workload("tiny", n_levels=n_levels)
+    n = np.logspace(-2, 9, 67, dtype=np.float32)
+    T = np.geomspace(5.0, 3000.0, 53).astype(np.float32)
+    nn, TT = np.meshgrid(n, T, indexing="ij")
+    nn, TT = np.ascontiguousarray(nn.ravel()), np.ascontiguousarray(TT.ravel())
+    cfg = cfg.with_(T_bar=T_bar, nx=nn.size, ny=1, nz=1)
+    pop = iris(cfg).levelpop(dev(nn), dev(TT)).cpu().numpy().reshape(n_levels, -1)
+    assert_pops(pop, Oracle(cfg).levelpop(nn, TT))
+
+
+# ------------------------------------------------------------------------------------------------
+# whole path on the BASELINE workloads (resized where the oracle would take minutes)
+def run_observe(cfg, f, algo, beam=True, noise=True):
+    return iris(cfg, algo).observe(*dev_fields(f), beam=beam, noise=noise).cpu().numpy()
+
+
+@pytest.mark.parametrize("algo", ALGOS)
+def test_observe_tiny_full(algo):
+    cfg, r = make_workload("tiny")
+    f = make_fields(cfg, r)
+    cube = run_observe(cfg, f, ALGOS[algo])
+    ref = Oracle(cfg).observe(f)
+    worst = assert_spectra(cube, ref)
+    assert ref.max() > 1.0
+    print("tiny/%s: worst pixel at %.3g of tolerance" % (algo, worst))
+
+
+@pytest.mark.parametrize("algo", ALGOS)
+def test_observe_small_dust(algo):
+    cfg, r = make_workload("small", n=48)
+    f = make_fields(cfg, r)
+    cube = run_observe(cfg, f, ALGOS[algo])
+    ref = Oracle(cfg).observe(f)
+    worst = assert_spectra(cube, ref)
+    print("small(48^3)/%s: worst pixel at %.3g of tolerance" % (algo, worst))
+
+
+@pytest.mark.parametrize("algo", ALGOS)
+def test_observe_medium_layers_beam_noise(algo):
+    cfg, r = make_workload("medium", n=40)
+    f = make_fields(cfg, r)
+    o = Oracle(cfg)
+    it = iris(cfg, ALGOS[algo])
+    d = dev_fields(f)
+    raw = it.observe(*d, beam=False, noise=False).cpu().numpy()
+    ref_raw = o.observe(f, beam=False, noise=False)
+    assert_spectra(raw, ref_raw, what="raw")
+    smooth = it.observe(*d, beam=True, noise=False).cpu().numpy()
+    ref_smooth = o.observe(f, beam=True, noise=False)
+    assert_spectra(smooth, ref_smooth, what="beam")
+    full = it.observe(*d).cpu().numpy()
+    ref_full = o.observe(f)
+    assert_spectra(full, ref_full, extra=8e-6 * cfg.noise_sigma, peak_of=ref_smooth, what="beam+noise")
+    assert abs((full - smooth).std() - cfg.noise_sigma) < 0.01
+
+
+@pytest.mark.parametrize("algo", ALGOS)
+def test_observe_ragged_shapes(algo):
+    """Sizes that are multiples of nothing: partial warps, partial channel blocks, partial beam tiles."""
+    cfg, r = make_workload("small", nx=37, ny=5, nz=19, nv=101)
+    cfg = cfg.with_(beam_fwhm_px=2.0, v0_cms=-25.0e5)
+    f = make_fields(cfg, r)
+    cube = run_observe(cfg, f, ALGOS[algo])
+    assert_spectra(cube, Oracle(cfg).observe(f))
+
+
+@pytest.mark.parametrize("algo", ALGOS)
+@pytest.mark.parametrize("shape", [dict(nx=1, ny=1, nz=1, nv=1), dict(nx=3, ny=2, nz=1, nv=7), dict(nx=2, ny=2, nz=64, nv=2)])
+def test_observe_degenerate_shapes(algo, shape):
+    cfg, r = make_workload("small", **shape)
+    cfg = cfg.with_(v0_cms=-0.5 * (shape["nv"] - 1) * cfg.dv_cms)
+    f = make_fields(cfg, r)
+    f["vlos"] = (0.01 * f["vlos"]).astype(np.float32)
+    cube = run_observe(cfg, f, ALGOS[algo])
+    assert_spectra(cube, Oracle(cfg).observe(f))
+
+
+@pytest.mark.parametrize("algo", ALGOS)
+@pytest.mark.parametrize("case", ["thick", "very_thin", "narrow_line", "cold_dust_absorption", "heavy_dust"])
+def test_observe_regimes(algo, case):
+    cfg, r = make_workload("small", n=24, nv=128)
+    f = make_fields(cfg, r)
+    f["vlos"] = (0.25 * f["vlos"]).astype(np.float32)
+    if case == "thick":
+        cfg = cfg.with_(abundance=2e-4)                    # tau_peak in the thousands
+    elif case == "very_thin":
+        cfg = cfg.with_(abundance=2e-11)                   # peak T ~ 1e-5 K: the absolute floor and small-tau accuracy
+    elif case == "narrow_line":
+        cfg = cfg.with_(microturb_cms=0.0, dv_cms=1.0e5, v0_cms=-63.5e5)   # thermal b ~ 0.2 km/s << channel width
+    elif case == "cold_dust_absorption":
+        cfg = cfg.with_(kappa_gas_cm2_g=1.0)               # 100x dust: negative features
+        f["Tdust"] = np.full_like(f["Tdust"], 150.0)
+    elif case == "heavy_dust":
+        cfg = cfg.with_(kappa_gas_cm2_g=60.0)              # total dust optical depth >> 40: exercises the G rescale
+    cube = run_observe(cfg, f, ALGOS[algo])
+    ref = Oracle(cfg).observe(f)
+    worst = assert_spectra(cube, ref)
+    if case == "cold_dust_absorption":
+        assert ref.min() < -1e-3
+    print("%s/%s: worst %.3g of tolerance, peak %.3g K" % (case, algo, worst, np.abs(ref).max()))
+
+
+@pytest.mark.parametrize("algo", ALGOS)
+def test_observe_special_inputs(algo):
+    cfg, r = make_workload("small", n=16, nv=64)
+    f = make_fields(cfg, r)
+    f["vlos"] = (0.1 * f["vlos"]).astype(np.float32)
+    # no tracer: continuum-subtracted cube is identically zero
+    z = run_observe(cfg.with_(abundance=0.0), f, ALGOS[algo])
+    assert np.all(z == 0.0)
+    # T_inf cut-off removes the hot half of the cells
+    c2 = cfg.with_(T_inf=75.0)
+    assert_spectra(run_observe(c2, f, ALGOS[algo]), Oracle(c2).observe(f))
+    # pure A + C level balance and no background (T_bar = T_cmb = 0)
+    c3 = cfg.with_(T_bar=0.0, T_cmb=0.0)
+    assert_spectra(run_observe(c3, f, ALGOS[algo]), Oracle(c3).observe(f))
+    # lines far outside the band: nothing but zeros, and nothing non-finite
+    f4 = dict(f); f4["vlos"] = np.full_like(f["vlos"], 5.0e7)
+    assert np.all(run_observe(cfg, f4, ALGOS[algo]) == 0.0)
+
+
+@pytest.mark.parametrize("algo", ALGOS)
+@pytest.mark.parametrize("mode", [dict(out_unit=0), dict(out_unit=2), dict(out_unit=2, subtract_space=1),
+                                  dict(subtract_continuum=False), dict(subtract_continuum=False, out_unit=0),
+                                  dict(subtract_continuum=False, out_unit=2)])
+def test_observe_output_modes(algo, mode):
+    cfg, r = make_workload("small", n=16, nv=64)
+    cfg = cfg.with_(kappa_gas_cm2_g=0.3, **mode)
+    f = make_fields(cfg, r)
+    f["vlos"] = (0.1 * f["vlos"]).astype(np.float32)
+    cube = run_observe(cfg, f, ALGOS[algo]).astype(np.float64)
+    ref = Oracle(cfg).observe(f)
+    K = krj(cfg.nu0_Hz)
+    hnk = 6.62607015e-27 * cfg.nu0_Hz / KB_
+    # the tolerance is defined on the continuum-subtracted Rayleigh-Jeans spectrum of the same pixels
+    sub = Oracle(cfg.with_(subtract_continuum=True, subtract_space=0, out_unit=1)).observe(f)
+    if cfg.subtract_continuum and cfg.subtract_space == 1:
+        # T_B(total) - T_B(continuum): dT_B/dT_RJ <= 2.6 for T_B >= T_cmb = 2.725 K at 220 GHz, plus the
+        # fp32 rounding of the two brightness temperatures themselves
+        tb_tot = Oracle(cfg.with_(subtract_continuum=False, subtract_space=0)).observe(f)
+        assert_spectra(cube, ref, floor=3e-6, rel=3e-4, extra=3e-7 * np.abs(tb_tot), peak_of=sub)
+        return
+    if cfg.out_unit == 2:
+        # map both back to Rayleigh-Jeans Kelvin with the exact inverse of Eq. 4.9.1 (odd extension)
+        inv = lambda t: np.sign(t) * hnk / np.expm1(hnk / np.maximum(np.abs(t), 1e-300))
+        cube, ref = inv(cube), inv(ref)
+    scale = 1.0 / K if cfg.out_unit == 0 else 1.0
+    extra = 0.0 if cfg.subtract_continuum else 3e-7 * np.abs(ref)
+    assert_spectra(cube, ref, floor=1e-6 * scale, extra=extra, peak_of=sub * scale)
+
+
+# ------------------------------------------------------------------------------------------------
+# K2+K3+K4 alone, also with caller-supplied populations
+@pytest.mark.parametrize("algo", ALGOS)
+def test_transfer_intensities(algo):
+    cfg, r = make_workload("small", n=24, nv=96)
+    f = make_fields(cfg, r)
+    f["vlos"] = (0.2 * f["vlos"]).astype(np.float32)
+    o = Oracle(cfg)
+    coef = o.coefficients(f["nH2"], f["Tgas"], f["Tdust"])
+    It, Ic = o.march(coef, f["vlos"])
+    K = krj(cfg.nu0_Hz)
+    it = iris(cfg, ALGOS[algo])
+    d = dev_fields(f)
+    for pop in (None, it.levelpop(d[0], d[1])):
+        gt, gc = it.transfer(*d, pop=pop)
+        gt = gt.cpu().numpy().reshape(-1, cfg.nv).astype(np.float64)
+        gc = gc.cpu().numpy().ravel().astype(np.float64)
+        assert np.allclose(gc, Ic, rtol=2e-6)
+        assert_spectra(gt * K, It * K, extra=3e-7 * It * K, peak_of=(It - Ic[:, None]) * K, what="I_total")
+
+
+# ------------------------------------------------------------------------------------------------
+# K6 / K7 alone
+def test_beam_and_noise_kernels():
+    cfg, _ = make_workload("medium", nx=45, ny=70, nz=1, nv=33)
+    cfg = cfg.with_(seed=987654321012345, noise_mu=0.05)
+    rng = np.random.default_rng(5)
+    img = rng.standard_normal((cfg.ny, cfg.nx, cfg.nv)).astype(np.float32)
+    it = iris(cfg)
+    o = Oracle(cfg)
+    out = it.beam(dev(img)).cpu().numpy()
+    assert np.abs(out - o.beam(img)).max() < 2e-6
+    noisy = it.noise(dev(img)).cpu().numpy()
+    ref = o.noise(img)
+    assert np.abs(noisy - ref).max() < 8e-6 * cfg.noise_sigma + 3e-7 * np.abs(ref).max()
+    # gamma mode 1 and a wide beam (radius 17)
+    cfg2 = cfg.with_(noise_gamma_mode=1, beam_fwhm_px=10.0)
+    it2, o2 = iris(cfg2), Oracle(cfg2)
+    assert np.abs(it2.noise(dev(img)).cpu().numpy() - o2.noise(img)).max() < 8e-6 * cfg.noise_sigma + 3e-7 * np.abs(ref).max()
+    assert np.abs(it2.beam(dev(img)).cpu().numpy() - o2.beam(img)).max() < 2e-6
+
+
+# ------------------------------------------------------------------------------------------------
+# full BASELINE sizes in the launch configuration bench.py times, on sampled columns
+def _sampled_check(name, n_cols, seed):
+    cfg, r = make_workload(name)
+    f = make_fields(cfg, r)
+    it = iris(cfg)
+    d = dev_fields(f)
+    cube = it.observe(*d, beam=False, noise=False)
+    rng = np.random.default_rng(seed)
+    plane = cfg.nx * cfg.ny
+    pix = np.sort(rng.choice(plane, size=n_cols, replace=False))
+    got = cube.reshape(plane, cfg.nv)[torch.from_numpy(pix).cuda()].cpu().numpy()
+    # the same columns as an independent (nz, 1, n_cols) problem for the oracle (columns do not interact)
+    sub = {k: np.ascontiguousarray(f[k].reshape(cfg.nz, plane)[:, pix]).reshape(cfg.nz, 1, n_cols)
+           for k in ("nH2", "Tgas", "Tdust", "vlos")}
+    cfg_s = cfg.with_(nx=n_cols, ny=1, beam_fwhm_px=0.0, noise_sigma=0.0)
+    ref = Oracle(cfg_s).observe(sub, beam=False, noise=False).reshape(n_cols, cfg.nv)
+    worst = assert_spectra(got, ref, what=name + " sampled columns")
+    # level populations on a subsample of cells
+    cells = rng.choice(cfg.n_cells, size=20000, replace=False)
+    pop = it.levelpop(d[0], d[1]).reshape(cfg.n_levels, -1)[:, torch.from_numpy(np.sort(cells)).cuda()].cpu().numpy()
+    cs = np.sort(cells)
+    cfg_p = cfg.with_(nx=cs.size, ny=1, nz=1)
+    assert_pops(pop, Oracle(cfg_p).levelpop(f["nH2"].ravel()[cs], f["Tgas"].ravel()[cs]))
+    # properties that hold at any size
+    c = cube.cpu().numpy()
+    assert np.all(np.isfinite(c))
+    print("%s full size: worst sampled pixel at %.3g of tolerance; cube max %.3g K min %.3g K" % (name, worst, c.max(), c.min()))
+    return cfg, f, it, d, cube
+
+
+def test_full_size_medium_sampled():
+    cfg, f, it, d, raw = _sampled_check("medium", 48, 11)
+    # beam + noise at full size: beam of the GPU raw cube equals the oracle beam on a window around sampled pixels
+    full = it.observe(*d)
+    smooth = it.observe(*d, beam=True, noise=False)
+    dz = (full - smooth).flatten()[:: 97].cpu().numpy()
+    assert abs(dz.std() - cfg.noise_sigma) < 2e-3 and abs(dz.mean()) < 2e-3
+    o = Oracle(cfg)
+    y0, x0, w = 100, 37, 20
+    patch = raw[y0 - 6:y0 + w + 6, x0 - 6:x0 + w + 6].cpu().numpy()
+    ref = o.beam(patch)[6:-6, 6:-6]
+    got = smooth[y0:y0 + w, x0:x0 + w].cpu().numpy()
+    assert np.abs(got - ref).max() <= 1e-5 * np.abs(ref).max() + 1e-6
+
+
+def test_full_size_large_sampled():
+    _sampled_check("large", 32, 12)
