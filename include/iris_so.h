@@ -148,6 +148,24 @@ iris_so_status iris_so_observe_adjoint(iris_so_ctx *ctx, const float *d_nH2, con
                                        const float *d_Tdust, const float *d_vlos, const float *d_w,
                                        float *d_grad_nH2, void *cuda_stream);
 
+/* Measurement support.  iris_so_profile(ctx, 1) makes every later call bracket each stage's kernels with
+ * CUDA events on the caller's stream (no synchronisation); iris_so_profile(ctx, 0) switches it off; both
+ * discard what was recorded.  iris_so_profile_read waits for the recorded events and returns the summed
+ * device time and the number of kernel launches of one stage since profiling was switched on. */
+#define IRIS_SO_STAGE_CELL 0      /* K1 + K2 */
+#define IRIS_SO_STAGE_TRANSFER 1  /* K3 + K4 + K5 */
+#define IRIS_SO_STAGE_BEAM 2      /* K6 (+ K7 fused) */
+#define IRIS_SO_STAGE_NOISE 3     /* K7 alone */
+#define IRIS_SO_STAGE_ADJOINT 4   /* K8 + K9 */
+#define IRIS_SO_NUM_STAGES 5
+iris_so_status iris_so_profile(iris_so_ctx *ctx, int32_t enable);
+iris_so_status iris_so_profile_read(iris_so_ctx *ctx, int32_t stage, double *total_ms, uint64_t *launches);
+
+/* Work counter for roofline accounting: number of (cell, channel) updates inside the line windows of the
+ * coefficient planes left in the context by the last transfer / observe call (the updates the line-window
+ * algorithm evaluates; the dense algorithm evaluates nx*ny*nz*nv).  Synchronises the stream. */
+iris_so_status iris_so_transfer_work(iris_so_ctx *ctx, uint64_t *window_updates, void *cuda_stream);
+
 /* Stand-alone post-processing stages (also used inside iris_so_observe). */
 /* K6: separable Gaussian beam of FWHM beam_fwhm_px on d_in -> d_out (must not alias), zero padding,
  * radius ceil(4 sigma), weights normalised to sum 1.  d_tmp is a cube-sized temporary or NULL (context

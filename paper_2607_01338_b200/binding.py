@@ -15,7 +15,9 @@ DECLARED_SYMBOLS = (
     "iris_so_create", "iris_so_destroy", "iris_so_last_error", "iris_so_status_string", "iris_so_version",
     "iris_so_launch_count", "iris_so_scratch_bytes", "iris_so_levelpop", "iris_so_transfer", "iris_so_observe",
     "iris_so_observe_stages", "iris_so_observe_host", "iris_so_observe_adjoint", "iris_so_beam", "iris_so_noise",
+    "iris_so_profile", "iris_so_profile_read", "iris_so_transfer_work",
 )
+STAGES = {"cell": 0, "transfer": 1, "beam": 2, "noise": 3, "adjoint": 4}
 
 
 class IrisSOError(RuntimeError):
@@ -90,6 +92,12 @@ def load_library():
     lib.iris_so_beam.argtypes = [vp, fp, fp, fp, vp]
     lib.iris_so_noise.restype = st
     lib.iris_so_noise.argtypes = [vp, fp, vp]
+    lib.iris_so_profile.restype = st
+    lib.iris_so_profile.argtypes = [vp, C.c_int32]
+    lib.iris_so_profile_read.restype = st
+    lib.iris_so_profile_read.argtypes = [vp, C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_uint64)]
+    lib.iris_so_transfer_work.restype = st
+    lib.iris_so_transfer_work.argtypes = [vp, C.POINTER(C.c_uint64), vp]
     _lib = lib
     return lib
 
@@ -173,6 +181,23 @@ class IrisSO:
 
     def scratch_bytes(self):
         return int(self.lib.iris_so_scratch_bytes(self._h))
+
+    def profile(self, enable=True):
+        self._check(self.lib.iris_so_profile(self._h, 1 if enable else 0))
+
+    def profile_read(self):
+        """{stage: (total_ms, launches)} since profiling was switched on (waits for the recorded events)."""
+        out = {}
+        for name, sid in STAGES.items():
+            ms, n = C.c_double(), C.c_uint64()
+            self._check(self.lib.iris_so_profile_read(self._h, sid, C.byref(ms), C.byref(n)))
+            out[name] = (ms.value, int(n.value))
+        return out
+
+    def transfer_work(self):
+        n = C.c_uint64()
+        self._check(self.lib.iris_so_transfer_work(self._h, C.byref(n), self._stream()))
+        return int(n.value)
 
     # -- entry points ----------------------------------------------------------------------------
     def levelpop(self, nH2, Tgas, pop=None):

@@ -49,6 +49,12 @@ struct iris_so_ctx {
   uint64_t scratch_bytes = 0;
   uint64_t launches = 0;
   std::string err;
+  // optional per-stage timing (iris_so_profile)
+  struct ProfRec { int stage; uint64_t launches; cudaEvent_t a, b; };
+  bool profiling = false;
+  std::vector<ProfRec> recs;
+  std::vector<cudaEvent_t> event_pool;
+  unsigned long long* d_counter = nullptr;
 };
 
 namespace {
@@ -77,6 +83,33 @@ iris_so_status ensure(iris_so_ctx* ctx, float** p, size_t bytes, const char* wha
   if (e != cudaSuccess) { *p = nullptr; cudaGetLastError(); return cuda_fail(ctx, e, what); }
   ctx->scratch_bytes += bytes;
   return IRIS_SO_OK;
+}
+
+// Brackets the kernels a stage launches with two events on the caller's stream when profiling is on.
+struct ProfScope {
+  iris_so_ctx* ctx; cudaStream_t st; int stage; uint64_t l0; cudaEvent_t a = nullptr;
+  ProfScope(iris_so_ctx* c, int stage_, cudaStream_t s) : ctx(c), st(s), stage(stage_), l0(c->launches) {
+    if (!ctx->profiling) return;
+    a = take(); if (a) cudaEventRecord(a, st);
+  }
+  ~ProfScope() {
+    if (!a) return;
+    cudaEvent_t b = take();
+    if (!b) return;
+    cudaEventRecord(b, st);
+    ctx->recs.push_back({stage, ctx->launches - l0, a, b});
+  }
+  cudaEvent_t take() {
+    if (!ctx->event_pool.empty()) { cudaEvent_t e = ctx->event_pool.back(); ctx->event_pool.pop_back(); return e; }
+    cudaEvent_t e = nullptr;
+    if (cudaEventCreate(&e) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    return e;
+  }
+};
+
+void prof_reset(iris_so_ctx* ctx) {
+  for (auto& r : ctx->recs) { ctx->event_pool.push_back(r.a); ctx->event_pool.push_back(r.b); }
+  ctx->recs.clear();
 }
 
 double planck_krj(double hnu_k, double T) { return T > 0.0 ? hnu_k / std::expm1(hnu_k / T) : 0.0; }
@@ -249,6 +282,7 @@ iris_so_status run_coefficients(iris_so_ctx* ctx, const float* n, const float* T
                                 const float* pop, cudaStream_t st) {
   iris_so_status s = ensure(ctx, &ctx->d_coef, sizeof(float) * 6 * (size_t)ctx->ncell, "cudaMalloc(coefficient planes)");
   if (s != IRIS_SO_OK) return s;
+  ProfScope prof(ctx, IRIS_SO_STAGE_CELL, st);
   if (pop) {
     iris::coef_from_pop_kernel<<<(unsigned)((ctx->ncell + 255) / 256), 256, 0, st>>>(ctx->cc, ctx->ncell, n, T, Td, v, pop,
                                                                                      ctx->d_coef);
@@ -268,6 +302,7 @@ iris_so_status run_transfer(iris_so_ctx* ctx, const iris::MarchConsts& mc, float
   const int npix = (int)ctx->npix, nz = ctx->cfg.nz, nv = ctx->cfg.nv;
   int algo = ctx->cfg.transfer_algo;
   if (algo == IRIS_SO_ALGO_AUTO) algo = IRIS_SO_ALGO_WINDOW;
+  ProfScope prof(ctx, IRIS_SO_STAGE_TRANSFER, st);
   if (algo == IRIS_SO_ALGO_DENSE) {
     constexpr int CB = 16, NW = 4;
     dim3 block(32, NW), grid((npix + 31) / 32, (nv + CB * NW - 1) / (CB * NW));
@@ -289,6 +324,7 @@ iris_so_status run_beam(iris_so_ctx* ctx, const float* in, float* out, float* tm
     if (s != IRIS_SO_OK) return s;
     tmp = ctx->d_tmp;
   }
+  ProfScope prof(ctx, IRIS_SO_STAGE_BEAM, st);
   iris::NoiseConsts off = ctx->nc; off.on = 0;
   iris::NoiseConsts nz2 = ctx->nc; nz2.on = noise ? ctx->nc.on : 0;
   dim3 block(32, 8);
@@ -304,6 +340,7 @@ iris_so_status run_beam(iris_so_ctx* ctx, const float* in, float* out, float* tm
 }
 
 iris_so_status run_noise(iris_so_ctx* ctx, float* cube, cudaStream_t st) {
+  ProfScope prof(ctx, IRIS_SO_STAGE_NOISE, st);
   iris::noise_kernel<<<(unsigned)((ctx->nvox + 255) / 256), 256, 0, st>>>(ctx->nc, cube, ctx->nvox);
   IRIS_CHECK_LAUNCH(ctx, "noise_kernel");
   return IRIS_SO_OK;
@@ -371,7 +408,9 @@ iris_so_status iris_so_create(const iris_so_config* cfg, iris_so_ctx** out) {
 
 void iris_so_destroy(iris_so_ctx* ctx) {
   if (!ctx) return;
-  cudaFree(ctx->d_coef); cudaFree(ctx->d_tmp); cudaFree(ctx->d_stage); cudaFree(ctx->d_adj);
+  cudaFree(ctx->d_coef); cudaFree(ctx->d_tmp); cudaFree(ctx->d_stage); cudaFree(ctx->d_adj); cudaFree(ctx->d_counter);
+  prof_reset(ctx);
+  for (cudaEvent_t e : ctx->event_pool) cudaEventDestroy(e);
   delete ctx;
 }
 
@@ -436,6 +475,48 @@ iris_so_status iris_so_observe_host(iris_so_ctx* ctx, const float* h_nH2, const 
   if ((s = iris_so_observe(ctx, f[0], f[1], f[2], f[3], d_cube, stream)) != IRIS_SO_OK) return s;
   if ((e = cudaMemcpyAsync(h_cube, d_cube, cb, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(ctx, e, "D2H copy");
   if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(ctx, e, "cudaStreamSynchronize");
+  return IRIS_SO_OK;
+}
+
+iris_so_status iris_so_profile(iris_so_ctx* ctx, int32_t enable) {
+  if (!ctx) return IRIS_SO_EINVAL;
+  prof_reset(ctx);
+  ctx->profiling = enable != 0;
+  return IRIS_SO_OK;
+}
+
+iris_so_status iris_so_profile_read(iris_so_ctx* ctx, int32_t stage, double* total_ms, uint64_t* launches) {
+  if (!ctx) return IRIS_SO_EINVAL;
+  if (stage < 0 || stage >= IRIS_SO_NUM_STAGES || !total_ms || !launches)
+    return fail(ctx, IRIS_SO_EINVAL, "iris_so_profile_read: bad stage or NULL output");
+  double ms = 0.0; uint64_t n = 0;
+  for (auto& r : ctx->recs) {
+    if (r.stage != stage) continue;
+    cudaError_t e = cudaEventSynchronize(r.b);
+    float t = 0.0f;
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&t, r.a, r.b);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "iris_so_profile_read");
+    ms += t; n += r.launches;
+  }
+  *total_ms = ms; *launches = n;
+  return IRIS_SO_OK;
+}
+
+iris_so_status iris_so_transfer_work(iris_so_ctx* ctx, uint64_t* window_updates, void* stream) {
+  if (!ctx) return IRIS_SO_EINVAL;
+  if (!window_updates) return fail(ctx, IRIS_SO_EINVAL, "iris_so_transfer_work: NULL output");
+  if (!ctx->d_coef) return fail(ctx, IRIS_SO_EINVAL, "iris_so_transfer_work: no coefficient planes yet (call observe / transfer first)");
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  cudaError_t e;
+  if (!ctx->d_counter && (e = cudaMalloc(reinterpret_cast<void**>(&ctx->d_counter), sizeof(unsigned long long))) != cudaSuccess)
+    return cuda_fail(ctx, e, "cudaMalloc(counter)");
+  if ((e = cudaMemsetAsync(ctx->d_counter, 0, sizeof(unsigned long long), st)) != cudaSuccess) return cuda_fail(ctx, e, "memset");
+  iris::window_work_kernel<<<(unsigned)((ctx->ncell + 255) / 256), 256, 0, st>>>(ctx->d_coef, ctx->ncell, ctx->cfg.nv, ctx->d_counter);
+  IRIS_CHECK_LAUNCH(ctx, "window_work_kernel");
+  unsigned long long h = 0;
+  if ((e = cudaMemcpyAsync(&h, ctx->d_counter, sizeof h, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(ctx, e, "D2H");
+  if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(ctx, e, "cudaStreamSynchronize");
+  *window_updates = h;
   return IRIS_SO_OK;
 }
 

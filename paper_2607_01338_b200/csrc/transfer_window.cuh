@@ -21,6 +21,30 @@
 
 namespace iris {
 
+// Channel window [klo, khi] of one cell (empty if the returned width is 0).
+__device__ __forceinline__ int line_window(float e_c, float a_c, float c_los, float s, int nv, int& klo, int& khi) {
+  const float sig = fmaxf(fabsf(a_c), e_c);
+  const float Xw2 = __logf(sig) + 18.420681f;                  // ln(sig / 1e-8)
+  const float Xw = fminf(sqrtf(fmaxf(Xw2, 0.0f)), IRIS_ERFC_TMAX);
+  const float hw = Xw * rcp_approx(s);
+  klo = max(0, (int)floorf(c_los - hw));
+  khi = min(nv - 1, (int)floorf(c_los + hw));
+  return (Xw2 > 0.0f) ? max(khi - klo + 1, 0) : 0;
+}
+
+// Sum of the window widths over all cells (work counter for roofline accounting).
+__global__ void __launch_bounds__(256) window_work_kernel(const float* __restrict__ coef, int64_t ncell, int nv,
+                                                          unsigned long long* __restrict__ total) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  int w = 0;
+  if (i < ncell) {
+    int klo, khi;
+    w = line_window(coef[i], coef[ncell + i], coef[2 * ncell + i], coef[3 * ncell + i], nv, klo, khi);
+  }
+  w = __reduce_add_sync(0xffffffffu, w);
+  if ((threadIdx.x & 31) == 0 && w) atomicAdd(total, (unsigned long long)w);
+}
+
 template <int LPP, bool DUST>
 __global__ void __launch_bounds__(128)
 transfer_window_kernel(MarchConsts mc, const float* __restrict__ coef, int64_t ncell, int npix, int nz, int nv,
@@ -54,13 +78,8 @@ transfer_window_kernel(MarchConsts mc, const float* __restrict__ coef, int64_t n
       if (DUST) { n_td = p[4 * ncell]; n_sd = p[5 * ncell]; }
     }
     // line window
-    const float sig = fmaxf(fabsf(a_c), e_c);
-    const float Xw2 = __logf(sig) + 18.420681f;                  // ln(sig / 1e-8)
-    const float Xw = fminf(sqrtf(fmaxf(Xw2, 0.0f)), IRIS_ERFC_TMAX);
-    const float hw = Xw * rcp_approx(s);
-    const int klo = max(0, (int)floorf(c_los - hw));
-    const int khi = min(nv - 1, (int)floorf(c_los + hw));
-    const int W = (Xw2 > 0.0f) ? khi - klo + 1 : 0;
+    int klo, khi;
+    const int W = line_window(e_c, a_c, c_los, s, nv, klo, khi);
     const int npass = __reduce_max_sync(FULL, (W + LPP - 1) / LPP);
 
     DustStep d;
