@@ -1,7 +1,27 @@
-// K8 / K9: reverse-scan adjoint d(sum w * cube) / d n_H2 (placeholder until the kernels land).
+// K8 / K9: gradient of L = sum_{y,x,v} what * cube_raw with respect to n_H2 of every cell
+// (what = beam-adjoint of the caller's weights; cube_raw = the noise-free cube before the beam).
+//
+// The paper obtains this gradient from PyTorch autograd through the whole observation.
+// Here it is written out: the adjoint of the formal step (Eq. 4.8.5-4.8.7)
+//   T' = T E_T + (J + S_d tau_d) w(tau_T),   tau_T = tau_L + tau_d,  E_T = exp(-tau_T),  w = (1 - E_T) / tau_T
+// is  lambda_k = lambda_{k+1} E_T  with
+//   dT'/dJ = w,   dT'/dtau_T = -T E_T + (J + S_d tau_d) w'(tau_T),   explicit dT'/dtau_d += S_d w.
+// Instead of a reverse scan (which needs every intermediate intensity, or an unstable division by E_T),
+// the adjoint variable is evaluated in closed form during a second FORWARD march:
+//   lambda_{k+1}[v] = scale * what[v] * exp(-(totL[v] - cumL_k[v])) * exp(-(totD - cumD_k)),
+// where totL[v] is the line optical depth of the whole ray in channel v (first march) and cumL_k its running
+// sum: only sums of optical depths, stable for any tau.  One warp owns one pixel; its per-channel state
+// (remaining line depth, attenuated weights, the scaled difference spectrum Dt of transfer_window.cuh) lives
+// in shared memory; only the channels inside a cell's line window are touched, plus -- with dust -- one
+// dense dot product per cell for the dust-attenuation term of the channels outside the window.
+//
+// Chain rule to n_H2 (K9): e_c = c_e n x_u, a_c = c_a n (x_l g_u/g_l - x_u), tau_d = c_d n, and
+// y = n dx/dn solves  y Q = -x Q_C  (Q the generator of the level balance, Q_C its collisional part) with
+// sum(y) = 0; it is obtained from the elimination factors the GTH solve of K1 leaves in registers.
 #pragma once
 #include "cell_kernels.cuh"
 #include "transfer_common.cuh"
+#include "transfer_window.cuh"
 
 namespace iris {
 
@@ -9,14 +29,325 @@ struct AdjointConsts {
   float c_e, c_a, c_d, gr;
   int upper, lower;
   float T_inf;
-  float scale;      // d(out) / d(D in Kelvin)
-  int subtract;
+  float scale;      // d(cube_raw) / d(D in Kelvin): 1 for T_RJ output, 1 / K_RJ for intensity output
+  int subtract;     // 1: cube_raw = total - continuum
 };
 
-inline cudaError_t launch_adjoint(const MarchConsts&, const AdjointConsts&, const LevelConsts&, int, const float*, int64_t,
-                                  int, int, int, bool, const float*, const float*, const float*, float*, cudaStream_t,
-                                  uint64_t*) {
-  return cudaErrorNotSupported;
+// Level fractions x and their logarithmic density derivative y = n dx/dn.
+template <int N>
+__device__ __forceinline__ void level_fractions_grad(const LevelConsts& lc, float n, float T, float (&x)[N], float (&y)[N]) {
+  float R[N][N];
+  const float invT = 1.0f / T;
+  const float kf = n * exp2f(lc.Texp * log2f(T * lc.inv_Tref));
+  float q[N];
+#pragma unroll
+  for (int i = 1; i < N; ++i) q[i] = expf(-lc.dE_adj[i] * invT);
+#pragma unroll
+  for (int u = 1; u < N; ++u) {
+    float bz = 1.0f;
+#pragma unroll
+    for (int l = u - 1; l >= 0; --l) {
+      bz *= q[l + 1];
+      const int p = pair_index(u, l);
+      R[u][l] = fmaf(kf, lc.coll[p], lc.rad_down[p]);
+      R[l][u] = fmaf(kf * bz, lc.coll_gr[p], lc.rad_up[p]);
+    }
+  }
+  float inv[N];
+#pragma unroll
+  for (int m = N - 1; m >= 1; --m) {
+    float s = 0.0f;
+#pragma unroll
+    for (int j = 0; j < m; ++j) s += R[m][j];
+    inv[m] = 1.0f / s;
+#pragma unroll
+    for (int i = 0; i < m; ++i) R[i][m] *= inv[m];
+#pragma unroll
+    for (int i = 0; i < m; ++i)
+#pragma unroll
+      for (int j = 0; j < m; ++j)
+        if (i != j) R[i][j] = fmaf(R[i][m], R[m][j], R[i][j]);
+  }
+  x[0] = 1.0f;
+  float tot = 1.0f;
+#pragma unroll
+  for (int j = 1; j < N; ++j) {
+    float s = 0.0f;
+#pragma unroll
+    for (int i = 0; i < j; ++i) s = fmaf(x[i], R[i][j], s);
+    x[j] = s;
+    tot += s;
+  }
+  const float itot = 1.0f / tot;
+#pragma unroll
+  for (int j = 0; j < N; ++j) x[j] *= itot;
+  // right-hand side b = -x Q_C: net collisional outflow of every level (pairwise, so that sum(b) = 0)
+  float b[N];
+#pragma unroll
+  for (int j = 0; j < N; ++j) b[j] = 0.0f;
+#pragma unroll
+  for (int u = 1; u < N; ++u) {
+    float bz = 1.0f;
+#pragma unroll
+    for (int l = u - 1; l >= 0; --l) {
+      bz *= q[l + 1];
+      const int p = pair_index(u, l);
+      const float f = x[u] * (kf * lc.coll[p]) - x[l] * (kf * bz * lc.coll_gr[p]);   // net flow u -> l
+      b[u] += f;
+      b[l] -= f;
+    }
+  }
+  // the same eliminations applied to b, then back-substitution with y_0 = 0
+#pragma unroll
+  for (int m = N - 1; m >= 1; --m) {
+    const float t = b[m] * inv[m];
+#pragma unroll
+    for (int j = 0; j < m; ++j) b[j] = fmaf(t, R[m][j], b[j]);
+  }
+  y[0] = 0.0f;
+  float sy = 0.0f;
+#pragma unroll
+  for (int m = 1; m < N; ++m) {
+    float s = -b[m] * inv[m];
+#pragma unroll
+    for (int i = 0; i < m; ++i) s = fmaf(y[i], R[i][m], s);
+    y[m] = s;
+    sy += s;
+  }
+#pragma unroll
+  for (int j = 0; j < N; ++j) y[j] = fmaf(-sy, x[j], y[j]);     // project onto sum(y) = 0
+}
+
+// K9 (per cell): d e_c / d n and d a_c / d n  ->  dcoef[2][ncell]
+template <int N>
+__global__ void __launch_bounds__(128) coef_grad_kernel(LevelConsts lc, AdjointConsts ac, int64_t ncell,
+                                                        const float* __restrict__ nH2, const float* __restrict__ Tgas,
+                                                        float* __restrict__ dcoef) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= ncell) return;
+  const float n = nH2[i], T = Tgas[i];
+  float x[N], y[N];
+  level_fractions_grad<N>(lc, n, T, x, y);
+  float xu = 0.0f, xl = 0.0f;
+#pragma unroll
+  for (int l = 0; l < N; ++l) {
+    if (l == ac.upper) xu = x[l] + y[l];
+    if (l == ac.lower) xl = x[l] + y[l];
+  }
+  float de = ac.c_e * xu, da = ac.c_a * fmaf(xl, ac.gr, -xu);
+  if (T > ac.T_inf) { de = 0.0f; da = 0.0f; }
+  dcoef[i] = de;
+  dcoef[ncell + i] = da;
+}
+
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+// w(tau) = (1 - exp(-tau)) / tau and w'(tau) = (exp(-tau)(1 + tau) - 1) / tau^2, accurate for every tau.
+__device__ __forceinline__ void w_and_wprime(float tau, float m /* 1 - exp(-tau) */, float& w, float& wp) {
+  if (fabsf(tau) < 0.25f) {
+    float p = fmaf(tau, -1.0f / 5040.0f, 1.0f / 720.0f);
+    p = fmaf(p, tau, -1.0f / 120.0f);
+    p = fmaf(p, tau, 1.0f / 24.0f);
+    p = fmaf(p, tau, -1.0f / 6.0f);
+    p = fmaf(p, tau, 0.5f);
+    w = fmaf(-p, tau, 1.0f);                       // 1 - tau/2 + tau^2/6 - ...
+    float r = fmaf(tau, -1.0f / 5760.0f, 1.0f / 840.0f);
+    r = fmaf(r, tau, -1.0f / 144.0f);
+    r = fmaf(r, tau, 1.0f / 30.0f);
+    r = fmaf(r, tau, -0.125f);
+    r = fmaf(r, tau, 1.0f / 3.0f);
+    wp = fmaf(r, tau, -0.5f);                      // -1/2 + tau/3 - tau^2/8 + ...
+  } else {
+    const float it = 1.0f / tau;
+    w = m * it;
+    wp = (fmaf(1.0f - m, 1.0f + tau, -1.0f)) * it * it;
+  }
+}
+
+// Channel erf difference of channel c in a cell (both edges evaluated by the calling lane).
+__device__ __forceinline__ float channel_derf(int c, float c_los, float s) {
+  const float x_lo = ((float)c - c_los) * s, x_hi = ((float)(c + 1) - c_los) * s;
+  const float G_lo = signed_erfc(x_lo), G_hi = signed_erfc(x_hi);
+  return (copysignf(1.0f, G_hi) - copysignf(1.0f, G_lo)) - (G_hi - G_lo);
+}
+
+// K8: one warp per pixel.  Shared memory per warp: 5 * nv floats (xrem, P, Q, Dt, what).
+template <bool DUST>
+__global__ void __launch_bounds__(128)
+adjoint_march_kernel(MarchConsts mc, AdjointConsts ac, const float* __restrict__ coef, const float* __restrict__ dcoef,
+                     int64_t ncell, int npix, int nz, int nv, const float* __restrict__ what, float* __restrict__ grad) {
+  extern __shared__ float sm[];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, wpc = blockDim.x >> 5;
+  const int pix = blockIdx.x * wpc + warp;
+  if (pix >= npix) return;                                   // whole warps only; no CTA-wide barrier below
+  float* xrem = sm + (size_t)warp * 5 * nv;                  // line optical depth still ahead of the march
+  float* P = xrem + nv;                                      // what * exp(-xrem)
+  float* Q = P + nv;                                         // what * (1 - exp(-xrem))
+  float* Dt = Q + nv;                                        // (I_total - I_cont) * G, as in transfer_window.cuh
+  float* wh = Dt + nv;
+  float Wtot = 0.0f;
+  for (int c = lane; c < nv; c += 32) {
+    const float w = what[(int64_t)pix * nv + c];
+    wh[c] = w; xrem[c] = 0.0f; Dt[c] = 0.0f;
+    Wtot += w;
+  }
+  Wtot = warp_sum(Wtot);
+  __syncwarp();
+
+  // first march: total line optical depth per channel and total dust optical depth
+  float totD = 0.0f;
+  const float* p = coef + pix;
+  for (int z = 0; z < nz; ++z, p += npix) {
+    const float e_c = p[0], a_c = p[ncell], c_los = p[2 * ncell], s = p[3 * ncell];
+    if (DUST) totD += p[4 * ncell];
+    int klo, khi;
+    const int W = line_window(e_c, a_c, c_los, s, nv, klo, khi);
+    if (W > 0)
+      for (int c = klo + lane; c <= khi; c += 32) xrem[c] = fmaf(a_c, channel_derf(c, c_los, s), xrem[c]);
+    __syncwarp();
+  }
+  for (int c = lane; c < nv; c += 32) {
+    const float xr = xrem[c], w = wh[c];
+    P[c] = w * exp_neg(xr);
+    Q[c] = w * one_minus_exp_neg(xr);
+  }
+  __syncwarp();
+
+  // second march: forward state and closed-form adjoint together
+  float C = mc.T_bg, G = 1.0f, cumD = 0.0f;
+  p = coef + pix;
+  for (int z = 0; z < nz; ++z, p += npix) {
+    const float e_c = p[0], a_c = p[ncell], c_los = p[2 * ncell], s = p[3 * ncell];
+    const float tau_d = DUST ? p[4 * ncell] : 0.0f, S_d = DUST ? p[5 * ncell] : 0.0f;
+    int klo, khi;
+    const int W = line_window(e_c, a_c, c_los, s, nv, klo, khi);
+    float E_d = 1.0f, m_d = 0.0f, Gn = 1.0f, Lam = 1.0f;
+    if (DUST) {
+      E_d = exp_neg(tau_d);
+      m_d = one_minus_exp_neg(tau_d);
+      Gn = G * ex2_approx(tau_d * 1.4426950408889634f);
+      cumD += tau_d;
+      Lam = exp_neg(totD - cumD);                            // dust attenuation between this cell and the observer
+    }
+    const float invG = 1.0f / G, CG = C * G;
+    const float sc = DUST ? 0.0f : (a_c != 0.0f ? e_c / a_c : 0.0f) - C;
+    float acc_e = 0.0f, acc_a = 0.0f, acc_d = 0.0f, accW = 0.0f, accQ = 0.0f, accPD = 0.0f;
+    if (W > 0) {
+      for (int c = klo + lane; c <= khi; c += 32) {
+        const float dErf = channel_derf(c, c_los, s);
+        const float tau_L = a_c * dErf, J_L = e_c * dErf, tau_T = tau_L + tau_d;
+        const float xr = xrem[c] - tau_L;
+        const float w = wh[c];
+        const float Pn = w * exp_neg(xr);
+        xrem[c] = xr; P[c] = Pn; Q[c] = w * one_minus_exp_neg(xr);
+        const float Dto = Dt[c];
+        const float Tk = fmaf(Dto, invG, C);
+        const float mT = one_minus_exp_neg(tau_T);
+        float wT, wpT;
+        w_and_wprime(tau_T, mT, wT, wpT);
+        const float src = fmaf(S_d, tau_d, J_L);
+        const float dIdtau = fmaf(-Tk, 1.0f - mT, src * wpT);
+        acc_e = fmaf(Pn * wT, dErf, acc_e);
+        acc_a = fmaf(Pn * dIdtau, dErf, acc_a);
+        acc_d = fmaf(Pn, fmaf(S_d, wT, dIdtau), acc_d);
+        accW += w;
+        // forward step (same cancellation-free form as transfer_window_kernel)
+        float Dn;
+        if (DUST) {
+          const float m = one_minus_exp_neg(tau_L);
+          const float r = rcp_approx(tau_T == 0.0f ? 1.0f : tau_T);
+          const float Em = E_d * m;
+          const float t1 = m_d + Em;
+          const float t2 = fmaf(tau_d, Em, -tau_L * m_d);
+          const float num = fmaf(J_L, t1, S_d * t2);
+          Dn = fmaf(-(Dto + CG), m, Dto);
+          Dn = fmaf(Gn * r, num, Dn);
+        } else {
+          Dn = update_nodust(Dto, dErf, a_c, sc);
+        }
+        Dt[c] = Dn;
+      }
+    }
+    if (DUST) {
+      // channels outside the window: only the dust of this cell acts on them
+      for (int c = lane; c < nv; c += 32)
+        if (W == 0 || c < klo || c > khi) { accQ += Q[c]; accPD = fmaf(P[c], Dt[c], accPD); }
+    }
+    acc_e = warp_sum(acc_e); acc_a = warp_sum(acc_a);
+    if (DUST) { acc_d = warp_sum(acc_d); accW = warp_sum(accW); accQ = warp_sum(accQ); accPD = warp_sum(accPD); }
+    if (lane == 0) {
+      const int64_t cell = (int64_t)z * npix + pix;
+      const float pre = ac.scale * Lam;
+      float g = pre * (acc_e * dcoef[cell] + acc_a * dcoef[ncell + cell]);
+      if (DUST) {
+        const float sub = ac.subtract ? 1.0f : 0.0f;
+        const float dSC = S_d - C;
+        const float outside = fmaf(dSC, (1.0f - sub) * (Wtot - accW) - accQ, -invG * accPD);
+        const float g_d = pre * (acc_d - sub * E_d * dSC * accW + E_d * outside);
+        g = fmaf(g_d, ac.c_d, g);
+      }
+      grad[cell] = g;
+    }
+    if (DUST) {
+      C = fmaf(C, E_d, S_d * m_d);
+      G = Gn;
+      if (G > 1.0e18f) {
+        const float inv = 1.0f / G;
+        __syncwarp();
+        for (int c = lane; c < nv; c += 32) Dt[c] *= inv;
+        G = 1.0f;
+      }
+    }
+    __syncwarp();
+  }
+}
+
+template <int N>
+inline void launch_coef_grad(const LevelConsts& lc, const AdjointConsts& ac, int64_t ncell, const float* n, const float* T,
+                             float* dcoef, cudaStream_t st) {
+  coef_grad_kernel<N><<<(unsigned)((ncell + 127) / 128), 128, 0, st>>>(lc, ac, ncell, n, T, dcoef);
+}
+
+// K9 then K8.  dcoef: scratch [2][ncell].  Returns the first CUDA error; *launches is advanced per kernel.
+inline cudaError_t launch_adjoint(const MarchConsts& mc, const AdjointConsts& ac, const LevelConsts& lc, int n_levels,
+                                  const float* coef, float* dcoef, int64_t ncell, int npix, int nz, int nv, bool dust,
+                                  const float* nH2, const float* Tgas, const float* what, float* grad, cudaStream_t st,
+                                  uint64_t* launches) {
+  switch (n_levels) {
+    case 2: launch_coef_grad<2>(lc, ac, ncell, nH2, Tgas, dcoef, st); break;
+    case 3: launch_coef_grad<3>(lc, ac, ncell, nH2, Tgas, dcoef, st); break;
+    case 4: launch_coef_grad<4>(lc, ac, ncell, nH2, Tgas, dcoef, st); break;
+    case 5: launch_coef_grad<5>(lc, ac, ncell, nH2, Tgas, dcoef, st); break;
+    case 6: launch_coef_grad<6>(lc, ac, ncell, nH2, Tgas, dcoef, st); break;
+    case 7: launch_coef_grad<7>(lc, ac, ncell, nH2, Tgas, dcoef, st); break;
+    case 8: launch_coef_grad<8>(lc, ac, ncell, nH2, Tgas, dcoef, st); break;
+    case 9: launch_coef_grad<9>(lc, ac, ncell, nH2, Tgas, dcoef, st); break;
+    default: launch_coef_grad<10>(lc, ac, ncell, nH2, Tgas, dcoef, st); break;
+  }
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  ++*launches;
+  int wpc = 4;
+  while (wpc > 1 && (size_t)wpc * 5 * nv * sizeof(float) > 200 * 1024) wpc >>= 1;
+  const size_t smem = (size_t)wpc * 5 * nv * sizeof(float);
+  if (smem > 227 * 1024) return cudaErrorInvalidConfiguration;
+  const unsigned grid = (unsigned)((npix + wpc - 1) / wpc);
+  if (dust) {
+    e = cudaFuncSetAttribute(adjoint_march_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    adjoint_march_kernel<true><<<grid, wpc * 32, smem, st>>>(mc, ac, coef, dcoef, ncell, npix, nz, nv, what, grad);
+  } else {
+    e = cudaFuncSetAttribute(adjoint_march_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    adjoint_march_kernel<false><<<grid, wpc * 32, smem, st>>>(mc, ac, coef, dcoef, ncell, npix, nz, nv, what, grad);
+  }
+  e = cudaGetLastError();
+  if (e == cudaSuccess) ++*launches;
+  return e;
 }
 
 }  // namespace iris

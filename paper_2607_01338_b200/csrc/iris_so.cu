@@ -545,18 +545,23 @@ iris_so_status iris_so_observe_adjoint(iris_so_ctx* ctx, const float* d_nH2, con
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   iris_so_status s = run_coefficients(ctx, d_nH2, d_Tgas, d_Tdust, d_vlos, nullptr, st);
   if (s != IRIS_SO_OK) return s;
-  // what = G^T w (the beam is symmetric and zero padded, so its adjoint is the same convolution)
+  // scratch: d(e_c)/dn and d(a_c)/dn per cell, then (with a beam) what = G^T w -- the beam is symmetric and zero
+  // padded, so its adjoint is the same convolution
+  const size_t dcoef_floats = 2 * (size_t)ctx->ncell;
+  const size_t need = sizeof(float) * (dcoef_floats + (c.beam_fwhm_px > 0.0 ? (size_t)ctx->nvox : 0));
+  if (ctx->d_adj && ctx->adj_bytes < need) { cudaFree(ctx->d_adj); ctx->d_adj = nullptr; ctx->scratch_bytes -= ctx->adj_bytes; }
+  if ((s = ensure(ctx, &ctx->d_adj, need, "cudaMalloc(adjoint scratch)")) != IRIS_SO_OK) return s;
+  ctx->adj_bytes = need;
+  float* dcoef = ctx->d_adj;
   const float* what = d_w;
   if (c.beam_fwhm_px > 0.0) {
-    const size_t need = sizeof(float) * (size_t)ctx->nvox;
-    if (ctx->d_adj && ctx->adj_bytes < need) { cudaFree(ctx->d_adj); ctx->d_adj = nullptr; ctx->scratch_bytes -= ctx->adj_bytes; }
-    if ((s = ensure(ctx, &ctx->d_adj, need, "cudaMalloc(adjoint weights)")) != IRIS_SO_OK) return s;
-    ctx->adj_bytes = need;
-    if ((s = run_beam(ctx, d_w, ctx->d_adj, nullptr, false, st)) != IRIS_SO_OK) return s;
-    what = ctx->d_adj;
+    float* wb = ctx->d_adj + dcoef_floats;
+    if ((s = run_beam(ctx, d_w, wb, nullptr, false, st)) != IRIS_SO_OK) return s;
+    what = wb;
   }
-  cudaError_t e = iris::launch_adjoint(ctx->mc, ctx->ac, ctx->lc, c.n_levels, ctx->d_coef, ctx->ncell, (int)ctx->npix, c.nz,
-                                       c.nv, c.dust_on != 0, d_nH2, d_Tgas, what, d_grad, st, &ctx->launches);
+  ProfScope prof(ctx, IRIS_SO_STAGE_ADJOINT, st);
+  cudaError_t e = iris::launch_adjoint(ctx->mc, ctx->ac, ctx->lc, c.n_levels, ctx->d_coef, dcoef, ctx->ncell, (int)ctx->npix,
+                                       c.nz, c.nv, c.dust_on != 0, d_nH2, d_Tgas, what, d_grad, st, &ctx->launches);
   if (e != cudaSuccess) return cuda_fail(ctx, e, "launch of adjoint kernels");
   return IRIS_SO_OK;
 }

@@ -1,0 +1,120 @@
+"""GPU parity of the gradient path (K8 + K9, BASELINE config 5): iris_so_observe_adjoint against the oracle's
+float64 finite differences of L = sum(w * cube) (noise-free, beam applied), and against the oracle's analytic
+float64 adjoint (itself pinned to finite differences in tests/test_oracle_pins.py) on every cell.
+
+Tolerance (north_star): relative error <= 1e-3.  A cell's gradient is a sum over channels of terms of both
+signs, so "relative" is taken per cell against |g| plus a floor of 1e-4 of the largest |g| in the cube
+(DESIGN.md section 6)."""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+
+from iris_inputs import make_fields, make_workload, weight_cube
+from oracle import Oracle
+
+pytestmark = pytest.mark.gpu
+
+REL, FLOOR = 1.0e-3, 1.0e-4
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def gpu_grad(cfg, f, w):
+    from paper_2607_01338_b200 import IrisSO
+    g = IrisSO(cfg).observe_adjoint(*[dev(f[k]) for k in ("nH2", "Tgas", "Tdust", "vlos")], dev(w.astype(np.float32)))
+    return g.cpu().numpy().astype(np.float64)
+
+
+def excess(g, ref, scale):
+    """max over cells of |g - ref| / (REL * |ref| + REL * FLOOR * scale); <= 1 passes."""
+    return float(np.max(np.abs(g - ref) / (REL * np.abs(ref) + REL * FLOOR * scale)))
+
+
+def check(cfg, f, w, n_fd=48, seed=5, label=""):
+    o = Oracle(cfg)
+    what = o.beam(w.astype(np.float64)) if cfg.beam_fwhm_px > 0 else w.astype(np.float64)
+    ref = o.grad_adjoint(f, what)
+    g = gpu_grad(cfg, f, w).reshape(ref.shape)
+    assert np.all(np.isfinite(g))
+    scale = np.abs(ref).max()
+    assert scale > 0
+    worst = excess(g, ref, scale)
+    # finite differences on a seeded sample of cells, biased to cells that matter
+    rng = np.random.default_rng(seed)
+    order = np.argsort(-np.abs(ref).ravel())
+    cells = np.unique(np.concatenate([order[: n_fd // 2], rng.choice(cfg.n_cells, size=n_fd // 2, replace=False)]))
+    gfd = o.grad_fd(f, what, cells, eps=1e-5)
+    worst_fd = excess(g.ravel()[cells], gfd, scale)
+    print("adjoint %s: worst vs analytic %.3g, vs finite differences %.3g of tolerance (max|g| %.3g)" %
+          (label, worst, worst_fd, scale))
+    assert worst <= 1.0 and worst_fd <= 1.0
+    return g
+
+
+def test_adjoint_tiny_no_dust():
+    cfg, r = make_workload("tiny", n=16, nv=64)
+    f = make_fields(cfg, r)
+    f["vlos"] = (0.15 * f["vlos"]).astype(np.float32)
+    check(cfg, f, weight_cube(cfg), label="tiny")
+
+
+@pytest.mark.parametrize("case", ["dust_beam", "thick", "intensity_out", "no_subtraction", "heavy_dust", "five_levels"])
+def test_adjoint_regimes(case):
+    kw = dict(n=20, nv=96)
+    if case == "five_levels":
+        kw["n_levels"] = 5
+    cfg, r = make_workload("batch", **kw)
+    f = make_fields(cfg, r)
+    f["vlos"] = (0.2 * f["vlos"]).astype(np.float32)
+    if case == "thick":
+        cfg = cfg.with_(abundance=2e-5)
+    elif case == "intensity_out":
+        cfg = cfg.with_(out_unit=0)
+    elif case == "no_subtraction":
+        cfg = cfg.with_(subtract_continuum=False)
+    elif case == "heavy_dust":
+        cfg = cfg.with_(kappa_gas_cm2_g=5.0)
+    check(cfg, f, weight_cube(cfg), label=case)
+
+
+def test_adjoint_ragged_and_degenerate_shapes():
+    cfg, r = make_workload("batch", n=8, nx=5, ny=3, nz=37, nv=45)
+    f = make_fields(cfg, r)
+    f["vlos"] = (0.1 * f["vlos"]).astype(np.float32)
+    check(cfg, f, weight_cube(cfg), n_fd=20, label="ragged")
+    cfg1, r1 = make_workload("batch", n=1, nx=1, ny=1, nz=1, nv=1)
+    cfg1 = cfg1.with_(dv_cms=4.0e5, v0_cms=0.0, beam_fwhm_px=0.0)
+    f1 = make_fields(cfg1, r1)
+    f1["vlos"] = np.zeros_like(f1["vlos"])
+    check(cfg1, f1, np.ones((1, 1, 1), np.float32), n_fd=2, label="1x1x1")
+
+
+def test_adjoint_is_linear_in_w_and_zero_without_weights():
+    cfg, r = make_workload("batch", n=12, nv=64)
+    f = make_fields(cfg, r)
+    f["vlos"] = (0.15 * f["vlos"]).astype(np.float32)
+    w1 = weight_cube(cfg, seed=2000); w2 = weight_cube(cfg, seed=2001)
+    g1, g2, g12 = gpu_grad(cfg, f, w1), gpu_grad(cfg, f, w2), gpu_grad(cfg, f, w1 + 2 * w2)
+    s = np.abs(g12).max()
+    assert np.max(np.abs(g12 - (g1 + 2 * g2))) <= 2e-5 * s
+    assert np.all(gpu_grad(cfg, f, np.zeros_like(w1)) == 0.0)
+
+
+def test_batch_workload_cubes_and_gradient():
+    """BASELINE config 5 at reduced size: independent seeded cubes, each rendered with dust, beam and noise,
+    plus the gradient for the seeded weight cube."""
+    from paper_2607_01338_b200 import IrisSO
+    from parity import assert_spectra
+    for i in range(3):
+        cfg, r = make_workload("batch", n=24, nv=128, seed=1000 + i)
+        f = make_fields(cfg, r)
+        d = [dev(f[k]) for k in ("nH2", "Tgas", "Tdust", "vlos")]
+        cube = IrisSO(cfg).observe(*d).cpu().numpy()
+        ref = Oracle(cfg).observe(f)
+        clean = Oracle(cfg).observe(f, noise=False)
+        assert_spectra(cube, ref, extra=8e-6 * cfg.noise_sigma, peak_of=clean, what="batch cube %d" % i)
+        check(cfg, f, weight_cube(cfg), n_fd=24, label="batch cube %d (v_edge %.0f, sigma_t %.1f km/s)" %
+              (i, f["meta"]["v_edge_kms"], f["meta"]["sigma_t_kms"]))
