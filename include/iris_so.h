@@ -53,7 +53,10 @@ typedef enum {
 /* transfer_algo */
 #define IRIS_SO_ALGO_AUTO 0     /* = IRIS_SO_ALGO_WINDOW */
 #define IRIS_SO_ALGO_DENSE 1    /* every (cell, channel) update evaluated; register-resident channel blocks */
-#define IRIS_SO_ALGO_WINDOW 2   /* only channels inside each cell's line window are updated; exact in fp32 */
+#define IRIS_SO_ALGO_WINDOW 2   /* only channels inside each cell's line window are updated; exact in fp32.
+                                 * Profile from the channel-centre expansion when dv / xi <= 0.55 (every cell then
+                                 * has dv / b <= 0.55), otherwise from erfc at the channel edges */
+#define IRIS_SO_ALGO_WINDOW_EDGE 3 /* line window with the erfc-at-the-edges profile for any channel width */
 
 typedef struct {
   /* grid: Cartesian analogue of the paper's (r, l, b) lattice; rays = z columns */
@@ -165,6 +168,10 @@ iris_so_status iris_so_profile_read(iris_so_ctx *ctx, int32_t stage, double *tot
  * coefficient planes left in the context by the last transfer / observe call (the updates the line-window
  * algorithm evaluates; the dense algorithm evaluates nx*ny*nz*nv).  Synchronises the stream. */
 iris_so_status iris_so_transfer_work(iris_so_ctx *ctx, uint64_t *window_updates, void *cuda_stream);
+
+/* Name of the LOS transfer kernel this context launches ("transfer_series_kernel", "transfer_window_kernel"
+ * or "transfer_dense_kernel"); static storage. */
+const char *iris_so_transfer_kernel(const iris_so_ctx *ctx);
 
 /* Stand-alone post-processing stages (also used inside iris_so_observe). */
 /* K6: separable Gaussian beam of FWHM beam_fwhm_px on d_in -> d_out (must not alias), zero padding,

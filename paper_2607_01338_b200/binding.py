@@ -8,14 +8,14 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libiris_so.so")
 _lib = None
 
-ALGO_AUTO, ALGO_DENSE, ALGO_WINDOW = 0, 1, 2
+ALGO_AUTO, ALGO_DENSE, ALGO_WINDOW, ALGO_WINDOW_EDGE = 0, 1, 2, 3
 
 # every entry point include/iris_so.h declares
 DECLARED_SYMBOLS = (
     "iris_so_create", "iris_so_destroy", "iris_so_last_error", "iris_so_status_string", "iris_so_version",
     "iris_so_launch_count", "iris_so_scratch_bytes", "iris_so_levelpop", "iris_so_transfer", "iris_so_observe",
     "iris_so_observe_stages", "iris_so_observe_host", "iris_so_observe_adjoint", "iris_so_beam", "iris_so_noise",
-    "iris_so_profile", "iris_so_profile_read", "iris_so_transfer_work",
+    "iris_so_profile", "iris_so_profile_read", "iris_so_transfer_work", "iris_so_transfer_kernel",
 )
 STAGES = {"cell": 0, "transfer": 1, "beam": 2, "noise": 3, "adjoint": 4}
 
@@ -96,6 +96,8 @@ def load_library():
     lib.iris_so_profile.argtypes = [vp, C.c_int32]
     lib.iris_so_profile_read.restype = st
     lib.iris_so_profile_read.argtypes = [vp, C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_uint64)]
+    lib.iris_so_transfer_kernel.restype = C.c_char_p
+    lib.iris_so_transfer_kernel.argtypes = [vp]
     lib.iris_so_transfer_work.restype = st
     lib.iris_so_transfer_work.argtypes = [vp, C.POINTER(C.c_uint64), vp]
     _lib = lib
@@ -193,6 +195,10 @@ class IrisSO:
             self._check(self.lib.iris_so_profile_read(self._h, sid, C.byref(ms), C.byref(n)))
             out[name] = (ms.value, int(n.value))
         return out
+
+    def transfer_kernel(self):
+        """Name of the LOS transfer kernel this context launches."""
+        return self.lib.iris_so_transfer_kernel(self._h).decode()
 
     def transfer_work(self):
         n = C.c_uint64()

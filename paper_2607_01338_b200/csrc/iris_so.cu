@@ -16,6 +16,7 @@
 #include "post_kernels.cuh"
 #include "transfer_dense.cuh"
 #include "transfer_window.cuh"
+#include "transfer_series.cuh"
 #include "adjoint_kernels.cuh"
 
 namespace {
@@ -164,7 +165,7 @@ iris_so_status validate(const iris_so_config* c, std::string& why) {
   if (!(c->beam_fwhm_px >= 0.0)) return bad("beam_fwhm_px must be >= 0");
   if (!(c->noise_sigma >= 0.0) || !std::isfinite(c->noise_mu)) return bad("bad noise parameters");
   if (c->noise_gamma_mode < 0 || c->noise_gamma_mode > 1) return bad("bad noise_gamma_mode");
-  if (c->transfer_algo < 0 || c->transfer_algo > 2) return bad("bad transfer_algo");
+  if (c->transfer_algo < 0 || c->transfer_algo > 3) return bad("bad transfer_algo");
   return IRIS_SO_OK;
 }
 
@@ -296,12 +297,20 @@ iris_so_status run_coefficients(iris_so_ctx* ctx, const float* n, const float* T
   return IRIS_SO_OK;
 }
 
+// Which transfer kernel the configuration selects: 1 dense, 2 window + centre-expansion profile, 3 window + erfc edges.
+int resolved_algo(const iris_so_config& c) {
+  int algo = c.transfer_algo;
+  if (algo == IRIS_SO_ALGO_AUTO) algo = IRIS_SO_ALGO_WINDOW;
+  if (algo == IRIS_SO_ALGO_WINDOW && !(c.microturb_cms > 0.0 && c.dv_cms <= (double)iris::kSeriesMaxS * c.microturb_cms))
+    algo = IRIS_SO_ALGO_WINDOW_EDGE;      // b >= xi bounds dv / b only when there is microturbulence
+  return algo;
+}
+
 // K3 (+K4, K5) from ctx->d_coef
 iris_so_status run_transfer(iris_so_ctx* ctx, const iris::MarchConsts& mc, float* out, float* out_cont, cudaStream_t st) {
   const bool dust = ctx->cfg.dust_on != 0;
   const int npix = (int)ctx->npix, nz = ctx->cfg.nz, nv = ctx->cfg.nv;
-  int algo = ctx->cfg.transfer_algo;
-  if (algo == IRIS_SO_ALGO_AUTO) algo = IRIS_SO_ALGO_WINDOW;
+  const int algo = resolved_algo(ctx->cfg);
   ProfScope prof(ctx, IRIS_SO_STAGE_TRANSFER, st);
   if (algo == IRIS_SO_ALGO_DENSE) {
     constexpr int CB = 16, NW = 4;
@@ -311,9 +320,11 @@ iris_so_status run_transfer(iris_so_ctx* ctx, const iris::MarchConsts& mc, float
     IRIS_CHECK_LAUNCH(ctx, "transfer_dense_kernel");
     return IRIS_SO_OK;
   }
-  cudaError_t e = iris::launch_transfer_window(mc, ctx->d_coef, ctx->ncell, npix, nz, nv, dust, ctx->sm_count, out, out_cont, st);
+  cudaError_t e = algo == IRIS_SO_ALGO_WINDOW
+                      ? iris::launch_transfer_series(mc, ctx->d_coef, ctx->ncell, npix, nz, nv, dust, out, out_cont, st)
+                      : iris::launch_transfer_window(mc, ctx->d_coef, ctx->ncell, npix, nz, nv, dust, ctx->sm_count, out, out_cont, st);
   ctx->launches++;
-  if (e != cudaSuccess) return cuda_fail(ctx, e, "launch of transfer_window_kernel");
+  if (e != cudaSuccess) return cuda_fail(ctx, e, "launch of the line-window transfer kernel");
   return IRIS_SO_OK;
 }
 
@@ -364,6 +375,15 @@ const char* iris_so_status_string(iris_so_status s) {
 }
 
 const char* iris_so_last_error(const iris_so_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_error.c_str(); }
+
+const char* iris_so_transfer_kernel(const iris_so_ctx* ctx) {
+  if (!ctx) return "";
+  switch (resolved_algo(ctx->cfg)) {
+    case IRIS_SO_ALGO_DENSE: return "transfer_dense_kernel";
+    case IRIS_SO_ALGO_WINDOW: return "transfer_series_kernel";
+    default: return "transfer_window_kernel";
+  }
+}
 
 uint64_t iris_so_launch_count(const iris_so_ctx* ctx) { return ctx ? ctx->launches : 0; }
 uint64_t iris_so_scratch_bytes(const iris_so_ctx* ctx) { return ctx ? ctx->scratch_bytes : 0; }

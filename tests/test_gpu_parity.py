@@ -13,7 +13,7 @@ from parity import assert_pops, assert_spectra, krj
 
 pytestmark = pytest.mark.gpu
 
-ALGOS = {"window": 2, "dense": 1}
+ALGOS = {"window": 2, "window_edge": 3, "dense": 1}
 KB_ = 1.380649e-16
 
 
@@ -238,6 +238,27 @@ def test_beam_and_noise_kernels():
     it2, o2 = iris(cfg2), Oracle(cfg2)
     assert np.abs(it2.noise(dev(img)).cpu().numpy() - o2.noise(img)).max() < 8e-6 * cfg.noise_sigma + 3e-7 * np.abs(ref).max()
     assert np.abs(it2.beam(dev(img)).cpu().numpy() - o2.beam(img)).max() < 2e-6
+
+
+def test_window_kernel_selection_and_series_limit():
+    """ALGO_WINDOW takes the channel-centre expansion only when dv / xi <= 0.55 bounds dv / b for every cell;
+    at that limit (and with thick lines, where the profile wings carry the optical depth) it still meets the
+    tolerance; wider channels or no microturbulence fall back to the erfc-edge kernel."""
+    cfg, r = make_workload("small", n=24, nv=160)
+    f = make_fields(cfg, r)
+    f["vlos"] = (0.25 * f["vlos"]).astype(np.float32)
+    f["Tgas"] = np.full_like(f["Tgas"], 5.0)                # b ~ xi: dv / b at the limit in every cell
+    lim = cfg.with_(dv_cms=0.5499e5, v0_cms=(0.5 - 80) * 0.5499e5)
+    for c, want in ((lim, "transfer_series_kernel"), (lim.with_(dv_cms=0.56e5), "transfer_window_kernel"),
+                    (lim.with_(microturb_cms=0.0), "transfer_window_kernel")):
+        it = iris(c, 2)
+        assert it.transfer_kernel() == want
+        it.close()
+    assert iris(lim, 1).transfer_kernel() == "transfer_dense_kernel"
+    for ab in (2e-6, 2e-4, 2e-2):
+        c = lim.with_(abundance=ab)
+        worst = assert_spectra(run_observe(c, f, 2), Oracle(c).observe(f), what="series at dv/b = 0.55, X = %g" % ab)
+        print("series limit, abundance %g: worst %.3g of tolerance" % (ab, worst))
 
 
 # ------------------------------------------------------------------------------------------------
