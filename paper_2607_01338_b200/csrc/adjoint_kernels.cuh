@@ -33,11 +33,12 @@ struct AdjointConsts {
   int subtract;     // 1: cube_raw = total - continuum
 };
 
-// Level fractions x and their logarithmic density derivative y = n dx/dn.
-template <int N>
+// Level fractions x and their logarithmic density derivative y = n dx/dn.  BW: bandwidth of the rate matrix
+// (see level_fractions in cell_kernels.cuh).
+template <int N, int BW>
 __device__ __forceinline__ void level_fractions_grad(const LevelConsts& lc, float n, float T, float (&x)[N], float (&y)[N]) {
   float R[N][N];
-  const float invT = 1.0f / T;
+  const float invT = rcp_approx(T);
   const float kf = n * exp2f(lc.Texp * log2f(T * lc.inv_Tref));
   float q[N];
 #pragma unroll
@@ -47,6 +48,7 @@ __device__ __forceinline__ void level_fractions_grad(const LevelConsts& lc, floa
     float bz = 1.0f;
 #pragma unroll
     for (int l = u - 1; l >= 0; --l) {
+      if (u - l > BW) continue;
       bz *= q[l + 1];
       const int p = pair_index(u, l);
       R[u][l] = fmaf(kf, lc.coll[p], lc.rad_down[p]);
@@ -56,17 +58,20 @@ __device__ __forceinline__ void level_fractions_grad(const LevelConsts& lc, floa
   float inv[N];
 #pragma unroll
   for (int m = N - 1; m >= 1; --m) {
+    const int lo = m - BW > 0 ? m - BW : 0;
     float s = 0.0f;
 #pragma unroll
-    for (int j = 0; j < m; ++j) s += R[m][j];
-    inv[m] = 1.0f / s;
+    for (int j = 0; j < m; ++j)
+      if (j >= lo) s += R[m][j];
+    inv[m] = rcp_approx(s);
 #pragma unroll
-    for (int i = 0; i < m; ++i) R[i][m] *= inv[m];
+    for (int i = 0; i < m; ++i)
+      if (i >= lo) R[i][m] *= inv[m];
 #pragma unroll
     for (int i = 0; i < m; ++i)
 #pragma unroll
       for (int j = 0; j < m; ++j)
-        if (i != j) R[i][j] = fmaf(R[i][m], R[m][j], R[i][j]);
+        if (i != j && i >= lo && j >= lo) R[i][j] = fmaf(R[i][m], R[m][j], R[i][j]);
   }
   x[0] = 1.0f;
   float tot = 1.0f;
@@ -74,11 +79,12 @@ __device__ __forceinline__ void level_fractions_grad(const LevelConsts& lc, floa
   for (int j = 1; j < N; ++j) {
     float s = 0.0f;
 #pragma unroll
-    for (int i = 0; i < j; ++i) s = fmaf(x[i], R[i][j], s);
+    for (int i = 0; i < j; ++i)
+      if (j - i <= BW) s = fmaf(x[i], R[i][j], s);
     x[j] = s;
     tot += s;
   }
-  const float itot = 1.0f / tot;
+  const float itot = rcp_approx(tot);
 #pragma unroll
   for (int j = 0; j < N; ++j) x[j] *= itot;
   // right-hand side b = -x Q_C: net collisional outflow of every level (pairwise, so that sum(b) = 0)
@@ -90,6 +96,7 @@ __device__ __forceinline__ void level_fractions_grad(const LevelConsts& lc, floa
     float bz = 1.0f;
 #pragma unroll
     for (int l = u - 1; l >= 0; --l) {
+      if (u - l > BW) continue;
       bz *= q[l + 1];
       const int p = pair_index(u, l);
       const float f = x[u] * (kf * lc.coll[p]) - x[l] * (kf * bz * lc.coll_gr[p]);   // net flow u -> l
@@ -102,7 +109,8 @@ __device__ __forceinline__ void level_fractions_grad(const LevelConsts& lc, floa
   for (int m = N - 1; m >= 1; --m) {
     const float t = b[m] * inv[m];
 #pragma unroll
-    for (int j = 0; j < m; ++j) b[j] = fmaf(t, R[m][j], b[j]);
+    for (int j = 0; j < m; ++j)
+      if (m - j <= BW) b[j] = fmaf(t, R[m][j], b[j]);
   }
   y[0] = 0.0f;
   float sy = 0.0f;
@@ -110,7 +118,8 @@ __device__ __forceinline__ void level_fractions_grad(const LevelConsts& lc, floa
   for (int m = 1; m < N; ++m) {
     float s = -b[m] * inv[m];
 #pragma unroll
-    for (int i = 0; i < m; ++i) s = fmaf(y[i], R[i][m], s);
+    for (int i = 0; i < m; ++i)
+      if (m - i <= BW) s = fmaf(y[i], R[i][m], s);
     y[m] = s;
     sy += s;
   }
@@ -119,7 +128,7 @@ __device__ __forceinline__ void level_fractions_grad(const LevelConsts& lc, floa
 }
 
 // K9 (per cell): d e_c / d n and d a_c / d n  ->  dcoef[2][ncell]
-template <int N>
+template <int N, int BW>
 __global__ void __launch_bounds__(128) coef_grad_kernel(LevelConsts lc, AdjointConsts ac, int64_t ncell,
                                                         const float* __restrict__ nH2, const float* __restrict__ Tgas,
                                                         float* __restrict__ dcoef) {
@@ -127,7 +136,7 @@ __global__ void __launch_bounds__(128) coef_grad_kernel(LevelConsts lc, AdjointC
   if (i >= ncell) return;
   const float n = nH2[i], T = Tgas[i];
   float x[N], y[N];
-  level_fractions_grad<N>(lc, n, T, x, y);
+  level_fractions_grad<N, BW>(lc, n, T, x, y);
   float xu = 0.0f, xl = 0.0f;
 #pragma unroll
   for (int l = 0; l < N; ++l) {
@@ -306,27 +315,31 @@ adjoint_march_kernel(MarchConsts mc, AdjointConsts ac, const float* __restrict__
   }
 }
 
+// band <= kBandNarrow selects the banded elimination (BW = kBandNarrow), anything wider the dense one.
 template <int N>
-inline void launch_coef_grad(const LevelConsts& lc, const AdjointConsts& ac, int64_t ncell, const float* n, const float* T,
-                             float* dcoef, cudaStream_t st) {
-  coef_grad_kernel<N><<<(unsigned)((ncell + 127) / 128), 128, 0, st>>>(lc, ac, ncell, n, T, dcoef);
+inline void launch_coef_grad(const LevelConsts& lc, const AdjointConsts& ac, int band, int64_t ncell, const float* n,
+                             const float* T, float* dcoef, cudaStream_t st) {
+  const unsigned grid = (unsigned)((ncell + 127) / 128);
+  constexpr int BN = kBandNarrow < N - 1 ? kBandNarrow : N - 1;
+  if (band <= BN) coef_grad_kernel<N, BN><<<grid, 128, 0, st>>>(lc, ac, ncell, n, T, dcoef);
+  else coef_grad_kernel<N, N - 1><<<grid, 128, 0, st>>>(lc, ac, ncell, n, T, dcoef);
 }
 
 // K9 then K8.  dcoef: scratch [2][ncell].  Returns the first CUDA error; *launches is advanced per kernel.
 inline cudaError_t launch_adjoint(const MarchConsts& mc, const AdjointConsts& ac, const LevelConsts& lc, int n_levels,
-                                  const float* coef, float* dcoef, int64_t ncell, int npix, int nz, int nv, bool dust,
-                                  const float* nH2, const float* Tgas, const float* what, float* grad, cudaStream_t st,
-                                  uint64_t* launches) {
+                                  int band, const float* coef, float* dcoef, int64_t ncell, int npix, int nz, int nv,
+                                  bool dust, const float* nH2, const float* Tgas, const float* what, float* grad,
+                                  cudaStream_t st, uint64_t* launches) {
   switch (n_levels) {
-    case 2: launch_coef_grad<2>(lc, ac, ncell, nH2, Tgas, dcoef, st); break;
-    case 3: launch_coef_grad<3>(lc, ac, ncell, nH2, Tgas, dcoef, st); break;
-    case 4: launch_coef_grad<4>(lc, ac, ncell, nH2, Tgas, dcoef, st); break;
-    case 5: launch_coef_grad<5>(lc, ac, ncell, nH2, Tgas, dcoef, st); break;
-    case 6: launch_coef_grad<6>(lc, ac, ncell, nH2, Tgas, dcoef, st); break;
-    case 7: launch_coef_grad<7>(lc, ac, ncell, nH2, Tgas, dcoef, st); break;
-    case 8: launch_coef_grad<8>(lc, ac, ncell, nH2, Tgas, dcoef, st); break;
-    case 9: launch_coef_grad<9>(lc, ac, ncell, nH2, Tgas, dcoef, st); break;
-    default: launch_coef_grad<10>(lc, ac, ncell, nH2, Tgas, dcoef, st); break;
+    case 2: launch_coef_grad<2>(lc, ac, band, ncell, nH2, Tgas, dcoef, st); break;
+    case 3: launch_coef_grad<3>(lc, ac, band, ncell, nH2, Tgas, dcoef, st); break;
+    case 4: launch_coef_grad<4>(lc, ac, band, ncell, nH2, Tgas, dcoef, st); break;
+    case 5: launch_coef_grad<5>(lc, ac, band, ncell, nH2, Tgas, dcoef, st); break;
+    case 6: launch_coef_grad<6>(lc, ac, band, ncell, nH2, Tgas, dcoef, st); break;
+    case 7: launch_coef_grad<7>(lc, ac, band, ncell, nH2, Tgas, dcoef, st); break;
+    case 8: launch_coef_grad<8>(lc, ac, band, ncell, nH2, Tgas, dcoef, st); break;
+    case 9: launch_coef_grad<9>(lc, ac, band, ncell, nH2, Tgas, dcoef, st); break;
+    default: launch_coef_grad<10>(lc, ac, band, ncell, nH2, Tgas, dcoef, st); break;
   }
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;

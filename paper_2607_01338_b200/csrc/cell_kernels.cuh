@@ -25,6 +25,9 @@ namespace iris {
 constexpr int kMaxLevels = 10;
 constexpr int kMaxPairs = kMaxLevels * (kMaxLevels - 1) / 2;
 
+// Bandwidth (largest |i - j| with a non-zero rate) up to which the banded elimination is instantiated.
+constexpr int kBandNarrow = 2;
+
 // pair index of (u > l)
 __host__ __device__ constexpr int pair_index(int u, int l) { return u * (u - 1) / 2 + l; }
 
@@ -35,6 +38,7 @@ struct LevelConsts {
   float coll[kMaxPairs];        // K_ul(T_ref)
   float coll_gr[kMaxPairs];     // K_ul(T_ref) g_u / g_l
   float inv_Tref, Texp;
+  float rate_scale;             // every rate above has been multiplied by this (1 / largest Einstein A)
 };
 
 struct CoefConsts {
@@ -50,10 +54,17 @@ struct CoefConsts {
 };
 
 // Level fractions of one cell.  N is a template parameter so that the rate matrix lives in registers.
-template <int N>
+// BW is the bandwidth of the rate matrix: rates i -> j with |i - j| > BW are zero (the host checks this against
+// the molecule, iris_so_create).  State elimination of the highest state m only couples the states m-BW..m-1
+// among themselves, so the band is preserved and the elimination costs O(N BW^2) instead of O(N^3); BW = N-1 is
+// the dense case.  The rigid-rotor workloads (radiative dJ = 1, collisional dJ <= 2) have BW = 2.
+// The fractions do not change when every rate is multiplied by one constant; the host divides all rates by the
+// largest Einstein A (LevelConsts::rate_scale), which keeps the pivots far from the fp32 denormal range so that
+// the reciprocals can be MUFU.RCP (1 ulp, flush-to-zero).
+template <int N, int BW>
 __device__ __forceinline__ void level_fractions(const LevelConsts& lc, float n, float T, float (&x)[N]) {
-  float R[N][N];   // R[i][j]: rate i -> j (i != j)
-  const float invT = 1.0f / T;
+  float R[N][N];   // R[i][j]: rate i -> j (i != j); only |i - j| <= BW is touched
+  const float invT = rcp_approx(T);
   // n * (T / T_ref)^p
   const float kf = n * exp2f(lc.Texp * log2f(T * lc.inv_Tref));
   float q[N];      // Boltzmann factors of adjacent levels, exp(-(E_i - E_{i-1}) / T)
@@ -64,6 +75,7 @@ __device__ __forceinline__ void level_fractions(const LevelConsts& lc, float n, 
     float bz = 1.0f;
 #pragma unroll
     for (int l = u - 1; l >= 0; --l) {
+      if (u - l > BW) continue;
       bz *= q[l + 1];                                   // exp(-(E_u - E_l) / T), Eq. 3.7.2
       const int p = pair_index(u, l);
       R[u][l] = fmaf(kf, lc.coll[p], lc.rad_down[p]);
@@ -73,17 +85,20 @@ __device__ __forceinline__ void level_fractions(const LevelConsts& lc, float n, 
   // GTH elimination of states N-1 .. 1
 #pragma unroll
   for (int m = N - 1; m >= 1; --m) {
+    const int lo = m - BW > 0 ? m - BW : 0;
     float s = 0.0f;
 #pragma unroll
-    for (int j = 0; j < m; ++j) s += R[m][j];
-    const float inv = 1.0f / s;
+    for (int j = 0; j < m; ++j)
+      if (j >= lo) s += R[m][j];
+    const float inv = rcp_approx(s);
 #pragma unroll
-    for (int i = 0; i < m; ++i) R[i][m] *= inv;
+    for (int i = 0; i < m; ++i)
+      if (i >= lo) R[i][m] *= inv;
 #pragma unroll
     for (int i = 0; i < m; ++i)
 #pragma unroll
       for (int j = 0; j < m; ++j)
-        if (i != j) R[i][j] = fmaf(R[i][m], R[m][j], R[i][j]);
+        if (i != j && i >= lo && j >= lo) R[i][j] = fmaf(R[i][m], R[m][j], R[i][j]);
   }
   x[0] = 1.0f;
   float tot = 1.0f;
@@ -91,11 +106,12 @@ __device__ __forceinline__ void level_fractions(const LevelConsts& lc, float n, 
   for (int j = 1; j < N; ++j) {
     float s = 0.0f;
 #pragma unroll
-    for (int i = 0; i < j; ++i) s = fmaf(x[i], R[i][j], s);
+    for (int i = 0; i < j; ++i)
+      if (j - i <= BW) s = fmaf(x[i], R[i][j], s);
     x[j] = s;
     tot += s;
   }
-  const float inv = 1.0f / tot;
+  const float inv = rcp_approx(tot);
 #pragma unroll
   for (int j = 0; j < N; ++j) x[j] *= inv;
 }
@@ -111,23 +127,23 @@ __device__ __forceinline__ void cell_coefficients(const CoefConsts& cc, float n,
   o[2] = fmaf(vlos - cc.v0, cc.inv_dv, 0.5f);
   o[3] = cc.dv * rsqrtf(fmaf(cc.c_b, T, cc.xi2));
   o[4] = cc.c_d * n;
-  o[5] = cc.dust_on ? cc.hnu_k / expm1f(cc.hnu_k / Td) : 0.0f;
+  o[5] = cc.dust_on ? cc.hnu_k * rcp_approx(expm1f(cc.hnu_k * rcp_approx(Td))) : 0.0f;
 }
 
 // K1: pop[N][ncell]
-template <int N>
+template <int N, int BW>
 __global__ void __launch_bounds__(128) levelpop_kernel(LevelConsts lc, int64_t ncell, const float* __restrict__ nH2,
                                                        const float* __restrict__ Tgas, float* __restrict__ pop) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= ncell) return;
   float x[N];
-  level_fractions<N>(lc, nH2[i], Tgas[i], x);
+  level_fractions<N, BW>(lc, nH2[i], Tgas[i], x);
 #pragma unroll
   for (int l = 0; l < N; ++l) pop[(int64_t)l * ncell + i] = x[l];
 }
 
 // K1 + K2 fused: coef[6][ncell]; populations never leave registers.
-template <int N>
+template <int N, int BW>
 __global__ void __launch_bounds__(128) cellcoef_kernel(LevelConsts lc, CoefConsts cc, int64_t ncell,
                                                        const float* __restrict__ nH2, const float* __restrict__ Tgas,
                                                        const float* __restrict__ Tdust, const float* __restrict__ vlos,
@@ -136,7 +152,7 @@ __global__ void __launch_bounds__(128) cellcoef_kernel(LevelConsts lc, CoefConst
   if (i >= ncell) return;
   const float n = nH2[i], T = Tgas[i];
   float x[N];
-  level_fractions<N>(lc, n, T, x);
+  level_fractions<N, BW>(lc, n, T, x);
   float xu = 0.0f, xl = 0.0f;
 #pragma unroll
   for (int l = 0; l < N; ++l) {       // static indexing keeps x[] in registers

@@ -5,6 +5,7 @@
 
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -40,6 +41,7 @@ struct iris_so_ctx {
   iris::BeamConsts bc;
   iris::NoiseConsts nc;
   iris::AdjointConsts ac;
+  int band = 1;                 // largest u - l with a non-zero radiative or collisional rate
   int device = 0, sm_count = 0;
   int64_t ncell = 0, npix = 0, nvox = 0;
   float* d_coef = nullptr;      // [6][ncell]
@@ -182,7 +184,15 @@ void fold_constants(iris_so_ctx* ctx) {
   const int N = c.n_levels;
   iris::LevelConsts& lc = ctx->lc;
   std::memset(&lc, 0, sizeof lc);
+  ctx->band = 1;
+  for (int u = 1; u < N; ++u)
+    for (int l = 0; l < u; ++l)
+      if ((ctx->A[u * N + l] != 0.0 || ctx->Kd[u * N + l] != 0.0) && u - l > ctx->band) ctx->band = u - l;
   for (int i = 1; i < N; ++i) lc.dE_adj[i] = (float)(ctx->energy[i] - ctx->energy[i - 1]);
+  double Amax = 0.0;
+  for (double a : ctx->A) Amax = std::max(Amax, a);
+  const double rs = Amax > 0.0 ? 1.0 / Amax : 1.0;              // common rate scale (fractions are invariant)
+  lc.rate_scale = (float)rs;
   for (int u = 1; u < N; ++u)
     for (int l = 0; l < u; ++l) {
       const int p = iris::pair_index(u, l);
@@ -193,10 +203,10 @@ void fold_constants(iris_so_ctx* ctx) {
         const double hnu_k = ctx->energy[u] - ctx->energy[l];   // h nu_ul / k
         ngam = 1.0 / std::expm1(hnu_k / c.T_bar);               // photon occupation of B_nu(T_bar), Eq. 3.6.2
       }
-      lc.rad_down[p] = (float)(A * (1.0 + ngam));               // A_ul + B_ul J
-      lc.rad_up[p] = (float)(gr * A * ngam);                    // B_lu J
-      lc.coll[p] = (float)K;
-      lc.coll_gr[p] = (float)(K * gr);
+      lc.rad_down[p] = (float)(rs * A * (1.0 + ngam));          // A_ul + B_ul J
+      lc.rad_up[p] = (float)(rs * gr * A * ngam);               // B_lu J
+      lc.coll[p] = (float)(rs * K);
+      lc.coll_gr[p] = (float)(rs * K * gr);
     }
   lc.inv_Tref = (float)(1.0 / c.coll_T_ref);
   lc.Texp = (float)c.coll_T_exp;
@@ -259,14 +269,20 @@ void fold_constants(iris_so_ctx* ctx) {
 template <int N>
 void launch_levelpop(iris_so_ctx* ctx, const float* n, const float* T, float* pop, cudaStream_t st) {
   const int64_t nc = ctx->ncell;
-  iris::levelpop_kernel<N><<<(unsigned)((nc + 127) / 128), 128, 0, st>>>(ctx->lc, nc, n, T, pop);
+  const unsigned grid = (unsigned)((nc + 127) / 128);
+  constexpr int BN = iris::kBandNarrow < N - 1 ? iris::kBandNarrow : N - 1;
+  if (ctx->band <= BN) iris::levelpop_kernel<N, BN><<<grid, 128, 0, st>>>(ctx->lc, nc, n, T, pop);
+  else iris::levelpop_kernel<N, N - 1><<<grid, 128, 0, st>>>(ctx->lc, nc, n, T, pop);
 }
 
 template <int N>
 void launch_cellcoef(iris_so_ctx* ctx, const float* n, const float* T, const float* Td, const float* v, float* coef,
                      cudaStream_t st) {
   const int64_t nc = ctx->ncell;
-  iris::cellcoef_kernel<N><<<(unsigned)((nc + 127) / 128), 128, 0, st>>>(ctx->lc, ctx->cc, nc, n, T, Td, v, coef);
+  const unsigned grid = (unsigned)((nc + 127) / 128);
+  constexpr int BN = iris::kBandNarrow < N - 1 ? iris::kBandNarrow : N - 1;
+  if (ctx->band <= BN) iris::cellcoef_kernel<N, BN><<<grid, 128, 0, st>>>(ctx->lc, ctx->cc, nc, n, T, Td, v, coef);
+  else iris::cellcoef_kernel<N, N - 1><<<grid, 128, 0, st>>>(ctx->lc, ctx->cc, nc, n, T, Td, v, coef);
 }
 
 #define IRIS_DISPATCH_N(N_, CALL)                       \
@@ -580,7 +596,7 @@ iris_so_status iris_so_observe_adjoint(iris_so_ctx* ctx, const float* d_nH2, con
     what = wb;
   }
   ProfScope prof(ctx, IRIS_SO_STAGE_ADJOINT, st);
-  cudaError_t e = iris::launch_adjoint(ctx->mc, ctx->ac, ctx->lc, c.n_levels, ctx->d_coef, dcoef, ctx->ncell, (int)ctx->npix,
+  cudaError_t e = iris::launch_adjoint(ctx->mc, ctx->ac, ctx->lc, c.n_levels, ctx->band, ctx->d_coef, dcoef, ctx->ncell, (int)ctx->npix,
                                        c.nz, c.nv, c.dust_on != 0, d_nH2, d_Tgas, what, d_grad, st, &ctx->launches);
   if (e != cudaSuccess) return cuda_fail(ctx, e, "launch of adjoint kernels");
   return IRIS_SO_OK;

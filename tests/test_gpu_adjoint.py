@@ -61,7 +61,8 @@ def test_adjoint_tiny_no_dust():
     check(cfg, f, weight_cube(cfg), label="tiny")
 
 
-@pytest.mark.parametrize("case", ["dust_beam", "thick", "intensity_out", "no_subtraction", "heavy_dust", "five_levels"])
+@pytest.mark.parametrize("case", ["dust_beam", "thick", "intensity_out", "no_subtraction", "heavy_dust", "five_levels",
+                                  "dense_collisions"])
 def test_adjoint_regimes(case):
     kw = dict(n=20, nv=96)
     if case == "five_levels":
@@ -77,6 +78,12 @@ def test_adjoint_regimes(case):
         cfg = cfg.with_(subtract_continuum=False)
     elif case == "heavy_dust":
         cfg = cfg.with_(kappa_gas_cm2_g=5.0)
+    elif case == "dense_collisions":      # every dJ collides: the dense (not the banded) state elimination
+        Kd = np.array(cfg.coll_down_ref, dtype=np.float64, copy=True)
+        for u in range(1, cfg.n_levels):
+            for l in range(u):
+                Kd[u, l] = 1e-11 / (u - l)
+        cfg = cfg.with_(coll_down_ref=Kd)
     check(cfg, f, weight_cube(cfg), label=case)
 
 

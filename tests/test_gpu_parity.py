@@ -57,6 +57,41 @@ def test_levelpop_extremes(n_levels, T_bar):
     assert_pops(pop, Oracle(cfg).levelpop(nn, TT))
 
 
+def _with_collisions_up_to(cfg, max_dj, seed=5):
+    """Same molecule with seeded collisional de-excitation rates for every dJ <= max_dj (and a weak dJ = 2
+    radiative transition when max_dj >= 3): exercises the banded (dJ <= 2) and the dense elimination."""
+    rng = np.random.default_rng(seed)
+    N = cfg.n_levels
+    Kd = np.array(cfg.coll_down_ref, dtype=np.float64, copy=True)
+    A = np.array(cfg.einstein_A, dtype=np.float64, copy=True)
+    for u in range(1, N):
+        for l in range(u):
+            Kd[u, l] = 0.0 if u - l > max_dj else 1e-11 * rng.uniform(0.2, 2.0) / (u - l)
+    if max_dj >= 3:
+        for u in range(2, N):
+            A[u, u - 2] = 1e-3 * A[u, u - 1]
+    return cfg.with_(coll_down_ref=Kd, einstein_A=A)
+
+
+@pytest.mark.parametrize("n_levels", [4, 7, 10])
+@pytest.mark.parametrize("max_dj", [1, 2, 3, 9])
+def test_levelpop_rate_matrix_bandwidth(n_levels, max_dj):
+    """Bandwidth 1 and 2 take the banded state elimination, 3 and above the dense one; both must give the
+    oracle's populations (and the same cube) for the same molecule."""
+    cfg, r = make_workload("tiny", n=12, n_levels=n_levels)
+    cfg = _with_collisions_up_to(cfg, min(max_dj, n_levels - 1))
+    n = np.logspace(-1, 8, 41, dtype=np.float32)
+    T = np.geomspace(8.0, 1500.0, 37).astype(np.float32)
+    nn, TT = np.meshgrid(n, T, indexing="ij")
+    nn, TT = np.ascontiguousarray(nn.ravel()), np.ascontiguousarray(TT.ravel())
+    cfg1 = cfg.with_(nx=nn.size, ny=1, nz=1)
+    pop = iris(cfg1).levelpop(dev(nn), dev(TT)).cpu().numpy().reshape(n_levels, -1)
+    assert_pops(pop, Oracle(cfg1).levelpop(nn, TT))
+    f = make_fields(cfg, r)
+    cube = iris(cfg).observe(*dev_fields(f)).cpu().numpy()
+    assert_spectra(cube, Oracle(cfg).observe(f), what="cube, collisions up to dJ=%d" % max_dj)
+
+
 # ------------------------------------------------------------------------------------------------
 # whole path on the BASELINE workloads (resized where the oracle would take minutes)
 def run_observe(cfg, f, algo, beam=True, noise=True):
