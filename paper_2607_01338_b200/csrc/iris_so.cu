@@ -337,7 +337,8 @@ iris_so_status run_transfer(iris_so_ctx* ctx, const iris::MarchConsts& mc, float
     return IRIS_SO_OK;
   }
   cudaError_t e = algo == IRIS_SO_ALGO_WINDOW
-                      ? iris::launch_transfer_series(mc, ctx->d_coef, ctx->ncell, npix, nz, nv, dust, out, out_cont, st)
+                      ? iris::launch_transfer_series(mc, ctx->d_coef, ctx->ncell, npix, nz, nv, dust,
+                                                     (float)(ctx->cfg.dv_cms / ctx->cfg.microturb_cms), out, out_cont, st)
                       : iris::launch_transfer_window(mc, ctx->d_coef, ctx->ncell, npix, nz, nv, dust, ctx->sm_count, out, out_cont, st);
   ctx->launches++;
   if (e != cudaSuccess) return cuda_fail(ctx, e, "launch of the line-window transfer kernel");

@@ -1,58 +1,75 @@
 // K3 (line-window formulation, narrow channels): the production LOS transfer kernel.
 //
 // Same recurrence and the same line window as transfer_window.cuh (difference form D = I^[T] - I^[C],
-// Dt = D * exp(sum tau_d), updates only inside |x| <= X_w), with two changes that remove most of the
-// instructions of that kernel:
+// Dt = D * exp(sum tau_d), updates only inside |x| <= X_w), with the instruction count per update cut to what
+// the recurrence needs:
 //
 // 1. Profile.  When a channel is narrower than ~half a Doppler width (s = dv / b <= kSeriesMaxS), the channel
 //    integral of the Gaussian profile (Eq. 4.6.3) is evaluated from the channel CENTRE x by
 //    the Taylor expansion of the integrand about the centre,
 //      erf(x + s/2) - erf(x - s/2) = (2 s / sqrt(pi)) exp(-x^2) [1 + (s^2/24) H_2(x) + (s^4/1920) H_4(x)
 //                                     + (s^6/322560) H_6(x) + (s^8/92897280) H_8(x)],   H_n = Hermite polynomials,
-//    i.e. exp(-x^2) times a degree-4 polynomial in x^2 whose five coefficients depend on the cell only.
-//    Truncation error at s = 0.55: <= 2e-7 relative for |x| <= 3, <= 2e-9 absolute everywhere (the error is
-//    relative to a value that is itself < 1e-9 beyond |x| = 4.4).  One MUFU.EX2 + 7 FP32 instructions per
-//    channel, no edge sharing between lanes, no sign handling.
-// 2. Per-cell work is done ONCE per cell, not once per lane: the march is cut into chunks of LPP cells; in
-//    phase A lane (g, i) of a warp turns the six coefficients of cell z0 + i of pixel g into a 16-float
-//    "march record" (window, scaled coordinates, polynomial, dust factors) in shared memory; in phase B the
-//    LPP lanes of pixel g walk the LPP cells, reading each record with four broadcast LDS.128.
+//    i.e. exp(-x^2) times a polynomial in x^2 whose coefficients depend on the cell only.  Degree 4 in x^2 up to
+//    s = 0.55 (truncation <= 2e-7 relative for |x| <= 3, <= 2e-9 absolute everywhere); degree 3 up to s = 0.3
+//    (the dropped term is s^8 x^8 / 362880 <= 1.5e-6 relative at |x| = 3.2, where the profile is 4e-5 of its peak).
+// 2. Units.  The line opacity is folded into the polynomial, and everything is carried in base-2 units, so the
+//    line optical depth of the update comes out of ONE multiply:  t = tau_L log2(e) = 2^(-x'^2) * polA(x'^2),
+//    x' = x sqrt(log2 e);  1 - exp(-tau_L) = 1 - 2^(-t);  1 / tau_T = log2(e) / (t + tau_d log2(e)).
+// 3. Per-cell work is done ONCE per cell, not once per lane: the march is cut into chunks of LPP cells; in
+//    phase A every lane turns the six coefficients of one (cell, pixel) of the chunk into a "march record"
+//    (window, scaled coordinates, polynomial, dust factors) in shared memory; in phase B the LPP lanes of a pixel
+//    walk the LPP cells, reading each record with broadcast LDS.128 one cell ahead of its use.
+// 4. The update loop is branch-free (predicated loads / stores) and two passes are in flight per lane.
 //
 // Mapping as in transfer_window.cuh: a warp owns 32/LPP adjacent pixels, LPP lanes per pixel; the spectrum
 // Dt[nv] of each pixel lives in shared memory for the whole march, bank-interleaved (channel c of pixel g at
-// word (c / LPP) * 32 + g * LPP + c % LPP: the lanes of a warp always hit 32 distinct banks).
+// word (c / LPP) * 32 + g * LPP + c % LPP: the lanes of a warp always hit 32 distinct banks).  Records are
+// stored quantity-major ([float4 index][record]) so that both the phase-A stores and the phase-B broadcast
+// loads are conflict-free.
 #pragma once
 #include "transfer_common.cuh"
 #include "transfer_window.cuh"
 
 namespace iris {
 
-constexpr float kSeriesMaxS = 0.55f;   // largest dv / b the centre expansion is used for
+constexpr float kSeriesMaxS = 0.55f;    // largest dv / b the centre expansion is used for
+constexpr float kSeriesDeg3MaxS = 0.3f; // largest dv / b for the degree-3 polynomial
 
-// March record of one cell (16 floats, four float4):
-//   r0 = { As, tau_d | sc, x0, xs }     As = a_c 2 s / sqrt(pi)  (tau_L = As g);  x0, xs: scaled centre of channel
-//                                       klo and scaled step, x' = x sqrt(log2 e) so that exp(-x^2) = 2^(-x'^2)
-//   r1 = { P, Q, R, bits(klo | khi << 16) }     num = g P + m (Q g + R)   (dust);  klo > khi: empty window
-//   r2 = { p0, p1, p2, p3 }             polynomial in u' = x'^2
-//   r3 = { p4, E_d, S_d m_d, exp(tau_d) }
-struct SeriesRecord { float4 r0, r1, r2, r3; };
+// March record of one (cell, pixel): NQ float4
+//   q0 = { x0, xs, tdp | sc, bits(klo | W << 16) }   x0: scaled centre of channel klo, xs: scaled channel step,
+//                                                    tdp = tau_d log2(e) + 1e-30 (dust), sc = S_L - T_bg (no dust),
+//                                                    W = window width in channels (0: empty)
+//   q1 = { pA0, pA1, pA2, pA3 }                      polA(u') = As' pol(u'),  As' = a_c (2 s / sqrt(pi)) log2(e)
+//   q2 = { P', Q', R', E_d }                         num' = t P' + m (Q' t + R')   (to be scaled by G')
+//   q3 = { S_d m_d, exp(tau_d), pA4, - }             (without dust: pA4 in q2.x)
+template <bool DUST, int DEG>
+struct SeriesLayout {
+  static constexpr int NQ = DUST ? 4 : (DEG > 3 ? 3 : 2);
+};
+
+struct SeriesRecord { float4 q0, q1, q2, q3; };
 
 // Phase A: coefficients of one cell -> march record.
-template <bool DUST>
+template <bool DUST, int DEG>
 __device__ __forceinline__ SeriesRecord make_series_record(float e_c, float a_c, float c_los, float s, float tau_d,
                                                            float S_d, float T_bg, int nv) {
+  constexpr float LOG2E = 1.4426950408889634f;
   SeriesRecord r;
   int klo, khi;
-  const int W = line_window(e_c, a_c, c_los, s, nv, klo, khi);
-  if (W <= 0) { klo = 1; khi = 0; }
+  int W = line_window(e_c, a_c, c_los, s, nv, klo, khi);
+  if (W <= 0) { W = 0; klo = 0; }
+  // |a_c| is kept above 1e-10 e_c: the source function e_c / a_c stays finite where the opacity crosses zero
+  // (changes tau_L by < 1e-10 e_c, i.e. < 1e-7 for a 1000 K line)
+  const float a_min = fmaxf(1.0e-10f * e_c, 1.0e-30f);
+  const float a_safe = fabsf(a_c) < a_min ? a_min : a_c;
   const float sp = 1.1283791670955126f * s;                 // 2 s / sqrt(pi)
-  const float a_safe = (a_c == 0.0f) ? 1.0e-30f : a_c;      // keeps e_c / a_c finite; tau_L stays ~0
   const float As = a_safe * sp, Es = e_c * sp;
+  const float Asp = As * LOG2E;
   const float xs = 1.2011224087864498f * s;                 // s sqrt(log2 e)
-  r.r0.x = As;
-  r.r0.z = ((float)klo + 0.5f - c_los) * xs;
-  r.r0.w = xs;
-  // polynomial in u = x^2, then rescaled to u' = u log2(e):  p'_k = p_k ln(2)^k
+  r.q0.x = ((float)klo + 0.5f - c_los) * xs;
+  r.q0.y = xs;
+  r.q0.w = __int_as_float(klo | (W << 16));
+  // polynomial in u = x^2, rescaled to u' = u log2(e) (p'_k = p_k ln(2)^k) and multiplied by As'
   const float s2 = s * s, s4 = s2 * s2, s6 = s4 * s2, s8 = s4 * s4;
   const float p0 = 1.0f - s2 * (1.0f / 12.0f) + s4 * (1.0f / 160.0f) - s6 * (1.0f / 2688.0f) + s8 * (1.0f / 55296.0f);
   const float p1 = s2 * (1.0f / 6.0f) - s4 * (1.0f / 40.0f) + s6 * (1.0f / 448.0f) - s8 * (1.0f / 6912.0f);
@@ -60,64 +77,141 @@ __device__ __forceinline__ SeriesRecord make_series_record(float e_c, float a_c,
   const float p3 = s6 * (1.0f / 5040.0f) - s8 * (1.0f / 25920.0f);
   const float p4 = s8 * (1.0f / 362880.0f);
   constexpr float L1 = 0.6931471805599453f, L2 = L1 * L1, L3 = L2 * L1, L4 = L2 * L2;
-  r.r2 = make_float4(p0, p1 * L1, p2 * L2, p3 * L3);
-  r.r3.x = p4 * L4;
-  r.r1.w = __int_as_float(klo | (khi << 16));
+  r.q1 = make_float4(Asp * p0, Asp * (p1 * L1), Asp * (p2 * L2), Asp * (p3 * L3));
+  r.q3.z = DEG > 3 ? Asp * (p4 * L4) : 0.0f;
+  r.q3.w = 0.0f;
   if (DUST) {
     const float E_d = exp_neg(tau_d);
     const float m_d = one_minus_exp_neg(tau_d);
-    r.r0.y = tau_d;
-    r.r1.x = m_d * fmaf(-S_d, As, Es);
-    r.r1.y = E_d * Es;
-    r.r1.z = E_d * S_d * tau_d;
-    r.r3.y = E_d;
-    r.r3.z = S_d * m_d;
-    r.r3.w = ex2_approx(tau_d * 1.4426950408889634f);
+    const float iA = LOG2E * rcp_approx(Asp);
+    r.q0.z = fmaf(tau_d, LOG2E, 1.0e-30f);
+    r.q2.x = m_d * fmaf(-S_d, As, Es) * iA;
+    r.q2.y = E_d * Es * iA;
+    r.q2.z = E_d * S_d * tau_d * LOG2E;
+    r.q2.w = E_d;
+    r.q3.x = S_d * m_d;
+    r.q3.y = ex2_approx(tau_d * LOG2E);
   } else {
-    r.r0.y = Es / As - T_bg;      // sc = S_L - C, C = T_bg throughout
-    r.r1.x = r.r1.y = r.r1.z = 0.0f;
-    r.r3.y = 1.0f; r.r3.z = 0.0f; r.r3.w = 1.0f;
+    r.q0.z = Es * rcp_approx(As) - T_bg;      // sc = S_L - C, C = T_bg throughout
+    r.q2 = make_float4(r.q3.z, 0.0f, 0.0f, 1.0f);   // pA4 travels in q2.x when there is no dust (NQ = 3)
+    r.q3.x = 0.0f; r.q3.y = 1.0f;
   }
   return r;
 }
 
-template <int LPP, bool DUST>
+// One update of one channel: Dt -> Dt'.  x: scaled channel centre.
+template <bool DUST, int DEG>
+__device__ __forceinline__ float series_update(float Dt, float x, const float4& q0, const float4& q1, float pA4,
+                                               float CG, float Pn, float Qn, float Rn) {
+  constexpr float L1 = 0.6931471805599453f, L2 = L1 * L1, L3 = L2 * L1, L4 = L2 * L2;
+  const float u = x * x;
+  float pol;
+  if (DEG > 3) { pol = fmaf(pA4, u, q1.w); pol = fmaf(pol, u, q1.z); }
+  else pol = fmaf(q1.w, u, q1.z);
+  pol = fmaf(pol, u, q1.y);
+  pol = fmaf(pol, u, q1.x);
+  const float t = ex2_approx(-u) * pol;                 // tau_L log2(e)
+  const float big = 1.0f - ex2_approx(-t);
+  float q = fmaf(t, -L4 / 24.0f, L3 / 6.0f);
+  q = fmaf(q, t, -L2 / 2.0f);
+  q = fmaf(q, t, L1);
+  const float m = fabsf(t) < 0.115f ? q * t : big;      // 1 - exp(-tau_L); Taylor below tau_L = 0.08
+  if (DUST) {
+    const float rr = rcp_approx(t + q0.z);
+    const float num = fmaf(m, fmaf(Qn, t, Rn), t * Pn);
+    Dt = fmaf(-(Dt + CG), m, Dt);
+    return fmaf(rr, num, Dt);
+  }
+  return fmaf(q0.z - Dt, m, Dt);
+}
+
+template <int LPP, bool DUST, int DEG>
 __global__ void __launch_bounds__(128)
 transfer_series_kernel(MarchConsts mc, const float* __restrict__ coef, int64_t ncell, int npix, int nz, int nv,
                        int nvp, float* __restrict__ out, float* __restrict__ out_cont) {
   extern __shared__ float4 smem4[];
   constexpr int PPW = 32 / LPP;
+  constexpr int NQ = SeriesLayout<DUST, DEG>::NQ;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, wpc = blockDim.x >> 5;
   const int g = lane / LPP, i = lane % LPP;
-  const int pix = (blockIdx.x * wpc + warp) * PPW + g;
+  const int pix0 = (blockIdx.x * wpc + warp) * PPW;
+  const int pix = pix0 + g;
   const bool valid = pix < npix;
-  const int pl = valid ? pix : npix - 1;
-  // shared memory: records [wpc][LPP cells][PPW pixels][4 float4], then spectra [wpc][nvp / LPP rows][32]
-  float4* rec = smem4 + (size_t)warp * (LPP * PPW * 4);
-  float* spec = reinterpret_cast<float*>(smem4 + (size_t)wpc * (LPP * PPW * 4));
+  // shared memory: records [wpc][NQ][32], then spectra [wpc][nvp / LPP rows][32]
+  float4* rec = smem4 + (size_t)warp * (NQ * 32);
+  float* spec = reinterpret_cast<float*>(smem4 + (size_t)wpc * (NQ * 32));
   float* sp = spec + (size_t)warp * nvp * PPW + g * LPP;
   for (int c = i; c < nvp; c += LPP) sp[(c / LPP) * 32 + i] = 0.0f;
 
   float C = mc.T_bg;      // continuum before the current cell
   float G = 1.0f;         // exp(dust optical depth accumulated so far), since the last rescale
 
-  // phase-A operands of the first chunk: lane (g, i) <-> cell z = i of pixel g
-  const float* p = coef + pl + (int64_t)i * npix;
+  // phase A: lane L makes record L of the chunk = (cell L / PPW, pixel L % PPW)
+  const int ja = lane / PPW, ga = lane % PPW;
+  const float* p = coef + min(pix0 + ga, npix - 1) + (int64_t)ja * npix;
   float l_e = 0.0f, l_a = 0.0f, l_c = 0.0f, l_s = 1.0f, l_td = 0.0f, l_sd = 0.0f;
-  if (i < nz) {
+  if (ja < nz) {
     l_e = p[0]; l_a = p[ncell]; l_c = p[2 * ncell]; l_s = p[3 * ncell];
     if (DUST) { l_td = p[4 * ncell]; l_sd = p[5 * ncell]; }
   }
 
+  // one cell of phase B for this lane's pixel, given the cell's record in registers
+  auto cell_step = [&](const float4& q0, const float4& q1, const float4& q2, const float4& q3) {
+    const int kk = __float_as_int(q0.w);
+    const int klo = kk & 0xffff, W = (int)((unsigned)kk >> 16);
+    const int npass = __reduce_max_sync(0xffffffffu, (W + LPP - 1) / LPP);   // 0 for an empty window
+    float CG = 0.0f, Pn = 0.0f, Qn = 0.0f, Rn = 0.0f;
+    if (DUST) {
+      const float Gn = G * q3.y;
+      CG = C * G;
+      C = fmaf(C, q2.w, q3.x);
+      Pn = q2.x * Gn; Qn = q2.y * Gn; Rn = q2.z * Gn;
+      G = Gn;
+    }
+    const float pA4 = DUST ? q3.z : q2.x;
+    if (npass > 0) {
+      int c = klo + i;
+      const int cend = klo + W;                    // one past the last channel of the window
+      float x = fmaf((float)i, q0.y, q0.x);
+      const float step = (float)LPP * q0.y;
+      float* d = sp + (c / LPP) * 32 + (c % LPP);
+      int ps = 0;
+      for (; ps + 2 <= npass; ps += 2) {
+        const bool okA = c < cend, okB = c + LPP < cend;
+        float DA = okA ? d[0] : 0.0f;
+        float DB = okB ? d[32] : 0.0f;
+        DA = series_update<DUST, DEG>(DA, x, q0, q1, pA4, CG, Pn, Qn, Rn);
+        DB = series_update<DUST, DEG>(DB, x + step, q0, q1, pA4, CG, Pn, Qn, Rn);
+        if (okA) d[0] = DA;
+        if (okB) d[32] = DB;
+        x = fmaf(2.0f, step, x); c += 2 * LPP; d += 64;
+      }
+      if (ps < npass) {
+        const bool okA = c < cend;
+        float DA = okA ? d[0] : 0.0f;
+        DA = series_update<DUST, DEG>(DA, x, q0, q1, pA4, CG, Pn, Qn, Rn);
+        if (okA) d[0] = DA;
+      }
+    }
+    if (DUST && G > 1.0e18f) {   // rare: fold the accumulated dust attenuation into the stored spectrum
+      const float inv = 1.0f / G;
+      __syncwarp(__activemask());
+      for (int cc = i; cc < nvp; cc += LPP) sp[(cc / LPP) * 32 + i] *= inv;
+      G = 1.0f;
+    }
+  };
+
   for (int z0 = 0; z0 < nz; z0 += LPP) {
     // ---- phase A: one record per lane
     {
-      const SeriesRecord r = make_series_record<DUST>(l_e, l_a, l_c, l_s, l_td, l_sd, mc.T_bg, nv);
+      const SeriesRecord r = make_series_record<DUST, DEG>(l_e, l_a, l_c, l_s, l_td, l_sd, mc.T_bg, nv);
       __syncwarp();                      // phase B of the previous chunk is done with the records
-      float4* q = rec + (i * PPW + g) * 4;
-      q[0] = r.r0; q[1] = r.r1; q[2] = r.r2; q[3] = r.r3;
+      rec[lane] = r.q0;
+      rec[32 + lane] = r.q1;
+      if (NQ > 2) rec[64 + lane] = r.q2;
+      if (NQ > 3) rec[96 + lane] = r.q3;
       // prefetch the next chunk's coefficients
-      const int zn = z0 + LPP + i;
+      const int zn = z0 + LPP + ja;
       l_e = 0.0f; l_a = 0.0f; l_td = 0.0f;
       if (zn < nz) {
         p += (int64_t)LPP * npix;
@@ -126,59 +220,19 @@ transfer_series_kernel(MarchConsts mc, const float* __restrict__ coef, int64_t n
       }
       __syncwarp();
     }
-    // ---- phase B: the LPP lanes of a pixel walk the cells of the chunk
+    // ---- phase B: the LPP lanes of a pixel walk the cells of the chunk, records read one cell ahead
     const int ncz = min(LPP, nz - z0);
-    for (int j = 0; j < ncz; ++j) {
-      const float4* q = rec + (j * PPW + g) * 4;
-      const float4 r0 = q[0], r1 = q[1], r2 = q[2], r3 = q[3];
-      const int kk = __float_as_int(r1.w);
-      const int klo = kk & 0xffff, khi = (int)((unsigned)kk >> 16);
-      const int npass = __reduce_max_sync(0xffffffffu, (khi - klo + LPP) / LPP);   // 0 for an empty window
-      float CG = 0.0f, Pn = 0.0f, Qn = 0.0f, Rn = 0.0f;
-      if (DUST) {
-        const float Gn = G * r3.w;
-        CG = C * G;
-        C = fmaf(C, r3.y, r3.z);
-        Pn = r1.x * Gn; Qn = r1.y * Gn; Rn = r1.z * Gn;
-        G = Gn;
-      }
-      if (npass > 0) {
-        int c = klo + i;
-        float x = fmaf((float)i, r0.w, r0.z);
-        const float step = (float)LPP * r0.w;
-        float* d = sp + (c / LPP) * 32 + (c % LPP);
-#pragma unroll 2
-        for (int ps = 0; ps < npass; ++ps) {
-          const float u = x * x;
-          float pol = fmaf(r3.x, u, r2.w);
-          pol = fmaf(pol, u, r2.z);
-          pol = fmaf(pol, u, r2.y);
-          pol = fmaf(pol, u, r2.x);
-          const float gpr = ex2_approx(-u) * pol;           // dErf / (2 s / sqrt(pi))
-          const float tau_L = r0.x * gpr;
-          const float m = one_minus_exp_neg(tau_L);
-          if (c <= khi) {
-            float Dt = *d;
-            if (DUST) {
-              const float tau_T = tau_L + r0.y;
-              const float rr = rcp_approx(tau_T == 0.0f ? 1.0f : tau_T);
-              const float num = fmaf(m, fmaf(Qn, gpr, Rn), gpr * Pn);
-              Dt = fmaf(-(Dt + CG), m, Dt);
-              Dt = fmaf(rr, num, Dt);
-            } else {
-              Dt = fmaf(r0.y - Dt, m, Dt);
-            }
-            *d = Dt;
-          }
-          x += step; c += LPP; d += 32;
-        }
-      }
-      if (DUST && G > 1.0e18f) {   // rare: fold the accumulated dust attenuation into the stored spectrum
-        const float inv = 1.0f / G;
-        __syncwarp(__activemask());
-        for (int cc = i; cc < nvp; cc += LPP) sp[(cc / LPP) * 32 + i] *= inv;
-        G = 1.0f;
-      }
+    const float4* rq = rec + g;
+    float4 a0 = rq[0], a1 = rq[32], a2 = NQ > 2 ? rq[64] : float4{}, a3 = NQ > 3 ? rq[96] : float4{};
+    for (int j = 0; j < ncz; j += 2) {
+      const int jb = min(j + 1, ncz - 1) * PPW;
+      const float4 b0 = rq[jb], b1 = rq[32 + jb], b2 = NQ > 2 ? rq[64 + jb] : float4{}, b3 = NQ > 3 ? rq[96 + jb] : float4{};
+      cell_step(a0, a1, a2, a3);
+      const int jn = min(j + 2, ncz - 1) * PPW;
+      a0 = rq[jn]; a1 = rq[32 + jn];
+      if (NQ > 2) a2 = rq[64 + jn];
+      if (NQ > 3) a3 = rq[96 + jn];
+      if (j + 1 < ncz) cell_step(b0, b1, b2, b3);
     }
   }
   __syncwarp();
@@ -193,12 +247,13 @@ transfer_series_kernel(MarchConsts mc, const float* __restrict__ coef, int64_t n
   }
 }
 
-template <int LPP>
-inline cudaError_t launch_transfer_series_lpp(const MarchConsts& mc, const float* coef, int64_t ncell, int npix, int nz,
-                                              int nv, bool dust, float* out, float* out_cont, cudaStream_t st) {
+template <int LPP, bool DUST, int DEG>
+inline cudaError_t launch_transfer_series_t(const MarchConsts& mc, const float* coef, int64_t ncell, int npix, int nz,
+                                            int nv, float* out, float* out_cont, cudaStream_t st) {
   constexpr int PPW = 32 / LPP;
+  constexpr int NQ = SeriesLayout<DUST, DEG>::NQ;
   const int nvp = (nv + LPP - 1) / LPP * LPP;
-  const size_t rec_per_warp = (size_t)LPP * PPW * 4 * sizeof(float4);
+  const size_t rec_per_warp = (size_t)NQ * 32 * sizeof(float4);
   const size_t spec_per_warp = (size_t)PPW * nvp * sizeof(float);
   int wpc = 4;
   while (wpc > 1 && wpc * (rec_per_warp + spec_per_warp) > 200 * 1024) wpc >>= 1;
@@ -206,22 +261,21 @@ inline cudaError_t launch_transfer_series_lpp(const MarchConsts& mc, const float
   if (smem > 227 * 1024) return cudaErrorInvalidConfiguration;
   const int ppc = wpc * PPW;
   const unsigned grid = (unsigned)((npix + ppc - 1) / ppc);
-  cudaError_t e;
-  if (dust) {
-    e = cudaFuncSetAttribute(transfer_series_kernel<LPP, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    transfer_series_kernel<LPP, true><<<grid, wpc * 32, smem, st>>>(mc, coef, ncell, npix, nz, nv, nvp, out, out_cont);
-  } else {
-    e = cudaFuncSetAttribute(transfer_series_kernel<LPP, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    transfer_series_kernel<LPP, false><<<grid, wpc * 32, smem, st>>>(mc, coef, ncell, npix, nz, nv, nvp, out, out_cont);
-  }
+  cudaError_t e = cudaFuncSetAttribute(transfer_series_kernel<LPP, DUST, DEG>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       (int)smem);
+  if (e != cudaSuccess) return e;
+  transfer_series_kernel<LPP, DUST, DEG><<<grid, wpc * 32, smem, st>>>(mc, coef, ncell, npix, nz, nv, nvp, out, out_cont);
   return cudaGetLastError();
 }
 
+// s_max: upper bound of dv / b over all cells (dv / microturbulence); selects the polynomial degree.
 inline cudaError_t launch_transfer_series(const MarchConsts& mc, const float* coef, int64_t ncell, int npix, int nz, int nv,
-                                          bool dust, float* out, float* out_cont, cudaStream_t st) {
-  return launch_transfer_series_lpp<8>(mc, coef, ncell, npix, nz, nv, dust, out, out_cont, st);
+                                          bool dust, float s_max, float* out, float* out_cont, cudaStream_t st) {
+  const bool deg3 = s_max <= kSeriesDeg3MaxS;
+  if (dust) return deg3 ? launch_transfer_series_t<8, true, 3>(mc, coef, ncell, npix, nz, nv, out, out_cont, st)
+                        : launch_transfer_series_t<8, true, 4>(mc, coef, ncell, npix, nz, nv, out, out_cont, st);
+  return deg3 ? launch_transfer_series_t<8, false, 3>(mc, coef, ncell, npix, nz, nv, out, out_cont, st)
+              : launch_transfer_series_t<8, false, 4>(mc, coef, ncell, npix, nz, nv, out, out_cont, st);
 }
 
 }  // namespace iris
