@@ -19,13 +19,19 @@
 //    phase A every lane turns the six coefficients of one (cell, pixel) of the chunk into a "march record"
 //    (window, scaled coordinates, polynomial, dust factors) in shared memory; in phase B the LPP lanes of a pixel
 //    walk the LPP cells, reading each record with broadcast LDS.128 one cell ahead of its use.
-// 4. The update loop is branch-free (predicated loads / stores) and two passes are in flight per lane.
+// 4. Packed arithmetic.  A lane updates the two channels of an even-aligned PAIR with the packed fp32 instructions
+//    of sm_100 (fma/mul/add.rn.f32x2 -> FFMA2 / FMUL2 / FADD2): the kernel is bound by instruction issue, not by
+//    the FMA pipe, and a packed instruction does two updates per issue slot (profiles/r01_pipe_microbench.md).
+//    Only the MUFU operations (2 ex2 + 1 rcp per update) and the small-tau select stay scalar.  The window is
+//    widened to pair boundaries; the extra channel lies beyond |x| = X_w where the update is below the window
+//    threshold anyway, so no per-channel predicate is needed.  The loop is branch-free (predicated LDS.64 /
+//    STS.64) and two pair-passes are written stage by stage so that four dependency chains are in flight.
 //
-// Mapping as in transfer_window.cuh: a warp owns 32/LPP adjacent pixels, LPP lanes per pixel; the spectrum
-// Dt[nv] of each pixel lives in shared memory for the whole march, bank-interleaved (channel c of pixel g at
-// word (c / LPP) * 32 + g * LPP + c % LPP: the lanes of a warp always hit 32 distinct banks).  Records are
-// stored quantity-major ([float4 index][record]) so that both the phase-A stores and the phase-B broadcast
-// loads are conflict-free.
+// Mapping: a warp owns 32/LPP adjacent pixels, LPP lanes per pixel; the spectrum Dt[nv] of each pixel lives in
+// shared memory for the whole march.  Pair q = c / 2 of pixel g sits at word (q / LPP) * 64 + g * 2 LPP +
+// (q % LPP) * 2: each half-warp of an LDS.64 / STS.64 hits 32 distinct banks.  Records are stored
+// quantity-major ([float4 index][record]) so that both the phase-A stores and the phase-B broadcast loads are
+// conflict-free.
 #pragma once
 #include "transfer_common.cuh"
 #include "transfer_window.cuh"
@@ -36,11 +42,11 @@ constexpr float kSeriesMaxS = 0.55f;    // largest dv / b the centre expansion i
 constexpr float kSeriesDeg3MaxS = 0.3f; // largest dv / b for the degree-3 polynomial
 
 // March record of one (cell, pixel): NQ float4
-//   q0 = { x0, xs, tdp | sc, bits(klo | W << 16) }   x0: scaled centre of channel klo, xs: scaled channel step,
+//   q0 = { x0, xs, tdp | -sc, bits(qlo | nq << 16) } x0: scaled centre of channel 2 qlo, xs: scaled channel step,
 //                                                    tdp = tau_d log2(e) + 1e-30 (dust), sc = S_L - T_bg (no dust),
-//                                                    W = window width in channels (0: empty)
+//                                                    window = pairs qlo .. qlo + nq - 1 (nq = 0: empty)
 //   q1 = { pA0, pA1, pA2, pA3 }                      polA(u') = As' pol(u'),  As' = a_c (2 s / sqrt(pi)) log2(e)
-//   q2 = { P', Q', R', E_d }                         num' = t P' + m (Q' t + R')   (to be scaled by G')
+//   q2 = { P', -Q', -R', E_d }                       num' = t P' + m (Q' t + R')   (to be scaled by G')
 //   q3 = { S_d m_d, exp(tau_d), pA4, - }             (without dust: pA4 in q2.x)
 template <bool DUST, int DEG>
 struct SeriesLayout {
@@ -57,7 +63,8 @@ __device__ __forceinline__ SeriesRecord make_series_record(float e_c, float a_c,
   SeriesRecord r;
   int klo, khi;
   int W = line_window(e_c, a_c, c_los, s, nv, klo, khi);
-  if (W <= 0) { W = 0; klo = 0; }
+  int qlo = 0, nq = 0;
+  if (W > 0) { qlo = klo >> 1; nq = (khi >> 1) - qlo + 1; }
   // |a_c| is kept above 1e-10 e_c: the source function e_c / a_c stays finite where the opacity crosses zero
   // (changes tau_L by < 1e-10 e_c, i.e. < 1e-7 for a 1000 K line)
   const float a_min = fmaxf(1.0e-10f * e_c, 1.0e-30f);
@@ -66,9 +73,9 @@ __device__ __forceinline__ SeriesRecord make_series_record(float e_c, float a_c,
   const float As = a_safe * sp, Es = e_c * sp;
   const float Asp = As * LOG2E;
   const float xs = 1.2011224087864498f * s;                 // s sqrt(log2 e)
-  r.q0.x = ((float)klo + 0.5f - c_los) * xs;
+  r.q0.x = ((float)(2 * qlo) + 0.5f - c_los) * xs;
   r.q0.y = xs;
-  r.q0.w = __int_as_float(klo | (W << 16));
+  r.q0.w = __int_as_float(qlo | (nq << 16));
   // polynomial in u = x^2, rescaled to u' = u log2(e) (p'_k = p_k ln(2)^k) and multiplied by As'
   const float s2 = s * s, s4 = s2 * s2, s6 = s4 * s2, s8 = s4 * s4;
   const float p0 = 1.0f - s2 * (1.0f / 12.0f) + s4 * (1.0f / 160.0f) - s6 * (1.0f / 2688.0f) + s8 * (1.0f / 55296.0f);
@@ -86,43 +93,137 @@ __device__ __forceinline__ SeriesRecord make_series_record(float e_c, float a_c,
     const float iA = LOG2E * rcp_approx(Asp);
     r.q0.z = fmaf(tau_d, LOG2E, 1.0e-30f);
     r.q2.x = m_d * fmaf(-S_d, As, Es) * iA;
-    r.q2.y = E_d * Es * iA;
-    r.q2.z = E_d * S_d * tau_d * LOG2E;
+    r.q2.y = -E_d * Es * iA;
+    r.q2.z = -E_d * S_d * tau_d * LOG2E;
     r.q2.w = E_d;
     r.q3.x = S_d * m_d;
     r.q3.y = ex2_approx(tau_d * LOG2E);
   } else {
-    r.q0.z = Es * rcp_approx(As) - T_bg;      // sc = S_L - C, C = T_bg throughout
+    r.q0.z = T_bg - Es * rcp_approx(As);      // -sc = C - S_L, C = T_bg throughout
     r.q2 = make_float4(r.q3.z, 0.0f, 0.0f, 1.0f);   // pA4 travels in q2.x when there is no dust (NQ = 3)
     r.q3.x = 0.0f; r.q3.y = 1.0f;
   }
   return r;
 }
 
-// One update of one channel: Dt -> Dt'.  x: scaled channel centre.
-template <bool DUST, int DEG>
-__device__ __forceinline__ float series_update(float Dt, float x, const float4& q0, const float4& q1, float pA4,
-                                               float CG, float Pn, float Qn, float Rn) {
+// ---- packed fp32 pairs (sm_100: FFMA2 / FMUL2 / FADD2), carried in 64-bit registers
+typedef unsigned long long f32x2;
+
+__device__ __forceinline__ f32x2 pk(float lo, float hi) {
+  f32x2 r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ f32x2 pk1(float v) { return pk(v, v); }
+__device__ __forceinline__ void upk(f32x2 v, float& lo, float& hi) {
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) {
+  f32x2 r;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+  return r;
+}
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) {
+  f32x2 r;
+  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+  return r;
+}
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) {
+  f32x2 r;
+  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+  return r;
+}
+
+// Per-cell operands of the update, duplicated into both halves of a packed register.
+struct SeriesCellOps {
+  f32x2 p0, p1, p2, p3, p4;     // polA
+  f32x2 tdp_or_nsc;             // dust: tau_d log2(e) + 1e-30;  no dust: -(S_L - T_bg)
+  f32x2 CG, Pn, nQn, nRn;       // dust only (scaled by G')
+};
+
+// P consecutive pair-passes of one lane (pairs q, q + LPP, ...), written stage by stage over the 2 P channels so
+// that 2 P independent dependency chains are in flight (the SM issues in order: a lane-serial update would leave
+// the issue slot idle for the latency of every MUFU / FMA of the chain).  d: the lane's words of pair q; pairs at
+// or beyond qend are computed but neither loaded nor stored.  xx: scaled centres of the two channels of pair q.
+template <bool DUST, int DEG, int LPP, int P>
+__device__ __forceinline__ void series_passes(float* d, int q, int qend, f32x2 xx, f32x2 step2, const SeriesCellOps& o) {
   constexpr float L1 = 0.6931471805599453f, L2 = L1 * L1, L3 = L2 * L1, L4 = L2 * L2;
-  const float u = x * x;
-  float pol;
-  if (DEG > 3) { pol = fmaf(pA4, u, q1.w); pol = fmaf(pol, u, q1.z); }
-  else pol = fmaf(q1.w, u, q1.z);
-  pol = fmaf(pol, u, q1.y);
-  pol = fmaf(pol, u, q1.x);
-  const float t = ex2_approx(-u) * pol;                 // tau_L log2(e)
-  const float big = 1.0f - ex2_approx(-t);
-  float q = fmaf(t, -L4 / 24.0f, L3 / 6.0f);
-  q = fmaf(q, t, -L2 / 2.0f);
-  q = fmaf(q, t, L1);
-  const float m = fabsf(t) < 0.115f ? q * t : big;      // 1 - exp(-tau_L); Taylor below tau_L = 0.08
-  if (DUST) {
-    const float rr = rcp_approx(t + q0.z);
-    const float num = fmaf(m, fmaf(Qn, t, Rn), t * Pn);
-    Dt = fmaf(-(Dt + CG), m, Dt);
-    return fmaf(rr, num, Dt);
+  const f32x2 ONE = pk1(1.0f), NEG1 = pk1(-1.0f);
+  const f32x2 C4 = pk1(L4 / 24.0f), C3 = pk1(-L3 / 6.0f), C2 = pk1(L2 / 2.0f), C1 = pk1(-L1);   // -(1 - 2^-t) / t
+  bool ok[P];
+  f32x2 Dt[P], u[P], pol[P], t[P], mn[P], qq[P];
+#pragma unroll
+  for (int k = 0; k < P; ++k) {
+    ok[k] = q + k * LPP < qend;
+    float2 v = make_float2(0.0f, 0.0f);
+    if (ok[k]) v = *reinterpret_cast<const float2*>(d + 64 * k);
+    Dt[k] = pk(v.x, v.y);
+    u[k] = mul2(xx, xx);
+    xx = add2(xx, step2);
   }
-  return fmaf(q0.z - Dt, m, Dt);
+#pragma unroll
+  for (int k = 0; k < P; ++k) pol[k] = DEG > 3 ? fma2(fma2(o.p4, u[k], o.p3), u[k], o.p2) : fma2(o.p3, u[k], o.p2);
+#pragma unroll
+  for (int k = 0; k < P; ++k) pol[k] = fma2(pol[k], u[k], o.p1);
+#pragma unroll
+  for (int k = 0; k < P; ++k) pol[k] = fma2(pol[k], u[k], o.p0);
+#pragma unroll
+  for (int k = 0; k < P; ++k) {
+    float u0, u1;
+    upk(u[k], u0, u1);
+    t[k] = mul2(pk(ex2_approx(-u0), ex2_approx(-u1)), pol[k]);      // tau_L log2(e)
+  }
+  float t0[P], t1[P], f0[P], f1[P];
+#pragma unroll
+  for (int k = 0; k < P; ++k) {
+    upk(t[k], t0[k], t1[k]);
+    f0[k] = ex2_approx(-t0[k]);
+    f1[k] = ex2_approx(-t1[k]);
+    qq[k] = fma2(t[k], C4, C3);
+  }
+#pragma unroll
+  for (int k = 0; k < P; ++k) qq[k] = fma2(qq[k], t[k], C2);
+#pragma unroll
+  for (int k = 0; k < P; ++k) qq[k] = fma2(qq[k], t[k], C1);
+#pragma unroll
+  for (int k = 0; k < P; ++k) {
+    // mn = -(1 - exp(-tau_L)) = 2^-t - 1; Taylor below tau_L = 0.08
+    const f32x2 sm = mul2(qq[k], t[k]);
+    const f32x2 bg = add2(pk(f0[k], f1[k]), NEG1);
+    float s0, s1, b0, b1;
+    upk(sm, s0, s1);
+    upk(bg, b0, b1);
+    mn[k] = pk(fabsf(t0[k]) < 0.115f ? s0 : b0, fabsf(t1[k]) < 0.115f ? s1 : b1);
+  }
+  if (DUST) {
+    f32x2 rr[P], num[P];
+#pragma unroll
+    for (int k = 0; k < P; ++k) {
+      const f32x2 tt = add2(t[k], o.tdp_or_nsc);
+      float a0, a1;
+      upk(tt, a0, a1);
+      rr[k] = pk(rcp_approx(a0), rcp_approx(a1));
+      num[k] = fma2(o.nQn, t[k], o.nRn);                       // -(Q t + R)
+    }
+#pragma unroll
+    for (int k = 0; k < P; ++k) {
+      num[k] = fma2(mn[k], num[k], mul2(t[k], o.Pn));           // t P + m (Q t + R)
+      Dt[k] = fma2(add2(Dt[k], o.CG), mn[k], Dt[k]);            // Dt - (Dt + C G) m
+    }
+#pragma unroll
+    for (int k = 0; k < P; ++k) Dt[k] = fma2(rr[k], num[k], Dt[k]);
+  } else {
+#pragma unroll
+    for (int k = 0; k < P; ++k) Dt[k] = fma2(add2(Dt[k], o.tdp_or_nsc), mn[k], Dt[k]);   // Dt + (sc - Dt) m
+  }
+  (void)ONE;
+#pragma unroll
+  for (int k = 0; k < P; ++k)
+    if (ok[k]) {
+      float2 v;
+      upk(Dt[k], v.x, v.y);
+      *reinterpret_cast<float2*>(d + 64 * k) = v;
+    }
 }
 
 template <int LPP, bool DUST, int DEG>
@@ -132,16 +233,18 @@ transfer_series_kernel(MarchConsts mc, const float* __restrict__ coef, int64_t n
   extern __shared__ float4 smem4[];
   constexpr int PPW = 32 / LPP;
   constexpr int NQ = SeriesLayout<DUST, DEG>::NQ;
+  constexpr int ROW = 2 * 32;                   // words per row of LPP pairs x PPW pixels
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, wpc = blockDim.x >> 5;
   const int g = lane / LPP, i = lane % LPP;
   const int pix0 = (blockIdx.x * wpc + warp) * PPW;
   const int pix = pix0 + g;
   const bool valid = pix < npix;
-  // shared memory: records [wpc][NQ][32], then spectra [wpc][nvp / LPP rows][32]
+  const int npair = nvp / 2;                    // nvp is a multiple of 2 LPP
+  // shared memory: records [wpc][NQ][32], then spectra [wpc][npair / LPP rows][ROW]
   float4* rec = smem4 + (size_t)warp * (NQ * 32);
   float* spec = reinterpret_cast<float*>(smem4 + (size_t)wpc * (NQ * 32));
-  float* sp = spec + (size_t)warp * nvp * PPW + g * LPP;
-  for (int c = i; c < nvp; c += LPP) sp[(c / LPP) * 32 + i] = 0.0f;
+  float* sp = spec + (size_t)warp * nvp * PPW + g * (2 * LPP);      // pair q of this pixel: sp[(q / LPP) * ROW + (q % LPP) * 2]
+  for (int q = i; q < npair; q += LPP) *reinterpret_cast<float2*>(sp + (q / LPP) * ROW + i * 2) = make_float2(0.0f, 0.0f);
 
   float C = mc.T_bg;      // continuum before the current cell
   float G = 1.0f;         // exp(dust optical depth accumulated so far), since the last rescale
@@ -158,8 +261,8 @@ transfer_series_kernel(MarchConsts mc, const float* __restrict__ coef, int64_t n
   // one cell of phase B for this lane's pixel, given the cell's record in registers
   auto cell_step = [&](const float4& q0, const float4& q1, const float4& q2, const float4& q3) {
     const int kk = __float_as_int(q0.w);
-    const int klo = kk & 0xffff, W = (int)((unsigned)kk >> 16);
-    const int npass = __reduce_max_sync(0xffffffffu, (W + LPP - 1) / LPP);   // 0 for an empty window
+    const int qlo = kk & 0xffff, nq = (int)((unsigned)kk >> 16);
+    const int npass = __reduce_max_sync(0xffffffffu, (nq + LPP - 1) / LPP);   // 0 for an empty window
     float CG = 0.0f, Pn = 0.0f, Qn = 0.0f, Rn = 0.0f;
     if (DUST) {
       const float Gn = G * q3.y;
@@ -168,35 +271,34 @@ transfer_series_kernel(MarchConsts mc, const float* __restrict__ coef, int64_t n
       Pn = q2.x * Gn; Qn = q2.y * Gn; Rn = q2.z * Gn;
       G = Gn;
     }
-    const float pA4 = DUST ? q3.z : q2.x;
     if (npass > 0) {
-      int c = klo + i;
-      const int cend = klo + W;                    // one past the last channel of the window
-      float x = fmaf((float)i, q0.y, q0.x);
-      const float step = (float)LPP * q0.y;
-      float* d = sp + (c / LPP) * 32 + (c % LPP);
-      int ps = 0;
-      for (; ps + 2 <= npass; ps += 2) {
-        const bool okA = c < cend, okB = c + LPP < cend;
-        float DA = okA ? d[0] : 0.0f;
-        float DB = okB ? d[32] : 0.0f;
-        DA = series_update<DUST, DEG>(DA, x, q0, q1, pA4, CG, Pn, Qn, Rn);
-        DB = series_update<DUST, DEG>(DB, x + step, q0, q1, pA4, CG, Pn, Qn, Rn);
-        if (okA) d[0] = DA;
-        if (okB) d[32] = DB;
-        x = fmaf(2.0f, step, x); c += 2 * LPP; d += 64;
+      SeriesCellOps o;
+      o.p0 = pk1(q1.x); o.p1 = pk1(q1.y); o.p2 = pk1(q1.z); o.p3 = pk1(q1.w);
+      o.p4 = pk1(DUST ? q3.z : q2.x);
+      o.tdp_or_nsc = pk1(q0.z);
+      o.CG = pk1(CG); o.Pn = pk1(Pn); o.nQn = pk1(Qn); o.nRn = pk1(Rn);
+      int q = qlo + i;
+      const int qend = qlo + nq;                   // one past the last pair of the window
+      const float x = fmaf((float)(2 * i), q0.y, q0.x);
+      f32x2 xx = pk(x, x + q0.y);
+      const f32x2 step2 = pk1((float)(2 * LPP) * q0.y);
+      float* d = sp + (q / LPP) * ROW + (q % LPP) * 2;
+      int rem = npass;
+      while (rem >= 2) {
+        series_passes<DUST, DEG, LPP, 2>(d, q, qend, xx, step2, o);
+        xx = add2(xx, add2(step2, step2)); q += 2 * LPP; d += 2 * ROW; rem -= 2;
       }
-      if (ps < npass) {
-        const bool okA = c < cend;
-        float DA = okA ? d[0] : 0.0f;
-        DA = series_update<DUST, DEG>(DA, x, q0, q1, pA4, CG, Pn, Qn, Rn);
-        if (okA) d[0] = DA;
-      }
+      if (rem == 1) series_passes<DUST, DEG, LPP, 1>(d, q, qend, xx, step2, o);
     }
     if (DUST && G > 1.0e18f) {   // rare: fold the accumulated dust attenuation into the stored spectrum
       const float inv = 1.0f / G;
       __syncwarp(__activemask());
-      for (int cc = i; cc < nvp; cc += LPP) sp[(cc / LPP) * 32 + i] *= inv;
+      for (int qq = i; qq < npair; qq += LPP) {
+        float2* w = reinterpret_cast<float2*>(sp + (qq / LPP) * ROW + i * 2);
+        float2 v = *w;
+        v.x *= inv; v.y *= inv;
+        *w = v;
+      }
       G = 1.0f;
     }
   };
@@ -241,7 +343,18 @@ transfer_series_kernel(MarchConsts mc, const float* __restrict__ coef, int64_t n
   if (valid) {
     if (out != nullptr) {
       float* o = out + (int64_t)pix * nv;
-      for (int c = i; c < nv; c += LPP) o[c] = convert_out(sp[(c / LPP) * 32 + i] * invG, C, mc);
+      const bool al = ((((int64_t)pix * nv) & 1) == 0);      // float2 stores need an even element offset
+      for (int q = i; 2 * q < nv; q += LPP) {
+        const float2 v = *reinterpret_cast<const float2*>(sp + (q / LPP) * ROW + i * 2);
+        const float r0 = convert_out(v.x * invG, C, mc);
+        if (2 * q + 1 < nv) {
+          const float r1 = convert_out(v.y * invG, C, mc);
+          if (al) *reinterpret_cast<float2*>(o + 2 * q) = make_float2(r0, r1);
+          else { o[2 * q] = r0; o[2 * q + 1] = r1; }
+        } else {
+          o[2 * q] = r0;
+        }
+      }
     }
     if (out_cont != nullptr && i == 0) out_cont[pix] = C * mc.inv_KRJ;
   }
@@ -252,7 +365,7 @@ inline cudaError_t launch_transfer_series_t(const MarchConsts& mc, const float* 
                                             int nv, float* out, float* out_cont, cudaStream_t st) {
   constexpr int PPW = 32 / LPP;
   constexpr int NQ = SeriesLayout<DUST, DEG>::NQ;
-  const int nvp = (nv + LPP - 1) / LPP * LPP;
+  const int nvp = (nv + 2 * LPP - 1) / (2 * LPP) * (2 * LPP);      // whole rows of LPP channel pairs
   const size_t rec_per_warp = (size_t)NQ * 32 * sizeof(float4);
   const size_t spec_per_warp = (size_t)PPW * nvp * sizeof(float);
   int wpc = 4;
