@@ -30,10 +30,21 @@ from iris_inputs import make_fields, make_workload  # noqa: E402
 METRIC = "los_transfer_cell_channel_updates_per_s"
 UNIT = "updates/s"
 
-# Algorithmic instruction counts (thread-level FP32/ALU/SFU instructions the method needs)
-INSTR_PER_UPDATE = {True: 44, False: 31}        # keyed by dust_on
-INSTR_PER_PIXEL_CELL = {True: 37, False: 28}
-SM_COUNT, LANES_PER_SM_CLK = 148, 128           # 4 sub-partitions x 32 lanes, one warp instruction per clock each
+# Algorithmic work of the LOS transfer kernel.  Per evaluated (cell, channel) update the
+# recurrence needs 3 SFU operations (2^(-x^2) of the profile, 2^(-t) of 1 - exp(-tau_L), 1 / tau_T) -- 2 without dust --
+# and 17 (13) FP32 multiply-adds; per (pixel, cell) it needs 5 SFU operations (window: log, sqrt, 1 / s; dust:
+# exp(-tau_d); source function: 1 / a_c) and about 60 FP32 operations.  Peaks measured on this pool's B200
+# (profiles/r01_pipe_microbench.md): MUFU 0.50 warp instructions / clk / SM = 16 lanes, FFMA 3.90 = 124.9 lanes.
+SFU_PER_UPDATE = {True: 3, False: 2}            # keyed by dust_on
+FP32_PER_UPDATE = {True: 17, False: 13}
+SFU_PER_PIXEL_CELL = {True: 5, False: 4}
+FP32_PER_PIXEL_CELL = 60
+SM_COUNT, SFU_LANES_PER_SM_CLK, FP32_LANES_PER_SM_CLK = 148, 16.0, 124.9
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum of one launch from the committed `ncu --set full` captures
+# (profiles/r01_v3.md), keyed by (workload, kernel)
+NCU_TRAFFIC_BYTES = {("large", "transfer_series_kernel"): 4271062000}
 
 
 def env_rank():
@@ -266,27 +277,36 @@ def bench_workload(torch, dist, name, algo, steps, warmup, rank, peaks, want_e2e
 
     res = dict(cfg=cfg, fields=fields, value=value, ms=ms_max, ms_per_step=ms_max / steps, launches=launches, clocks=clocks,
                stages={k: {"ms_per_step": v[0] / steps, "launches_per_step": v[1] / steps} for k, v in prof.items() if v[1]})
-    # roofline of the dominant kernel (LOS transfer)
+    # roofline of the dominant kernel (LOS transfer): the slower of HBM bytes, SFU operations and FP32 operations
     t_k3 = prof["transfer"][0] / max(prof["transfer"][1], 1) * 1e-3          # seconds per launch
     ncell = cfg.nx * cfg.ny * cfg.nz
     win_updates = it.transfer_work()
-    n_upd = updates if algo == "dense" else win_updates
-    instr = n_upd * INSTR_PER_UPDATE[cfg.dust_on] + ncell * INSTR_PER_PIXEL_CELL[cfg.dust_on]
-    peak = SM_COUNT * LANES_PER_SM_CLK * peaks["sm_max_mhz"] * 1e6
+    dense_kernel = it.transfer_kernel() == "transfer_dense_kernel"
+    n_upd = updates if dense_kernel else win_updates
+    clk = peaks["sm_max_mhz"] * 1e6
+    sfu_ops = n_upd * SFU_PER_UPDATE[cfg.dust_on] + ncell * SFU_PER_PIXEL_CELL[cfg.dust_on]
+    fp32_ops = n_upd * FP32_PER_UPDATE[cfg.dust_on] + ncell * FP32_PER_PIXEL_CELL
+    sfu_peak = SM_COUNT * SFU_LANES_PER_SM_CLK * clk
+    fp32_peak = SM_COUNT * FP32_LANES_PER_SM_CLK * clk
     alg_bytes = 24 * ncell + 4 * cfg.nx * cfg.ny * cfg.nv
+    t_sfu, t_fp32, t_hbm = sfu_ops / sfu_peak, fp32_ops / fp32_peak, alg_bytes / (peaks["hbm_gbs"] * 1e9)
     res["roofline"] = {
-        "bound": "alu", "kernel": "transfer_%s_kernel" % algo, "algorithm": algo,
-        "achieved": instr / t_k3 / 1e12, "peak": peak / 1e12, "unit": "Tinstr/s (thread-level FP32/SFU/ALU instructions)",
-        "frac": instr / t_k3 / peak, "traffic": None,
-        "peak_source": "148 SMs x 128 lanes/clk x %.0f MHz max SM clock (MEASURED_PEAKS.json, %s)" % (peaks["sm_max_mhz"], peaks["source"]),
+        "bound": "alu", "pipe": "sfu (MUFU.EX2 / MUFU.RCP)", "kernel": it.transfer_kernel(), "algorithm": algo,
+        "achieved": sfu_ops / t_k3 / 1e12, "peak": sfu_peak / 1e12, "unit": "Tops/s (SFU lane operations)",
+        "frac": t_sfu / t_k3, "traffic": NCU_TRAFFIC_BYTES.get((cfg.name, it.transfer_kernel())),
+        "peak_source": "148 SMs x 16 SFU lanes/clk (measured MUFU issue rate, profiles/r01_pipe_microbench.md) x %.0f MHz "
+                       "max SM clock (MEASURED_PEAKS.json, %s)" % (peaks["sm_max_mhz"], peaks["source"]),
         "ms_per_launch": t_k3 * 1e3, "updates_evaluated": n_upd, "updates_nominal": updates,
-        "instr_per_update": INSTR_PER_UPDATE[cfg.dust_on], "instr_per_pixel_cell": INSTR_PER_PIXEL_CELL[cfg.dust_on],
+        "sfu_per_update": SFU_PER_UPDATE[cfg.dust_on], "sfu_per_pixel_cell": SFU_PER_PIXEL_CELL[cfg.dust_on],
+        "floors_ms": {"sfu": t_sfu * 1e3, "fp32": t_fp32 * 1e3, "hbm": t_hbm * 1e3},
         "nominal_updates_per_s": updates / t_k3,
+        "fp32": {"ops": fp32_ops, "achieved_Tops_s": fp32_ops / t_k3 / 1e12, "peak_Tops_s": fp32_peak / 1e12,
+                 "frac": t_fp32 / t_k3},
         "hbm": {"algorithmic_bytes": alg_bytes, "achieved_gbs": alg_bytes / t_k3 / 1e9, "peak_gbs": peaks["hbm_gbs"],
-                "frac": alg_bytes / t_k3 / 1e9 / peaks["hbm_gbs"]},
+                "frac": t_hbm / t_k3},
     }
     if clocks and clocks.get("sm_mhz"):
-        res["roofline"]["frac_at_measured_clock"] = instr / t_k3 / (SM_COUNT * LANES_PER_SM_CLK * clocks["sm_mhz"] * 1e6)
+        res["roofline"]["frac_at_measured_clock"] = res["roofline"]["frac"] * peaks["sm_max_mhz"] / clocks["sm_mhz"]
 
     if want_dense_probe and algo != "dense":
         itd = IrisSO(cfg, transfer_algo=ALGO_DENSE)
@@ -298,9 +318,9 @@ def bench_workload(torch, dist, name, algo, steps, warmup, rank, peaks, want_e2e
             itd.observe(*d, cube=cube, beam=False, noise=False)
         pd = itd.profile_read()
         t_d = pd["transfer"][0] / pd["transfer"][1] * 1e-3
-        instr_d = updates * INSTR_PER_UPDATE[cfg.dust_on] + ncell * INSTR_PER_PIXEL_CELL[cfg.dust_on]
-        res["dense_probe"] = {"kernel": "transfer_dense_kernel", "ms_per_launch": t_d * 1e3, "updates_per_s": updates / t_d,
-                              "achieved_Tinstr_s": instr_d / t_d / 1e12, "frac": instr_d / t_d / peak}
+        res["dense_probe"] = {"kernel": "transfer_dense_kernel", "ms_per_launch": t_d * 1e3, "nominal_updates_per_s": updates / t_d,
+                              "note": "north_star's literal kernel (register-resident channel blocks, erfc edges); it skips "
+                                      "16-channel blocks beyond the erfc range, so no roofline fraction is quoted for it"}
         itd.close()
 
     if want_e2e:
