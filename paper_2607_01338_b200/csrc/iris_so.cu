@@ -355,15 +355,12 @@ iris_so_status run_beam(iris_so_ctx* ctx, const float* in, float* out, float* tm
   ProfScope prof(ctx, IRIS_SO_STAGE_BEAM, st);
   iris::NoiseConsts off = ctx->nc; off.on = 0;
   iris::NoiseConsts nz2 = ctx->nc; nz2.on = noise ? ctx->nc.on : 0;
-  dim3 block(32, 8);
   // pass 1 along x: a = x (stride nv), b = y (stride nx*nv)
-  dim3 g1((c.nv + 31) / 32, (c.nx + iris::kBeamTA - 1) / iris::kBeamTA, c.ny);
-  iris::beam_pass_kernel<<<g1, block, 0, st>>>(ctx->bc, off, in, tmp, c.nx, c.ny, c.nv, (int64_t)c.nv, (int64_t)c.nx * c.nv);
-  IRIS_CHECK_LAUNCH(ctx, "beam_pass_kernel(x)");
+  iris::launch_beam_pass(ctx->bc, off, in, tmp, c.nx, c.ny, c.nv, (int64_t)c.nv, (int64_t)c.nx * c.nv, st);
+  IRIS_CHECK_LAUNCH(ctx, "beam pass (x)");
   // pass 2 along y: a = y (stride nx*nv), b = x (stride nv)
-  dim3 g2((c.nv + 31) / 32, (c.ny + iris::kBeamTA - 1) / iris::kBeamTA, c.nx);
-  iris::beam_pass_kernel<<<g2, block, 0, st>>>(ctx->bc, nz2, tmp, out, c.ny, c.nx, c.nv, (int64_t)c.nx * c.nv, (int64_t)c.nv);
-  IRIS_CHECK_LAUNCH(ctx, "beam_pass_kernel(y)");
+  iris::launch_beam_pass(ctx->bc, nz2, tmp, out, c.ny, c.nx, c.nv, (int64_t)c.nx * c.nv, (int64_t)c.nv, st);
+  IRIS_CHECK_LAUNCH(ctx, "beam pass (y)");
   return IRIS_SO_OK;
 }
 

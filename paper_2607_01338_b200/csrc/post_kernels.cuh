@@ -64,6 +64,85 @@ beam_pass_kernel(BeamConsts bc, NoiseConsts nc, const float* __restrict__ in, fl
   }
 }
 
+// Register formulation of the same pass (even nv, R <= 16): a thread owns a PAIR of channels and TA consecutive
+// positions along a; it streams the TA + 2 RB input rows once (8-byte loads, a warp reads 256 contiguous bytes per
+// row) and scatters each row into the TA packed accumulators it contributes to (fma.rn.f32x2), so every loaded
+// value feeds up to 2 RB + 1 outputs of the same thread and no shared memory is involved: 2 RB + 1 packed FMAs + 2
+// loads + 1 store per pair of outputs, against 13 LDS + 13 FFMA + addressing per single output of the tiled kernel.
+// RB is the compile-time radius class (taps beyond the configured radius are zero).
+template <int RB>
+struct BeamTaps { float w[2 * RB + 1]; };
+
+template <int RB, int TA>
+__global__ void __launch_bounds__(128)
+beam_pass_reg_kernel(BeamTaps<RB> taps, NoiseConsts nc, const float* __restrict__ in, float* __restrict__ out, int na,
+                     int nb, int nv, int64_t stride_a, int64_t stride_b) {
+  const int vp = blockIdx.x * 32 + threadIdx.x;            // channel pair
+  const int a0 = (blockIdx.y * blockDim.y + threadIdx.y) * TA;
+  const int b = blockIdx.z;
+  if (2 * vp >= nv || a0 >= na) return;
+  const int64_t base = (int64_t)b * stride_b + 2 * vp;
+  unsigned long long acc[TA];
+#pragma unroll
+  for (int i = 0; i < TA; ++i) acc[i] = 0ull;
+#pragma unroll
+  for (int r = 0; r < TA + 2 * RB; ++r) {
+    const int a = a0 - RB + r;
+    float2 v = make_float2(0.0f, 0.0f);
+    if (a >= 0 && a < na) v = *reinterpret_cast<const float2*>(in + base + (int64_t)a * stride_a);
+    unsigned long long vv;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(vv) : "f"(v.x), "f"(v.y));
+#pragma unroll
+    for (int i = 0; i < TA; ++i) {
+      const int k = r - i;                                  // tap index of input row r for output i
+      if (k >= 0 && k <= 2 * RB) {
+        unsigned long long ww;
+        asm("mov.b64 %0, {%1, %1};" : "=l"(ww) : "f"(taps.w[k]));
+        asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc[i]) : "l"(ww), "l"(vv));
+      }
+    }
+  }
+#pragma unroll
+  for (int i = 0; i < TA; ++i) {
+    const int a = a0 + i;
+    if (a < na) {
+      float2 o;
+      asm("mov.b64 {%0, %1}, %2;" : "=f"(o.x), "=f"(o.y) : "l"(acc[i]));
+      const int64_t idx = base + (int64_t)a * stride_a;
+      if (nc.on) {
+        o.x += fmaf(nc.sigma, voxel_normal(nc, (uint64_t)idx), nc.mu);
+        o.y += fmaf(nc.sigma, voxel_normal(nc, (uint64_t)idx + 1), nc.mu);
+      }
+      *reinterpret_cast<float2*>(out + idx) = o;
+    }
+  }
+}
+
+template <int RB>
+inline void launch_beam_pass_reg(const BeamConsts& bc, const NoiseConsts& nc, const float* in, float* out, int na, int nb,
+                                 int nv, int64_t stride_a, int64_t stride_b, cudaStream_t st) {
+  constexpr int TA = 16;
+  BeamTaps<RB> taps;
+  for (int k = 0; k <= 2 * RB; ++k) {
+    const int d = k - (RB - bc.R);
+    taps.w[k] = (d >= 0 && d <= 2 * bc.R) ? bc.g[d] : 0.0f;
+  }
+  const int tiles = (na + TA - 1) / TA;
+  dim3 block(32, 4), grid((nv / 2 + 31) / 32, (tiles + 3) / 4, nb);
+  beam_pass_reg_kernel<RB, TA><<<grid, block, 0, st>>>(taps, nc, in, out, na, nb, nv, stride_a, stride_b);
+}
+
+// One pass with the best kernel for (R, nv): register formulation when nv is even and R <= 16, tiled otherwise.
+inline void launch_beam_pass(const BeamConsts& bc, const NoiseConsts& nc, const float* in, float* out, int na, int nb,
+                             int nv, int64_t stride_a, int64_t stride_b, cudaStream_t st) {
+  const bool aligned = (nv % 2 == 0) && ((reinterpret_cast<uintptr_t>(in) | reinterpret_cast<uintptr_t>(out)) % 8 == 0);
+  if (aligned && bc.R <= 4) return launch_beam_pass_reg<4>(bc, nc, in, out, na, nb, nv, stride_a, stride_b, st);
+  if (aligned && bc.R <= 8) return launch_beam_pass_reg<8>(bc, nc, in, out, na, nb, nv, stride_a, stride_b, st);
+  if (aligned && bc.R <= 16) return launch_beam_pass_reg<16>(bc, nc, in, out, na, nb, nv, stride_a, stride_b, st);
+  dim3 block(32, 8), grid((nv + 31) / 32, (na + kBeamTA - 1) / kBeamTA, nb);
+  beam_pass_kernel<<<grid, block, 0, st>>>(bc, nc, in, out, na, nb, nv, stride_a, stride_b);
+}
+
 // K7 alone (no beam configured): in-place.
 __global__ void __launch_bounds__(256) noise_kernel(NoiseConsts nc, float* __restrict__ cube, int64_t nvox) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;

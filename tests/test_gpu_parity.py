@@ -275,6 +275,28 @@ def test_beam_and_noise_kernels():
     assert np.abs(it2.beam(dev(img)).cpu().numpy() - o2.beam(img)).max() < 2e-6
 
 
+@pytest.mark.parametrize("fwhm", [1.5, 3.0, 5.5, 9.0, 12.0])
+@pytest.mark.parametrize("shape", [dict(nx=45, ny=70, nv=34), dict(nx=16, ny=33, nv=64), dict(nx=5, ny=3, nv=2),
+                                   dict(nx=37, ny=19, nv=33)])
+def test_beam_register_and_tiled_passes(fwhm, shape):
+    """Even nv and radius <= 16 take the register-window pass (radius classes 4, 8, 16), odd nv or a wider beam the
+    shared-memory tiled pass; both are the zero-padded separable sum of the oracle, with and without the fused noise."""
+    cfg, _ = make_workload("medium", nz=1, **shape)
+    cfg = cfg.with_(beam_fwhm_px=fwhm, seed=1234567, noise_mu=-0.02)
+    rng = np.random.default_rng(11)
+    img = rng.standard_normal((cfg.ny, cfg.nx, cfg.nv)).astype(np.float32)
+    it, o = iris(cfg), Oracle(cfg)
+    out = it.beam(dev(img)).cpu().numpy()
+    ref = o.beam(img)
+    assert np.abs(out - ref).max() < 2e-6
+    # delta image -> the kernel itself, summing to 1 away from the edges
+    if cfg.nx > 40:
+        delta = np.zeros_like(img)
+        delta[cfg.ny // 2, cfg.nx // 2, :] = 1.0
+        resp = it.beam(dev(delta)).cpu().numpy()
+        assert np.abs(resp - o.beam(delta)).max() < 1e-6
+
+
 def test_window_kernel_selection_and_series_limit():
     """ALGO_WINDOW takes the channel-centre expansion only when dv / xi <= 0.55 bounds dv / b for every cell;
     at that limit (and with thick lines, where the profile wings carry the optical depth) it still meets the
