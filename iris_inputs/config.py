@@ -49,6 +49,10 @@ class ObsConfig:
     noise_sigma: float = 0.0      # 0 (with mu = 0) = no noise
     noise_gamma_mode: int = 0     # 0: gamma = 1; 1: one gamma ~ U[0,1) per cube (Eq. 4.12.1)
     seed: int = 0
+    # transfer / integration modes (PAPER.md sections 4.4 - 4.8); all 0 = the hot path
+    transfer_mode: int = 0        # 0 optically thick, 1 selectively thin, 2 optically thin
+    integration: int = 0          # 0 formal, 1 smooth (TR + BDF2; Simpson in thin mode)
+    subsample: int = 0            # thick mode: 0 = channel-integrated profile; odd f = fine grid + Simpson (Eq. 4.5.1)
     # free-form label, ignored by both implementations
     name: str = field(default="", compare=False)
 

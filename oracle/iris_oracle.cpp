@@ -50,6 +50,11 @@ struct orc_config {
   double beam_fwhm_px, noise_mu, noise_sigma;
   int32_t noise_gamma_mode;
   uint64_t seed;
+  // transfer / integration modes of sections 4.4 - 4.8; all 0 = the hot path (reading R1)
+  int32_t transfer_mode;   // 0 optically thick (4.5), 1 selectively thin (4.6), 2 optically thin (4.7)
+  int32_t integration;     // 0 formal, 1 smooth (4.8: TR first step + BDF2; 4.7.7: Simpson in thin mode)
+  int32_t subsample;       // thick mode only: 0 = channel-integrated profile (R1); odd f >= 1 = fine velocity
+                           // grid with f added midpoints per channel + Simpson over frequency (4.5, Eq. 4.5.1)
 };
 
 // Planck function B_nu(T), Eq. 3.2.1 = Eq. 3.6.2 = Eq. 4.9.1.
@@ -248,6 +253,135 @@ static double formal_step(double I, double j, double alpha, double h) {
   return I * std::exp(-tau) + j * h * w_of_tau(tau);
 }
 
+// ---------------------------------------------------------------------------------------------
+// O6b  The other transfer / integration modes of the paper (sections 4.5 - 4.8), one spectral point of one
+// column at a time.  A "point" carries a profile weight per cell:
+//   p_n = phibar_k(cell n)            channel-integrated profile, Eq. 4.6.3 (coarse grid)
+//   p_n = phi(nu_point; cell n)       point profile, Eq. 3.3.3 (fine grid of the thick mode, section 4.5)
+// and the per-cell coefficients  jL_n = j0_n p_n,  aL_n = kappa0_n p_n,  jD_n = alpha_d,n S_d,n,  aD_n = alpha_d,n.
+//
+// Readings: S23 selectively thin uses the continuum intensity of the SAME grid index as the
+// coefficients (formal: the continuum after its own step of that cell, "we simply solve for the continuum step
+// first"); S24 smooth integration treats cell n as the point x_n = n h with y_0 = I_bg at the
+// farthest cell and takes R - 1 steps (TR for the first, BDF2 after); S25 thin-smooth Simpson panels
+// span two cell spacings [x_2m, x_2m+2] (Eq. 4.7.7 with its h = 2 cell spacings, "sum of order floor((R-1)/2)"),
+// a left-over last interval (R even) is integrated by the trapezoidal rule; S26 the ReLU of PAPER.md:709, 717, 738
+// is applied after every smooth step and after every selectively-thin step, to total and continuum alike.
+static double relu(double x) { return x > 0.0 ? x : 0.0; }
+
+// p[n], n = 0..R-1: profile weights of this spectral point; cont[n]: continuum intensity at grid index n as
+// produced by orc_continuum_column for the same integration (needed by the selectively thin mode).
+// Returns the total intensity of this spectral point at the observer.
+static double total_point(const orc_config *c, int R, const double *p, const double *j0, const double *k0,
+                          const double *ad, const double *Sd, const double *cont, double Ibg) {
+  const double h = c->cell_cm;
+  const int mode = c->transfer_mode;
+  if (mode == 2) {                                   // optically thin, Eq. 4.7.3 - 4.7.4
+    if (c->integration == 0) {                       // Eq. 4.7.6: midpoint sum
+      double I = Ibg;
+      for (int n = 0; n < R; ++n) I += h * (j0[n] * p[n] + ad[n] * Sd[n]);
+      return I;
+    }
+    double I = Ibg;                                  // Eq. 4.7.7: Simpson panels of two cell spacings
+    int n = 0;
+    for (; n + 2 < R; n += 2) {
+      const double f0 = j0[n] * p[n] + ad[n] * Sd[n], f1 = j0[n + 1] * p[n + 1] + ad[n + 1] * Sd[n + 1],
+                   f2 = j0[n + 2] * p[n + 2] + ad[n + 2] * Sd[n + 2];
+      I += (2.0 * h / 6.0) * (f0 + 4.0 * f1 + f2);
+    }
+    if (n + 1 < R) I += 0.5 * h * ((j0[n] * p[n] + ad[n] * Sd[n]) + (j0[n + 1] * p[n + 1] + ad[n + 1] * Sd[n + 1]));
+    return I;
+  }
+  // thick (Eq. 4.8.6 - 4.8.8) or selectively thin (Eq. 4.8.14 - 4.8.15) coefficients at grid index n;
+  // Ic = continuum intensity paired with index n
+  auto jT = [&](int n, double Ic) {
+    return mode == 0 ? j0[n] * p[n] + ad[n] * Sd[n] : j0[n] * p[n] + ad[n] * Sd[n] - k0[n] * p[n] * Ic;
+  };
+  auto aT = [&](int n) { return mode == 0 ? k0[n] * p[n] + ad[n] : ad[n]; };
+  if (c->integration == 0) {                         // formal, Eq. 4.8.5; cont[n] = continuum after cell n
+    double I = Ibg;
+    for (int n = 0; n < R; ++n) {
+      I = formal_step(I, jT(n, cont[n]), aT(n), h);
+      if (mode == 1) I = relu(I);
+    }
+    return I;
+  }
+  // smooth: y_0 = I_bg at x_0; TR (Eq. 4.8.12) for the first step, BDF2 (Eq. 4.8.10) after; cont[n] = continuum at x_n
+  if (R < 2) return Ibg;
+  double Im = Ibg;
+  double I = relu((h * (jT(0, cont[0]) + jT(1, cont[1])) + (2.0 - h * aT(0)) * Im) / (2.0 + h * aT(1)));
+  for (int n = 2; n < R; ++n) {
+    const double In = relu((2.0 * h * jT(n, cont[n]) + 4.0 * I - Im) / (3.0 + 2.0 * h * aT(n)));
+    Im = I;
+    I = In;
+  }
+  return I;
+}
+
+// Continuum baseline of one column, Eq. 3.1.3 with Eq. 4.4.3 - 4.4.5, in the chosen mode
+// and integration.  cont[n] as total_point expects it; returns the continuum at the observer.
+static double continuum_column(const orc_config *c, int R, const double *ad, const double *Sd, double Ibg, double *cont) {
+  const double h = c->cell_cm;
+  if (c->transfer_mode == 2) {                       // thin: Eq. 4.7.5 (cont[] unused by total_point)
+    std::vector<double> zero(R, 0.0);
+    for (int n = 0; n < R; ++n) cont[n] = 0.0;
+    return total_point(c, R, zero.data(), zero.data(), zero.data(), ad, Sd, cont, Ibg);
+  }
+  if (c->integration == 0) {
+    double I = Ibg;
+    for (int n = 0; n < R; ++n) {
+      I = formal_step(I, ad[n] * Sd[n], ad[n], h);
+      if (c->transfer_mode == 1) I = relu(I);
+      cont[n] = I;
+    }
+    return I;
+  }
+  cont[0] = Ibg;
+  if (R < 2) return Ibg;
+  cont[1] = relu((h * (ad[0] * Sd[0] + ad[1] * Sd[1]) + (2.0 - h * ad[0]) * cont[0]) / (2.0 + h * ad[1]));
+  for (int n = 2; n < R; ++n)
+    cont[n] = relu((2.0 * h * ad[n] * Sd[n] + 4.0 * cont[n - 1] - cont[n - 2]) / (3.0 + 2.0 * h * ad[n]));
+  return cont[R - 1];
+}
+
+// One column in any mode other than the hot path.  Coarse grid: one point per channel with phibar.  Fine grid
+// (thick mode, subsample = f odd): points at spacing dv / (f + 1) from the lower edge of channel 0; the channel
+// average is the composite Simpson rule over the (f + 1) / 2 panels of the channel (Eq. 4.5.1, 4.4.1 - 4.4.2).
+static void march_column_modes(const orc_config *c, const double *coef, const float *vlos, int64_t pix,
+                               double *I_tot, double *I_cont) {
+  const int64_t plane = (int64_t)c->nx * c->ny, ncell = plane * c->nz;
+  const int R = c->nz;
+  const double Ibg = orc_planck(c->nu0_Hz, c->T_cmb);
+  std::vector<double> j0(R), k0(R), b(R), ad(R), Sd(R), vl(R), cont(R), p(R);
+  for (int n = 0; n < R; ++n) {
+    const int64_t cell = (int64_t)n * plane + pix;
+    j0[n] = coef[cell]; k0[n] = coef[ncell + cell]; b[n] = coef[2 * ncell + cell];
+    ad[n] = coef[3 * ncell + cell]; Sd[n] = coef[4 * ncell + cell]; vl[n] = (double)vlos[cell];
+  }
+  *I_cont = continuum_column(c, R, ad.data(), Sd.data(), Ibg, cont.data());
+  const int f = (c->transfer_mode == 0) ? c->subsample : 0;
+  if (f == 0) {
+    for (int v = 0; v < c->nv; ++v) {
+      for (int n = 0; n < R; ++n) p[n] = orc_phibar(c, v, vl[n], b[n]);
+      I_tot[v] = total_point(c, R, p.data(), j0.data(), k0.data(), ad.data(), Sd.data(), cont.data(), Ibg);
+    }
+    return;
+  }
+  const int m = f + 1;                                // fine intervals per channel
+  const double dvf = c->dv_cms / m;
+  std::vector<double> If((size_t)c->nv * m + 1);
+  for (size_t q = 0; q < If.size(); ++q) {
+    const double vel = c->v0_cms - 0.5 * c->dv_cms + q * dvf;
+    for (int n = 0; n < R; ++n) p[n] = orc_phi_point(c, vel, vl[n], b[n]);
+    If[q] = total_point(c, R, p.data(), j0.data(), k0.data(), ad.data(), Sd.data(), cont.data(), Ibg);
+  }
+  for (int v = 0; v < c->nv; ++v) {
+    double acc = 0.0;
+    for (int q = 0; q < m; q += 2) acc += If[(size_t)v * m + q] + 4.0 * If[(size_t)v * m + q + 1] + If[(size_t)v * m + q + 2];
+    I_tot[v] = acc * (2.0 * dvf / 6.0) / c->dv_cms;   // (1 / Delta nu_W) * integral, in velocity units
+  }
+}
+
 // March one pixel column (k = 0 far ... nz-1 near; reading S11) for all channels.
 // coef = {j0, kappa0, b, alpha_d, S_d} planes [5][ncell], vlos plane float32.
 // Total: alpha = kappa0 phibar + alpha_d, j = j0 phibar + alpha_d S_d   (Eq. 4.8.6-4.8.7, 4.6.4)
@@ -255,6 +389,10 @@ static double formal_step(double I, double j, double alpha, double h) {
 // Both start from I_bg = B_nu0(T_cmb).  No ReLU clamp (smooth integrator only).
 void orc_march_column(const orc_config *c, const double *coef, const float *vlos, int64_t pix,
                       double *I_tot /*[nv]*/, double *I_cont /*[1]*/) {
+  if (c->transfer_mode != 0 || c->integration != 0 || c->subsample != 0) {
+    march_column_modes(c, coef, vlos, pix, I_tot, I_cont);
+    return;
+  }
   const int64_t plane = (int64_t)c->nx * c->ny, ncell = plane * c->nz;
   const double h = c->cell_cm;
   const double Ibg = orc_planck(c->nu0_Hz, c->T_cmb);

@@ -53,6 +53,7 @@ class _Cfg(C.Structure):
         ("beam_fwhm_px", C.c_double), ("noise_mu", C.c_double), ("noise_sigma", C.c_double),
         ("noise_gamma_mode", C.c_int32),
         ("seed", C.c_uint64),
+        ("transfer_mode", C.c_int32), ("integration", C.c_int32), ("subsample", C.c_int32),
     ]
 
 
