@@ -94,6 +94,16 @@ typedef struct {
   uint64_t seed;                /* noise seed (Philox4x32-10 key) */
   /* implementation choice, does not change the mathematics */
   int32_t transfer_algo;        /* IRIS_SO_ALGO_* */
+  /* The paper's other transfer / integration modes (sections 4.4 - 4.8).  All three 0 = the hot
+   * path above (optically thick, formal integration, channel-integrated profile).  Any other combination runs
+   * transfer_modes_kernel; iris_so_observe_adjoint then returns IRIS_SO_EUNSUPPORTED. */
+  int32_t transfer_mode;        /* 0 optically thick (4.5), 1 selectively thin (4.6, Eq. 4.8.13-4.8.15),
+                                 * 2 optically thin (4.7, Eq. 4.7.3-4.7.5) */
+  int32_t integration;          /* 0 formal (Eq. 4.8.5 / 4.7.6), 1 smooth (trapezoidal first step Eq. 4.8.12 + BDF2
+                                 * Eq. 4.8.10 with the ReLU of PAPER.md:709; Simpson along the ray Eq. 4.7.7 in thin mode) */
+  int32_t subsample;            /* thick mode only: 0 = channel-integrated profile (Eq. 4.6.3); odd f >= 1 = point
+                                 * profile (Eq. 3.3.3) on a fine velocity grid with f added midpoints per channel,
+                                 * averaged over the channel by Simpson's rule (Eq. 4.5.1) */
 } iris_so_config;
 
 /* Validates and copies the configuration (including the host arrays), selects the current CUDA device.
@@ -169,8 +179,8 @@ iris_so_status iris_so_profile_read(iris_so_ctx *ctx, int32_t stage, double *tot
  * algorithm evaluates; the dense algorithm evaluates nx*ny*nz*nv).  Synchronises the stream. */
 iris_so_status iris_so_transfer_work(iris_so_ctx *ctx, uint64_t *window_updates, void *cuda_stream);
 
-/* Name of the LOS transfer kernel this context launches ("transfer_series_kernel", "transfer_window_kernel"
- * or "transfer_dense_kernel"); static storage. */
+/* Name of the LOS transfer kernel this context launches ("transfer_series_kernel", "transfer_window_kernel",
+ * "transfer_dense_kernel" or "transfer_modes_kernel"); static storage. */
 const char *iris_so_transfer_kernel(const iris_so_ctx *ctx);
 
 /* Stand-alone post-processing stages (also used inside iris_so_observe). */

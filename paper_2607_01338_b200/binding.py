@@ -46,6 +46,7 @@ class _Config(C.Structure):
         ("noise_gamma_mode", C.c_int32),
         ("seed", C.c_uint64),
         ("transfer_algo", C.c_int32),
+        ("transfer_mode", C.c_int32), ("integration", C.c_int32), ("subsample", C.c_int32),
     ]
 
 
@@ -116,7 +117,7 @@ def _make_config(cfg, transfer_algo):
         elif name == "transfer_algo":
             s.transfer_algo = int(transfer_algo)
         else:
-            val = getattr(cfg, name)
+            val = getattr(cfg, name, 0)
             setattr(s, name, float(val) if ctype is C.c_double else int(val))
     ptr = lambda a: a.ctypes.data_as(C.POINTER(C.c_double))
     s.energy_K, s.weight, s.einstein_A, s.coll_down_ref = (ptr(a) for a in keep)

@@ -18,6 +18,7 @@
 #include "transfer_dense.cuh"
 #include "transfer_window.cuh"
 #include "transfer_series.cuh"
+#include "transfer_modes.cuh"
 #include "adjoint_kernels.cuh"
 
 namespace {
@@ -168,6 +169,11 @@ iris_so_status validate(const iris_so_config* c, std::string& why) {
   if (!(c->noise_sigma >= 0.0) || !std::isfinite(c->noise_mu)) return bad("bad noise parameters");
   if (c->noise_gamma_mode < 0 || c->noise_gamma_mode > 1) return bad("bad noise_gamma_mode");
   if (c->transfer_algo < 0 || c->transfer_algo > 3) return bad("bad transfer_algo");
+  if (c->transfer_mode < 0 || c->transfer_mode > 2) return bad("transfer_mode must be 0 (thick), 1 (selectively thin) or 2 (thin)");
+  if (c->integration < 0 || c->integration > 1) return bad("integration must be 0 (formal) or 1 (smooth)");
+  if (c->subsample < 0 || c->subsample > 255 || (c->subsample > 0 && c->subsample % 2 == 0))
+    return bad("subsample must be 0 or an odd number of added midpoints per channel (<= 255)");
+  if (c->subsample > 0 && c->transfer_mode != 0) return bad("subsample (fine velocity grid) applies to the thick mode only");
   return IRIS_SO_OK;
 }
 
@@ -322,12 +328,23 @@ int resolved_algo(const iris_so_config& c) {
   return algo;
 }
 
+bool hot_path_mode(const iris_so_config& c) { return c.transfer_mode == 0 && c.integration == 0 && c.subsample == 0; }
+
 // K3 (+K4, K5) from ctx->d_coef
 iris_so_status run_transfer(iris_so_ctx* ctx, const iris::MarchConsts& mc, float* out, float* out_cont, cudaStream_t st) {
   const bool dust = ctx->cfg.dust_on != 0;
   const int npix = (int)ctx->npix, nz = ctx->cfg.nz, nv = ctx->cfg.nv;
   const int algo = resolved_algo(ctx->cfg);
   ProfScope prof(ctx, IRIS_SO_STAGE_TRANSFER, st);
+  if (!hot_path_mode(ctx->cfg)) {
+    iris::ModeConsts md;
+    md.mode = ctx->cfg.transfer_mode; md.smooth = ctx->cfg.integration;
+    md.fine_m = ctx->cfg.subsample > 0 ? ctx->cfg.subsample + 1 : 0;
+    cudaError_t e = iris::launch_transfer_modes(mc, md, ctx->d_coef, ctx->ncell, npix, nz, nv, out, out_cont, st);
+    ctx->launches++;
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "launch of transfer_modes_kernel");
+    return IRIS_SO_OK;
+  }
   if (algo == IRIS_SO_ALGO_DENSE) {
     constexpr int CB = 16, NW = 4;
     dim3 block(32, NW), grid((npix + 31) / 32, (nv + CB * NW - 1) / (CB * NW));
@@ -392,6 +409,7 @@ const char* iris_so_last_error(const iris_so_ctx* ctx) { return ctx ? ctx->err.c
 
 const char* iris_so_transfer_kernel(const iris_so_ctx* ctx) {
   if (!ctx) return "";
+  if (!hot_path_mode(ctx->cfg)) return "transfer_modes_kernel";
   switch (resolved_algo(ctx->cfg)) {
     case IRIS_SO_ALGO_DENSE: return "transfer_dense_kernel";
     case IRIS_SO_ALGO_WINDOW: return "transfer_series_kernel";
@@ -576,6 +594,8 @@ iris_so_status iris_so_observe_adjoint(iris_so_ctx* ctx, const float* d_nH2, con
   const iris_so_config& c = ctx->cfg;
   if ((c.subtract_continuum && c.subtract_space != 0) || c.out_unit == 2)
     return fail(ctx, IRIS_SO_EUNSUPPORTED, "adjoint needs intensity-space subtraction and out_unit 0 or 1");
+  if (!hot_path_mode(c))
+    return fail(ctx, IRIS_SO_EUNSUPPORTED, "adjoint is implemented for the thick / formal / channel-integrated mode only");
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   iris_so_status s = run_coefficients(ctx, d_nH2, d_Tgas, d_Tdust, d_vlos, nullptr, st);
   if (s != IRIS_SO_OK) return s;

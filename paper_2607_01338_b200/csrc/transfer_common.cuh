@@ -68,7 +68,7 @@ __device__ __forceinline__ float update_dust(float D, float dErf, float e_c, flo
   const float J_L = e_c * dErf;
   const float m = one_minus_exp_neg(tau_L);
   const float tau_T = tau_L + d.tau_d;
-  const float r = rcp_approx(tau_T == 0.0f ? 1.0f : tau_T);
+  const float r = rcp_approx(fabsf(tau_T) < 1.0e-30f ? 1.0f : tau_T);   // also keeps denormal tau_T away from rcp.ftz
   const float Em = d.E_d * m;
   const float t1 = d.m_d + Em;
   const float t2 = fmaf(d.tau_d, Em, -tau_L * d.m_d);

@@ -1,0 +1,137 @@
+"""GPU parity of the paper's other transfer / integration modes (transfer_modes_kernel, through the C ABI) against
+the float64 oracle on the same seeded inputs: optically thin / selectively thin / thick, formal / smooth, and the
+fine velocity grid with Simpson's rule.  Tolerances: tests/parity.py."""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+
+from iris_inputs import make_fields, make_workload
+from iris_inputs.fields import KMS
+from oracle import Oracle
+from parity import assert_spectra, krj
+
+pytestmark = pytest.mark.gpu
+
+# (transfer_mode, integration, subsample)
+MODES = {"thin_formal": (2, 0, 0), "thin_smooth": (2, 1, 0), "selthin_formal": (1, 0, 0), "selthin_smooth": (1, 1, 0),
+         "thick_smooth": (0, 1, 0), "thick_formal_sub1": (0, 0, 1), "thick_formal_sub3": (0, 0, 3),
+         "thick_smooth_sub1": (0, 1, 1), "thick_smooth_sub7": (0, 1, 7)}
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def dev_fields(f):
+    return [dev(f[k]) for k in ("nH2", "Tgas", "Tdust", "vlos")]
+
+
+def with_mode(cfg, name):
+    m, i, s = MODES[name]
+    return cfg.with_(transfer_mode=m, integration=i, subsample=s)
+
+
+def gpu_cube(cfg, f, **kw):
+    from paper_2607_01338_b200 import IrisSO
+    it = IrisSO(cfg)
+    assert it.transfer_kernel() == "transfer_modes_kernel"
+    return it.observe(*dev_fields(f), **kw).cpu().numpy()
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_modes_small_dust(mode):
+    cfg, r = make_workload("small", n=32, nv=96)
+    cfg = with_mode(cfg, mode)
+    f = make_fields(cfg, r)
+    f["vlos"] = (0.3 * f["vlos"]).astype(np.float32)
+    cube = gpu_cube(cfg, f)
+    ref = Oracle(cfg).observe(f)
+    worst = assert_spectra(cube, ref, what=mode)
+    assert np.abs(ref).max() > 0.05
+    print("%s: worst pixel at %.3g of tolerance, peak %.3g K" % (mode, worst, np.abs(ref).max()))
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_modes_tiny_no_dust_ragged(mode):
+    """Dust off (tau_d = 0 everywhere), sizes that fill neither the 32-pixel nor the 8-channel tile, odd and even nz."""
+    for nz in (19, 20):
+        cfg, r = make_workload("tiny", nx=37, ny=3, nz=nz, nv=45)
+        cfg = with_mode(cfg, mode).with_(v0_cms=-11.0 * KMS)
+        f = make_fields(cfg, r)
+        f["vlos"] = (0.1 * f["vlos"]).astype(np.float32)
+        assert_spectra(gpu_cube(cfg, f), Oracle(cfg).observe(f), what="%s nz=%d" % (mode, nz))
+
+
+@pytest.mark.parametrize("mode", MODES)
+@pytest.mark.parametrize("shape", [dict(nx=1, ny=1, nz=1, nv=1), dict(nx=2, ny=1, nz=2, nv=3), dict(nx=3, ny=2, nz=3, nv=9)])
+def test_modes_degenerate_shapes(mode, shape):
+    cfg, r = make_workload("small", **shape)
+    cfg = with_mode(cfg, mode).with_(v0_cms=-0.5 * (shape["nv"] - 1) * cfg.dv_cms)
+    f = make_fields(cfg, r)
+    f["vlos"] = (0.01 * f["vlos"]).astype(np.float32)
+    assert_spectra(gpu_cube(cfg, f), Oracle(cfg).observe(f), what=mode)
+
+
+@pytest.mark.parametrize("mode", ["selthin_formal", "selthin_smooth", "thick_smooth", "thick_smooth_sub1"])
+@pytest.mark.parametrize("case", ["thick_line", "opaque_dust_clamp", "absorption"])
+def test_modes_regimes(mode, case):
+    """Large optical depths (A-stability of BDF2), the ReLU clamp, and lines in absorption."""
+    cfg, r = make_workload("small", n=20, nv=96)
+    cfg = with_mode(cfg, mode)
+    f = make_fields(cfg, r)
+    f["vlos"] = (0.25 * f["vlos"]).astype(np.float32)
+    if case == "thick_line":
+        cfg = cfg.with_(abundance=2e-4)
+    elif case == "opaque_dust_clamp":
+        # bright background, cold dust that turns opaque abruptly: the smooth continuum overshoots below zero and is clamped
+        cfg = cfg.with_(T_cmb=60.0, kappa_gas_cm2_g=3.0)
+        f["Tdust"] = np.full_like(f["Tdust"], 3.0)
+        f["nH2"][: cfg.nz // 2] *= 1e-3
+        f["nH2"][cfg.nz // 2:] *= 30.0
+    else:
+        cfg = cfg.with_(kappa_gas_cm2_g=1.0)
+        f["Tdust"] = np.full_like(f["Tdust"], 150.0)
+    o = Oracle(cfg)
+    cfg_tot = cfg.with_(subtract_continuum=False)
+    cube = gpu_cube(cfg, f)
+    ref = o.observe(f)
+    # a clamped spectrum is compared on the total intensity scale as well (the subtracted cube can be ~ -continuum)
+    tot = gpu_cube(cfg_tot, f)
+    ref_tot = Oracle(cfg_tot).observe(f)
+    assert_spectra(tot, ref_tot, extra=3e-7 * np.abs(ref_tot).max(axis=-1, keepdims=True), what=mode + " total")
+    assert_spectra(cube, ref, extra=3e-7 * np.abs(ref_tot).max(axis=-1, keepdims=True), what=mode + " subtracted")
+
+
+@pytest.mark.parametrize("mode", ["thin_formal", "selthin_smooth", "thick_smooth_sub1"])
+def test_modes_transfer_intensities_and_output_units(mode):
+    from paper_2607_01338_b200 import IrisSO
+    cfg, r = make_workload("small", n=16, nv=64)
+    cfg = with_mode(cfg, mode)
+    f = make_fields(cfg, r)
+    f["vlos"] = (0.2 * f["vlos"]).astype(np.float32)
+    o = Oracle(cfg)
+    It, Ic = IrisSO(cfg).transfer(*dev_fields(f))
+    coef = o.coefficients(f["nH2"], f["Tgas"], f["Tdust"])
+    rt, rc = o.march(coef, f["vlos"])
+    K = krj(cfg.nu0_Hz)
+    It, Ic = It.cpu().numpy().reshape(-1, cfg.nv).astype(np.float64), Ic.cpu().numpy().ravel().astype(np.float64)
+    assert np.allclose(Ic, rc, rtol=3e-6)
+    line = np.abs(rt - rc[:, None]).max(axis=1)
+    err = np.abs(It - rt).max(axis=1)
+    assert np.all(err <= 1e-4 * line + 1e-6 / K + 3e-7 * np.abs(rt).max(axis=1))
+    # Planck-space subtraction through the same kernel
+    cfg_p = cfg.with_(out_unit=2, subtract_space=1)
+    assert_spectra(gpu_cube(cfg_p, f), Oracle(cfg_p).observe(f), rel=2.6e-4, floor=2.6e-6, what=mode + " planck")
+
+
+def test_modes_adjoint_is_refused_and_bad_modes_are_rejected():
+    from paper_2607_01338_b200 import IrisSO, IrisSOError
+    cfg, r = make_workload("batch", n=8, nv=16)
+    f = make_fields(cfg, r)
+    it = IrisSO(cfg.with_(transfer_mode=2))
+    with pytest.raises(IrisSOError):
+        it.observe_adjoint(*dev_fields(f), dev(np.ones((cfg.ny, cfg.nx, cfg.nv), np.float32)))
+    for bad in (dict(transfer_mode=3), dict(integration=2), dict(subsample=2), dict(subsample=1, transfer_mode=1)):
+        with pytest.raises(IrisSOError):
+            IrisSO(cfg.with_(**bad))
