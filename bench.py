@@ -345,6 +345,41 @@ def bench_workload(torch, dist, name, algo, steps, warmup, rank, peaks, want_e2e
     return res
 
 
+MODE_PROBES = {"thick_smooth_subsample1 (the paper's production mode)": (0, 1, 1), "thick_formal_subsample1": (0, 0, 1),
+               "thick_smooth": (0, 1, 0), "selectively_thin_formal": (1, 0, 0), "selectively_thin_smooth": (1, 1, 0),
+               "thin_formal": (2, 0, 0), "thin_smooth": (2, 1, 0)}
+
+
+def bench_modes(torch, warmup):
+    """transfer_modes_kernel on the medium cube: ms per launch and spectral-point updates per second for the paper's
+    other transfer / integration modes (every (cell, point) is evaluated: dense algorithm)."""
+    from paper_2607_01338_b200 import IrisSO
+    dev = torch.device("cuda", torch.cuda.current_device())
+    cfg0, recipe = make_workload("medium")
+    fields = make_fields(cfg0, recipe)
+    d = [torch.from_numpy(fields[k]).to(dev) for k in ("nH2", "Tgas", "Tdust", "vlos")]
+    out = {}
+    for name, (m, i, sub) in MODE_PROBES.items():
+        cfg = cfg0.with_(transfer_mode=m, integration=i, subsample=sub)
+        it = IrisSO(cfg)
+        cube = torch.empty(it.shape_cube, dtype=torch.float32, device=dev)
+        for _ in range(warmup):
+            it.observe(*d, cube=cube)
+        torch.cuda.synchronize()
+        it.profile(True)
+        for _ in range(3):
+            it.observe(*d, cube=cube)
+        prof = it.profile_read()
+        it.profile(False)
+        t = prof["transfer"][0] / prof["transfer"][1] * 1e-3
+        points = cfg.nv * (3 * (sub + 1) // 2 if sub else 1)      # (f + 1) / 2 Simpson panels x 3 points per channel
+        out[name] = {"kernel": it.transfer_kernel(), "ms_per_launch": t * 1e3,
+                     "point_updates_per_s": cfg.nx * cfg.ny * cfg.nz * points / t,
+                     "ms_per_cube": sum(v[0] for v in prof.values()) / 3}
+        it.close()
+    return out
+
+
 def run_ours(args):
     import torch
     rank, local_rank, world = env_rank()
@@ -372,6 +407,8 @@ def run_ours(args):
             "what": "iris_so_observe on BASELINE config 2 (medium: 256^2 x (256+32) cells, 512 channels, dust, beam 3 px, noise 0.25 K)",
             "stages": med["stages"], "transfer_roofline_frac": med["roofline"]["frac"],
             "transfer_nominal_updates_per_s": med["roofline"]["nominal_updates_per_s"]}
+    if not args.no_extras and world == 1:
+        extra["other_modes_256x256x288_512ch"] = bench_modes(torch, max(args.warmup, 3))
     if rank != 0:
         return 0
     cb = None

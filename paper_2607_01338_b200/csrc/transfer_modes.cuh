@@ -22,9 +22,11 @@
 //                     a_n = A_n + t_d,n (thick) or t_d,n (selectively thin);  C_n by the same formulas with E = A = 0
 // none of which cancels.  The ReLU acts on the true intensities: I^[T] = D + C >= 0, C >= 0 (reading S26).
 //
-// Mapping: a CTA is 32 pixels x 8 channels; lanes run along pixels, so the six coefficient planes are read with
-// 128-byte coalesced loads (every plane of a column is re-read once per 8 channels, from L2); the result tile is
-// transposed through shared memory so that each pixel writes 32 contiguous bytes.
+// Mapping: a thread owns one pixel and NPT consecutive spectral points in registers (8 channels with their 9 shared
+// erfc edges, or the 9 fine points of 8 / m channels, or one Simpson panel of 3 points at a time for finer grids); lanes
+// run along pixels, so the six coefficient planes are read with 128-byte coalesced loads and the per-cell continuum /
+// dust scalars are computed once per NPT points; a block of points farther than 5.5 Doppler widths from the line centre
+// skips the profile evaluation (its weights are zero); each thread writes its channels as contiguous 16-byte stores.
 #pragma once
 #include "transfer_common.cuh"
 
@@ -35,145 +37,241 @@ struct ModeConsts {
   int fine_m;            // 0: channel-integrated profile; else fine intervals per channel (f + 1, even)
 };
 
-// State of one spectral point: D at the last two grid indices.
-struct ModePoint { float D, Dm; };
-
-// Continuum step at grid index n (n = 0: initial condition).  Returns the new continuum; *C_unc receives the value
-// before the ReLU (the difference recurrences are derived from the unclamped relation).
-__device__ __forceinline__ float continuum_step(const ModeConsts& md, int n, float C, float Cm, float td, float Jd,
-                                                float Sd, float td_prev, float Jd_prev, float wn, float* C_unc) {
-  float c;
-  if (md.mode == 2) c = md.smooth ? fmaf(wn, Jd, C) : C + Jd;
-  else if (!md.smooth) c = fmaf(C, exp_neg(td), Sd * one_minus_exp_neg(td));
-  else if (n == 0) c = C;
-  else if (n == 1) c = (Jd_prev + Jd + (2.0f - td_prev) * C) / (2.0f + td);
-  else c = (2.0f * Jd + 4.0f * C - Cm) / fmaf(2.0f, td, 3.0f);
-  *C_unc = c;
-  return (md.mode != 2 && (md.smooth || md.mode == 1)) ? fmaxf(c, 0.0f) : c;
-}
-
 // w(t) = (1 - exp(-t)) / t, w(0) = 1
 __device__ __forceinline__ float w_of(float t) {
   return fabsf(t) < 1.0e-3f ? fmaf(t, fmaf(t, 1.0f / 6.0f, -0.5f), 1.0f) : one_minus_exp_neg(t) / t;
 }
 
-template <int NP>
-__global__ void __launch_bounds__(256)
+constexpr float kModesXmax = 5.5f;     // profile weights beyond this many Doppler widths are dropped (< 1e-13 of the peak)
+
+// PROF 0: channel-integrated profile, 8 channels per thread (NPT = 8 weights from 9 edges)
+// PROF 1: fine grid with m = 2, 4 or 8 intervals per channel: 9 points = 8 / m channels per thread
+// PROF 2: fine grid, any even m: one channel per thread, one Simpson panel (3 points) per march
+template <int MODE, bool SMOOTH, int PROF>
+__global__ void __launch_bounds__(128)
 transfer_modes_kernel(MarchConsts mc, ModeConsts md, const float* __restrict__ coef, int64_t ncell, int npix, int nz,
                       int nv, float* __restrict__ out, float* __restrict__ out_cont) {
-  __shared__ float tile[8][33];
-  const int lane = threadIdx.x, ty = threadIdx.y;
-  const int pix = blockIdx.x * 32 + lane;
-  const int v = blockIdx.y * 8 + ty;
-  const bool active = pix < npix && v < nv;
-  const int pl = min(pix, npix - 1);
+  constexpr int NPT = PROF == 0 ? 8 : (PROF == 1 ? 9 : 3);
+  const int pix = blockIdx.x * 32 + threadIdx.x;
+  const int blk = blockIdx.y * blockDim.y + threadIdx.y;      // channel block of this thread
   const int m = md.fine_m;
-  const int npanel = m > 0 ? m / 2 : 1;
-  const bool dust = true;      // tau_d = 0 planes when dust is off: the same formulas hold
-  (void)dust;
+  const int cpb = PROF == 0 ? 8 : (PROF == 1 ? 8 / m : 1);    // channels per thread
+  const int v0 = blk * cpb;
+  if (pix >= npix || v0 >= nv) return;
+  const int npanel = PROF == 2 ? m / 2 : 1;
+  const float inv_m = PROF == 0 ? 1.0f : 1.0f / (float)m;
+  const int Rs = (nz & 1) ? nz : nz - 1;                      // points covered by whole Simpson panels along the ray
   float Dacc = 0.0f, Cfin = mc.T_bg;
+  float Dfin[NPT];
 
   for (int panel = 0; panel < npanel; ++panel) {
-    ModePoint pt[NP];
+    float D[NPT], Dm[NPT];
 #pragma unroll
-    for (int k = 0; k < NP; ++k) pt[k].D = pt[k].Dm = 0.0f;
+    for (int k = 0; k < NPT; ++k) D[k] = Dm[k] = 0.0f;
     float C = mc.T_bg, Cm = mc.T_bg;
     float e_p = 0.0f, a_p = 0.0f, c_p = 0.0f, s_p = 1.0f, td_p = 0.0f, Jd_p = 0.0f;   // coefficients of grid index n - 1
-    const float* p = coef + pl;
-    const int Rs = (nz & 1) ? nz : nz - 1;               // points covered by whole Simpson panels along the ray
+    // position (channel-edge index units) of point 0 and spacing of the points
+    const float pos0 = PROF == 2 ? (float)v0 + (float)(2 * panel) * inv_m : (float)v0;
+    const float dpos = PROF == 0 ? 1.0f : inv_m;
+    const float* p = coef + pix;
     for (int n = 0; n < nz; ++n, p += npix) {
       const float e_c = p[0], a_c = p[ncell], c_los = p[2 * ncell], s = p[3 * ncell];
       const float td = p[4 * ncell], Sd = p[5 * ncell];
       const float Jd = td * Sd;
       float wn = 0.0f;
-      if (md.mode == 2 && md.smooth) {
+      if (MODE == 2 && SMOOTH) {
         if (Rs >= 3 && n < Rs) wn = (n == 0 || n == Rs - 1) ? (1.0f / 3.0f) : ((n & 1) ? (4.0f / 3.0f) : (2.0f / 3.0f));
         if (!(nz & 1) && nz >= 2 && n >= nz - 2) wn += 0.5f;
       }
+      // ---- per-cell scalars: continuum step, dust factors
       float C_unc;
-      const float Cn = continuum_step(md, n, C, Cm, td, Jd, Sd, td_p, Jd_p, wn, &C_unc);
-      const float Ed = (md.mode == 1 && !md.smooth) ? exp_neg(td) : 1.0f;
-      const float wd = (md.mode == 1 && !md.smooth) ? w_of(td) : 1.0f;
+      if (MODE == 2) C_unc = SMOOTH ? fmaf(wn, Jd, C) : C + Jd;
+      else if (!SMOOTH) C_unc = fmaf(C, exp_neg(td), Sd * one_minus_exp_neg(td));
+      else if (n == 0) C_unc = C;
+      else if (n == 1) C_unc = (Jd_p + Jd + (2.0f - td_p) * C) * rcp_approx(2.0f + td);
+      else C_unc = (2.0f * Jd + 4.0f * C - Cm) * rcp_approx(fmaf(2.0f, td, 3.0f));
+      const float Cn = (MODE != 2 && (SMOOTH || MODE == 1)) ? fmaxf(C_unc, 0.0f) : C_unc;
+      float Ed = 1.0f, wd = 1.0f;
       DustStep ds;
-      if (md.mode == 0 && !md.smooth) {
+      if (MODE == 1 && !SMOOTH) { Ed = exp_neg(td); wd = w_of(td); }
+      if (MODE == 0 && !SMOOTH) {
         ds.tau_d = td; ds.S_d = Sd; ds.C = C;
         ds.E_d = exp_neg(td);
         ds.m_d = one_minus_exp_neg(td);
       }
+      // ---- profile weights of the NPT points in this cell ("erf-difference" units); zero far from the line
+      float pw[NPT], pwp[NPT];
+      const float x0 = (pos0 - c_los) * s;
+      const float x1 = x0 + (PROF == 0 ? (float)NPT : (float)(NPT - 1) * dpos) * s;
+      const bool near = x0 < kModesXmax && x1 > -kModesXmax;
+      if (near) {
+        if (PROF == 0) {
+          float G_lo = signed_erfc(x0), xl = x0;
 #pragma unroll
-      for (int k = 0; k < NP; ++k) {
-        // profile weight of this point in this cell (in "erf-difference" units) and of the previous cell
-        float pw, pw_prev = 0.0f;
-        if (m == 0) {
-          const float x_lo = ((float)v - c_los) * s, x_hi = ((float)(v + 1) - c_los) * s;
-          pw = erf_diff(x_lo, signed_erfc(x_lo), x_hi, signed_erfc(x_hi));
-          if (md.smooth && n == 1) {
-            const float y_lo = ((float)v - c_p) * s_p, y_hi = ((float)(v + 1) - c_p) * s_p;
-            pw_prev = erf_diff(y_lo, signed_erfc(y_lo), y_hi, signed_erfc(y_hi));
+          for (int k = 0; k < NPT; ++k) {
+            const float xh = ((pos0 + (float)(k + 1)) - c_los) * s;
+            const float G_hi = signed_erfc(xh);
+            pw[k] = erf_diff(xl, G_lo, xh, G_hi);
+            xl = xh; G_lo = G_hi;
           }
         } else {
-          const float pos = (float)v + (float)(2 * panel + k) / (float)m;      // channel-edge index units
-          const float x = (pos - c_los) * s;
-          pw = 1.1283791670955126f * s * ex2_approx(-1.4426950408889634f * x * x);
-          if (md.smooth && n == 1) {
-            const float y = (pos - c_p) * s_p;
-            pw_prev = 1.1283791670955126f * s_p * ex2_approx(-1.4426950408889634f * y * y);
+#pragma unroll
+          for (int k = 0; k < NPT; ++k) {
+            const float x = ((pos0 + (float)k * dpos) - c_los) * s;
+            pw[k] = fabsf(x) < kModesXmax ? 1.1283791670955126f * s * ex2_approx(-1.4426950408889634f * x * x) : 0.0f;
           }
         }
-        const float E = e_c * pw, A = a_c * pw;
-        float D = pt[k].D, Dn;
-        if (md.mode == 2) {
-          Dn = md.smooth ? fmaf(wn, E, D) : D + E;
-        } else if (!md.smooth) {
-          if (md.mode == 1) {
-            Dn = fmaf(D, Ed, (E - A * Cn) * wd);
-            Dn = fmaxf(Dn, -Cn);                           // ReLU on I_T = D + C (C' >= 0 here)
-          } else {
-            Dn = update_dust(D, pw, e_c, a_c, ds);         // Eq. 4.8.5 in difference form (transfer_common.cuh)
+      } else {
+#pragma unroll
+        for (int k = 0; k < NPT; ++k) pw[k] = 0.0f;
+      }
+      if (SMOOTH && MODE != 2 && n == 1) {            // trapezoidal first step needs the weights of grid index 0 too
+        if (PROF == 0) {
+          float xl = (pos0 - c_p) * s_p, G_lo = signed_erfc(xl);
+#pragma unroll
+          for (int k = 0; k < NPT; ++k) {
+            const float xh = ((pos0 + (float)(k + 1)) - c_p) * s_p;
+            const float G_hi = signed_erfc(xh);
+            pwp[k] = (fabsf(xl) < kModesXmax || fabsf(xh) < kModesXmax) ? erf_diff(xl, G_lo, xh, G_hi) : 0.0f;
+            xl = xh; G_lo = G_hi;
           }
         } else {
-          const float Ccoef = md.mode == 0 ? C_unc : Cn;   // continuum the line term is paired with (see header)
+#pragma unroll
+          for (int k = 0; k < NPT; ++k) {
+            const float x = ((pos0 + (float)k * dpos) - c_p) * s_p;
+            pwp[k] = fabsf(x) < kModesXmax ? 1.1283791670955126f * s_p * ex2_approx(-1.4426950408889634f * x * x) : 0.0f;
+          }
+        }
+      }
+      // ---- far from the line every weight is zero: the step of every point is the dust-only step
+      if (!near && !(SMOOTH && MODE != 2 && n == 1)) {
+        if (MODE == 2) {
+          // nothing is emitted into these points
+        } else if (!SMOOTH) {
+          const float att = MODE == 1 ? Ed : ds.E_d;
+#pragma unroll
+          for (int k = 0; k < NPT; ++k) {
+            const float Dn = D[k] * att;
+            D[k] = MODE == 1 ? fmaxf(Dn, -Cn) : Dn;
+          }
+        } else if (n >= 2) {
+          const float r = rcp_approx(fmaf(2.0f, td, 3.0f));
+#pragma unroll
+          for (int k = 0; k < NPT; ++k) {
+            const float Du = fmaf(4.0f, D[k], -Dm[k]) * r;
+            Dm[k] = D[k];
+            D[k] = (C_unc >= 0.0f) ? fmaxf(Du, -C_unc) : fmaxf(Du + C_unc, 0.0f);
+          }
+        }
+        Cm = C; C = Cn;
+        e_p = e_c; a_p = a_c; c_p = c_los; s_p = s; td_p = td; Jd_p = Jd;
+        continue;
+      }
+      // ---- the step of every point
+#pragma unroll
+      for (int k = 0; k < NPT; ++k) {
+        const float E = e_c * pw[k], A = a_c * pw[k];
+        const float Dk = D[k];
+        float Dn;
+        if (MODE == 2) {
+          Dn = SMOOTH ? fmaf(wn, E, Dk) : Dk + E;
+        } else if (!SMOOTH) {
+          if (MODE == 1) Dn = fmaxf(fmaf(Dk, Ed, (E - A * Cn) * wd), -Cn);       // ReLU on I_T = D + C (C' >= 0 here)
+          else Dn = update_dust(Dk, pw[k], e_c, a_c, ds);                       // Eq. 4.8.5 in difference form
+        } else {
+          const float Ccoef = MODE == 0 ? C_unc : Cn;    // continuum the line term is paired with (see header)
           float Du;
           if (n == 0) Du = 0.0f;
           else if (n == 1) {
-            const float Ep = e_p * pw_prev, Ap = a_p * pw_prev;
-            const float a0 = (md.mode == 0 ? Ap : 0.0f) + td_p, a1 = (md.mode == 0 ? A : 0.0f) + td;
-            Du = ((Ep - Ap * C) + (E - A * Ccoef) + (2.0f - a0) * D) / (2.0f + a1);
+            const float Ep = e_p * pwp[k], Ap = a_p * pwp[k];
+            const float a0 = (MODE == 0 ? Ap : 0.0f) + td_p, a1 = (MODE == 0 ? A : 0.0f) + td;
+            Du = ((Ep - Ap * C) + (E - A * Ccoef) + (2.0f - a0) * Dk) * rcp_approx(2.0f + a1);
           } else {
-            const float an = (md.mode == 0 ? A : 0.0f) + td;
-            Du = (2.0f * (E - A * Ccoef) + 4.0f * D - pt[k].Dm) / fmaf(2.0f, an, 3.0f);
+            const float an = (MODE == 0 ? A : 0.0f) + td;
+            Du = (2.0f * (E - A * Ccoef) + 4.0f * Dk - Dm[k]) * rcp_approx(fmaf(2.0f, an, 3.0f));
           }
           // ReLU on the true intensities: I_T = relu(Du + C_unc), C = relu(C_unc)
           Dn = (C_unc >= 0.0f) ? fmaxf(Du, -C_unc) : fmaxf(Du + C_unc, 0.0f);
         }
-        pt[k].Dm = D;
-        pt[k].D = Dn;
+        Dm[k] = Dk;
+        D[k] = Dn;
       }
       Cm = C; C = Cn;
       e_p = e_c; a_p = a_c; c_p = c_los; s_p = s; td_p = td; Jd_p = Jd;
     }
     Cfin = C;
-    if (m == 0) Dacc = pt[0].D;
-    else Dacc += (pt[0].D + 4.0f * pt[NP > 1 ? 1 : 0].D + pt[NP > 2 ? 2 : 0].D) / (3.0f * (float)m);
+    if (PROF == 2) Dacc += (D[0] + 4.0f * D[1] + D[2]) * (inv_m * (1.0f / 3.0f));
+#pragma unroll
+    for (int k = 0; k < NPT; ++k) Dfin[k] = D[k];
   }
 
-  tile[ty][lane] = active ? convert_out(Dacc, Cfin, mc) : 0.0f;
-  __syncthreads();
-  if (out != nullptr) {
-    const int t = ty * 32 + lane;
-    const int pp = t >> 3, cc = t & 7;
-    const int opix = blockIdx.x * 32 + pp, ov = blockIdx.y * 8 + cc;
-    if (opix < npix && ov < nv) out[(int64_t)opix * nv + ov] = tile[cc][pp];
+  // ---- channel values of this thread -> convert and store
+  float res[8];
+  int nch = min(cpb, nv - v0);
+  if (PROF == 0) {
+#pragma unroll
+    for (int k = 0; k < 8; ++k) res[k] = convert_out(Dfin[k], Cfin, mc);
+  } else if (PROF == 1) {
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {                     // at most 4 channels (m = 2)
+      float acc = 0.0f;
+#pragma unroll
+      for (int j = 0; j < 8; j += 2) {                // panels of the channel: points c m + j .. c m + j + 2, j < m
+        const int q = c * m + j;
+        if (j < m && c < cpb) {
+          float d0 = 0.0f, d1 = 0.0f, d2 = 0.0f;
+#pragma unroll
+          for (int k = 0; k < NPT; ++k) {             // static indexing keeps Dfin in registers
+            if (k == q) d0 = Dfin[k];
+            if (k == q + 1) d1 = Dfin[k];
+            if (k == q + 2) d2 = Dfin[k];
+          }
+          acc += d0 + 4.0f * d1 + d2;
+        }
+      }
+      res[c] = convert_out(acc * (inv_m * (1.0f / 3.0f)), Cfin, mc);
+    }
+  } else {
+    res[0] = convert_out(Dacc, Cfin, mc);
   }
-  if (out_cont != nullptr && blockIdx.y == 0 && ty == 0 && pix < npix) out_cont[pix] = Cfin * mc.inv_KRJ;
+  if (out != nullptr) {
+    float* o = out + (int64_t)pix * nv + v0;
+    if (PROF == 0 && nch == 8 && (((int64_t)pix * nv + v0) & 3) == 0) {
+      reinterpret_cast<float4*>(o)[0] = make_float4(res[0], res[1], res[2], res[3]);
+      reinterpret_cast<float4*>(o)[1] = make_float4(res[4], res[5], res[6], res[7]);
+    } else {
+#pragma unroll
+      for (int k = 0; k < 8; ++k)
+        if (k < nch) o[k] = res[k];
+    }
+  }
+  if (out_cont != nullptr && blk == 0) out_cont[pix] = Cfin * mc.inv_KRJ;
+}
+
+template <int MODE, bool SMOOTH>
+inline cudaError_t launch_transfer_modes_t(const MarchConsts& mc, const ModeConsts& md, const float* coef, int64_t ncell,
+                                           int npix, int nz, int nv, float* out, float* out_cont, cudaStream_t st) {
+  const int m = md.fine_m;
+  const int prof = m == 0 ? 0 : ((m == 2 || m == 4 || m == 8) ? 1 : 2);
+  const int cpb = prof == 0 ? 8 : (prof == 1 ? 8 / m : 1);
+  const int nblk = (nv + cpb - 1) / cpb;
+  dim3 block(32, 4), grid((npix + 31) / 32, (nblk + 3) / 4);
+  if (prof == 0) transfer_modes_kernel<MODE, SMOOTH, 0><<<grid, block, 0, st>>>(mc, md, coef, ncell, npix, nz, nv, out, out_cont);
+  else if (prof == 1) transfer_modes_kernel<MODE, SMOOTH, 1><<<grid, block, 0, st>>>(mc, md, coef, ncell, npix, nz, nv, out, out_cont);
+  else transfer_modes_kernel<MODE, SMOOTH, 2><<<grid, block, 0, st>>>(mc, md, coef, ncell, npix, nz, nv, out, out_cont);
+  return cudaGetLastError();
 }
 
 inline cudaError_t launch_transfer_modes(const MarchConsts& mc, const ModeConsts& md, const float* coef, int64_t ncell,
                                          int npix, int nz, int nv, float* out, float* out_cont, cudaStream_t st) {
-  dim3 block(32, 8), grid((npix + 31) / 32, (nv + 7) / 8);
-  if (md.fine_m > 0) transfer_modes_kernel<3><<<grid, block, 0, st>>>(mc, md, coef, ncell, npix, nz, nv, out, out_cont);
-  else transfer_modes_kernel<1><<<grid, block, 0, st>>>(mc, md, coef, ncell, npix, nz, nv, out, out_cont);
-  return cudaGetLastError();
+  switch (md.mode * 2 + (md.smooth ? 1 : 0)) {
+    case 0: return launch_transfer_modes_t<0, false>(mc, md, coef, ncell, npix, nz, nv, out, out_cont, st);
+    case 1: return launch_transfer_modes_t<0, true>(mc, md, coef, ncell, npix, nz, nv, out, out_cont, st);
+    case 2: return launch_transfer_modes_t<1, false>(mc, md, coef, ncell, npix, nz, nv, out, out_cont, st);
+    case 3: return launch_transfer_modes_t<1, true>(mc, md, coef, ncell, npix, nz, nv, out, out_cont, st);
+    case 4: return launch_transfer_modes_t<2, false>(mc, md, coef, ncell, npix, nz, nv, out, out_cont, st);
+    default: return launch_transfer_modes_t<2, true>(mc, md, coef, ncell, npix, nz, nv, out, out_cont, st);
+  }
 }
 
 }  // namespace iris

@@ -135,3 +135,25 @@ def test_modes_adjoint_is_refused_and_bad_modes_are_rejected():
     for bad in (dict(transfer_mode=3), dict(integration=2), dict(subsample=2), dict(subsample=1, transfer_mode=1)):
         with pytest.raises(IrisSOError):
             IrisSO(cfg.with_(**bad))
+
+
+@pytest.mark.parametrize("mode", ["thick_smooth_sub1", "selthin_formal", "thin_smooth"])
+def test_modes_full_size_medium_sampled(mode):
+    """BASELINE config "medium" at full size (256 x 256 x 288 cells, 512 channels), in the launch configuration
+    bench.py times: seeded pixel columns against the oracle (columns are independent before the beam)."""
+    from paper_2607_01338_b200 import IrisSO
+    cfg, r = make_workload("medium")
+    cfg = with_mode(cfg, mode)
+    f = make_fields(cfg, r)
+    cube = IrisSO(cfg).observe(*dev_fields(f), beam=False, noise=False)
+    n_cols = 24
+    plane = cfg.nx * cfg.ny
+    pix = np.sort(np.random.default_rng(21).choice(plane, size=n_cols, replace=False))
+    got = cube.reshape(plane, cfg.nv)[torch.from_numpy(pix).cuda()].cpu().numpy()
+    sub = {k: np.ascontiguousarray(f[k].reshape(cfg.nz, plane)[:, pix]).reshape(cfg.nz, 1, n_cols)
+           for k in ("nH2", "Tgas", "Tdust", "vlos")}
+    cfg_s = cfg.with_(nx=n_cols, ny=1, beam_fwhm_px=0.0, noise_sigma=0.0)
+    ref = Oracle(cfg_s).observe(sub, beam=False, noise=False).reshape(n_cols, cfg.nv)
+    worst = assert_spectra(got, ref, what=mode + " medium, sampled columns")
+    assert bool(torch.isfinite(cube).all())
+    print("%s medium full size: worst sampled pixel at %.3g of tolerance" % (mode, worst))
