@@ -380,6 +380,63 @@ def bench_modes(torch, warmup):
     return out
 
 
+def bench_small_configs(torch, warmup):
+    """BASELINE configs 0, 1 and 4 (tiny, small, batch): whole-path time per cube, and for the batch config the
+    reverse-scan adjoint d(sum w cube)/d n_H2 (K8 + K9) and the 64-cube render rate (cubes rendered back to back on
+    one stream, one context, fields of all cubes resident in HBM)."""
+    from paper_2607_01338_b200 import IrisSO
+    from iris_inputs import weight_cube
+    dev = torch.device("cuda", torch.cuda.current_device())
+    out = {}
+
+    def timed(fn, reps):
+        for _ in range(warmup):
+            fn()
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(reps):
+            fn()
+        b.record()
+        torch.cuda.synchronize()
+        return a.elapsed_time(b) / reps
+
+    for name in ("tiny", "small"):
+        cfg, recipe = make_workload(name)
+        f = make_fields(cfg, recipe)
+        d = [torch.from_numpy(f[k]).to(dev) for k in ("nH2", "Tgas", "Tdust", "vlos")]
+        it = IrisSO(cfg)
+        cube = torch.empty(it.shape_cube, dtype=torch.float32, device=dev)
+        ms = timed(lambda: it.observe(*d, cube=cube), 50)
+        out[name] = {"ms_per_cube": ms, "nominal_updates_per_s": cfg.nx * cfg.ny * cfg.nz * cfg.nv / (ms * 1e-3),
+                     "what": "%dx%dx%d cells, %d channels" % (cfg.nx, cfg.ny, cfg.nz, cfg.nv)}
+        it.close()
+    # batch: 64 independent seeded cubes (8 distinct field sets cycled, all resident), then the adjoint of one
+    cfg, recipe = make_workload("batch", seed=1000)
+    sets = []
+    for i in range(8):
+        c_i, r_i = make_workload("batch", seed=1000 + i)
+        f = make_fields(c_i, r_i)
+        sets.append([torch.from_numpy(f[k]).to(dev) for k in ("nH2", "Tgas", "Tdust", "vlos")])
+    it = IrisSO(cfg)
+    cubes = torch.empty((64,) + tuple(it.shape_cube), dtype=torch.float32, device=dev)
+
+    def render64():
+        for i in range(64):
+            it.observe(*sets[i % 8], cube=cubes[i])
+
+    ms64 = timed(render64, 3)
+    w = torch.from_numpy(weight_cube(cfg)).to(dev)
+    grad = torch.empty((cfg.nz, cfg.ny, cfg.nx), dtype=torch.float32, device=dev)
+    ms_adj = timed(lambda: it.observe_adjoint(*sets[0], w, grad=grad), 10)
+    out["batch"] = {"cubes": 64, "ms_per_64_cubes": ms64, "cubes_per_s": 64e3 / ms64, "adjoint_ms_per_cube": ms_adj,
+                    "nominal_updates_per_s": 64 * cfg.nx * cfg.ny * cfg.nz * cfg.nv / (ms64 * 1e-3),
+                    "what": "64 x (%dx%dx%d cells, %d channels, dust, beam %.3g px, noise %.3g K)"
+                            % (cfg.nx, cfg.ny, cfg.nz, cfg.nv, cfg.beam_fwhm_px, cfg.noise_sigma)}
+    it.close()
+    return out
+
+
 def run_ours(args):
     import torch
     rank, local_rank, world = env_rank()
@@ -409,6 +466,7 @@ def run_ours(args):
             "transfer_nominal_updates_per_s": med["roofline"]["nominal_updates_per_s"]}
     if not args.no_extras and world == 1:
         extra["other_modes_256x256x288_512ch"] = bench_modes(torch, max(args.warmup, 3))
+        extra["other_configs"] = bench_small_configs(torch, max(args.warmup, 3))
     if rank != 0:
         return 0
     cb = None
