@@ -219,11 +219,18 @@ adjoint_march_kernel(MarchConsts mc, AdjointConsts ac, const float* __restrict__
       for (int c = klo + lane; c <= khi; c += 32) xrem[c] = fmaf(a_c, channel_derf(c, c_los, s), xrem[c]);
     __syncwarp();
   }
+  // SQ = sum_c Q[c] and SPD = sum_c P[c] Dt[c] over ALL channels are carried as running sums: a cell changes
+  // them only through the channels of its window, so the sums over the channels OUTSIDE the window (which only
+  // the dust of the cell acts on) are SQ - sum_window Q and SPD - sum_window P Dt -- no pass over all nv channels.
+  float SQ = 0.0f, SPD = 0.0f;
   for (int c = lane; c < nv; c += 32) {
     const float xr = xrem[c], w = wh[c];
     P[c] = w * exp_neg(xr);
-    Q[c] = w * one_minus_exp_neg(xr);
+    const float q = w * one_minus_exp_neg(xr);
+    Q[c] = q;
+    SQ += q;
   }
+  SQ = warp_sum(SQ);
   __syncwarp();
 
   // second march: forward state and closed-form adjoint together
@@ -245,6 +252,7 @@ adjoint_march_kernel(MarchConsts mc, AdjointConsts ac, const float* __restrict__
     const float invG = 1.0f / G, CG = C * G;
     const float sc = DUST ? 0.0f : (a_c != 0.0f ? e_c / a_c : 0.0f) - C;
     float acc_e = 0.0f, acc_a = 0.0f, acc_d = 0.0f, accW = 0.0f, accQ = 0.0f, accPD = 0.0f;
+    float winQ_old = 0.0f, winQ_new = 0.0f, winPD_old = 0.0f, winPD_new = 0.0f;
     if (W > 0) {
       for (int c = klo + lane; c <= khi; c += 32) {
         const float dErf = channel_derf(c, c_los, s);
@@ -252,8 +260,13 @@ adjoint_march_kernel(MarchConsts mc, AdjointConsts ac, const float* __restrict__
         const float xr = xrem[c] - tau_L;
         const float w = wh[c];
         const float Pn = w * exp_neg(xr);
-        xrem[c] = xr; P[c] = Pn; Q[c] = w * one_minus_exp_neg(xr);
+        const float Qn = w * one_minus_exp_neg(xr);
         const float Dto = Dt[c];
+        if (DUST) {
+          winQ_old += Q[c]; winQ_new += Qn;
+          winPD_old = fmaf(P[c], Dto, winPD_old);
+        }
+        xrem[c] = xr; P[c] = Pn; Q[c] = Qn;
         const float Tk = fmaf(Dto, invG, C);
         const float mT = one_minus_exp_neg(tau_T);
         float wT, wpT;
@@ -279,15 +292,22 @@ adjoint_march_kernel(MarchConsts mc, AdjointConsts ac, const float* __restrict__
           Dn = update_nodust(Dto, dErf, a_c, sc);
         }
         Dt[c] = Dn;
+        if (DUST) winPD_new = fmaf(Pn, Dn, winPD_new);
       }
     }
-    if (DUST) {
-      // channels outside the window: only the dust of this cell acts on them
-      for (int c = lane; c < nv; c += 32)
-        if (W == 0 || c < klo || c > khi) { accQ += Q[c]; accPD = fmaf(P[c], Dt[c], accPD); }
-    }
     acc_e = warp_sum(acc_e); acc_a = warp_sum(acc_a);
-    if (DUST) { acc_d = warp_sum(acc_d); accW = warp_sum(accW); accQ = warp_sum(accQ); accPD = warp_sum(accPD); }
+    if (DUST) {
+      acc_d = warp_sum(acc_d); accW = warp_sum(accW);
+      if (W > 0) {
+        winQ_old = warp_sum(winQ_old); winQ_new = warp_sum(winQ_new);
+        winPD_old = warp_sum(winPD_old); winPD_new = warp_sum(winPD_new);
+      }
+      // channels outside the window: only the dust of this cell acts on them
+      accQ = SQ - winQ_old;
+      accPD = SPD - winPD_old;
+      SQ += winQ_new - winQ_old;
+      SPD += winPD_new - winPD_old;
+    }
     if (lane == 0) {
       const int64_t cell = (int64_t)z * npix + pix;
       const float pre = ac.scale * Lam;
@@ -308,6 +328,7 @@ adjoint_march_kernel(MarchConsts mc, AdjointConsts ac, const float* __restrict__
         const float inv = 1.0f / G;
         __syncwarp();
         for (int c = lane; c < nv; c += 32) Dt[c] *= inv;
+        SPD *= inv;
         G = 1.0f;
       }
     }
