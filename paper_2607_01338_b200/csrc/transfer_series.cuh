@@ -262,7 +262,7 @@ transfer_series_kernel(MarchConsts mc, const float* __restrict__ coef, int64_t n
   auto cell_step = [&](const float4& q0, const float4& q1, const float4& q2, const float4& q3) {
     const int kk = __float_as_int(q0.w);
     const int qlo = kk & 0xffff, nq = (int)((unsigned)kk >> 16);
-    const int npass = __reduce_max_sync(0xffffffffu, (nq + LPP - 1) / LPP);   // 0 for an empty window
+    const int npass = (nq + LPP - 1) / LPP;      // pair-passes of THIS pixel (the warp runs the longest of its pixels)
     float CG = 0.0f, Pn = 0.0f, Qn = 0.0f, Rn = 0.0f;
     if (DUST) {
       const float Gn = G * q3.y;
