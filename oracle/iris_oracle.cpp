@@ -15,6 +15,7 @@
 // Units: CGS throughout.  Field arrays are float32 [nz][ny][nx] (x fastest, k = 0 far side) and are
 // widened to double on load; every intermediate and every output is double.
 
+#include <algorithm>
 #include <cmath>
 #include <cstdint>
 #include <cstring>
@@ -708,6 +709,66 @@ void orc_grad_adjoint(const orc_config *c, const float *nH2, const float *Tgas, 
       grad[cell] = g_j0 * dj0 + g_k0 * dk0 + g_ad * dad;
     }
   }
+}
+
+// ---------------------------------------------------------------------------------------------
+// O11  Density tracing ("simple observation", section 5.10): "a projection of column density per
+// unit velocity over dimensions of longitude, latitude, and velocity".  Reading S28: every cell adds its
+// column density n_H2 h to the channel that contains its line-of-sight velocity (channel k covers
+// [v0 + (k - 1/2) dv, v0 + (k + 1/2) dv)), cells outside the band add nothing, and the cube is that sum divided by
+// the channel width: cube[ny][nx][nv] in cm^-2 per (cm/s).
+void orc_density_trace(const orc_config *c, const float *nH2, const float *vlos, double *cube) {
+  const int64_t plane = (int64_t)c->nx * c->ny;
+  for (int64_t i = 0; i < plane * c->nv; ++i) cube[i] = 0.0;
+  for (int k = 0; k < c->nz; ++k)
+    for (int64_t p = 0; p < plane; ++p) {
+      const int64_t cell = (int64_t)k * plane + p;
+      const double pos = ((double)vlos[cell] - c->v0_cms) / c->dv_cms + 0.5;
+      const double fl = std::floor(pos);
+      if (fl < 0.0 || fl >= (double)c->nv) continue;
+      cube[p * c->nv + (int64_t)fl] += (double)nH2[cell] * c->cell_cm / c->dv_cms;
+    }
+}
+
+// O12  Error metrics of section 5.1.  T1, T2: cubes [ny][nx][nv] (l = x, b = y).
+//   TSRE(T1, T2) = 2 |T1 - T2| / (|T1| + |T2|) if min(|T1|, |T2|) > T_min, else 0             Eq. 5.1.1
+//   mean-TSRE_lbv = mean over all voxels; mean-TSRE_lb / _lv = mean over the pixels of the images obtained by
+//   averaging each cube over v / over b first (Eq. 5.1.2 - 5.1.3; reading G8: both arguments of TSRE_lv are l-v
+//   images; reading S29: the means run over ALL elements, inactive ones counting 0, as the equations are written)
+//   TAM(T) = mean of T over the voxels with |T| > T_min                                        Eq. 5.1.4 - 5.1.5
+// out = { TSRE_lbv, TSRE_lb, TSRE_lv, TAM(T1), TAM(T2), max T1, max T2, active(T1), active(T2) }; TAM of a cube with
+// no active voxel is 0.
+static double tsre(double a, double b, double Tmin) {
+  const double fa = std::fabs(a), fb = std::fabs(b);
+  return (fa > Tmin && fb > Tmin) ? 2.0 * std::fabs(a - b) / (fa + fb) : 0.0;
+}
+
+void orc_metrics(int ny, int nx, int nv, const double *T1, const double *T2, double Tmin, double *out) {
+  const int64_t plane = (int64_t)ny * nx, nvox = plane * nv;
+  double s_lbv = 0.0, tam1 = 0.0, tam2 = 0.0, mx1 = -INFINITY, mx2 = -INFINITY;
+  int64_t n1 = 0, n2 = 0;
+  for (int64_t i = 0; i < nvox; ++i) {
+    s_lbv += tsre(T1[i], T2[i], Tmin);
+    if (std::fabs(T1[i]) > Tmin) { tam1 += T1[i]; ++n1; }
+    if (std::fabs(T2[i]) > Tmin) { tam2 += T2[i]; ++n2; }
+    mx1 = std::max(mx1, T1[i]); mx2 = std::max(mx2, T2[i]);
+  }
+  double s_lb = 0.0;
+  for (int64_t p = 0; p < plane; ++p) {
+    double a = 0.0, b = 0.0;
+    for (int v = 0; v < nv; ++v) { a += T1[p * nv + v]; b += T2[p * nv + v]; }
+    s_lb += tsre(a / nv, b / nv, Tmin);
+  }
+  double s_lv = 0.0;
+  for (int x = 0; x < nx; ++x)
+    for (int v = 0; v < nv; ++v) {
+      double a = 0.0, b = 0.0;
+      for (int y = 0; y < ny; ++y) { a += T1[((int64_t)y * nx + x) * nv + v]; b += T2[((int64_t)y * nx + x) * nv + v]; }
+      s_lv += tsre(a / ny, b / ny, Tmin);
+    }
+  out[0] = s_lbv / (double)nvox; out[1] = s_lb / (double)plane; out[2] = s_lv / ((double)nx * nv);
+  out[3] = n1 ? tam1 / (double)n1 : 0.0; out[4] = n2 ? tam2 / (double)n2 : 0.0;
+  out[5] = mx1; out[6] = mx2; out[7] = (double)n1; out[8] = (double)n2;
 }
 
 }  // extern "C"

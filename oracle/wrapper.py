@@ -252,6 +252,25 @@ class Oracle:
         self.lib.orc_observe(self._p(), *[_fp(a) for a in f], C.c_int(mask), _dp(cube))
         return cube
 
+    # -- diagnostics (sections 5.1, 5.10) ---------------------------------------------------------
+    def density_trace(self, fields):
+        """Column density per unit velocity, cube[ny, nx, nv] float64 (cm^-2 per cm/s)."""
+        n, v = _f32(fields["nH2"]).ravel(), _f32(fields["vlos"]).ravel()
+        cube = np.zeros((int(self.s.ny), int(self.s.nx), int(self.s.nv)))
+        self.lib.orc_density_trace(self._p(), _fp(n), _fp(v), _dp(cube))
+        return cube
+
+    def metrics(self, T1, T2, T_min=5e-2):
+        """dict of mean-TSRE (lbv, lb, lv), TAM, maxima and active counts of two cubes [ny, nx, nv]."""
+        a = np.ascontiguousarray(T1, dtype=np.float64)
+        b = np.ascontiguousarray(T2, dtype=np.float64)
+        assert a.shape == b.shape and a.ndim == 3
+        out = np.zeros(9)
+        self.lib.orc_metrics(C.c_int(a.shape[0]), C.c_int(a.shape[1]), C.c_int(a.shape[2]), _dp(a), _dp(b),
+                             C.c_double(T_min), _dp(out))
+        keys = ("tsre_lbv", "tsre_lb", "tsre_lv", "tam1", "tam2", "max1", "max2", "active1", "active2")
+        return dict(zip(keys, out.tolist()))
+
     # -- gradient --------------------------------------------------------------------------------
     def grad_fd(self, fields, what, cells, eps=1e-4):
         self._omp()

@@ -234,3 +234,74 @@ def test_fine_grid_undersampling_failure_mode():
     fine = march(cfg.with_(subsample=63), f)[2]
     assert np.max(np.abs(coarse - I_int)) / line > 0.2
     assert np.max(np.abs(fine - I_int)) / line < 2e-4
+
+
+# ------------------------------------------------------------------------------------------------
+# diagnostics: density tracing (section 5.10) and the error metrics of section 5.1
+def test_density_trace_conserves_column_density_and_bins_by_velocity():
+    cfg, r = make_workload("tiny", n=6, nv=64)
+    f = make_fields(cfg, r)
+    f["vlos"] = (0.4 * f["vlos"]).astype(np.float32)
+    o = Oracle(cfg)
+    cube = o.density_trace(f)
+    plane = cfg.nx * cfg.ny
+    n = f["nH2"].reshape(cfg.nz, plane).astype(np.float64)
+    v = f["vlos"].reshape(cfg.nz, plane).astype(np.float64)
+    lo, hi = cfg.v0_cms - cfg.dv_cms / 2, cfg.v0_cms + (cfg.nv - 0.5) * cfg.dv_cms
+    inband = (v >= lo) & (v < hi)
+    assert inband.mean() > 0.2 and (~inband).any()
+    # total column density of the in-band cells: sum_v cube dv = sum_z n h
+    assert np.allclose(cube.reshape(plane, cfg.nv).sum(axis=1) * cfg.dv_cms, (n * inband).sum(axis=0) * cfg.cell_cm, rtol=1e-12)
+    # against numpy's histogram of one column
+    p = int(np.argmax(inband.sum(axis=0)))
+    edges = lo + cfg.dv_cms * np.arange(cfg.nv + 1)
+    hist, _ = np.histogram(v[:, p], bins=edges, weights=n[:, p] * cfg.cell_cm / cfg.dv_cms)
+    assert np.allclose(cube.reshape(plane, cfg.nv)[p], hist, rtol=1e-12)
+
+
+def test_density_trace_is_the_thin_observation_of_an_isothermal_cold_cloud():
+    """Section 5.10 / Eq. 5.10.1: with one temperature, no dust and no absorption the optically thin line cube is
+    proportional to the density-tracing cube.  Lines much narrower than a channel and velocities at channel centres make
+    the channel-integrated profile an indicator of the channel, so the proportionality is exact: the constant is
+    (h nu0 / 4 pi) X x_u(T) A_ul dv / dnu_W  with x_u from the LTE limit (high density)."""
+    cfg, r = make_workload("tiny", n=4, nv=32)
+    cfg = cfg.with_(transfer_mode=2, microturb_cms=0.0, dv_cms=4.0 * KMS, v0_cms=-62.0 * KMS, subtract_continuum=True, out_unit=0)
+    rng = np.random.default_rng(3)
+    shape = (cfg.nz, cfg.ny, cfg.nx)
+    f = dict(nH2=(1e12 * rng.uniform(0.5, 2.0, shape)).astype(np.float32), Tgas=np.full(shape, 15.0, np.float32),
+             Tdust=np.full(shape, 15.0, np.float32),
+             vlos=(cfg.v0_cms + cfg.dv_cms * rng.integers(0, cfg.nv, shape)).astype(np.float32))
+    o = Oracle(cfg)
+    line = o.observe(f, beam=False, noise=False)              # I_T - I_C in cgs
+    trace = o.density_trace(f)
+    x = cfg.weight * np.exp(-cfg.energy_K / 15.0)
+    x /= x.sum()
+    A = cfg.einstein_A[cfg.line_upper, cfg.line_lower]
+    const = H * cfg.nu0_Hz / (4 * np.pi) * cfg.abundance * x[cfg.line_upper] * A * cfg.dv_cms / (cfg.nu0_Hz * cfg.dv_cms / CL)
+    assert trace.max() > 0
+    assert np.allclose(line, const * trace, rtol=2e-5, atol=1e-12 * (const * trace).max())
+
+
+def test_tsre_and_tam_definitions():
+    o = Oracle(make_workload("tiny", n=2, nv=4)[0])
+    rng = np.random.default_rng(0)
+    T1 = rng.normal(0.0, 0.2, (5, 7, 6))
+    T2 = T1 * rng.uniform(0.5, 1.5, T1.shape) + rng.normal(0.0, 0.02, T1.shape)
+    m = o.metrics(T1, T2)
+    Tmin = 5e-2
+    act = (np.abs(T1) > Tmin) & (np.abs(T2) > Tmin)
+    ts = np.where(act, 2 * np.abs(T1 - T2) / (np.abs(T1) + np.abs(T2) + 1e-300), 0.0)
+    assert m["tsre_lbv"] == pytest.approx(ts.mean(), rel=1e-12)
+    def img(a, b):
+        ok = (np.abs(a) > Tmin) & (np.abs(b) > Tmin)
+        return np.where(ok, 2 * np.abs(a - b) / (np.abs(a) + np.abs(b) + 1e-300), 0.0).mean()
+    assert m["tsre_lb"] == pytest.approx(img(T1.mean(axis=2), T2.mean(axis=2)), rel=1e-12)
+    assert m["tsre_lv"] == pytest.approx(img(T1.mean(axis=0), T2.mean(axis=0)), rel=1e-12)
+    assert m["tam1"] == pytest.approx(T1[np.abs(T1) > Tmin].mean(), rel=1e-12) and m["active1"] == (np.abs(T1) > Tmin).sum()
+    assert m["max2"] == T2.max()
+    # properties the paper states (PAPER.md:868): identical cubes -> 0; opposite signs -> 200 %; capped at 200 %
+    assert o.metrics(T1, T1)["tsre_lbv"] == 0.0
+    big = np.full((2, 2, 2), 1.0)
+    assert o.metrics(big, -big)["tsre_lbv"] == pytest.approx(2.0)
+    assert o.metrics(big, 1e9 * big)["tsre_lbv"] == pytest.approx(2.0, rel=1e-8)
+    assert o.metrics(big, 1e-3 * big)["tsre_lbv"] == 0.0 and o.metrics(1e-3 * big, big)["tam1"] == 0.0
