@@ -192,6 +192,20 @@ iris_so_status iris_so_beam(iris_so_ctx *ctx, const float *d_in, float *d_out, f
 /* K7: d_cube += gamma (mu + sigma z), z = Box-Muller of Philox4x32-10(key = seed, counter = voxel index). */
 iris_so_status iris_so_noise(iris_so_ctx *ctx, float *d_cube, void *cuda_stream);
 
+/* Diagnostics of PAPER.md section 5.
+ * Density tracing ("simple observation", section 5.10): d_cube [ny][nx][nv] = column density per
+ * unit velocity, cm^-2 per (cm/s): every cell adds n_H2 * cell_cm / dv_cms to the channel that contains its v_los
+ * (channel k covers [v0 + (k - 1/2) dv, v0 + (k + 1/2) dv)); cells outside the band add nothing.  Asynchronous. */
+iris_so_status iris_so_density_trace(iris_so_ctx *ctx, const float *d_nH2, const float *d_vlos, float *d_cube,
+                                     void *cuda_stream);
+/* Error metrics of section 5.1 (Eq. 5.1.1 - 5.1.5) of two cubes [ny][nx][nv] (l = x, b = y):
+ * h_out[9] = { mean-TSRE over voxels, mean-TSRE of the l-b images (cube means over v), mean-TSRE of the l-v images
+ * (cube means over y), TAM(T1), TAM(T2), max T1, max T2, active voxels of T1, of T2 }; TSRE counts 0 where either
+ * |T| <= T_min, the means run over all elements, TAM of a cube without active voxels is 0.  T_min <= 0 selects the
+ * paper's 5e-2 K.  Synchronises the stream. */
+iris_so_status iris_so_metrics(iris_so_ctx *ctx, const float *d_T1, const float *d_T2, double T_min, double *h_out,
+                               void *cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -16,6 +16,7 @@ DECLARED_SYMBOLS = (
     "iris_so_launch_count", "iris_so_scratch_bytes", "iris_so_levelpop", "iris_so_transfer", "iris_so_observe",
     "iris_so_observe_stages", "iris_so_observe_host", "iris_so_observe_adjoint", "iris_so_beam", "iris_so_noise",
     "iris_so_profile", "iris_so_profile_read", "iris_so_transfer_work", "iris_so_transfer_kernel",
+    "iris_so_density_trace", "iris_so_metrics",
 )
 STAGES = {"cell": 0, "transfer": 1, "beam": 2, "noise": 3, "adjoint": 4}
 
@@ -101,6 +102,10 @@ def load_library():
     lib.iris_so_transfer_kernel.argtypes = [vp]
     lib.iris_so_transfer_work.restype = st
     lib.iris_so_transfer_work.argtypes = [vp, C.POINTER(C.c_uint64), vp]
+    lib.iris_so_density_trace.restype = st
+    lib.iris_so_density_trace.argtypes = [vp, fp, fp, fp, vp]
+    lib.iris_so_metrics.restype = st
+    lib.iris_so_metrics.argtypes = [vp, fp, fp, C.c_double, C.POINTER(C.c_double), vp]
     _lib = lib
     return lib
 
@@ -285,3 +290,21 @@ class IrisSO:
     def noise(self, cube):
         self._check(self.lib.iris_so_noise(self._h, self._dev(cube, self.n_vox, "cube"), self._stream()))
         return cube
+
+    def density_trace(self, nH2, vlos, cube=None):
+        """Column density per unit velocity (section 5.10), float32 CUDA tensor [ny, nx, nv]."""
+        import torch
+        if cube is None:
+            cube = torch.empty(self.shape_cube, dtype=torch.float32, device=nH2.device)
+        self._check(self.lib.iris_so_density_trace(self._h, self._dev(nH2, self.n_cells, "nH2"),
+                                                   self._dev(vlos, self.n_cells, "vlos"),
+                                                   self._dev(cube, self.n_vox, "cube"), self._stream()))
+        return cube
+
+    def metrics(self, T1, T2, T_min=5e-2):
+        """Section 5.1 metrics of two cubes [ny, nx, nv]: dict of mean-TSRE (lbv, lb, lv), TAM, maxima, active counts."""
+        out = (C.c_double * 9)()
+        self._check(self.lib.iris_so_metrics(self._h, self._dev(T1, self.n_vox, "T1"), self._dev(T2, self.n_vox, "T2"),
+                                             C.c_double(T_min), out, self._stream()))
+        keys = ("tsre_lbv", "tsre_lb", "tsre_lv", "tam1", "tam2", "max1", "max2", "active1", "active2")
+        return dict(zip(keys, [float(v) for v in out]))

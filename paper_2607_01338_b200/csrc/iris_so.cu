@@ -20,6 +20,7 @@
 #include "transfer_series.cuh"
 #include "transfer_modes.cuh"
 #include "adjoint_kernels.cuh"
+#include "diagnostics.cuh"
 
 namespace {
 
@@ -59,6 +60,7 @@ struct iris_so_ctx {
   std::vector<ProfRec> recs;
   std::vector<cudaEvent_t> event_pool;
   unsigned long long* d_counter = nullptr;
+  double* d_metrics = nullptr;
 };
 
 namespace {
@@ -460,7 +462,7 @@ iris_so_status iris_so_create(const iris_so_config* cfg, iris_so_ctx** out) {
 
 void iris_so_destroy(iris_so_ctx* ctx) {
   if (!ctx) return;
-  cudaFree(ctx->d_coef); cudaFree(ctx->d_tmp); cudaFree(ctx->d_stage); cudaFree(ctx->d_adj); cudaFree(ctx->d_counter);
+  cudaFree(ctx->d_coef); cudaFree(ctx->d_tmp); cudaFree(ctx->d_stage); cudaFree(ctx->d_adj); cudaFree(ctx->d_counter); cudaFree(ctx->d_metrics);
   prof_reset(ctx);
   for (cudaEvent_t e : ctx->event_pool) cudaEventDestroy(e);
   delete ctx;
@@ -617,6 +619,49 @@ iris_so_status iris_so_observe_adjoint(iris_so_ctx* ctx, const float* d_nH2, con
   cudaError_t e = iris::launch_adjoint(ctx->mc, ctx->ac, ctx->lc, c.n_levels, ctx->band, ctx->d_coef, dcoef, ctx->ncell, (int)ctx->npix,
                                        c.nz, c.nv, c.dust_on != 0, d_nH2, d_Tgas, what, d_grad, st, &ctx->launches);
   if (e != cudaSuccess) return cuda_fail(ctx, e, "launch of adjoint kernels");
+  return IRIS_SO_OK;
+}
+
+iris_so_status iris_so_density_trace(iris_so_ctx* ctx, const float* d_nH2, const float* d_vlos, float* d_cube, void* stream) {
+  if (!ctx) return IRIS_SO_EINVAL;
+  if (!d_nH2 || !d_vlos || !d_cube) return fail(ctx, IRIS_SO_EINVAL, "iris_so_density_trace: NULL pointer");
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const iris_so_config& c = ctx->cfg;
+  cudaError_t e = cudaMemsetAsync(d_cube, 0, sizeof(float) * (size_t)ctx->nvox, st);
+  if (e != cudaSuccess) return cuda_fail(ctx, e, "cudaMemsetAsync(cube)");
+  iris::density_trace_kernel<<<(unsigned)((ctx->npix + 127) / 128), 128, 0, st>>>(
+      d_nH2, d_vlos, (int)ctx->npix, c.nz, c.nv, c.v0_cms, c.dv_cms, (float)(c.cell_cm / c.dv_cms), d_cube);
+  IRIS_CHECK_LAUNCH(ctx, "density_trace_kernel");
+  return IRIS_SO_OK;
+}
+
+iris_so_status iris_so_metrics(iris_so_ctx* ctx, const float* d_T1, const float* d_T2, double T_min, double* h_out, void* stream) {
+  if (!ctx) return IRIS_SO_EINVAL;
+  if (!d_T1 || !d_T2 || !h_out) return fail(ctx, IRIS_SO_EINVAL, "iris_so_metrics: NULL pointer");
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const iris_so_config& c = ctx->cfg;
+  if (!(T_min > 0.0)) T_min = 5.0e-2;
+  cudaError_t e;
+  if (!ctx->d_metrics && (e = cudaMalloc(reinterpret_cast<void**>(&ctx->d_metrics), 9 * sizeof(double))) != cudaSuccess)
+    return cuda_fail(ctx, e, "cudaMalloc(metrics)");
+  double init[9] = {0, 0, 0, 0, 0, -INFINITY, -INFINITY, 0, 0};
+  if ((e = cudaMemcpyAsync(ctx->d_metrics, init, sizeof init, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_fail(ctx, e, "H2D");
+  if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(ctx, e, "cudaStreamSynchronize");   // init is a stack array
+  iris::metrics_pixel_kernel<<<(unsigned)((ctx->npix * 32 + 255) / 256), 256, 0, st>>>(d_T1, d_T2, (int)ctx->npix, c.nv, T_min,
+                                                                                   ctx->d_metrics);
+  IRIS_CHECK_LAUNCH(ctx, "metrics_pixel_kernel");
+  const int64_t nlv = (int64_t)c.nx * c.nv;
+  iris::metrics_lv_kernel<<<(unsigned)((nlv + 255) / 256), 256, 0, st>>>(d_T1, d_T2, c.ny, c.nx, c.nv, T_min, ctx->d_metrics);
+  IRIS_CHECK_LAUNCH(ctx, "metrics_lv_kernel");
+  double r[9];
+  if ((e = cudaMemcpyAsync(r, ctx->d_metrics, sizeof r, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(ctx, e, "D2H");
+  if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(ctx, e, "cudaStreamSynchronize");
+  h_out[0] = r[0] / (double)ctx->nvox;
+  h_out[1] = r[1] / (double)ctx->npix;
+  h_out[2] = r[2] / (double)nlv;
+  h_out[3] = r[7] > 0.0 ? r[3] / r[7] : 0.0;
+  h_out[4] = r[8] > 0.0 ? r[4] / r[8] : 0.0;
+  h_out[5] = r[5]; h_out[6] = r[6]; h_out[7] = r[7]; h_out[8] = r[8];
   return IRIS_SO_OK;
 }
 

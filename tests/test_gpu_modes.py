@@ -157,3 +157,36 @@ def test_modes_full_size_medium_sampled(mode):
     worst = assert_spectra(got, ref, what=mode + " medium, sampled columns")
     assert bool(torch.isfinite(cube).all())
     print("%s medium full size: worst sampled pixel at %.3g of tolerance" % (mode, worst))
+
+
+# ------------------------------------------------------------------------------------------------
+# diagnostics of section 5: density tracing and the TSRE / TAM metrics
+@pytest.mark.parametrize("shape", [dict(n=24, nv=96), dict(nx=37, ny=5, nz=19, nv=45), dict(nx=1, ny=1, nz=1, nv=1)])
+def test_density_trace_matches_oracle(shape):
+    from paper_2607_01338_b200 import IrisSO
+    cfg, r = make_workload("small", **shape)
+    f = make_fields(cfg, r)
+    f["vlos"] = (0.5 * f["vlos"]).astype(np.float32)
+    got = IrisSO(cfg).density_trace(dev(f["nH2"]), dev(f["vlos"])).cpu().numpy().astype(np.float64)
+    ref = Oracle(cfg).density_trace(f)
+    # the channel of every cell is decided identically (both in double); the sums differ by fp32 accumulation only
+    assert np.array_equal(got > 0, ref > 0)
+    assert np.allclose(got, ref, rtol=2e-5, atol=0)
+
+
+def test_metrics_match_oracle():
+    from paper_2607_01338_b200 import IrisSO
+    cfg, r = make_workload("small", n=24, nv=80)
+    f = make_fields(cfg, r)
+    f["vlos"] = (0.3 * f["vlos"]).astype(np.float32)
+    it = IrisSO(cfg)
+    d = dev_fields(f)
+    T1 = it.observe(*d)
+    T2 = IrisSO(cfg.with_(transfer_mode=1)).observe(*d)            # selectively thin against thick
+    got = it.metrics(T1, T2)
+    ref = Oracle(cfg).metrics(T1.cpu().numpy(), T2.cpu().numpy())
+    assert ref["active1"] > 100 and ref["tsre_lbv"] > 0
+    for k in ref:
+        assert got[k] == pytest.approx(ref[k], rel=1e-9, abs=1e-12), k
+    same = it.metrics(T1, T1)
+    assert same["tsre_lbv"] == 0.0 and same["tsre_lv"] == 0.0 and same["tam1"] == same["tam2"]
