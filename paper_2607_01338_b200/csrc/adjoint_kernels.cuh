@@ -38,11 +38,9 @@ struct AdjointConsts {
 template <int N, int BW>
 __device__ __forceinline__ void level_fractions_grad(const LevelConsts& lc, float n, float T, float (&x)[N], float (&y)[N]) {
   float R[N][N];
-  const float invT = rcp_approx(T);
   const float kf = n * exp2f(lc.Texp * log2f(T * lc.inv_Tref));
   float q[N];
-#pragma unroll
-  for (int i = 1; i < N; ++i) q[i] = expf(-lc.dE_adj[i] * invT);
+  boltzmann_adjacent<N>(lc, T, q);
 #pragma unroll
   for (int u = 1; u < N; ++u) {
     float bz = 1.0f;
@@ -50,9 +48,9 @@ __device__ __forceinline__ void level_fractions_grad(const LevelConsts& lc, floa
     for (int l = u - 1; l >= 0; --l) {
       if (u - l > BW) continue;
       bz *= q[l + 1];
-      const int p = pair_index(u, l);
-      R[u][l] = fmaf(kf, lc.coll[p], lc.rad_down[p]);
-      R[l][u] = fmaf(kf * bz, lc.coll_gr[p], lc.rad_up[p]);
+      const float4 pr = lc.pr[pair_index(u, l)];
+      R[u][l] = fmaf(kf, pr.x, pr.y);
+      R[l][u] = fmaf(kf * bz, pr.z, pr.w);
     }
   }
   float inv[N];
@@ -98,8 +96,8 @@ __device__ __forceinline__ void level_fractions_grad(const LevelConsts& lc, floa
     for (int l = u - 1; l >= 0; --l) {
       if (u - l > BW) continue;
       bz *= q[l + 1];
-      const int p = pair_index(u, l);
-      const float f = x[u] * (kf * lc.coll[p]) - x[l] * (kf * bz * lc.coll_gr[p]);   // net flow u -> l
+      const float4 pr = lc.pr[pair_index(u, l)];
+      const float f = x[u] * (kf * pr.x) - x[l] * (kf * bz * pr.z);   // net flow u -> l
       b[u] += f;
       b[l] -= f;
     }

@@ -32,14 +32,28 @@ constexpr int kBandNarrow = 2;
 __host__ __device__ constexpr int pair_index(int u, int l) { return u * (u - 1) / 2 + l; }
 
 struct LevelConsts {
-  float dE_adj[kMaxLevels];     // (E_i - E_{i-1}) / k  [K], i >= 1
-  float rad_down[kMaxPairs];    // A_ul + B_ul J_ul = A_ul (1 + n_gamma)
-  float rad_up[kMaxPairs];      // B_lu J_ul = (g_u / g_l) A_ul n_gamma
-  float coll[kMaxPairs];        // K_ul(T_ref)
-  float coll_gr[kMaxPairs];     // K_ul(T_ref) g_u / g_l
+  float ndE2[kMaxLevels];       // -(E_i - E_{i-1}) / k * log2(e)  [K], i >= 1: Boltzmann factor = 2^(ndE2 / T)
+  // per pair (u > l), packed so that one 16-byte constant load feeds both rate FMAs:
+  //   x = K_ul(T_ref), y = A_ul + B_ul J_ul = A_ul (1 + n_gamma), z = K_ul(T_ref) g_u / g_l, w = B_lu J_ul
+  float4 pr[kMaxPairs];
   float inv_Tref, Texp;
   float rate_scale;             // every rate above has been multiplied by this (1 / largest Einstein A)
 };
+
+// Boltzmann factors of adjacent levels, q[i] = exp(-(E_i - E_{i-1}) / T), i >= 1: one MUFU.EX2 each.  The product
+// ndE2 / T is formed with its rounding error (FMA residual) and the error is applied to first order, so the factor
+// keeps ~2 ulp even where |ndE2 / T| ~ 15 (T = 5 K), where the rounding of the argument alone would cost 1e-6.
+template <int N>
+__device__ __forceinline__ void boltzmann_adjacent(const LevelConsts& lc, float T, float (&q)[N]) {
+  const float invT = 1.0f / T;
+#pragma unroll
+  for (int i = 1; i < N; ++i) {
+    const float t = lc.ndE2[i] * invT;
+    const float r = fmaf(lc.ndE2[i], invT, -t);
+    const float e = ex2_approx(t);
+    q[i] = fmaf(e * 0.6931471805599453f, r, e);
+  }
+}
 
 struct CoefConsts {
   int upper, lower;
@@ -51,6 +65,7 @@ struct CoefConsts {
   float dv, inv_dv, v0;
   float T_inf;
   int dust_on;
+  float pick_upper[kMaxLevels], pick_lower[kMaxLevels];   // one-hot vectors of the line's levels
 };
 
 // Level fractions of one cell.  N is a template parameter so that the rate matrix lives in registers.
@@ -62,14 +77,13 @@ struct CoefConsts {
 // largest Einstein A (LevelConsts::rate_scale), which keeps the pivots far from the fp32 denormal range so that
 // the reciprocals can be MUFU.RCP (1 ulp, flush-to-zero).
 template <int N, int BW>
-__device__ __forceinline__ void level_fractions(const LevelConsts& lc, float n, float T, float (&x)[N]) {
+__device__ __forceinline__ void level_fractions(const LevelConsts& lc, float n, float T, float (&x)[N],
+                                                float* inv_tot = nullptr) {
   float R[N][N];   // R[i][j]: rate i -> j (i != j); only |i - j| <= BW is touched
-  const float invT = rcp_approx(T);
   // n * (T / T_ref)^p
   const float kf = n * exp2f(lc.Texp * log2f(T * lc.inv_Tref));
   float q[N];      // Boltzmann factors of adjacent levels, exp(-(E_i - E_{i-1}) / T)
-#pragma unroll
-  for (int i = 1; i < N; ++i) q[i] = expf(-lc.dE_adj[i] * invT);
+  boltzmann_adjacent<N>(lc, T, q);
 #pragma unroll
   for (int u = 1; u < N; ++u) {
     float bz = 1.0f;
@@ -77,9 +91,9 @@ __device__ __forceinline__ void level_fractions(const LevelConsts& lc, float n, 
     for (int l = u - 1; l >= 0; --l) {
       if (u - l > BW) continue;
       bz *= q[l + 1];                                   // exp(-(E_u - E_l) / T), Eq. 3.7.2
-      const int p = pair_index(u, l);
-      R[u][l] = fmaf(kf, lc.coll[p], lc.rad_down[p]);
-      R[l][u] = fmaf(kf * bz, lc.coll_gr[p], lc.rad_up[p]);
+      const float4 pr = lc.pr[pair_index(u, l)];
+      R[u][l] = fmaf(kf, pr.x, pr.y);
+      R[l][u] = fmaf(kf * bz, pr.z, pr.w);
     }
   }
   // GTH elimination of states N-1 .. 1
@@ -112,6 +126,7 @@ __device__ __forceinline__ void level_fractions(const LevelConsts& lc, float n, 
     tot += s;
   }
   const float inv = rcp_approx(tot);
+  if (inv_tot != nullptr) { *inv_tot = inv; return; }      // caller scales the levels it needs
 #pragma unroll
   for (int j = 0; j < N; ++j) x[j] *= inv;
 }
@@ -151,14 +166,17 @@ __global__ void __launch_bounds__(128) cellcoef_kernel(LevelConsts lc, CoefConst
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= ncell) return;
   const float n = nH2[i], T = Tgas[i];
-  float x[N];
-  level_fractions<N, BW>(lc, n, T, x);
+  float x[N], inv;
+  level_fractions<N, BW>(lc, n, T, x, &inv);      // unnormalised fractions and 1 / their sum
+  // the two levels of the line, picked with one-hot constant vectors (static indexing keeps x[] in registers; a
+  // dot product with constant operands is half the instructions of N compare-select pairs)
   float xu = 0.0f, xl = 0.0f;
 #pragma unroll
-  for (int l = 0; l < N; ++l) {       // static indexing keeps x[] in registers
-    if (l == cc.upper) xu = x[l];
-    if (l == cc.lower) xl = x[l];
+  for (int l = 0; l < N; ++l) {
+    xu = fmaf(x[l], cc.pick_upper[l], xu);
+    xl = fmaf(x[l], cc.pick_lower[l], xl);
   }
+  xu *= inv; xl *= inv;
   float o[6];
   cell_coefficients(cc, n, T, Tdust[i], vlos[i], xu, xl, o);
 #pragma unroll

@@ -196,7 +196,7 @@ void fold_constants(iris_so_ctx* ctx) {
   for (int u = 1; u < N; ++u)
     for (int l = 0; l < u; ++l)
       if ((ctx->A[u * N + l] != 0.0 || ctx->Kd[u * N + l] != 0.0) && u - l > ctx->band) ctx->band = u - l;
-  for (int i = 1; i < N; ++i) lc.dE_adj[i] = (float)(ctx->energy[i] - ctx->energy[i - 1]);
+  for (int i = 1; i < N; ++i) lc.ndE2[i] = (float)(-(ctx->energy[i] - ctx->energy[i - 1]) * 1.4426950408889634);
   double Amax = 0.0;
   for (double a : ctx->A) Amax = std::max(Amax, a);
   const double rs = Amax > 0.0 ? 1.0 / Amax : 1.0;              // common rate scale (fractions are invariant)
@@ -211,10 +211,10 @@ void fold_constants(iris_so_ctx* ctx) {
         const double hnu_k = ctx->energy[u] - ctx->energy[l];   // h nu_ul / k
         ngam = 1.0 / std::expm1(hnu_k / c.T_bar);               // photon occupation of B_nu(T_bar), Eq. 3.6.2
       }
-      lc.rad_down[p] = (float)(rs * A * (1.0 + ngam));          // A_ul + B_ul J
-      lc.rad_up[p] = (float)(rs * gr * A * ngam);               // B_lu J
-      lc.coll[p] = (float)(rs * K);
-      lc.coll_gr[p] = (float)(rs * K * gr);
+      lc.pr[p].x = (float)(rs * K);                             // K_ul(T_ref)
+      lc.pr[p].y = (float)(rs * A * (1.0 + ngam));              // A_ul + B_ul J
+      lc.pr[p].z = (float)(rs * K * gr);                        // K_ul(T_ref) g_u / g_l
+      lc.pr[p].w = (float)(rs * gr * A * ngam);                 // B_lu J
     }
   lc.inv_Tref = (float)(1.0 / c.coll_T_ref);
   lc.Texp = (float)c.coll_T_exp;
@@ -228,6 +228,7 @@ void fold_constants(iris_so_ctx* ctx) {
   const double pref = H_PLANCK * nu / (4.0 * PI) * c.abundance * c.cell_cm / (2.0 * dnuW);
   iris::CoefConsts& cc = ctx->cc;
   cc.upper = u; cc.lower = l; cc.gr = (float)gr;
+  for (int i = 0; i < iris::kMaxLevels; ++i) { cc.pick_upper[i] = i == u ? 1.0f : 0.0f; cc.pick_lower[i] = i == l ? 1.0f : 0.0f; }
   cc.c_e = (float)(KRJ * pref * A);
   cc.c_a = (float)(pref * Bul);
   cc.c_d = c.dust_on ? (float)(c.kappa_gas_cm2_g * c.mass_per_H2_g * c.cell_cm) : 0.0f;
