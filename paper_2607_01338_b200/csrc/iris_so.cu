@@ -61,6 +61,8 @@ struct iris_so_ctx {
   std::vector<cudaEvent_t> event_pool;
   unsigned long long* d_counter = nullptr;
   double* d_metrics = nullptr;
+  cudaStream_t s_in = nullptr, s_out = nullptr;      // copy streams of the host-buffer path
+  std::vector<cudaEvent_t> slab_events;
 };
 
 namespace {
@@ -464,6 +466,9 @@ iris_so_status iris_so_create(const iris_so_config* cfg, iris_so_ctx** out) {
 void iris_so_destroy(iris_so_ctx* ctx) {
   if (!ctx) return;
   cudaFree(ctx->d_coef); cudaFree(ctx->d_tmp); cudaFree(ctx->d_stage); cudaFree(ctx->d_adj); cudaFree(ctx->d_counter); cudaFree(ctx->d_metrics);
+  if (ctx->s_in) cudaStreamDestroy(ctx->s_in);
+  if (ctx->s_out) cudaStreamDestroy(ctx->s_out);
+  for (auto ev : ctx->slab_events) cudaEventDestroy(ev);
   prof_reset(ctx);
   for (cudaEvent_t e : ctx->event_pool) cudaEventDestroy(e);
   delete ctx;
@@ -513,23 +518,94 @@ iris_so_status iris_so_observe(iris_so_ctx* ctx, const float* d_nH2, const float
   return iris_so_observe_stages(ctx, d_nH2, d_Tgas, d_Tdust, d_vlos, 3, d_cube, stream);
 }
 
+// Host-buffer path.  Pixel columns are independent up to the beam, so the sky plane is cut into slabs of rows and
+// the three legs are pipelined on three streams: H2D of slab k+1 (four strided field copies into a compact
+// [nz][rows][nx] staging slab), K1-K5 of slab k on the caller's stream, D2H of the finished cube rows of slab k-1
+// (PCIe is full duplex).  With a beam or noise configured the cube stays on the device until every slab is done, the
+// post-processing runs on the whole cube and one D2H follows.
 iris_so_status iris_so_observe_host(iris_so_ctx* ctx, const float* h_nH2, const float* h_Tgas, const float* h_Tdust,
                                     const float* h_vlos, float* h_cube, void* stream) {
   if (!ctx) return IRIS_SO_EINVAL;
   if (!h_nH2 || !h_Tgas || !h_Tdust || !h_vlos || !h_cube) return fail(ctx, IRIS_SO_EINVAL, "iris_so_observe_host: NULL pointer");
   cudaStream_t st = static_cast<cudaStream_t>(stream);
-  const size_t fb = sizeof(float) * (size_t)ctx->ncell, cb = sizeof(float) * (size_t)ctx->nvox;
+  const iris_so_config cfg0 = ctx->cfg;
+  const int64_t ncell0 = ctx->ncell, npix0 = ctx->npix, nvox0 = ctx->nvox;
+  const size_t fb = sizeof(float) * (size_t)ncell0, cb = sizeof(float) * (size_t)nvox0;
   iris_so_status s = ensure(ctx, &ctx->d_stage, 4 * fb + cb, "cudaMalloc(host-path staging)");
   if (s != IRIS_SO_OK) return s;
-  float* f[4] = {ctx->d_stage, ctx->d_stage + ctx->ncell, ctx->d_stage + 2 * ctx->ncell, ctx->d_stage + 3 * ctx->ncell};
-  float* d_cube = ctx->d_stage + 4 * ctx->ncell;
+  float* f[4] = {ctx->d_stage, ctx->d_stage + ncell0, ctx->d_stage + 2 * ncell0, ctx->d_stage + 3 * ncell0};
+  float* d_cube = ctx->d_stage + 4 * ncell0;
   const float* h[4] = {h_nH2, h_Tgas, h_Tdust, h_vlos};
   cudaError_t e;
-  for (int i = 0; i < 4; ++i)
-    if ((e = cudaMemcpyAsync(f[i], h[i], fb, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_fail(ctx, e, "H2D copy");
-  if ((s = iris_so_observe(ctx, f[0], f[1], f[2], f[3], d_cube, stream)) != IRIS_SO_OK) return s;
-  if ((e = cudaMemcpyAsync(h_cube, d_cube, cb, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(ctx, e, "D2H copy");
-  if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(ctx, e, "cudaStreamSynchronize");
+  // slab height: about 48 MB of field data per slab, at least 3 slabs, else one shot
+  const size_t row_bytes = (size_t)cfg0.nz * cfg0.nx * sizeof(float) * 4;
+  int rows = (int)std::max<size_t>(1, (48u << 20) / std::max<size_t>(row_bytes, 1));
+  rows = std::min(rows, cfg0.ny);
+  const int nslab = (cfg0.ny + rows - 1) / rows;
+  if (nslab < 3) {
+    for (int i = 0; i < 4; ++i)
+      if ((e = cudaMemcpyAsync(f[i], h[i], fb, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_fail(ctx, e, "H2D copy");
+    if ((s = iris_so_observe(ctx, f[0], f[1], f[2], f[3], d_cube, stream)) != IRIS_SO_OK) return s;
+    if ((e = cudaMemcpyAsync(h_cube, d_cube, cb, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(ctx, e, "D2H copy");
+    if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(ctx, e, "cudaStreamSynchronize");
+    return IRIS_SO_OK;
+  }
+  if ((s = ensure(ctx, &ctx->d_coef, sizeof(float) * 6 * (size_t)ncell0, "cudaMalloc(coefficient planes)")) != IRIS_SO_OK) return s;
+  if (!ctx->s_in) {
+    if ((e = cudaStreamCreateWithFlags(&ctx->s_in, cudaStreamNonBlocking)) != cudaSuccess) return cuda_fail(ctx, e, "cudaStreamCreate");
+    if ((e = cudaStreamCreateWithFlags(&ctx->s_out, cudaStreamNonBlocking)) != cudaSuccess) return cuda_fail(ctx, e, "cudaStreamCreate");
+  }
+  while ((int)ctx->slab_events.size() < 2 * nslab + 1) {
+    cudaEvent_t ev;
+    if ((e = cudaEventCreateWithFlags(&ev, cudaEventDisableTiming)) != cudaSuccess) return cuda_fail(ctx, e, "cudaEventCreate");
+    ctx->slab_events.push_back(ev);
+  }
+  const bool post = (cfg0.beam_fwhm_px > 0.0) || ctx->nc.on;
+  cudaEvent_t ev_start = ctx->slab_events[2 * nslab];
+  iris_so_status rs = IRIS_SO_OK;
+  cudaError_t ce = cudaSuccess;
+  const char* what = "";
+#define HOSTPATH_CU(call, text) do { if (ce == cudaSuccess && rs == IRIS_SO_OK) { ce = (call); if (ce != cudaSuccess) what = (text); } } while (0)
+  HOSTPATH_CU(cudaEventRecord(ev_start, st), "cudaEventRecord");
+  HOSTPATH_CU(cudaStreamWaitEvent(ctx->s_in, ev_start, 0), "cudaStreamWaitEvent");      // staging may still be in use on st
+  HOSTPATH_CU(cudaStreamWaitEvent(ctx->s_out, ev_start, 0), "cudaStreamWaitEvent");
+  for (int k = 0; k < nslab; ++k) {
+    const int y0 = k * rows, ny_k = std::min(rows, cfg0.ny - y0);
+    const int64_t cells_before = (int64_t)cfg0.nz * y0 * cfg0.nx;         // compact slabs are stored back to back
+    const size_t width = (size_t)ny_k * cfg0.nx * sizeof(float), spitch = (size_t)cfg0.ny * cfg0.nx * sizeof(float);
+    for (int i = 0; i < 4; ++i)
+      HOSTPATH_CU(cudaMemcpy2DAsync(f[i] + cells_before, width, h[i] + (size_t)y0 * cfg0.nx, spitch, width, (size_t)cfg0.nz,
+                                    cudaMemcpyHostToDevice, ctx->s_in), "H2D slab copy");
+    HOSTPATH_CU(cudaEventRecord(ctx->slab_events[2 * k], ctx->s_in), "cudaEventRecord");
+    HOSTPATH_CU(cudaStreamWaitEvent(st, ctx->slab_events[2 * k], 0), "cudaStreamWaitEvent");
+    if (ce != cudaSuccess || rs != IRIS_SO_OK) break;
+    // K1-K5 of the slab as a (nx, ny_k, nz) problem
+    ctx->cfg.ny = ny_k;
+    ctx->npix = (int64_t)ny_k * cfg0.nx; ctx->ncell = ctx->npix * cfg0.nz; ctx->nvox = ctx->npix * cfg0.nv;
+    float* cube_k = d_cube + (int64_t)y0 * cfg0.nx * cfg0.nv;
+    rs = run_coefficients(ctx, f[0] + cells_before, f[1] + cells_before, f[2] + cells_before, f[3] + cells_before, nullptr, st);
+    if (rs == IRIS_SO_OK) rs = run_transfer(ctx, ctx->mc, cube_k, nullptr, st);
+    ctx->cfg = cfg0; ctx->ncell = ncell0; ctx->npix = npix0; ctx->nvox = nvox0;
+    if (!post) {
+      HOSTPATH_CU(cudaEventRecord(ctx->slab_events[2 * k + 1], st), "cudaEventRecord");
+      HOSTPATH_CU(cudaStreamWaitEvent(ctx->s_out, ctx->slab_events[2 * k + 1], 0), "cudaStreamWaitEvent");
+      HOSTPATH_CU(cudaMemcpyAsync(h_cube + (size_t)y0 * cfg0.nx * cfg0.nv, cube_k, sizeof(float) * (size_t)ny_k * cfg0.nx * cfg0.nv,
+                                  cudaMemcpyDeviceToHost, ctx->s_out), "D2H slab copy");
+    }
+  }
+  if (post && ce == cudaSuccess && rs == IRIS_SO_OK) {
+    if (cfg0.beam_fwhm_px > 0.0) rs = run_beam(ctx, d_cube, d_cube, nullptr, ctx->nc.on != 0, st);
+    else rs = run_noise(ctx, d_cube, st);
+    HOSTPATH_CU(cudaMemcpyAsync(h_cube, d_cube, cb, cudaMemcpyDeviceToHost, st), "D2H copy");
+  }
+#undef HOSTPATH_CU
+  // always drain the three streams before returning (also on error: nothing may still be writing h_cube)
+  cudaError_t e1 = cudaStreamSynchronize(ctx->s_in), e2 = cudaStreamSynchronize(st), e3 = cudaStreamSynchronize(ctx->s_out);
+  if (rs != IRIS_SO_OK) return rs;
+  if (ce != cudaSuccess) return cuda_fail(ctx, ce, what);
+  if (e1 != cudaSuccess) return cuda_fail(ctx, e1, "cudaStreamSynchronize(copy-in)");
+  if (e2 != cudaSuccess) return cuda_fail(ctx, e2, "cudaStreamSynchronize");
+  if (e3 != cudaSuccess) return cuda_fail(ctx, e3, "cudaStreamSynchronize(copy-out)");
   return IRIS_SO_OK;
 }
 

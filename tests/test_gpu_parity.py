@@ -366,3 +366,34 @@ def test_full_size_medium_sampled():
 
 def test_full_size_large_sampled():
     _sampled_check("large", 32, 12)
+
+
+# ------------------------------------------------------------------------------------------------
+# host-buffer path (iris_so_observe_host): single shot and slab-pipelined, identical to the device path
+@pytest.mark.parametrize("case", ["one_shot", "slabs_plain", "slabs_beam_noise", "slabs_ragged_pageable"])
+def test_observe_host_equals_device_path(case):
+    """The slab pipeline (H2D of slab k+1 | K1-K5 of slab k | D2H of slab k-1) must give the cube of the device path
+    bit for bit: the kernels are the same and every pixel column is independent before the beam."""
+    if case == "one_shot":
+        cfg, r = make_workload("small", n=24, nv=64)
+    elif case == "slabs_ragged_pageable":
+        cfg, r = make_workload("small", nx=300, ny=150, nz=160, nv=72)      # 768 KB of fields per row: slabs of 62, 62, 26 rows
+    else:
+        cfg, r = make_workload("small", nx=256, ny=80, nz=512, nv=96)       # 2 MB of fields per row: slabs of 24, 24, 24, 8 rows
+    if case == "slabs_beam_noise":
+        cfg = cfg.with_(beam_fwhm_px=3.0, noise_sigma=0.25, seed=11)
+    f = make_fields(cfg, r)
+    it = iris(cfg)
+    ref = it.observe(*dev_fields(f)).cpu()
+    pin = case != "slabs_ragged_pageable"
+    h = [torch.from_numpy(np.ascontiguousarray(f[k])) for k in ("nH2", "Tgas", "Tdust", "vlos")]
+    hc = torch.empty(it.shape_cube, dtype=torch.float32)
+    if pin:
+        h = [t.pin_memory() for t in h]
+        hc = hc.pin_memory()
+    it.observe_host(*h, hc)
+    assert torch.equal(hc, ref)
+    hc.zero_()
+    it.observe_host(*h, hc)                                                 # second call reuses streams and events
+    assert torch.equal(hc, ref)
+    assert torch.equal(it.observe(*dev_fields(f)).cpu(), ref)               # and leaves the context usable at full size
