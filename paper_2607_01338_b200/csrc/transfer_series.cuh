@@ -150,13 +150,10 @@ __device__ __forceinline__ void series_passes(float* d, int q, int qend, f32x2 x
   constexpr float L1 = 0.6931471805599453f, L2 = L1 * L1, L3 = L2 * L1, L4 = L2 * L2;
   const f32x2 ONE = pk1(1.0f), NEG1 = pk1(-1.0f);
   const f32x2 C4 = pk1(L4 / 24.0f), C3 = pk1(-L3 / 6.0f), C2 = pk1(L2 / 2.0f), C1 = pk1(-L1);   // -(1 - 2^-t) / t
-  bool ok[P];
   f32x2 Dt[P], u[P], pol[P], t[P], mn[P], qq[P];
 #pragma unroll
   for (int k = 0; k < P; ++k) {
-    ok[k] = q + k * LPP < qend;
-    float2 v = make_float2(0.0f, 0.0f);
-    if (ok[k]) v = *reinterpret_cast<const float2*>(d + 64 * k);
+    const float2 v = *reinterpret_cast<const float2*>(d + 64 * k);
     Dt[k] = pk(v.x, v.y);
     u[k] = mul2(xx, xx);
     xx = add2(xx, step2);
@@ -218,12 +215,12 @@ __device__ __forceinline__ void series_passes(float* d, int q, int qend, f32x2 x
   }
   (void)ONE;
 #pragma unroll
-  for (int k = 0; k < P; ++k)
-    if (ok[k]) {
-      float2 v;
-      upk(Dt[k], v.x, v.y);
-      *reinterpret_cast<float2*>(d + 64 * k) = v;
-    }
+  for (int k = 0; k < P; ++k) {
+    float2 v;
+    upk(Dt[k], v.x, v.y);
+    *reinterpret_cast<float2*>(d + 64 * k) = v;
+  }
+  (void)q; (void)qend;
 }
 
 template <int LPP, bool DUST, int DEG>
@@ -365,7 +362,9 @@ inline cudaError_t launch_transfer_series_t(const MarchConsts& mc, const float* 
                                             int nv, float* out, float* out_cont, cudaStream_t st) {
   constexpr int PPW = 32 / LPP;
   constexpr int NQ = SeriesLayout<DUST, DEG>::NQ;
-  const int nvp = (nv + 2 * LPP - 1) / (2 * LPP) * (2 * LPP);      // whole rows of LPP channel pairs
+  // whole rows of LPP channel pairs, plus one row: the last pass of a window runs all LPP lanes of the pixel, up to
+  // LPP - 1 pairs past the window (their update is below the window threshold, or lands in this padding)
+  const int nvp = (nv + 2 * LPP - 1) / (2 * LPP) * (2 * LPP) + 2 * LPP;
   const size_t rec_per_warp = (size_t)NQ * 32 * sizeof(float4);
   const size_t spec_per_warp = (size_t)PPW * nvp * sizeof(float);
   int wpc = 4;
