@@ -452,7 +452,7 @@ def run_ours(args):
     uuid = str(torch.cuda.get_device_properties(torch.cuda.current_device()).uuid)
     uuid = uuid if uuid.startswith("GPU-") else "GPU-" + uuid
 
-    main = bench_workload(torch, dist, args.workload, args.algo, args.steps, args.warmup, rank, peaks, want_e2e=True,
+    main = bench_workload(torch, dist, args.workload, args.algo, args.steps, args.warmup, rank, peaks, want_e2e=not args.no_e2e,
                           want_dense_probe=(world == 1 and not args.no_extras), sampler_uuid=uuid if rank == 0 else None)
     cfg = main["cfg"]
     extra = {}
@@ -496,6 +496,7 @@ def main():
     ap.add_argument("--algo", default="window", choices=["window", "dense"])
     ap.add_argument("--no-extras", action="store_true", help="skip the medium-cube and dense-algorithm side measurements")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs: its slab pipeline launches per slab)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)

@@ -482,9 +482,11 @@ void orc_beam(int ny, int nx, int nv, double fwhm_px, const double *in, double *
 // ---------------------------------------------------------------------------------------------
 // O9  Noise, Eq. 4.12.1: T += gamma (mu + sigma z), z ~ N(0,1) independently per voxel.
 // Reading S10: z comes from the counter-based generator Philox4x32-10 (Salmon et al. 2011)
-// with key = (seed lo, seed hi) and counter = (voxel lo, voxel hi, 0, 0); the first two output words
-// give u1 = ((r0 >> 8) + 0.5) 2^-24, u2 = ((r1 >> 8) + 0.5) 2^-24 and Box-Muller
-// z = sqrt(-2 ln u1) cos(2 pi u2).  gamma (reading S9): mode 0 -> 1; mode 1 -> one draw per cube,
+// with key = (seed lo, seed hi); one call, counter = (voxel / 4 lo, voxel / 4 hi, 0, 0), serves four consecutive
+// voxels: words (r0, r1) the voxels 4c, 4c+1 and words (r2, r3) the voxels 4c+2, 4c+3; a word pair gives
+// u1 = ((ra >> 8) + 0.5) 2^-24, u2 = ((rb >> 8) + 0.5) 2^-24 and the two independent Box-Muller deviates
+// z = sqrt(-2 ln u1) cos(2 pi u2) for the even voxel, sqrt(-2 ln u1) sin(2 pi u2) for the odd one.
+// gamma (reading S9): mode 0 -> 1; mode 1 -> one draw per cube,
 // gamma = (r0 >> 8) 2^-24 of counter (0, 0, 1, 0).
 void orc_philox4x32_10(uint64_t seed, uint64_t ctr_lo, uint64_t ctr_hi, uint32_t out[4]) {
   uint32_t c0 = (uint32_t)ctr_lo, c1 = (uint32_t)(ctr_lo >> 32), c2 = (uint32_t)ctr_hi, c3 = (uint32_t)(ctr_hi >> 32);
@@ -504,10 +506,12 @@ void orc_philox4x32_10(uint64_t seed, uint64_t ctr_lo, uint64_t ctr_hi, uint32_t
 
 double orc_normal(uint64_t seed, uint64_t voxel) {
   uint32_t r[4];
-  orc_philox4x32_10(seed, voxel, 0, r);
-  const double u1 = ((double)(r[0] >> 8) + 0.5) / 16777216.0;
-  const double u2 = ((double)(r[1] >> 8) + 0.5) / 16777216.0;
-  return std::sqrt(-2.0 * std::log(u1)) * std::cos(2.0 * kPi * u2);
+  orc_philox4x32_10(seed, voxel >> 2, 0, r);
+  const int p = (int)((voxel >> 1) & 1);
+  const double u1 = ((double)(r[2 * p] >> 8) + 0.5) / 16777216.0;
+  const double u2 = ((double)(r[2 * p + 1] >> 8) + 0.5) / 16777216.0;
+  const double R = std::sqrt(-2.0 * std::log(u1));
+  return (voxel & 1) ? R * std::sin(2.0 * kPi * u2) : R * std::cos(2.0 * kPi * u2);
 }
 
 double orc_noise_gamma(const orc_config *c) {

@@ -388,7 +388,7 @@ iris_so_status run_beam(iris_so_ctx* ctx, const float* in, float* out, float* tm
 
 iris_so_status run_noise(iris_so_ctx* ctx, float* cube, cudaStream_t st) {
   ProfScope prof(ctx, IRIS_SO_STAGE_NOISE, st);
-  iris::noise_kernel<<<(unsigned)((ctx->nvox + 255) / 256), 256, 0, st>>>(ctx->nc, cube, ctx->nvox);
+  iris::noise_kernel<<<(unsigned)(((ctx->nvox + 3) / 4 + 255) / 256), 256, 0, st>>>(ctx->nc, cube, ctx->nvox);
   IRIS_CHECK_LAUNCH(ctx, "noise_kernel");
   return IRIS_SO_OK;
 }

@@ -17,14 +17,33 @@ struct NoiseConsts {
   int on;
 };
 
-// z ~ N(0,1) of voxel `idx`: Box-Muller on the first two words of Philox4x32-10(key, counter = idx).
+// z ~ N(0,1) per voxel (reading S10): one Philox4x32-10(key, counter = voxel / 4) call serves four
+// consecutive voxels; words (r0, r1) the voxels 4c, 4c+1, words (r2, r3) the voxels 4c+2, 4c+3; a word pair gives
+// u1, u2 and the two Box-Muller deviates sqrt(-2 ln u1) cos(2 pi u2) (even voxel), sqrt(-2 ln u1) sin(2 pi u2) (odd).
 // The uniforms use the top 24 bits, so they are exact in fp32 and identical to the float64 definition.
-__device__ __forceinline__ float voxel_normal(const NoiseConsts& nc, uint64_t idx) {
+__device__ __forceinline__ void box_muller_pair(uint32_t ra, uint32_t rb, float& z_even, float& z_odd) {
+  const float u1 = ((float)(ra >> 8) + 0.5f) * (1.0f / 16777216.0f);
+  const float u2 = ((float)(rb >> 8) + 0.5f) * (1.0f / 16777216.0f);
+  const float R = sqrtf(-2.0f * logf(u1));
+  float sn, cs;
+  sincospif(2.0f * u2, &sn, &cs);
+  z_even = R * cs;
+  z_odd = R * sn;
+}
+
+// the deviates of the voxel pair (idx, idx + 1), idx even
+__device__ __forceinline__ void voxel_normal_pair(const NoiseConsts& nc, uint64_t idx, float& z0, float& z1) {
   uint32_t r[4];
-  philox4x32_10(nc.k0, nc.k1, (uint32_t)idx, (uint32_t)(idx >> 32), 0u, 0u, r);
-  const float u1 = ((float)(r[0] >> 8) + 0.5f) * (1.0f / 16777216.0f);
-  const float u2 = ((float)(r[1] >> 8) + 0.5f) * (1.0f / 16777216.0f);
-  return sqrtf(-2.0f * logf(u1)) * cospif(2.0f * u2);
+  const uint64_t c = idx >> 2;
+  philox4x32_10(nc.k0, nc.k1, (uint32_t)c, (uint32_t)(c >> 32), 0u, 0u, r);
+  const bool hi = (idx >> 1) & 1;
+  box_muller_pair(hi ? r[2] : r[0], hi ? r[3] : r[1], z0, z1);
+}
+
+__device__ __forceinline__ float voxel_normal(const NoiseConsts& nc, uint64_t idx) {
+  float z0, z1;
+  voxel_normal_pair(nc, idx & ~1ull, z0, z1);
+  return (idx & 1) ? z1 : z0;
 }
 
 // One 1-D pass of the beam along a spatial axis "a" of a cube laid out with the channel fastest.
@@ -109,9 +128,11 @@ beam_pass_reg_kernel(BeamTaps<RB> taps, NoiseConsts nc, const float* __restrict_
       float2 o;
       asm("mov.b64 {%0, %1}, %2;" : "=f"(o.x), "=f"(o.y) : "l"(acc[i]));
       const int64_t idx = base + (int64_t)a * stride_a;
-      if (nc.on) {
-        o.x += fmaf(nc.sigma, voxel_normal(nc, (uint64_t)idx), nc.mu);
-        o.y += fmaf(nc.sigma, voxel_normal(nc, (uint64_t)idx + 1), nc.mu);
+      if (nc.on) {                 // idx is even: the two channels of the thread share one Box-Muller pair
+        float z0, z1;
+        voxel_normal_pair(nc, (uint64_t)idx, z0, z1);
+        o.x += fmaf(nc.sigma, z0, nc.mu);
+        o.y += fmaf(nc.sigma, z1, nc.mu);
       }
       *reinterpret_cast<float2*>(out + idx) = o;
     }
@@ -143,11 +164,19 @@ inline void launch_beam_pass(const BeamConsts& bc, const NoiseConsts& nc, const 
   beam_pass_kernel<<<grid, block, 0, st>>>(bc, nc, in, out, na, nb, nv, stride_a, stride_b);
 }
 
-// K7 alone (no beam configured): in-place.
+// K7 alone (no beam configured): in-place, four consecutive voxels (one Philox call) per thread.
 __global__ void __launch_bounds__(256) noise_kernel(NoiseConsts nc, float* __restrict__ cube, int64_t nvox) {
-  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= nvox) return;
-  cube[i] += fmaf(nc.sigma, voxel_normal(nc, (uint64_t)i), nc.mu);
+  const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t i0 = 4 * c;
+  if (i0 >= nvox) return;
+  uint32_t r[4];
+  philox4x32_10(nc.k0, nc.k1, (uint32_t)c, (uint32_t)((uint64_t)c >> 32), 0u, 0u, r);
+  float z[4];
+  box_muller_pair(r[0], r[1], z[0], z[1]);
+  box_muller_pair(r[2], r[3], z[2], z[3]);
+#pragma unroll
+  for (int k = 0; k < 4; ++k)
+    if (i0 + k < nvox) cube[i0 + k] += fmaf(nc.sigma, z[k], nc.mu);
 }
 
 }  // namespace iris

@@ -423,11 +423,18 @@ def test_noise_statistics_and_definition():
     assert abs(z.std() - 1.0) < 4 / math.sqrt(2 * n)
     assert abs(np.mean(z[1:] * z[:-1])) < 4 / math.sqrt(n)            # lag-1 correlation
     assert abs(np.mean(z ** 3)) < 0.03 and abs(np.mean(z ** 4) - 3.0) < 0.08
-    # voxel i depends only on (seed, i): Box-Muller on the first two Philox words
-    r = o.philox(12345, 777)
-    u1, u2 = ((r[0] >> 8) + 0.5) / 2 ** 24, ((r[1] >> 8) + 0.5) / 2 ** 24
-    assert z[777] == pytest.approx(math.sqrt(-2 * math.log(u1)) * math.cos(2 * math.pi * u2), rel=1e-9)
-    assert o.normal(12345, 777) == pytest.approx(z[777], rel=1e-9)
+    for lag in (2, 3, 4):                                              # the four voxels of one Philox call, and beyond
+        assert abs(np.mean(z[lag:] * z[:-lag])) < 4 / math.sqrt(n)
+    z2sq = z ** 2 - 1.0                                                # cos / sin partners share a radius only
+    assert abs(np.mean(z2sq[0::2] * z2sq[1::2])) < 6 / math.sqrt(n / 2)
+    # voxel i depends only on (seed, i): one Philox call per four voxels, Box-Muller cos / sin per word pair
+    for i in (776, 777, 778, 779):
+        r = o.philox(12345, i // 4)
+        p = (i // 2) % 2
+        u1, u2 = ((r[2 * p] >> 8) + 0.5) / 2 ** 24, ((r[2 * p + 1] >> 8) + 0.5) / 2 ** 24
+        trig = math.sin if i % 2 else math.cos
+        assert z[i] == pytest.approx(math.sqrt(-2 * math.log(u1)) * trig(2 * math.pi * u2), rel=1e-9, abs=1e-12)
+        assert o.normal(12345, i) == pytest.approx(z[i], rel=1e-9, abs=1e-12)
     # different seed -> different field; gamma mode 1 scales the whole cube by one U[0,1) draw
     z2 = Oracle(cfg.with_(seed=12346)).noise(np.zeros(1000))
     assert abs(np.corrcoef(z2, o.noise(np.zeros(1000)))[0, 1]) < 0.15
