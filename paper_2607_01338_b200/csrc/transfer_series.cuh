@@ -258,6 +258,19 @@ transfer_series_kernel(MarchConsts mc, const float* __restrict__ coef, int64_t n
     if (DUST) { l_td = p[4 * ncell]; l_sd = p[5 * ncell]; }
   }
 
+  // rare: fold the accumulated dust attenuation into the stored spectrum (keeps G inside the fp32 range)
+  auto rescale_spectrum = [&]() {
+    const float inv = 1.0f / G;
+    __syncwarp(__activemask());
+    for (int qq = i; qq < npair; qq += LPP) {
+      float2* w = reinterpret_cast<float2*>(sp + (qq / LPP) * ROW + i * 2);
+      float2 v = *w;
+      v.x *= inv; v.y *= inv;
+      *w = v;
+    }
+    G = 1.0f;
+  };
+
   // one cell of phase B for this lane's pixel, given the cell's record in registers
   auto cell_step = [&](const float4& q0, const float4& q1, const float4& q2, const float4& q3) {
     const int kk = __float_as_int(q0.w);
@@ -290,24 +303,15 @@ transfer_series_kernel(MarchConsts mc, const float* __restrict__ coef, int64_t n
       }
       if (rem == 1) series_passes<DUST, DEG, LPP, 1>(d, q, qend, xx, step2, o);
     }
-    if (DUST && G > 1.0e18f) {   // rare: fold the accumulated dust attenuation into the stored spectrum
-      const float inv = 1.0f / G;
-      __syncwarp(__activemask());
-      for (int qq = i; qq < npair; qq += LPP) {
-        float2* w = reinterpret_cast<float2*>(sp + (qq / LPP) * ROW + i * 2);
-        float2 v = *w;
-        v.x *= inv; v.y *= inv;
-        *w = v;
-      }
-      G = 1.0f;
-    }
+    if (DUST && G > 1.0e18f) rescale_spectrum();
   };
 
+  bool chunk_busy = true;
   for (int z0 = 0; z0 < nz; z0 += LPP) {
     // ---- phase A: one record per lane
     {
       const SeriesRecord r = make_series_record<DUST, DEG>(l_e, l_a, l_c, l_s, l_td, l_sd, mc.T_bg, nv);
-      __syncwarp();                      // phase B of the previous chunk is done with the records
+      chunk_busy = __any_sync(0xffffffffu, ((unsigned)__float_as_int(r.q0.w) >> 16) != 0u);   // also: phase B is done
       rec[lane] = r.q0;
       rec[32 + lane] = r.q1;
       if (NQ > 2) rec[64 + lane] = r.q2;
@@ -325,6 +329,20 @@ transfer_series_kernel(MarchConsts mc, const float* __restrict__ coef, int64_t n
     // ---- phase B: the LPP lanes of a pixel walk the cells of the chunk, records read one cell ahead
     const int ncz = min(LPP, nz - z0);
     const float4* rq = rec + g;
+    if (!chunk_busy) {
+      // no pixel of the warp has a line in any cell of the chunk (columns whose velocity is outside the band): only
+      // the continuum and the accumulated dust attenuation advance
+      if (DUST) {
+        for (int j = 0; j < ncz; ++j) {
+          const float E_d = rq[64 + j * PPW].w;
+          const float4 c3 = rq[96 + j * PPW];
+          C = fmaf(C, E_d, c3.x);
+          G *= c3.y;
+          if (G > 1.0e18f) rescale_spectrum();
+        }
+      }
+      continue;
+    }
     float4 a0 = rq[0], a1 = rq[32], a2 = NQ > 2 ? rq[64] : float4{}, a3 = NQ > 3 ? rq[96] : float4{};
     for (int j = 0; j < ncz; j += 2) {
       const int jb = min(j + 1, ncz - 1) * PPW;
