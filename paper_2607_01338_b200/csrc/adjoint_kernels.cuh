@@ -153,6 +153,58 @@ __device__ __forceinline__ float warp_sum(float v) {
   return v;
 }
 
+// Sums of eight per-lane values over the warp in 17 shuffles instead of 40: three exchange steps halve the number of
+// values a lane carries (lanes with the bit set keep the upper half), two more finish the one value that is left, and
+// the eight totals (index j at lane 4 j) are broadcast back.
+__device__ __forceinline__ void warp_sum8(float (&v)[8]) {
+  const unsigned FULL = 0xffffffffu;
+  const int lane = threadIdx.x & 31;
+  const bool b4 = lane & 16, b3 = lane & 8, b2 = lane & 4;
+  float a[4], b[2], r;
+#pragma unroll
+  for (int j = 0; j < 4; ++j) {
+    const float send = b4 ? v[j] : v[j + 4];
+    a[j] = (b4 ? v[j + 4] : v[j]) + __shfl_xor_sync(FULL, send, 16);
+  }
+#pragma unroll
+  for (int j = 0; j < 2; ++j) {
+    const float send = b3 ? a[j] : a[j + 2];
+    b[j] = (b3 ? a[j + 2] : a[j]) + __shfl_xor_sync(FULL, send, 8);
+  }
+  {
+    const float send = b2 ? b[0] : b[1];
+    r = (b2 ? b[1] : b[0]) + __shfl_xor_sync(FULL, send, 4);
+  }
+  r += __shfl_xor_sync(FULL, r, 2);
+  r += __shfl_xor_sync(FULL, r, 1);
+#pragma unroll
+  for (int j = 0; j < 8; ++j) v[j] = __shfl_sync(FULL, r, 4 * j);
+}
+
+// Channel integral of the Gaussian profile from the channel CENTRE (dv / b <= 0.55; same expansion as
+// transfer_series.cuh): erf(x + s/2) - erf(x - s/2) = (2 s / sqrt(pi)) exp(-x^2) P(x^2), P of degree 4 with
+// coefficients that depend on the cell only.
+struct CentreProfile {
+  float p0, p1, p2, p3, p4;     // already multiplied by 2 s / sqrt(pi)
+  __device__ __forceinline__ void set(float s) {
+    const float sp = 1.1283791670955126f * s;
+    const float s2 = s * s, s4 = s2 * s2, s6 = s4 * s2, s8 = s4 * s4;
+    p0 = sp * (1.0f - s2 * (1.0f / 12.0f) + s4 * (1.0f / 160.0f) - s6 * (1.0f / 2688.0f) + s8 * (1.0f / 55296.0f));
+    p1 = sp * (s2 * (1.0f / 6.0f) - s4 * (1.0f / 40.0f) + s6 * (1.0f / 448.0f) - s8 * (1.0f / 6912.0f));
+    p2 = sp * (s4 * (1.0f / 120.0f) - s6 * (1.0f / 672.0f) + s8 * (1.0f / 6912.0f));
+    p3 = sp * (s6 * (1.0f / 5040.0f) - s8 * (1.0f / 25920.0f));
+    p4 = sp * (s8 * (1.0f / 362880.0f));
+  }
+  __device__ __forceinline__ float at(float x) const {
+    const float u = x * x;
+    float pol = fmaf(p4, u, p3);
+    pol = fmaf(pol, u, p2);
+    pol = fmaf(pol, u, p1);
+    pol = fmaf(pol, u, p0);
+    return pol * ex2_approx(-1.4426950408889634f * u);
+  }
+};
+
 // w(tau) = (1 - exp(-tau)) / tau and w'(tau) = (exp(-tau)(1 + tau) - 1) / tau^2, accurate for every tau.
 __device__ __forceinline__ void w_and_wprime(float tau, float m /* 1 - exp(-tau) */, float& w, float& wp) {
   if (fabsf(tau) < 0.25f) {
@@ -169,7 +221,7 @@ __device__ __forceinline__ void w_and_wprime(float tau, float m /* 1 - exp(-tau)
     r = fmaf(r, tau, 1.0f / 3.0f);
     wp = fmaf(r, tau, -0.5f);                      // -1/2 + tau/3 - tau^2/8 + ...
   } else {
-    const float it = 1.0f / tau;
+    const float it = rcp_approx(tau);
     w = m * it;
     wp = (fmaf(1.0f - m, 1.0f + tau, -1.0f)) * it * it;
   }
@@ -183,7 +235,7 @@ __device__ __forceinline__ float channel_derf(int c, float c_los, float s) {
 }
 
 // K8: one warp per pixel.  Shared memory per warp: 5 * nv floats (xrem, P, Q, Dt, what).
-template <bool DUST>
+template <bool DUST, bool SERIES>
 __global__ void __launch_bounds__(128)
 adjoint_march_kernel(MarchConsts mc, AdjointConsts ac, const float* __restrict__ coef, const float* __restrict__ dcoef,
                      int64_t ncell, int npix, int nz, int nv, const float* __restrict__ what, float* __restrict__ grad) {
@@ -213,8 +265,14 @@ adjoint_march_kernel(MarchConsts mc, AdjointConsts ac, const float* __restrict__
     if (DUST) totD += p[4 * ncell];
     int klo, khi;
     const int W = line_window(e_c, a_c, c_los, s, nv, klo, khi);
-    if (W > 0)
-      for (int c = klo + lane; c <= khi; c += 32) xrem[c] = fmaf(a_c, channel_derf(c, c_los, s), xrem[c]);
+    if (W > 0) {
+      CentreProfile prof;
+      if (SERIES) prof.set(s);
+      for (int c = klo + lane; c <= khi; c += 32) {
+        const float dErf = SERIES ? prof.at(((float)c + 0.5f - c_los) * s) : channel_derf(c, c_los, s);
+        xrem[c] = fmaf(a_c, dErf, xrem[c]);
+      }
+    }
     __syncwarp();
   }
   // SQ = sum_c Q[c] and SPD = sum_c P[c] Dt[c] over ALL channels are carried as running sums: a cell changes
@@ -252,8 +310,10 @@ adjoint_march_kernel(MarchConsts mc, AdjointConsts ac, const float* __restrict__
     float acc_e = 0.0f, acc_a = 0.0f, acc_d = 0.0f, accW = 0.0f, accQ = 0.0f, accPD = 0.0f;
     float winQ_old = 0.0f, winQ_new = 0.0f, winPD_old = 0.0f, winPD_new = 0.0f;
     if (W > 0) {
+      CentreProfile prof;
+      if (SERIES) prof.set(s);
       for (int c = klo + lane; c <= khi; c += 32) {
-        const float dErf = channel_derf(c, c_los, s);
+        const float dErf = SERIES ? prof.at(((float)c + 0.5f - c_los) * s) : channel_derf(c, c_los, s);
         const float tau_L = a_c * dErf, J_L = e_c * dErf, tau_T = tau_L + tau_d;
         const float xr = xrem[c] - tau_L;
         const float w = wh[c];
@@ -293,12 +353,14 @@ adjoint_march_kernel(MarchConsts mc, AdjointConsts ac, const float* __restrict__
         if (DUST) winPD_new = fmaf(Pn, Dn, winPD_new);
       }
     }
-    acc_e = warp_sum(acc_e); acc_a = warp_sum(acc_a);
-    if (DUST) {
-      acc_d = warp_sum(acc_d); accW = warp_sum(accW);
+    if (!DUST) {
+      acc_e = warp_sum(acc_e); acc_a = warp_sum(acc_a);
+    } else {
       if (W > 0) {
-        winQ_old = warp_sum(winQ_old); winQ_new = warp_sum(winQ_new);
-        winPD_old = warp_sum(winPD_old); winPD_new = warp_sum(winPD_new);
+        float r8[8] = {acc_e, acc_a, acc_d, accW, winQ_old, winQ_new, winPD_old, winPD_new};
+        warp_sum8(r8);
+        acc_e = r8[0]; acc_a = r8[1]; acc_d = r8[2]; accW = r8[3];
+        winQ_old = r8[4]; winQ_new = r8[5]; winPD_old = r8[6]; winPD_new = r8[7];
       }
       // channels outside the window: only the dust of this cell acts on them
       accQ = SQ - winQ_old;
@@ -344,10 +406,10 @@ inline void launch_coef_grad(const LevelConsts& lc, const AdjointConsts& ac, int
   else coef_grad_kernel<N, N - 1><<<grid, 128, 0, st>>>(lc, ac, ncell, n, T, dcoef);
 }
 
-// K9 then K8.  dcoef: scratch [2][ncell].  Returns the first CUDA error; *launches is advanced per kernel.
+// K9 then K8.  dcoef: scratch [2][ncell].  series: every cell has dv / b <= 0.55 (channel-centre profile expansion).  Returns the first CUDA error; *launches is advanced per kernel.
 inline cudaError_t launch_adjoint(const MarchConsts& mc, const AdjointConsts& ac, const LevelConsts& lc, int n_levels,
                                   int band, const float* coef, float* dcoef, int64_t ncell, int npix, int nz, int nv,
-                                  bool dust, const float* nH2, const float* Tgas, const float* what, float* grad,
+                                  bool dust, bool series, const float* nH2, const float* Tgas, const float* what, float* grad,
                                   cudaStream_t st, uint64_t* launches) {
   switch (n_levels) {
     case 2: launch_coef_grad<2>(lc, ac, band, ncell, nH2, Tgas, dcoef, st); break;
@@ -368,15 +430,15 @@ inline cudaError_t launch_adjoint(const MarchConsts& mc, const AdjointConsts& ac
   const size_t smem = (size_t)wpc * 5 * nv * sizeof(float);
   if (smem > 227 * 1024) return cudaErrorInvalidConfiguration;
   const unsigned grid = (unsigned)((npix + wpc - 1) / wpc);
-  if (dust) {
-    e = cudaFuncSetAttribute(adjoint_march_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    adjoint_march_kernel<true><<<grid, wpc * 32, smem, st>>>(mc, ac, coef, dcoef, ncell, npix, nz, nv, what, grad);
-  } else {
-    e = cudaFuncSetAttribute(adjoint_march_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    adjoint_march_kernel<false><<<grid, wpc * 32, smem, st>>>(mc, ac, coef, dcoef, ncell, npix, nz, nv, what, grad);
-  }
+#define IRIS_LAUNCH_ADJ(D_, S_)                                                                                        \
+  do {                                                                                                                 \
+    e = cudaFuncSetAttribute(adjoint_march_kernel<D_, S_>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);    \
+    if (e != cudaSuccess) return e;                                                                                    \
+    adjoint_march_kernel<D_, S_><<<grid, wpc * 32, smem, st>>>(mc, ac, coef, dcoef, ncell, npix, nz, nv, what, grad);   \
+  } while (0)
+  if (dust) { if (series) IRIS_LAUNCH_ADJ(true, true); else IRIS_LAUNCH_ADJ(true, false); }
+  else { if (series) IRIS_LAUNCH_ADJ(false, true); else IRIS_LAUNCH_ADJ(false, false); }
+#undef IRIS_LAUNCH_ADJ
   e = cudaGetLastError();
   if (e == cudaSuccess) ++*launches;
   return e;

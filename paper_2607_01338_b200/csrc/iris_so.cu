@@ -694,7 +694,8 @@ iris_so_status iris_so_observe_adjoint(iris_so_ctx* ctx, const float* d_nH2, con
   }
   ProfScope prof(ctx, IRIS_SO_STAGE_ADJOINT, st);
   cudaError_t e = iris::launch_adjoint(ctx->mc, ctx->ac, ctx->lc, c.n_levels, ctx->band, ctx->d_coef, dcoef, ctx->ncell, (int)ctx->npix,
-                                       c.nz, c.nv, c.dust_on != 0, d_nH2, d_Tgas, what, d_grad, st, &ctx->launches);
+                                       c.nz, c.nv, c.dust_on != 0, resolved_algo(c) == IRIS_SO_ALGO_WINDOW, d_nH2, d_Tgas, what,
+                                       d_grad, st, &ctx->launches);
   if (e != cudaSuccess) return cuda_fail(ctx, e, "launch of adjoint kernels");
   return IRIS_SO_OK;
 }
