@@ -350,7 +350,10 @@ iris_so_status run_transfer(iris_so_ctx* ctx, const iris::MarchConsts& mc, float
     if (e != cudaSuccess) return cuda_fail(ctx, e, "launch of transfer_modes_kernel");
     return IRIS_SO_OK;
   }
-  if (algo == IRIS_SO_ALGO_DENSE) {
+  // the line-window kernels keep whole spectra in shared memory: beyond ~13000 channels they do not fit and the
+  // dense kernel (spectra in registers, any nv) takes over
+  const bool fits = (size_t)(32 / 8) * ((size_t)nv + 32) * sizeof(float) + 2048 <= 227u * 1024u;
+  if (algo == IRIS_SO_ALGO_DENSE || !fits) {
     constexpr int CB = 16, NW = 4;
     dim3 block(32, NW), grid((npix + 31) / 32, (nv + CB * NW - 1) / (CB * NW));
     if (dust) iris::transfer_dense_kernel<CB, true><<<grid, block, 0, st>>>(mc, ctx->d_coef, ctx->ncell, npix, nz, nv, out, out_cont);
@@ -415,6 +418,7 @@ const char* iris_so_last_error(const iris_so_ctx* ctx) { return ctx ? ctx->err.c
 const char* iris_so_transfer_kernel(const iris_so_ctx* ctx) {
   if (!ctx) return "";
   if (!hot_path_mode(ctx->cfg)) return "transfer_modes_kernel";
+  if ((size_t)(32 / 8) * ((size_t)ctx->cfg.nv + 32) * sizeof(float) + 2048 > 227u * 1024u) return "transfer_dense_kernel";
   switch (resolved_algo(ctx->cfg)) {
     case IRIS_SO_ALGO_DENSE: return "transfer_dense_kernel";
     case IRIS_SO_ALGO_WINDOW: return "transfer_series_kernel";

@@ -397,3 +397,14 @@ def test_observe_host_equals_device_path(case):
     it.observe_host(*h, hc)                                                 # second call reuses streams and events
     assert torch.equal(hc, ref)
     assert torch.equal(it.observe(*dev_fields(f)).cpu(), ref)               # and leaves the context usable at full size
+
+
+def test_very_many_channels_fall_back_to_the_dense_kernel():
+    """Spectra of more than ~13000 channels do not fit the shared memory of the line-window kernels."""
+    cfg, r = make_workload("small", nx=5, ny=3, nz=12, nv=16384)
+    cfg = cfg.with_(dv_cms=0.01e5, v0_cms=-0.01e5 * 8191.5)
+    f = make_fields(cfg, r)
+    f["vlos"] = (0.3 * f["vlos"]).astype(np.float32)
+    it = iris(cfg)
+    assert it.transfer_kernel() == "transfer_dense_kernel"
+    assert_spectra(it.observe(*dev_fields(f)).cpu().numpy(), Oracle(cfg).observe(f))
