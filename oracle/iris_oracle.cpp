@@ -585,7 +585,8 @@ void orc_brute_column(const orc_config *c, const double *coef, const float *vlos
 // sum_v what[pixel][v] * d(cube_raw[pixel][v]) with what = G^T w (beam adjoint = same symmetric
 // zero-padded convolution, reading S20); `what` is computed by the caller with orc_beam.
 static void raw_column(const orc_config *c, const float *nH2, const float *Tgas, const float *Tdust,
-                       const float *vlos, int64_t pix, int64_t cell_mod, double n_mod, double *out) {
+                       const float *vlos, int64_t pix, int64_t cell_mod, double n_mod, double *out,
+                       double x_mod = 1.0 /* factor on the tracer abundance of cell_mod */) {
   const int64_t plane = (int64_t)c->nx * c->ny;
   const double h = c->cell_cm;
   const double Ibg = orc_planck(c->nu0_Hz, c->T_cmb);
@@ -597,6 +598,7 @@ static void raw_column(const orc_config *c, const float *nH2, const float *Tgas,
     double x[32], o[5];
     orc_levelpop_cell(c, n, (double)Tgas[cell], x);
     orc_cell_coefficients(c, n, (double)Tgas[cell], (double)Tdust[cell], x, o);
+    if (cell == cell_mod) { o[0] *= x_mod; o[1] *= x_mod; }      // j0, kappa0 are linear in the abundance (Eq. 4.2.1)
     for (int v = 0; v < c->nv; ++v) {
       const double pb = orc_phibar(c, v, (double)vlos[cell], o[2]);
       It[v] = formal_step(It[v], o[0] * pb + o[3] * o[4], o[1] * pb + o[3], h);
@@ -623,6 +625,24 @@ void orc_grad_fd(const orc_config *c, const float *nH2, const float *Tgas, const
   }
 }
 
+// (a') Abundance-only gradient ("abundance-only differentiability"): dL / d ln X_c for a per-cell factor on
+// the tracer abundance, by central differences (the level fractions do not depend on the abundance: Eq. 4.2.1).
+void orc_grad_fd_abundance(const orc_config *c, const float *nH2, const float *Tgas, const float *Tdust,
+                           const float *vlos, const double *what, int64_t nprobe, const int64_t *cells, double eps,
+                           double *grad) {
+  const int64_t plane = (int64_t)c->nx * c->ny;
+#pragma omp parallel for schedule(dynamic, 1)
+  for (int64_t q = 0; q < nprobe; ++q) {
+    const int64_t cell = cells[q], pix = cell % plane;
+    std::vector<double> a(c->nv), b(c->nv);
+    raw_column(c, nH2, Tgas, Tdust, vlos, pix, cell, (double)nH2[cell], a.data(), 1.0 + eps);
+    raw_column(c, nH2, Tgas, Tdust, vlos, pix, cell, (double)nH2[cell], b.data(), 1.0 - eps);
+    double s = 0.0;
+    for (int v = 0; v < c->nv; ++v) s += what[pix * c->nv + v] * (a[v] - b[v]);
+    grad[q] = s / (2.0 * eps);
+  }
+}
+
 // (b) Analytic reverse-scan adjoint in float64, for out_unit = T_RJ or I with
 // intensity-space subtraction.  Used to pin (a) against itself on every cell of a small cube and as
 // the dense reference for the GPU adjoint.  grad[ncell].
@@ -637,8 +657,8 @@ static double wprime_of_tau(double tau) {
   return (std::exp(-tau) * (1.0 + tau) - 1.0) / (tau * tau);
 }
 
-void orc_grad_adjoint(const orc_config *c, const float *nH2, const float *Tgas, const float *Tdust,
-                      const float *vlos, const double *what, double *grad) {
+static void grad_adjoint_impl(const orc_config *c, const float *nH2, const float *Tgas, const float *Tdust,
+                              const float *vlos, const double *what, double *grad, bool wrt_abundance) {
   const int64_t plane = (int64_t)c->nx * c->ny;
   const int N = c->n_levels, nz = c->nz, nv = c->nv;
   const double h = c->cell_cm;
@@ -710,9 +730,20 @@ void orc_grad_adjoint(const orc_config *c, const float *nH2, const float *Tgas, 
       double dk0 = pref * X * ((x[l] + n * dx[l]) * Blu - (x[u] + n * dx[u]) * Bul);
       if (T > c->T_inf) { dj0 = 0.0; dk0 = 0.0; }
       const double dad = c->dust_on ? c->kappa_gas_cm2_g * c->mass_per_H2_g : 0.0;
-      grad[cell] = g_j0 * dj0 + g_k0 * dk0 + g_ad * dad;
+      grad[cell] = wrt_abundance ? g_j0 * co[5 * k] + g_k0 * co[5 * k + 1]      // d / d ln X_c: j0, kappa0 linear in X
+                                 : g_j0 * dj0 + g_k0 * dk0 + g_ad * dad;
     }
   }
+}
+
+void orc_grad_adjoint(const orc_config *c, const float *nH2, const float *Tgas, const float *Tdust,
+                      const float *vlos, const double *what, double *grad) {
+  grad_adjoint_impl(c, nH2, Tgas, Tdust, vlos, what, grad, false);
+}
+
+void orc_grad_adjoint_abundance(const orc_config *c, const float *nH2, const float *Tgas, const float *Tdust,
+                                const float *vlos, const double *what, double *grad) {
+  grad_adjoint_impl(c, nH2, Tgas, Tdust, vlos, what, grad, true);
 }
 
 // ---------------------------------------------------------------------------------------------

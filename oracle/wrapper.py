@@ -272,20 +272,23 @@ class Oracle:
         return dict(zip(keys, out.tolist()))
 
     # -- gradient --------------------------------------------------------------------------------
-    def grad_fd(self, fields, what, cells, eps=1e-4):
+    def grad_fd(self, fields, what, cells, eps=1e-4, wrt="nH2"):
+        """Central finite differences of L = sum(what * raw cube) w.r.t. n_H2 of the listed cells (wrt="nH2") or
+        w.r.t. the logarithm of a per-cell factor on the tracer abundance (wrt="abundance")."""
         self._omp()
         f = [_f32(fields[k]).ravel() for k in ("nH2", "Tgas", "Tdust", "vlos")]
         what = np.ascontiguousarray(what, dtype=np.float64)
         cells = np.ascontiguousarray(cells, dtype=np.int64)
         g = np.zeros(cells.size)
-        self.lib.orc_grad_fd(self._p(), *[_fp(a) for a in f], _dp(what), C.c_int64(cells.size), _ip(cells),
-                             C.c_double(eps), _dp(g))
+        fn = self.lib.orc_grad_fd if wrt == "nH2" else self.lib.orc_grad_fd_abundance
+        fn(self._p(), *[_fp(a) for a in f], _dp(what), C.c_int64(cells.size), _ip(cells), C.c_double(eps), _dp(g))
         return g
 
-    def grad_adjoint(self, fields, what):
+    def grad_adjoint(self, fields, what, wrt="nH2"):
         self._omp()
         f = [_f32(fields[k]).ravel() for k in ("nH2", "Tgas", "Tdust", "vlos")]
         what = np.ascontiguousarray(what, dtype=np.float64)
         g = np.zeros(self.n_cells)
-        self.lib.orc_grad_adjoint(self._p(), *[_fp(a) for a in f], _dp(what), _dp(g))
+        fn = self.lib.orc_grad_adjoint if wrt == "nH2" else self.lib.orc_grad_adjoint_abundance
+        fn(self._p(), *[_fp(a) for a in f], _dp(what), _dp(g))
         return g.reshape(int(self.s.nz), int(self.s.ny), int(self.s.nx))

@@ -494,3 +494,39 @@ def test_adjoint_matches_finite_differences_and_is_linear_in_w():
     g2 = o.grad_adjoint(f, o.beam(w2))
     g12 = o.grad_adjoint(f, o.beam(w + 3 * w2))
     assert np.allclose(g12, g + 3 * g2, rtol=1e-10, atol=1e-12 * np.abs(g12).max())
+
+
+def test_abundance_gradient_pins():
+    """Abundance-only gradient: dL / d ln X_c for a per-cell factor on the tracer abundance."""
+    cfg, r = make_workload("tiny", n=6, nv=32)
+    cfg = cfg.with_(dust_on=True, kappa_gas_cm2_g=0.05)
+    f = make_fields(cfg, r)
+    f["vlos"] = (0.2 * f["vlos"]).astype(np.float32)
+    o = Oracle(cfg)
+    rng = np.random.default_rng(4)
+    w = rng.random((cfg.ny, cfg.nx, cfg.nv))
+    g = o.grad_adjoint(f, w, wrt="abundance")
+    cells = rng.choice(cfg.n_cells, size=40, replace=False)
+    gfd = o.grad_fd(f, w, cells, eps=1e-5, wrt="abundance")
+    assert np.allclose(g.ravel()[cells], gfd, rtol=2e-6, atol=1e-9 * np.abs(gfd).max())
+    # the sum over cells is the derivative w.r.t. the logarithm of the GLOBAL abundance: two whole observations
+    def L(X):
+        return float((w * Oracle(cfg.with_(abundance=X)).observe(f, beam=False, noise=False)).sum())
+    X, e = cfg.abundance, 1e-5
+    assert (L(X * (1 + e)) - L(X * (1 - e))) / (2 * e) == pytest.approx(g.sum(), rel=1e-5)
+    # optically thin limit, no dust, no background: cell c adds K_RJ j0 h phibar_k to channel k, so
+    # dL / d ln X_c = sum_k w_k K_RJ j0_c h phibar_k(c)  -- a closed form per cell
+    cfg_t = cfg.with_(abundance=2e-13, dust_on=False, T_cmb=0.0)
+    ot = Oracle(cfg_t)
+    gt = ot.grad_adjoint(f, w, wrt="abundance").reshape(cfg.nz, -1)
+    coef = ot.coefficients(f["nH2"], f["Tgas"], f["Tdust"])
+    plane = cfg.nx * cfg.ny
+    KRJ = CL ** 2 / (2 * KB * cfg.nu0_Hz ** 2)
+    dnuW = cfg.nu0_Hz * cfg.dv_cms / CL
+    vk = cfg.v0_cms + np.arange(cfg.nv) * cfg.dv_cms
+    p = 14
+    vl = f["vlos"].reshape(cfg.nz, plane).astype(np.float64)[:, p, None]
+    b = coef[2].reshape(cfg.nz, plane)[:, p, None]
+    pb = (special.erf((vk[None] + cfg.dv_cms / 2 - vl) / b) - special.erf((vk[None] - cfg.dv_cms / 2 - vl) / b)) / (2 * dnuW)
+    expect = KRJ * coef[0].reshape(cfg.nz, plane)[:, p] * cfg.cell_cm * (pb * w.reshape(plane, cfg.nv)[p][None]).sum(axis=1)
+    assert np.allclose(gt[:, p], expect, rtol=1e-4, atol=1e-9 * np.abs(expect).max())
