@@ -161,6 +161,13 @@ iris_so_status iris_so_observe_adjoint(iris_so_ctx *ctx, const float *d_nH2, con
                                        const float *d_Tdust, const float *d_vlos, const float *d_w,
                                        float *d_grad_nH2, void *cuda_stream);
 
+/* Abundance-only gradient: d L / d ln X_c of the same L for a per-cell factor X_c on the tracer abundance
+ * (the level fractions do not depend on it, Eq. 4.2.1); the sum over cells is the derivative with respect to the
+ * logarithm of the global abundance.  Same requirements and layouts as iris_so_observe_adjoint. */
+iris_so_status iris_so_observe_adjoint_abundance(iris_so_ctx *ctx, const float *d_nH2, const float *d_Tgas,
+                                                 const float *d_Tdust, const float *d_vlos, const float *d_w,
+                                                 float *d_grad_lnX, void *cuda_stream);
+
 /* Measurement support.  iris_so_profile(ctx, 1) makes every later call bracket each stage's kernels with
  * CUDA events on the caller's stream (no synchronisation); iris_so_profile(ctx, 0) switches it off; both
  * discard what was recorded.  iris_so_profile_read waits for the recorded events and returns the summed

@@ -16,7 +16,7 @@ DECLARED_SYMBOLS = (
     "iris_so_launch_count", "iris_so_scratch_bytes", "iris_so_levelpop", "iris_so_transfer", "iris_so_observe",
     "iris_so_observe_stages", "iris_so_observe_host", "iris_so_observe_adjoint", "iris_so_beam", "iris_so_noise",
     "iris_so_profile", "iris_so_profile_read", "iris_so_transfer_work", "iris_so_transfer_kernel",
-    "iris_so_density_trace", "iris_so_metrics",
+    "iris_so_density_trace", "iris_so_metrics", "iris_so_observe_adjoint_abundance",
 )
 STAGES = {"cell": 0, "transfer": 1, "beam": 2, "noise": 3, "adjoint": 4}
 
@@ -90,6 +90,8 @@ def load_library():
     lib.iris_so_observe_host.argtypes = [vp, fp, fp, fp, fp, fp, vp]
     lib.iris_so_observe_adjoint.restype = st
     lib.iris_so_observe_adjoint.argtypes = [vp, fp, fp, fp, fp, fp, fp, vp]
+    lib.iris_so_observe_adjoint_abundance.restype = st
+    lib.iris_so_observe_adjoint_abundance.argtypes = [vp, fp, fp, fp, fp, fp, fp, vp]
     lib.iris_so_beam.restype = st
     lib.iris_so_beam.argtypes = [vp, fp, fp, fp, vp]
     lib.iris_so_noise.restype = st
@@ -268,12 +270,14 @@ class IrisSO:
                                                   hp(vlos, n, "vlos"), hp(cube, self.n_vox, "cube"), self._stream()))
         return cube
 
-    def observe_adjoint(self, nH2, Tgas, Tdust, vlos, w, grad=None):
+    def observe_adjoint(self, nH2, Tgas, Tdust, vlos, w, grad=None, wrt="nH2"):
+        """d(sum w * cube) / d n_H2 per cell (wrt="nH2") or / d ln X per cell (wrt="abundance")."""
         import torch
         n = self.n_cells
         if grad is None:
             grad = torch.empty(self.shape_fields, dtype=torch.float32, device=nH2.device)
-        self._check(self.lib.iris_so_observe_adjoint(
+        fn = self.lib.iris_so_observe_adjoint if wrt == "nH2" else self.lib.iris_so_observe_adjoint_abundance
+        self._check(fn(
             self._h, self._dev(nH2, n, "nH2"), self._dev(Tgas, n, "Tgas"), self._dev(Tdust, n, "Tdust"),
             self._dev(vlos, n, "vlos"), self._dev(w, self.n_vox, "w"), self._dev(grad, n, "grad"), self._stream()))
         return grad

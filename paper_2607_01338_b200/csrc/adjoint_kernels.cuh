@@ -410,7 +410,10 @@ inline void launch_coef_grad(const LevelConsts& lc, const AdjointConsts& ac, int
 inline cudaError_t launch_adjoint(const MarchConsts& mc, const AdjointConsts& ac, const LevelConsts& lc, int n_levels,
                                   int band, const float* coef, float* dcoef, int64_t ncell, int npix, int nz, int nv,
                                   bool dust, bool series, const float* nH2, const float* Tgas, const float* what, float* grad,
-                                  cudaStream_t st, uint64_t* launches) {
+                                  cudaStream_t st, uint64_t* launches, bool wrt_abundance = false) {
+  // abundance-only gradient: e_c and a_c are linear in the tracer abundance, so d e_c / d ln X = e_c, d a_c / d ln X = a_c
+  // (the first two coefficient planes take the place of dcoef) and the dust does not depend on it (ac.c_d = 0)
+  if (wrt_abundance) goto march;
   switch (n_levels) {
     case 2: launch_coef_grad<2>(lc, ac, band, ncell, nH2, Tgas, dcoef, st); break;
     case 3: launch_coef_grad<3>(lc, ac, band, ncell, nH2, Tgas, dcoef, st); break;
@@ -422,9 +425,14 @@ inline cudaError_t launch_adjoint(const MarchConsts& mc, const AdjointConsts& ac
     case 9: launch_coef_grad<9>(lc, ac, band, ncell, nH2, Tgas, dcoef, st); break;
     default: launch_coef_grad<10>(lc, ac, band, ncell, nH2, Tgas, dcoef, st); break;
   }
-  cudaError_t e = cudaGetLastError();
-  if (e != cudaSuccess) return e;
-  ++*launches;
+  {
+    cudaError_t e0 = cudaGetLastError();
+    if (e0 != cudaSuccess) return e0;
+    ++*launches;
+  }
+march:
+  cudaError_t e;
+  const float* dc = wrt_abundance ? coef : dcoef;
   int wpc = 4;
   while (wpc > 1 && (size_t)wpc * 5 * nv * sizeof(float) > 200 * 1024) wpc >>= 1;
   const size_t smem = (size_t)wpc * 5 * nv * sizeof(float);
@@ -434,7 +442,7 @@ inline cudaError_t launch_adjoint(const MarchConsts& mc, const AdjointConsts& ac
   do {                                                                                                                 \
     e = cudaFuncSetAttribute(adjoint_march_kernel<D_, S_>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);    \
     if (e != cudaSuccess) return e;                                                                                    \
-    adjoint_march_kernel<D_, S_><<<grid, wpc * 32, smem, st>>>(mc, ac, coef, dcoef, ncell, npix, nz, nv, what, grad);   \
+    adjoint_march_kernel<D_, S_><<<grid, wpc * 32, smem, st>>>(mc, ac, coef, dc, ncell, npix, nz, nv, what, grad);      \
   } while (0)
   if (dust) { if (series) IRIS_LAUNCH_ADJ(true, true); else IRIS_LAUNCH_ADJ(true, false); }
   else { if (series) IRIS_LAUNCH_ADJ(false, true); else IRIS_LAUNCH_ADJ(false, false); }

@@ -669,8 +669,9 @@ iris_so_status iris_so_noise(iris_so_ctx* ctx, float* d_cube, void* stream) {
   return run_noise(ctx, d_cube, static_cast<cudaStream_t>(stream));
 }
 
-iris_so_status iris_so_observe_adjoint(iris_so_ctx* ctx, const float* d_nH2, const float* d_Tgas, const float* d_Tdust,
-                                       const float* d_vlos, const float* d_w, float* d_grad, void* stream) {
+static iris_so_status observe_adjoint_impl(iris_so_ctx* ctx, const float* d_nH2, const float* d_Tgas, const float* d_Tdust,
+                                          const float* d_vlos, const float* d_w, float* d_grad, void* stream,
+                                          bool wrt_abundance) {
   if (!ctx) return IRIS_SO_EINVAL;
   if (!d_nH2 || !d_Tgas || !d_Tdust || !d_vlos || !d_w || !d_grad)
     return fail(ctx, IRIS_SO_EINVAL, "iris_so_observe_adjoint: NULL pointer");
@@ -697,11 +698,24 @@ iris_so_status iris_so_observe_adjoint(iris_so_ctx* ctx, const float* d_nH2, con
     what = wb;
   }
   ProfScope prof(ctx, IRIS_SO_STAGE_ADJOINT, st);
-  cudaError_t e = iris::launch_adjoint(ctx->mc, ctx->ac, ctx->lc, c.n_levels, ctx->band, ctx->d_coef, dcoef, ctx->ncell, (int)ctx->npix,
+  iris::AdjointConsts ac = ctx->ac;
+  if (wrt_abundance) ac.c_d = 0.0f;                    // the dust does not depend on the tracer abundance
+  cudaError_t e = iris::launch_adjoint(ctx->mc, ac, ctx->lc, c.n_levels, ctx->band, ctx->d_coef, dcoef, ctx->ncell, (int)ctx->npix,
                                        c.nz, c.nv, c.dust_on != 0, resolved_algo(c) == IRIS_SO_ALGO_WINDOW, d_nH2, d_Tgas, what,
-                                       d_grad, st, &ctx->launches);
+                                       d_grad, st, &ctx->launches, wrt_abundance);
   if (e != cudaSuccess) return cuda_fail(ctx, e, "launch of adjoint kernels");
   return IRIS_SO_OK;
+}
+
+iris_so_status iris_so_observe_adjoint(iris_so_ctx* ctx, const float* d_nH2, const float* d_Tgas, const float* d_Tdust,
+                                       const float* d_vlos, const float* d_w, float* d_grad, void* stream) {
+  return observe_adjoint_impl(ctx, d_nH2, d_Tgas, d_Tdust, d_vlos, d_w, d_grad, stream, false);
+}
+
+iris_so_status iris_so_observe_adjoint_abundance(iris_so_ctx* ctx, const float* d_nH2, const float* d_Tgas,
+                                                 const float* d_Tdust, const float* d_vlos, const float* d_w,
+                                                 float* d_grad, void* stream) {
+  return observe_adjoint_impl(ctx, d_nH2, d_Tgas, d_Tdust, d_vlos, d_w, d_grad, stream, true);
 }
 
 iris_so_status iris_so_density_trace(iris_so_ctx* ctx, const float* d_nH2, const float* d_vlos, float* d_cube, void* stream) {

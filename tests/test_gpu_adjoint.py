@@ -125,3 +125,33 @@ def test_batch_workload_cubes_and_gradient():
         assert_spectra(cube, ref, extra=8e-6 * cfg.noise_sigma, peak_of=clean, what="batch cube %d" % i)
         check(cfg, f, weight_cube(cfg), n_fd=24, label="batch cube %d (v_edge %.0f, sigma_t %.1f km/s)" %
               (i, f["meta"]["v_edge_kms"], f["meta"]["sigma_t_kms"]))
+
+
+@pytest.mark.parametrize("case", ["dust_beam", "thick", "no_dust"])
+def test_abundance_gradient(case):
+    """iris_so_observe_adjoint_abundance: dL / d ln X per cell against the oracle's analytic adjoint (every cell) and its
+    finite differences (sampled cells)."""
+    from paper_2607_01338_b200 import IrisSO
+    if case == "no_dust":
+        cfg, r = make_workload("tiny", n=16, nv=64)
+    else:
+        cfg, r = make_workload("batch", n=20, nv=96)
+    f = make_fields(cfg, r)
+    f["vlos"] = (0.2 * f["vlos"]).astype(np.float32)
+    if case == "thick":
+        cfg = cfg.with_(abundance=2e-5)
+    w = weight_cube(cfg)
+    o = Oracle(cfg)
+    what = o.beam(w.astype(np.float64)) if cfg.beam_fwhm_px > 0 else w.astype(np.float64)
+    ref = o.grad_adjoint(f, what, wrt="abundance")
+    g = IrisSO(cfg).observe_adjoint(*[dev(f[k]) for k in ("nH2", "Tgas", "Tdust", "vlos")], dev(w.astype(np.float32)),
+                                    wrt="abundance").cpu().numpy().astype(np.float64).reshape(ref.shape)
+    # d / d ln X is (emission term) - (absorption term), both carried in fp32: where a line is saturated they cancel, so
+    # the floor is 3e-7 of the largest gradient instead of the 1e-7 of the density gradient (DESIGN.md, tolerances)
+    scale = 3.0 * np.abs(ref).max()
+    assert scale > 0 and np.all(np.isfinite(g))
+    worst = excess(g, ref, scale)
+    cells = np.argsort(-np.abs(ref).ravel())[:24]
+    worst_fd = excess(g.ravel()[cells], o.grad_fd(f, what, cells, eps=1e-5, wrt="abundance"), scale)
+    print("abundance gradient %s: worst vs analytic %.3g, vs finite differences %.3g of tolerance" % (case, worst, worst_fd))
+    assert worst <= 1.0 and worst_fd <= 1.0
