@@ -408,3 +408,28 @@ def test_very_many_channels_fall_back_to_the_dense_kernel():
     it = iris(cfg)
     assert it.transfer_kernel() == "transfer_dense_kernel"
     assert_spectra(it.observe(*dev_fields(f)).cpu().numpy(), Oracle(cfg).observe(f))
+
+
+def test_several_lines_share_one_level_solve():
+    """Multiple lines of one molecule: one context per line; the level populations are solved once
+    (iris_so_levelpop) and handed to every line's iris_so_transfer, which must give what that line's own solve gives
+    and what the oracle gives for that line."""
+    from iris_inputs.molecule import line_frequency
+    cfg21, r = make_workload("small", n=20, nv=96)
+    f = make_fields(cfg21, r)
+    f["vlos"] = (0.25 * f["vlos"]).astype(np.float32)
+    d = dev_fields(f)
+    pop = iris(cfg21).levelpop(d[0], d[1])
+    for up in (1, 2, 3, 4):
+        cfg = cfg21.with_(line_upper=up, line_lower=up - 1, nu0_Hz=line_frequency(cfg21.energy_K, up, up - 1),
+                          kappa_gas_cm2_g=cfg21.kappa_gas_cm2_g * (up / 2.0) ** 1.8)      # kappa_nu of this line's frequency
+        it = iris(cfg)
+        It_shared, Ic_shared = it.transfer(*d, pop=pop)
+        It_own, Ic_own = it.transfer(*d)
+        assert torch.equal(It_shared, It_own) and torch.equal(Ic_shared, Ic_own)
+        o = Oracle(cfg)
+        rt, rc = o.march(o.coefficients(f["nH2"], f["Tgas"], f["Tdust"]), f["vlos"])
+        K = krj(cfg.nu0_Hz)
+        got = It_shared.cpu().numpy().reshape(-1, cfg.nv).astype(np.float64)
+        line = np.abs(rt - rc[:, None]).max(axis=1)
+        assert np.all(np.abs(got - rt).max(axis=1) <= 1e-4 * line + 1e-6 / K + 3e-7 * np.abs(rt).max(axis=1)), "J=%d-%d" % (up, up - 1)
