@@ -234,27 +234,76 @@ __device__ __forceinline__ float channel_derf(int c, float c_los, float s) {
   return (copysignf(1.0f, G_hi) - copysignf(1.0f, G_lo)) - (G_hi - G_lo);
 }
 
-// K8: one warp per pixel.  Shared memory per warp: 5 * nv floats (xrem, P, Q, Dt, what).
-template <bool DUST, bool SERIES>
+// Sums over the LPP lanes of a pixel (aligned lane groups of a warp).
+template <int LPP>
+__device__ __forceinline__ float seg_sum(float v, unsigned gmask) {
+#pragma unroll
+  for (int o = LPP / 2; o > 0; o >>= 1) v += __shfl_xor_sync(gmask, v, o);
+  return v;
+}
+
+// Eight sums over the LPP lanes of a pixel at once: three exchange steps halve the number of values a lane carries
+// (lanes with the bit set keep the upper half), the remaining steps finish the one value that is left, and the eight
+// totals (index j at lane (LPP / 8) j of the group) are broadcast back: 7 + log2(LPP / 8) + 8 shuffles instead of
+// 8 log2(LPP).
+template <int LPP>
+__device__ __forceinline__ void seg_sum8(float (&v)[8], unsigned gmask, int gbase) {
+  constexpr int H = LPP / 2;
+  const int lane = threadIdx.x & 31;
+  const bool b1 = lane & H, b2 = lane & (H / 2), b3 = lane & (H / 4);
+  float a[4], b[2], r;
+#pragma unroll
+  for (int j = 0; j < 4; ++j) {
+    const float send = b1 ? v[j] : v[j + 4];
+    a[j] = (b1 ? v[j + 4] : v[j]) + __shfl_xor_sync(gmask, send, H);
+  }
+#pragma unroll
+  for (int j = 0; j < 2; ++j) {
+    const float send = b2 ? a[j] : a[j + 2];
+    b[j] = (b2 ? a[j + 2] : a[j]) + __shfl_xor_sync(gmask, send, H / 2);
+  }
+  {
+    const float send = b3 ? b[0] : b[1];
+    r = (b3 ? b[1] : b[0]) + __shfl_xor_sync(gmask, send, H / 4);
+  }
+#pragma unroll
+  for (int o = H / 8; o > 0; o >>= 1) r += __shfl_xor_sync(gmask, r, o);
+#pragma unroll
+  for (int j = 0; j < 8; ++j) v[j] = __shfl_sync(gmask, r, gbase + (H / 4) * j);
+}
+
+// K8: LPP lanes per pixel, 32 / LPP pixels per warp (the launcher picks 16 or 32 from nv: five spectra per pixel live in
+// shared memory).  Shared memory per warp: 5 arrays (xrem, P, Q, Dt, what) of nvp * PPW floats, channel c
+// of pixel g at word (c / LPP) * 32 + g * LPP + c % LPP of its array (conflict-free for the lanes of a warp).  The
+// per-cell scalars (window, dust factors, gradient assembly) are computed once per pixel group, so more pixels per warp
+// means fewer instructions per (pixel, cell).
+template <bool DUST, bool SERIES, int LPP>
 __global__ void __launch_bounds__(128)
 adjoint_march_kernel(MarchConsts mc, AdjointConsts ac, const float* __restrict__ coef, const float* __restrict__ dcoef,
-                     int64_t ncell, int npix, int nz, int nv, const float* __restrict__ what, float* __restrict__ grad) {
+                     int64_t ncell, int npix, int nz, int nv, int nvp, const float* __restrict__ what,
+                     float* __restrict__ grad) {
   extern __shared__ float sm[];
+  constexpr int PPW = 32 / LPP;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, wpc = blockDim.x >> 5;
-  const int pix = blockIdx.x * wpc + warp;
-  if (pix >= npix) return;                                   // whole warps only; no CTA-wide barrier below
-  float* xrem = sm + (size_t)warp * 5 * nv;                  // line optical depth still ahead of the march
-  float* P = xrem + nv;                                      // what * exp(-xrem)
-  float* Q = P + nv;                                         // what * (1 - exp(-xrem))
-  float* Dt = Q + nv;                                        // (I_total - I_cont) * G, as in transfer_window.cuh
-  float* wh = Dt + nv;
+  const int g = lane / LPP, i = lane % LPP, gbase = g * LPP;
+  const unsigned gmask = LPP == 32 ? 0xffffffffu : (((1u << (LPP & 31)) - 1u) << gbase);
+  const int pix_raw = (blockIdx.x * wpc + warp) * PPW + g;
+  const bool valid = pix_raw < npix;
+  const int pix = valid ? pix_raw : npix - 1;                // idle groups shadow the last pixel and write nothing
+  const size_t arr = (size_t)nvp * PPW;
+  float* xrem = sm + (size_t)warp * 5 * arr + gbase;         // line optical depth still ahead of the march
+  float* P = xrem + arr;                                     // what * exp(-xrem)
+  float* Q = P + arr;                                        // what * (1 - exp(-xrem))
+  float* Dt = Q + arr;                                       // (I_total - I_cont) * G, as in transfer_window.cuh
+  float* wh = Dt + arr;
+#define IDX(c) (((c) / LPP) * 32 + ((c) % LPP))
   float Wtot = 0.0f;
-  for (int c = lane; c < nv; c += 32) {
+  for (int c = i; c < nv; c += LPP) {
     const float w = what[(int64_t)pix * nv + c];
-    wh[c] = w; xrem[c] = 0.0f; Dt[c] = 0.0f;
+    wh[IDX(c)] = w; xrem[IDX(c)] = 0.0f; Dt[IDX(c)] = 0.0f;
     Wtot += w;
   }
-  Wtot = warp_sum(Wtot);
+  Wtot = seg_sum<LPP>(Wtot, gmask);
   __syncwarp();
 
   // first march: total line optical depth per channel and total dust optical depth
@@ -268,9 +317,9 @@ adjoint_march_kernel(MarchConsts mc, AdjointConsts ac, const float* __restrict__
     if (W > 0) {
       CentreProfile prof;
       if (SERIES) prof.set(s);
-      for (int c = klo + lane; c <= khi; c += 32) {
+      for (int c = klo + i; c <= khi; c += LPP) {
         const float dErf = SERIES ? prof.at(((float)c + 0.5f - c_los) * s) : channel_derf(c, c_los, s);
-        xrem[c] = fmaf(a_c, dErf, xrem[c]);
+        xrem[IDX(c)] = fmaf(a_c, dErf, xrem[IDX(c)]);
       }
     }
     __syncwarp();
@@ -279,14 +328,14 @@ adjoint_march_kernel(MarchConsts mc, AdjointConsts ac, const float* __restrict__
   // them only through the channels of its window, so the sums over the channels OUTSIDE the window (which only
   // the dust of the cell acts on) are SQ - sum_window Q and SPD - sum_window P Dt -- no pass over all nv channels.
   float SQ = 0.0f, SPD = 0.0f;
-  for (int c = lane; c < nv; c += 32) {
-    const float xr = xrem[c], w = wh[c];
-    P[c] = w * exp_neg(xr);
+  for (int c = i; c < nv; c += LPP) {
+    const float xr = xrem[IDX(c)], w = wh[IDX(c)];
+    P[IDX(c)] = w * exp_neg(xr);
     const float q = w * one_minus_exp_neg(xr);
-    Q[c] = q;
+    Q[IDX(c)] = q;
     SQ += q;
   }
-  SQ = warp_sum(SQ);
+  SQ = seg_sum<LPP>(SQ, gmask);
   __syncwarp();
 
   // second march: forward state and closed-form adjoint together
@@ -312,19 +361,20 @@ adjoint_march_kernel(MarchConsts mc, AdjointConsts ac, const float* __restrict__
     if (W > 0) {
       CentreProfile prof;
       if (SERIES) prof.set(s);
-      for (int c = klo + lane; c <= khi; c += 32) {
+      for (int c = klo + i; c <= khi; c += LPP) {
+        const int k = IDX(c);
         const float dErf = SERIES ? prof.at(((float)c + 0.5f - c_los) * s) : channel_derf(c, c_los, s);
         const float tau_L = a_c * dErf, J_L = e_c * dErf, tau_T = tau_L + tau_d;
-        const float xr = xrem[c] - tau_L;
-        const float w = wh[c];
+        const float xr = xrem[k] - tau_L;
+        const float w = wh[k];
         const float Pn = w * exp_neg(xr);
         const float Qn = w * one_minus_exp_neg(xr);
-        const float Dto = Dt[c];
+        const float Dto = Dt[k];
         if (DUST) {
-          winQ_old += Q[c]; winQ_new += Qn;
-          winPD_old = fmaf(P[c], Dto, winPD_old);
+          winQ_old += Q[k]; winQ_new += Qn;
+          winPD_old = fmaf(P[k], Dto, winPD_old);
         }
-        xrem[c] = xr; P[c] = Pn; Q[c] = Qn;
+        xrem[k] = xr; P[k] = Pn; Q[k] = Qn;
         const float Tk = fmaf(Dto, invG, C);
         const float mT = one_minus_exp_neg(tau_T);
         float wT, wpT;
@@ -339,7 +389,7 @@ adjoint_march_kernel(MarchConsts mc, AdjointConsts ac, const float* __restrict__
         float Dn;
         if (DUST) {
           const float m = one_minus_exp_neg(tau_L);
-          const float r = rcp_approx(tau_T == 0.0f ? 1.0f : tau_T);
+          const float r = rcp_approx(fabsf(tau_T) < 1.0e-30f ? 1.0f : tau_T);
           const float Em = E_d * m;
           const float t1 = m_d + Em;
           const float t2 = fmaf(tau_d, Em, -tau_L * m_d);
@@ -349,16 +399,16 @@ adjoint_march_kernel(MarchConsts mc, AdjointConsts ac, const float* __restrict__
         } else {
           Dn = update_nodust(Dto, dErf, a_c, sc);
         }
-        Dt[c] = Dn;
+        Dt[k] = Dn;
         if (DUST) winPD_new = fmaf(Pn, Dn, winPD_new);
       }
     }
     if (!DUST) {
-      acc_e = warp_sum(acc_e); acc_a = warp_sum(acc_a);
+      acc_e = seg_sum<LPP>(acc_e, gmask); acc_a = seg_sum<LPP>(acc_a, gmask);
     } else {
-      if (W > 0) {
+      if (W > 0) {                                           // W is the same for the LPP lanes of the pixel
         float r8[8] = {acc_e, acc_a, acc_d, accW, winQ_old, winQ_new, winPD_old, winPD_new};
-        warp_sum8(r8);
+        seg_sum8<LPP>(r8, gmask, gbase);
         acc_e = r8[0]; acc_a = r8[1]; acc_d = r8[2]; accW = r8[3];
         winQ_old = r8[4]; winQ_new = r8[5]; winPD_old = r8[6]; winPD_new = r8[7];
       }
@@ -368,32 +418,33 @@ adjoint_march_kernel(MarchConsts mc, AdjointConsts ac, const float* __restrict__
       SQ += winQ_new - winQ_old;
       SPD += winPD_new - winPD_old;
     }
-    if (lane == 0) {
+    if (i == 0 && valid) {
       const int64_t cell = (int64_t)z * npix + pix;
       const float pre = ac.scale * Lam;
-      float g = pre * (acc_e * dcoef[cell] + acc_a * dcoef[ncell + cell]);
+      float gr = pre * (acc_e * dcoef[cell] + acc_a * dcoef[ncell + cell]);
       if (DUST) {
         const float sub = ac.subtract ? 1.0f : 0.0f;
         const float dSC = S_d - C;
         const float outside = fmaf(dSC, (1.0f - sub) * (Wtot - accW) - accQ, -invG * accPD);
         const float g_d = pre * (acc_d - sub * E_d * dSC * accW + E_d * outside);
-        g = fmaf(g_d, ac.c_d, g);
+        gr = fmaf(g_d, ac.c_d, gr);
       }
-      grad[cell] = g;
+      grad[cell] = gr;
     }
     if (DUST) {
       C = fmaf(C, E_d, S_d * m_d);
       G = Gn;
-      if (G > 1.0e18f) {
+      if (G > 1.0e18f) {                                     // the same for the LPP lanes of the pixel
         const float inv = 1.0f / G;
-        __syncwarp();
-        for (int c = lane; c < nv; c += 32) Dt[c] *= inv;
+        __syncwarp(gmask);
+        for (int c = i; c < nv; c += LPP) Dt[IDX(c)] *= inv;
         SPD *= inv;
         G = 1.0f;
       }
     }
     __syncwarp();
   }
+#undef IDX
 }
 
 // band <= kBandNarrow selects the banded elimination (BW = kBandNarrow), anything wider the dense one.
@@ -433,19 +484,32 @@ inline cudaError_t launch_adjoint(const MarchConsts& mc, const AdjointConsts& ac
 march:
   cudaError_t e;
   const float* dc = wrt_abundance ? coef : dcoef;
+  // lanes per pixel: 16 (two pixels per warp) up to 384 channels, one warp per pixel beyond: five spectra per pixel live
+  // in shared memory.  Measured on 128^3 x 256 channels: 8 lanes 1.35 ms, 16 lanes 1.05 ms, 32 lanes 1.24 ms.
+  const int lpp = nv <= 384 ? 16 : 32;
+  const int ppw = 32 / lpp;
+  const int nvp = (nv + lpp - 1) / lpp * lpp;
+  const size_t per_warp = (size_t)5 * nvp * ppw * sizeof(float);
   int wpc = 4;
-  while (wpc > 1 && (size_t)wpc * 5 * nv * sizeof(float) > 200 * 1024) wpc >>= 1;
-  const size_t smem = (size_t)wpc * 5 * nv * sizeof(float);
+  while (wpc > 1 && wpc * per_warp > 200 * 1024) wpc >>= 1;
+  const size_t smem = wpc * per_warp;
   if (smem > 227 * 1024) return cudaErrorInvalidConfiguration;
-  const unsigned grid = (unsigned)((npix + wpc - 1) / wpc);
-#define IRIS_LAUNCH_ADJ(D_, S_)                                                                                        \
-  do {                                                                                                                 \
-    e = cudaFuncSetAttribute(adjoint_march_kernel<D_, S_>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);    \
-    if (e != cudaSuccess) return e;                                                                                    \
-    adjoint_march_kernel<D_, S_><<<grid, wpc * 32, smem, st>>>(mc, ac, coef, dc, ncell, npix, nz, nv, what, grad);      \
+  const unsigned grid = (unsigned)((npix + wpc * ppw - 1) / (wpc * ppw));
+#define IRIS_LAUNCH_ADJ(D_, S_, L_)                                                                                        \
+  do {                                                                                                                     \
+    e = cudaFuncSetAttribute(adjoint_march_kernel<D_, S_, L_>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);    \
+    if (e != cudaSuccess) return e;                                                                                        \
+    adjoint_march_kernel<D_, S_, L_><<<grid, wpc * 32, smem, st>>>(mc, ac, coef, dc, ncell, npix, nz, nv, nvp, what, grad); \
   } while (0)
-  if (dust) { if (series) IRIS_LAUNCH_ADJ(true, true); else IRIS_LAUNCH_ADJ(true, false); }
-  else { if (series) IRIS_LAUNCH_ADJ(false, true); else IRIS_LAUNCH_ADJ(false, false); }
+#define IRIS_LAUNCH_ADJ_L(D_, S_)                                         \
+  do {                                                                    \
+    if (lpp == 8) IRIS_LAUNCH_ADJ(D_, S_, 8);                             \
+    else if (lpp == 16) IRIS_LAUNCH_ADJ(D_, S_, 16);                      \
+    else IRIS_LAUNCH_ADJ(D_, S_, 32);                                     \
+  } while (0)
+  if (dust) { if (series) IRIS_LAUNCH_ADJ_L(true, true); else IRIS_LAUNCH_ADJ_L(true, false); }
+  else { if (series) IRIS_LAUNCH_ADJ_L(false, true); else IRIS_LAUNCH_ADJ_L(false, false); }
+#undef IRIS_LAUNCH_ADJ_L
 #undef IRIS_LAUNCH_ADJ
   e = cudaGetLastError();
   if (e == cudaSuccess) ++*launches;
