@@ -53,6 +53,10 @@ class ObsConfig:
     transfer_mode: int = 0        # 0 optically thick, 1 selectively thin, 2 optically thin
     integration: int = 0          # 0 formal, 1 smooth (TR + BDF2; Simpson in thin mode)
     subsample: int = 0            # thick mode: 0 = channel-integrated profile; odd f = fine grid + Simpson (Eq. 4.5.1)
+    # tabulated collision rates of several partners; None = the power law coll_down_ref (T/T_ref)^p
+    coll_T_grid: np.ndarray = None        # [nT] ascending temperatures (K)
+    coll_table: np.ndarray = None         # [P, nT, n_levels, n_levels] K_ul of partner p at T_grid[t], 0 where u <= l
+    coll_partner_frac: np.ndarray = None  # [P] number density of partner p per n_H2
     # free-form label, ignored by both implementations
     name: str = field(default="", compare=False)
 

@@ -56,6 +56,12 @@ struct orc_config {
   int32_t integration;     // 0 formal, 1 smooth (4.8: TR first step + BDF2; 4.7.7: Simpson in thin mode)
   int32_t subsample;       // thick mode only: 0 = channel-integrated profile (R1); odd f >= 1 = fine velocity
                            // grid with f added midpoints per channel + Simpson over frequency (4.5, Eq. 4.5.1)
+  // tabulated collision rates of several partners (LAMDA tables "interpolated in temperature";
+  // H, para-H2, ortho-H2 at 3:1, He at 0.1 per H).  coll_n_partners = 0: the power law above.
+  int32_t coll_n_partners, coll_nT;
+  const double *coll_T_grid;        // [nT] ascending temperatures
+  const double *coll_table;         // [P][nT][n_levels * n_levels]  K_ul of partner p at T_grid[t], 0 where u <= l
+  const double *coll_partner_frac;  // [P] number density of partner p per n_H2
 };
 
 // Planck function B_nu(T), Eq. 3.2.1 = Eq. 3.6.2 = Eq. 4.9.1.
@@ -85,6 +91,32 @@ double orc_rayleigh_jeans_T(double nu, double I) { return kC * kC * I / (2.0 * k
 //   K_lu = K_ul (g_u / g_l) exp(-(E_u - E_l) / T_gas)  (Eq. 3.7.2, detailed balance)
 //   B_ul = c^2 / (2 h nu^3) A_ul,  B_lu = (g_u / g_l) B_ul   (Eq. 3.7.1)
 //   J_ul = B_nu_ul(T_bar)                              (Eq. 3.6.2, reading G2: the temperature is T_bar)
+// Tabulated de-excitation rate per unit n_H2 (reading S30): every partner's table is interpolated linearly
+// in temperature between its grid points and held constant outside the grid (the LAMDA convention), and the partners
+// add with their number densities per n_H2:  K_ul(T) = sum_p f_p K^p_ul(T)   (Eq. 3.6.3 summed over partners).
+static double table_rate(const orc_config *c, int u, int l, double T) {
+  const int N = c->n_levels, nT = c->coll_nT;
+  const double *Tg = c->coll_T_grid;
+  int t0 = 0;
+  double w = 0.0;
+  if (nT > 1) {
+    if (T <= Tg[0]) { t0 = 0; w = 0.0; }
+    else if (T >= Tg[nT - 1]) { t0 = nT - 2; w = 1.0; }
+    else {
+      while (t0 + 2 < nT && T >= Tg[t0 + 1]) ++t0;
+      w = (T - Tg[t0]) / (Tg[t0 + 1] - Tg[t0]);
+    }
+  }
+  double K = 0.0;
+  for (int p = 0; p < c->coll_n_partners; ++p) {
+    const double *tab = c->coll_table + ((int64_t)p * nT) * N * N;
+    const double k0 = tab[(int64_t)t0 * N * N + u * N + l];
+    const double k1 = nT > 1 ? tab[(int64_t)(t0 + 1) * N * N + u * N + l] : k0;
+    K += c->coll_partner_frac[p] * (k0 + w * (k1 - k0));
+  }
+  return K;
+}
+
 void orc_rates(const orc_config *c, double nH2, double Tgas, double *R) {
   const int N = c->n_levels;
   for (int i = 0; i < N * N; ++i) R[i] = 0.0;
@@ -93,11 +125,17 @@ void orc_rates(const orc_config *c, double nH2, double Tgas, double *R) {
       const double dE = c->energy_K[u] - c->energy_K[l];   // (E_u - E_l) / k, Kelvin
       const double gr = c->weight[u] / c->weight[l];
       double down = 0.0, up = 0.0;
-      const double Kul = c->coll_down_ref[u * N + l];
-      if (Kul != 0.0) {
-        const double K = Kul * std::pow(Tgas / c->coll_T_ref, c->coll_T_exp);
+      if (c->coll_n_partners > 0) {
+        const double K = table_rate(c, u, l, Tgas);
         down += K * nH2;
         up += K * gr * std::exp(-dE / Tgas) * nH2;
+      } else {
+        const double Kul = c->coll_down_ref[u * N + l];
+        if (Kul != 0.0) {
+          const double K = Kul * std::pow(Tgas / c->coll_T_ref, c->coll_T_exp);
+          down += K * nH2;
+          up += K * gr * std::exp(-dE / Tgas) * nH2;
+        }
       }
       const double A = c->einstein_A[u * N + l];
       if (A != 0.0) {

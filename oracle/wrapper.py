@@ -54,6 +54,9 @@ class _Cfg(C.Structure):
         ("noise_gamma_mode", C.c_int32),
         ("seed", C.c_uint64),
         ("transfer_mode", C.c_int32), ("integration", C.c_int32), ("subsample", C.c_int32),
+        ("coll_n_partners", C.c_int32), ("coll_nT", C.c_int32),
+        ("coll_T_grid", C.POINTER(C.c_double)), ("coll_table", C.POINTER(C.c_double)),
+        ("coll_partner_frac", C.POINTER(C.c_double)),
     ]
 
 
@@ -83,15 +86,32 @@ class Oracle:
         self._keep = [np.ascontiguousarray(np.asarray(getattr(cfg, k), dtype=np.float64))
                       for k in ("energy_K", "weight", "einstein_A", "coll_down_ref")]
         s = _Cfg()
+        table = getattr(cfg, "coll_table", None)
+        if table is not None:
+            tab = np.ascontiguousarray(np.asarray(table, dtype=np.float64))
+            grid = np.ascontiguousarray(np.asarray(cfg.coll_T_grid, dtype=np.float64))
+            frac = np.ascontiguousarray(np.asarray(cfg.coll_partner_frac, dtype=np.float64))
+            n = len(self._keep[0])
+            assert tab.ndim == 4 and tab.shape[1:] == (grid.size, n, n) and frac.shape == (tab.shape[0],)
+            self._keep += [tab, grid, frac]
         for name, ctype in _Cfg._fields_:
-            if name in ("energy_K", "weight", "einstein_A", "coll_down_ref"):
+            if name in ("energy_K", "weight", "einstein_A", "coll_down_ref", "coll_T_grid", "coll_table",
+                        "coll_partner_frac"):
+                continue
+            if name == "coll_n_partners":
+                s.coll_n_partners = 0 if table is None else int(tab.shape[0])
+                continue
+            if name == "coll_nT":
+                s.coll_nT = 0 if table is None else int(grid.size)
                 continue
             if name == "n_levels":
                 s.n_levels = len(self._keep[0])
                 continue
             val = getattr(cfg, name)
             setattr(s, name, float(val) if ctype is C.c_double else int(val))
-        s.energy_K, s.weight, s.einstein_A, s.coll_down_ref = (_dp(a) for a in self._keep)
+        s.energy_K, s.weight, s.einstein_A, s.coll_down_ref = (_dp(a) for a in self._keep[:4])
+        if table is not None:
+            s.coll_table, s.coll_T_grid, s.coll_partner_frac = (_dp(a) for a in self._keep[4:7])
         self.s = s
         self.N = int(s.n_levels)
         self.threads = threads

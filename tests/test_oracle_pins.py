@@ -530,3 +530,41 @@ def test_abundance_gradient_pins():
     pb = (special.erf((vk[None] + cfg.dv_cms / 2 - vl) / b) - special.erf((vk[None] - cfg.dv_cms / 2 - vl) / b)) / (2 * dnuW)
     expect = KRJ * coef[0].reshape(cfg.nz, plane)[:, p] * cfg.cell_cm * (pb * w.reshape(plane, cfg.nv)[p][None]).sum(axis=1)
     assert np.allclose(gt[:, p], expect, rtol=1e-4, atol=1e-9 * np.abs(expect).max())
+
+
+# ------------------------------------------------------------------------------------------------
+# tabulated collision rates of several partners
+def _power_law_table(cfg, T_grid, split=(1.0,)):
+    """The configuration's own power law K_ul(T_ref) (T / T_ref)^p sampled on T_grid, split over partners whose
+    fractions times tables add up to it."""
+    T_grid = np.asarray(T_grid, dtype=np.float64)
+    base = cfg.coll_down_ref[None] * (T_grid[:, None, None] / cfg.coll_T_ref) ** cfg.coll_T_exp
+    frac = np.asarray([0.75, 0.25, 0.2][: len(split)], dtype=np.float64)
+    table = np.stack([base * sh / fr for sh, fr in zip(split, frac)])
+    return cfg.with_(coll_T_grid=T_grid, coll_table=table, coll_partner_frac=frac)
+
+
+def test_tabulated_rates_reduce_to_the_power_law_and_add_over_partners():
+    cfg = base_cfg(10)
+    o = Oracle(cfg)
+    # at the grid points the table IS the power law; between them linear interpolation of T^0.2 on a 1 K grid is off by <= 1e-5
+    grid = np.arange(5.0, 200.5, 1.0)
+    ot = Oracle(_power_law_table(cfg, grid))
+    for nH2, T in ((1e3, 50.0), (3e5, 119.0), (10.0, 20.0)):
+        assert np.allclose(ot.rates(nH2, T), o.rates(nH2, T), rtol=1e-12)
+        assert np.allclose(ot.levelpop_cell(nH2, T + 0.37), o.levelpop_cell(nH2, T + 0.37), rtol=1e-4)
+    # three partners (para-H2, ortho-H2, He) whose weighted tables add up to the same total: identical rates
+    o3 = Oracle(_power_law_table(cfg, grid, split=(0.2, 0.5, 0.3)))
+    assert np.allclose(o3.rates(2e4, 77.3), ot.rates(2e4, 77.3), rtol=1e-13)
+    # linear interpolation between two grid points, constant outside the grid (reading S30)
+    coarse = _power_law_table(cfg, [20.0, 100.0])
+    oc = Oracle(coarse)
+    K = lambda T: cfg.coll_down_ref[3, 2] * (T / cfg.coll_T_ref) ** cfg.coll_T_exp
+    R = oc.rates(1.0, 60.0) - Oracle(cfg.with_(coll_down_ref=0 * cfg.coll_down_ref)).rates(1.0, 60.0)
+    assert R[3, 2] == pytest.approx(0.5 * (K(20.0) + K(100.0)), rel=1e-12)
+    Rlo = oc.rates(1.0, 7.0) - Oracle(cfg.with_(coll_down_ref=0 * cfg.coll_down_ref)).rates(1.0, 7.0)
+    Rhi = oc.rates(1.0, 500.0) - Oracle(cfg.with_(coll_down_ref=0 * cfg.coll_down_ref)).rates(1.0, 500.0)
+    assert Rlo[3, 2] == pytest.approx(K(20.0), rel=1e-12) and Rhi[3, 2] == pytest.approx(K(100.0), rel=1e-12)
+    # detailed balance survives (Eq. 3.7.2): LTE limit is Boltzmann at the gas temperature
+    x = oc.levelpop_cell(1e13, 63.0)
+    assert np.allclose(x, boltzmann(cfg, 63.0), rtol=1e-6)
