@@ -104,6 +104,16 @@ typedef struct {
   int32_t subsample;            /* thick mode only: 0 = channel-integrated profile (Eq. 4.6.3); odd f >= 1 = point
                                  * profile (Eq. 3.3.3) on a fine velocity grid with f added midpoints per channel,
                                  * averaged over the channel by Simpson's rule (Eq. 4.5.1) */
+  /* Tabulated collision rates of several partners (LAMDA tables interpolated in temperature; H,
+   * para-H2, ortho-H2 at 3:1, He at 0.1 per H).  coll_n_partners = 0: the power law coll_down_ref (T / T_ref)^exp above.
+   * Otherwise K_ul(T) = sum_p coll_partner_frac[p] * K^p_ul(T) per unit n_H2, every table interpolated linearly in T
+   * between its grid points and held constant outside the grid; coll_down_ref / coll_T_ref / coll_T_exp are ignored.
+   * Host arrays, copied by create. */
+  int32_t coll_n_partners;          /* 0 .. 8 */
+  int32_t coll_nT;                  /* 1 .. 64 grid temperatures */
+  const double *coll_T_grid;        /* [coll_nT] strictly ascending, > 0 */
+  const double *coll_table;         /* [coll_n_partners][coll_nT][n_levels * n_levels] K_ul (cm^3/s) for u > l, else 0 */
+  const double *coll_partner_frac;  /* [coll_n_partners] number density of the partner per n_H2, >= 0 */
 } iris_so_config;
 
 /* Validates and copies the configuration (including the host arrays), selects the current CUDA device.

@@ -48,6 +48,9 @@ class _Config(C.Structure):
         ("seed", C.c_uint64),
         ("transfer_algo", C.c_int32),
         ("transfer_mode", C.c_int32), ("integration", C.c_int32), ("subsample", C.c_int32),
+        ("coll_n_partners", C.c_int32), ("coll_nT", C.c_int32),
+        ("coll_T_grid", C.POINTER(C.c_double)), ("coll_table", C.POINTER(C.c_double)),
+        ("coll_partner_frac", C.POINTER(C.c_double)),
     ]
 
 
@@ -116,10 +119,23 @@ def _make_config(cfg, transfer_algo):
     keep = [np.ascontiguousarray(np.asarray(getattr(cfg, k), dtype=np.float64))
             for k in ("energy_K", "weight", "einstein_A", "coll_down_ref")]
     s = _Config()
+    table = getattr(cfg, "coll_table", None)
+    if table is not None:
+        tab = np.ascontiguousarray(np.asarray(table, dtype=np.float64))
+        grid = np.ascontiguousarray(np.asarray(cfg.coll_T_grid, dtype=np.float64))
+        frac = np.ascontiguousarray(np.asarray(cfg.coll_partner_frac, dtype=np.float64))
+        n = len(keep[0])
+        if tab.ndim != 4 or tab.shape[1:] != (grid.size, n, n) or frac.shape != (tab.shape[0],):
+            raise ValueError("coll_table must be [P, nT, n_levels, n_levels] with coll_T_grid [nT], coll_partner_frac [P]")
+        keep += [tab, grid, frac]
     for name, ctype in _Config._fields_:
-        if name in ("energy_K", "weight", "einstein_A", "coll_down_ref"):
+        if name in ("energy_K", "weight", "einstein_A", "coll_down_ref", "coll_T_grid", "coll_table", "coll_partner_frac"):
             continue
-        if name == "n_levels":
+        if name == "coll_n_partners":
+            s.coll_n_partners = 0 if table is None else int(tab.shape[0])
+        elif name == "coll_nT":
+            s.coll_nT = 0 if table is None else int(grid.size)
+        elif name == "n_levels":
             s.n_levels = len(keep[0])
         elif name == "transfer_algo":
             s.transfer_algo = int(transfer_algo)
@@ -127,7 +143,9 @@ def _make_config(cfg, transfer_algo):
             val = getattr(cfg, name, 0)
             setattr(s, name, float(val) if ctype is C.c_double else int(val))
     ptr = lambda a: a.ctypes.data_as(C.POINTER(C.c_double))
-    s.energy_K, s.weight, s.einstein_A, s.coll_down_ref = (ptr(a) for a in keep)
+    s.energy_K, s.weight, s.einstein_A, s.coll_down_ref = (ptr(a) for a in keep[:4])
+    if table is not None:
+        s.coll_table, s.coll_T_grid, s.coll_partner_frac = (ptr(a) for a in keep[4:7])
     return s, keep
 
 

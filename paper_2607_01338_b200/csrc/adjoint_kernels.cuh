@@ -35,12 +35,28 @@ struct AdjointConsts {
 
 // Level fractions x and their logarithmic density derivative y = n dx/dn.  BW: bandwidth of the rate matrix
 // (see level_fractions in cell_kernels.cuh).
-template <int N, int BW>
-__device__ __forceinline__ void level_fractions_grad(const LevelConsts& lc, float n, float T, float (&x)[N], float (&y)[N]) {
+template <int N, int BW, bool TABLE>
+__device__ __forceinline__ void level_fractions_grad(const LevelConsts& lc, float n, float T, float (&x)[N],
+                                                     float (&y)[N]) {
+  const CollTable& tb = lc.tb;
   float R[N][N];
-  const float kf = n * exp2f(lc.Texp * log2f(T * lc.inv_Tref));
+  float kf = n, wt = 0.0f;
+  int t0 = 0;
+  if (TABLE) locate_temperature(tb, T, t0, wt);
+  else kf = n * exp2f(lc.Texp * log2f(T * lc.inv_Tref));
   float q[N];
   boltzmann_adjacent<N>(lc, T, q);
+  // collisional de-excitation rates of the band (per unit kf), and the same times g_u / g_l
+  auto coll = [&](int u, int l, float& Kd, float& Kg) {
+    const float4 pr = lc.pr[pair_index(u, l)];
+    Kd = pr.x; Kg = pr.z;
+    if (TABLE) {
+      const float2 k0 = tb.K[t0 * kMaxPairs + pair_index(u, l)];
+      const float2 k1 = tb.K[min(t0 + 1, tb.nT - 1) * kMaxPairs + pair_index(u, l)];
+      Kd = fmaf(wt, k1.x - k0.x, k0.x);
+      Kg = fmaf(wt, k1.y - k0.y, k0.y);
+    }
+  };
 #pragma unroll
   for (int u = 1; u < N; ++u) {
     float bz = 1.0f;
@@ -49,8 +65,10 @@ __device__ __forceinline__ void level_fractions_grad(const LevelConsts& lc, floa
       if (u - l > BW) continue;
       bz *= q[l + 1];
       const float4 pr = lc.pr[pair_index(u, l)];
-      R[u][l] = fmaf(kf, pr.x, pr.y);
-      R[l][u] = fmaf(kf * bz, pr.z, pr.w);
+      float Kd, Kg;
+      coll(u, l, Kd, Kg);
+      R[u][l] = fmaf(kf, Kd, pr.y);
+      R[l][u] = fmaf(kf * bz, Kg, pr.w);
     }
   }
   float inv[N];
@@ -96,8 +114,9 @@ __device__ __forceinline__ void level_fractions_grad(const LevelConsts& lc, floa
     for (int l = u - 1; l >= 0; --l) {
       if (u - l > BW) continue;
       bz *= q[l + 1];
-      const float4 pr = lc.pr[pair_index(u, l)];
-      const float f = x[u] * (kf * pr.x) - x[l] * (kf * bz * pr.z);   // net flow u -> l
+      float Kd, Kg;
+      coll(u, l, Kd, Kg);
+      const float f = x[u] * (kf * Kd) - x[l] * (kf * bz * Kg);   // net flow u -> l
       b[u] += f;
       b[l] -= f;
     }
@@ -126,7 +145,7 @@ __device__ __forceinline__ void level_fractions_grad(const LevelConsts& lc, floa
 }
 
 // K9 (per cell): d e_c / d n and d a_c / d n  ->  dcoef[2][ncell]
-template <int N, int BW>
+template <int N, int BW, bool TABLE>
 __global__ void __launch_bounds__(128) coef_grad_kernel(LevelConsts lc, AdjointConsts ac, int64_t ncell,
                                                         const float* __restrict__ nH2, const float* __restrict__ Tgas,
                                                         float* __restrict__ dcoef) {
@@ -134,7 +153,7 @@ __global__ void __launch_bounds__(128) coef_grad_kernel(LevelConsts lc, AdjointC
   if (i >= ncell) return;
   const float n = nH2[i], T = Tgas[i];
   float x[N], y[N];
-  level_fractions_grad<N, BW>(lc, n, T, x, y);
+  level_fractions_grad<N, BW, TABLE>(lc, n, T, x, y);
   float xu = 0.0f, xl = 0.0f;
 #pragma unroll
   for (int l = 0; l < N; ++l) {
@@ -453,8 +472,14 @@ inline void launch_coef_grad(const LevelConsts& lc, const AdjointConsts& ac, int
                              const float* T, float* dcoef, cudaStream_t st) {
   const unsigned grid = (unsigned)((ncell + 127) / 128);
   constexpr int BN = kBandNarrow < N - 1 ? kBandNarrow : N - 1;
-  if (band <= BN) coef_grad_kernel<N, BN><<<grid, 128, 0, st>>>(lc, ac, ncell, n, T, dcoef);
-  else coef_grad_kernel<N, N - 1><<<grid, 128, 0, st>>>(lc, ac, ncell, n, T, dcoef);
+  const bool table = lc.tb.K != nullptr;
+  if (band <= BN) {
+    if (table) coef_grad_kernel<N, BN, true><<<grid, 128, 0, st>>>(lc, ac, ncell, n, T, dcoef);
+    else coef_grad_kernel<N, BN, false><<<grid, 128, 0, st>>>(lc, ac, ncell, n, T, dcoef);
+  } else {
+    if (table) coef_grad_kernel<N, N - 1, true><<<grid, 128, 0, st>>>(lc, ac, ncell, n, T, dcoef);
+    else coef_grad_kernel<N, N - 1, false><<<grid, 128, 0, st>>>(lc, ac, ncell, n, T, dcoef);
+  }
 }
 
 // K9 then K8.  dcoef: scratch [2][ncell].  series: every cell has dv / b <= 0.55 (channel-centre profile expansion).  Returns the first CUDA error; *launches is advanced per kernel.

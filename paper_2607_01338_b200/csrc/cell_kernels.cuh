@@ -31,6 +31,15 @@ constexpr int kBandNarrow = 2;
 // pair index of (u > l)
 __host__ __device__ constexpr int pair_index(int u, int l) { return u * (u - 1) / 2 + l; }
 
+// Tabulated collision rates (several partners folded on the host: K_ul(T) = sum_p f_p K^p_ul(T)),
+// interpolated linearly in temperature and held constant outside the grid.  Device arrays owned by the context:
+// T[nT] ascending, K[nT][kMaxPairs] = { K_ul, K_ul g_u / g_l } (both times LevelConsts::rate_scale).
+struct CollTable {
+  const float* T;
+  const float2* K;
+  int nT;
+};
+
 struct LevelConsts {
   float ndE2[kMaxLevels];       // -(E_i - E_{i-1}) / k * log2(e)  [K], i >= 1: Boltzmann factor = 2^(ndE2 / T)
   // per pair (u > l), packed so that one 16-byte constant load feeds both rate FMAs:
@@ -38,7 +47,21 @@ struct LevelConsts {
   float4 pr[kMaxPairs];
   float inv_Tref, Texp;
   float rate_scale;             // every rate above has been multiplied by this (1 / largest Einstein A)
+  CollTable tb;                 // tb.K == nullptr: the power law K_ul(T_ref) (T / T_ref)^Texp of pr[].x / pr[].z
 };
+
+// interval t0 and weight w of temperature T: K = K[t0] + w (K[t0 + 1] - K[t0])
+__device__ __forceinline__ void locate_temperature(const CollTable& tb, float T, int& t0, float& w) {
+  if (tb.nT < 2) { t0 = 0; w = 0.0f; return; }
+  int lo = 0, hi = tb.nT - 1;              // invariant: T[lo] <= T < T[hi] once T is inside the grid
+  while (hi - lo > 1) {
+    const int mid = (lo + hi) >> 1;
+    if (T >= tb.T[mid]) lo = mid; else hi = mid;
+  }
+  t0 = lo;
+  const float a = tb.T[lo], b = tb.T[lo + 1];
+  w = fminf(fmaxf((T - a) / (b - a), 0.0f), 1.0f);
+}
 
 // Boltzmann factors of adjacent levels, q[i] = exp(-(E_i - E_{i-1}) / T), i >= 1: one MUFU.EX2 each.  The product
 // ndE2 / T is formed with its rounding error (FMA residual) and the error is applied to first order, so the factor
@@ -76,12 +99,16 @@ struct CoefConsts {
 // The fractions do not change when every rate is multiplied by one constant; the host divides all rates by the
 // largest Einstein A (LevelConsts::rate_scale), which keeps the pivots far from the fp32 denormal range so that
 // the reciprocals can be MUFU.RCP (1 ulp, flush-to-zero).
-template <int N, int BW>
+template <int N, int BW, bool TABLE = false>
 __device__ __forceinline__ void level_fractions(const LevelConsts& lc, float n, float T, float (&x)[N],
                                                 float* inv_tot = nullptr) {
+  const CollTable* tb = &lc.tb;
   float R[N][N];   // R[i][j]: rate i -> j (i != j); only |i - j| <= BW is touched
-  // n * (T / T_ref)^p
-  const float kf = n * exp2f(lc.Texp * log2f(T * lc.inv_Tref));
+  // power law: n * (T / T_ref)^p times K_ul(T_ref); table: n times the interpolated K_ul(T)
+  float kf = n, wt = 0.0f;
+  int t0 = 0;
+  if (TABLE) locate_temperature(*tb, T, t0, wt);
+  else kf = n * exp2f(lc.Texp * log2f(T * lc.inv_Tref));
   float q[N];      // Boltzmann factors of adjacent levels, exp(-(E_i - E_{i-1}) / T)
   boltzmann_adjacent<N>(lc, T, q);
 #pragma unroll
@@ -92,8 +119,15 @@ __device__ __forceinline__ void level_fractions(const LevelConsts& lc, float n, 
       if (u - l > BW) continue;
       bz *= q[l + 1];                                   // exp(-(E_u - E_l) / T), Eq. 3.7.2
       const float4 pr = lc.pr[pair_index(u, l)];
-      R[u][l] = fmaf(kf, pr.x, pr.y);
-      R[l][u] = fmaf(kf * bz, pr.z, pr.w);
+      float Kd = pr.x, Kg = pr.z;
+      if (TABLE) {
+        const float2 k0 = tb->K[t0 * kMaxPairs + pair_index(u, l)];
+        const float2 k1 = tb->K[min(t0 + 1, tb->nT - 1) * kMaxPairs + pair_index(u, l)];
+        Kd = fmaf(wt, k1.x - k0.x, k0.x);
+        Kg = fmaf(wt, k1.y - k0.y, k0.y);
+      }
+      R[u][l] = fmaf(kf, Kd, pr.y);
+      R[l][u] = fmaf(kf * bz, Kg, pr.w);
     }
   }
   // GTH elimination of states N-1 .. 1
@@ -146,19 +180,19 @@ __device__ __forceinline__ void cell_coefficients(const CoefConsts& cc, float n,
 }
 
 // K1: pop[N][ncell]
-template <int N, int BW>
+template <int N, int BW, bool TABLE>
 __global__ void __launch_bounds__(128) levelpop_kernel(LevelConsts lc, int64_t ncell, const float* __restrict__ nH2,
                                                        const float* __restrict__ Tgas, float* __restrict__ pop) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= ncell) return;
   float x[N];
-  level_fractions<N, BW>(lc, nH2[i], Tgas[i], x);
+  level_fractions<N, BW, TABLE>(lc, nH2[i], Tgas[i], x);
 #pragma unroll
   for (int l = 0; l < N; ++l) pop[(int64_t)l * ncell + i] = x[l];
 }
 
 // K1 + K2 fused: coef[6][ncell]; populations never leave registers.
-template <int N, int BW>
+template <int N, int BW, bool TABLE>
 __global__ void __launch_bounds__(128) cellcoef_kernel(LevelConsts lc, CoefConsts cc, int64_t ncell,
                                                        const float* __restrict__ nH2, const float* __restrict__ Tgas,
                                                        const float* __restrict__ Tdust, const float* __restrict__ vlos,
@@ -167,7 +201,7 @@ __global__ void __launch_bounds__(128) cellcoef_kernel(LevelConsts lc, CoefConst
   if (i >= ncell) return;
   const float n = nH2[i], T = Tgas[i];
   float x[N], inv;
-  level_fractions<N, BW>(lc, n, T, x, &inv);      // unnormalised fractions and 1 / their sum
+  level_fractions<N, BW, TABLE>(lc, n, T, x, &inv);      // unnormalised fractions and 1 / their sum
   // the two levels of the line, picked with one-hot constant vectors (static indexing keeps x[] in registers; a
   // dot product with constant operands is half the instructions of N compare-select pairs)
   float xu = 0.0f, xl = 0.0f;

@@ -37,6 +37,9 @@ thread_local std::string g_create_error;
 struct iris_so_ctx {
   iris_so_config cfg;
   std::vector<double> energy, weight, A, Kd;
+  std::vector<double> Keff;     // tabulated rates folded over the partners: [nT][N*N] per unit n_H2 (empty: power law)
+  std::vector<double> Tgrid;
+  float* d_colltab = nullptr;   // device copy: nT temperatures, then nT * kMaxPairs float2 {K, K g_u/g_l} * rate_scale
   iris::LevelConsts lc;
   iris::CoefConsts cc;
   iris::MarchConsts mc;
@@ -149,12 +152,12 @@ iris_so_status validate(const iris_so_config* c, std::string& why) {
   for (int u = 0; u < N; ++u) {
     double down = 0.0;
     for (int l = 0; l < N; ++l) {
-      const double a = c->einstein_A[u * N + l], k = c->coll_down_ref[u * N + l];
+      const double a = c->einstein_A[u * N + l], k = c->coll_n_partners > 0 ? 0.0 : c->coll_down_ref[u * N + l];
       if (l >= u && (a != 0.0 || k != 0.0)) return bad("einstein_A / coll_down_ref must be 0 for u <= l");
       if (a < 0.0 || k < 0.0 || !std::isfinite(a) || !std::isfinite(k)) return bad("rates must be finite and >= 0");
       down += a + k;
     }
-    if (u > 0 && !(down > 0.0)) return bad("every excited level needs a downward rate");
+    if (u > 0 && !(down > 0.0) && c->coll_n_partners == 0) return bad("every excited level needs a downward rate");
   }
   if (!(c->coll_T_ref > 0.0)) return bad("coll_T_ref must be > 0");
   if (c->line_upper <= c->line_lower || c->line_lower < 0 || c->line_upper >= N) return bad("bad line levels");
@@ -173,6 +176,22 @@ iris_so_status validate(const iris_so_config* c, std::string& why) {
   if (!(c->noise_sigma >= 0.0) || !std::isfinite(c->noise_mu)) return bad("bad noise parameters");
   if (c->noise_gamma_mode < 0 || c->noise_gamma_mode > 1) return bad("bad noise_gamma_mode");
   if (c->transfer_algo < 0 || c->transfer_algo > 3) return bad("bad transfer_algo");
+  if (c->coll_n_partners < 0 || c->coll_n_partners > 8) return bad("coll_n_partners must be in [0, 8]");
+  if (c->coll_n_partners > 0) {
+    if (c->coll_nT < 1 || c->coll_nT > 64) return bad("coll_nT must be in [1, 64]");
+    if (!c->coll_T_grid || !c->coll_table || !c->coll_partner_frac) return bad("collision table arrays must not be NULL");
+    for (int t = 0; t < c->coll_nT; ++t)
+      if (!(c->coll_T_grid[t] > 0.0) || (t > 0 && !(c->coll_T_grid[t] > c->coll_T_grid[t - 1])))
+        return bad("coll_T_grid must be positive and strictly ascending");
+    for (int p = 0; p < c->coll_n_partners; ++p)
+      if (!(c->coll_partner_frac[p] >= 0.0) || !std::isfinite(c->coll_partner_frac[p])) return bad("bad coll_partner_frac");
+    const int64_t nt = (int64_t)c->coll_n_partners * c->coll_nT * N * N;
+    for (int64_t q = 0; q < nt; ++q) {
+      const int ul = (int)(q % (N * N)), u = ul / N, l = ul % N;
+      const double k = c->coll_table[q];
+      if (k < 0.0 || !std::isfinite(k) || (l >= u && k != 0.0)) return bad("coll_table must be finite, >= 0 and 0 for u <= l");
+    }
+  }
   if (c->transfer_mode < 0 || c->transfer_mode > 2) return bad("transfer_mode must be 0 (thick), 1 (selectively thin) or 2 (thin)");
   if (c->integration < 0 || c->integration > 1) return bad("integration must be 0 (formal) or 1 (smooth)");
   if (c->subsample < 0 || c->subsample > 255 || (c->subsample > 0 && c->subsample % 2 == 0))
@@ -282,8 +301,14 @@ void launch_levelpop(iris_so_ctx* ctx, const float* n, const float* T, float* po
   const int64_t nc = ctx->ncell;
   const unsigned grid = (unsigned)((nc + 127) / 128);
   constexpr int BN = iris::kBandNarrow < N - 1 ? iris::kBandNarrow : N - 1;
-  if (ctx->band <= BN) iris::levelpop_kernel<N, BN><<<grid, 128, 0, st>>>(ctx->lc, nc, n, T, pop);
-  else iris::levelpop_kernel<N, N - 1><<<grid, 128, 0, st>>>(ctx->lc, nc, n, T, pop);
+  const bool table = ctx->lc.tb.K != nullptr;
+  if (ctx->band <= BN) {
+    if (table) iris::levelpop_kernel<N, BN, true><<<grid, 128, 0, st>>>(ctx->lc, nc, n, T, pop);
+    else iris::levelpop_kernel<N, BN, false><<<grid, 128, 0, st>>>(ctx->lc, nc, n, T, pop);
+  } else {
+    if (table) iris::levelpop_kernel<N, N - 1, true><<<grid, 128, 0, st>>>(ctx->lc, nc, n, T, pop);
+    else iris::levelpop_kernel<N, N - 1, false><<<grid, 128, 0, st>>>(ctx->lc, nc, n, T, pop);
+  }
 }
 
 template <int N>
@@ -292,8 +317,14 @@ void launch_cellcoef(iris_so_ctx* ctx, const float* n, const float* T, const flo
   const int64_t nc = ctx->ncell;
   const unsigned grid = (unsigned)((nc + 127) / 128);
   constexpr int BN = iris::kBandNarrow < N - 1 ? iris::kBandNarrow : N - 1;
-  if (ctx->band <= BN) iris::cellcoef_kernel<N, BN><<<grid, 128, 0, st>>>(ctx->lc, ctx->cc, nc, n, T, Td, v, coef);
-  else iris::cellcoef_kernel<N, N - 1><<<grid, 128, 0, st>>>(ctx->lc, ctx->cc, nc, n, T, Td, v, coef);
+  const bool table = ctx->lc.tb.K != nullptr;
+  if (ctx->band <= BN) {
+    if (table) iris::cellcoef_kernel<N, BN, true><<<grid, 128, 0, st>>>(ctx->lc, ctx->cc, nc, n, T, Td, v, coef);
+    else iris::cellcoef_kernel<N, BN, false><<<grid, 128, 0, st>>>(ctx->lc, ctx->cc, nc, n, T, Td, v, coef);
+  } else {
+    if (table) iris::cellcoef_kernel<N, N - 1, true><<<grid, 128, 0, st>>>(ctx->lc, ctx->cc, nc, n, T, Td, v, coef);
+    else iris::cellcoef_kernel<N, N - 1, false><<<grid, 128, 0, st>>>(ctx->lc, ctx->cc, nc, n, T, Td, v, coef);
+  }
 }
 
 #define IRIS_DISPATCH_N(N_, CALL)                       \
@@ -457,19 +488,66 @@ iris_so_status iris_so_create(const iris_so_config* cfg, iris_so_ctx** out) {
   ctx->Kd.assign(cfg->coll_down_ref, cfg->coll_down_ref + N * N);
   ctx->cfg.energy_K = ctx->energy.data(); ctx->cfg.weight = ctx->weight.data();
   ctx->cfg.einstein_A = ctx->A.data(); ctx->cfg.coll_down_ref = ctx->Kd.data();
+  if (cfg->coll_n_partners > 0) {
+    const int nT = cfg->coll_nT;
+    ctx->Tgrid.assign(cfg->coll_T_grid, cfg->coll_T_grid + nT);
+    ctx->Keff.assign((size_t)nT * N * N, 0.0);
+    for (int p = 0; p < cfg->coll_n_partners; ++p)
+      for (int64_t q = 0; q < (int64_t)nT * N * N; ++q)
+        ctx->Keff[q] += cfg->coll_partner_frac[p] * cfg->coll_table[(int64_t)p * nT * N * N + q];
+    // the copied configuration must not point into the caller's arrays: the folded table takes their place
+    ctx->cfg.coll_T_grid = ctx->Tgrid.data(); ctx->cfg.coll_table = nullptr; ctx->cfg.coll_partner_frac = nullptr;
+    // Kd = the largest rate over the grid: band detection and validation of "a downward rate exists"
+    for (int q = 0; q < N * N; ++q) {
+      double m = 0.0;
+      for (int t = 0; t < nT; ++t) m = std::max(m, ctx->Keff[(size_t)t * N * N + q]);
+      ctx->Kd[q] = m;
+    }
+  }
   ctx->device = dev;
   cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, dev);
   ctx->npix = (int64_t)cfg->nx * cfg->ny;
   ctx->ncell = ctx->npix * cfg->nz;
   ctx->nvox = ctx->npix * cfg->nv;
   fold_constants(ctx);
+  if (!ctx->Keff.empty()) {
+    // device table in the kernels' layout
+    const int nT = cfg->coll_nT;
+    std::vector<float> h((size_t)nT + (size_t)nT * iris::kMaxPairs * 2, 0.0f);
+    for (int t = 0; t < nT; ++t) h[t] = (float)ctx->Tgrid[t];
+    const double rs = ctx->lc.rate_scale;
+    for (int t = 0; t < nT; ++t)
+      for (int u = 1; u < N; ++u)
+        for (int l = 0; l < u; ++l) {
+          const double K = ctx->Keff[(size_t)t * N * N + u * N + l];
+          const size_t o = (size_t)nT + ((size_t)t * iris::kMaxPairs + iris::pair_index(u, l)) * 2;
+          h[o] = (float)(rs * K);
+          h[o + 1] = (float)(rs * K * ctx->weight[u] / ctx->weight[l]);
+        }
+    // the float2 rows must be 8-byte aligned: pad the temperature block to an even count
+    const size_t toff = (size_t)(nT + 1) / 2 * 2;
+    std::vector<float> hd(toff + (size_t)nT * iris::kMaxPairs * 2, 0.0f);
+    std::copy(h.begin(), h.begin() + nT, hd.begin());
+    std::copy(h.begin() + nT, h.end(), hd.begin() + toff);
+    cudaError_t ce = cudaMalloc(reinterpret_cast<void**>(&ctx->d_colltab), hd.size() * sizeof(float));
+    if (ce == cudaSuccess) ce = cudaMemcpy(ctx->d_colltab, hd.data(), hd.size() * sizeof(float), cudaMemcpyHostToDevice);
+    if (ce != cudaSuccess) {
+      cudaGetLastError();
+      iris_so_status st = cuda_fail(nullptr, ce, "upload of the collision table");
+      iris_so_destroy(ctx);
+      return st;
+    }
+    ctx->lc.tb.T = ctx->d_colltab;
+    ctx->lc.tb.K = reinterpret_cast<const float2*>(ctx->d_colltab + toff);
+    ctx->lc.tb.nT = nT;
+  }
   *out = ctx;
   return IRIS_SO_OK;
 }
 
 void iris_so_destroy(iris_so_ctx* ctx) {
   if (!ctx) return;
-  cudaFree(ctx->d_coef); cudaFree(ctx->d_tmp); cudaFree(ctx->d_stage); cudaFree(ctx->d_adj); cudaFree(ctx->d_counter); cudaFree(ctx->d_metrics);
+  cudaFree(ctx->d_coef); cudaFree(ctx->d_tmp); cudaFree(ctx->d_stage); cudaFree(ctx->d_adj); cudaFree(ctx->d_counter); cudaFree(ctx->d_metrics); cudaFree(ctx->d_colltab);
   if (ctx->s_in) cudaStreamDestroy(ctx->s_in);
   if (ctx->s_out) cudaStreamDestroy(ctx->s_out);
   for (auto ev : ctx->slab_events) cudaEventDestroy(ev);

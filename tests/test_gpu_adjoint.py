@@ -155,3 +155,20 @@ def test_abundance_gradient(case):
     worst_fd = excess(g.ravel()[cells], o.grad_fd(f, what, cells, eps=1e-5, wrt="abundance"), scale)
     print("abundance gradient %s: worst vs analytic %.3g, vs finite differences %.3g of tolerance" % (case, worst, worst_fd))
     assert worst <= 1.0 and worst_fd <= 1.0
+
+
+def test_adjoint_with_tabulated_rates():
+    """The density derivative of the level balance with tabulated multi-partner rates (K9 TABLE variant)."""
+    rng = np.random.default_rng(2)
+    cfg, r = make_workload("batch", n=16, nv=64)
+    grid = np.array([10.0, 30.0, 60.0, 100.0, 200.0, 500.0])
+    N = cfg.n_levels
+    tab = np.zeros((2, grid.size, N, N))
+    for p in range(2):
+        for u in range(1, N):
+            for l in range(max(0, u - 2), u):
+                tab[p, :, u, l] = rng.uniform(0.5, 2.0) * 1e-11 * (grid / 100.0) ** rng.uniform(0.0, 0.5) / (u - l)
+    cfg = cfg.with_(coll_T_grid=grid, coll_table=tab, coll_partner_frac=np.array([0.8, 0.2]))
+    f = make_fields(cfg, r)
+    f["vlos"] = (0.2 * f["vlos"]).astype(np.float32)
+    check(cfg, f, weight_cube(cfg), n_fd=32, label="tabulated rates")

@@ -433,3 +433,57 @@ def test_several_lines_share_one_level_solve():
         got = It_shared.cpu().numpy().reshape(-1, cfg.nv).astype(np.float64)
         line = np.abs(rt - rc[:, None]).max(axis=1)
         assert np.all(np.abs(got - rt).max(axis=1) <= 1e-4 * line + 1e-6 / K + 3e-7 * np.abs(rt).max(axis=1)), "J=%d-%d" % (up, up - 1)
+
+
+# ------------------------------------------------------------------------------------------------
+# tabulated collision rates of several partners
+def _with_tables(cfg, max_dj, n_partners=3, seed=9):
+    """Seeded, smooth, non-power-law tables on a LAMDA-like uneven temperature grid for n_partners partners."""
+    rng = np.random.default_rng(seed)
+    N = cfg.n_levels
+    grid = np.array([5.0, 10.0, 20.0, 30.0, 50.0, 70.0, 100.0, 150.0, 200.0, 300.0, 500.0, 1000.0, 2000.0])
+    tab = np.zeros((n_partners, grid.size, N, N))
+    for p in range(n_partners):
+        for u in range(1, N):
+            for l in range(max(0, u - max_dj), u):
+                amp, slope, bump = rng.uniform(0.3, 3.0) * 1e-11, rng.uniform(-0.2, 0.6), rng.uniform(0.0, 0.5)
+                tab[p, :, u, l] = amp * (grid / 100.0) ** slope * (1.0 + bump * np.exp(-((np.log(grid) - 4.0) ** 2))) / (u - l)
+    frac = np.array([0.25, 0.75, 0.2, 0.05][:n_partners])
+    return cfg.with_(coll_T_grid=grid, coll_table=tab, coll_partner_frac=frac)
+
+
+@pytest.mark.parametrize("n_levels,max_dj", [(5, 2), (10, 2), (10, 9), (7, 4), (2, 1)])
+def test_levelpop_with_tabulated_rates(n_levels, max_dj):
+    cfg, r = make_workload("tiny", n=12, n_levels=n_levels)
+    cfg = _with_tables(cfg, min(max_dj, n_levels - 1))
+    n = np.logspace(-1, 8, 41, dtype=np.float32)
+    T = np.geomspace(3.0, 3000.0, 61).astype(np.float32)            # below, inside and above the grid
+    nn, TT = np.meshgrid(n, T, indexing="ij")
+    nn, TT = np.ascontiguousarray(nn.ravel()), np.ascontiguousarray(TT.ravel())
+    cfg1 = cfg.with_(nx=nn.size, ny=1, nz=1)
+    pop = iris(cfg1).levelpop(dev(nn), dev(TT)).cpu().numpy().reshape(n_levels, -1)
+    assert_pops(pop, Oracle(cfg1).levelpop(nn, TT))
+    # temperatures exactly on grid points
+    Tg = np.asarray(cfg.coll_T_grid, dtype=np.float32)
+    cfg2 = cfg.with_(nx=Tg.size, ny=1, nz=1)
+    ng = np.full(Tg.size, 3e3, np.float32)
+    assert_pops(iris(cfg2).levelpop(dev(ng), dev(Tg)).cpu().numpy().reshape(n_levels, -1), Oracle(cfg2).levelpop(ng, Tg))
+    f = make_fields(cfg, r)
+    assert_spectra(iris(cfg).observe(*dev_fields(f)).cpu().numpy(), Oracle(cfg).observe(f), what="cube with tabulated rates")
+
+
+def test_tabulated_rates_single_temperature_and_validation():
+    from paper_2607_01338_b200 import IrisSOError
+    cfg, r = make_workload("tiny", n=8, n_levels=5)
+    one = cfg.with_(coll_T_grid=np.array([100.0]), coll_table=cfg.coll_down_ref[None, None].copy(),
+                    coll_partner_frac=np.array([1.0]))                # one grid point = constant rates = exponent 0
+    f = make_fields(cfg, r)
+    a = iris(one).levelpop(dev(f["nH2"]), dev(f["Tgas"]))
+    b = iris(cfg.with_(coll_T_exp=0.0)).levelpop(dev(f["nH2"]), dev(f["Tgas"]))
+    assert torch.allclose(a, b, rtol=2e-6, atol=0)
+    bad_grid = one.with_(coll_T_grid=np.array([100.0, 50.0]), coll_table=np.repeat(cfg.coll_down_ref[None, None], 2, axis=1))
+    with pytest.raises(IrisSOError):
+        iris(bad_grid)
+    neg = one.with_(coll_table=-cfg.coll_down_ref[None, None])
+    with pytest.raises(IrisSOError):
+        iris(neg)
