@@ -434,6 +434,30 @@ def bench_small_configs(torch, warmup):
                     "what": "64 x (%dx%dx%d cells, %d channels, dust, beam %.3g px, noise %.3g K)"
                             % (cfg.nx, cfg.ny, cfg.nz, cfg.nv, cfg.beam_fwhm_px, cfg.noise_sigma)}
     it.close()
+    # level populations from tabulated rates of three partners on a 13-point temperature grid (medium cube, K1 + K2 only)
+    cfg, recipe = make_workload("medium")
+    grid = np.array([5.0, 10.0, 20.0, 30.0, 50.0, 70.0, 100.0, 150.0, 200.0, 300.0, 500.0, 1000.0, 2000.0])
+    base = cfg.coll_down_ref[None] * (grid[:, None, None] / cfg.coll_T_ref) ** cfg.coll_T_exp
+    frac = np.array([0.25, 0.75, 0.2])
+    cfg_t = cfg.with_(coll_T_grid=grid, coll_table=np.stack([base * 0.3 / frac[0], base * 0.5 / frac[1], base * 0.2 / frac[2]]),
+                      coll_partner_frac=frac)
+    f = make_fields(cfg, recipe)
+    d = [torch.from_numpy(f[k]).to(dev) for k in ("nH2", "Tgas", "Tdust", "vlos")]
+    res = {}
+    for label, c in (("power_law", cfg), ("tabulated_3_partners", cfg_t)):
+        it = IrisSO(c)
+        cube = torch.empty(it.shape_cube, dtype=torch.float32, device=dev)
+        for _ in range(warmup):
+            it.observe(*d, cube=cube)
+        torch.cuda.synchronize()
+        it.profile(True)
+        for _ in range(5):
+            it.observe(*d, cube=cube)
+        prof = it.profile_read()
+        it.profile(False)
+        res[label] = prof["cell"][0] / prof["cell"][1]
+        it.close()
+    out["cell_kernel_ms_medium"] = res
     return out
 
 
