@@ -8,6 +8,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -619,9 +620,11 @@ iris_so_status iris_so_observe_host(iris_so_ctx* ctx, const float* h_nH2, const 
   float* d_cube = ctx->d_stage + 4 * ncell0;
   const float* h[4] = {h_nH2, h_Tgas, h_Tdust, h_vlos};
   cudaError_t e;
-  // slab height: about 48 MB of field data per slab, at least 3 slabs, else one shot
+  // slab height: 128 MB of field data per slab (a sixth of the fields for smaller cubes), at least 3 slabs, else one shot
   const size_t row_bytes = (size_t)cfg0.nz * cfg0.nx * sizeof(float) * 4;
-  int rows = (int)std::max<size_t>(1, (48u << 20) / std::max<size_t>(row_bytes, 1));
+  // (measured on the 512^3 cube, 2.1 GB of fields: 16 MB slabs 49.3 ms, 48 MB 48.5, 128 MB 43.3, 256 MB 44.8, 512 MB 47.4)
+  const size_t slab_bytes = std::min<size_t>((size_t)128 << 20, std::max<size_t>((size_t)16 << 20, 4 * fb / 6));
+  int rows = (int)std::max<size_t>(1, slab_bytes / std::max<size_t>(row_bytes, 1));
   rows = std::min(rows, cfg0.ny);
   const int nslab = (cfg0.ny + rows - 1) / rows;
   if (nslab < 3) {

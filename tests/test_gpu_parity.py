@@ -377,9 +377,9 @@ def test_observe_host_equals_device_path(case):
     if case == "one_shot":
         cfg, r = make_workload("small", n=24, nv=64)
     elif case == "slabs_ragged_pageable":
-        cfg, r = make_workload("small", nx=300, ny=150, nz=160, nv=72)      # 768 KB of fields per row: slabs of 62, 62, 26 rows
+        cfg, r = make_workload("small", nx=300, ny=150, nz=160, nv=72)      # 768 KB of fields per row, 115 MB in all: six ragged slabs of 25 rows
     else:
-        cfg, r = make_workload("small", nx=256, ny=80, nz=512, nv=96)       # 2 MB of fields per row: slabs of 24, 24, 24, 8 rows
+        cfg, r = make_workload("small", nx=256, ny=80, nz=512, nv=96)       # 2 MB of fields per row, 168 MB in all: slabs of 14 rows, the last one ragged
     if case == "slabs_beam_noise":
         cfg = cfg.with_(beam_fwhm_px=3.0, noise_sigma=0.25, seed=11)
     f = make_fields(cfg, r)
