@@ -172,3 +172,43 @@ def test_adjoint_with_tabulated_rates():
     f = make_fields(cfg, r)
     f["vlos"] = (0.2 * f["vlos"]).astype(np.float32)
     check(cfg, f, weight_cube(cfg), n_fd=32, label="tabulated rates")
+
+
+def test_batch_workload_full_size_sampled():
+    """BASELINE config 5 at full size (one of the 64 cubes: 128^3 cells, 256 channels, dust, beam 3 px, noise 0.25 K), in
+    the launch configuration bench.py times: seeded pixel columns of the raw cube against the oracle, the beam on a patch,
+    and the reverse-scan gradient against the oracle's finite differences on sampled cells (relative error <= 1e-3)."""
+    from paper_2607_01338_b200 import IrisSO
+    from parity import assert_spectra
+    cfg, r = make_workload("batch", seed=1003)
+    f = make_fields(cfg, r)
+    d = [dev(f[k]) for k in ("nH2", "Tgas", "Tdust", "vlos")]
+    it = IrisSO(cfg)
+    raw = it.observe(*d, beam=False, noise=False)
+    plane, n_cols = cfg.nx * cfg.ny, 32
+    rng = np.random.default_rng(77)
+    pix = np.sort(rng.choice(plane, size=n_cols, replace=False))
+    got = raw.reshape(plane, cfg.nv)[torch.from_numpy(pix).cuda()].cpu().numpy()
+    sub = {k: np.ascontiguousarray(f[k].reshape(cfg.nz, plane)[:, pix]).reshape(cfg.nz, 1, n_cols)
+           for k in ("nH2", "Tgas", "Tdust", "vlos")}
+    cfg_s = cfg.with_(nx=n_cols, ny=1, beam_fwhm_px=0.0, noise_sigma=0.0)
+    ref = Oracle(cfg_s).observe(sub, beam=False, noise=False).reshape(n_cols, cfg.nv)
+    assert_spectra(got, ref, what="batch cube, sampled columns")
+    o = Oracle(cfg)
+    smooth = it.observe(*d, beam=True, noise=False)
+    y0, x0, wd = 60, 21, 16
+    patch = raw[y0 - 6:y0 + wd + 6, x0 - 6:x0 + wd + 6].cpu().numpy()
+    assert np.abs(smooth[y0:y0 + wd, x0:x0 + wd].cpu().numpy() - o.beam(patch)[6:-6, 6:-6]).max() <= 1e-5 * np.abs(patch).max() + 1e-6
+    full = it.observe(*d)
+    dz = (full - smooth).flatten()[::53].cpu().numpy()
+    assert abs(dz.std() - cfg.noise_sigma) < 2e-3 and abs(dz.mean()) < 2e-3
+    # gradient of L = sum(w * cube): finite differences of the oracle on sampled cells (biased to the cells that matter)
+    w = weight_cube(cfg)
+    g = it.observe_adjoint(*d, dev(w)).cpu().numpy().astype(np.float64).ravel()
+    what = o.beam(w.astype(np.float64))
+    order = np.argsort(-np.abs(g))
+    cells = np.unique(np.concatenate([order[:16], rng.choice(cfg.n_cells, size=16, replace=False)]))
+    gfd = o.grad_fd(f, what, cells, eps=1e-5)
+    worst = excess(g[cells], gfd, np.abs(g).max())
+    print("batch cube at full size: gradient vs finite differences at %.3g of tolerance (max|g| %.3g)" % (worst, np.abs(g).max()))
+    assert np.all(np.isfinite(g)) and worst <= 1.0
