@@ -487,3 +487,8 @@ def test_tabulated_rates_single_temperature_and_validation():
     neg = one.with_(coll_table=-cfg.coll_down_ref[None, None])
     with pytest.raises(IrisSOError):
         iris(neg)
+
+
+def test_full_size_small_sampled():
+    """BASELINE config "small" at full size (128^3 cells, 256 channels, dust, tau_peak up to ~20)."""
+    _sampled_check("small", 64, 13)
