@@ -367,9 +367,10 @@ adjoint_march_kernel(MarchConsts mc, AdjointConsts ac, const float* __restrict__
     const int W = line_window(e_c, a_c, c_los, s, nv, klo, khi);
     float E_d = 1.0f, m_d = 0.0f, Gn = 1.0f, Lam = 1.0f;
     if (DUST) {
-      E_d = exp_neg(tau_d);
-      m_d = one_minus_exp_neg(tau_d);
-      Gn = G * ex2_approx(tau_d * 1.4426950408889634f);
+      const float td_e = fminf(tau_d, kMaxTauDCell);
+      E_d = exp_neg(td_e);
+      m_d = one_minus_exp_neg(td_e);
+      Gn = G * ex2_approx(td_e * 1.4426950408889634f);
       cumD += tau_d;
       Lam = exp_neg(totD - cumD);                            // dust attenuation between this cell and the observer
     }
@@ -453,7 +454,7 @@ adjoint_march_kernel(MarchConsts mc, AdjointConsts ac, const float* __restrict__
     if (DUST) {
       C = fmaf(C, E_d, S_d * m_d);
       G = Gn;
-      if (G > 1.0e18f) {                                     // the same for the LPP lanes of the pixel
+      if (G > kFoldG) {                                     // the same for the LPP lanes of the pixel
         const float inv = 1.0f / G;
         __syncwarp(gmask);
         for (int c = i; c < nv; c += LPP) Dt[IDX(c)] *= inv;

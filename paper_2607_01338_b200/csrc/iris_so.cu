@@ -367,12 +367,33 @@ int resolved_algo(const iris_so_config& c) {
 
 bool hot_path_mode(const iris_so_config& c) { return c.transfer_mode == 0 && c.integration == 0 && c.subsample == 0; }
 
+bool spectra_fit_shared(const iris_so_config& c) {
+  return (size_t)(32 / 8) * ((size_t)c.nv + 32) * sizeof(float) + 2048 <= 227u * 1024u;
+}
+
+// Selectively thin and optically thin transfer with formal integration and the channel-integrated profile are identities
+// outside a cell's line window too (in the dust-scaled spectrum), so they run through the line-window series kernel
+// (template MODE 1 / 2) whenever it applies; transfer_algo = IRIS_SO_ALGO_DENSE keeps them on transfer_modes_kernel.
+bool windowed_thin_mode(const iris_so_config& c) {
+  return (c.transfer_mode == 1 || c.transfer_mode == 2) && c.integration == 0 && c.subsample == 0 &&
+         c.transfer_algo != IRIS_SO_ALGO_DENSE && c.microturb_cms > 0.0 &&
+         c.dv_cms <= (double)iris::kSeriesMaxS * c.microturb_cms && spectra_fit_shared(c);
+}
+
 // K3 (+K4, K5) from ctx->d_coef
 iris_so_status run_transfer(iris_so_ctx* ctx, const iris::MarchConsts& mc, float* out, float* out_cont, cudaStream_t st) {
   const bool dust = ctx->cfg.dust_on != 0;
   const int npix = (int)ctx->npix, nz = ctx->cfg.nz, nv = ctx->cfg.nv;
   const int algo = resolved_algo(ctx->cfg);
   ProfScope prof(ctx, IRIS_SO_STAGE_TRANSFER, st);
+  if (windowed_thin_mode(ctx->cfg)) {
+    cudaError_t e = iris::launch_transfer_series(mc, ctx->d_coef, ctx->ncell, npix, nz, nv, dust,
+                                                 (float)(ctx->cfg.dv_cms / ctx->cfg.microturb_cms), out, out_cont, st,
+                                                 ctx->cfg.transfer_mode);
+    ctx->launches++;
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "launch of the line-window transfer kernel");
+    return IRIS_SO_OK;
+  }
   if (!hot_path_mode(ctx->cfg)) {
     iris::ModeConsts md;
     md.mode = ctx->cfg.transfer_mode; md.smooth = ctx->cfg.integration;
@@ -449,6 +470,7 @@ const char* iris_so_last_error(const iris_so_ctx* ctx) { return ctx ? ctx->err.c
 
 const char* iris_so_transfer_kernel(const iris_so_ctx* ctx) {
   if (!ctx) return "";
+  if (windowed_thin_mode(ctx->cfg)) return "transfer_series_kernel";
   if (!hot_path_mode(ctx->cfg)) return "transfer_modes_kernel";
   if ((size_t)(32 / 8) * ((size_t)ctx->cfg.nv + 32) * sizeof(float) + 2048 > 227u * 1024u) return "transfer_dense_kernel";
   switch (resolved_algo(ctx->cfg)) {

@@ -16,6 +16,12 @@
 
 namespace iris {
 
+// The windowed kernels store the spectrum multiplied by G = exp(dust optical depth so far) and fold G back into it when
+// it passes kFoldG.  A single cell's exp(+-tau_d) is taken at min(tau_d, kMaxTauDCell): exp(-50) = 2e-22 is nothing in
+// fp32, and kFoldG exp(50) times any intensity in K stays inside the fp32 range (a cell with tau_d ~ 100 would overflow).
+constexpr float kMaxTauDCell = 50.0f;
+constexpr float kFoldG = 1.0e10f;
+
 // coefficient plane order written by K2
 enum { Q_E = 0, Q_A = 1, Q_CLOS = 2, Q_S = 3, Q_TAUD = 4, Q_SD = 5 };
 

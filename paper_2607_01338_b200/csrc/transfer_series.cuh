@@ -56,7 +56,10 @@ struct SeriesLayout {
 struct SeriesRecord { float4 q0, q1, q2, q3; };
 
 // Phase A: coefficients of one cell -> march record.
-template <bool DUST, int DEG>
+// MODE 0: optically thick formal step (the hot path).  MODE 1: selectively thin, formal (Eq. 4.8.13 - 4.8.15): the
+// polynomial gives the erf difference itself, q2 = { e_c w(tau_d), a_c w(tau_d), -, E_d }.  MODE 2: optically thin, formal
+// (Eq. 4.7.3 - 4.7.6): the polynomial gives E = e_c dErf, no attenuation (E_d = exp(tau_d) = 1), continuum adds tau_d S_d.
+template <bool DUST, int DEG, int MODE = 0>
 __device__ __forceinline__ SeriesRecord make_series_record(float e_c, float a_c, float c_los, float s, float tau_d,
                                                            float S_d, float T_bg, int nv) {
   constexpr float LOG2E = 1.4426950408889634f;
@@ -71,7 +74,7 @@ __device__ __forceinline__ SeriesRecord make_series_record(float e_c, float a_c,
   const float a_safe = fabsf(a_c) < a_min ? a_min : a_c;
   const float sp = 1.1283791670955126f * s;                 // 2 s / sqrt(pi)
   const float As = a_safe * sp, Es = e_c * sp;
-  const float Asp = As * LOG2E;
+  const float Asp = MODE == 0 ? As * LOG2E : (MODE == 1 ? sp : Es);   // what the polynomial is scaled by
   const float xs = 1.2011224087864498f * s;                 // s sqrt(log2 e)
   r.q0.x = ((float)(2 * qlo) + 0.5f - c_los) * xs;
   r.q0.y = xs;
@@ -87,9 +90,24 @@ __device__ __forceinline__ SeriesRecord make_series_record(float e_c, float a_c,
   r.q1 = make_float4(Asp * p0, Asp * (p1 * L1), Asp * (p2 * L2), Asp * (p3 * L3));
   r.q3.z = DEG > 3 ? Asp * (p4 * L4) : 0.0f;
   r.q3.w = 0.0f;
-  if (DUST) {
-    const float E_d = exp_neg(tau_d);
-    const float m_d = one_minus_exp_neg(tau_d);
+  if (MODE == 2) {
+    r.q0.z = 0.0f;
+    r.q2 = make_float4(0.0f, 0.0f, 0.0f, 1.0f);
+    r.q3.x = tau_d * S_d;
+    r.q3.y = 1.0f;
+  } else if (MODE == 1) {
+    const float td_e = fminf(tau_d, kMaxTauDCell);
+    const float E_d = exp_neg(td_e);
+    const float m_d = one_minus_exp_neg(td_e);
+    const float w_d = fabsf(tau_d) < 1.0e-3f ? fmaf(tau_d, fmaf(tau_d, 1.0f / 6.0f, -0.5f), 1.0f) : m_d * rcp_approx(tau_d);
+    r.q0.z = 0.0f;
+    r.q2 = make_float4(e_c * w_d, a_c * w_d, 0.0f, E_d);
+    r.q3.x = S_d * m_d;
+    r.q3.y = ex2_approx(td_e * LOG2E);
+  } else if (DUST) {
+    const float td_e = fminf(tau_d, kMaxTauDCell);
+    const float E_d = exp_neg(td_e);
+    const float m_d = one_minus_exp_neg(td_e);
     const float iA = LOG2E * rcp_approx(Asp);
     r.q0.z = fmaf(tau_d, LOG2E, 1.0e-30f);
     r.q2.x = m_d * fmaf(-S_d, As, Es) * iA;
@@ -97,7 +115,7 @@ __device__ __forceinline__ SeriesRecord make_series_record(float e_c, float a_c,
     r.q2.z = -E_d * S_d * tau_d * LOG2E;
     r.q2.w = E_d;
     r.q3.x = S_d * m_d;
-    r.q3.y = ex2_approx(tau_d * LOG2E);
+    r.q3.y = ex2_approx(td_e * LOG2E);
   } else {
     r.q0.z = T_bg - Es * rcp_approx(As);      // -sc = C - S_L, C = T_bg throughout
     r.q2 = make_float4(r.q3.z, 0.0f, 0.0f, 1.0f);   // pA4 travels in q2.x when there is no dust (NQ = 3)
@@ -145,7 +163,7 @@ struct SeriesCellOps {
 // that 2 P independent dependency chains are in flight (the SM issues in order: a lane-serial update would leave
 // the issue slot idle for the latency of every MUFU / FMA of the chain).  d: the lane's words of pair q; pairs at
 // or beyond qend are computed but neither loaded nor stored.  xx: scaled centres of the two channels of pair q.
-template <bool DUST, int DEG, int LPP, int P>
+template <bool DUST, int DEG, int LPP, int P, int MODE = 0>
 __device__ __forceinline__ void series_passes(float* d, int q, int qend, f32x2 xx, f32x2 step2, const SeriesCellOps& o) {
   constexpr float L1 = 0.6931471805599453f, L2 = L1 * L1, L3 = L2 * L1, L4 = L2 * L2;
   const f32x2 ONE = pk1(1.0f), NEG1 = pk1(-1.0f);
@@ -168,8 +186,25 @@ __device__ __forceinline__ void series_passes(float* d, int q, int qend, f32x2 x
   for (int k = 0; k < P; ++k) {
     float u0, u1;
     upk(u[k], u0, u1);
-    t[k] = mul2(pk(ex2_approx(-u0), ex2_approx(-u1)), pol[k]);      // tau_L log2(e)
+    t[k] = mul2(pk(ex2_approx(-u0), ex2_approx(-u1)), pol[k]);      // tau_L log2(e)  (MODE 1: dErf, MODE 2: e_c dErf)
   }
+  if constexpr (MODE != 0) {
+    // thin: Dt += E.  selectively thin: Dt' = max(Dt + K dErf, -C' G'),  K = G' w(tau_d) (e_c - a_c C') in o.Pn, the clamp in o.CG
+#pragma unroll
+    for (int k = 0; k < P; ++k) {
+      if (MODE == 2) Dt[k] = add2(Dt[k], t[k]);
+      else {
+        const f32x2 v = fma2(o.Pn, t[k], Dt[k]);
+        float v0, v1, c0, c1;
+        upk(v, v0, v1);
+        upk(o.CG, c0, c1);
+        Dt[k] = pk(fmaxf(v0, c0), fmaxf(v1, c1));
+      }
+      float2 w;
+      upk(Dt[k], w.x, w.y);
+      *reinterpret_cast<float2*>(d + 64 * k) = w;
+    }
+  } else {
   float t0[P], t1[P], f0[P], f1[P];
 #pragma unroll
   for (int k = 0; k < P; ++k) {
@@ -220,13 +255,14 @@ __device__ __forceinline__ void series_passes(float* d, int q, int qend, f32x2 x
     upk(Dt[k], v.x, v.y);
     *reinterpret_cast<float2*>(d + 64 * k) = v;
   }
+  }
   (void)q; (void)qend;
 }
 
 // __launch_bounds__ names a minimum of 3 CTAs per SM (what the 1024-channel spectra allow): without it ptxas holds the
 // kernel to 68 registers and schedules the two pair-passes of the loop back to back; with it it takes 86 registers and
 // overlaps them (large: 6.61 -> 6.27 ms).
-template <int LPP, bool DUST, int DEG>
+template <int LPP, bool DUST, int DEG, int MODE>
 __global__ void __launch_bounds__(128, 3)
 transfer_series_kernel(MarchConsts mc, const float* __restrict__ coef, int64_t ncell, int npix, int nz, int nv,
                        int nvp, float* __restrict__ out, float* __restrict__ out_cont) {
@@ -281,7 +317,12 @@ transfer_series_kernel(MarchConsts mc, const float* __restrict__ coef, int64_t n
       const float Gn = G * q3.y;
       CG = C * G;
       C = fmaf(C, q2.w, q3.x);
-      Pn = q2.x * Gn; Qn = q2.y * Gn; Rn = q2.z * Gn;
+      if (MODE == 1) {                       // selectively thin: K = G' w_d (e_c - a_c C'), clamp at I_T = 0: D >= -C'
+        Pn = Gn * fmaf(-q2.y, C, q2.x);
+        CG = -C * Gn;
+      } else {
+        Pn = q2.x * Gn; Qn = q2.y * Gn; Rn = q2.z * Gn;
+      }
       G = Gn;
     }
     if (npass > 0) {
@@ -298,19 +339,19 @@ transfer_series_kernel(MarchConsts mc, const float* __restrict__ coef, int64_t n
       float* d = sp + (q / LPP) * ROW + (q % LPP) * 2;
       int rem = npass;
       while (rem >= 2) {
-        series_passes<DUST, DEG, LPP, 2>(d, q, qend, xx, step2, o);
+        series_passes<DUST, DEG, LPP, 2, MODE>(d, q, qend, xx, step2, o);
         xx = add2(xx, add2(step2, step2)); q += 2 * LPP; d += 2 * ROW; rem -= 2;
       }
-      if (rem == 1) series_passes<DUST, DEG, LPP, 1>(d, q, qend, xx, step2, o);
+      if (rem == 1) series_passes<DUST, DEG, LPP, 1, MODE>(d, q, qend, xx, step2, o);
     }
-    if (DUST && G > 1.0e18f) rescale_spectrum();
+    if (DUST && G > kFoldG) rescale_spectrum();
   };
 
   bool chunk_busy = true;
   for (int z0 = 0; z0 < nz; z0 += LPP) {
     // ---- phase A: one record per lane
     {
-      const SeriesRecord r = make_series_record<DUST, DEG>(l_e, l_a, l_c, l_s, l_td, l_sd, mc.T_bg, nv);
+      const SeriesRecord r = make_series_record<DUST, DEG, MODE>(l_e, l_a, l_c, l_s, l_td, l_sd, mc.T_bg, nv);
       chunk_busy = __any_sync(0xffffffffu, ((unsigned)__float_as_int(r.q0.w) >> 16) != 0u);   // also: phase B is done
       rec[lane] = r.q0;
       rec[32 + lane] = r.q1;
@@ -338,7 +379,7 @@ transfer_series_kernel(MarchConsts mc, const float* __restrict__ coef, int64_t n
           const float4 c3 = rq[96 + j * PPW];
           C = fmaf(C, E_d, c3.x);
           G *= c3.y;
-          if (G > 1.0e18f) rescale_spectrum();
+          if (G > kFoldG) rescale_spectrum();
         }
       }
       continue;
@@ -378,7 +419,7 @@ transfer_series_kernel(MarchConsts mc, const float* __restrict__ coef, int64_t n
   }
 }
 
-template <int LPP, bool DUST, int DEG>
+template <int LPP, bool DUST, int DEG, int MODE = 0>
 inline cudaError_t launch_transfer_series_t(const MarchConsts& mc, const float* coef, int64_t ncell, int npix, int nz,
                                             int nv, float* out, float* out_cont, cudaStream_t st) {
   constexpr int PPW = 32 / LPP;
@@ -394,17 +435,23 @@ inline cudaError_t launch_transfer_series_t(const MarchConsts& mc, const float* 
   if (smem > 227 * 1024) return cudaErrorInvalidConfiguration;
   const int ppc = wpc * PPW;
   const unsigned grid = (unsigned)((npix + ppc - 1) / ppc);
-  cudaError_t e = cudaFuncSetAttribute(transfer_series_kernel<LPP, DUST, DEG>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+  cudaError_t e = cudaFuncSetAttribute(transfer_series_kernel<LPP, DUST, DEG, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                        (int)smem);
   if (e != cudaSuccess) return e;
-  transfer_series_kernel<LPP, DUST, DEG><<<grid, wpc * 32, smem, st>>>(mc, coef, ncell, npix, nz, nv, nvp, out, out_cont);
+  transfer_series_kernel<LPP, DUST, DEG, MODE><<<grid, wpc * 32, smem, st>>>(mc, coef, ncell, npix, nz, nv, nvp, out, out_cont);
   return cudaGetLastError();
 }
 
 // s_max: upper bound of dv / b over all cells (dv / microturbulence); selects the polynomial degree.
+// mode: 0 optically thick, 1 selectively thin, 2 optically thin (formal integration, channel-integrated profile); modes 1
+// and 2 always run the dust instantiation (tau_d = S_d = 0 planes when the dust is off).
 inline cudaError_t launch_transfer_series(const MarchConsts& mc, const float* coef, int64_t ncell, int npix, int nz, int nv,
-                                          bool dust, float s_max, float* out, float* out_cont, cudaStream_t st) {
+                                          bool dust, float s_max, float* out, float* out_cont, cudaStream_t st, int mode = 0) {
   const bool deg3 = s_max <= kSeriesDeg3MaxS;
+  if (mode == 1) return deg3 ? launch_transfer_series_t<8, true, 3, 1>(mc, coef, ncell, npix, nz, nv, out, out_cont, st)
+                             : launch_transfer_series_t<8, true, 4, 1>(mc, coef, ncell, npix, nz, nv, out, out_cont, st);
+  if (mode == 2) return deg3 ? launch_transfer_series_t<8, true, 3, 2>(mc, coef, ncell, npix, nz, nv, out, out_cont, st)
+                             : launch_transfer_series_t<8, true, 4, 2>(mc, coef, ncell, npix, nz, nv, out, out_cont, st);
   if (dust) return deg3 ? launch_transfer_series_t<8, true, 3>(mc, coef, ncell, npix, nz, nv, out, out_cont, st)
                         : launch_transfer_series_t<8, true, 4>(mc, coef, ncell, npix, nz, nv, out, out_cont, st);
   return deg3 ? launch_transfer_series_t<8, false, 3>(mc, coef, ncell, npix, nz, nv, out, out_cont, st)

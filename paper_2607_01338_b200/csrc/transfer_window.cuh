@@ -86,10 +86,11 @@ transfer_window_kernel(MarchConsts mc, const float* __restrict__ coef, int64_t n
     float CG = 0.0f, Gn = 1.0f, sc = 0.0f;
     if (DUST) {
       d.tau_d = tau_d; d.S_d = S_d; d.C = C;
-      d.E_d = exp_neg(tau_d);
-      d.m_d = one_minus_exp_neg(tau_d);
+      const float td_e = fminf(tau_d, kMaxTauDCell);
+      d.E_d = exp_neg(td_e);
+      d.m_d = one_minus_exp_neg(td_e);
       CG = C * G;
-      Gn = G * ex2_approx(tau_d * 1.4426950408889634f);          // G after this cell
+      Gn = G * ex2_approx(td_e * 1.4426950408889634f);           // G after this cell
       C = fmaf(C, d.E_d, S_d * d.m_d);
     } else {
       sc = (a_c != 0.0f ? e_c / a_c : 0.0f) - C;
@@ -132,7 +133,7 @@ transfer_window_kernel(MarchConsts mc, const float* __restrict__ coef, int64_t n
     }
     if (DUST) {
       G = Gn;
-      if (G > 1.0e18f) {   // rare: fold the accumulated dust attenuation into the stored spectrum
+      if (G > kFoldG) {   // rare: fold the accumulated dust attenuation into the stored spectrum
         const float inv = 1.0f / G;
         __syncwarp(__activemask());
         for (int cc = i; cc < nvp; cc += LPP) sp[(cc / LPP) * 32 + i] *= inv;

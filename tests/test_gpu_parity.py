@@ -160,7 +160,7 @@ def test_observe_degenerate_shapes(algo, shape):
 
 
 @pytest.mark.parametrize("algo", ALGOS)
-@pytest.mark.parametrize("case", ["thick", "very_thin", "narrow_line", "cold_dust_absorption", "heavy_dust"])
+@pytest.mark.parametrize("case", ["thick", "very_thin", "narrow_line", "cold_dust_absorption", "heavy_dust", "opaque_cells"])
 def test_observe_regimes(algo, case):
     cfg, r = make_workload("small", n=24, nv=128)
     f = make_fields(cfg, r)
@@ -176,6 +176,11 @@ def test_observe_regimes(algo, case):
         f["Tdust"] = np.full_like(f["Tdust"], 150.0)
     elif case == "heavy_dust":
         cfg = cfg.with_(kappa_gas_cm2_g=60.0)              # total dust optical depth >> 40: exercises the G rescale
+    elif case == "opaque_cells":
+        # dust optical depths of ~100 in single cells of the near half (exp(tau_d) alone leaves the fp32 range)
+        cfg = cfg.with_(kappa_gas_cm2_g=3.0)
+        f["nH2"][: cfg.nz // 2] *= 1e-3
+        f["nH2"][cfg.nz // 2:] *= 30.0
     cube = run_observe(cfg, f, ALGOS[algo])
     ref = Oracle(cfg).observe(f)
     worst = assert_spectra(cube, ref)
