@@ -74,9 +74,14 @@ transfer_modes_kernel(MarchConsts mc, ModeConsts md, const float* __restrict__ c
     const float pos0 = PROF == 2 ? (float)v0 + (float)(2 * panel) * inv_m : (float)v0;
     const float dpos = PROF == 0 ? 1.0f : inv_m;
     const float* p = coef + pix;
-    for (int n = 0; n < nz; ++n, p += npix) {
-      const float e_c = p[0], a_c = p[ncell], c_los = p[2 * ncell], s = p[3 * ncell];
-      const float td = p[4 * ncell], Sd = p[5 * ncell];
+    // the coefficients of the next cell are loaded one cell ahead (the march of a point is a dependent chain)
+    float n_e = p[0], n_a = p[ncell], n_c = p[2 * ncell], n_s = p[3 * ncell], n_td = p[4 * ncell], n_sd = p[5 * ncell];
+    for (int n = 0; n < nz; ++n) {
+      const float e_c = n_e, a_c = n_a, c_los = n_c, s = n_s, td = n_td, Sd = n_sd;
+      if (n + 1 < nz) {
+        p += npix;
+        n_e = p[0]; n_a = p[ncell]; n_c = p[2 * ncell]; n_s = p[3 * ncell]; n_td = p[4 * ncell]; n_sd = p[5 * ncell];
+      }
       const float Jd = td * Sd;
       float wn = 0.0f;
       if (MODE == 2 && SMOOTH) {
@@ -91,6 +96,9 @@ transfer_modes_kernel(MarchConsts mc, ModeConsts md, const float* __restrict__ c
       else if (n == 1) C_unc = (Jd_p + Jd + (2.0f - td_p) * C) * rcp_approx(2.0f + td);
       else C_unc = (2.0f * Jd + 4.0f * C - Cm) * rcp_approx(fmaf(2.0f, td, 3.0f));
       const float Cn = (MODE != 2 && (SMOOTH || MODE == 1)) ? fmaxf(C_unc, 0.0f) : C_unc;
+      // ReLU of the smooth integrator on D: D' = relu(Du + C_unc) - relu(C_unc) = max(Du + relu_add, relu_min) with
+      // (0, -C_unc) where the continuum is not clamped and (C_unc, 0) where it is
+      const float relu_add = C_unc >= 0.0f ? 0.0f : C_unc, relu_min = C_unc >= 0.0f ? -C_unc : 0.0f;
       float Ed = 1.0f, wd = 1.0f;
       DustStep ds;
       if (MODE == 1 && !SMOOTH) { Ed = exp_neg(td); wd = w_of(td); }
@@ -158,9 +166,9 @@ transfer_modes_kernel(MarchConsts mc, ModeConsts md, const float* __restrict__ c
           const float r = rcp_approx(fmaf(2.0f, td, 3.0f));
 #pragma unroll
           for (int k = 0; k < NPT; ++k) {
-            const float Du = fmaf(4.0f, D[k], -Dm[k]) * r;
+            const float Du = fmaf(fmaf(4.0f, D[k], -Dm[k]), r, relu_add);
             Dm[k] = D[k];
-            D[k] = (C_unc >= 0.0f) ? fmaxf(Du, -C_unc) : fmaxf(Du + C_unc, 0.0f);
+            D[k] = fmaxf(Du, relu_min);
           }
         }
         Cm = C; C = Cn;
@@ -191,7 +199,7 @@ transfer_modes_kernel(MarchConsts mc, ModeConsts md, const float* __restrict__ c
             Du = (2.0f * (E - A * Ccoef) + 4.0f * Dk - Dm[k]) * rcp_approx(fmaf(2.0f, an, 3.0f));
           }
           // ReLU on the true intensities: I_T = relu(Du + C_unc), C = relu(C_unc)
-          Dn = (C_unc >= 0.0f) ? fmaxf(Du, -C_unc) : fmaxf(Du + C_unc, 0.0f);
+          Dn = fmaxf(Du + relu_add, relu_min);
         }
         Dm[k] = Dk;
         D[k] = Dn;
