@@ -69,18 +69,27 @@ transfer_modes_kernel(MarchConsts mc, ModeConsts md, const float* __restrict__ c
 #pragma unroll
     for (int k = 0; k < NPT; ++k) D[k] = Dm[k] = 0.0f;
     float C = mc.T_bg, Cm = mc.T_bg;
-    float e_p = 0.0f, a_p = 0.0f, c_p = 0.0f, s_p = 1.0f, td_p = 0.0f, Jd_p = 0.0f;   // coefficients of grid index n - 1
     // position (channel-edge index units) of point 0 and spacing of the points
     const float pos0 = PROF == 2 ? (float)v0 + (float)(2 * panel) * inv_m : (float)v0;
     const float dpos = PROF == 0 ? 1.0f : inv_m;
     const float* p = coef + pix;
     // the coefficients of the next cell are loaded one cell ahead (the march of a point is a dependent chain)
     float n_e = p[0], n_a = p[ncell], n_c = p[2 * ncell], n_s = p[3 * ncell], n_td = p[4 * ncell], n_sd = p[5 * ncell];
-    for (int n = 0; n < nz; ++n) {
+    // One cell.  Dc holds the points at grid index n - 1 and Dp those at n - 2; the new values are written over Dp, so
+    // the caller alternates the two arrays instead of moving 2 NPT registers per cell (modes without a second-order
+    // history pass the same array twice).
+    auto step = [&](const int n, float (&Dc)[NPT], float (&Dp)[NPT]) {
       const float e_c = n_e, a_c = n_a, c_los = n_c, s = n_s, td = n_td, Sd = n_sd;
       if (n + 1 < nz) {
         p += npix;
         n_e = p[0]; n_a = p[ncell]; n_c = p[2 * ncell]; n_s = p[3 * ncell]; n_td = p[4 * ncell]; n_sd = p[5 * ncell];
+      }
+      // the trapezoidal first step also needs the coefficients of grid index 0
+      float e_p = 0.0f, a_p = 0.0f, c_p = 0.0f, s_p = 1.0f, td_p = 0.0f, Jd_p = 0.0f;
+      if (SMOOTH && MODE != 2 && n == 1) {
+        const float* q = coef + pix;
+        e_p = q[0]; a_p = q[ncell]; c_p = q[2 * ncell]; s_p = q[3 * ncell]; td_p = q[4 * ncell];
+        Jd_p = td_p * q[5 * ncell];
       }
       const float Jd = td * Sd;
       float wn = 0.0f;
@@ -159,27 +168,25 @@ transfer_modes_kernel(MarchConsts mc, ModeConsts md, const float* __restrict__ c
           const float att = MODE == 1 ? Ed : ds.E_d;
 #pragma unroll
           for (int k = 0; k < NPT; ++k) {
-            const float Dn = D[k] * att;
-            D[k] = MODE == 1 ? fmaxf(Dn, -Cn) : Dn;
+            const float Dn = Dc[k] * att;
+            Dp[k] = MODE == 1 ? fmaxf(Dn, -Cn) : Dn;
           }
         } else if (n >= 2) {
           const float r = rcp_approx(fmaf(2.0f, td, 3.0f));
 #pragma unroll
-          for (int k = 0; k < NPT; ++k) {
-            const float Du = fmaf(fmaf(4.0f, D[k], -Dm[k]), r, relu_add);
-            Dm[k] = D[k];
-            D[k] = fmaxf(Du, relu_min);
-          }
+          for (int k = 0; k < NPT; ++k) Dp[k] = fmaxf(fmaf(fmaf(4.0f, Dc[k], -Dp[k]), r, relu_add), relu_min);
+        } else {
+#pragma unroll
+          for (int k = 0; k < NPT; ++k) Dp[k] = Dc[k];      // n = 0 of the smooth march: nothing happens yet
         }
         Cm = C; C = Cn;
-        e_p = e_c; a_p = a_c; c_p = c_los; s_p = s; td_p = td; Jd_p = Jd;
-        continue;
+        return;
       }
       // ---- the step of every point
 #pragma unroll
       for (int k = 0; k < NPT; ++k) {
         const float E = e_c * pw[k], A = a_c * pw[k];
-        const float Dk = D[k];
+        const float Dk = Dc[k];
         float Dn;
         if (MODE == 2) {
           Dn = SMOOTH ? fmaf(wn, E, Dk) : Dk + E;
@@ -196,16 +203,26 @@ transfer_modes_kernel(MarchConsts mc, ModeConsts md, const float* __restrict__ c
             Du = ((Ep - Ap * C) + (E - A * Ccoef) + (2.0f - a0) * Dk) * rcp_approx(2.0f + a1);
           } else {
             const float an = (MODE == 0 ? A : 0.0f) + td;
-            Du = (2.0f * (E - A * Ccoef) + 4.0f * Dk - Dm[k]) * rcp_approx(fmaf(2.0f, an, 3.0f));
+            Du = (2.0f * (E - A * Ccoef) + 4.0f * Dk - Dp[k]) * rcp_approx(fmaf(2.0f, an, 3.0f));
           }
           // ReLU on the true intensities: I_T = relu(Du + C_unc), C = relu(C_unc)
           Dn = fmaxf(Du + relu_add, relu_min);
         }
-        Dm[k] = Dk;
-        D[k] = Dn;
+        Dp[k] = Dn;
       }
       Cm = C; C = Cn;
-      e_p = e_c; a_p = a_c; c_p = c_los; s_p = s; td_p = td; Jd_p = Jd;
+    };
+    bool in_Dm = false;                 // which array holds the final points
+    if (SMOOTH && MODE != 2) {
+      int n = 0;
+      for (; n + 1 < nz; n += 2) { step(n, D, Dm); step(n + 1, Dm, D); }
+      if (n < nz) { step(n, D, Dm); in_Dm = true; }
+    } else {
+      for (int n = 0; n < nz; ++n) step(n, D, D);
+    }
+    if (in_Dm) {
+#pragma unroll
+      for (int k = 0; k < NPT; ++k) D[k] = Dm[k];
     }
     Cfin = C;
     if (PROF == 2) Dacc += (D[0] + 4.0f * D[1] + D[2]) * (inv_m * (1.0f / 3.0f));
