@@ -42,9 +42,10 @@ __device__ __forceinline__ float w_of(float t) {
   return fabsf(t) < 1.0e-3f ? fmaf(t, fmaf(t, 1.0f / 6.0f, -0.5f), 1.0f) : one_minus_exp_neg(t) / t;
 }
 
+constexpr int kModesCh0 = 16;         // channels per thread with the channel-integrated profile (PROF 0)
 constexpr float kModesXmax = 5.5f;     // profile weights beyond this many Doppler widths are dropped (< 1e-13 of the peak)
 
-// PROF 0: channel-integrated profile, 8 channels per thread (NPT = 8 weights from 9 edges)
+// PROF 0: channel-integrated profile, kModesCh0 channels per thread (NPT weights from NPT + 1 edges)
 // PROF 1: fine grid with m = 4 or 8 intervals per channel: 9 points = 8 / m channels per thread
 // PROF 3: fine grid with m = 2 (the paper's production mode, f = 1): 17 points = 8 channels per thread
 // PROF 2: fine grid, any even m: one channel per thread, one Simpson panel (3 points) per march
@@ -52,11 +53,11 @@ template <int MODE, bool SMOOTH, int PROF>
 __global__ void __launch_bounds__(128)
 transfer_modes_kernel(MarchConsts mc, ModeConsts md, const float* __restrict__ coef, int64_t ncell, int npix, int nz,
                       int nv, float* __restrict__ out, float* __restrict__ out_cont) {
-  constexpr int NPT = PROF == 0 ? 8 : (PROF == 1 ? 9 : (PROF == 3 ? 17 : 3));
+  constexpr int NPT = PROF == 0 ? kModesCh0 : (PROF == 1 ? 9 : (PROF == 3 ? 17 : 3));
   const int pix = blockIdx.x * 32 + threadIdx.x;
   const int blk = blockIdx.y * blockDim.y + threadIdx.y;      // channel block of this thread
   const int m = md.fine_m;
-  const int cpb = (PROF == 0 || PROF == 3) ? 8 : (PROF == 1 ? 8 / m : 1);    // channels per thread
+  const int cpb = PROF == 0 ? kModesCh0 : (PROF == 3 ? 8 : (PROF == 1 ? 8 / m : 1));    // channels per thread
   const int v0 = blk * cpb;
   if (pix >= npix || v0 >= nv) return;
   const int npanel = PROF == 2 ? m / 2 : 1;
@@ -232,11 +233,12 @@ transfer_modes_kernel(MarchConsts mc, ModeConsts md, const float* __restrict__ c
   }
 
   // ---- channel values of this thread -> convert and store
-  float res[8];
+  constexpr int NRES = PROF == 0 ? kModesCh0 : 8;
+  float res[NRES];
   int nch = min(cpb, nv - v0);
   if constexpr (PROF == 0) {
 #pragma unroll
-    for (int k = 0; k < 8; ++k) res[k] = convert_out(Dfin[k], Cfin, mc);
+    for (int k = 0; k < NRES; ++k) res[k] = convert_out(Dfin[k], Cfin, mc);
   } else if constexpr (PROF == 3) {
 #pragma unroll
     for (int c = 0; c < 8; ++c)
@@ -266,12 +268,13 @@ transfer_modes_kernel(MarchConsts mc, ModeConsts md, const float* __restrict__ c
   }
   if (out != nullptr) {
     float* o = out + (int64_t)pix * nv + v0;
-    if ((PROF == 0 || PROF == 3) && nch == 8 && (((int64_t)pix * nv + v0) & 3) == 0) {
-      reinterpret_cast<float4*>(o)[0] = make_float4(res[0], res[1], res[2], res[3]);
-      reinterpret_cast<float4*>(o)[1] = make_float4(res[4], res[5], res[6], res[7]);
+    if ((PROF == 0 || PROF == 3) && nch == NRES && (((int64_t)pix * nv + v0) & 3) == 0) {
+#pragma unroll
+      for (int k = 0; k < NRES; k += 4)
+        reinterpret_cast<float4*>(o)[k / 4] = make_float4(res[k], res[k + 1], res[k + 2], res[k + 3]);
     } else {
 #pragma unroll
-      for (int k = 0; k < 8; ++k)
+      for (int k = 0; k < NRES; ++k)
         if (k < nch) o[k] = res[k];
     }
   }
@@ -283,7 +286,7 @@ inline cudaError_t launch_transfer_modes_t(const MarchConsts& mc, const ModeCons
                                            int npix, int nz, int nv, float* out, float* out_cont, cudaStream_t st) {
   const int m = md.fine_m;
   const int prof = m == 0 ? 0 : (m == 2 ? 3 : ((m == 4 || m == 8) ? 1 : 2));
-  const int cpb = (prof == 0 || prof == 3) ? 8 : (prof == 1 ? 8 / m : 1);
+  const int cpb = prof == 0 ? kModesCh0 : (prof == 3 ? 8 : (prof == 1 ? 8 / m : 1));
   const int nblk = (nv + cpb - 1) / cpb;
   dim3 block(32, 4), grid((npix + 31) / 32, (nblk + 3) / 4);
   if (prof == 0) transfer_modes_kernel<MODE, SMOOTH, 0><<<grid, block, 0, st>>>(mc, md, coef, ncell, npix, nz, nv, out, out_cont);
