@@ -398,6 +398,7 @@ iris_so_status run_transfer(iris_so_ctx* ctx, const iris::MarchConsts& mc, float
     iris::ModeConsts md;
     md.mode = ctx->cfg.transfer_mode; md.smooth = ctx->cfg.integration;
     md.fine_m = ctx->cfg.subsample > 0 ? ctx->cfg.subsample + 1 : 0;
+    md.nx = ctx->cfg.nx;
     cudaError_t e = iris::launch_transfer_modes(mc, md, ctx->d_coef, ctx->ncell, npix, nz, nv, out, out_cont, st);
     ctx->launches++;
     if (e != cudaSuccess) return cuda_fail(ctx, e, "launch of transfer_modes_kernel");

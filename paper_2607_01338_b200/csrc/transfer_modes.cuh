@@ -35,6 +35,7 @@ namespace iris {
 struct ModeConsts {
   int mode, smooth;      // transfer mode 0 / 1 / 2, integration 0 / 1
   int fine_m;            // 0: channel-integrated profile; else fine intervals per channel (f + 1, even)
+  int nx;                // pixels per image row (npix = nx * rows)
 };
 
 // w(t) = (1 - exp(-t)) / t, w(0) = 1
@@ -54,7 +55,12 @@ __global__ void __launch_bounds__(128)
 transfer_modes_kernel(MarchConsts mc, ModeConsts md, const float* __restrict__ coef, int64_t ncell, int npix, int nz,
                       int nv, float* __restrict__ out, float* __restrict__ out_cont) {
   constexpr int NPT = PROF == 0 ? kModesCh0 : (PROF == 1 ? 9 : (PROF == 3 ? 17 : 3));
-  const int pix = blockIdx.x * 32 + threadIdx.x;
+  // a warp takes a tile of 8 x 4 pixels: whole 32-byte sectors of every plane, and a quarter of the spread in
+  // line-of-sight velocity that 32 pixels along x have (the dust-only path is taken when NO pixel of the warp is near
+  // the line, and rotation shifts the line by several channels per pixel along x)
+  const int tiles_x = (md.nx + 7) >> 3;
+  const int px = (blockIdx.x % tiles_x) * 8 + (threadIdx.x & 7), py = (blockIdx.x / tiles_x) * 4 + (threadIdx.x >> 3);
+  const int pix = px < md.nx ? py * md.nx + px : npix;
   const int blk = blockIdx.y * blockDim.y + threadIdx.y;      // channel block of this thread
   const int m = md.fine_m;
   const int cpb = PROF == 0 ? kModesCh0 : (PROF == 3 ? 8 : (PROF == 1 ? 8 / m : 1));    // channels per thread
@@ -288,7 +294,8 @@ inline cudaError_t launch_transfer_modes_t(const MarchConsts& mc, const ModeCons
   const int prof = m == 0 ? 0 : (m == 2 ? 3 : ((m == 4 || m == 8) ? 1 : 2));
   const int cpb = prof == 0 ? kModesCh0 : (prof == 3 ? 8 : (prof == 1 ? 8 / m : 1));
   const int nblk = (nv + cpb - 1) / cpb;
-  dim3 block(32, 4), grid((npix + 31) / 32, (nblk + 3) / 4);
+  const int rows = npix / md.nx;
+  dim3 block(32, 4), grid(((md.nx + 7) / 8) * ((rows + 3) / 4), (nblk + 3) / 4);
   if (prof == 0) transfer_modes_kernel<MODE, SMOOTH, 0><<<grid, block, 0, st>>>(mc, md, coef, ncell, npix, nz, nv, out, out_cont);
   else if (prof == 1) transfer_modes_kernel<MODE, SMOOTH, 1><<<grid, block, 0, st>>>(mc, md, coef, ncell, npix, nz, nv, out, out_cont);
   else if (prof == 3) transfer_modes_kernel<MODE, SMOOTH, 3><<<grid, block, 0, st>>>(mc, md, coef, ncell, npix, nz, nv, out, out_cont);
