@@ -328,9 +328,17 @@ adjoint_march_kernel(MarchConsts mc, AdjointConsts ac, const float* __restrict__
   // first march: total line optical depth per channel and total dust optical depth
   float totD = 0.0f;
   const float* p = coef + pix;
-  for (int z = 0; z < nz; ++z, p += npix) {
-    const float e_c = p[0], a_c = p[ncell], c_los = p[2 * ncell], s = p[3 * ncell];
-    if (DUST) totD += p[4 * ncell];
+  // both marches load the coefficients of a cell one cell ahead
+  float n_e = p[0], n_a = p[ncell], n_c = p[2 * ncell], n_s = p[3 * ncell];
+  float n_td = DUST ? p[4 * ncell] : 0.0f, n_sd = 0.0f;
+  for (int z = 0; z < nz; ++z) {
+    const float e_c = n_e, a_c = n_a, c_los = n_c, s = n_s;
+    if (DUST) totD += n_td;
+    if (z + 1 < nz) {
+      p += npix;
+      n_e = p[0]; n_a = p[ncell]; n_c = p[2 * ncell]; n_s = p[3 * ncell];
+      if (DUST) n_td = p[4 * ncell];
+    }
     int klo, khi;
     const int W = line_window(e_c, a_c, c_los, s, nv, klo, khi);
     if (W > 0) {
@@ -360,9 +368,16 @@ adjoint_march_kernel(MarchConsts mc, AdjointConsts ac, const float* __restrict__
   // second march: forward state and closed-form adjoint together
   float C = mc.T_bg, G = 1.0f, cumD = 0.0f;
   p = coef + pix;
-  for (int z = 0; z < nz; ++z, p += npix) {
-    const float e_c = p[0], a_c = p[ncell], c_los = p[2 * ncell], s = p[3 * ncell];
-    const float tau_d = DUST ? p[4 * ncell] : 0.0f, S_d = DUST ? p[5 * ncell] : 0.0f;
+  n_e = p[0]; n_a = p[ncell]; n_c = p[2 * ncell]; n_s = p[3 * ncell];
+  if (DUST) { n_td = p[4 * ncell]; n_sd = p[5 * ncell]; }
+  for (int z = 0; z < nz; ++z) {
+    const float e_c = n_e, a_c = n_a, c_los = n_c, s = n_s;
+    const float tau_d = DUST ? n_td : 0.0f, S_d = DUST ? n_sd : 0.0f;
+    if (z + 1 < nz) {
+      p += npix;
+      n_e = p[0]; n_a = p[ncell]; n_c = p[2 * ncell]; n_s = p[3 * ncell];
+      if (DUST) { n_td = p[4 * ncell]; n_sd = p[5 * ncell]; }
+    }
     int klo, khi;
     const int W = line_window(e_c, a_c, c_los, s, nv, klo, khi);
     float E_d = 1.0f, m_d = 0.0f, Gn = 1.0f, Lam = 1.0f;
