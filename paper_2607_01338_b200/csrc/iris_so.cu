@@ -409,9 +409,10 @@ iris_so_status run_transfer(iris_so_ctx* ctx, const iris::MarchConsts& mc, float
   const bool fits = (size_t)(32 / 8) * ((size_t)nv + 32) * sizeof(float) + 2048 <= 227u * 1024u;
   if (algo == IRIS_SO_ALGO_DENSE || !fits) {
     constexpr int CB = 16, NW = 4;
-    dim3 block(32, NW), grid((npix + 31) / 32, (nv + CB * NW - 1) / (CB * NW));
-    if (dust) iris::transfer_dense_kernel<CB, true><<<grid, block, 0, st>>>(mc, ctx->d_coef, ctx->ncell, npix, nz, nv, out, out_cont);
-    else iris::transfer_dense_kernel<CB, false><<<grid, block, 0, st>>>(mc, ctx->d_coef, ctx->ncell, npix, nz, nv, out, out_cont);
+    const int nx = ctx->cfg.nx, rows = npix / nx;
+    dim3 block(32, NW), grid(((nx + 7) / 8) * ((rows + 3) / 4), (nv + CB * NW - 1) / (CB * NW));
+    if (dust) iris::transfer_dense_kernel<CB, true><<<grid, block, 0, st>>>(mc, ctx->d_coef, ctx->ncell, npix, nx, nz, nv, out, out_cont);
+    else iris::transfer_dense_kernel<CB, false><<<grid, block, 0, st>>>(mc, ctx->d_coef, ctx->ncell, npix, nx, nz, nv, out, out_cont);
     IRIS_CHECK_LAUNCH(ctx, "transfer_dense_kernel");
     return IRIS_SO_OK;
   }

@@ -1,8 +1,9 @@
 // K3 (dense formulation): LOS transfer with register-resident channel blocks.
 //
-// Thread <-> (pixel, block of CB consecutive channels).  A warp holds 32 consecutive pixels of the sky
-// plane (x fastest) and one channel block, so the six coefficient planes are read with fully coalesced
-// 128-byte requests, once per z step, and reused for the CB channels a thread keeps in registers.  The
+// Thread <-> (pixel, block of CB consecutive channels).  A warp holds an 8 x 4 tile of pixels of the sky plane
+// (whole 32-byte sectors of every plane; a quarter of the spread in line-of-sight velocity that 32 pixels
+// along x have, so fewer warps have to evaluate a block that only some of their pixels need) and one channel
+// block; the six planes are read once per z step and reused for the CB channels a thread keeps in registers.  The
 // CB + 1 channel edges of a block share their erfc evaluations.  A block farther than the erfc fit range
 // from the line centre only attenuates by the dust (D *= E_d) -- exact in fp32 because erfc underflows
 // the fp32 sum there.  The continuum march (K4) is a scalar per thread; subtraction / unit conversion
@@ -14,9 +15,11 @@ namespace iris {
 
 template <int CB, bool DUST>
 __global__ void __launch_bounds__(128)
-transfer_dense_kernel(MarchConsts mc, const float* __restrict__ coef, int64_t ncell, int npix, int nz, int nv,
+transfer_dense_kernel(MarchConsts mc, const float* __restrict__ coef, int64_t ncell, int npix, int nx, int nz, int nv,
                       float* __restrict__ out, float* __restrict__ out_cont) {
-  const int pix = blockIdx.x * 32 + threadIdx.x;
+  const int tiles_x = (nx + 7) >> 3;
+  const int px = (blockIdx.x % tiles_x) * 8 + (threadIdx.x & 7), py = (blockIdx.x / tiles_x) * 4 + (threadIdx.x >> 3);
+  const int pix = px < nx ? py * nx + px : npix;
   const int cb = blockIdx.y * blockDim.y + threadIdx.y;
   const int k0 = cb * CB;
   if (pix >= npix || k0 >= nv) return;
