@@ -266,6 +266,7 @@ void fold_constants(iris_so_ctx* ctx) {
   mc.T_bg = (float)planck_krj(H_PLANCK * nu / K_BOLTZ, c.T_cmb);
   mc.inv_KRJ = (float)(1.0 / KRJ);
   mc.out_mode = out_mode_of(c);
+  mc.fine_m = 0;
 
   iris::BeamConsts& bc = ctx->bc;
   std::memset(&bc, 0, sizeof bc);
@@ -380,12 +381,28 @@ bool windowed_thin_mode(const iris_so_config& c) {
          c.dv_cms <= (double)iris::kSeriesMaxS * c.microturb_cms && spectra_fit_shared(c);
 }
 
+// Optically thick formal transfer on the fine velocity grid (subsample = f > 0): the same line-window march over the
+// nv (f + 1) + 1 points of the fine grid with the point profile, Simpson's rule per channel in the epilogue (MODE 3).
+bool windowed_fine_mode(const iris_so_config& c) {
+  if (!(c.transfer_mode == 0 && c.integration == 0 && c.subsample > 0 && c.transfer_algo != IRIS_SO_ALGO_DENSE)) return false;
+  const size_t points = (size_t)c.nv * (size_t)(c.subsample + 1) + 1;
+  return (size_t)(32 / 8) * (points + 32) * sizeof(float) + 2048 <= 227u * 1024u;
+}
+
 // K3 (+K4, K5) from ctx->d_coef
 iris_so_status run_transfer(iris_so_ctx* ctx, const iris::MarchConsts& mc, float* out, float* out_cont, cudaStream_t st) {
   const bool dust = ctx->cfg.dust_on != 0;
   const int npix = (int)ctx->npix, nz = ctx->cfg.nz, nv = ctx->cfg.nv;
   const int algo = resolved_algo(ctx->cfg);
   ProfScope prof(ctx, IRIS_SO_STAGE_TRANSFER, st);
+  if (windowed_fine_mode(ctx->cfg)) {
+    iris::MarchConsts mf = mc;
+    mf.fine_m = ctx->cfg.subsample + 1;
+    cudaError_t e = iris::launch_transfer_series(mf, ctx->d_coef, ctx->ncell, npix, nz, nv, dust, 0.0f, out, out_cont, st, 3);
+    ctx->launches++;
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "launch of the line-window transfer kernel (fine grid)");
+    return IRIS_SO_OK;
+  }
   if (windowed_thin_mode(ctx->cfg)) {
     cudaError_t e = iris::launch_transfer_series(mc, ctx->d_coef, ctx->ncell, npix, nz, nv, dust,
                                                  (float)(ctx->cfg.dv_cms / ctx->cfg.microturb_cms), out, out_cont, st,
@@ -472,7 +489,7 @@ const char* iris_so_last_error(const iris_so_ctx* ctx) { return ctx ? ctx->err.c
 
 const char* iris_so_transfer_kernel(const iris_so_ctx* ctx) {
   if (!ctx) return "";
-  if (windowed_thin_mode(ctx->cfg)) return "transfer_series_kernel";
+  if (windowed_thin_mode(ctx->cfg) || windowed_fine_mode(ctx->cfg)) return "transfer_series_kernel";
   if (!hot_path_mode(ctx->cfg)) return "transfer_modes_kernel";
   if ((size_t)(32 / 8) * ((size_t)ctx->cfg.nv + 32) * sizeof(float) + 2048 > 227u * 1024u) return "transfer_dense_kernel";
   switch (resolved_algo(ctx->cfg)) {

@@ -41,6 +41,7 @@ struct MarchConsts {
   float hnu_k;      // h nu0 / k
   float inv_KRJ;    // 2 k nu0^2 / c^2  (Kelvin -> CGS intensity)
   int out_mode;
+  int fine_m;       // fine velocity grid of the series kernel's MODE 3: intervals per channel (f + 1); 0 elsewhere
 };
 
 // Planck brightness temperature of a Rayleigh-Jeans temperature (Eq. 4.9.1 with I = T_rj / K_RJ):

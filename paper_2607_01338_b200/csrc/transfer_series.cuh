@@ -59,12 +59,20 @@ struct SeriesRecord { float4 q0, q1, q2, q3; };
 // MODE 0: optically thick formal step (the hot path).  MODE 1: selectively thin, formal (Eq. 4.8.13 - 4.8.15): the
 // polynomial gives the erf difference itself, q2 = { e_c w(tau_d), a_c w(tau_d), -, E_d }.  MODE 2: optically thin, formal
 // (Eq. 4.7.3 - 4.7.6): the polynomial gives E = e_c dErf, no attenuation (E_d = exp(tau_d) = 1), continuum adds tau_d S_d.
+// MODE 3: optically thick formal step on the fine velocity grid (Eq. 4.5.1): the spectrum holds the nv m + 1 POINTS
+// k / m (channel-edge units), the profile is the point value (2 s / sqrt(pi)) exp(-x^2) of Eq. 3.3.3 in erf-difference
+// units (polynomial = 1), the points are spaced s / m Doppler widths; Simpson's rule over a channel is the epilogue.
 template <bool DUST, int DEG, int MODE = 0>
 __device__ __forceinline__ SeriesRecord make_series_record(float e_c, float a_c, float c_los, float s, float tau_d,
-                                                           float S_d, float T_bg, int nv) {
+                                                           float S_d, float T_bg, int nv, int fine_m) {
   constexpr float LOG2E = 1.4426950408889634f;
   SeriesRecord r;
   int klo, khi;
+  const float s_amp = s;                       // the amplitude is per channel width in every mode
+  if (MODE == 3) {                             // point k sits where "channel" k of width 1 / m has its centre
+    c_los = fmaf(c_los, (float)fine_m, 0.5f);
+    s = s / (float)fine_m;
+  }
   int W = line_window(e_c, a_c, c_los, s, nv, klo, khi);
   int qlo = 0, nq = 0;
   if (W > 0) { qlo = klo >> 1; nq = (khi >> 1) - qlo + 1; }
@@ -72,15 +80,15 @@ __device__ __forceinline__ SeriesRecord make_series_record(float e_c, float a_c,
   // (changes tau_L by < 1e-10 e_c, i.e. < 1e-7 for a 1000 K line)
   const float a_min = fmaxf(1.0e-10f * e_c, 1.0e-30f);
   const float a_safe = fabsf(a_c) < a_min ? a_min : a_c;
-  const float sp = 1.1283791670955126f * s;                 // 2 s / sqrt(pi)
+  const float sp = 1.1283791670955126f * s_amp;             // 2 s / sqrt(pi)
   const float As = a_safe * sp, Es = e_c * sp;
-  const float Asp = MODE == 0 ? As * LOG2E : (MODE == 1 ? sp : Es);   // what the polynomial is scaled by
+  const float Asp = (MODE == 0 || MODE == 3) ? As * LOG2E : (MODE == 1 ? sp : Es);   // what the polynomial is scaled by
   const float xs = 1.2011224087864498f * s;                 // s sqrt(log2 e)
   r.q0.x = ((float)(2 * qlo) + 0.5f - c_los) * xs;
   r.q0.y = xs;
   r.q0.w = __int_as_float(qlo | (nq << 16));
   // polynomial in u = x^2, rescaled to u' = u log2(e) (p'_k = p_k ln(2)^k) and multiplied by As'
-  const float s2 = s * s, s4 = s2 * s2, s6 = s4 * s2, s8 = s4 * s4;
+  const float s2 = MODE == 3 ? 0.0f : s * s, s4 = s2 * s2, s6 = s4 * s2, s8 = s4 * s4;
   const float p0 = 1.0f - s2 * (1.0f / 12.0f) + s4 * (1.0f / 160.0f) - s6 * (1.0f / 2688.0f) + s8 * (1.0f / 55296.0f);
   const float p1 = s2 * (1.0f / 6.0f) - s4 * (1.0f / 40.0f) + s6 * (1.0f / 448.0f) - s8 * (1.0f / 6912.0f);
   const float p2 = s4 * (1.0f / 120.0f) - s6 * (1.0f / 672.0f) + s8 * (1.0f / 6912.0f);
@@ -188,7 +196,7 @@ __device__ __forceinline__ void series_passes(float* d, int q, int qend, f32x2 x
     upk(u[k], u0, u1);
     t[k] = mul2(pk(ex2_approx(-u0), ex2_approx(-u1)), pol[k]);      // tau_L log2(e)  (MODE 1: dErf, MODE 2: e_c dErf)
   }
-  if constexpr (MODE != 0) {
+  if constexpr (MODE == 1 || MODE == 2) {
     // thin: Dt += E.  selectively thin: Dt' = max(Dt + K dErf, -C' G'),  K = G' w(tau_d) (e_c - a_c C') in o.Pn, the clamp in o.CG
 #pragma unroll
     for (int k = 0; k < P; ++k) {
@@ -276,6 +284,7 @@ transfer_series_kernel(MarchConsts mc, const float* __restrict__ coef, int64_t n
   const int pix = pix0 + g;
   const bool valid = pix < npix;
   const int npair = nvp / 2;                    // nvp is a multiple of 2 LPP
+  const int npts = MODE == 3 ? nv * mc.fine_m + 1 : nv;      // spectral points held per pixel
   // shared memory: records [wpc][NQ][32], then spectra [wpc][npair / LPP rows][ROW]
   float4* rec = smem4 + (size_t)warp * (NQ * 32);
   float* spec = reinterpret_cast<float*>(smem4 + (size_t)wpc * (NQ * 32));
@@ -351,7 +360,7 @@ transfer_series_kernel(MarchConsts mc, const float* __restrict__ coef, int64_t n
   for (int z0 = 0; z0 < nz; z0 += LPP) {
     // ---- phase A: one record per lane
     {
-      const SeriesRecord r = make_series_record<DUST, DEG, MODE>(l_e, l_a, l_c, l_s, l_td, l_sd, mc.T_bg, nv);
+      const SeriesRecord r = make_series_record<DUST, DEG, MODE>(l_e, l_a, l_c, l_s, l_td, l_sd, mc.T_bg, npts, mc.fine_m);
       chunk_busy = __any_sync(0xffffffffu, ((unsigned)__float_as_int(r.q0.w) >> 16) != 0u);   // also: phase B is done
       rec[lane] = r.q0;
       rec[32 + lane] = r.q1;
@@ -399,6 +408,21 @@ transfer_series_kernel(MarchConsts mc, const float* __restrict__ coef, int64_t n
   __syncwarp();
 
   const float invG = 1.0f / G;
+  if (MODE == 3) {
+    // Simpson's rule over the m + 1 points of every channel (Eq. 4.5.1), then subtraction / conversion
+    if (valid && out != nullptr) {
+      const int m = mc.fine_m;
+      const float wgt = invG / (3.0f * (float)m);
+      auto point = [&](int k) { return sp[((k >> 1) / LPP) * ROW + ((k >> 1) % LPP) * 2 + (k & 1)]; };
+      for (int c = i; c < nv; c += LPP) {
+        float acc = 0.0f;
+        for (int j = 0; j < m; j += 2) acc += point(c * m + j) + 4.0f * point(c * m + j + 1) + point(c * m + j + 2);
+        out[(int64_t)pix * nv + c] = convert_out(acc * wgt, C, mc);
+      }
+    }
+    if (valid && out_cont != nullptr && i == 0) out_cont[pix] = C * mc.inv_KRJ;
+    return;
+  }
   if (valid) {
     if (out != nullptr) {
       float* o = out + (int64_t)pix * nv;
@@ -424,9 +448,10 @@ inline cudaError_t launch_transfer_series_t(const MarchConsts& mc, const float* 
                                             int nv, float* out, float* out_cont, cudaStream_t st) {
   constexpr int PPW = 32 / LPP;
   constexpr int NQ = SeriesLayout<DUST, DEG>::NQ;
+  const int npts = MODE == 3 ? nv * mc.fine_m + 1 : nv;
   // whole rows of LPP channel pairs, plus one row: the last pass of a window runs all LPP lanes of the pixel, up to
   // LPP - 1 pairs past the window (their update is below the window threshold, or lands in this padding)
-  const int nvp = (nv + 2 * LPP - 1) / (2 * LPP) * (2 * LPP) + 2 * LPP;
+  const int nvp = (npts + 2 * LPP - 1) / (2 * LPP) * (2 * LPP) + 2 * LPP;
   const size_t rec_per_warp = (size_t)NQ * 32 * sizeof(float4);
   const size_t spec_per_warp = (size_t)PPW * nvp * sizeof(float);
   int wpc = 4;
@@ -443,8 +468,9 @@ inline cudaError_t launch_transfer_series_t(const MarchConsts& mc, const float* 
 }
 
 // s_max: upper bound of dv / b over all cells (dv / microturbulence); selects the polynomial degree.
-// mode: 0 optically thick, 1 selectively thin, 2 optically thin (formal integration, channel-integrated profile); modes 1
-// and 2 always run the dust instantiation (tau_d = S_d = 0 planes when the dust is off).
+// mode: 0 optically thick, 1 selectively thin, 2 optically thin (formal integration, channel-integrated profile), 3 optically
+// thick on the fine velocity grid of mc.fine_m intervals per channel; modes 1 - 3 always run the dust instantiation
+// (tau_d = S_d = 0 planes when the dust is off).
 inline cudaError_t launch_transfer_series(const MarchConsts& mc, const float* coef, int64_t ncell, int npix, int nz, int nv,
                                           bool dust, float s_max, float* out, float* out_cont, cudaStream_t st, int mode = 0) {
   const bool deg3 = s_max <= kSeriesDeg3MaxS;
@@ -452,6 +478,7 @@ inline cudaError_t launch_transfer_series(const MarchConsts& mc, const float* co
                              : launch_transfer_series_t<8, true, 4, 1>(mc, coef, ncell, npix, nz, nv, out, out_cont, st);
   if (mode == 2) return deg3 ? launch_transfer_series_t<8, true, 3, 2>(mc, coef, ncell, npix, nz, nv, out, out_cont, st)
                              : launch_transfer_series_t<8, true, 4, 2>(mc, coef, ncell, npix, nz, nv, out, out_cont, st);
+  if (mode == 3) return launch_transfer_series_t<8, true, 3, 3>(mc, coef, ncell, npix, nz, nv, out, out_cont, st);
   if (dust) return deg3 ? launch_transfer_series_t<8, true, 3>(mc, coef, ncell, npix, nz, nv, out, out_cont, st)
                         : launch_transfer_series_t<8, true, 4>(mc, coef, ncell, npix, nz, nv, out, out_cont, st);
   return deg3 ? launch_transfer_series_t<8, false, 3>(mc, coef, ncell, npix, nz, nv, out, out_cont, st)

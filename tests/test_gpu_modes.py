@@ -13,13 +13,16 @@ from parity import assert_spectra, krj
 
 pytestmark = pytest.mark.gpu
 
-# (transfer_mode, integration, subsample).  The two formal modes with the channel-integrated profile run through the
-# line-window series kernel by default; the "_dense" entries force transfer_modes_kernel (transfer_algo = 1).
+# (transfer_mode, integration, subsample).  The formal modes (thin and selectively thin with the channel-integrated
+# profile, thick on the fine grid) run through the line-window series kernel by default; the "_dense" entries force
+# transfer_modes_kernel (transfer_algo = 1).
 MODES = {"thin_formal": (2, 0, 0), "thin_smooth": (2, 1, 0), "selthin_formal": (1, 0, 0), "selthin_smooth": (1, 1, 0),
          "thick_smooth": (0, 1, 0), "thick_formal_sub1": (0, 0, 1), "thick_formal_sub3": (0, 0, 3),
          "thick_smooth_sub1": (0, 1, 1), "thick_smooth_sub7": (0, 1, 7),
-         "thin_formal_dense": (2, 0, 0), "selthin_formal_dense": (1, 0, 0)}
-WINDOWED = ("thin_formal", "selthin_formal")
+         "thin_formal_dense": (2, 0, 0), "selthin_formal_dense": (1, 0, 0),
+         "thick_formal_sub1_dense": (0, 0, 1), "thick_formal_sub3_dense": (0, 0, 3)}
+WINDOWED = ("thin_formal", "selthin_formal")          # series kernel when dv <= 0.55 xi
+WINDOWED_FINE = ("thick_formal_sub1", "thick_formal_sub3")   # series kernel on the fine grid, any channel width
 
 
 def dev(a):
@@ -41,7 +44,8 @@ def gpu_cube(cfg, f, **kw):
     dense = cfg.name.endswith("_dense")
     it = IrisSO(cfg, transfer_algo=1 if dense else 0)
     # the series kernel needs dv <= 0.55 xi; every workload here has it except where a test says otherwise
-    windowed = cfg.name in WINDOWED and cfg.microturb_cms > 0 and cfg.dv_cms <= 0.55 * cfg.microturb_cms
+    windowed = (cfg.name in WINDOWED and cfg.microturb_cms > 0 and cfg.dv_cms <= 0.55 * cfg.microturb_cms) or \
+        cfg.name in WINDOWED_FINE
     assert it.transfer_kernel() == ("transfer_series_kernel" if windowed else "transfer_modes_kernel"), cfg.name
     return it.observe(*dev_fields(f), **kw).cpu().numpy()
 
@@ -81,7 +85,7 @@ def test_modes_degenerate_shapes(mode, shape):
 
 
 @pytest.mark.parametrize("mode", ["selthin_formal", "selthin_formal_dense", "thin_formal", "selthin_smooth", "thick_smooth",
-                                  "thick_smooth_sub1"])
+                                  "thick_smooth_sub1", "thick_formal_sub1", "thick_formal_sub3_dense"])
 @pytest.mark.parametrize("case", ["thick_line", "opaque_dust_clamp", "absorption"])
 def test_modes_regimes(mode, case):
     """Large optical depths (A-stability of BDF2), the ReLU clamp, and lines in absorption."""
@@ -111,7 +115,7 @@ def test_modes_regimes(mode, case):
     assert_spectra(cube, ref, extra=3e-7 * np.abs(ref_tot).max(axis=-1, keepdims=True), what=mode + " subtracted")
 
 
-@pytest.mark.parametrize("mode", ["thin_formal", "selthin_formal", "selthin_smooth", "thick_smooth_sub1"])
+@pytest.mark.parametrize("mode", ["thin_formal", "selthin_formal", "selthin_smooth", "thick_smooth_sub1", "thick_formal_sub1"])
 def test_modes_transfer_intensities_and_output_units(mode):
     from paper_2607_01338_b200 import IrisSO
     cfg, r = make_workload("small", n=16, nv=64)
@@ -145,7 +149,7 @@ def test_modes_adjoint_is_refused_and_bad_modes_are_rejected():
             IrisSO(cfg.with_(**bad))
 
 
-@pytest.mark.parametrize("mode", ["thick_smooth_sub1", "selthin_formal", "thin_formal", "thin_smooth"])
+@pytest.mark.parametrize("mode", ["thick_smooth_sub1", "thick_formal_sub1", "selthin_formal", "thin_formal", "thin_smooth"])
 def test_modes_full_size_medium_sampled(mode):
     """BASELINE config "medium" at full size (256 x 256 x 288 cells, 512 channels), in the launch configuration
     bench.py times: seeded pixel columns against the oracle (columns are independent before the beam)."""
