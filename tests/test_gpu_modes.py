@@ -39,14 +39,15 @@ def with_mode(cfg, name):
     return cfg
 
 
-def gpu_cube(cfg, f, **kw):
+def gpu_cube(cfg, f, expect_kernel=True, **kw):
     from paper_2607_01338_b200 import IrisSO
     dense = cfg.name.endswith("_dense")
     it = IrisSO(cfg, transfer_algo=1 if dense else 0)
     # the series kernel needs dv <= 0.55 xi; every workload here has it except where a test says otherwise
     windowed = (cfg.name in WINDOWED and cfg.microturb_cms > 0 and cfg.dv_cms <= 0.55 * cfg.microturb_cms) or \
         cfg.name in WINDOWED_FINE
-    assert it.transfer_kernel() == ("transfer_series_kernel" if windowed else "transfer_modes_kernel"), cfg.name
+    if expect_kernel:
+        assert it.transfer_kernel() == ("transfer_series_kernel" if windowed else "transfer_modes_kernel"), cfg.name
     return it.observe(*dev_fields(f), **kw).cpu().numpy()
 
 
@@ -135,6 +136,40 @@ def test_modes_transfer_intensities_and_output_units(mode):
     # Planck-space subtraction through the same kernel
     cfg_p = cfg.with_(out_unit=2, subtract_space=1)
     assert_spectra(gpu_cube(cfg_p, f), Oracle(cfg_p).observe(f), rel=2.6e-4, floor=2.6e-6, what=mode + " planck")
+
+
+def test_modes_kernel_selection_and_fallbacks():
+    """Which kernel runs a mode (iris_so_transfer_kernel), and parity where the series kernel hands over to the dense
+    modes kernel: channels wider than 0.55 xi (thin modes), fine grids that do not fit shared memory."""
+    from paper_2607_01338_b200 import IrisSO
+    cfg, r = make_workload("small", nx=6, ny=2, nz=12, nv=64)
+    names = {}
+    for mode in ("thin_formal", "selthin_formal", "thick_formal_sub1", "thick_formal_sub3", "thick_smooth", "thin_smooth"):
+        names[mode] = IrisSO(with_mode(cfg, mode)).transfer_kernel()
+    assert names == {"thin_formal": "transfer_series_kernel", "selthin_formal": "transfer_series_kernel",
+                     "thick_formal_sub1": "transfer_series_kernel", "thick_formal_sub3": "transfer_series_kernel",
+                     "thick_smooth": "transfer_modes_kernel", "thin_smooth": "transfer_modes_kernel"}
+    # wide channels: 1 km/s against xi = 1 km/s
+    wide = cfg.with_(dv_cms=1.0 * KMS, v0_cms=-31.5 * KMS)
+    f = make_fields(wide, r)
+    f["vlos"] = (0.2 * f["vlos"]).astype(np.float32)
+    for mode in ("thin_formal", "selthin_formal"):
+        c = with_mode(wide, mode)
+        assert IrisSO(c).transfer_kernel() == "transfer_modes_kernel"
+        assert_spectra(gpu_cube(c, f), Oracle(c).observe(f), what=mode + " wide channels")
+    c = with_mode(wide, "thick_formal_sub1")                      # the point profile has no such limit
+    assert IrisSO(c).transfer_kernel() == "transfer_series_kernel"
+    assert_spectra(gpu_cube(c, f), Oracle(c).observe(f), what="thick_formal_sub1 wide channels")
+    # 4000 channels x 4 intervals = 16001 points per spectrum: beyond shared memory
+    big = cfg.with_(nv=4000, dv_cms=0.05 * KMS, v0_cms=-0.5 * 3999 * 0.05 * KMS)
+    fb = make_fields(big, r)
+    fb["vlos"] = (0.2 * fb["vlos"]).astype(np.float32)
+    c = with_mode(big, "thick_formal_sub3")
+    assert IrisSO(c).transfer_kernel() == "transfer_modes_kernel"
+    assert IrisSO(with_mode(big, "thick_formal_sub1")).transfer_kernel() == "transfer_series_kernel"
+    for mode in ("thick_formal_sub3", "thick_formal_sub1"):
+        c = with_mode(big, mode)
+        assert_spectra(gpu_cube(c, fb, expect_kernel=False), Oracle(c).observe(fb), what=mode + " 4000 channels")
 
 
 def test_modes_adjoint_is_refused_and_bad_modes_are_rejected():
