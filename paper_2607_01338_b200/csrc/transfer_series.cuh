@@ -454,8 +454,13 @@ inline cudaError_t launch_transfer_series_t(const MarchConsts& mc, const float* 
   const int nvp = (npts + 2 * LPP - 1) / (2 * LPP) * (2 * LPP) + 2 * LPP;
   const size_t rec_per_warp = (size_t)NQ * 32 * sizeof(float4);
   const size_t spec_per_warp = (size_t)PPW * nvp * sizeof(float);
-  int wpc = 4;
-  while (wpc > 1 && wpc * (rec_per_warp + spec_per_warp) > 200 * 1024) wpc >>= 1;
+  // warps per CTA: the count that leaves most warps resident in the 227 KB of an SM (ties: the larger CTA)
+  int wpc = 1, best = 0;
+  for (int w = 4; w >= 1; w >>= 1) {
+    const size_t per_cta = w * (rec_per_warp + spec_per_warp) + 1024;
+    const int resident = per_cta <= 227 * 1024 ? (int)((227 * 1024) / per_cta) * w : 0;
+    if (resident > best) { best = resident; wpc = w; }
+  }
   const size_t smem = wpc * (rec_per_warp + spec_per_warp);
   if (smem > 227 * 1024) return cudaErrorInvalidConfiguration;
   const int ppc = wpc * PPW;
