@@ -20,6 +20,7 @@
 #include "transfer_window.cuh"
 #include "transfer_series.cuh"
 #include "transfer_modes.cuh"
+#include "transfer_smooth.cuh"
 #include "adjoint_kernels.cuh"
 #include "diagnostics.cuh"
 
@@ -64,6 +65,7 @@ struct iris_so_ctx {
   std::vector<ProfRec> recs;
   std::vector<cudaEvent_t> event_pool;
   unsigned long long* d_counter = nullptr;
+  int* d_gate = nullptr;          // flag raised by transfer_smooth_window_kernel when the dense kernel has to take over
   double* d_metrics = nullptr;
   cudaStream_t s_in = nullptr, s_out = nullptr;      // copy streams of the host-buffer path
   std::vector<cudaEvent_t> slab_events;
@@ -389,6 +391,14 @@ bool windowed_fine_mode(const iris_so_config& c) {
   return (size_t)(32 / 8) * (points + 32) * sizeof(float) + 2048 <= 227u * 1024u;
 }
 
+// Optically thick transfer with the smooth integrator as a line-window march (transfer_smooth.cuh), followed by the
+// dense modes kernel gated on the flag the window kernel raises when a ReLU fires where it does not look.
+bool windowed_smooth_mode(const iris_so_config& c) {
+  if (!(c.transfer_mode == 0 && c.integration == 1 && c.transfer_algo != IRIS_SO_ALGO_DENSE && c.nz >= 2)) return false;
+  if (c.subsample == 0 && !(c.microturb_cms > 0.0 && c.dv_cms <= (double)iris::kSeriesMaxS * c.microturb_cms)) return false;
+  return iris::smooth_window_smem_per_warp(c.nv, c.subsample > 0 ? c.subsample + 1 : 0) + 1024 <= 227u * 1024u;
+}
+
 // K3 (+K4, K5) from ctx->d_coef
 iris_so_status run_transfer(iris_so_ctx* ctx, const iris::MarchConsts& mc, float* out, float* out_cont, cudaStream_t st) {
   const bool dust = ctx->cfg.dust_on != 0;
@@ -416,6 +426,21 @@ iris_so_status run_transfer(iris_so_ctx* ctx, const iris::MarchConsts& mc, float
     md.mode = ctx->cfg.transfer_mode; md.smooth = ctx->cfg.integration;
     md.fine_m = ctx->cfg.subsample > 0 ? ctx->cfg.subsample + 1 : 0;
     md.nx = ctx->cfg.nx;
+    md.gate = nullptr;
+    if (windowed_smooth_mode(ctx->cfg)) {
+      if (!ctx->d_gate) {
+        cudaError_t e = cudaMalloc(reinterpret_cast<void**>(&ctx->d_gate), sizeof(int));
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "cudaMalloc(gate)");
+      }
+      cudaError_t e = cudaMemsetAsync(ctx->d_gate, 0, sizeof(int), st);
+      if (e != cudaSuccess) return cuda_fail(ctx, e, "cudaMemsetAsync(gate)");
+      iris::MarchConsts mf = mc;
+      mf.fine_m = md.fine_m;
+      e = iris::launch_transfer_smooth_window(mf, ctx->d_coef, ctx->ncell, npix, nz, nv, out, out_cont, ctx->d_gate, st);
+      ctx->launches++;
+      if (e != cudaSuccess) return cuda_fail(ctx, e, "launch of transfer_smooth_window_kernel");
+      md.gate = ctx->d_gate;
+    }
     cudaError_t e = iris::launch_transfer_modes(mc, md, ctx->d_coef, ctx->ncell, npix, nz, nv, out, out_cont, st);
     ctx->launches++;
     if (e != cudaSuccess) return cuda_fail(ctx, e, "launch of transfer_modes_kernel");
@@ -490,6 +515,7 @@ const char* iris_so_last_error(const iris_so_ctx* ctx) { return ctx ? ctx->err.c
 const char* iris_so_transfer_kernel(const iris_so_ctx* ctx) {
   if (!ctx) return "";
   if (windowed_thin_mode(ctx->cfg) || windowed_fine_mode(ctx->cfg)) return "transfer_series_kernel";
+  if (windowed_smooth_mode(ctx->cfg)) return "transfer_smooth_window_kernel";
   if (!hot_path_mode(ctx->cfg)) return "transfer_modes_kernel";
   if ((size_t)(32 / 8) * ((size_t)ctx->cfg.nv + 32) * sizeof(float) + 2048 > 227u * 1024u) return "transfer_dense_kernel";
   switch (resolved_algo(ctx->cfg)) {
@@ -589,7 +615,7 @@ iris_so_status iris_so_create(const iris_so_config* cfg, iris_so_ctx** out) {
 
 void iris_so_destroy(iris_so_ctx* ctx) {
   if (!ctx) return;
-  cudaFree(ctx->d_coef); cudaFree(ctx->d_tmp); cudaFree(ctx->d_stage); cudaFree(ctx->d_adj); cudaFree(ctx->d_counter); cudaFree(ctx->d_metrics); cudaFree(ctx->d_colltab);
+  cudaFree(ctx->d_coef); cudaFree(ctx->d_tmp); cudaFree(ctx->d_stage); cudaFree(ctx->d_adj); cudaFree(ctx->d_counter); cudaFree(ctx->d_gate); cudaFree(ctx->d_metrics); cudaFree(ctx->d_colltab);
   if (ctx->s_in) cudaStreamDestroy(ctx->s_in);
   if (ctx->s_out) cudaStreamDestroy(ctx->s_out);
   for (auto ev : ctx->slab_events) cudaEventDestroy(ev);

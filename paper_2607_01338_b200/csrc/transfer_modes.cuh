@@ -36,6 +36,7 @@ struct ModeConsts {
   int mode, smooth;      // transfer mode 0 / 1 / 2, integration 0 / 1
   int fine_m;            // 0: channel-integrated profile; else fine intervals per channel (f + 1, even)
   int nx;                // pixels per image row (npix = nx * rows)
+  const int* gate;       // nullptr, or a device flag: the kernel returns at once while it is 0 (transfer_smooth.cuh)
 };
 
 // w(t) = (1 - exp(-t)) / t, w(0) = 1
@@ -54,6 +55,7 @@ template <int MODE, bool SMOOTH, int PROF>
 __global__ void __launch_bounds__(128)
 transfer_modes_kernel(MarchConsts mc, ModeConsts md, const float* __restrict__ coef, int64_t ncell, int npix, int nz,
                       int nv, float* __restrict__ out, float* __restrict__ out_cont) {
+  if (md.gate != nullptr && *md.gate == 0) return;
   constexpr int NPT = PROF == 0 ? kModesCh0 : (PROF == 1 ? 9 : (PROF == 3 ? 17 : 3));
   // a warp takes a tile of 8 x 4 pixels: whole 32-byte sectors of every plane, and a quarter of the spread in
   // line-of-sight velocity that 32 pixels along x have (the dust-only path is taken when NO pixel of the warp is near

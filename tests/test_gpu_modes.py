@@ -14,15 +14,14 @@ from parity import assert_spectra, krj
 pytestmark = pytest.mark.gpu
 
 # (transfer_mode, integration, subsample).  The formal modes (thin and selectively thin with the channel-integrated
-# profile, thick on the fine grid) run through the line-window series kernel by default; the "_dense" entries force
-# transfer_modes_kernel (transfer_algo = 1).
+# profile, thick on the fine grid) run through the line-window series kernel by default and the thick smooth modes
+# through the line-window smooth kernel; the "_dense" entries force transfer_modes_kernel (transfer_algo = 1).
 MODES = {"thin_formal": (2, 0, 0), "thin_smooth": (2, 1, 0), "selthin_formal": (1, 0, 0), "selthin_smooth": (1, 1, 0),
          "thick_smooth": (0, 1, 0), "thick_formal_sub1": (0, 0, 1), "thick_formal_sub3": (0, 0, 3),
          "thick_smooth_sub1": (0, 1, 1), "thick_smooth_sub7": (0, 1, 7),
          "thin_formal_dense": (2, 0, 0), "selthin_formal_dense": (1, 0, 0),
-         "thick_formal_sub1_dense": (0, 0, 1), "thick_formal_sub3_dense": (0, 0, 3)}
-WINDOWED = ("thin_formal", "selthin_formal")          # series kernel when dv <= 0.55 xi
-WINDOWED_FINE = ("thick_formal_sub1", "thick_formal_sub3")   # series kernel on the fine grid, any channel width
+         "thick_formal_sub1_dense": (0, 0, 1), "thick_formal_sub3_dense": (0, 0, 3),
+         "thick_smooth_dense": (0, 1, 0), "thick_smooth_sub1_dense": (0, 1, 1)}
 
 
 def dev(a):
@@ -39,15 +38,24 @@ def with_mode(cfg, name):
     return cfg
 
 
+def expected_kernel(cfg, dense):
+    """What iris_so_transfer_kernel should name for a configuration."""
+    m, i, s = cfg.transfer_mode, cfg.integration, cfg.subsample
+    narrow = cfg.microturb_cms > 0 and cfg.dv_cms <= 0.55 * cfg.microturb_cms
+    if not dense:
+        if i == 0 and ((s == 0 and m in (1, 2) and narrow) or (m == 0 and s > 0)):
+            return "transfer_series_kernel"
+        if i == 1 and m == 0 and cfg.nz >= 2 and (s > 0 or narrow):
+            return "transfer_smooth_window_kernel"
+    return "transfer_modes_kernel"
+
+
 def gpu_cube(cfg, f, expect_kernel=True, **kw):
     from paper_2607_01338_b200 import IrisSO
     dense = cfg.name.endswith("_dense")
     it = IrisSO(cfg, transfer_algo=1 if dense else 0)
-    # the series kernel needs dv <= 0.55 xi; every workload here has it except where a test says otherwise
-    windowed = (cfg.name in WINDOWED and cfg.microturb_cms > 0 and cfg.dv_cms <= 0.55 * cfg.microturb_cms) or \
-        cfg.name in WINDOWED_FINE
     if expect_kernel:
-        assert it.transfer_kernel() == ("transfer_series_kernel" if windowed else "transfer_modes_kernel"), cfg.name
+        assert it.transfer_kernel() == expected_kernel(cfg, dense), cfg.name
     return it.observe(*dev_fields(f), **kw).cpu().numpy()
 
 
@@ -86,7 +94,8 @@ def test_modes_degenerate_shapes(mode, shape):
 
 
 @pytest.mark.parametrize("mode", ["selthin_formal", "selthin_formal_dense", "thin_formal", "selthin_smooth", "thick_smooth",
-                                  "thick_smooth_sub1", "thick_formal_sub1", "thick_formal_sub3_dense"])
+                                  "thick_smooth_sub1", "thick_formal_sub1", "thick_formal_sub3_dense", "thick_smooth_dense",
+                                  "thick_smooth_sub1_dense"])
 @pytest.mark.parametrize("case", ["thick_line", "opaque_dust_clamp", "absorption"])
 def test_modes_regimes(mode, case):
     """Large optical depths (A-stability of BDF2), the ReLU clamp, and lines in absorption."""
@@ -148,7 +157,7 @@ def test_modes_kernel_selection_and_fallbacks():
         names[mode] = IrisSO(with_mode(cfg, mode)).transfer_kernel()
     assert names == {"thin_formal": "transfer_series_kernel", "selthin_formal": "transfer_series_kernel",
                      "thick_formal_sub1": "transfer_series_kernel", "thick_formal_sub3": "transfer_series_kernel",
-                     "thick_smooth": "transfer_modes_kernel", "thin_smooth": "transfer_modes_kernel"}
+                     "thick_smooth": "transfer_smooth_window_kernel", "thin_smooth": "transfer_modes_kernel"}
     # wide channels: 1 km/s against xi = 1 km/s
     wide = cfg.with_(dv_cms=1.0 * KMS, v0_cms=-31.5 * KMS)
     f = make_fields(wide, r)
@@ -184,7 +193,8 @@ def test_modes_adjoint_is_refused_and_bad_modes_are_rejected():
             IrisSO(cfg.with_(**bad))
 
 
-@pytest.mark.parametrize("mode", ["thick_smooth_sub1", "thick_formal_sub1", "selthin_formal", "thin_formal", "thin_smooth"])
+@pytest.mark.parametrize("mode", ["thick_smooth_sub1", "thick_smooth_sub1_dense", "thick_smooth", "thick_formal_sub1",
+                                  "selthin_formal", "thin_formal", "thin_smooth"])
 def test_modes_full_size_medium_sampled(mode):
     """BASELINE config "medium" at full size (256 x 256 x 288 cells, 512 channels), in the launch configuration
     bench.py times: seeded pixel columns against the oracle (columns are independent before the beam)."""
@@ -192,7 +202,9 @@ def test_modes_full_size_medium_sampled(mode):
     cfg, r = make_workload("medium")
     cfg = with_mode(cfg, mode)
     f = make_fields(cfg, r)
-    cube = IrisSO(cfg).observe(*dev_fields(f), beam=False, noise=False)
+    it = IrisSO(cfg, transfer_algo=1 if mode.endswith("_dense") else 0)
+    assert it.transfer_kernel() == expected_kernel(cfg, mode.endswith("_dense"))
+    cube = it.observe(*dev_fields(f), beam=False, noise=False)
     n_cols = 24
     plane = cfg.nx * cfg.ny
     pix = np.sort(np.random.default_rng(21).choice(plane, size=n_cols, replace=False))
