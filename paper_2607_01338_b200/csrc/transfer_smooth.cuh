@@ -33,29 +33,39 @@ namespace iris {
 
 constexpr int kSmoothLPP = 16;          // lanes per pixel = cells a window stays active (K)
 
-// profile weight ("erf-difference" units) of a point at x Doppler widths from the line centre
+// profile weight ("erf-difference" units) of a point at x Doppler widths from the line centre, as a function of
+// u = x^2 log2(e): (2 s / sqrt(pi)) 2^-u P(u); P = 1 for the point profile, the degree-4 polynomial of the channel
+// integral from the channel centre (transfer_series.cuh) otherwise.  Zero beyond 5.5 Doppler widths (transfer_modes.cuh).
+template <bool POINT>
 struct SmoothProfile {
   float p0, p1, p2, p3, p4;
-  __device__ __forceinline__ void set(float s_amp, bool point) {
+  __device__ __forceinline__ void set(float s_amp) {
     const float sp = 1.1283791670955126f * s_amp;               // 2 s / sqrt(pi)
-    const float s2 = point ? 0.0f : s_amp * s_amp, s4 = s2 * s2, s6 = s4 * s2, s8 = s4 * s4;
+    if (POINT) { p0 = sp; p1 = p2 = p3 = p4 = 0.0f; return; }
+    constexpr float L1 = 0.6931471805599453f, L2 = L1 * L1, L3 = L2 * L1, L4 = L2 * L2;   // u = x^2 log2(e)
+    const float s2 = s_amp * s_amp, s4 = s2 * s2, s6 = s4 * s2, s8 = s4 * s4;
     p0 = sp * (1.0f - s2 * (1.0f / 12.0f) + s4 * (1.0f / 160.0f) - s6 * (1.0f / 2688.0f) + s8 * (1.0f / 55296.0f));
-    p1 = sp * (s2 * (1.0f / 6.0f) - s4 * (1.0f / 40.0f) + s6 * (1.0f / 448.0f) - s8 * (1.0f / 6912.0f));
-    p2 = sp * (s4 * (1.0f / 120.0f) - s6 * (1.0f / 672.0f) + s8 * (1.0f / 6912.0f));
-    p3 = sp * (s6 * (1.0f / 5040.0f) - s8 * (1.0f / 25920.0f));
-    p4 = sp * (s8 * (1.0f / 362880.0f));
+    p1 = sp * L1 * (s2 * (1.0f / 6.0f) - s4 * (1.0f / 40.0f) + s6 * (1.0f / 448.0f) - s8 * (1.0f / 6912.0f));
+    p2 = sp * L2 * (s4 * (1.0f / 120.0f) - s6 * (1.0f / 672.0f) + s8 * (1.0f / 6912.0f));
+    p3 = sp * L3 * (s6 * (1.0f / 5040.0f) - s8 * (1.0f / 25920.0f));
+    p4 = sp * L4 * (s8 * (1.0f / 362880.0f));
   }
-  __device__ __forceinline__ float at(float x) const {
-    const float u = x * x;
-    if (u > 30.25f) return 0.0f;                                // beyond 5.5 Doppler widths (transfer_modes.cuh)
-    float pol = fmaf(p4, u, p3);
-    pol = fmaf(pol, u, p2);
-    pol = fmaf(pol, u, p1);
-    pol = fmaf(pol, u, p0);
-    return pol * ex2_approx(-1.4426950408889634f * u);
+  // xs = x sqrt(log2 e)
+  __device__ __forceinline__ float at(float xs) const {
+    const float u = xs * xs;
+    float pol = p0;
+    if (!POINT) {
+      pol = fmaf(p4, u, p3);
+      pol = fmaf(pol, u, p2);
+      pol = fmaf(pol, u, p1);
+      pol = fmaf(pol, u, p0);
+    }
+    const float v = pol * ex2_approx(-u);
+    return u > 43.64f ? 0.0f : v;                               // 5.5^2 log2(e)
   }
 };
 
+template <bool POINT>
 __global__ void __launch_bounds__(128)
 transfer_smooth_window_kernel(MarchConsts mc, const float* __restrict__ coef, int64_t ncell, int npix, int nz, int nv,
                               int nvp /* padded points per spectrum */, float* __restrict__ out,
@@ -69,7 +79,7 @@ transfer_smooth_window_kernel(MarchConsts mc, const float* __restrict__ coef, in
   const bool valid = pix_raw < npix;
   const int pix = valid ? pix_raw : npix - 1;                   // idle groups shadow the last pixel and write nothing
   const int m = mc.fine_m;
-  const bool point = m > 0;
+  constexpr bool point = POINT;           // fine grid with the point profile (m > 0) or channel integrals (m = 0)
   const int npts = point ? nv * m + 1 : nv;
   const size_t arr = (size_t)nvp * PPW;
   float* cur = sm + (size_t)warp * 2 * arr + g * LPP;           // U_n-1 = D_n-1 / d_n-1 when cell n is entered
@@ -133,26 +143,38 @@ transfer_smooth_window_kernel(MarchConsts mc, const float* __restrict__ coef, in
     const float inv_dn = 1.0f / d_n;
 
     if (ehi >= elo) {
-      SmoothProfile prof, prof0;
-      prof.set(s_ch, point);
-      if (n == 1) prof0.set(s_0 * fm, point);
-      for (int k = elo + i; k <= ehi; k += LPP) {
-        const int w = IDX(k);
-        const float pw = prof.at(((float)k + 0.5f - c_los) * s);
-        const float E = e_c * pw, A = a_c * pw;
-        float Du;
-        if (n == 1) {
-          const float pw0 = prof0.at(((float)k + 0.5f - c_0) * s_0);
-          const float E0 = e_0 * pw0, A0 = a_0 * pw0;
-          Du = ((E0 - A0 * C) + (E - A * C_unc)) * rcp_approx(2.0f + A + td);       // D_0 = 0
-        } else {
-          const float Dk = cur[w] * d_c, Dm = prv[w] * d_m;
-          Du = (2.0f * (E - A * C_unc) + 4.0f * Dk - Dm) * rcp_approx(fmaf(2.0f, A + td, 3.0f));
+      constexpr float SQL2E = 1.2011224087864498f;              // sqrt(log2 e)
+      SmoothProfile<POINT> prof;
+      prof.set(s_ch);
+      const float xstep = (float)LPP * s * SQL2E;
+      float xs = ((float)(elo + i) + 0.5f - c_los) * (s * SQL2E);
+      if (n == 1) {
+        // trapezoidal step over the windows of cells 0 and 1 (D_0 = 0)
+        SmoothProfile<POINT> prof0;
+        prof0.set(s_0 * fm);
+        for (int k = elo + i; k <= ehi; k += LPP, xs += xstep) {
+          const float pw = prof.at(xs);
+          const float pw0 = prof0.at(((float)k + 0.5f - c_0) * (s_0 * SQL2E));
+          const float E = e_c * pw, A = a_c * pw, E0 = e_0 * pw0, A0 = a_0 * pw0;
+          const float Du = ((E0 - A0 * C) + (E - A * C_unc)) * rcp_approx(2.0f + A + td);
+          const float U = fmaxf(Du + relu_add, relu_min) * inv_dn;              // ReLU on D + C and on C
+          prv[IDX(k)] = U;
+          u_min = fminf(u_min, U);
         }
-        const float Dn = fmaxf(Du + relu_add, relu_min);        // ReLU on D + C and on C
-        const float U = Dn * inv_dn;
-        prv[w] = U;
-        u_min = fminf(u_min, U);
+      } else {
+        // BDF2: D_n = [2 p (e_c - a_c C_n) + 4 U d_n-1 - V d_n-2] / (3 + 2 tau_d + 2 a_c p)
+        const float g2 = 2.0f * fmaf(-a_c, C_unc, e_c), a2 = 2.0f * a_c, den0 = fmaf(2.0f, td, 3.0f);
+        const float c4 = 4.0f * d_c, cm = -d_m;
+        int w = IDX(elo + i);
+        // consecutive points of a lane are LPP apart: one row (32 words) further
+        for (int k = elo + i; k <= ehi; k += LPP, xs += xstep, w += 32) {
+          const float pw = prof.at(xs);
+          const float lin = fmaf(cur[w], c4, prv[w] * cm);
+          const float Du = fmaf(pw, g2, lin) * rcp_approx(fmaf(pw, a2, den0));
+          const float U = fmaxf(Du + relu_add, relu_min) * inv_dn;              // ReLU on D + C and on C
+          prv[w] = U;
+          u_min = fminf(u_min, U);
+        }
       }
     }
     __syncwarp();
@@ -214,10 +236,17 @@ inline cudaError_t launch_transfer_smooth_window(const MarchConsts& mc, const fl
   if (best == 0) return cudaErrorInvalidConfiguration;
   const size_t smem = wpc * per_warp;
   const int ppc = wpc * (32 / kSmoothLPP);
-  cudaError_t e = cudaFuncSetAttribute(transfer_smooth_window_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (e != cudaSuccess) return e;
-  transfer_smooth_window_kernel<<<(unsigned)((npix + ppc - 1) / ppc), wpc * 32, smem, st>>>(mc, coef, ncell, npix, nz, nv, nvp,
-                                                                                            out, out_cont, gate);
+  const unsigned grid = (unsigned)((npix + ppc - 1) / ppc);
+  cudaError_t e;
+  if (mc.fine_m > 0) {
+    e = cudaFuncSetAttribute(transfer_smooth_window_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    transfer_smooth_window_kernel<true><<<grid, wpc * 32, smem, st>>>(mc, coef, ncell, npix, nz, nv, nvp, out, out_cont, gate);
+  } else {
+    e = cudaFuncSetAttribute(transfer_smooth_window_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    transfer_smooth_window_kernel<false><<<grid, wpc * 32, smem, st>>>(mc, coef, ncell, npix, nz, nv, nvp, out, out_cont, gate);
+  }
   return cudaGetLastError();
 }
 
