@@ -197,8 +197,15 @@ iris_so_status iris_so_profile_read(iris_so_ctx *ctx, int32_t stage, double *tot
 iris_so_status iris_so_transfer_work(iris_so_ctx *ctx, uint64_t *window_updates, void *cuda_stream);
 
 /* Name of the LOS transfer kernel this context launches ("transfer_series_kernel", "transfer_window_kernel",
- * "transfer_dense_kernel" or "transfer_modes_kernel"); static storage. */
+ * "transfer_dense_kernel", "transfer_modes_kernel" or "transfer_smooth_window_kernel"); static storage. */
 const char *iris_so_transfer_kernel(const iris_so_ctx *ctx);
+
+/* The optically thick mode with the smooth integrator (integration = 1; trapezoidal + BDF2 steps with the ReLU of
+ * PAPER.md:709) is marched over line windows; the march is exact unless a ReLU fires outside the windows, which the
+ * kernel detects: the dense kernel, launched right after it and gated on a device flag, then recomputes the cube.
+ * *fell_back = 1 if that happened in the last transfer / observe call of this context, 0 if not (also 0 for every other
+ * mode).  Synchronises the stream. */
+iris_so_status iris_so_smooth_fallback(iris_so_ctx *ctx, int32_t *fell_back, void *cuda_stream);
 
 /* Stand-alone post-processing stages (also used inside iris_so_observe). */
 /* K6: separable Gaussian beam of FWHM beam_fwhm_px on d_in -> d_out (must not alias), zero padding,

@@ -15,7 +15,7 @@ DECLARED_SYMBOLS = (
     "iris_so_create", "iris_so_destroy", "iris_so_last_error", "iris_so_status_string", "iris_so_version",
     "iris_so_launch_count", "iris_so_scratch_bytes", "iris_so_levelpop", "iris_so_transfer", "iris_so_observe",
     "iris_so_observe_stages", "iris_so_observe_host", "iris_so_observe_adjoint", "iris_so_beam", "iris_so_noise",
-    "iris_so_profile", "iris_so_profile_read", "iris_so_transfer_work", "iris_so_transfer_kernel",
+    "iris_so_profile", "iris_so_profile_read", "iris_so_transfer_work", "iris_so_transfer_kernel", "iris_so_smooth_fallback",
     "iris_so_density_trace", "iris_so_metrics", "iris_so_observe_adjoint_abundance",
 )
 STAGES = {"cell": 0, "transfer": 1, "beam": 2, "noise": 3, "adjoint": 4}
@@ -107,6 +107,8 @@ def load_library():
     lib.iris_so_transfer_kernel.argtypes = [vp]
     lib.iris_so_transfer_work.restype = st
     lib.iris_so_transfer_work.argtypes = [vp, C.POINTER(C.c_uint64), vp]
+    lib.iris_so_smooth_fallback.restype = st
+    lib.iris_so_smooth_fallback.argtypes = [vp, C.POINTER(C.c_int32), vp]
     lib.iris_so_density_trace.restype = st
     lib.iris_so_density_trace.argtypes = [vp, fp, fp, fp, vp]
     lib.iris_so_metrics.restype = st
@@ -230,6 +232,12 @@ class IrisSO:
         n = C.c_uint64()
         self._check(self.lib.iris_so_transfer_work(self._h, C.byref(n), self._stream()))
         return int(n.value)
+
+    def smooth_fallback(self):
+        """True if the last smooth-integrator call of this context handed over to the dense kernel."""
+        n = C.c_int32()
+        self._check(self.lib.iris_so_smooth_fallback(self._h, C.byref(n), self._stream()))
+        return bool(n.value)
 
     # -- entry points ----------------------------------------------------------------------------
     def levelpop(self, nH2, Tgas, pop=None):

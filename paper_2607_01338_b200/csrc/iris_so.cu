@@ -803,6 +803,20 @@ iris_so_status iris_so_transfer_work(iris_so_ctx* ctx, uint64_t* window_updates,
   return IRIS_SO_OK;
 }
 
+iris_so_status iris_so_smooth_fallback(iris_so_ctx* ctx, int32_t* fell_back, void* stream) {
+  if (!ctx) return IRIS_SO_EINVAL;
+  if (!fell_back) return fail(ctx, IRIS_SO_EINVAL, "iris_so_smooth_fallback: NULL output");
+  *fell_back = 0;
+  if (!ctx->d_gate || !windowed_smooth_mode(ctx->cfg)) return IRIS_SO_OK;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  int h = 0;
+  cudaError_t e;
+  if ((e = cudaMemcpyAsync(&h, ctx->d_gate, sizeof h, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(ctx, e, "D2H");
+  if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(ctx, e, "cudaStreamSynchronize");
+  *fell_back = h != 0;
+  return IRIS_SO_OK;
+}
+
 iris_so_status iris_so_beam(iris_so_ctx* ctx, const float* d_in, float* d_out, float* d_tmp, void* stream) {
   if (!ctx) return IRIS_SO_EINVAL;
   if (!d_in || !d_out) return fail(ctx, IRIS_SO_EINVAL, "iris_so_beam: NULL pointer");

@@ -13,13 +13,18 @@
 // that loses a factor ~3 per cell against it, so a point that no line has come near for K cells is a d_n to 3^-K, with
 // its own constant a.  The kernel stores U_n = D_n / d_n: such points are constants and are not touched.  A cell
 // updates, explicitly and with the ReLU, the points of its own window and of the windows of the K - 1 cells before it
-// (K = 16: 2e-8), taking D_n-1 = U d_n-1 and D_n-2 = V d_n-2 from the two stored spectra, which alternate roles.
+// (K = 12: 2e-6 of the last change of the point), taking D_n-1 = U d_n-1 and D_n-2 = V d_n-2 from the two stored
+// spectra, which alternate roles.
 //
 // What the window cannot see is a ReLU that fires OUTSIDE it: a far point a d_n + C_n < 0, or the continuum itself
 // clamped (C_n < 0 before the ReLU), or the dominant solution losing its sign (4 d_n-1 < d_n-2: a cell that turns
 // opaque abruptly).  Each lane keeps the most negative U it has stored and tests these three conditions per cell; if
 // one holds anywhere, the kernel raises *gate and the caller's next launch, transfer_modes_kernel gated on that
 // flag, recomputes the cube densely (exact in every case; the gate stays 0 for the paper's workloads).
+//
+// (The selectively thin mode is NOT run this way: its absorption saturates at I^[T] = 0, i.e. the ReLU keeps acting on
+// points long after the line has left them, and the gate fires on every thick workload; measured: 3.5 + 5.8 ms against
+// 5.8 ms for the dense kernel alone on the medium cube.)
 //
 // Mapping as in transfer_window.cuh: LPP = 16 lanes per pixel, 2 pixels per warp, both spectra of a pixel in shared
 // memory, point k at word (k / LPP) * 32 + g * LPP + k % LPP of its array.  Profile: the point value of Eq. 3.3.3 on
@@ -31,7 +36,8 @@
 
 namespace iris {
 
-constexpr int kSmoothLPP = 16;          // lanes per pixel = cells a window stays active (K)
+constexpr int kSmoothLPP = 16;          // lanes per pixel
+constexpr int kSmoothKeep = 12;         // cells a window stays active (K <= kSmoothLPP: lane i remembers cell n = i mod K)
 
 // profile weight ("erf-difference" units) of a point at x Doppler widths from the line centre, as a function of
 // u = x^2 log2(e): (2 s / sqrt(pi)) 2^-u P(u); P = 1 for the point profile, the degree-4 polynomial of the channel
@@ -95,7 +101,7 @@ transfer_smooth_window_kernel(MarchConsts mc, const float* __restrict__ coef, in
   float C = mc.T_bg, Cm = mc.T_bg;          // continuum at n - 1 and n - 2 (after the ReLU)
   float d_c = 1.0f, d_m = 1.0f;             // dominant homogeneous solution at n - 1 and n - 2
   float u_min = 0.0f;                       // most negative U this lane has stored
-  int ring_lo = 0x7fffffff, ring_hi = -1;   // window of the cell this lane remembers (cell n with n % LPP == i)
+  int ring_lo = 0x7fffffff, ring_hi = -1;   // window of the cell this lane remembers (cell n with n % K == i)
   bool risk = false;
   // cell 0, for the trapezoidal step
   float e_0 = 0.0f, a_0 = 0.0f, c_0 = 0.0f, s_0 = 1.0f, td_0 = 0.0f, Jd_0 = 0.0f;
@@ -114,7 +120,7 @@ transfer_smooth_window_kernel(MarchConsts mc, const float* __restrict__ coef, in
     // ---- window of this cell, remembered for LPP cells; the points to update are the union of what is remembered
     int klo, khi;
     const int W = line_window(e_c, a_c, c_los, s, npts, klo, khi);
-    if (i == (n % LPP)) { ring_lo = W > 0 ? klo : 0x7fffffff; ring_hi = W > 0 ? khi : -1; }
+    if (i == (n % kSmoothKeep)) { ring_lo = W > 0 ? klo : 0x7fffffff; ring_hi = W > 0 ? khi : -1; }
     int elo = ring_lo, ehi = ring_hi;
 #pragma unroll
     for (int o = LPP / 2; o > 0; o >>= 1) {
@@ -140,7 +146,7 @@ transfer_smooth_window_kernel(MarchConsts mc, const float* __restrict__ coef, in
     const float relu_add = C_unc >= 0.0f ? 0.0f : C_unc, relu_min = C_unc >= 0.0f ? -C_unc : 0.0f;
     // a ReLU outside the window (see the header): recompute densely
     if (C_unc < 0.0f || !(d_n > 1.0e-6f * d_c) || fmaf(u_min, d_n, C_unc) < 0.0f) risk = true;
-    const float inv_dn = 1.0f / d_n;
+    const float inv_dn = rcp_approx(d_n);
 
     if (ehi >= elo) {
       constexpr float SQL2E = 1.2011224087864498f;              // sqrt(log2 e)

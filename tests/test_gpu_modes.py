@@ -181,6 +181,35 @@ def test_modes_kernel_selection_and_fallbacks():
         assert_spectra(gpu_cube(c, fb, expect_kernel=False), Oracle(c).observe(fb), what=mode + " 4000 channels")
 
 
+def test_smooth_window_hands_over_when_a_relu_fires_outside_the_windows():
+    """opaque_dust_clamp makes the smooth continuum overshoot below zero (the ReLU clamps every spectral point, also
+    those no line window covers): the window kernel must notice, and the dense kernel, gated on its flag, must
+    deliver the cube.  On the unmodified workload the flag stays down."""
+    from paper_2607_01338_b200 import IrisSO
+    cfg, r = make_workload("small", n=20, nv=96)
+    for mode in ("thick_smooth", "thick_smooth_sub1"):
+        c = with_mode(cfg, mode)
+        f = make_fields(c, r)
+        f["vlos"] = (0.25 * f["vlos"]).astype(np.float32)
+        it = IrisSO(c)
+        assert it.transfer_kernel() == "transfer_smooth_window_kernel"
+        cube = it.observe(*dev_fields(f)).cpu().numpy()
+        assert not it.smooth_fallback()
+        assert_spectra(cube, Oracle(c).observe(f), what=mode)
+        c2 = c.with_(T_cmb=60.0, kappa_gas_cm2_g=3.0)
+        f["Tdust"] = np.full_like(f["Tdust"], 3.0)
+        f["nH2"][: c.nz // 2] *= 1e-3
+        f["nH2"][c.nz // 2:] *= 30.0
+        it2 = IrisSO(c2)
+        cube2 = it2.observe(*dev_fields(f)).cpu().numpy()
+        assert it2.smooth_fallback()
+        ref2 = Oracle(c2).observe(f)
+        ref_tot = Oracle(c2.with_(subtract_continuum=False)).observe(f)
+        assert_spectra(cube2, ref2, extra=3e-7 * np.abs(ref_tot).max(axis=-1, keepdims=True), what=mode + " clamped")
+        # every other mode reports 0
+        assert not IrisSO(with_mode(cfg, "thin_smooth")).smooth_fallback()
+
+
 def test_modes_adjoint_is_refused_and_bad_modes_are_rejected():
     from paper_2607_01338_b200 import IrisSO, IrisSOError
     cfg, r = make_workload("batch", n=8, nv=16)
@@ -205,6 +234,7 @@ def test_modes_full_size_medium_sampled(mode):
     it = IrisSO(cfg, transfer_algo=1 if mode.endswith("_dense") else 0)
     assert it.transfer_kernel() == expected_kernel(cfg, mode.endswith("_dense"))
     cube = it.observe(*dev_fields(f), beam=False, noise=False)
+    assert not it.smooth_fallback()          # the line-window march of the smooth integrator is exact on this workload
     n_cols = 24
     plane = cfg.nx * cfg.ny
     pix = np.sort(np.random.default_rng(21).choice(plane, size=n_cols, replace=False))
