@@ -269,6 +269,7 @@ void fold_constants(iris_so_ctx* ctx) {
   mc.inv_KRJ = (float)(1.0 / KRJ);
   mc.out_mode = out_mode_of(c);
   mc.fine_m = 0;
+  mc.ray_simpson = 0;
 
   iris::BeamConsts& bc = ctx->bc;
   std::memset(&bc, 0, sizeof bc);
@@ -378,7 +379,9 @@ bool spectra_fit_shared(const iris_so_config& c) {
 // outside a cell's line window too (in the dust-scaled spectrum), so they run through the line-window series kernel
 // (template MODE 1 / 2) whenever it applies; transfer_algo = IRIS_SO_ALGO_DENSE keeps them on transfer_modes_kernel.
 bool windowed_thin_mode(const iris_so_config& c) {
-  return (c.transfer_mode == 1 || c.transfer_mode == 2) && c.integration == 0 && c.subsample == 0 &&
+  const bool formal = (c.transfer_mode == 1 || c.transfer_mode == 2) && c.integration == 0;
+  const bool thin_simpson = c.transfer_mode == 2 && c.integration == 1;     // a weighted sum along the ray: same kernel
+  return (formal || thin_simpson) && c.subsample == 0 &&
          c.transfer_algo != IRIS_SO_ALGO_DENSE && c.microturb_cms > 0.0 &&
          c.dv_cms <= (double)iris::kSeriesMaxS * c.microturb_cms && spectra_fit_shared(c);
 }
@@ -414,7 +417,9 @@ iris_so_status run_transfer(iris_so_ctx* ctx, const iris::MarchConsts& mc, float
     return IRIS_SO_OK;
   }
   if (windowed_thin_mode(ctx->cfg)) {
-    cudaError_t e = iris::launch_transfer_series(mc, ctx->d_coef, ctx->ncell, npix, nz, nv, dust,
+    iris::MarchConsts mt = mc;
+    mt.ray_simpson = ctx->cfg.integration == 1 ? 1 : 0;
+    cudaError_t e = iris::launch_transfer_series(mt, ctx->d_coef, ctx->ncell, npix, nz, nv, dust,
                                                  (float)(ctx->cfg.dv_cms / ctx->cfg.microturb_cms), out, out_cont, st,
                                                  ctx->cfg.transfer_mode);
     ctx->launches++;

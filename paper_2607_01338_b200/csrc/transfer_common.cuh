@@ -42,6 +42,7 @@ struct MarchConsts {
   float inv_KRJ;    // 2 k nu0^2 / c^2  (Kelvin -> CGS intensity)
   int out_mode;
   int fine_m;       // fine velocity grid of the series kernel's MODE 3: intervals per channel (f + 1); 0 elsewhere
+  int ray_simpson;  // series kernel MODE 2 (optically thin): 1 = Simpson weights along the ray (Eq. 4.7.7), 0 = Eq. 4.7.6
 };
 
 // Planck brightness temperature of a Rayleigh-Jeans temperature (Eq. 4.9.1 with I = T_rj / K_RJ):

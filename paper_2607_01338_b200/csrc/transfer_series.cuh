@@ -55,6 +55,16 @@ struct SeriesLayout {
 
 struct SeriesRecord { float4 q0, q1, q2, q3; };
 
+// Weights of the sum along the ray in the optically thin mode with smooth integration (Eq. 4.7.7, reading S25): composite
+// Simpson's rule over the largest odd number of cells, the last interval of an even count by the trapezoidal rule.
+__device__ __forceinline__ float ray_simpson_weight(int n, int nz) {
+  const int Rs = (nz & 1) ? nz : nz - 1;
+  float wn = 0.0f;
+  if (Rs >= 3 && n < Rs) wn = (n == 0 || n == Rs - 1) ? (1.0f / 3.0f) : ((n & 1) ? (4.0f / 3.0f) : (2.0f / 3.0f));
+  if (!(nz & 1) && nz >= 2 && n >= nz - 2) wn += 0.5f;
+  return wn;
+}
+
 // Phase A: coefficients of one cell -> march record.
 // MODE 0: optically thick formal step (the hot path).  MODE 1: selectively thin, formal (Eq. 4.8.13 - 4.8.15): the
 // polynomial gives the erf difference itself, q2 = { e_c w(tau_d), a_c w(tau_d), -, E_d }.  MODE 2: optically thin, formal
@@ -63,8 +73,9 @@ struct SeriesRecord { float4 q0, q1, q2, q3; };
 // k / m (channel-edge units), the profile is the point value (2 s / sqrt(pi)) exp(-x^2) of Eq. 3.3.3 in erf-difference
 // units (polynomial = 1), the points are spaced s / m Doppler widths; Simpson's rule over a channel is the epilogue.
 template <bool DUST, int DEG, int MODE = 0>
+// wn: weight of the cell in the sum along the ray (MODE 2 only; 1 for the midpoint sum of Eq. 4.7.6).
 __device__ __forceinline__ SeriesRecord make_series_record(float e_c, float a_c, float c_los, float s, float tau_d,
-                                                           float S_d, float T_bg, int nv, int fine_m) {
+                                                           float S_d, float T_bg, int nv, int fine_m, float wn = 1.0f) {
   constexpr float LOG2E = 1.4426950408889634f;
   SeriesRecord r;
   int klo, khi;
@@ -81,7 +92,7 @@ __device__ __forceinline__ SeriesRecord make_series_record(float e_c, float a_c,
   const float a_min = fmaxf(1.0e-10f * e_c, 1.0e-30f);
   const float a_safe = fabsf(a_c) < a_min ? a_min : a_c;
   const float sp = 1.1283791670955126f * s_amp;             // 2 s / sqrt(pi)
-  const float As = a_safe * sp, Es = e_c * sp;
+  const float As = a_safe * sp, Es = (MODE == 2 ? wn : 1.0f) * e_c * sp;
   const float Asp = (MODE == 0 || MODE == 3) ? As * LOG2E : (MODE == 1 ? sp : Es);   // what the polynomial is scaled by
   const float xs = 1.2011224087864498f * s;                 // s sqrt(log2 e)
   r.q0.x = ((float)(2 * qlo) + 0.5f - c_los) * xs;
@@ -101,7 +112,7 @@ __device__ __forceinline__ SeriesRecord make_series_record(float e_c, float a_c,
   if (MODE == 2) {
     r.q0.z = 0.0f;
     r.q2 = make_float4(0.0f, 0.0f, 0.0f, 1.0f);
-    r.q3.x = tau_d * S_d;
+    r.q3.x = wn * tau_d * S_d;
     r.q3.y = 1.0f;
   } else if (MODE == 1) {
     const float td_e = fminf(tau_d, kMaxTauDCell);
@@ -360,7 +371,9 @@ transfer_series_kernel(MarchConsts mc, const float* __restrict__ coef, int64_t n
   for (int z0 = 0; z0 < nz; z0 += LPP) {
     // ---- phase A: one record per lane
     {
-      const SeriesRecord r = make_series_record<DUST, DEG, MODE>(l_e, l_a, l_c, l_s, l_td, l_sd, mc.T_bg, npts, mc.fine_m);
+      float wn = 1.0f;
+      if (MODE == 2 && mc.ray_simpson) wn = ray_simpson_weight(z0 + ja, nz);
+      const SeriesRecord r = make_series_record<DUST, DEG, MODE>(l_e, l_a, l_c, l_s, l_td, l_sd, mc.T_bg, npts, mc.fine_m, wn);
       chunk_busy = __any_sync(0xffffffffu, ((unsigned)__float_as_int(r.q0.w) >> 16) != 0u);   // also: phase B is done
       rec[lane] = r.q0;
       rec[32 + lane] = r.q1;

@@ -21,7 +21,7 @@ MODES = {"thin_formal": (2, 0, 0), "thin_smooth": (2, 1, 0), "selthin_formal": (
          "thick_smooth_sub1": (0, 1, 1), "thick_smooth_sub7": (0, 1, 7),
          "thin_formal_dense": (2, 0, 0), "selthin_formal_dense": (1, 0, 0),
          "thick_formal_sub1_dense": (0, 0, 1), "thick_formal_sub3_dense": (0, 0, 3),
-         "thick_smooth_dense": (0, 1, 0), "thick_smooth_sub1_dense": (0, 1, 1)}
+         "thick_smooth_dense": (0, 1, 0), "thick_smooth_sub1_dense": (0, 1, 1), "thin_smooth_dense": (2, 1, 0)}
 
 
 def dev(a):
@@ -44,6 +44,8 @@ def expected_kernel(cfg, dense):
     narrow = cfg.microturb_cms > 0 and cfg.dv_cms <= 0.55 * cfg.microturb_cms
     if not dense:
         if i == 0 and ((s == 0 and m in (1, 2) and narrow) or (m == 0 and s > 0)):
+            return "transfer_series_kernel"
+        if i == 1 and m == 2 and narrow:                       # Simpson's rule along the ray: a weighted thin sum
             return "transfer_series_kernel"
         if i == 1 and m == 0 and cfg.nz >= 2 and (s > 0 or narrow):
             return "transfer_smooth_window_kernel"
@@ -157,12 +159,12 @@ def test_modes_kernel_selection_and_fallbacks():
         names[mode] = IrisSO(with_mode(cfg, mode)).transfer_kernel()
     assert names == {"thin_formal": "transfer_series_kernel", "selthin_formal": "transfer_series_kernel",
                      "thick_formal_sub1": "transfer_series_kernel", "thick_formal_sub3": "transfer_series_kernel",
-                     "thick_smooth": "transfer_smooth_window_kernel", "thin_smooth": "transfer_modes_kernel"}
+                     "thick_smooth": "transfer_smooth_window_kernel", "thin_smooth": "transfer_series_kernel"}
     # wide channels: 1 km/s against xi = 1 km/s
     wide = cfg.with_(dv_cms=1.0 * KMS, v0_cms=-31.5 * KMS)
     f = make_fields(wide, r)
     f["vlos"] = (0.2 * f["vlos"]).astype(np.float32)
-    for mode in ("thin_formal", "selthin_formal"):
+    for mode in ("thin_formal", "selthin_formal", "thin_smooth"):
         c = with_mode(wide, mode)
         assert IrisSO(c).transfer_kernel() == "transfer_modes_kernel"
         assert_spectra(gpu_cube(c, f), Oracle(c).observe(f), what=mode + " wide channels")
