@@ -183,6 +183,27 @@ def test_modes_kernel_selection_and_fallbacks():
         assert_spectra(gpu_cube(c, fb, expect_kernel=False), Oracle(c).observe(fb), what=mode + " 4000 channels")
 
 
+@pytest.mark.parametrize("mode", ["thick_smooth_sub1", "thick_smooth", "thick_formal_sub1", "thin_smooth"])
+def test_window_kernels_agree_with_the_dense_kernel_on_every_pixel_of_medium(mode):
+    """The sampled-column tests above compare 24 columns of the medium cube with the oracle; here EVERY pixel of the cube
+    from the line-window kernel of a mode is compared with the dense modes kernel (itself checked against the oracle),
+    at half the parity tolerance."""
+    from paper_2607_01338_b200 import IrisSO
+    cfg, r = make_workload("medium")
+    cfg = with_mode(cfg, mode)
+    f = make_fields(cfg, r)
+    d = dev_fields(f)
+    it = IrisSO(cfg)
+    assert it.transfer_kernel() != "transfer_modes_kernel"
+    win = it.observe(*d, beam=False, noise=False)
+    assert not it.smooth_fallback()
+    dense = IrisSO(cfg, transfer_algo=1).observe(*d, beam=False, noise=False)
+    peak = dense.abs().amax(dim=-1, keepdim=True)
+    excess = ((win - dense).abs() / (0.5e-4 * peak + 0.5e-6)).max().item()
+    print("%s: window against dense kernel on all %d pixels: worst at %.3g of half the tolerance" % (mode, cfg.nx * cfg.ny, excess))
+    assert excess <= 1.0
+
+
 def test_smooth_window_hands_over_when_a_relu_fires_outside_the_windows():
     """opaque_dust_clamp makes the smooth continuum overshoot below zero (the ReLU clamps every spectral point, also
     those no line window covers): the window kernel must notice, and the dense kernel, gated on its flag, must
