@@ -203,8 +203,8 @@ const char *iris_so_transfer_kernel(const iris_so_ctx *ctx);
 /* The optically thick mode with the smooth integrator (integration = 1; trapezoidal + BDF2 steps with the ReLU of
  * PAPER.md:709) is marched over line windows; the march is exact unless a ReLU fires outside the windows, which the
  * kernel detects: the dense kernel, launched right after it and gated on a device flag, then recomputes the cube.
- * *fell_back = 1 if that happened in the last transfer / observe call of this context, 0 if not (also 0 for every other
- * mode).  Synchronises the stream. */
+ * *fell_back = 1 if that happened in the last transfer / observe call of this context (for iris_so_observe_host: in the
+ * last slab of pixel rows it processed), 0 if not (also 0 for every other mode).  Synchronises the stream. */
 iris_so_status iris_so_smooth_fallback(iris_so_ctx *ctx, int32_t *fell_back, void *cuda_stream);
 
 /* Stand-alone post-processing stages (also used inside iris_so_observe). */
