@@ -375,7 +375,8 @@ def test_full_size_large_sampled():
 
 # ------------------------------------------------------------------------------------------------
 # host-buffer path (iris_so_observe_host): single shot and slab-pipelined, identical to the device path
-@pytest.mark.parametrize("case", ["one_shot", "slabs_plain", "slabs_beam_noise", "slabs_ragged_pageable"])
+@pytest.mark.parametrize("case", ["one_shot", "slabs_plain", "slabs_beam_noise", "slabs_ragged_pageable",
+                                  "slabs_production_mode"])
 def test_observe_host_equals_device_path(case):
     """The slab pipeline (H2D of slab k+1 | K1-K5 of slab k | D2H of slab k-1) must give the cube of the device path
     bit for bit: the kernels are the same and every pixel column is independent before the beam."""
@@ -387,6 +388,8 @@ def test_observe_host_equals_device_path(case):
         cfg, r = make_workload("small", nx=256, ny=80, nz=512, nv=96)       # 2 MB of fields per row, 168 MB in all: slabs of 14 rows, the last one ragged
     if case == "slabs_beam_noise":
         cfg = cfg.with_(beam_fwhm_px=3.0, noise_sigma=0.25, seed=11)
+    if case == "slabs_production_mode":      # smooth integrator on the fine grid: window kernel + gated dense kernel per slab
+        cfg = cfg.with_(transfer_mode=0, integration=1, subsample=1, beam_fwhm_px=3.0)
     f = make_fields(cfg, r)
     it = iris(cfg)
     ref = it.observe(*dev_fields(f)).cpu()
