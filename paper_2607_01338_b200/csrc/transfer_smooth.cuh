@@ -33,6 +33,7 @@
 #pragma once
 #include "transfer_common.cuh"
 #include "transfer_window.cuh"
+#include "transfer_series.cuh"       // packed f32x2 helpers
 
 namespace iris {
 
@@ -168,18 +169,39 @@ transfer_smooth_window_kernel(MarchConsts mc, const float* __restrict__ coef, in
           u_min = fminf(u_min, U);
         }
       } else {
-        // BDF2: D_n = [2 p (e_c - a_c C_n) + 4 U d_n-1 - V d_n-2] / (3 + 2 tau_d + 2 a_c p)
-        const float g2 = 2.0f * fmaf(-a_c, C_unc, e_c), a2 = 2.0f * a_c, den0 = fmaf(2.0f, td, 3.0f);
-        const float c4 = 4.0f * d_c, cm = -d_m;
-        int w = IDX(elo + i);
-        // consecutive points of a lane are LPP apart: one row (32 words) further
-        for (int k = elo + i; k <= ehi; k += LPP, xs += xstep, w += 32) {
-          const float pw = prof.at(xs);
-          const float lin = fmaf(cur[w], c4, prv[w] * cm);
-          const float Du = fmaf(pw, g2, lin) * rcp_approx(fmaf(pw, a2, den0));
-          const float U = fmaxf(Du + relu_add, relu_min) * inv_dn;              // ReLU on D + C and on C
-          prv[w] = U;
-          u_min = fminf(u_min, U);
+        // BDF2: D_n = [2 p (e_c - a_c C_n) + 4 U d_n-1 - V d_n-2] / (3 + 2 tau_d + 2 a_c p), on even-aligned PAIRS of
+        // points with packed arithmetic (fma / mul / add.rn.f32x2): a lane takes points k, k + 1, the LPP lanes of a
+        // pixel 2 LPP consecutive points (two rows of its spectra) per pass.  A pair may reach one point beyond the
+        // window on either side; the step is as valid there.
+        const f32x2 g2 = pk1(2.0f * fmaf(-a_c, C_unc, e_c)), a2 = pk1(2.0f * a_c), den0 = pk1(fmaf(2.0f, td, 3.0f));
+        const f32x2 c4 = pk1(4.0f * d_c), cm = pk1(-d_m), radd = pk1(relu_add), idn = pk1(inv_dn), pp0 = pk1(prof.p0);
+        const f32x2 pp1 = pk1(prof.p1), pp2 = pk1(prof.p2), pp3 = pk1(prof.p3), pp4 = pk1(prof.p4);
+        const int k0 = (elo & ~1) + 2 * i;
+        const float xa = ((float)k0 + 0.5f - c_los) * (s * SQL2E), xb = s * SQL2E;
+        f32x2 xx = pk(xa, xa + xb);
+        const f32x2 xstep2 = pk1(2.0f * (float)LPP * xb);
+        for (int k = k0; k <= ehi; k += 2 * LPP, xx = add2(xx, xstep2)) {
+          const int w = IDX(k);
+          const f32x2 u = mul2(xx, xx);
+          float u0, u1;
+          upk(u, u0, u1);
+          f32x2 pw = pk(ex2_approx(-u0), ex2_approx(-u1));
+          if (POINT) pw = mul2(pw, pp0);
+          else pw = mul2(pw, fma2(fma2(fma2(fma2(pp4, u, pp3), u, pp2), u, pp1), u, pp0));
+          const float2 Uo = *reinterpret_cast<const float2*>(cur + w), Vo = *reinterpret_cast<const float2*>(prv + w);
+          const f32x2 lin = fma2(pk(Uo.x, Uo.y), c4, mul2(pk(Vo.x, Vo.y), cm));
+          const f32x2 den = fma2(pw, a2, den0);
+          float e0, e1;
+          upk(den, e0, e1);
+          const f32x2 Du = add2(mul2(fma2(pw, g2, lin), pk(rcp_approx(e0), rcp_approx(e1))), radd);
+          float D0, D1;
+          upk(Du, D0, D1);
+          const f32x2 U = mul2(pk(fmaxf(D0, relu_min), fmaxf(D1, relu_min)), idn);      // ReLU on D + C and on C
+          float2 Un;
+          upk(U, Un.x, Un.y);
+          if (k + 1 >= npts) Un.y = 0.0f;                                               // padding, not a point
+          *reinterpret_cast<float2*>(prv + w) = Un;
+          u_min = fminf(u_min, fminf(Un.x, Un.y));
         }
       }
     }
