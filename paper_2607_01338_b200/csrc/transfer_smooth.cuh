@@ -102,7 +102,8 @@ transfer_smooth_window_kernel(MarchConsts mc, const float* __restrict__ coef, in
   float C = mc.T_bg, Cm = mc.T_bg;          // continuum at n - 1 and n - 2 (after the ReLU)
   float d_c = 1.0f, d_m = 1.0f;             // dominant homogeneous solution at n - 1 and n - 2
   float u_min = 0.0f;                       // most negative U this lane has stored
-  int ring_lo = 0x7fffffff, ring_hi = -1;   // window of the cell this lane remembers (cell n with n % K == i)
+  unsigned ring = 0u;                       // window of the cell this lane remembers (cell n with n % K == i)
+  int slot = 0;                             // n % K
   bool risk = false;
   // cell 0, for the trapezoidal step
   float e_0 = 0.0f, a_0 = 0.0f, c_0 = 0.0f, s_0 = 1.0f, td_0 = 0.0f, Jd_0 = 0.0f;
@@ -121,13 +122,15 @@ transfer_smooth_window_kernel(MarchConsts mc, const float* __restrict__ coef, in
     // ---- window of this cell, remembered for LPP cells; the points to update are the union of what is remembered
     int klo, khi;
     const int W = line_window(e_c, a_c, c_los, s, npts, klo, khi);
-    if (i == (n % kSmoothKeep)) { ring_lo = W > 0 ? klo : 0x7fffffff; ring_hi = W > 0 ? khi : -1; }
-    int elo = ring_lo, ehi = ring_hi;
+    // (remembered as one word, hi in the upper and 0xffff - lo in the lower half: the union of the LPP windows is a
+    // halfword maximum, __vmaxu2, per exchange; an empty window is 0)
+    if (i == slot) ring = W > 0 ? (((unsigned)khi << 16) | (0xffffu - (unsigned)klo)) : 0u;
+    slot = slot + 1 == kSmoothKeep ? 0 : slot + 1;
+    unsigned un = ring;
 #pragma unroll
-    for (int o = LPP / 2; o > 0; o >>= 1) {
-      elo = min(elo, __shfl_xor_sync(gmask, elo, o));
-      ehi = max(ehi, __shfl_xor_sync(gmask, ehi, o));
-    }
+    for (int o = LPP / 2; o > 0; o >>= 1) un = __vmaxu2(un, __shfl_xor_sync(gmask, un, o));
+    // no window at all: lo = 0xffff, hi = 0 (ehi < elo)
+    const int elo = 0xffff - (int)(un & 0xffffu), ehi = (int)(un >> 16);
     if (n == 0) {                                               // D_0 = 0, C_0 = T_bg: nothing moves yet
       e_0 = e_c; a_0 = a_c; c_0 = c_los; s_0 = s; td_0 = td; Jd_0 = Jd;
       continue;
