@@ -201,10 +201,13 @@ iris_so_status iris_so_transfer_work(iris_so_ctx *ctx, uint64_t *window_updates,
 const char *iris_so_transfer_kernel(const iris_so_ctx *ctx);
 
 /* The optically thick mode with the smooth integrator (integration = 1; trapezoidal + BDF2 steps with the ReLU of
- * PAPER.md:709) is marched over line windows; the march is exact unless a ReLU fires outside the windows, which the
- * kernel detects: the dense kernel, launched right after it and gated on a device flag, then recomputes the cube.
- * *fell_back = 1 if that happened in the last transfer / observe call of this context (for iris_so_observe_host: in the
- * last slab of pixel rows it processed), 0 if not (also 0 for every other mode).  Synchronises the stream. */
+ * PAPER.md:709) is marched over line windows; the march of a pixel is exact unless a ReLU fires outside its windows or
+ * the dust is so opaque per cell (a sustained tau_d above ~0.1) that a point the windows have left has not yet settled
+ * on the dominant solution of the homogeneous BDF2 step (Eq. 4.8.10), both of which the kernel detects per
+ * pixel: it lists the pixel, and the dense kernel, launched right after it and driven by that list, recomputes the
+ * listed pixels.  *fell_back = the number of pixels that were handed over in the last transfer / observe call of this
+ * context (for iris_so_observe_host: summed over the slabs of pixel rows of that call); 0 for every other mode.
+ * Synchronises the stream. */
 iris_so_status iris_so_smooth_fallback(iris_so_ctx *ctx, int32_t *fell_back, void *cuda_stream);
 
 /* Stand-alone post-processing stages (also used inside iris_so_observe). */

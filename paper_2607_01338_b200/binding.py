@@ -234,10 +234,10 @@ class IrisSO:
         return int(n.value)
 
     def smooth_fallback(self):
-        """True if the last smooth-integrator call of this context handed over to the dense kernel."""
+        """Number of pixels the last smooth-integrator call of this context handed over to the dense kernel."""
         n = C.c_int32()
         self._check(self.lib.iris_so_smooth_fallback(self._h, C.byref(n), self._stream()))
-        return bool(n.value)
+        return int(n.value)
 
     # -- entry points ----------------------------------------------------------------------------
     def levelpop(self, nH2, Tgas, pop=None):

@@ -65,7 +65,9 @@ struct iris_so_ctx {
   std::vector<ProfRec> recs;
   std::vector<cudaEvent_t> event_pool;
   unsigned long long* d_counter = nullptr;
-  int* d_gate = nullptr;          // flag raised by transfer_smooth_window_kernel when the dense kernel has to take over
+  int* d_gate = nullptr;          // [0] pixels transfer_smooth_window_kernel handed over to the dense kernel (zeroed per launch),
+                                  // [1] their number accumulated over the launches of one public call (slabs of the host path),
+                                  // [2 ..] the list of those pixels (npix entries)
   double* d_metrics = nullptr;
   cudaStream_t s_in = nullptr, s_out = nullptr;      // copy streams of the host-buffer path
   std::vector<cudaEvent_t> slab_events;
@@ -432,19 +434,19 @@ iris_so_status run_transfer(iris_so_ctx* ctx, const iris::MarchConsts& mc, float
     md.fine_m = ctx->cfg.subsample > 0 ? ctx->cfg.subsample + 1 : 0;
     md.nx = ctx->cfg.nx;
     md.gate = nullptr;
+    md.list = nullptr;
     if (windowed_smooth_mode(ctx->cfg)) {
-      if (!ctx->d_gate) {
-        cudaError_t e = cudaMalloc(reinterpret_cast<void**>(&ctx->d_gate), sizeof(int));
-        if (e != cudaSuccess) return cuda_fail(ctx, e, "cudaMalloc(gate)");
-      }
+      if (!ctx->d_gate) return fail(ctx, IRIS_SO_ECUDA, "gate flag not allocated");      // begin_call allocates it
       cudaError_t e = cudaMemsetAsync(ctx->d_gate, 0, sizeof(int), st);
       if (e != cudaSuccess) return cuda_fail(ctx, e, "cudaMemsetAsync(gate)");
       iris::MarchConsts mf = mc;
       mf.fine_m = md.fine_m;
-      e = iris::launch_transfer_smooth_window(mf, ctx->d_coef, ctx->ncell, npix, nz, nv, out, out_cont, ctx->d_gate, st);
+      e = iris::launch_transfer_smooth_window(mf, ctx->d_coef, ctx->ncell, npix, nz, nv, out, out_cont, ctx->d_gate,
+                                              ctx->d_gate + 2, st);
       ctx->launches++;
       if (e != cudaSuccess) return cuda_fail(ctx, e, "launch of transfer_smooth_window_kernel");
       md.gate = ctx->d_gate;
+      md.list = ctx->d_gate + 2;
     }
     cudaError_t e = iris::launch_transfer_modes(mc, md, ctx->d_coef, ctx->ncell, npix, nz, nv, out, out_cont, st);
     ctx->launches++;
@@ -469,6 +471,16 @@ iris_so_status run_transfer(iris_so_ctx* ctx, const iris::MarchConsts& mc, float
                       : iris::launch_transfer_window(mc, ctx->d_coef, ctx->ncell, npix, nz, nv, dust, ctx->sm_count, out, out_cont, st);
   ctx->launches++;
   if (e != cudaSuccess) return cuda_fail(ctx, e, "launch of the line-window transfer kernel");
+  return IRIS_SO_OK;
+}
+
+// Start of a public call that runs the transfer: clears the accumulated fallback flag of the smooth window kernel.
+iris_so_status begin_call(iris_so_ctx* ctx, cudaStream_t st) {
+  if (!windowed_smooth_mode(ctx->cfg)) return IRIS_SO_OK;
+  cudaError_t e;
+  if (!ctx->d_gate && (e = cudaMalloc(reinterpret_cast<void**>(&ctx->d_gate), (2 + (size_t)ctx->npix) * sizeof(int))) != cudaSuccess)
+    return cuda_fail(ctx, e, "cudaMalloc(gate)");
+  if ((e = cudaMemsetAsync(ctx->d_gate, 0, 2 * sizeof(int), st)) != cudaSuccess) return cuda_fail(ctx, e, "cudaMemsetAsync(gate)");
   return IRIS_SO_OK;
 }
 
@@ -646,8 +658,9 @@ iris_so_status iris_so_transfer(iris_so_ctx* ctx, const float* d_nH2, const floa
   if (!d_nH2 || !d_Tgas || !d_Tdust || !d_vlos) return fail(ctx, IRIS_SO_EINVAL, "iris_so_transfer: NULL field pointer");
   if (!d_I_total && !d_I_cont) return fail(ctx, IRIS_SO_EINVAL, "iris_so_transfer: no output requested");
   cudaStream_t st = static_cast<cudaStream_t>(stream);
-  iris_so_status s = run_coefficients(ctx, d_nH2, d_Tgas, d_Tdust, d_vlos, d_pop, st);
+  iris_so_status s = begin_call(ctx, st);
   if (s != IRIS_SO_OK) return s;
+  if ((s = run_coefficients(ctx, d_nH2, d_Tgas, d_Tdust, d_vlos, d_pop, st)) != IRIS_SO_OK) return s;
   iris::MarchConsts mc = ctx->mc;
   mc.out_mode = iris::OUT_I_TOT;
   return run_transfer(ctx, mc, d_I_total, d_I_cont, st);
@@ -658,8 +671,9 @@ iris_so_status iris_so_observe_stages(iris_so_ctx* ctx, const float* d_nH2, cons
   if (!ctx) return IRIS_SO_EINVAL;
   if (!d_nH2 || !d_Tgas || !d_Tdust || !d_vlos || !d_cube) return fail(ctx, IRIS_SO_EINVAL, "iris_so_observe: NULL pointer");
   cudaStream_t st = static_cast<cudaStream_t>(stream);
-  iris_so_status s = run_coefficients(ctx, d_nH2, d_Tgas, d_Tdust, d_vlos, nullptr, st);
+  iris_so_status s = begin_call(ctx, st);
   if (s != IRIS_SO_OK) return s;
+  if ((s = run_coefficients(ctx, d_nH2, d_Tgas, d_Tdust, d_vlos, nullptr, st)) != IRIS_SO_OK) return s;
   if ((s = run_transfer(ctx, ctx->mc, d_cube, nullptr, st)) != IRIS_SO_OK) return s;
   const bool beam = (stage_mask & 1) && ctx->cfg.beam_fwhm_px > 0.0;
   const bool noise = (stage_mask & 2) && ctx->nc.on;
@@ -708,6 +722,7 @@ iris_so_status iris_so_observe_host(iris_so_ctx* ctx, const float* h_nH2, const 
     return IRIS_SO_OK;
   }
   if ((s = ensure(ctx, &ctx->d_coef, sizeof(float) * 6 * (size_t)ncell0, "cudaMalloc(coefficient planes)")) != IRIS_SO_OK) return s;
+  if ((s = begin_call(ctx, st)) != IRIS_SO_OK) return s;
   if (!ctx->s_in) {
     if ((e = cudaStreamCreateWithFlags(&ctx->s_in, cudaStreamNonBlocking)) != cudaSuccess) return cuda_fail(ctx, e, "cudaStreamCreate");
     if ((e = cudaStreamCreateWithFlags(&ctx->s_out, cudaStreamNonBlocking)) != cudaSuccess) return cuda_fail(ctx, e, "cudaStreamCreate");
@@ -816,9 +831,9 @@ iris_so_status iris_so_smooth_fallback(iris_so_ctx* ctx, int32_t* fell_back, voi
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   int h = 0;
   cudaError_t e;
-  if ((e = cudaMemcpyAsync(&h, ctx->d_gate, sizeof h, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(ctx, e, "D2H");
+  if ((e = cudaMemcpyAsync(&h, ctx->d_gate + 1, sizeof h, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(ctx, e, "D2H");
   if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(ctx, e, "cudaStreamSynchronize");
-  *fell_back = h != 0;
+  *fell_back = h;
   return IRIS_SO_OK;
 }
 

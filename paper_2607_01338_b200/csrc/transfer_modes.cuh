@@ -36,7 +36,9 @@ struct ModeConsts {
   int mode, smooth;      // transfer mode 0 / 1 / 2, integration 0 / 1
   int fine_m;            // 0: channel-integrated profile; else fine intervals per channel (f + 1, even)
   int nx;                // pixels per image row (npix = nx * rows)
-  const int* gate;       // nullptr, or a device flag: the kernel returns at once while it is 0 (transfer_smooth.cuh)
+  const int* gate;       // nullptr, or the device counter of the pixels transfer_smooth_window_kernel handed over
+                         // (transfer_smooth.cuh): the kernel then recomputes those pixels only (none: it returns at once)
+  const int* list;       // their pixel indices, gate[0] of them
 };
 
 // w(t) = (1 - exp(-t)) / t, w(0) = 1
@@ -55,14 +57,19 @@ template <int MODE, bool SMOOTH, int PROF>
 __global__ void __launch_bounds__(128)
 transfer_modes_kernel(MarchConsts mc, ModeConsts md, const float* __restrict__ coef, int64_t ncell, int npix, int nz,
                       int nv, float* __restrict__ out, float* __restrict__ out_cont) {
-  if (md.gate != nullptr && *md.gate == 0) return;
   constexpr int NPT = PROF == 0 ? kModesCh0 : (PROF == 1 ? 9 : (PROF == 3 ? 17 : 3));
   // a warp takes a tile of 8 x 4 pixels: whole 32-byte sectors of every plane, and a quarter of the spread in
   // line-of-sight velocity that 32 pixels along x have (the dust-only path is taken when NO pixel of the warp is near
   // the line, and rotation shifts the line by several channels per pixel along x)
   const int tiles_x = (md.nx + 7) >> 3;
   const int px = (blockIdx.x % tiles_x) * 8 + (threadIdx.x & 7), py = (blockIdx.x / tiles_x) * 4 + (threadIdx.x >> 3);
-  const int pix = px < md.nx ? py * md.nx + px : npix;
+  int pix = px < md.nx ? py * md.nx + px : npix;
+  if (md.gate != nullptr) {
+    // hand-over launch: thread slot -> entry of the list of flagged pixels (the grid is sized for all pixels; the blocks
+    // beyond the list return at once)
+    const int slot = blockIdx.x * 32 + threadIdx.x;
+    pix = slot < *md.gate ? md.list[slot] : npix;
+  }
   const int blk = blockIdx.y * blockDim.y + threadIdx.y;      // channel block of this thread
   const int m = md.fine_m;
   const int cpb = PROF == 0 ? kModesCh0 : (PROF == 3 ? 8 : (PROF == 1 ? 8 / m : 1));    // channels per thread
@@ -297,7 +304,7 @@ inline cudaError_t launch_transfer_modes_t(const MarchConsts& mc, const ModeCons
   const int cpb = prof == 0 ? kModesCh0 : (prof == 3 ? 8 : (prof == 1 ? 8 / m : 1));
   const int nblk = (nv + cpb - 1) / cpb;
   const int rows = npix / md.nx;
-  dim3 block(32, 4), grid(((md.nx + 7) / 8) * ((rows + 3) / 4), (nblk + 3) / 4);
+  dim3 block(32, 4), grid(md.gate != nullptr ? (npix + 31) / 32 : ((md.nx + 7) / 8) * ((rows + 3) / 4), (nblk + 3) / 4);
   if (prof == 0) transfer_modes_kernel<MODE, SMOOTH, 0><<<grid, block, 0, st>>>(mc, md, coef, ncell, npix, nz, nv, out, out_cont);
   else if (prof == 1) transfer_modes_kernel<MODE, SMOOTH, 1><<<grid, block, 0, st>>>(mc, md, coef, ncell, npix, nz, nv, out, out_cont);
   else if (prof == 3) transfer_modes_kernel<MODE, SMOOTH, 3><<<grid, block, 0, st>>>(mc, md, coef, ncell, npix, nz, nv, out, out_cont);

@@ -19,8 +19,17 @@
 // What the window cannot see is a ReLU that fires OUTSIDE it: a far point a d_n + C_n < 0, or the continuum itself
 // clamped (C_n < 0 before the ReLU), or the dominant solution losing its sign (4 d_n-1 < d_n-2: a cell that turns
 // opaque abruptly).  Each lane keeps the most negative U it has stored and tests these three conditions per cell; if
-// one holds anywhere, the kernel raises *gate and the caller's next launch, transfer_modes_kernel gated on that
-// flag, recomputes the cube densely (exact in every case; the gate stays 0 for the paper's workloads).
+// one holds for a pixel, the kernel appends the pixel to a list (gate[0] counts its entries) and the caller's next
+// launch, transfer_modes_kernel driven by that list, recomputes those pixels densely (exact in every case; the list
+// stays empty or short for the paper's workloads).
+//
+// Fourth condition: "a factor ~3 per cell" holds for tau_d << 1 only.  The roots of the homogeneous step are
+// [2 +- sqrt(1 - 2 tau_d)] / (3 + 2 tau_d): the recessive solution loses rho(tau_d) = [2 - sqrt(1 - 2 tau_d)] /
+// [2 + sqrt(1 - 2 tau_d)] per cell against the dominant one (1/3 at tau_d = 0, 0.44 at 0.2, 0.63 at 0.4, 1 at 0.5; beyond
+// 0.5 the roots are complex and there is no dominant solution at all).  A point released K cells ago is a d_n to the
+// PRODUCT of rho over those K cells, so the kernel keeps rho of the last K cells (lane i remembers cell n = i mod K,
+// like the windows) and hands over when their product exceeds kSmoothReleaseTol (3^-12 = 1.9e-6 without dust; the
+// budget is reached at a sustained tau_d of 0.1 per cell).
 //
 // (The selectively thin mode is NOT run this way: its absorption saturates at I^[T] = 0, i.e. the ReLU keeps acting on
 // points long after the line has left them, and the gate fires on every thick workload; measured: 3.5 + 5.8 ms against
@@ -39,6 +48,7 @@ namespace iris {
 
 constexpr int kSmoothLPP = 16;          // lanes per pixel
 constexpr int kSmoothKeep = 12;         // cells a window stays active (K <= kSmoothLPP: lane i remembers cell n = i mod K)
+constexpr float kSmoothReleaseTol = 1.0e-5f;   // largest recessive / dominant ratio a released point may carry
 
 // profile weight ("erf-difference" units) of a point at x Doppler widths from the line centre, as a function of
 // u = x^2 log2(e): (2 s / sqrt(pi)) 2^-u P(u); P = 1 for the point profile, the degree-4 polynomial of the channel
@@ -76,7 +86,7 @@ template <bool POINT>
 __global__ void __launch_bounds__(128)
 transfer_smooth_window_kernel(MarchConsts mc, const float* __restrict__ coef, int64_t ncell, int npix, int nz, int nv,
                               int nvp /* padded points per spectrum */, float* __restrict__ out,
-                              float* __restrict__ out_cont, int* __restrict__ gate) {
+                              float* __restrict__ out_cont, int* __restrict__ gate, int* __restrict__ gate_list) {
   extern __shared__ float sm[];
   constexpr int LPP = kSmoothLPP, PPW = 32 / LPP;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, wpc = blockDim.x >> 5;
@@ -103,6 +113,7 @@ transfer_smooth_window_kernel(MarchConsts mc, const float* __restrict__ coef, in
   float d_c = 1.0f, d_m = 1.0f;             // dominant homogeneous solution at n - 1 and n - 2
   float u_min = 0.0f;                       // most negative U this lane has stored
   unsigned ring = 0u;                       // window of the cell this lane remembers (cell n with n % K == i)
+  float rho_ring = i < kSmoothKeep ? (1.0f / 3.0f) : 1.0f;   // rho of that cell (lanes K .. LPP - 1 remember nothing)
   int slot = 0;                             // n % K
   bool risk = false;
   // cell 0, for the trapezoidal step
@@ -124,11 +135,20 @@ transfer_smooth_window_kernel(MarchConsts mc, const float* __restrict__ coef, in
     const int W = line_window(e_c, a_c, c_los, s, npts, klo, khi);
     // (remembered as one word, hi in the upper and 0xffff - lo in the lower half: the union of the LPP windows is a
     // halfword maximum, __vmaxu2, per exchange; an empty window is 0)
-    if (i == slot) ring = W > 0 ? (((unsigned)khi << 16) | (0xffffu - (unsigned)klo)) : 0u;
+    if (i == slot) {
+      ring = W > 0 ? (((unsigned)khi << 16) | (0xffffu - (unsigned)klo)) : 0u;
+      const float sq = sqrtf(fmaxf(fmaf(-2.0f, td, 1.0f), 0.0f));
+      rho_ring = __fdividef(2.0f - sq, 2.0f + sq);
+    }
     slot = slot + 1 == kSmoothKeep ? 0 : slot + 1;
     unsigned un = ring;
+    float rho_prod = rho_ring;
 #pragma unroll
-    for (int o = LPP / 2; o > 0; o >>= 1) un = __vmaxu2(un, __shfl_xor_sync(gmask, un, o));
+    for (int o = LPP / 2; o > 0; o >>= 1) {
+      un = __vmaxu2(un, __shfl_xor_sync(gmask, un, o));
+      rho_prod *= __shfl_xor_sync(gmask, rho_prod, o);
+    }
+    if (rho_prod > kSmoothReleaseTol) risk = true;              // released points would not be a d_n any more
     // no window at all: lo = 0xffff, hi = 0 (ehi < elo)
     const int elo = 0xffff - (int)(un & 0xffffu), ehi = (int)(un >> 16);
     if (n == 0) {                                               // D_0 = 0, C_0 = T_bg: nothing moves yet
@@ -224,7 +244,9 @@ transfer_smooth_window_kernel(MarchConsts mc, const float* __restrict__ coef, in
     }
   }
   __syncwarp();
-  if (__any_sync(0xffffffffu, risk && valid) && lane == 0) atomicExch(gate, 1);
+  // hand the pixel over: gate[0] = pixels listed by this launch, gate[1] = pixels handed over since the public call began
+  const bool group_risk = (__ballot_sync(0xffffffffu, risk && valid) & gmask) != 0u;
+  if (group_risk && i == 0) { gate_list[atomicAdd(gate, 1)] = pix; atomicAdd(gate + 1, 1); }
 
   if (valid) {
     // the points are D = U d; nz = 1 leaves D = 0
@@ -254,7 +276,8 @@ inline size_t smooth_window_smem_per_warp(int nv, int fine_m) {
 }
 
 inline cudaError_t launch_transfer_smooth_window(const MarchConsts& mc, const float* coef, int64_t ncell, int npix, int nz,
-                                                 int nv, float* out, float* out_cont, int* gate, cudaStream_t st) {
+                                                 int nv, float* out, float* out_cont, int* gate, int* gate_list,
+                                                 cudaStream_t st) {
   const int npts = mc.fine_m > 0 ? nv * mc.fine_m + 1 : nv;
   const int nvp = (npts + kSmoothLPP - 1) / kSmoothLPP * kSmoothLPP;
   const size_t per_warp = smooth_window_smem_per_warp(nv, mc.fine_m);
@@ -272,11 +295,11 @@ inline cudaError_t launch_transfer_smooth_window(const MarchConsts& mc, const fl
   if (mc.fine_m > 0) {
     e = cudaFuncSetAttribute(transfer_smooth_window_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    transfer_smooth_window_kernel<true><<<grid, wpc * 32, smem, st>>>(mc, coef, ncell, npix, nz, nv, nvp, out, out_cont, gate);
+    transfer_smooth_window_kernel<true><<<grid, wpc * 32, smem, st>>>(mc, coef, ncell, npix, nz, nv, nvp, out, out_cont, gate, gate_list);
   } else {
     e = cudaFuncSetAttribute(transfer_smooth_window_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    transfer_smooth_window_kernel<false><<<grid, wpc * 32, smem, st>>>(mc, coef, ncell, npix, nz, nv, nvp, out, out_cont, gate);
+    transfer_smooth_window_kernel<false><<<grid, wpc * 32, smem, st>>>(mc, coef, ncell, npix, nz, nv, nvp, out, out_cont, gate, gate_list);
   }
   return cudaGetLastError();
 }

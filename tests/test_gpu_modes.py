@@ -196,7 +196,9 @@ def test_window_kernels_agree_with_the_dense_kernel_on_every_pixel_of_medium(mod
     it = IrisSO(cfg)
     assert it.transfer_kernel() != "transfer_modes_kernel"
     win = it.observe(*d, beam=False, noise=False)
-    assert not it.smooth_fallback()
+    # the window march of the smooth integrator hands a pixel over where a few very dense cells in a row make the dust
+    # opaque per cell (n_H2 is lognormal with sigma_ln = 2): a handful of the 65536 pixels
+    assert it.smooth_fallback() <= (cfg.nx * cfg.ny) // 200
     dense = IrisSO(cfg, transfer_algo=1).observe(*d, beam=False, noise=False)
     peak = dense.abs().amax(dim=-1, keepdim=True)
     excess = ((win - dense).abs() / (0.5e-4 * peak + 0.5e-6)).max().item()
@@ -225,12 +227,46 @@ def test_smooth_window_hands_over_when_a_relu_fires_outside_the_windows():
         f["nH2"][c.nz // 2:] *= 30.0
         it2 = IrisSO(c2)
         cube2 = it2.observe(*dev_fields(f)).cpu().numpy()
-        assert it2.smooth_fallback()
+        assert it2.smooth_fallback() > 0
         ref2 = Oracle(c2).observe(f)
         ref_tot = Oracle(c2.with_(subtract_continuum=False)).observe(f)
         assert_spectra(cube2, ref2, extra=3e-7 * np.abs(ref_tot).max(axis=-1, keepdims=True), what=mode + " clamped")
         # every other mode reports 0
         assert not IrisSO(with_mode(cfg, "thin_smooth")).smooth_fallback()
+
+
+@pytest.mark.parametrize("mode", ["thick_smooth", "thick_smooth_sub1", "thick_smooth_dense", "thick_smooth_sub1_dense"])
+@pytest.mark.parametrize("tau_d", [0.05, 0.2, 0.3, 0.4, 0.45, 0.6])
+def test_smooth_window_behind_sustained_moderate_dust(mode, tau_d):
+    """A line 17 or more cells from the observer behind uniform dust of tau_d per cell (Eq. 4.8.10: the
+    homogeneous BDF2 step has roots [2 +- sqrt(1 - 2 tau_d)] / (3 + 2 tau_d); the recessive solution dies as 3^-n only for
+    tau_d << 1, and beyond tau_d = 0.5 the roots are complex).  The window kernel freezes a point 12 cells after the
+    last line has touched it, which is exact only while the product of the root ratios over those cells is small: at
+    tau_d >= 0.2 it must hand over to the dense kernel (flag up), at 0.05 it must not, and the cube must match the
+    oracle either way.  The "_dense" twins are the control."""
+    from paper_2607_01338_b200 import IrisSO
+    n_far, n_near = 8, 16
+    cfg, r = make_workload("small", nx=24, ny=6, nz=n_far + n_near, nv=96)
+    cfg = with_mode(cfg, mode)
+    f = make_fields(cfg, r)
+    f["vlos"] = (0.25 * f["vlos"]).astype(np.float32)
+    n_slab = 1.0e4
+    cfg = cfg.with_(kappa_gas_cm2_g=tau_d / (cfg.mass_per_H2_g * n_slab * cfg.cell_cm))
+    # the near slab: uniform density, no line inside the band (its velocity is far outside), dust of tau_d per cell
+    f["nH2"][n_far:] = n_slab
+    f["vlos"][n_far:] = 4.0e7
+    f["Tdust"][n_far:] = 25.0
+    dense = mode.endswith("_dense")
+    it = IrisSO(cfg, transfer_algo=1 if dense else 0)
+    assert it.transfer_kernel() == expected_kernel(cfg, dense)
+    cube = it.observe(*dev_fields(f)).cpu().numpy()
+    if not dense:
+        # every pixel sees the slab: all of them are handed over from tau_d = 0.2 on, none at 0.05
+        assert it.smooth_fallback() == (cfg.nx * cfg.ny if tau_d >= 0.2 else 0), "pixels handed over at tau_d = %g" % tau_d
+    ref = Oracle(cfg).observe(f)
+    assert np.abs(ref).max() > 30e-6                      # the attenuated line is still far above the 1e-6 K floor
+    worst = assert_spectra(cube, ref, what="%s tau_d=%g" % (mode, tau_d))
+    print("%s behind %d cells of tau_d = %g: worst pixel at %.3g of tolerance, peak %.3g K" % (mode, n_near, tau_d, worst, np.abs(ref).max()))
 
 
 def test_modes_adjoint_is_refused_and_bad_modes_are_rejected():
@@ -257,7 +293,7 @@ def test_modes_full_size_medium_sampled(mode):
     it = IrisSO(cfg, transfer_algo=1 if mode.endswith("_dense") else 0)
     assert it.transfer_kernel() == expected_kernel(cfg, mode.endswith("_dense"))
     cube = it.observe(*dev_fields(f), beam=False, noise=False)
-    assert not it.smooth_fallback()          # the line-window march of the smooth integrator is exact on this workload
+    assert it.smooth_fallback() <= (cfg.nx * cfg.ny) // 200      # pixels handed over to the dense kernel: a handful
     n_cols = 24
     plane = cfg.nx * cfg.ny
     pix = np.sort(np.random.default_rng(21).choice(plane, size=n_cols, replace=False))

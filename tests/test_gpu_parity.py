@@ -376,7 +376,7 @@ def test_full_size_large_sampled():
 # ------------------------------------------------------------------------------------------------
 # host-buffer path (iris_so_observe_host): single shot and slab-pipelined, identical to the device path
 @pytest.mark.parametrize("case", ["one_shot", "slabs_plain", "slabs_beam_noise", "slabs_ragged_pageable",
-                                  "slabs_production_mode"])
+                                  "slabs_production_mode", "slabs_production_mode_handover_in_first_slab"])
 def test_observe_host_equals_device_path(case):
     """The slab pipeline (H2D of slab k+1 | K1-K5 of slab k | D2H of slab k-1) must give the cube of the device path
     bit for bit: the kernels are the same and every pixel column is independent before the beam."""
@@ -388,11 +388,16 @@ def test_observe_host_equals_device_path(case):
         cfg, r = make_workload("small", nx=256, ny=80, nz=512, nv=96)       # 2 MB of fields per row, 168 MB in all: slabs of 14 rows, the last one ragged
     if case == "slabs_beam_noise":
         cfg = cfg.with_(beam_fwhm_px=3.0, noise_sigma=0.25, seed=11)
-    if case == "slabs_production_mode":      # smooth integrator on the fine grid: window kernel + gated dense kernel per slab
+    if case.startswith("slabs_production_mode"):  # smooth integrator on the fine grid: window kernel + list-driven dense kernel per slab
         cfg = cfg.with_(transfer_mode=0, integration=1, subsample=1, beam_fwhm_px=3.0)
     f = make_fields(cfg, r)
+    if case.endswith("handover_in_first_slab"):   # opaque dust (tau_d ~ 0.3 per cell) in the first pixel rows only
+        f["nH2"][:, :10, :] = 0.3 / (cfg.kappa_gas_cm2_g * cfg.mass_per_H2_g * cfg.cell_cm)
     it = iris(cfg)
     ref = it.observe(*dev_fields(f)).cpu()
+    handed_over = it.smooth_fallback()
+    if case.endswith("handover_in_first_slab"):
+        assert 10 * cfg.nx <= handed_over < 14 * cfg.nx
     pin = case != "slabs_ragged_pageable"
     h = [torch.from_numpy(np.ascontiguousarray(f[k])) for k in ("nH2", "Tgas", "Tdust", "vlos")]
     hc = torch.empty(it.shape_cube, dtype=torch.float32)
@@ -401,6 +406,7 @@ def test_observe_host_equals_device_path(case):
         hc = hc.pin_memory()
     it.observe_host(*h, hc)
     assert torch.equal(hc, ref)
+    assert it.smooth_fallback() == handed_over          # summed over the slabs, not the last slab's
     hc.zero_()
     it.observe_host(*h, hc)                                                 # second call reuses streams and events
     assert torch.equal(hc, ref)
