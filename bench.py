@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """Benchmark of the IRIS-SO hot path (BASELINE.json metric) -- one JSON line on stdout.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload large] [--algo flat|series|dense]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload large] [--algo window|dense]
 
 A "step" is one pass of the whole hot path (iris_so_observe: K1..K7) over one synthetic cube of the
 workload.  `value` = whole-job (cell x channel) updates per second = N * nx*ny*nz*nv * K / t, inputs resident
@@ -251,12 +251,12 @@ def timed_steps(torch, it, d, steps, cube):
 
 
 def bench_workload(torch, dist, name, algo, steps, warmup, rank, peaks, want_e2e, want_dense_probe, sampler_uuid):
-    from paper_2607_01338_b200 import IrisSO, ALGO_DENSE, ALGO_WINDOW, ALGO_FLAT
+    from paper_2607_01338_b200 import IrisSO, ALGO_DENSE, ALGO_WINDOW
     dev = torch.device("cuda", torch.cuda.current_device())
     cfg, recipe = make_workload(name)
     fields = make_fields(cfg, recipe, seed=recipe["seed"] + rank)
     d = [torch.from_numpy(fields[k]).to(dev) for k in ("nH2", "Tgas", "Tdust", "vlos")]
-    it = IrisSO(cfg, transfer_algo={"dense": ALGO_DENSE, "series": ALGO_WINDOW, "flat": ALGO_FLAT}[algo])
+    it = IrisSO(cfg, transfer_algo=ALGO_DENSE if algo == "dense" else ALGO_WINDOW)
     cube = torch.empty(it.shape_cube, dtype=torch.float32, device=dev)
     for _ in range(max(warmup, 3)):
         it.observe(*d, cube=cube)
@@ -520,8 +520,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="large", choices=["tiny", "small", "medium", "large"])
-    ap.add_argument("--algo", default="flat", choices=["flat", "series", "dense"],
-                    help="LOS transfer kernel: flat segment stream (default), one cell at a time (series), dense cross-check")
+    ap.add_argument("--algo", default="window", choices=["window", "dense"])
     ap.add_argument("--no-extras", action="store_true", help="skip the medium-cube and dense-algorithm side measurements")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs: its slab pipeline launches per slab)")

@@ -51,15 +51,12 @@ typedef enum {
 } iris_so_status;
 
 /* transfer_algo */
-#define IRIS_SO_ALGO_AUTO 0     /* = IRIS_SO_ALGO_FLAT */
+#define IRIS_SO_ALGO_AUTO 0     /* = IRIS_SO_ALGO_WINDOW */
 #define IRIS_SO_ALGO_DENSE 1    /* every (cell, channel) update evaluated; register-resident channel blocks */
 #define IRIS_SO_ALGO_WINDOW 2   /* only channels inside each cell's line window are updated; exact in fp32.
                                  * Profile from the channel-centre expansion when dv / xi <= 0.55 (every cell then
                                  * has dv / b <= 0.55), otherwise from erfc at the channel edges */
 #define IRIS_SO_ALGO_WINDOW_EDGE 3 /* line window with the erfc-at-the-edges profile for any channel width */
-#define IRIS_SO_ALGO_FLAT 4     /* the line-window algorithm with the windows of a warp's pixels cut into segments of 8
-                                 * channels that are handed to the lanes as one stream (transfer_flat_kernel); same
-                                 * profile and the same fall-backs as IRIS_SO_ALGO_WINDOW */
 
 typedef struct {
   /* grid: Cartesian analogue of the paper's (r, l, b) lattice; rays = z columns */

@@ -5,7 +5,7 @@ The library is loaded lazily on first use; there is no CPU fallback -- a missing
 libiris_so.so raises, it never degrades to another implementation.
 """
 from .binding import (IrisSO, IrisSOError, lib_path, load_library, DECLARED_SYMBOLS,
-                      ALGO_AUTO, ALGO_DENSE, ALGO_WINDOW, ALGO_WINDOW_EDGE, ALGO_FLAT)
+                      ALGO_AUTO, ALGO_DENSE, ALGO_WINDOW, ALGO_WINDOW_EDGE)
 
 __all__ = ["IrisSO", "IrisSOError", "lib_path", "load_library", "DECLARED_SYMBOLS",
-           "ALGO_AUTO", "ALGO_DENSE", "ALGO_WINDOW", "ALGO_WINDOW_EDGE", "ALGO_FLAT"]
+           "ALGO_AUTO", "ALGO_DENSE", "ALGO_WINDOW", "ALGO_WINDOW_EDGE"]

@@ -8,7 +8,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libiris_so.so")
 _lib = None
 
-ALGO_AUTO, ALGO_DENSE, ALGO_WINDOW, ALGO_WINDOW_EDGE, ALGO_FLAT = 0, 1, 2, 3, 4
+ALGO_AUTO, ALGO_DENSE, ALGO_WINDOW, ALGO_WINDOW_EDGE = 0, 1, 2, 3
 
 # every entry point include/iris_so.h declares
 DECLARED_SYMBOLS = (

@@ -19,7 +19,6 @@
 #include "transfer_dense.cuh"
 #include "transfer_window.cuh"
 #include "transfer_series.cuh"
-#include "transfer_flat.cuh"
 #include "transfer_modes.cuh"
 #include "transfer_smooth.cuh"
 #include "adjoint_kernels.cuh"
@@ -181,7 +180,7 @@ iris_so_status validate(const iris_so_config* c, std::string& why) {
   if (!(c->beam_fwhm_px >= 0.0)) return bad("beam_fwhm_px must be >= 0");
   if (!(c->noise_sigma >= 0.0) || !std::isfinite(c->noise_mu)) return bad("bad noise parameters");
   if (c->noise_gamma_mode < 0 || c->noise_gamma_mode > 1) return bad("bad noise_gamma_mode");
-  if (c->transfer_algo < 0 || c->transfer_algo > 4) return bad("bad transfer_algo");
+  if (c->transfer_algo < 0 || c->transfer_algo > 3) return bad("bad transfer_algo");
   if (c->coll_n_partners < 0 || c->coll_n_partners > 8) return bad("coll_n_partners must be in [0, 8]");
   if (c->coll_n_partners > 0) {
     if (c->coll_nT < 1 || c->coll_nT > 64) return bad("coll_nT must be in [1, 64]");
@@ -363,15 +362,12 @@ iris_so_status run_coefficients(iris_so_ctx* ctx, const float* n, const float* T
   return IRIS_SO_OK;
 }
 
-// Which transfer kernel the configuration selects: 1 dense, 2 window + centre-expansion profile (one cell at a time),
-// 3 window + erfc edges, 4 window + centre-expansion profile as a flat segment stream.
+// Which transfer kernel the configuration selects: 1 dense, 2 window + centre-expansion profile, 3 window + erfc edges.
 int resolved_algo(const iris_so_config& c) {
   int algo = c.transfer_algo;
-  if (algo == IRIS_SO_ALGO_AUTO) algo = IRIS_SO_ALGO_FLAT;
-  if ((algo == IRIS_SO_ALGO_WINDOW || algo == IRIS_SO_ALGO_FLAT) &&
-      !(c.microturb_cms > 0.0 && c.dv_cms <= (double)iris::kSeriesMaxS * c.microturb_cms))
+  if (algo == IRIS_SO_ALGO_AUTO) algo = IRIS_SO_ALGO_WINDOW;
+  if (algo == IRIS_SO_ALGO_WINDOW && !(c.microturb_cms > 0.0 && c.dv_cms <= (double)iris::kSeriesMaxS * c.microturb_cms))
     algo = IRIS_SO_ALGO_WINDOW_EDGE;      // b >= xi bounds dv / b only when there is microturbulence
-  if (algo == IRIS_SO_ALGO_FLAT && iris::flat_smem_per_warp(c.nv) + 1024 > 227u * 1024u) algo = IRIS_SO_ALGO_WINDOW;
   return algo;
 }
 
@@ -469,15 +465,10 @@ iris_so_status run_transfer(iris_so_ctx* ctx, const iris::MarchConsts& mc, float
     IRIS_CHECK_LAUNCH(ctx, "transfer_dense_kernel");
     return IRIS_SO_OK;
   }
-  cudaError_t e;
-  if (algo == IRIS_SO_ALGO_FLAT)
-    e = iris::launch_transfer_flat(mc, ctx->d_coef, ctx->ncell, npix, nz, nv, dust,
-                                   (float)(ctx->cfg.dv_cms / ctx->cfg.microturb_cms), out, out_cont, st);
-  else if (algo == IRIS_SO_ALGO_WINDOW)
-    e = iris::launch_transfer_series(mc, ctx->d_coef, ctx->ncell, npix, nz, nv, dust,
-                                     (float)(ctx->cfg.dv_cms / ctx->cfg.microturb_cms), out, out_cont, st);
-  else
-    e = iris::launch_transfer_window(mc, ctx->d_coef, ctx->ncell, npix, nz, nv, dust, ctx->sm_count, out, out_cont, st);
+  cudaError_t e = algo == IRIS_SO_ALGO_WINDOW
+                      ? iris::launch_transfer_series(mc, ctx->d_coef, ctx->ncell, npix, nz, nv, dust,
+                                                     (float)(ctx->cfg.dv_cms / ctx->cfg.microturb_cms), out, out_cont, st)
+                      : iris::launch_transfer_window(mc, ctx->d_coef, ctx->ncell, npix, nz, nv, dust, ctx->sm_count, out, out_cont, st);
   ctx->launches++;
   if (e != cudaSuccess) return cuda_fail(ctx, e, "launch of the line-window transfer kernel");
   return IRIS_SO_OK;
@@ -547,7 +538,6 @@ const char* iris_so_transfer_kernel(const iris_so_ctx* ctx) {
   switch (resolved_algo(ctx->cfg)) {
     case IRIS_SO_ALGO_DENSE: return "transfer_dense_kernel";
     case IRIS_SO_ALGO_WINDOW: return "transfer_series_kernel";
-    case IRIS_SO_ALGO_FLAT: return "transfer_flat_kernel";
     default: return "transfer_window_kernel";
   }
 }
@@ -893,8 +883,7 @@ static iris_so_status observe_adjoint_impl(iris_so_ctx* ctx, const float* d_nH2,
   iris::AdjointConsts ac = ctx->ac;
   if (wrt_abundance) ac.c_d = 0.0f;                    // the dust does not depend on the tracer abundance
   cudaError_t e = iris::launch_adjoint(ctx->mc, ac, ctx->lc, c.n_levels, ctx->band, ctx->d_coef, dcoef, ctx->ncell, (int)ctx->npix,
-                                       c.nz, c.nv, c.dust_on != 0,
-                                       resolved_algo(c) == IRIS_SO_ALGO_WINDOW || resolved_algo(c) == IRIS_SO_ALGO_FLAT, d_nH2, d_Tgas, what,
+                                       c.nz, c.nv, c.dust_on != 0, resolved_algo(c) == IRIS_SO_ALGO_WINDOW, d_nH2, d_Tgas, what,
                                        d_grad, st, &ctx->launches, wrt_abundance);
   if (e != cudaSuccess) return cuda_fail(ctx, e, "launch of adjoint kernels");
   return IRIS_SO_OK;
