@@ -57,6 +57,14 @@ class ObsConfig:
     coll_T_grid: np.ndarray = None        # [nT] ascending temperatures (K)
     coll_table: np.ndarray = None         # [P, nT, n_levels, n_levels] K_ul of partner p at T_grid[t], 0 where u <= l
     coll_partner_frac: np.ndarray = None  # [P] number density of partner p per n_H2
+    # grid precomputation + interpolation of the line coefficients; 0 = level balance solved per cell
+    coef_grid: int = 0
+    grid_n_density: int = 128     # nodes along n_H2 (paper: 128)
+    grid_n_temp: int = 64         # nodes along T_gas (paper: 64)
+    grid_nH2_lo: float = 1.0e-2
+    grid_nH2_hi: float = 1.0e9
+    grid_T_lo: float = 5.0
+    grid_T_hi: float = 3000.0
     # free-form label, ignored by both implementations
     name: str = field(default="", compare=False)
 

@@ -62,6 +62,10 @@ struct orc_config {
   const double *coll_T_grid;        // [nT] ascending temperatures
   const double *coll_table;         // [P][nT][n_levels * n_levels]  K_ul of partner p at T_grid[t], 0 where u <= l
   const double *coll_partner_frac;  // [P] number density of partner p per n_H2
+  // grid precomputation of section 4.2 and the lookup of section 4.3; reading S31
+  int32_t coef_grid;                // 0: level balance solved per cell; 1: coefficients interpolated from the grid
+  int32_t grid_n_density, grid_n_temp;      // nodes along n_H2 and T_gas (paper: 128 and 64)
+  double grid_nH2_lo, grid_nH2_hi, grid_T_lo, grid_T_hi;   // first and last node of each axis
 };
 
 // Planck function B_nu(T), Eq. 3.2.1 = Eq. 3.6.2 = Eq. 4.9.1.
@@ -245,16 +249,97 @@ void orc_cell_coefficients(const orc_config *c, double nH2, double Tgas, double 
   out5[4] = c->dust_on ? orc_planck(nu0, Tdust) : 0.0;
 }
 
-// coef[5][ncell]; pop may be NULL (then solved here) or [N][ncell].
+// ---------------------------------------------------------------------------------------------
+// O4b  Grid precomputation (section 4.2) and runtime lookup (section 4.3).
+// "the frequency-independent line emission and absorption coefficients j^[L], alpha^[L] ... are solved over a 3D grid of
+// dimensions gas density, H2 abundance, and gas kinetic temperature"; "the grid gradients are also computed to allow
+// the runtime computation ... via a fast linear interpolation ... emission and absorption that exhibit linear
+// behavior, rather than merely constant behavior, outside observability grid bounds and between grid points"; grids
+// are "per tracer abundance" (Eq. 4.2.1: j = chi j~, alpha = chi alpha~).
+// Reading S31: the per-cell inputs of this path are n_H2 and T_gas (all hydrogen molecular, collision
+// partners in fixed proportion to n_H2), so the H2-abundance axis has a single node and the grid is two-dimensional;
+// nodes are spaced geometrically between the configured end points (the paper states neither spacing nor bounds);
+// the interpolation is multilinear IN THE VARIABLES n_H2 and T_gas inside the grid cell that contains the point, its
+// gradients being the finite differences of the node values; outside the grid the nearest cell's multilinear form is
+// continued (linear extrapolation along each axis).
+// grid[2][nT][nn]: j~ = j0 / X and alpha~ = kappa0 / X at the nodes.
+double orc_grid_node(double lo, double hi, int n, int i) {
+  return n > 1 ? lo * std::pow(hi / lo, (double)i / (double)(n - 1)) : lo;
+}
+
+void orc_grid_build(const orc_config *c, double *grid) {
+  const int nn = c->grid_n_density, nT = c->grid_n_temp;
+  orc_config c1 = *c;
+  c1.abundance = 1.0;                 // per tracer abundance, Eq. 4.2.1
+  c1.T_inf = std::numeric_limits<double>::infinity();     // the T_inf mask is applied after the lookup
+#pragma omp parallel for schedule(static)
+  for (int q = 0; q < nn * nT; ++q) {
+    const int i = q % nn, j = q / nn;
+    const double n = orc_grid_node(c->grid_nH2_lo, c->grid_nH2_hi, nn, i);
+    const double T = orc_grid_node(c->grid_T_lo, c->grid_T_hi, nT, j);
+    double x[32], o[5];
+    orc_levelpop_cell(&c1, n, T, x);
+    orc_cell_coefficients(&c1, n, T, T, x, o);
+    grid[q] = o[0];
+    grid[(int64_t)nn * nT + q] = o[1];
+  }
+}
+
+// Multilinear interpolation / extrapolation of one grid plane g[nT][nn] at (n, T).
+double orc_grid_lookup_plane(const double *g, int nn, int nT, double n_lo, double n_hi, double T_lo, double T_hi,
+                             double n, double T) {
+  // index of the grid cell: the last node not above the point, clamped to the first / last cell
+  auto cell_of = [](double lo, double hi, int cnt, double v) {
+    if (cnt < 2) return 0;
+    int i = (int)std::floor(std::log(v / lo) / std::log(hi / lo) * (cnt - 1));
+    if (!(v > 0.0)) i = 0;
+    i = std::max(0, std::min(cnt - 2, i));
+    // the logarithm may land one cell off at a node: settle it with the node values themselves
+    while (i > 0 && v < orc_grid_node(lo, hi, cnt, i)) --i;
+    while (i < cnt - 2 && v >= orc_grid_node(lo, hi, cnt, i + 1)) ++i;
+    return i;
+  };
+  const int i = cell_of(n_lo, n_hi, nn, n), j = cell_of(T_lo, T_hi, nT, T);
+  const int i1 = std::min(i + 1, nn - 1), j1 = std::min(j + 1, nT - 1);
+  const double n0 = orc_grid_node(n_lo, n_hi, nn, i), n1 = orc_grid_node(n_lo, n_hi, nn, i1);
+  const double T0 = orc_grid_node(T_lo, T_hi, nT, j), T1 = orc_grid_node(T_lo, T_hi, nT, j1);
+  const double u = n1 > n0 ? (n - n0) / (n1 - n0) : 0.0, v = T1 > T0 ? (T - T0) / (T1 - T0) : 0.0;
+  const double f00 = g[(int64_t)j * nn + i], f10 = g[(int64_t)j * nn + i1], f01 = g[(int64_t)j1 * nn + i],
+               f11 = g[(int64_t)j1 * nn + i1];
+  return f00 + (f10 - f00) * u + (f01 - f00) * v + (f11 - f10 - f01 + f00) * u * v;
+}
+
+// j0, kappa0 of one cell from the grid: lookup, abundance applied last, then the T_inf mask.
+void orc_grid_cell(const orc_config *c, const double *grid, double nH2, double Tgas, double *j0, double *k0) {
+  const int nn = c->grid_n_density, nT = c->grid_n_temp;
+  *j0 = c->abundance * orc_grid_lookup_plane(grid, nn, nT, c->grid_nH2_lo, c->grid_nH2_hi, c->grid_T_lo, c->grid_T_hi, nH2, Tgas);
+  *k0 = c->abundance * orc_grid_lookup_plane(grid + (int64_t)nn * nT, nn, nT, c->grid_nH2_lo, c->grid_nH2_hi, c->grid_T_lo,
+                                             c->grid_T_hi, nH2, Tgas);
+  if (Tgas > c->T_inf) { *j0 = 0.0; *k0 = 0.0; }
+}
+
+// coef[5][ncell]; pop may be NULL (then solved here, or looked up in the grid when coef_grid = 1) or [N][ncell].
 void orc_coefficients(const orc_config *c, int64_t ncell, const float *nH2, const float *Tgas,
                       const float *Tdust, const double *pop, double *coef) {
   const int N = c->n_levels;
+  std::vector<double> grid;
+  const bool use_grid = !pop && c->coef_grid != 0;
+  if (use_grid) {
+    grid.resize((size_t)2 * c->grid_n_density * c->grid_n_temp);
+    orc_grid_build(c, grid.data());
+  }
 #pragma omp parallel for schedule(static)
   for (int64_t i = 0; i < ncell; ++i) {
     double x[32], o[5];
-    if (pop) for (int l = 0; l < N; ++l) x[l] = pop[(int64_t)l * ncell + i];
-    else orc_levelpop_cell(c, (double)nH2[i], (double)Tgas[i], x);
-    orc_cell_coefficients(c, (double)nH2[i], (double)Tgas[i], (double)Tdust[i], x, o);
+    if (use_grid) {
+      for (int l = 0; l < N; ++l) x[l] = 0.0;       // the populations are not needed: the grid holds the line coefficients
+      orc_cell_coefficients(c, (double)nH2[i], (double)Tgas[i], (double)Tdust[i], x, o);
+      orc_grid_cell(c, grid.data(), (double)nH2[i], (double)Tgas[i], &o[0], &o[1]);
+    } else {
+      if (pop) for (int l = 0; l < N; ++l) x[l] = pop[(int64_t)l * ncell + i];
+      else orc_levelpop_cell(c, (double)nH2[i], (double)Tgas[i], x);
+      orc_cell_coefficients(c, (double)nH2[i], (double)Tgas[i], (double)Tdust[i], x, o);
+    }
     for (int q = 0; q < 5; ++q) coef[(int64_t)q * ncell + i] = o[q];
   }
 }

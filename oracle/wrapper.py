@@ -57,6 +57,8 @@ class _Cfg(C.Structure):
         ("coll_n_partners", C.c_int32), ("coll_nT", C.c_int32),
         ("coll_T_grid", C.POINTER(C.c_double)), ("coll_table", C.POINTER(C.c_double)),
         ("coll_partner_frac", C.POINTER(C.c_double)),
+        ("coef_grid", C.c_int32), ("grid_n_density", C.c_int32), ("grid_n_temp", C.c_int32),
+        ("grid_nH2_lo", C.c_double), ("grid_nH2_hi", C.c_double), ("grid_T_lo", C.c_double), ("grid_T_hi", C.c_double),
     ]
 
 
@@ -218,6 +220,32 @@ class Oracle:
             pp = _dp(pop)
         self.lib.orc_coefficients(self._p(), C.c_int64(nH2.size), _fp(nH2), _fp(Tgas), _fp(Tdust), pp, _dp(coef))
         return coef
+
+    # -- coefficient grid (sections 4.2 - 4.3) ---------------------------------------------------
+    def grid_build(self):
+        """grid[2, nT, nn]: j0 / X and kappa0 / X at the nodes."""
+        self._omp()
+        g = np.zeros((2, int(self.s.grid_n_temp), int(self.s.grid_n_density)))
+        self.lib.orc_grid_build(self._p(), _dp(g))
+        return g
+
+    def grid_nodes(self):
+        f = self.lib.orc_grid_node
+        f.restype = C.c_double
+        f.argtypes = [C.c_double, C.c_double, C.c_int, C.c_int]
+        nn, nT = int(self.s.grid_n_density), int(self.s.grid_n_temp)
+        return (np.array([f(self.s.grid_nH2_lo, self.s.grid_nH2_hi, nn, i) for i in range(nn)]),
+                np.array([f(self.s.grid_T_lo, self.s.grid_T_hi, nT, j) for j in range(nT)]))
+
+    def grid_lookup_plane(self, plane, nH2, Tgas):
+        """Multilinear interpolation / extrapolation of one plane [nT, nn] at (nH2, Tgas)."""
+        f = self.lib.orc_grid_lookup_plane
+        f.restype = C.c_double
+        f.argtypes = [C.POINTER(C.c_double), C.c_int, C.c_int] + [C.c_double] * 6
+        plane = np.ascontiguousarray(plane, dtype=np.float64)
+        nT, nn = plane.shape
+        return f(_dp(plane), nn, nT, self.s.grid_nH2_lo, self.s.grid_nH2_hi, self.s.grid_T_lo, self.s.grid_T_hi,
+                 float(nH2), float(Tgas))
 
     # -- transfer --------------------------------------------------------------------------------
     def march(self, coef, vlos, pix=None):
