@@ -464,6 +464,51 @@ def bench_small_configs(torch, warmup):
     return out
 
 
+def bench_grid(torch, warmup, large_fields=None):
+    """The coefficient grid of PAPER.md section 4.2 / 4.3 (coef_grid = 1, the paper's 128 x 64 nodes over n_H2 = 1e-2 .. 1e9
+    cm^-3 and T = 5 .. 3000 K) in place of the per-cell level solve: time of the cell stage (K1 + K2) per cube, and the
+    gap of the interpolated medium cube to the cube of the exact solve (reported, not a parity claim)."""
+    from paper_2607_01338_b200 import IrisSO
+    dev = torch.device("cuda", torch.cuda.current_device())
+    out = {}
+    for name in ("medium", "large"):
+        cfg, recipe = make_workload(name)
+        if name == "large" and large_fields is not None:
+            fields = large_fields
+        else:
+            fields = make_fields(cfg, recipe)
+        d = [torch.from_numpy(fields[k]).to(dev) for k in ("nH2", "Tgas", "Tdust", "vlos")]
+        cubes = {}
+        res = {}
+        for label, c in (("exact", cfg), ("grid", cfg.with_(coef_grid=1))):
+            it = IrisSO(c)
+            cube = torch.empty(it.shape_cube, dtype=torch.float32, device=dev)
+            for _ in range(warmup):
+                it.observe(*d, cube=cube, beam=False, noise=False)
+            torch.cuda.synchronize()
+            it.profile(True)
+            for _ in range(5):
+                it.observe(*d, cube=cube, beam=False, noise=False)
+            prof = it.profile_read()
+            it.profile(False)
+            res["cell_stage_ms_" + label] = prof["cell"][0] / prof["cell"][1]
+            if name == "medium":
+                cubes[label] = cube.clone()
+            it.close()
+            del cube
+        if name == "medium":
+            peak = cubes["exact"].abs().amax(dim=-1, keepdim=True)
+            res["max_abs_dT_over_pixel_peak"] = float(((cubes["grid"] - cubes["exact"]).abs() / (peak + 1e-3)).max())
+            res["max_abs_dT_K"] = float((cubes["grid"] - cubes["exact"]).abs().max())
+        ncell = cfg.nx * cfg.ny * cfg.nz
+        res["hbm_floor_ms"] = 40.0 * ncell / (measured_peaks()["hbm_gbs"] * 1e9) * 1e3     # 16 B of fields in, 24 B of planes out
+        out[name] = res
+        del d
+        torch.cuda.empty_cache()
+    out["grid"] = "128 x 64 nodes, n_H2 1e-2 .. 1e9 cm^-3, T 5 .. 3000 K (ObsConfig defaults)"
+    return out
+
+
 def run_ours(args):
     import torch
     rank, local_rank, world = env_rank()
@@ -494,6 +539,7 @@ def run_ours(args):
     if not args.no_extras and world == 1:
         extra["other_modes_256x256x288_512ch"] = bench_modes(torch, max(args.warmup, 3))
         extra["other_configs"] = bench_small_configs(torch, max(args.warmup, 3))
+        extra["coefficient_grid"] = bench_grid(torch, max(args.warmup, 3), main["fields"] if cfg.name == "large" else None)
     if rank != 0:
         return 0
     cb = None

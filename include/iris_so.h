@@ -114,6 +114,19 @@ typedef struct {
   const double *coll_T_grid;        /* [coll_nT] strictly ascending, > 0 */
   const double *coll_table;         /* [coll_n_partners][coll_nT][n_levels * n_levels] K_ul (cm^3/s) for u > l, else 0 */
   const double *coll_partner_frac;  /* [coll_n_partners] number density of the partner per n_H2, >= 0 */
+  /* Grid precomputation (section 4.2) and lookup (section 4.3).  coef_grid = 0: the
+   * level balance is solved per cell (K1).  coef_grid = 1: iris_so_create tabulates the line coefficients per tracer
+   * abundance (Eq. 4.2.1) on grid_n_density x grid_n_temp nodes, spaced geometrically from grid_nH2_lo to grid_nH2_hi and
+   * from grid_T_lo to grid_T_hi, with their finite-difference gradients, and observe / transfer interpolate them:
+   * multilinear in n_H2 and T_gas inside the grid cell that holds the point, the edge cell's form continued outside
+   * the grid; abundance and the T_inf mask are applied after the lookup.  (The paper's third axis, the H2 abundance,
+   * has one node here: the fields carry n_H2 and the partner fractions are configuration constants.)  The lookup
+   * replaces K1 only in calls that solve the populations internally; iris_so_levelpop is unaffected, and the adjoint
+   * entry points return IRIS_SO_EUNSUPPORTED. */
+  int32_t coef_grid;
+  int32_t grid_n_density, grid_n_temp;   /* 2 .. 4096 nodes each (paper: 128, 64) */
+  double grid_nH2_lo, grid_nH2_hi;       /* 0 < lo < hi, cm^-3 */
+  double grid_T_lo, grid_T_hi;           /* 0 < lo < hi, K */
 } iris_so_config;
 
 /* Validates and copies the configuration (including the host arrays), selects the current CUDA device.

@@ -51,6 +51,8 @@ class _Config(C.Structure):
         ("coll_n_partners", C.c_int32), ("coll_nT", C.c_int32),
         ("coll_T_grid", C.POINTER(C.c_double)), ("coll_table", C.POINTER(C.c_double)),
         ("coll_partner_frac", C.POINTER(C.c_double)),
+        ("coef_grid", C.c_int32), ("grid_n_density", C.c_int32), ("grid_n_temp", C.c_int32),
+        ("grid_nH2_lo", C.c_double), ("grid_nH2_hi", C.c_double), ("grid_T_lo", C.c_double), ("grid_T_hi", C.c_double),
     ]
 
 

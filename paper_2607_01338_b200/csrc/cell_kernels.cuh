@@ -217,6 +217,105 @@ __global__ void __launch_bounds__(128) cellcoef_kernel(LevelConsts lc, CoefConst
   for (int q = 0; q < 6; ++q) coef[(int64_t)q * ncell + i] = o[q];
 }
 
+// ---- Grid precomputation and lookup (section 4.2, and section 4.3) -------------
+// Instead of the level balance per cell, the two line coefficients per tracer abundance (Eq. 4.2.1) are tabulated
+// once per context on a (n_H2, T_gas) grid with geometrically spaced nodes and interpolated at run time: multilinear
+// in the variables n_H2 and T_gas inside the grid cell that holds the point, the same form continued outside the
+// grid ("linear behavior ... outside observability grid bounds and between grid points").  The device
+// holds, per grid cell, the value at its lower corner and its three finite differences ("the grid gradients are also
+// computed") for both coefficients, so a lookup is two 16-byte loads and six multiply-adds:
+//   f(n, T) = f00 + fx u + fy v + fxy u v,   u = (n - n_i) / (n_i+1 - n_i),  v = (T - T_j) / (T_j+1 - T_j)
+// with f = E = n x_u (emission) and f = A = n (x_l g_u / g_l - x_u) (absorption); e_c = c_e E, a_c = c_a A.
+struct GridConsts {
+  const float2* nodes_n;   // [nn]  { n_i, 1 / (n_i+1 - n_i) }   (the last entry repeats the last interval)
+  const float2* nodes_T;   // [nT]  { T_j, 1 / (T_j+1 - T_j) }
+  const float4* cells;     // [2][nT - 1][nn - 1]  { f00, fx, fy, fxy } of E, then of A
+  int nn, nT;
+  float log2_n_lo, inv_dlog2_n, log2_T_lo, inv_dlog2_T;   // cell index = floor((log2 v - log2 lo) * inv_dlog2)
+};
+
+// node values E, A at (n_i, T_j): nodeval[2][nT][nn]
+template <int N, int BW, bool TABLE>
+__global__ void __launch_bounds__(128) grid_nodes_kernel(LevelConsts lc, CoefConsts cc, GridConsts gc,
+                                                         float* __restrict__ nodeval) {
+  const int q = blockIdx.x * blockDim.x + threadIdx.x;
+  if (q >= gc.nn * gc.nT) return;
+  const int i = q % gc.nn, j = q / gc.nn;
+  const float n = gc.nodes_n[i].x, T = gc.nodes_T[j].x;
+  float x[N], inv;
+  level_fractions<N, BW, TABLE>(lc, n, T, x, &inv);
+  float xu = 0.0f, xl = 0.0f;
+#pragma unroll
+  for (int l = 0; l < N; ++l) {
+    xu = fmaf(x[l], cc.pick_upper[l], xu);
+    xl = fmaf(x[l], cc.pick_lower[l], xl);
+  }
+  xu *= inv; xl *= inv;
+  nodeval[q] = n * xu;
+  nodeval[gc.nn * gc.nT + q] = n * fmaf(xl, cc.gr, -xu);
+}
+
+// per grid cell: lower-corner value and finite differences
+__global__ void __launch_bounds__(128) grid_cells_kernel(int nn, int nT, const float* __restrict__ nodeval,
+                                                         float4* __restrict__ cells) {
+  const int q = blockIdx.x * blockDim.x + threadIdx.x;
+  const int nc = (nn - 1) * (nT - 1);
+  if (q >= 2 * nc) return;
+  const int plane = q / nc, r = q % nc, i = r % (nn - 1), j = r / (nn - 1);
+  const float* g = nodeval + (size_t)plane * nn * nT;
+  const float f00 = g[j * nn + i], f10 = g[j * nn + i + 1], f01 = g[(j + 1) * nn + i], f11 = g[(j + 1) * nn + i + 1];
+  cells[q] = make_float4(f00, f10 - f00, f01 - f00, (f11 - f10) - (f01 - f00));
+}
+
+// K2 with the lookup in place of K1: coef[6][ncell].  One cell of the lookup:
+__device__ __forceinline__ void grid_cell(const CoefConsts& cc, const GridConsts& gc, float n, float T, float Td, float vlos,
+                                          float (&o)[6]) {
+  // grid cell (clamped to the first / last one: the multilinear form is continued outside the grid; a point that
+  // lands in a neighbouring cell by the rounding of the logarithm sees the same value, the interpolant is continuous)
+  const float fi = floorf((__log2f(fmaxf(n, 1.0e-37f)) - gc.log2_n_lo) * gc.inv_dlog2_n);
+  const float fj = floorf((__log2f(fmaxf(T, 1.0e-37f)) - gc.log2_T_lo) * gc.inv_dlog2_T);
+  const int i = (int)fminf(fmaxf(fi, 0.0f), (float)(gc.nn - 2)), j = (int)fminf(fmaxf(fj, 0.0f), (float)(gc.nT - 2));
+  const float2 gn = __ldg(gc.nodes_n + i), gT = __ldg(gc.nodes_T + j);
+  const float u = (n - gn.x) * gn.y, v = (T - gT.x) * gT.y;
+  const int nc = (gc.nn - 1) * (gc.nT - 1), q = j * (gc.nn - 1) + i;
+  const float4 fe = __ldg(gc.cells + q), fa = __ldg(gc.cells + nc + q);
+  const float E = fmaf(fmaf(fe.w, v, fe.y), u, fmaf(fe.z, v, fe.x));
+  const float A = fmaf(fmaf(fa.w, v, fa.y), u, fmaf(fa.z, v, fa.x));
+  cell_coefficients(cc, 1.0f, T, Td, vlos, E, 0.0f, o);      // Doppler width, line centre, Planck source; e = c_e E
+  o[1] = T > cc.T_inf ? 0.0f : cc.c_a * A;
+  o[4] = cc.c_d * n;
+}
+
+// Four consecutive cells per thread (16-byte loads and stores: the kernel moves 40 bytes per cell and nothing else
+// bounds it); `aligned` = every plane starts on a 16-byte boundary, else the scalar tail loop takes all cells.
+__global__ void __launch_bounds__(256) cellcoef_grid_kernel(CoefConsts cc, GridConsts gc, int64_t ncell, int aligned,
+                                                            const float* __restrict__ nH2, const float* __restrict__ Tgas,
+                                                            const float* __restrict__ Tdust, const float* __restrict__ vlos,
+                                                            float* __restrict__ coef) {
+  const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t c0 = 4 * t;
+  if (c0 >= ncell) return;
+  if (aligned && c0 + 4 <= ncell) {
+    const float4 n4 = *reinterpret_cast<const float4*>(nH2 + c0), T4 = *reinterpret_cast<const float4*>(Tgas + c0),
+                 d4 = *reinterpret_cast<const float4*>(Tdust + c0), v4 = *reinterpret_cast<const float4*>(vlos + c0);
+    float o[4][6];
+    grid_cell(cc, gc, n4.x, T4.x, d4.x, v4.x, o[0]);
+    grid_cell(cc, gc, n4.y, T4.y, d4.y, v4.y, o[1]);
+    grid_cell(cc, gc, n4.z, T4.z, d4.z, v4.z, o[2]);
+    grid_cell(cc, gc, n4.w, T4.w, d4.w, v4.w, o[3]);
+#pragma unroll
+    for (int k = 0; k < 6; ++k)
+      *reinterpret_cast<float4*>(coef + (int64_t)k * ncell + c0) = make_float4(o[0][k], o[1][k], o[2][k], o[3][k]);
+    return;
+  }
+  for (int64_t c = c0; c < min(c0 + 4, ncell); ++c) {
+    float o[6];
+    grid_cell(cc, gc, nH2[c], Tgas[c], Tdust[c], vlos[c], o);
+#pragma unroll
+    for (int k = 0; k < 6; ++k) coef[(int64_t)k * ncell + c] = o[k];
+  }
+}
+
 // K2 alone, from caller-supplied populations pop[N][ncell].
 __global__ void __launch_bounds__(256) coef_from_pop_kernel(CoefConsts cc, int64_t ncell, const float* __restrict__ nH2,
                                                             const float* __restrict__ Tgas,

@@ -42,6 +42,8 @@ struct iris_so_ctx {
   std::vector<double> Keff;     // tabulated rates folded over the partners: [nT][N*N] per unit n_H2 (empty: power law)
   std::vector<double> Tgrid;
   float* d_colltab = nullptr;   // device copy: nT temperatures, then nT * kMaxPairs float2 {K, K g_u/g_l} * rate_scale
+  float* d_grid = nullptr;      // coefficient grid (coef_grid = 1): node tables, node values, cell coefficients
+  iris::GridConsts gc;
   iris::LevelConsts lc;
   iris::CoefConsts cc;
   iris::MarchConsts mc;
@@ -196,6 +198,14 @@ iris_so_status validate(const iris_so_config* c, std::string& why) {
       const double k = c->coll_table[q];
       if (k < 0.0 || !std::isfinite(k) || (l >= u && k != 0.0)) return bad("coll_table must be finite, >= 0 and 0 for u <= l");
     }
+  }
+  if (c->coef_grid < 0 || c->coef_grid > 1) return bad("coef_grid must be 0 or 1");
+  if (c->coef_grid == 1) {
+    if (c->grid_n_density < 2 || c->grid_n_density > 4096 || c->grid_n_temp < 2 || c->grid_n_temp > 4096)
+      return bad("grid_n_density and grid_n_temp must be in [2, 4096]");
+    if (!(c->grid_nH2_lo > 0.0) || !(c->grid_nH2_hi > c->grid_nH2_lo) || !std::isfinite(c->grid_nH2_hi) ||
+        !(c->grid_T_lo > 0.0) || !(c->grid_T_hi > c->grid_T_lo) || !std::isfinite(c->grid_T_hi))
+      return bad("grid bounds must satisfy 0 < lo < hi");
   }
   if (c->transfer_mode < 0 || c->transfer_mode > 2) return bad("transfer_mode must be 0 (thick), 1 (selectively thin) or 2 (thin)");
   if (c->integration < 0 || c->integration > 1) return bad("integration must be 0 (formal) or 1 (smooth)");
@@ -353,6 +363,14 @@ iris_so_status run_coefficients(iris_so_ctx* ctx, const float* n, const float* T
     iris::coef_from_pop_kernel<<<(unsigned)((ctx->ncell + 255) / 256), 256, 0, st>>>(ctx->cc, ctx->ncell, n, T, Td, v, pop,
                                                                                      ctx->d_coef);
     IRIS_CHECK_LAUNCH(ctx, "coef_from_pop_kernel");
+  } else if (ctx->cfg.coef_grid == 1) {
+    // 16-byte accesses need aligned field pointers and planes that are a multiple of 4 cells apart
+    const int aligned = (ctx->ncell % 4 == 0) &&
+                        ((reinterpret_cast<uintptr_t>(n) | reinterpret_cast<uintptr_t>(T) | reinterpret_cast<uintptr_t>(Td) |
+                          reinterpret_cast<uintptr_t>(v)) % 16 == 0);
+    iris::cellcoef_grid_kernel<<<(unsigned)(((ctx->ncell + 3) / 4 + 255) / 256), 256, 0, st>>>(ctx->cc, ctx->gc, ctx->ncell, aligned, n,
+                                                                                               T, Td, v, ctx->d_coef);
+    IRIS_CHECK_LAUNCH(ctx, "cellcoef_grid_kernel");
   } else {
 #define CALL_(N) launch_cellcoef<N>(ctx, n, T, Td, v, ctx->d_coef, st)
     IRIS_DISPATCH_N(ctx->cfg.n_levels, CALL_)
@@ -510,6 +528,67 @@ iris_so_status run_noise(iris_so_ctx* ctx, float* cube, cudaStream_t st) {
   return IRIS_SO_OK;
 }
 
+template <int N>
+void launch_grid_nodes(iris_so_ctx* ctx, float* nodeval) {
+  const int nq = ctx->gc.nn * ctx->gc.nT;
+  const unsigned grid = (unsigned)((nq + 127) / 128);
+  constexpr int BN = iris::kBandNarrow < N - 1 ? iris::kBandNarrow : N - 1;
+  const bool table = ctx->lc.tb.K != nullptr;
+  if (ctx->band <= BN) {
+    if (table) iris::grid_nodes_kernel<N, BN, true><<<grid, 128>>>(ctx->lc, ctx->cc, ctx->gc, nodeval);
+    else iris::grid_nodes_kernel<N, BN, false><<<grid, 128>>>(ctx->lc, ctx->cc, ctx->gc, nodeval);
+  } else {
+    if (table) iris::grid_nodes_kernel<N, N - 1, true><<<grid, 128>>>(ctx->lc, ctx->cc, ctx->gc, nodeval);
+    else iris::grid_nodes_kernel<N, N - 1, false><<<grid, 128>>>(ctx->lc, ctx->cc, ctx->gc, nodeval);
+  }
+}
+
+// Grid precomputation: node tables on the host (double), node values and cell coefficients on the device.
+iris_so_status build_grid(iris_so_ctx* ctx) {
+  const iris_so_config& c = ctx->cfg;
+  const int nn = c.grid_n_density, nT = c.grid_n_temp;
+  std::vector<float> h(2 * (size_t)(nn + nT));
+  auto fill = [&](float* dst, int cnt, double lo, double hi) {
+    std::vector<double> node(cnt);
+    for (int i = 0; i < cnt; ++i) node[i] = (double)(float)(lo * std::pow(hi / lo, (double)i / (double)(cnt - 1)));
+    for (int i = 0; i < cnt; ++i) {
+      const int a = std::min(i, cnt - 2);
+      dst[2 * i] = (float)node[i];
+      dst[2 * i + 1] = (float)(1.0 / (node[a + 1] - node[a]));
+    }
+  };
+  fill(h.data(), nn, c.grid_nH2_lo, c.grid_nH2_hi);
+  fill(h.data() + 2 * nn, nT, c.grid_T_lo, c.grid_T_hi);
+  const size_t tab_f = h.size(), node_f = 2 * (size_t)nn * nT, cell_f = 8 * (size_t)(nn - 1) * (nT - 1);
+  const size_t node_off = (tab_f + 3) / 4 * 4, cell_off = (node_off + node_f + 3) / 4 * 4;      // 16-byte aligned blocks
+  cudaError_t e = cudaMalloc(reinterpret_cast<void**>(&ctx->d_grid), (cell_off + cell_f) * sizeof(float));
+  if (e != cudaSuccess) return cuda_fail(nullptr, e, "cudaMalloc(coefficient grid)");
+  if ((e = cudaMemcpy(ctx->d_grid, h.data(), tab_f * sizeof(float), cudaMemcpyHostToDevice)) != cudaSuccess)
+    return cuda_fail(nullptr, e, "upload of the grid nodes");
+  iris::GridConsts& gc = ctx->gc;
+  gc.nodes_n = reinterpret_cast<const float2*>(ctx->d_grid);
+  gc.nodes_T = reinterpret_cast<const float2*>(ctx->d_grid + 2 * nn);
+  gc.cells = reinterpret_cast<const float4*>(ctx->d_grid + cell_off);
+  gc.nn = nn; gc.nT = nT;
+  gc.log2_n_lo = (float)std::log2(c.grid_nH2_lo);
+  gc.inv_dlog2_n = (float)((nn - 1) / std::log2(c.grid_nH2_hi / c.grid_nH2_lo));
+  gc.log2_T_lo = (float)std::log2(c.grid_T_lo);
+  gc.inv_dlog2_T = (float)((nT - 1) / std::log2(c.grid_T_hi / c.grid_T_lo));
+  float* nodeval = ctx->d_grid + node_off;
+#define CALL_(N) launch_grid_nodes<N>(ctx, nodeval)
+  IRIS_DISPATCH_N(c.n_levels, CALL_)
+#undef CALL_
+  ctx->launches++;
+  if ((e = cudaGetLastError()) != cudaSuccess) return cuda_fail(nullptr, e, "launch of grid_nodes_kernel");
+  iris::grid_cells_kernel<<<(unsigned)((2 * (nn - 1) * (nT - 1) + 127) / 128), 128>>>(nn, nT, nodeval,
+                                                                                    reinterpret_cast<float4*>(ctx->d_grid + cell_off));
+  ctx->launches++;
+  if ((e = cudaGetLastError()) != cudaSuccess) return cuda_fail(nullptr, e, "launch of grid_cells_kernel");
+  if ((e = cudaDeviceSynchronize()) != cudaSuccess) return cuda_fail(nullptr, e, "grid precomputation");
+  ctx->scratch_bytes += (cell_off + cell_f) * sizeof(float);
+  return IRIS_SO_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -626,13 +705,17 @@ iris_so_status iris_so_create(const iris_so_config* cfg, iris_so_ctx** out) {
     ctx->lc.tb.K = reinterpret_cast<const float2*>(ctx->d_colltab + toff);
     ctx->lc.tb.nT = nT;
   }
+  if (cfg->coef_grid == 1) {
+    iris_so_status gs = build_grid(ctx);
+    if (gs != IRIS_SO_OK) { iris_so_destroy(ctx); return gs; }
+  }
   *out = ctx;
   return IRIS_SO_OK;
 }
 
 void iris_so_destroy(iris_so_ctx* ctx) {
   if (!ctx) return;
-  cudaFree(ctx->d_coef); cudaFree(ctx->d_tmp); cudaFree(ctx->d_stage); cudaFree(ctx->d_adj); cudaFree(ctx->d_counter); cudaFree(ctx->d_gate); cudaFree(ctx->d_metrics); cudaFree(ctx->d_colltab);
+  cudaFree(ctx->d_coef); cudaFree(ctx->d_tmp); cudaFree(ctx->d_stage); cudaFree(ctx->d_adj); cudaFree(ctx->d_counter); cudaFree(ctx->d_gate); cudaFree(ctx->d_metrics); cudaFree(ctx->d_colltab); cudaFree(ctx->d_grid);
   if (ctx->s_in) cudaStreamDestroy(ctx->s_in);
   if (ctx->s_out) cudaStreamDestroy(ctx->s_out);
   for (auto ev : ctx->slab_events) cudaEventDestroy(ev);
@@ -862,6 +945,8 @@ static iris_so_status observe_adjoint_impl(iris_so_ctx* ctx, const float* d_nH2,
     return fail(ctx, IRIS_SO_EUNSUPPORTED, "adjoint needs intensity-space subtraction and out_unit 0 or 1");
   if (!hot_path_mode(c))
     return fail(ctx, IRIS_SO_EUNSUPPORTED, "adjoint is implemented for the thick / formal / channel-integrated mode only");
+  if (c.coef_grid == 1)
+    return fail(ctx, IRIS_SO_EUNSUPPORTED, "adjoint differentiates the per-cell level solve: not available with coef_grid = 1");
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   iris_so_status s = run_coefficients(ctx, d_nH2, d_Tgas, d_Tdust, d_vlos, nullptr, st);
   if (s != IRIS_SO_OK) return s;
