@@ -65,6 +65,8 @@ class ObsConfig:
     grid_nH2_hi: float = 1.0e9
     grid_T_lo: float = 5.0
     grid_T_hi: float = 3000.0
+    # 0: dust source, background and unit conversion at nu0; 1: at every channel's own frequency
+    dust_per_channel: int = 0
     # free-form label, ignored by both implementations
     name: str = field(default="", compare=False)
 

@@ -66,6 +66,9 @@ struct orc_config {
   int32_t coef_grid;                // 0: level balance solved per cell; 1: coefficients interpolated from the grid
   int32_t grid_n_density, grid_n_temp;      // nodes along n_H2 and T_gas (paper: 128 and 64)
   double grid_nH2_lo, grid_nH2_hi, grid_T_lo, grid_T_hi;   // first and last node of each axis
+  // 0: dust source, background and unit conversion at nu0 (reading S6); 1: at every channel's own frequency (PAPER.md:513,
+  // "the Doppler-shifted Planck source function"; reading S32).  Hot-path mode only.
+  int32_t dust_per_channel;
 };
 
 // Planck function B_nu(T), Eq. 3.2.1 = Eq. 3.6.2 = Eq. 4.9.1.
@@ -536,6 +539,46 @@ void orc_march_column(const orc_config *c, const double *coef, const float *vlos
   *I_cont = Ic;
 }
 
+// O6c  The hot-path march with the dust source, the background and (in orc_observe) the unit conversion evaluated at
+// every channel's own frequency instead of nu0 (the dust emission coefficients "are then computed over all
+// points on the velocity/frequency-expanded physical-tensor grid according to the Doppler-shifted Planck source
+// function given in Equation 3.2.1"; the dust opacity stays "constant over the small frequency window" of the line).
+// Reading S32, with the classical Doppler shift of Eq. 4.3.1 and the radio convention of reading G9:
+//   channel k is observed at        nu_k  = nu0 (1 - v_k / c)
+//   a cell moving with v_los emits  nu'   = nu_k (1 + v_los / c)   in its own frame:  S_d = B_nu'(T_dust)
+//   the background enters as        I_bg  = B_nu_k(T_cmb)
+// The continuum is then a spectrum, not a scalar: I_cont[nv].  The line terms are unchanged (j0, kappa0 and the
+// profile are defined at the line).
+double orc_channel_frequency(const orc_config *c, int k) {
+  return c->nu0_Hz * (1.0 - (c->v0_cms + k * c->dv_cms) / kC);
+}
+
+void orc_march_column_perchannel(const orc_config *c, const double *coef, const float *vlos, const float *Tdust,
+                                 int64_t pix, double *I_tot /*[nv]*/, double *I_cont /*[nv]*/) {
+  const int64_t plane = (int64_t)c->nx * c->ny, ncell = plane * c->nz;
+  const double h = c->cell_cm;
+  for (int v = 0; v < c->nv; ++v) I_tot[v] = I_cont[v] = orc_planck(orc_channel_frequency(c, v), c->T_cmb);
+  for (int k = 0; k < c->nz; ++k) {
+    const int64_t cell = (int64_t)k * plane + pix;
+    const double j0 = coef[cell], k0 = coef[ncell + cell], b = coef[2 * ncell + cell], ad = coef[3 * ncell + cell];
+    const double vl = (double)vlos[cell], Td = (double)Tdust[cell];
+    for (int v = 0; v < c->nv; ++v) {
+      const double Sd = c->dust_on ? orc_planck(orc_channel_frequency(c, v) * (1.0 + vl / kC), Td) : 0.0;
+      const double pb = orc_phibar(c, v, vl, b);
+      I_tot[v] = formal_step(I_tot[v], j0 * pb + ad * Sd, k0 * pb + ad, h);
+      I_cont[v] = formal_step(I_cont[v], ad * Sd, ad, h);
+    }
+  }
+}
+
+// Columns pix[0..npix): I_tot[npix][nv], I_cont[npix][nv].
+void orc_march_perchannel(const orc_config *c, const double *coef, const float *vlos, const float *Tdust, int64_t npix,
+                          const int64_t *pix, double *I_tot, double *I_cont) {
+#pragma omp parallel for schedule(dynamic, 4)
+  for (int64_t p = 0; p < npix; ++p)
+    orc_march_column_perchannel(c, coef, vlos, Tdust, pix[p], I_tot + p * c->nv, I_cont + p * c->nv);
+}
+
 // Columns pix[0..npix): I_tot[npix][nv], I_cont[npix].
 void orc_march(const orc_config *c, const double *coef, const float *vlos, int64_t npix,
                const int64_t *pix, double *I_tot, double *I_cont) {
@@ -548,6 +591,15 @@ void orc_march(const orc_config *c, const double *coef, const float *vlos, int64
 //   subtract_space 0: D = I_tot - I_cont (intensity space == RJ space), then converted to out_unit
 //   subtract_space 1: T_B(I_tot) - T_B(I_cont)  (Planck space; result is in Kelvin)
 //   subtract_continuum 0: I_tot converted to out_unit.
+// nu: the frequency the conversion is made at (nu0, or the channel's own frequency with dust_per_channel = 1)
+double orc_convert_voxel_nu(const orc_config *c, double nu, double It, double Ic) {
+  if (c->subtract_continuum && c->subtract_space == 1) return orc_planck_TB(nu, It) - orc_planck_TB(nu, Ic);
+  const double D = c->subtract_continuum ? It - Ic : It;
+  if (c->out_unit == 0) return D;
+  if (c->out_unit == 1) return orc_rayleigh_jeans_T(nu, D);
+  return orc_planck_TB(nu, D);
+}
+
 double orc_convert_voxel(const orc_config *c, double It, double Ic) {
   const double nu = c->nu0_Hz;
   if (c->subtract_continuum && c->subtract_space == 1) return orc_planck_TB(nu, It) - orc_planck_TB(nu, Ic);
@@ -662,6 +714,13 @@ void orc_observe(const orc_config *c, const float *nH2, const float *Tgas, const
 #pragma omp parallel for schedule(dynamic, 4)
   for (int64_t p = 0; p < plane; ++p) {
     std::vector<double> It(c->nv);
+    if (c->dust_per_channel) {
+      std::vector<double> Icv(c->nv);
+      orc_march_column_perchannel(c, coef.data(), vlos, Tdust, p, It.data(), Icv.data());
+      for (int v = 0; v < c->nv; ++v)
+        cube[p * c->nv + v] = orc_convert_voxel_nu(c, orc_channel_frequency(c, v), It[v], Icv[v]);
+      continue;
+    }
     double Ic;
     orc_march_column(c, coef.data(), vlos, p, It.data(), &Ic);
     for (int v = 0; v < c->nv; ++v) cube[p * c->nv + v] = orc_convert_voxel(c, It[v], Ic);

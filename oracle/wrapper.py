@@ -59,6 +59,7 @@ class _Cfg(C.Structure):
         ("coll_partner_frac", C.POINTER(C.c_double)),
         ("coef_grid", C.c_int32), ("grid_n_density", C.c_int32), ("grid_n_temp", C.c_int32),
         ("grid_nH2_lo", C.c_double), ("grid_nH2_hi", C.c_double), ("grid_T_lo", C.c_double), ("grid_T_hi", C.c_double),
+        ("dust_per_channel", C.c_int32),
     ]
 
 
@@ -260,6 +261,24 @@ class Oracle:
         Ic = np.zeros(pix.size)
         self.lib.orc_march(self._p(), _dp(coef), _fp(vlos), C.c_int64(pix.size), _ip(pix), _dp(It), _dp(Ic))
         return It, Ic
+
+    def march_perchannel(self, coef, vlos, Tdust, pix=None):
+        """Hot-path march with the dust source / background at every channel's own frequency: I_tot[npix, nv], I_cont[npix, nv]."""
+        self._omp()
+        coef = np.ascontiguousarray(coef, dtype=np.float64)
+        vlos, Tdust = _f32(vlos).ravel(), _f32(Tdust).ravel()
+        plane = int(self.s.nx) * int(self.s.ny)
+        pix = np.arange(plane, dtype=np.int64) if pix is None else np.ascontiguousarray(pix, dtype=np.int64)
+        It = np.zeros((pix.size, int(self.s.nv)))
+        Ic = np.zeros((pix.size, int(self.s.nv)))
+        self.lib.orc_march_perchannel(self._p(), _dp(coef), _fp(vlos), _fp(Tdust), C.c_int64(pix.size), _ip(pix), _dp(It), _dp(Ic))
+        return It, Ic
+
+    def channel_frequency(self, k):
+        f = self.lib.orc_channel_frequency
+        f.restype = C.c_double
+        f.argtypes = [C.c_void_p, C.c_int]
+        return f(self._p(), int(k))
 
     def brute_column(self, coef, vlos, pix, nsub):
         coef = np.ascontiguousarray(coef, dtype=np.float64)

@@ -416,3 +416,66 @@ def test_tsre_and_tam_definitions():
     assert o.metrics(big, -big)["tsre_lbv"] == pytest.approx(2.0)
     assert o.metrics(big, 1e9 * big)["tsre_lbv"] == pytest.approx(2.0, rel=1e-8, abs=0.0)
     assert o.metrics(big, 1e-3 * big)["tsre_lbv"] == 0.0 and o.metrics(1e-3 * big, big)["tam1"] == 0.0
+
+
+# ------------------------------------------------------------------------------------------------
+# dust source, background and unit conversion at every channel's own frequency (reading S32)
+def _planck(nu, T):
+    return 2 * H * nu ** 3 / CL ** 2 / np.expm1(H * nu / (KB * T))
+
+
+def test_per_channel_dust_slab_closed_form_and_doppler_shift():
+    """Dust only, uniform slab: I_cont,k = B_nu'(T_d) (1 - e^-tau) + B_nu_k(T_cmb) e^-tau with nu_k = nu0 (1 - v_k / c) and,
+    for dust moving with v_los, nu' = nu_k (1 + v_los / c).  A dropped or mis-signed shift changes the answer by
+    3e-4 relative (v / c times d ln B / d ln nu), far above the 1e-12 asked here."""
+    cfg, _ = make_workload("tiny", n=2, nv=16)
+    cfg = cfg.with_(nz=7, abundance=0.0, dust_on=True, kappa_gas_cm2_g=0.8, dust_per_channel=1, dv_cms=8.0 * KMS, v0_cms=-60.0 * KMS)
+    o = Oracle(cfg)
+    for vl in (0.0, 3.1e6):
+        f = slab(cfg, n=2.0e3, T=40.0, Td=33.0)
+        f["vlos"] = np.full_like(f["vlos"], vl)
+        coef = o.coefficients(f["nH2"], f["Tgas"], f["Tdust"])
+        It, Ic = o.march_perchannel(coef, f["vlos"], f["Tdust"])
+        tau = coef[3, 0] * cfg.nz * cfg.cell_cm
+        assert 0.05 < tau < 5
+        vk = cfg.v0_cms + np.arange(cfg.nv) * cfg.dv_cms
+        nuk = cfg.nu0_Hz * (1 - vk / CL)
+        assert np.allclose([o.channel_frequency(k) for k in range(cfg.nv)], nuk, rtol=1e-15, atol=0.0)
+        vl32 = float(np.float32(vl))
+        expect = _planck(nuk * (1 + vl32 / CL), 33.0) * -np.expm1(-tau) + _planck(nuk, cfg.T_cmb) * np.exp(-tau)
+        assert np.allclose(Ic[0], expect, rtol=1e-12, atol=0.0) and np.allclose(It[0], Ic[0], rtol=1e-14, atol=0.0)
+        # against the channel-constant reading (S6): first order in v / c
+        _, Ic0 = Oracle(cfg.with_(dust_per_channel=0)).march(coef, f["vlos"])
+        gap = np.abs(Ic[0] / Ic0[0] - 1)
+        assert 1e-5 < gap.max() < 2e-3 and gap[np.argmin(np.abs(vk - vl))] < gap.max()
+
+
+def test_per_channel_dust_in_equilibrium_with_the_background_and_opaque_isothermal_slab():
+    cfg, _ = make_workload("tiny", n=2, nv=12)
+    cfg = cfg.with_(nz=5, abundance=0.0, dust_on=True, kappa_gas_cm2_g=2.0, dust_per_channel=1, dv_cms=5.0 * KMS, v0_cms=-27.5 * KMS)
+    # dust at rest at the background temperature: nothing changes, whatever tau, in every channel
+    f = slab(cfg, n=5.0e3, T=40.0, Td=cfg.T_cmb)
+    o = Oracle(cfg)
+    It, Ic = o.march_perchannel(o.coefficients(f["nH2"], f["Tgas"], f["Tdust"]), f["vlos"], f["Tdust"])
+    Td32 = float(np.float32(cfg.T_cmb))
+    for k in range(cfg.nv):
+        lo, hi = sorted((_planck(o.channel_frequency(k), Td32), _planck(o.channel_frequency(k), cfg.T_cmb)))
+        assert lo * (1 - 1e-13) <= Ic[0, k] <= hi * (1 + 1e-13)
+    # an opaque isothermal slab is a black body at every channel: Planck brightness temperature = T_d in all channels
+    c2 = cfg.with_(kappa_gas_cm2_g=400.0, out_unit=2, subtract_continuum=False)
+    f2 = slab(c2, n=5.0e3, T=40.0, Td=57.0)
+    cube = Oracle(c2).observe(f2, beam=False, noise=False)
+    assert np.allclose(cube, 57.0, rtol=1e-10, atol=0.0)
+    # ... which the channel-constant conversion does not give
+    It2, Ic2 = Oracle(c2).march_perchannel(Oracle(c2).coefficients(f2["nH2"], f2["Tgas"], f2["Tdust"]), f2["vlos"], f2["Tdust"])
+    assert abs(Oracle(c2).planck_TB(c2.nu0_Hz, It2[0, 0]) - 57.0) > 1e-3
+
+
+def test_per_channel_dust_leaves_the_line_terms_alone():
+    """Dust off: the per-channel background B_nu_k(T_cmb) is all that differs; with T_cmb = 0 the two readings agree."""
+    cfg, f = grid_case(n=4, nv=48, T_cmb=0.0, T_bar=2.725)
+    o = Oracle(cfg.with_(dust_per_channel=1))
+    coef = o.coefficients(f["nH2"], f["Tgas"], f["Tdust"])
+    It, Ic = o.march_perchannel(coef, f["vlos"], f["Tdust"])
+    It0, Ic0 = Oracle(cfg).march(coef, f["vlos"])
+    assert np.all(Ic == 0.0) and np.allclose(It, It0, rtol=1e-14, atol=0.0) and It0.max() > 0
