@@ -59,7 +59,9 @@ typedef enum {
 #define IRIS_SO_ALGO_WINDOW_EDGE 3 /* line window with the erfc-at-the-edges profile for any channel width */
 
 typedef struct {
-  /* grid: Cartesian analogue of the paper's (r, l, b) lattice; rays = z columns */
+  /* grid: rays = z columns.  The paper's observer-centred spherical lattice (l, b, r) with r sampled "at regular
+   * intervals" IS this layout: x = l, y = b, z = r with k = 0 the far end of the ray and cell_cm the
+   * radial step (every ray of the lattice is a column with a constant step; the cube comes out as [b][l][v]). */
   int32_t nx, ny, nz;
   double cell_cm;               /* step h along the ray (Eq. 4.8.7) */
   /* molecule (the paper reads these from a LAMDA file); host arrays, copied by create */
@@ -127,6 +129,14 @@ typedef struct {
   int32_t grid_n_density, grid_n_temp;   /* 2 .. 4096 nodes each (paper: 128, 64) */
   double grid_nH2_lo, grid_nH2_hi;       /* 0 < lo < hi, cm^-3 */
   double grid_T_lo, grid_T_hi;           /* 0 < lo < hi, K */
+  /* 0: the dust source B_nu(T_dust), the background B_nu(T_cmb) and the unit conversion are taken at nu0 (the continuum
+   * is one value per pixel).  1: at every channel's own frequency ("the Doppler-shifted Planck source
+   * function"): channel k is observed at nu_k = nu0 (1 - v_k / c) and the dust of a cell moving with v_los emits at
+   * nu_k (1 + v_los / c) in its own frame; the dust opacity stays constant over the band.  Hot-path mode only
+   * (transfer_mode = integration = subsample = 0; else create returns IRIS_SO_EUNSUPPORTED); runs through the dense
+   * kernel; iris_so_transfer then takes d_I_cont = NULL only (the continuum is a spectrum), the adjoint entry points
+   * return IRIS_SO_EUNSUPPORTED. */
+  int32_t dust_per_channel;
 } iris_so_config;
 
 /* Validates and copies the configuration (including the host arrays), selects the current CUDA device.

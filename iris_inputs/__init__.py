@@ -8,7 +8,7 @@ none of the method's arithmetic (no level balance, no profile, no transfer) and 
 """
 from .config import ObsConfig
 from .molecule import rigid_rotor
-from .fields import WORKLOADS, make_workload, make_fields, gaussian_random_field, weight_cube
+from .fields import WORKLOADS, make_workload, make_fields, gaussian_random_field, weight_cube, lattice_to_columns
 
 __all__ = ["ObsConfig", "rigid_rotor", "WORKLOADS", "make_workload", "make_fields",
-           "gaussian_random_field", "weight_cube"]
+           "gaussian_random_field", "weight_cube", "lattice_to_columns"]

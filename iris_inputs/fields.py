@@ -137,6 +137,14 @@ def make_fields(cfg, recipe, seed=None):
     return out
 
 
+def lattice_to_columns(t_lbr):
+    """A physical tensor on the paper's observer-centred spherical lattice, indexed (l, b, r) with r sampled at regular
+    intervals outward from the observer, as the [nz][ny][nx] column layout of this path: z = r with
+    k = 0 the FAR end of the ray, y = b, x = l.  A pure change of index order; cell_cm is the radial step."""
+    t = np.asarray(t_lbr)
+    return np.ascontiguousarray(np.transpose(t, (2, 1, 0))[::-1])
+
+
 def weight_cube(cfg, seed=2000):
     """Seeded weight cube w ~ U[0,1), float32 (ny, nx, nv), for L = sum(w * cube) (config "batch")."""
     rng = np.random.default_rng([int(seed), 11])

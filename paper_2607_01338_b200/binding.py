@@ -53,6 +53,7 @@ class _Config(C.Structure):
         ("coll_partner_frac", C.POINTER(C.c_double)),
         ("coef_grid", C.c_int32), ("grid_n_density", C.c_int32), ("grid_n_temp", C.c_int32),
         ("grid_nH2_lo", C.c_double), ("grid_nH2_hi", C.c_double), ("grid_T_lo", C.c_double), ("grid_T_hi", C.c_double),
+        ("dust_per_channel", C.c_int32),
     ]
 
 
@@ -259,7 +260,7 @@ class IrisSO:
         dev = nH2.device
         if I_total is None:
             I_total = torch.empty(self.shape_cube, dtype=torch.float32, device=dev)
-        if I_cont is None:
+        if I_cont is None and not getattr(self.cfg, "dust_per_channel", 0):     # (then the continuum is a spectrum: not returned)
             I_cont = torch.empty(self.shape_cube[:2], dtype=torch.float32, device=dev)
         self._check(self.lib.iris_so_transfer(
             self._h, self._dev(nH2, n, "nH2"), self._dev(Tgas, n, "Tgas"), self._dev(Tdust, n, "Tdust"),

@@ -207,6 +207,7 @@ iris_so_status validate(const iris_so_config* c, std::string& why) {
         !(c->grid_T_lo > 0.0) || !(c->grid_T_hi > c->grid_T_lo) || !std::isfinite(c->grid_T_hi))
       return bad("grid bounds must satisfy 0 < lo < hi");
   }
+  if (c->dust_per_channel < 0 || c->dust_per_channel > 1) return bad("dust_per_channel must be 0 or 1");
   if (c->transfer_mode < 0 || c->transfer_mode > 2) return bad("transfer_mode must be 0 (thick), 1 (selectively thin) or 2 (thin)");
   if (c->integration < 0 || c->integration > 1) return bad("integration must be 0 (formal) or 1 (smooth)");
   if (c->subsample < 0 || c->subsample > 255 || (c->subsample > 0 && c->subsample % 2 == 0))
@@ -282,6 +283,9 @@ void fold_constants(iris_so_ctx* ctx) {
   mc.out_mode = out_mode_of(c);
   mc.fine_m = 0;
   mc.ray_simpson = 0;
+  mc.v0_over_c = (float)(c.v0_cms / C_LIGHT);
+  mc.dv_over_c = (float)(c.dv_cms / C_LIGHT);
+  mc.hnu_k_over_Tcmb = c.T_cmb > 0.0 ? (float)(H_PLANCK * nu / K_BOLTZ / c.T_cmb) : 0.0f;
 
   iris::BeamConsts& bc = ctx->bc;
   std::memset(&bc, 0, sizeof bc);
@@ -474,11 +478,13 @@ iris_so_status run_transfer(iris_so_ctx* ctx, const iris::MarchConsts& mc, float
   // the line-window kernels keep whole spectra in shared memory: beyond ~13000 channels they do not fit and the
   // dense kernel (spectra in registers, any nv) takes over
   const bool fits = (size_t)(32 / 8) * ((size_t)nv + 32) * sizeof(float) + 2048 <= 227u * 1024u;
-  if (algo == IRIS_SO_ALGO_DENSE || !fits) {
+  if (algo == IRIS_SO_ALGO_DENSE || !fits || ctx->cfg.dust_per_channel) {
     constexpr int CB = 16, NW = 4;
     const int nx = ctx->cfg.nx, rows = npix / nx;
     dim3 block(32, NW), grid(((nx + 7) / 8) * ((rows + 3) / 4), (nv + CB * NW - 1) / (CB * NW));
-    if (dust) iris::transfer_dense_kernel<CB, true><<<grid, block, 0, st>>>(mc, ctx->d_coef, ctx->ncell, npix, nx, nz, nv, out, out_cont);
+    if (ctx->cfg.dust_per_channel)      // (with the dust off its planes are zero: the same instantiation)
+      iris::transfer_dense_kernel<CB, true, true><<<grid, block, 0, st>>>(mc, ctx->d_coef, ctx->ncell, npix, nx, nz, nv, out, out_cont);
+    else if (dust) iris::transfer_dense_kernel<CB, true><<<grid, block, 0, st>>>(mc, ctx->d_coef, ctx->ncell, npix, nx, nz, nv, out, out_cont);
     else iris::transfer_dense_kernel<CB, false><<<grid, block, 0, st>>>(mc, ctx->d_coef, ctx->ncell, npix, nx, nz, nv, out, out_cont);
     IRIS_CHECK_LAUNCH(ctx, "transfer_dense_kernel");
     return IRIS_SO_OK;
@@ -613,6 +619,7 @@ const char* iris_so_transfer_kernel(const iris_so_ctx* ctx) {
   if (windowed_thin_mode(ctx->cfg) || windowed_fine_mode(ctx->cfg)) return "transfer_series_kernel";
   if (windowed_smooth_mode(ctx->cfg)) return "transfer_smooth_window_kernel";
   if (!hot_path_mode(ctx->cfg)) return "transfer_modes_kernel";
+  if (ctx->cfg.dust_per_channel) return "transfer_dense_kernel";
   if ((size_t)(32 / 8) * ((size_t)ctx->cfg.nv + 32) * sizeof(float) + 2048 > 227u * 1024u) return "transfer_dense_kernel";
   switch (resolved_algo(ctx->cfg)) {
     case IRIS_SO_ALGO_DENSE: return "transfer_dense_kernel";
@@ -635,6 +642,8 @@ iris_so_status iris_so_create(const iris_so_config* cfg, iris_so_ctx** out) {
     if ((int)std::ceil(4.0 * sigma) > iris::kMaxBeamRadius)
       return fail(nullptr, IRIS_SO_EUNSUPPORTED, "beam radius ceil(4 sigma) exceeds 32 pixels");
   }
+  if (cfg->dust_per_channel && !hot_path_mode(*cfg))
+    return fail(nullptr, IRIS_SO_EUNSUPPORTED, "dust_per_channel = 1 is implemented for the thick / formal / channel-integrated mode only");
   int dev = 0, count = 0;
   cudaError_t e = cudaGetDeviceCount(&count);
   if (e != cudaSuccess || count == 0) {
@@ -740,6 +749,8 @@ iris_so_status iris_so_transfer(iris_so_ctx* ctx, const float* d_nH2, const floa
   if (!ctx) return IRIS_SO_EINVAL;
   if (!d_nH2 || !d_Tgas || !d_Tdust || !d_vlos) return fail(ctx, IRIS_SO_EINVAL, "iris_so_transfer: NULL field pointer");
   if (!d_I_total && !d_I_cont) return fail(ctx, IRIS_SO_EINVAL, "iris_so_transfer: no output requested");
+  if (ctx->cfg.dust_per_channel && d_I_cont)
+    return fail(ctx, IRIS_SO_EUNSUPPORTED, "iris_so_transfer: with dust_per_channel = 1 the continuum is a spectrum; pass d_I_cont = NULL");
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   iris_so_status s = begin_call(ctx, st);
   if (s != IRIS_SO_OK) return s;
@@ -947,6 +958,8 @@ static iris_so_status observe_adjoint_impl(iris_so_ctx* ctx, const float* d_nH2,
     return fail(ctx, IRIS_SO_EUNSUPPORTED, "adjoint is implemented for the thick / formal / channel-integrated mode only");
   if (c.coef_grid == 1)
     return fail(ctx, IRIS_SO_EUNSUPPORTED, "adjoint differentiates the per-cell level solve: not available with coef_grid = 1");
+  if (c.dust_per_channel)
+    return fail(ctx, IRIS_SO_EUNSUPPORTED, "adjoint is not available with dust_per_channel = 1");
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   iris_so_status s = run_coefficients(ctx, d_nH2, d_Tgas, d_Tdust, d_vlos, nullptr, st);
   if (s != IRIS_SO_OK) return s;

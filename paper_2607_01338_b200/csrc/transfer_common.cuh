@@ -43,7 +43,23 @@ struct MarchConsts {
   int out_mode;
   int fine_m;       // fine velocity grid of the series kernel's MODE 3: intervals per channel (f + 1); 0 elsewhere
   int ray_simpson;  // series kernel MODE 2 (optically thin): 1 = Simpson weights along the ray (Eq. 4.7.7), 0 = Eq. 4.7.6
+  // dust_per_channel = 1 (dense kernel only): channel k is observed at nu_k = nu0 (1 - v_k / c)
+  float v0_over_c, dv_over_c;   // v_k / c = v0_over_c + k dv_over_c
+  float hnu_k_over_Tcmb;        // h nu0 / (k T_cmb); 0 = no background
 };
+
+// Planck function at nu = r nu0 in the units of the march (Rayleigh-Jeans Kelvin AT nu0: I c^2 / (2 k nu0^2)), for
+// x0 = h nu0 / (k T):  (h nu0 / k) r^3 / (exp(x0 r) - 1)
+__device__ __forceinline__ float planck_krj_at(float hnu_k, float x0, float r) {
+  return x0 > 0.0f ? hnu_k * r * r * r * rcp_approx(expm1f(x0 * r)) : 0.0f;
+}
+
+// K5 at the channel's own frequency nu_k = r nu0: D, C in Rayleigh-Jeans Kelvin at nu0 (intensity = D inv_KRJ).
+__device__ __forceinline__ float planck_tb_at(float t, float hnu_k, float r) {
+  if (t == 0.0f) return 0.0f;
+  const float tb = hnu_k * r / log1pf(hnu_k * r * r * r / fabsf(t));
+  return copysignf(tb, t);
+}
 
 // Planck brightness temperature of a Rayleigh-Jeans temperature (Eq. 4.9.1 with I = T_rj / K_RJ):
 // T_B = (h nu / k) / ln(1 + (h nu / k) / T_rj); odd extension, T_B(0) = 0.
@@ -62,6 +78,19 @@ __device__ __forceinline__ float convert_out(float D, float C, const MarchConsts
     case OUT_TB_OF_SUB: return planck_tb_of_trj(D, mc.hnu_k);
     case OUT_TB_OF_TOT: return planck_tb_of_trj(D + C, mc.hnu_k);
     default: return planck_tb_of_trj(D + C, mc.hnu_k) - planck_tb_of_trj(C, mc.hnu_k);
+  }
+}
+
+__device__ __forceinline__ float convert_out_at(float D, float C, const MarchConsts& mc, float r) {
+  const float q = 1.0f / (r * r);                       // T_RJ at nu_k = T_RJ at nu0 * (nu0 / nu_k)^2
+  switch (mc.out_mode) {
+    case OUT_TRJ_SUB: return D * q;
+    case OUT_TRJ_TOT: return (D + C) * q;
+    case OUT_I_SUB: return D * mc.inv_KRJ;
+    case OUT_I_TOT: return (D + C) * mc.inv_KRJ;
+    case OUT_TB_OF_SUB: return planck_tb_at(D, mc.hnu_k, r);
+    case OUT_TB_OF_TOT: return planck_tb_at(D + C, mc.hnu_k, r);
+    default: return planck_tb_at(D + C, mc.hnu_k, r) - planck_tb_at(C, mc.hnu_k, r);
   }
 }
 

@@ -8,12 +8,18 @@
 // from the line centre only attenuates by the dust (D *= E_d) -- exact in fp32 because erfc underflows
 // the fp32 sum there.  The continuum march (K4) is a scalar per thread; subtraction / unit conversion
 // (K5) is the epilogue.  Output: CB consecutive floats per thread (float4 stores).
+//
+// PERCH (dust_per_channel = 1; "the Doppler-shifted Planck source function"): the dust source of a cell,
+// the background and the unit conversion are evaluated at every channel's own frequency, nu_k = nu0 (1 - v_k / c),
+// the dust of a cell moving with v_los emitting at nu' = nu_k (1 + v_los / c) in its own frame.  The continuum is then
+// one value per channel (CB more registers), the dust temperature is recovered from S_d(nu0) of the coefficient plane,
+// and every update costs one more exponential; this kernel, where a thread owns its channels, is the natural home.
 #pragma once
 #include "transfer_common.cuh"
 
 namespace iris {
 
-template <int CB, bool DUST>
+template <int CB, bool DUST, bool PERCH = false>
 __global__ void __launch_bounds__(128)
 transfer_dense_kernel(MarchConsts mc, const float* __restrict__ coef, int64_t ncell, int npix, int nx, int nz, int nv,
                       float* __restrict__ out, float* __restrict__ out_cont) {
@@ -28,6 +34,14 @@ transfer_dense_kernel(MarchConsts mc, const float* __restrict__ coef, int64_t nc
 #pragma unroll
   for (int i = 0; i < CB; ++i) D[i] = 0.0f;
   float C = mc.T_bg;
+  float Ck[PERCH ? CB : 1], rk[PERCH ? CB : 1];      // PERCH: continuum and nu_k / nu0 per channel
+  if (PERCH) {
+#pragma unroll
+    for (int i = 0; i < CB; ++i) {
+      rk[i] = 1.0f - fmaf((float)(k0 + i), mc.dv_over_c, mc.v0_over_c);
+      Ck[i] = planck_krj_at(mc.hnu_k, mc.hnu_k_over_Tcmb, rk[i]);
+    }
+  }
 
   const float* p = coef + pix;
   // software prefetch of the next cell's coefficients
@@ -48,6 +62,9 @@ transfer_dense_kernel(MarchConsts mc, const float* __restrict__ coef, int64_t nc
       d.m_d = one_minus_exp_neg(tau_d);
       C = fmaf(C, d.E_d, S_d * d.m_d);
     }
+    // PERCH: h nu0 / (k T_d) from S_d(nu0) = (h nu0 / k) / expm1(x_d), and 1 + v_los / c of the cell
+    const float x_d = (PERCH && S_d > 0.0f) ? log1pf(mc.hnu_k / S_d) : 0.0f;
+    const float r_cell = PERCH ? 1.0f + fmaf(c_los - 0.5f, mc.dv_over_c, mc.v0_over_c) : 1.0f;
     const float base = ((float)k0 - c_los) * s;          // x of the block's first edge
     const float top = fmaf((float)CB, s, base);          // x of its last edge
     if (top > -IRIS_ERFC_TMAX && base < IRIS_ERFC_TMAX && a_c != 0.0f) {
@@ -61,12 +78,20 @@ transfer_dense_kernel(MarchConsts mc, const float* __restrict__ coef, int64_t nc
         const float G_hi = signed_erfc(x_hi);
         const float sg_hi = copysignf(1.0f, x_hi);
         const float dErf = (sg_hi - sg_lo) - (G_hi - G_lo);
+        if (PERCH) {
+          d.S_d = planck_krj_at(mc.hnu_k, x_d, rk[i] * r_cell);
+          d.C = Ck[i];
+          Ck[i] = fmaf(Ck[i], d.E_d, d.S_d * d.m_d);
+        }
         D[i] = DUST ? update_dust(D[i], dErf, e_c, a_c, d) : update_nodust(D[i], dErf, a_c, sc);
         G_lo = G_hi; sg_lo = sg_hi;
       }
     } else if (DUST) {
 #pragma unroll
-      for (int i = 0; i < CB; ++i) D[i] *= d.E_d;
+      for (int i = 0; i < CB; ++i) {
+        D[i] *= d.E_d;
+        if (PERCH) Ck[i] = fmaf(Ck[i], d.E_d, planck_krj_at(mc.hnu_k, x_d, rk[i] * r_cell) * d.m_d);
+      }
     }
   }
 
@@ -76,14 +101,19 @@ transfer_dense_kernel(MarchConsts mc, const float* __restrict__ coef, int64_t nc
 #pragma unroll
       for (int i = 0; i < CB; i += 4) {
         float4 v;
-        v.x = convert_out(D[i], C, mc); v.y = convert_out(D[i + 1], C, mc);
-        v.z = convert_out(D[i + 2], C, mc); v.w = convert_out(D[i + 3], C, mc);
+        if (PERCH) {
+          v.x = convert_out_at(D[i], Ck[i], mc, rk[i]); v.y = convert_out_at(D[i + 1], Ck[i + 1], mc, rk[i + 1]);
+          v.z = convert_out_at(D[i + 2], Ck[i + 2], mc, rk[i + 2]); v.w = convert_out_at(D[i + 3], Ck[i + 3], mc, rk[i + 3]);
+        } else {
+          v.x = convert_out(D[i], C, mc); v.y = convert_out(D[i + 1], C, mc);
+          v.z = convert_out(D[i + 2], C, mc); v.w = convert_out(D[i + 3], C, mc);
+        }
         *reinterpret_cast<float4*>(o + i) = v;
       }
     } else {
 #pragma unroll
       for (int i = 0; i < CB; ++i)
-        if (k0 + i < nv) o[i] = convert_out(D[i], C, mc);
+        if (k0 + i < nv) o[i] = PERCH ? convert_out_at(D[i], Ck[i], mc, rk[i]) : convert_out(D[i], C, mc);
     }
   }
   if (out_cont != nullptr && cb == 0) out_cont[pix] = C * mc.inv_KRJ;

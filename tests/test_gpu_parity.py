@@ -506,3 +506,75 @@ def test_tabulated_rates_single_temperature_and_validation():
 def test_full_size_small_sampled():
     """BASELINE config "small" at full size (128^3 cells, 256 channels, dust, tau_peak up to ~20)."""
     _sampled_check("small", 64, 13)
+
+
+# ------------------------------------------------------------------------------------------------
+# SURVEY 8(f)-4: spherical-lattice input, dust at every channel's own frequency
+def test_spherical_lattice_tensor_is_the_column_layout():
+    """A physical tensor indexed (l, b, r), r at regular intervals outward from the observer, fed as
+    [nz = r reversed][ny = b][nx = l]: the cube [b][l][v] equals, ray by ray, what the oracle gives for each lattice ray
+    marched on its own from its far end (no neighbouring ray enters before the beam)."""
+    from iris_inputs import lattice_to_columns
+    nl, nb, nr = 21, 9, 40
+    cfg, r = make_workload("small", nx=nl, ny=nb, nz=nr, nv=96)
+    rng = np.random.default_rng(77)
+    t = dict(nH2=np.exp(rng.normal(6.5, 1.2, (nl, nb, nr))), Tgas=rng.uniform(30, 120, (nl, nb, nr)),
+             vlos=rng.normal(0.0, 6e5, (nl, nb, nr)))                 # (l, b, r), r = 0 next to the observer
+    t["Tdust"] = t["Tgas"]
+    f = {k: lattice_to_columns(v.astype(np.float32)) for k, v in t.items()}
+    assert f["nH2"].shape == (nr, nb, nl) and f["nH2"][0, 3, 5] == np.float32(t["nH2"][5, 3, nr - 1])
+    cube = iris(cfg).observe(*dev_fields(f)).cpu().numpy()
+    # one lattice ray at a time through the oracle: a 1 x 1 sky with the ray's cells from far to near
+    c1 = cfg.with_(nx=1, ny=1)
+    for l, b in ((0, 0), (5, 3), (20, 8), (11, 4)):
+        ray = {k: np.ascontiguousarray(v[l, b, ::-1].astype(np.float32)).reshape(nr, 1, 1) for k, v in t.items()}
+        assert_spectra(cube[b, l][None, None, :], Oracle(c1).observe(ray), what="lattice ray l=%d b=%d" % (l, b))
+
+
+@pytest.mark.parametrize("case", ["small_dust", "moving_dust_no_line", "planck_total", "dust_off", "ragged_intensity"])
+def test_dust_at_every_channels_own_frequency(case):
+    """dust_per_channel = 1 (reading S32) through the dense kernel against the oracle."""
+    shape = dict(nx=13, ny=3, nz=19, nv=45) if case == "ragged_intensity" else dict(n=24, nv=96)
+    cfg, r = make_workload("small", **shape)
+    cfg = cfg.with_(dust_per_channel=1, v0_cms=-0.5 * (cfg.nv - 1) * cfg.dv_cms)
+    f = make_fields(cfg, r)
+    f["vlos"] = (0.25 * f["vlos"]).astype(np.float32)
+    extra = 0.0
+    if case == "moving_dust_no_line":
+        cfg = cfg.with_(abundance=0.0, kappa_gas_cm2_g=30.0 * cfg.kappa_gas_cm2_g, subtract_continuum=False)
+    elif case == "planck_total":
+        cfg = cfg.with_(out_unit=2, subtract_continuum=False)
+    elif case == "dust_off":
+        cfg = cfg.with_(dust_on=False, kappa_gas_cm2_g=0.0)
+    elif case == "ragged_intensity":
+        cfg = cfg.with_(out_unit=0, subtract_continuum=False)
+    it = iris(cfg)
+    assert it.transfer_kernel() == "transfer_dense_kernel"
+    cube = it.observe(*dev_fields(f)).cpu().numpy()
+    ref = Oracle(cfg).observe(f)
+    if not cfg.subtract_continuum:
+        extra = 3e-7 * np.abs(ref).max(axis=-1, keepdims=True)       # storage rounding of the total (tests/parity.py)
+    floor = 1e-6 / krj(cfg.nu0_Hz) if cfg.out_unit == 0 else 1e-6
+    rel = 2.6e-4 if cfg.out_unit == 2 else 1e-4
+    worst = assert_spectra(cube, ref, floor=floor, rel=rel, extra=extra, what=case)
+    # and the flag matters: the channel-constant reading differs by more than the tolerance somewhere
+    if case in ("moving_dust_no_line", "planck_total"):
+        ref0 = Oracle(cfg.with_(dust_per_channel=0)).observe(f)
+        assert np.abs(ref0 - ref).max() > 1e-5 * np.abs(ref).max()
+    print("dust_per_channel %s: worst pixel at %.3g of tolerance" % (case, worst))
+
+
+def test_dust_per_channel_unsupported_combinations():
+    from paper_2607_01338_b200 import IrisSOError
+    cfg, r = make_workload("small", n=8, nv=16)
+    f = make_fields(cfg, r)
+    for bad in (dict(integration=1), dict(transfer_mode=2), dict(subsample=1)):
+        with pytest.raises(IrisSOError) as e:
+            iris(cfg.with_(dust_per_channel=1, **bad))
+        assert e.value.status == 2
+    it = iris(cfg.with_(dust_per_channel=1))
+    I_tot, I_cont = it.transfer(*dev_fields(f))
+    assert I_cont is None and bool(torch.isfinite(I_tot).all())
+    with pytest.raises(IrisSOError) as e:
+        it.transfer(*dev_fields(f), I_cont=torch.empty((cfg.ny, cfg.nx), dtype=torch.float32, device="cuda"))
+    assert e.value.status == 2
