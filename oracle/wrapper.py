@@ -12,7 +12,8 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "iris_oracle.cpp")
-_LIB = os.path.join(_HERE, "liboracle.so")
+# IRIS_ORACLE_LIB: an already built oracle library to load instead (the sanitizer build of tests/test_sanitizers.py)
+_LIB = os.environ.get("IRIS_ORACLE_LIB") or os.path.join(_HERE, "liboracle.so")
 _lock = threading.Lock()
 
 
@@ -23,6 +24,8 @@ def oracle_lib_path():
 def build_oracle(force=False):
     """Compile the oracle with g++ -O2 (+OpenMP over cells / pixel columns). Returns the .so path."""
     with _lock:
+        if os.environ.get("IRIS_ORACLE_LIB"):
+            return _LIB
         if (not force and os.path.exists(_LIB)
                 and os.path.getmtime(_LIB) >= os.path.getmtime(_SRC)):
             return _LIB

@@ -5,7 +5,8 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_LIB_PATH = os.path.join(_HERE, "libiris_so.so")
+# IRIS_SO_LIB: another build of the same library to load instead (the bounds-checked build of tests/test_sanitizers.py)
+_LIB_PATH = os.environ.get("IRIS_SO_LIB") or os.path.join(_HERE, "libiris_so.so")
 _lib = None
 
 ALGO_AUTO, ALGO_DENSE, ALGO_WINDOW, ALGO_WINDOW_EDGE = 0, 1, 2, 3

@@ -25,17 +25,23 @@ def needs_build():
     return any(os.path.getmtime(s) > t for s in sources())
 
 
-def build(force=False, verbose=False):
-    """Compile csrc/iris_so.cu -> libiris_so.so. Returns the library path."""
-    if not force and not needs_build():
-        return LIB
+LIB_CHECKED = os.path.join(HERE, "libiris_so_checked.so")
+
+
+def build(force=False, verbose=False, checked=False):
+    """Compile csrc/iris_so.cu -> libiris_so.so (checked: -> libiris_so_checked.so with -DIRIS_SO_CHECKED, the
+    bounds-checked build tests/test_sanitizers.py runs). Returns the library path."""
+    lib = LIB_CHECKED if checked else LIB
+    if not force and os.path.exists(lib) and all(os.path.getmtime(s) <= os.path.getmtime(lib) for s in sources()):
+        return lib
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    tmp = LIB + ".tmp%d" % os.getpid()
-    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp, os.path.join(CSRC, "iris_so.cu")]
+    tmp = lib + ".tmp%d" % os.getpid()
+    cmd = ([nvcc] + NVCC_FLAGS + (["-DIRIS_SO_CHECKED"] if checked else []) + (["-Xptxas", "-v"] if verbose else [])
+           + ["-o", tmp, os.path.join(CSRC, "iris_so.cu")])
     subprocess.run(cmd, check=True)
-    os.replace(tmp, LIB)
-    return LIB
+    os.replace(tmp, lib)
+    return lib
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv, checked="--checked" in sys.argv))

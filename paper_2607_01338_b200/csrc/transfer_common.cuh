@@ -14,6 +14,23 @@
 #pragma once
 #include "iris_math.cuh"
 
+// Checked build (python -m paper_2607_01338_b200.build --checked -> libiris_so_checked.so, tests/test_sanitizers.py):
+// every shared-memory access of the line-window kernels is tested against the region its warp owns and traps outside it
+// (compute-sanitizer is closed on the GPU pool this library is developed on; this is the bounds check of our own).
+#ifdef IRIS_SO_CHECKED
+#include <cstdio>
+#define IRIS_CHECK_SMEM(ptr, bytes, lo, hi)                                                                    \
+  do {                                                                                                         \
+    const char* p_ = reinterpret_cast<const char*>(ptr);                                                       \
+    if (p_ < reinterpret_cast<const char*>(lo) || p_ + (bytes) > reinterpret_cast<const char*>(hi)) {          \
+      printf("IRIS_SO_CHECKED: shared-memory access out of the warp's region at %s:%d\n", __FILE__, __LINE__);  \
+      __trap();                                                                                                \
+    }                                                                                                          \
+  } while (0)
+#else
+#define IRIS_CHECK_SMEM(ptr, bytes, lo, hi) ((void)0)
+#endif
+
 namespace iris {
 
 // The windowed kernels store the spectrum multiplied by G = exp(dust optical depth so far) and fold G back into it when

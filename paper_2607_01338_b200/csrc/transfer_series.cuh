@@ -357,6 +357,9 @@ transfer_series_kernel(MarchConsts mc, const float* __restrict__ coef, int64_t n
       f32x2 xx = pk(x, x + q0.y);
       const f32x2 step2 = pk1((float)(2 * LPP) * q0.y);
       float* d = sp + (q / LPP) * ROW + (q % LPP) * 2;
+      // (checked build) the pairs of every pass of this lane lie inside the spectra of this warp
+      IRIS_CHECK_SMEM(d, 8, spec + (size_t)warp * nvp * PPW, spec + (size_t)(warp + 1) * nvp * PPW);
+      IRIS_CHECK_SMEM(d + (npass - 1) * ROW, 8, spec + (size_t)warp * nvp * PPW, spec + (size_t)(warp + 1) * nvp * PPW);
       int rem = npass;
       while (rem >= 2) {
         series_passes<DUST, DEG, LPP, 2, MODE>(d, q, qend, xx, step2, o);
@@ -411,11 +414,13 @@ transfer_series_kernel(MarchConsts mc, const float* __restrict__ coef, int64_t n
       const int jb = min(j + 1, ncz - 1) * PPW;
       const float4 b0 = rq[jb], b1 = rq[32 + jb], b2 = NQ > 2 ? rq[64 + jb] : float4{}, b3 = NQ > 3 ? rq[96 + jb] : float4{};
       cell_step(a0, a1, a2, a3);
+      __syncwarp();      // the lane -> pair mapping follows each cell's window: cell j + 1 reads pairs other lanes wrote in cell j
       const int jn = min(j + 2, ncz - 1) * PPW;
       a0 = rq[jn]; a1 = rq[32 + jn];
       if (NQ > 2) a2 = rq[64 + jn];
       if (NQ > 3) a3 = rq[96 + jn];
       if (j + 1 < ncz) cell_step(b0, b1, b2, b3);
+      __syncwarp();
     }
   }
   __syncwarp();

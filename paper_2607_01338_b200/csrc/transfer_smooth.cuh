@@ -188,6 +188,7 @@ transfer_smooth_window_kernel(MarchConsts mc, const float* __restrict__ coef, in
           const float E = e_c * pw, A = a_c * pw, E0 = e_0 * pw0, A0 = a_0 * pw0;
           const float Du = ((E0 - A0 * C) + (E - A * C_unc)) * rcp_approx(2.0f + A + td);
           const float U = fmaxf(Du + relu_add, relu_min) * inv_dn;              // ReLU on D + C and on C
+          IRIS_CHECK_SMEM(prv + IDX(k), 4, sm + (size_t)warp * 2 * arr, sm + (size_t)(warp + 1) * 2 * arr);
           prv[IDX(k)] = U;
           u_min = fminf(u_min, U);
         }
@@ -205,6 +206,8 @@ transfer_smooth_window_kernel(MarchConsts mc, const float* __restrict__ coef, in
         const f32x2 xstep2 = pk1(2.0f * (float)LPP * xb);
         for (int k = k0; k <= ehi; k += 2 * LPP, xx = add2(xx, xstep2)) {
           const int w = IDX(k);
+          IRIS_CHECK_SMEM(cur + w, 8, sm + (size_t)warp * 2 * arr, sm + (size_t)(warp + 1) * 2 * arr);
+          IRIS_CHECK_SMEM(prv + w, 8, sm + (size_t)warp * 2 * arr, sm + (size_t)(warp + 1) * 2 * arr);
           const f32x2 u = mul2(xx, xx);
           float u0, u1;
           upk(u, u0, u1);
