@@ -42,9 +42,13 @@ FP32_PER_PIXEL_CELL = 60
 SM_COUNT, SFU_LANES_PER_SM_CLK, FP32_LANES_PER_SM_CLK = 148, 16.0, 124.9
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum of one launch from the committed `ncu --set full` captures
-# (profiles/r01_v3.md), keyed by (workload, kernel)
-NCU_TRAFFIC_BYTES = {("large", "transfer_series_kernel"): 4271062000}
+# STORED figures, not values of this run: dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel
+# from the committed `ncu --set full` capture of the named profiles/ pass, keyed by (workload, kernel).  Refreshed with
+# every profiles/ pass; `roofline.traffic_source` names the pass in the JSON line.
+NCU_TRAFFIC_BYTES = {
+    ("large", "transfer_series_kernel"): (4271062000, "profiles/r01_v4.md (round 1 capture; the update loop is unchanged since)"),
+    ("medium", "transfer_series_kernel"): (566401280, "profiles/r01_v4.md (round 1 capture: 453 + 113 MB)"),
+}
 
 
 def env_rank():
@@ -179,17 +183,23 @@ def omp_threads(threads=None):
         return os.cpu_count() or 1
 
 
-def cpu_baseline(cfg, fields, budget_s=15.0):
-    """Oracle, as it stands, on a bounded sample (about budget_s seconds of wall time on all host cores)."""
+def cpu_baseline(cfg, fields, budget_s=12.0):
+    """Oracle, as it stands, on a bounded sample: about budget_s seconds of wall time on all host cores, then about
+    budget_s / 2 seconds on ONE thread (BASELINE.md section 2 asks for both)."""
     th = omp_threads()
     n0 = max(2 * th, 16)
     dt, upd, th = oracle_sample(cfg, fields, n0)
     n = int(min(max(n0, n0 * budget_s / max(dt, 1e-3)), cfg.nx * cfg.ny, 65536))
     if n > n0:
         dt, upd, th = oracle_sample(cfg, fields, n)
+    per_col_1 = dt * th / max(n, 1)                       # a column on one thread, if the scaling were perfect
+    n1 = int(min(max(4, 0.5 * budget_s / max(per_col_1, 1e-4)), n))
+    dt1, upd1, _ = oracle_sample(cfg, fields, n1, threads=1)
     return dict(value=upd / dt, unit=UNIT, cores=th, kind="oracle",
                 sample="%d of %d seeded pixel columns of the %s workload (whole path K1-K5 per column, float64, g++ -O2, "
-                       "OpenMP over columns), %.1f s" % (min(n, cfg.nx * cfg.ny), cfg.nx * cfg.ny, cfg.name, dt))
+                       "OpenMP over columns), %.1f s" % (min(n, cfg.nx * cfg.ny), cfg.nx * cfg.ny, cfg.name, dt),
+                single_thread={"value": upd1 / dt1, "unit": UNIT, "cores": 1,
+                               "sample": "%d of the same columns on one thread, %.1f s" % (n1, dt1)})
 
 
 # --------------------------------------------------------------------------------------------------------
@@ -293,7 +303,9 @@ def bench_workload(torch, dist, name, algo, steps, warmup, rank, peaks, want_e2e
     res["roofline"] = {
         "bound": "alu", "pipe": "sfu (MUFU.EX2 / MUFU.RCP)", "kernel": it.transfer_kernel(), "algorithm": algo,
         "achieved": sfu_ops / t_k3 / 1e12, "peak": sfu_peak / 1e12, "unit": "Tops/s (SFU lane operations)",
-        "frac": t_sfu / t_k3, "traffic": NCU_TRAFFIC_BYTES.get((cfg.name, it.transfer_kernel())),
+        "frac": t_sfu / t_k3, "traffic": NCU_TRAFFIC_BYTES.get((cfg.name, it.transfer_kernel()), (None, None))[0],
+        "traffic_source": "stored ncu figure, not measured in this run: %s"
+                          % NCU_TRAFFIC_BYTES.get((cfg.name, it.transfer_kernel()), (None, "no capture for this workload / kernel"))[1],
         "peak_source": "148 SMs x 16 SFU lanes/clk (measured MUFU issue rate, profiles/r01_pipe_microbench.md) x %.0f MHz "
                        "max SM clock (MEASURED_PEAKS.json, %s)" % (peaks["sm_max_mhz"], peaks["source"]),
         "ms_per_launch": t_k3 * 1e3, "updates_evaluated": n_upd, "updates_nominal": updates,
