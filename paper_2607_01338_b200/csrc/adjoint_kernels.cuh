@@ -224,26 +224,28 @@ struct CentreProfile {
   }
 };
 
-// w(tau) = (1 - exp(-tau)) / tau and w'(tau) = (exp(-tau)(1 + tau) - 1) / tau^2, accurate for every tau.
-__device__ __forceinline__ void w_and_wprime(float tau, float m /* 1 - exp(-tau) */, float& w, float& wp) {
-  if (fabsf(tau) < 0.25f) {
-    float p = fmaf(tau, -1.0f / 5040.0f, 1.0f / 720.0f);
-    p = fmaf(p, tau, -1.0f / 120.0f);
-    p = fmaf(p, tau, 1.0f / 24.0f);
-    p = fmaf(p, tau, -1.0f / 6.0f);
-    p = fmaf(p, tau, 0.5f);
-    w = fmaf(-p, tau, 1.0f);                       // 1 - tau/2 + tau^2/6 - ...
-    float r = fmaf(tau, -1.0f / 5760.0f, 1.0f / 840.0f);
-    r = fmaf(r, tau, -1.0f / 144.0f);
-    r = fmaf(r, tau, 1.0f / 30.0f);
-    r = fmaf(r, tau, -0.125f);
-    r = fmaf(r, tau, 1.0f / 3.0f);
-    wp = fmaf(r, tau, -0.5f);                      // -1/2 + tau/3 - tau^2/8 + ...
-  } else {
-    const float it = rcp_approx(tau);
-    w = m * it;
-    wp = (fmaf(1.0f - m, 1.0f + tau, -1.0f)) * it * it;
-  }
+// w(tau) = (1 - exp(-tau)) / tau and w'(tau) = (exp(-tau)(1 + tau) - 1) / tau^2 from m = 1 - exp(-tau) and it = 1 / tau,
+// accurate for every tau: the closed form of w' loses a factor 2 / tau of relative accuracy to cancellation, and the
+// abundance gradient of a saturated line is itself a difference of an emission and an absorption term, so the series
+// take over below |tau| = 0.25 (both forms are evaluated and selected: no divergent branch).
+__device__ __forceinline__ void w_and_wprime(float tau, float m, float em /* exp(-tau) */, float it, float& w, float& wp) {
+  float p = fmaf(tau, -1.0f / 5040.0f, 1.0f / 720.0f);
+  p = fmaf(p, tau, -1.0f / 120.0f);
+  p = fmaf(p, tau, 1.0f / 24.0f);
+  p = fmaf(p, tau, -1.0f / 6.0f);
+  p = fmaf(p, tau, 0.5f);
+  const float ws = fmaf(-p, tau, 1.0f);                       // 1 - tau/2 + tau^2/6 - ...
+  float r = fmaf(tau, -1.0f / 5760.0f, 1.0f / 840.0f);
+  r = fmaf(r, tau, -1.0f / 144.0f);
+  r = fmaf(r, tau, 1.0f / 30.0f);
+  r = fmaf(r, tau, -0.125f);
+  r = fmaf(r, tau, 1.0f / 3.0f);
+  const float wps = fmaf(r, tau, -0.5f);                      // -1/2 + tau/3 - tau^2/8 + ...
+  const float wb = m * it;
+  const float wpb = fmaf(em, 1.0f + tau, -1.0f) * it * it;
+  const bool small = fabsf(tau) < 0.25f;
+  w = small ? ws : wb;
+  wp = small ? wps : wpb;
 }
 
 // Channel erf difference of channel c in a cell (both edges evaluated by the calling lane).
@@ -411,11 +413,15 @@ adjoint_march_kernel(MarchConsts mc, AdjointConsts ac, const float* __restrict__
         }
         xrem[k] = xr; P[k] = Pn; Q[k] = Qn;
         const float Tk = fmaf(Dto, invG, C);
-        const float mT = one_minus_exp_neg(tau_T);
+        // 1 - exp(-tau_T) = m_d + E_d m: no second exponential, and 1 / tau_T serves w, w' and the forward step
+        const float m = one_minus_exp_neg(tau_L);
+        const float mT = fmaf(E_d, m, m_d);
+        const float eT = E_d * (1.0f - m);                   // exp(-tau_T) itself (1 - mT would be rounding noise at large tau)
+        const float r = rcp_approx(fabsf(tau_T) < 1.0e-30f ? 1.0f : tau_T);
         float wT, wpT;
-        w_and_wprime(tau_T, mT, wT, wpT);
+        w_and_wprime(tau_T, mT, eT, r, wT, wpT);
         const float src = fmaf(S_d, tau_d, J_L);
-        const float dIdtau = fmaf(-Tk, 1.0f - mT, src * wpT);
+        const float dIdtau = fmaf(-Tk, eT, src * wpT);
         acc_e = fmaf(Pn * wT, dErf, acc_e);
         acc_a = fmaf(Pn * dIdtau, dErf, acc_a);
         acc_d = fmaf(Pn, fmaf(S_d, wT, dIdtau), acc_d);
@@ -423,8 +429,6 @@ adjoint_march_kernel(MarchConsts mc, AdjointConsts ac, const float* __restrict__
         // forward step (same cancellation-free form as transfer_window_kernel)
         float Dn;
         if (DUST) {
-          const float m = one_minus_exp_neg(tau_L);
-          const float r = rcp_approx(fabsf(tau_T) < 1.0e-30f ? 1.0f : tau_T);
           const float Em = E_d * m;
           const float t1 = m_d + Em;
           const float t2 = fmaf(tau_d, Em, -tau_L * m_d);
@@ -432,7 +436,7 @@ adjoint_march_kernel(MarchConsts mc, AdjointConsts ac, const float* __restrict__
           Dn = fmaf(-(Dto + CG), m, Dto);
           Dn = fmaf(Gn * r, num, Dn);
         } else {
-          Dn = update_nodust(Dto, dErf, a_c, sc);
+          Dn = fmaf(sc - Dto, m, Dto);      // D + (S_L - C - D) m
         }
         Dt[k] = Dn;
         if (DUST) winPD_new = fmaf(Pn, Dn, winPD_new);
