@@ -388,9 +388,21 @@ def bench_modes(torch, warmup):
         t = prof["transfer"][0] / 3 * 1e-3
         points = cfg.nv * (3 * (sub + 1) // 2 if sub else 1)      # (f + 1) / 2 Simpson panels x 3 points per channel
         out[name] = {"kernel": it.transfer_kernel(), "ms_per_launch": t * 1e3,
-                     "launches_per_call": prof["transfer"][1] / 3, "fell_back": it.smooth_fallback(),
+                     "launches_per_call": prof["transfer"][1] / 3, "pixels_handed_over": it.smooth_fallback(),
                      "point_updates_per_s": cfg.nx * cfg.ny * cfg.nz * points / t,
                      "ms_per_cube": sum(v[0] for v in prof.values()) / 3}
+        if m == 0 and it.transfer_kernel() != "transfer_modes_kernel":
+            # roofline of the thick modes on their line-window kernels: SFU operations per evaluated
+            # point update -- formal 3 (profile, exp(-tau_L), 1 / tau_T), smooth 2 (profile, 1 / (3 + 2 tau)) -- and 5 per
+            # (pixel, cell); evaluated = points inside the windows (formal) / inside the 12-cell hulls (smooth)
+            evaluated = it.transfer_work()
+            per_update = 2 if i == 1 else 3
+            ncell = cfg.nx * cfg.ny * cfg.nz
+            sfu = per_update * evaluated + 5 * ncell
+            t_floor = sfu / (SM_COUNT * SFU_LANES_PER_SM_CLK * measured_peaks()["sm_max_mhz"] * 1e6)
+            out[name]["roofline"] = {"bound": "alu", "pipe": "sfu", "updates_evaluated": evaluated, "sfu_per_update": per_update,
+                                     "floor_ms": t_floor * 1e3, "frac": t_floor / t,
+                                     "note": "time includes the list-driven dense launch for the pixels handed over"}
         it.close()
     return out
 

@@ -216,7 +216,10 @@ iris_so_status iris_so_profile_read(iris_so_ctx *ctx, int32_t stage, double *tot
 
 /* Work counter for roofline accounting: number of (cell, channel) updates inside the line windows of the
  * coefficient planes left in the context by the last transfer / observe call (the updates the line-window
- * algorithm evaluates; the dense algorithm evaluates nx*ny*nz*nv).  Synchronises the stream. */
+ * algorithm evaluates; the dense algorithm evaluates nx*ny*nz*nv).  With subsample > 0 the windows are counted in
+ * points of the fine velocity grid; with the smooth integrator on its line-window kernel (integration = 1, thick mode)
+ * the count is that of the points the kernel steps: per cell the hull of the windows of the last 12 cells.
+ * Synchronises the stream. */
 iris_so_status iris_so_transfer_work(iris_so_ctx *ctx, uint64_t *window_updates, void *cuda_stream);
 
 /* Name of the LOS transfer kernel this context launches ("transfer_series_kernel", "transfer_window_kernel",

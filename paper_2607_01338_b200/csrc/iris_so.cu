@@ -908,8 +908,16 @@ iris_so_status iris_so_transfer_work(iris_so_ctx* ctx, uint64_t* window_updates,
   if (!ctx->d_counter && (e = cudaMalloc(reinterpret_cast<void**>(&ctx->d_counter), sizeof(unsigned long long))) != cudaSuccess)
     return cuda_fail(ctx, e, "cudaMalloc(counter)");
   if ((e = cudaMemsetAsync(ctx->d_counter, 0, sizeof(unsigned long long), st)) != cudaSuccess) return cuda_fail(ctx, e, "memset");
-  iris::window_work_kernel<<<(unsigned)((ctx->ncell + 255) / 256), 256, 0, st>>>(ctx->d_coef, ctx->ncell, ctx->cfg.nv, ctx->d_counter);
-  IRIS_CHECK_LAUNCH(ctx, "window_work_kernel");
+  const int fine_m = ctx->cfg.subsample > 0 ? ctx->cfg.subsample + 1 : 0;
+  if (windowed_smooth_mode(ctx->cfg)) {
+    iris::hull_work_kernel<<<(unsigned)((ctx->npix + 127) / 128), 128, 0, st>>>(ctx->d_coef, ctx->ncell, (int)ctx->npix, ctx->cfg.nz,
+                                                                                ctx->cfg.nv, fine_m, iris::kSmoothKeep, ctx->d_counter);
+    IRIS_CHECK_LAUNCH(ctx, "hull_work_kernel");
+  } else {
+    iris::window_work_kernel<<<(unsigned)((ctx->ncell + 255) / 256), 256, 0, st>>>(ctx->d_coef, ctx->ncell, ctx->cfg.nv, fine_m,
+                                                                                   ctx->d_counter);
+    IRIS_CHECK_LAUNCH(ctx, "window_work_kernel");
+  }
   unsigned long long h = 0;
   if ((e = cudaMemcpyAsync(&h, ctx->d_counter, sizeof h, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(ctx, e, "D2H");
   if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(ctx, e, "cudaStreamSynchronize");

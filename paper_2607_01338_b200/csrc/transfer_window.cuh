@@ -32,17 +32,56 @@ __device__ __forceinline__ int line_window(float e_c, float a_c, float c_los, fl
   return (Xw2 > 0.0f) ? max(khi - klo + 1, 0) : 0;
 }
 
-// Sum of the window widths over all cells (work counter for roofline accounting).
-__global__ void __launch_bounds__(256) window_work_kernel(const float* __restrict__ coef, int64_t ncell, int nv,
+// Sum of the window widths over all cells (work counter for roofline accounting).  fine_m > 0: the windows on the fine
+// velocity grid of fine_m intervals per channel (points k / fine_m, as the series kernel's MODE 3 and the smooth window
+// kernel see them).
+__global__ void __launch_bounds__(256) window_work_kernel(const float* __restrict__ coef, int64_t ncell, int nv, int fine_m,
                                                           unsigned long long* __restrict__ total) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   int w = 0;
   if (i < ncell) {
     int klo, khi;
-    w = line_window(coef[i], coef[ncell + i], coef[2 * ncell + i], coef[3 * ncell + i], nv, klo, khi);
+    if (fine_m > 0)
+      w = line_window(coef[i], coef[ncell + i], fmaf(coef[2 * ncell + i], (float)fine_m, 0.5f), coef[3 * ncell + i] / (float)fine_m,
+                      nv * fine_m + 1, klo, khi);
+    else
+      w = line_window(coef[i], coef[ncell + i], coef[2 * ncell + i], coef[3 * ncell + i], nv, klo, khi);
   }
   w = __reduce_add_sync(0xffffffffu, w);
   if ((threadIdx.x & 31) == 0 && w) atomicAdd(total, (unsigned long long)w);
+}
+
+// Work of the smooth window kernel: per (pixel, cell) the points of the HULL of the windows of the last `keep` cells (the
+// union of the first two windows for the trapezoidal step).  One thread per pixel.
+__global__ void __launch_bounds__(128) hull_work_kernel(const float* __restrict__ coef, int64_t ncell, int npix, int nz, int nv,
+                                                        int fine_m, int keep, unsigned long long* __restrict__ total) {
+  const int pix = blockIdx.x * blockDim.x + threadIdx.x;
+  unsigned long long cnt = 0ull;
+  if (pix < npix) {
+    int lo[16], hi[16];
+#pragma unroll
+    for (int k = 0; k < 16; ++k) { lo[k] = 0x7fffffff; hi[k] = -1; }
+    const int npts = fine_m > 0 ? nv * fine_m + 1 : nv;
+    for (int z = 0; z < nz; ++z) {
+      const int64_t c = (int64_t)z * npix + pix;
+      int klo, khi;
+      const float cl = fine_m > 0 ? fmaf(coef[2 * ncell + c], (float)fine_m, 0.5f) : coef[2 * ncell + c];
+      const float s = fine_m > 0 ? coef[3 * ncell + c] / (float)fine_m : coef[3 * ncell + c];
+      const int W = line_window(coef[c], coef[ncell + c], cl, s, npts, klo, khi);
+      // shift the remembered windows (static indexing keeps them in registers)
+#pragma unroll
+      for (int k = 15; k > 0; --k) { lo[k] = lo[k - 1]; hi[k] = hi[k - 1]; }
+      lo[0] = W > 0 ? klo : 0x7fffffff; hi[0] = W > 0 ? khi : -1;
+      if (z == 0) continue;
+      int elo = 0x7fffffff, ehi = -1;
+#pragma unroll
+      for (int k = 0; k < 16; ++k)
+        if (k < keep) { elo = min(elo, lo[k]); ehi = max(ehi, hi[k]); }
+      if (ehi >= elo) cnt += (unsigned long long)(ehi - elo + 1);
+    }
+  }
+  cnt = __reduce_add_sync(0xffffffffu, (unsigned)min(cnt, 0xffffffffull));
+  if ((threadIdx.x & 31) == 0 && cnt) atomicAdd(total, cnt);
 }
 
 template <int LPP, bool DUST>
