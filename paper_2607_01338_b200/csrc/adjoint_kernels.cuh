@@ -22,6 +22,7 @@
 #include "cell_kernels.cuh"
 #include "transfer_common.cuh"
 #include "transfer_window.cuh"
+#include "transfer_series.cuh"      // packed f32x2 helpers
 
 namespace iris {
 
@@ -293,6 +294,53 @@ __device__ __forceinline__ void seg_sum8(float (&v)[8], unsigned gmask, int gbas
   for (int j = 0; j < 8; ++j) v[j] = __shfl_sync(gmask, r, gbase + (H / 4) * j);
 }
 
+// ---- packed pairs (two adjacent channels per lane; f32x2 helpers of transfer_series.cuh)
+__device__ __forceinline__ f32x2 sel2(bool c0, bool c1, f32x2 a, f32x2 b) {      // per half: c ? a : b
+  float a0, a1, b0, b1;
+  upk(a, a0, a1);
+  upk(b, b0, b1);
+  return pk(c0 ? a0 : b0, c1 ? a1 : b1);
+}
+
+// exp(-tau) and 1 - exp(-tau) of a pair, the latter accurate for every tau (Taylor below |tau| = 0.15, as one_minus_exp_neg)
+__device__ __forceinline__ void exp_and_omen2(f32x2 tau, f32x2& e, f32x2& m) {
+  float t0, t1;
+  upk(tau, t0, t1);
+  e = pk(ex2_approx(t0 * -1.4426950408889634f), ex2_approx(t1 * -1.4426950408889634f));
+  const f32x2 big = fma2(e, pk1(-1.0f), pk1(1.0f));
+  const f32x2 nt = mul2(tau, pk1(-1.0f));
+  f32x2 p = fma2(tau, pk1(-1.0f / 120.0f), pk1(1.0f / 24.0f));
+  p = fma2(p, nt, pk1(1.0f / 6.0f));
+  p = fma2(p, nt, pk1(0.5f));
+  p = fma2(p, nt, pk1(1.0f));
+  m = sel2(fabsf(t0) < 0.15f, fabsf(t1) < 0.15f, mul2(p, tau), big);
+}
+
+// w(tau) and w'(tau) of a pair (see w_and_wprime)
+__device__ __forceinline__ void w_and_wprime2(f32x2 tau, f32x2 m, f32x2 em, f32x2 it, f32x2& w, f32x2& wp) {
+  f32x2 p = fma2(tau, pk1(-1.0f / 5040.0f), pk1(1.0f / 720.0f));
+  p = fma2(p, tau, pk1(-1.0f / 120.0f));
+  p = fma2(p, tau, pk1(1.0f / 24.0f));
+  p = fma2(p, tau, pk1(-1.0f / 6.0f));
+  p = fma2(p, tau, pk1(0.5f));
+  const f32x2 ws = fma2(mul2(p, pk1(-1.0f)), tau, pk1(1.0f));
+  f32x2 r = fma2(tau, pk1(-1.0f / 5760.0f), pk1(1.0f / 840.0f));
+  r = fma2(r, tau, pk1(-1.0f / 144.0f));
+  r = fma2(r, tau, pk1(1.0f / 30.0f));
+  r = fma2(r, tau, pk1(-0.125f));
+  r = fma2(r, tau, pk1(1.0f / 3.0f));
+  const f32x2 wps = fma2(r, tau, pk1(-0.5f));
+  const f32x2 wb = mul2(m, it);
+  const f32x2 wpb = mul2(mul2(fma2(em, add2(tau, pk1(1.0f)), pk1(-1.0f)), it), it);
+  float t0, t1;
+  upk(tau, t0, t1);
+  const bool s0 = fabsf(t0) < 0.25f, s1 = fabsf(t1) < 0.25f;
+  w = sel2(s0, s1, ws, wb);
+  wp = sel2(s0, s1, wps, wpb);
+}
+
+constexpr int kAdjRecFields = 6;      // float4 fields of a march record (adjoint_march_kernel)
+
 // K8: LPP lanes per pixel, 32 / LPP pixels per warp (the launcher picks 16 or 32 from nv: five spectra per pixel live in
 // shared memory).  Shared memory per warp: 5 arrays (xrem, P, Q, Dt, what) of nvp * PPW floats, channel c
 // of pixel g at word (c / LPP) * 32 + g * LPP + c % LPP of its array (conflict-free for the lanes of a warp).  The
@@ -319,45 +367,76 @@ adjoint_march_kernel(MarchConsts mc, AdjointConsts ac, const float* __restrict__
   float* wh = Dt + arr;
 #define IDX(c) (((c) / LPP) * 32 + ((c) % LPP))
   float Wtot = 0.0f;
-  for (int c = i; c < nv; c += LPP) {
-    const float w = what[(int64_t)pix * nv + c];
+  for (int c = i; c < nvp; c += LPP) {                         // (the padding channels carry no weight)
+    const float w = c < nv ? what[(int64_t)pix * nv + c] : 0.0f;
     wh[IDX(c)] = w; xrem[IDX(c)] = 0.0f; Dt[IDX(c)] = 0.0f;
     Wtot += w;
   }
   Wtot = seg_sum<LPP>(Wtot, gmask);
   __syncwarp();
 
-  // first march: total line optical depth per channel and total dust optical depth
+  // Both marches are cut into chunks of LPP cells.  Phase A: the lane (pixel g, cell j) works out, ONCE, what depends on
+  // its cell only -- window, profile polynomial, dust factors, and the quantities that depend on the march so far (G,
+  // the continuum C, the dust depth passed) as prefix scans over the lanes of the pixel -- and leaves a record in shared
+  // memory.  Phase B: the LPP lanes of the pixel walk the cells, reading each record with broadcast LDS.128.
+  float4* rec = reinterpret_cast<float4*>(sm + (size_t)(blockDim.x >> 5) * 5 * arr) + (size_t)warp * (kAdjRecFields * 32);
+  const int rl0 = gbase;                                     // records of this pixel: rec[f * 32 + gbase + j]
+
+  // ---- first march: total line optical depth per channel and total dust optical depth
   float totD = 0.0f;
-  const float* p = coef + pix;
-  // both marches load the coefficients of a cell one cell ahead
-  float n_e = p[0], n_a = p[ncell], n_c = p[2 * ncell], n_s = p[3 * ncell];
-  float n_td = DUST ? p[4 * ncell] : 0.0f, n_sd = 0.0f;
-  for (int z = 0; z < nz; ++z) {
-    const float e_c = n_e, a_c = n_a, c_los = n_c, s = n_s;
-    if (DUST) totD += n_td;
-    if (z + 1 < nz) {
-      p += npix;
-      n_e = p[0]; n_a = p[ncell]; n_c = p[2 * ncell]; n_s = p[3 * ncell];
-      if (DUST) n_td = p[4 * ncell];
-    }
-    int klo, khi;
-    const int W = line_window(e_c, a_c, c_los, s, nv, klo, khi);
-    if (W > 0) {
+  {
+    const float* pc = coef + pix + (int64_t)i * npix;
+    float l_e = 0.0f, l_a = 0.0f, l_c = 0.0f, l_s = 1.0f, l_td = 0.0f;
+    if (i < nz) { l_e = pc[0]; l_a = pc[ncell]; l_c = pc[2 * ncell]; l_s = pc[3 * ncell]; if (DUST) l_td = pc[4 * ncell]; }
+    for (int z0 = 0; z0 < nz; z0 += LPP) {
+      const bool mine = z0 + i < nz;
+      const float e_c = l_e, a_c = l_a, c_los = l_c, s = l_s;
+      if (DUST && mine) totD += l_td;
+      l_e = 0.0f; l_a = 0.0f;
+      if (z0 + LPP + i < nz) {
+        pc += (int64_t)LPP * npix;
+        l_e = pc[0]; l_a = pc[ncell]; l_c = pc[2 * ncell]; l_s = pc[3 * ncell];
+        if (DUST) l_td = pc[4 * ncell];
+      }
+      int klo = 0, khi = -1;
+      const int W = mine ? line_window(e_c, a_c, c_los, s, nv, klo, khi) : 0;
       CentreProfile prof;
-      if (SERIES) prof.set(s);
-      for (int c = klo + i; c <= khi; c += LPP) {
-        const float dErf = SERIES ? prof.at(((float)c + 0.5f - c_los) * s) : channel_derf(c, c_los, s);
-        xrem[IDX(c)] = fmaf(a_c, dErf, xrem[IDX(c)]);
+      prof.set(s);
+      rec[lane] = make_float4(s, c_los, __int_as_float(W > 0 ? (klo | (khi << 16)) : 0x0000ffff), a_c);
+      rec[32 + lane] = make_float4(a_c * prof.p0, a_c * prof.p1, a_c * prof.p2, a_c * prof.p3);
+      rec[64 + lane] = make_float4(a_c * prof.p4, 0.0f, 0.0f, 0.0f);
+      __syncwarp();
+      const int ncz = min(LPP, nz - z0);
+      for (int j = 0; j < ncz; ++j) {
+        const float4 r0 = rec[rl0 + j];
+        const int wb = __float_as_int(r0.z), lo = wb & 0xffff, hi = (int)((unsigned)wb >> 16);
+        if (hi >= lo) {
+          CentreProfile pa;
+          if (SERIES) {
+            const float4 r1 = rec[32 + rl0 + j];
+            pa.p0 = r1.x; pa.p1 = r1.y; pa.p2 = r1.z; pa.p3 = r1.w; pa.p4 = rec[64 + rl0 + j].x;
+          }
+          // a lane takes the even-aligned PAIR of channels c, c + 1 (the window widened to pair boundaries: the extra
+          // channel lies beyond |x| = X_w, both marches treat it alike)
+          for (int c = (lo & ~1) + 2 * i; c <= hi; c += 2 * LPP) {
+            float2* xp = reinterpret_cast<float2*>(xrem + IDX(c));
+            const float d0 = SERIES ? pa.at(((float)c + 0.5f - r0.y) * r0.x) : r0.w * channel_derf(c, r0.y, r0.x);
+            const float d1 = SERIES ? pa.at(((float)c + 1.5f - r0.y) * r0.x) : r0.w * channel_derf(c + 1, r0.y, r0.x);
+            float2 v = *xp;
+            v.x += d0; v.y += d1;                              // (the polynomial carries a_c)
+            *xp = v;
+          }
+        }
+        __syncwarp();
       }
     }
-    __syncwarp();
+    totD = seg_sum<LPP>(totD, gmask);
   }
   // SQ = sum_c Q[c] and SPD = sum_c P[c] Dt[c] over ALL channels are carried as running sums: a cell changes
   // them only through the channels of its window, so the sums over the channels OUTSIDE the window (which only
   // the dust of the cell acts on) are SQ - sum_window Q and SPD - sum_window P Dt -- no pass over all nv channels.
   float SQ = 0.0f, SPD = 0.0f;
-  for (int c = i; c < nv; c += LPP) {
+  for (int c = i; c < nvp; c += LPP) {
     const float xr = xrem[IDX(c)], w = wh[IDX(c)];
     P[IDX(c)] = w * exp_neg(xr);
     const float q = w * one_minus_exp_neg(xr);
@@ -367,121 +446,201 @@ adjoint_march_kernel(MarchConsts mc, AdjointConsts ac, const float* __restrict__
   SQ = seg_sum<LPP>(SQ, gmask);
   __syncwarp();
 
-  // second march: forward state and closed-form adjoint together
-  float C = mc.T_bg, G = 1.0f, cumD = 0.0f;
-  p = coef + pix;
-  n_e = p[0]; n_a = p[ncell]; n_c = p[2 * ncell]; n_s = p[3 * ncell];
-  if (DUST) { n_td = p[4 * ncell]; n_sd = p[5 * ncell]; }
-  for (int z = 0; z < nz; ++z) {
-    const float e_c = n_e, a_c = n_a, c_los = n_c, s = n_s;
-    const float tau_d = DUST ? n_td : 0.0f, S_d = DUST ? n_sd : 0.0f;
-    if (z + 1 < nz) {
-      p += npix;
-      n_e = p[0]; n_a = p[ncell]; n_c = p[2 * ncell]; n_s = p[3 * ncell];
-      if (DUST) { n_td = p[4 * ncell]; n_sd = p[5 * ncell]; }
-    }
-    int klo, khi;
-    const int W = line_window(e_c, a_c, c_los, s, nv, klo, khi);
-    float E_d = 1.0f, m_d = 0.0f, Gn = 1.0f, Lam = 1.0f;
-    if (DUST) {
-      const float td_e = fminf(tau_d, kMaxTauDCell);
-      E_d = exp_neg(td_e);
-      m_d = one_minus_exp_neg(td_e);
-      Gn = G * ex2_approx(td_e * 1.4426950408889634f);
-      cumD += tau_d;
-      Lam = exp_neg(totD - cumD);                            // dust attenuation between this cell and the observer
-    }
-    const float invG = 1.0f / G, CG = C * G;
-    const float sc = DUST ? 0.0f : (a_c != 0.0f ? e_c / a_c : 0.0f) - C;
-    float acc_e = 0.0f, acc_a = 0.0f, acc_d = 0.0f, accW = 0.0f, accQ = 0.0f, accPD = 0.0f;
-    float winQ_old = 0.0f, winQ_new = 0.0f, winPD_old = 0.0f, winPD_new = 0.0f;
-    if (W > 0) {
-      CentreProfile prof;
-      if (SERIES) prof.set(s);
-      for (int c = klo + i; c <= khi; c += LPP) {
-        const int k = IDX(c);
-        const float dErf = SERIES ? prof.at(((float)c + 0.5f - c_los) * s) : channel_derf(c, c_los, s);
-        const float tau_L = a_c * dErf, J_L = e_c * dErf, tau_T = tau_L + tau_d;
-        const float xr = xrem[k] - tau_L;
-        const float w = wh[k];
-        const float Pn = w * exp_neg(xr);
-        const float Qn = w * one_minus_exp_neg(xr);
-        const float Dto = Dt[k];
-        if (DUST) {
-          winQ_old += Q[k]; winQ_new += Qn;
-          winPD_old = fmaf(P[k], Dto, winPD_old);
-        }
-        xrem[k] = xr; P[k] = Pn; Q[k] = Qn;
-        const float Tk = fmaf(Dto, invG, C);
-        // 1 - exp(-tau_T) = m_d + E_d m: no second exponential, and 1 / tau_T serves w, w' and the forward step
-        const float m = one_minus_exp_neg(tau_L);
-        const float mT = fmaf(E_d, m, m_d);
-        const float eT = E_d * (1.0f - m);                   // exp(-tau_T) itself (1 - mT would be rounding noise at large tau)
-        const float r = rcp_approx(fabsf(tau_T) < 1.0e-30f ? 1.0f : tau_T);
-        float wT, wpT;
-        w_and_wprime(tau_T, mT, eT, r, wT, wpT);
-        const float src = fmaf(S_d, tau_d, J_L);
-        const float dIdtau = fmaf(-Tk, eT, src * wpT);
-        acc_e = fmaf(Pn * wT, dErf, acc_e);
-        acc_a = fmaf(Pn * dIdtau, dErf, acc_a);
-        acc_d = fmaf(Pn, fmaf(S_d, wT, dIdtau), acc_d);
-        accW += w;
-        // forward step (same cancellation-free form as transfer_window_kernel)
-        float Dn;
-        if (DUST) {
-          const float Em = E_d * m;
-          const float t1 = m_d + Em;
-          const float t2 = fmaf(tau_d, Em, -tau_L * m_d);
-          const float num = fmaf(J_L, t1, S_d * t2);
-          Dn = fmaf(-(Dto + CG), m, Dto);
-          Dn = fmaf(Gn * r, num, Dn);
-        } else {
-          Dn = fmaf(sc - Dto, m, Dto);      // D + (S_L - C - D) m
-        }
-        Dt[k] = Dn;
-        if (DUST) winPD_new = fmaf(Pn, Dn, winPD_new);
+  // ---- second march: forward state and closed-form adjoint together
+  float C_run = mc.T_bg, G_run = 1.0f, D_run = 0.0f;         // continuum, exp(dust depth) since the last fold, dust depth passed
+  const float* pc = coef + pix + (int64_t)i * npix;
+  const float* pd = dcoef + pix + (int64_t)i * npix;
+  float l_e = 0.0f, l_a = 0.0f, l_c = 0.0f, l_s = 1.0f, l_td = 0.0f, l_sd = 0.0f, l_de = 0.0f, l_da = 0.0f;
+  if (i < nz) {
+    l_e = pc[0]; l_a = pc[ncell]; l_c = pc[2 * ncell]; l_s = pc[3 * ncell];
+    if (DUST) { l_td = pc[4 * ncell]; l_sd = pc[5 * ncell]; }
+    l_de = pd[0]; l_da = pd[ncell];
+  }
+  for (int z0 = 0; z0 < nz; z0 += LPP) {
+    // a chunk whose dust could take G out of the fp32 range is marched one cell at a time (G is folded in between)
+    float tsum = DUST ? fminf(l_td, kMaxTauDCell) : 0.0f;
+    if (z0 + i >= nz) tsum = 0.0f;
+    tsum = seg_sum<LPP>(tsum, gmask);
+    const int step = __any_sync(0xffffffffu, tsum > 60.0f) ? 1 : LPP;
+    for (int jlo = 0; jlo < LPP && z0 + jlo < nz; jlo += step) {
+      const int jhi = jlo + step;
+      const bool mine = i >= jlo && i < jhi && z0 + i < nz;
+      // ---- phase A
+      const float e_c = l_e, a_c = l_a, c_los = l_c, s = l_s;
+      const float tau_d = (DUST && mine) ? l_td : 0.0f, S_d = DUST ? l_sd : 0.0f;
+      int klo = 0, khi = -1;
+      const int W = mine ? line_window(e_c, a_c, c_los, s, nv, klo, khi) : 0;
+      float E_d = 1.0f, m_d = 0.0f, Eg = 1.0f;
+      if (DUST && mine) {
+        const float td_e = fminf(tau_d, kMaxTauDCell);
+        E_d = exp_neg(td_e);
+        m_d = one_minus_exp_neg(td_e);
+        Eg = ex2_approx(td_e * 1.4426950408889634f);
       }
-    }
-    if (!DUST) {
-      acc_e = seg_sum<LPP>(acc_e, gmask); acc_a = seg_sum<LPP>(acc_a, gmask);
-    } else {
-      if (W > 0) {                                           // W is the same for the LPP lanes of the pixel
-        float r8[8] = {acc_e, acc_a, acc_d, accW, winQ_old, winQ_new, winPD_old, winPD_new};
-        seg_sum8<LPP>(r8, gmask, gbase);
-        acc_e = r8[0]; acc_a = r8[1]; acc_d = r8[2]; accW = r8[3];
-        winQ_old = r8[4]; winQ_new = r8[5]; winPD_old = r8[6]; winPD_new = r8[7];
-      }
-      // channels outside the window: only the dust of this cell acts on them
-      accQ = SQ - winQ_old;
-      accPD = SPD - winPD_old;
-      SQ += winQ_new - winQ_old;
-      SPD += winPD_new - winPD_old;
-    }
-    if (i == 0 && valid) {
-      const int64_t cell = (int64_t)z * npix + pix;
-      const float pre = ac.scale * Lam;
-      float gr = pre * (acc_e * dcoef[cell] + acc_a * dcoef[ncell + cell]);
+      // prefix scans over the cells of the pixel: G (product), C (affine map x -> E_d x + S_d m_d), dust depth (sum)
+      float Pg = Eg, Ac = E_d, Bc = mine ? S_d * m_d : 0.0f, Ds = tau_d;
       if (DUST) {
-        const float sub = ac.subtract ? 1.0f : 0.0f;
-        const float dSC = S_d - C;
-        const float outside = fmaf(dSC, (1.0f - sub) * (Wtot - accW) - accQ, -invG * accPD);
-        const float g_d = pre * (acc_d - sub * E_d * dSC * accW + E_d * outside);
-        gr = fmaf(g_d, ac.c_d, gr);
+#pragma unroll
+        for (int o = 1; o < LPP; o <<= 1) {
+          const float Pp = __shfl_up_sync(0xffffffffu, Pg, o), Ap = __shfl_up_sync(0xffffffffu, Ac, o),
+                      Bp = __shfl_up_sync(0xffffffffu, Bc, o), Dp = __shfl_up_sync(0xffffffffu, Ds, o);
+          if (i >= o) { Pg *= Pp; Bc = fmaf(Ac, Bp, Bc); Ac *= Ap; Ds += Dp; }
+        }
       }
-      grad[cell] = gr;
-    }
-    if (DUST) {
-      C = fmaf(C, E_d, S_d * m_d);
-      G = Gn;
-      if (G > kFoldG) {                                     // the same for the LPP lanes of the pixel
-        const float inv = 1.0f / G;
+      float Pex = __shfl_up_sync(0xffffffffu, Pg, 1), Aex = __shfl_up_sync(0xffffffffu, Ac, 1), Bex = __shfl_up_sync(0xffffffffu, Bc, 1);
+      if (i == 0) { Pex = 1.0f; Aex = 1.0f; Bex = 0.0f; }
+      const float Gpre = G_run * Pex, Gn = Gpre * Eg, C = fmaf(C_run, Aex, Bex);
+      const float Lam = DUST ? exp_neg(totD - (D_run + Ds)) : 1.0f;      // dust attenuation between this cell and the observer
+      {
+        const int last = gbase + LPP - 1;
+        const float Pl = __shfl_sync(0xffffffffu, Pg, last), Al = __shfl_sync(0xffffffffu, Ac, last),
+                    Bl = __shfl_sync(0xffffffffu, Bc, last), Dl = __shfl_sync(0xffffffffu, Ds, last);
+        G_run *= Pl; C_run = fmaf(C_run, Al, Bl); D_run += Dl;
+      }
+      CentreProfile prof;
+      prof.set(s);
+      rec[lane] = make_float4(s, c_los, __int_as_float(W > 0 ? (klo | (khi << 16)) : 0x0000ffff), a_c);
+      rec[32 + lane] = make_float4(prof.p0, prof.p1, prof.p2, prof.p3);
+      rec[64 + lane] = make_float4(prof.p4, e_c, tau_d, S_d);
+      rec[96 + lane] = make_float4(E_d, m_d, 1.0f / Gpre, C);
+      rec[128 + lane] = make_float4(C * Gpre, Gn, DUST ? 0.0f : (a_c != 0.0f ? e_c / a_c : 0.0f) - C, ac.scale * Lam);
+      rec[160 + lane] = make_float4(l_de, l_da, 0.0f, 0.0f);
+      // the next chunk's coefficients, requested before the cells of this one are walked
+      if (jhi >= LPP || z0 + jhi >= nz) {
+        l_e = 0.0f; l_a = 0.0f; l_td = 0.0f;
+        if (z0 + LPP + i < nz) {
+          pc += (int64_t)LPP * npix; pd += (int64_t)LPP * npix;
+          l_e = pc[0]; l_a = pc[ncell]; l_c = pc[2 * ncell]; l_s = pc[3 * ncell];
+          if (DUST) { l_td = pc[4 * ncell]; l_sd = pc[5 * ncell]; }
+          l_de = pd[0]; l_da = pd[ncell];
+        }
+      }
+      __syncwarp();
+      // ---- phase B
+      const int jend = min(jhi, min(LPP, nz - z0));
+      for (int j = jlo; j < jend; ++j) {
+        const float4 r0 = rec[rl0 + j], r2 = rec[64 + rl0 + j], r3 = rec[96 + rl0 + j], r4 = rec[128 + rl0 + j];
+        const float sj = r0.x, cl = r0.y, aj = r0.w, ej = r2.y, tdj = r2.z, Sdj = r2.w;
+        const float Edj = r3.x, mdj = r3.y, invG = r3.z, Cj = r3.w, CGj = r4.x, Gnj = r4.y, scj = r4.z;
+        const int wb = __float_as_int(r0.z), lo = wb & 0xffff, hi = (int)((unsigned)wb >> 16);
+        float acc_e = 0.0f, acc_a = 0.0f, acc_d = 0.0f, accW = 0.0f, accQ = 0.0f, accPD = 0.0f;
+        float winQ_old = 0.0f, winQ_new = 0.0f, winPD_old = 0.0f, winPD_new = 0.0f;
+        if (hi >= lo) {
+          CentreProfile prof;
+          if (SERIES) {
+            const float4 r1 = rec[32 + rl0 + j];
+            prof.p0 = r1.x; prof.p1 = r1.y; prof.p2 = r1.z; prof.p3 = r1.w; prof.p4 = r2.x;
+          }
+          // pairs of channels with packed arithmetic (a window of ~20 channels is one pass of 16 lanes instead of two)
+          f32x2 Ae = pk1(0.0f), Aa = pk1(0.0f), Ad = pk1(0.0f), AW = pk1(0.0f), AQo = pk1(0.0f), AQn = pk1(0.0f), APo = pk1(0.0f),
+                APn = pk1(0.0f);
+          const f32x2 ac2 = pk1(aj), ec2 = pk1(ej), td2 = pk1(tdj), Ed2 = pk1(Edj), md2 = pk1(mdj), Sd2 = pk1(Sdj);
+          const f32x2 invG2 = pk1(invG), C2 = pk1(Cj), CG2 = pk1(CGj), Gn2 = pk1(Gnj), src0 = pk1(Sdj * tdj), sc2 = pk1(scj);
+          for (int c = (lo & ~1) + 2 * i; c <= hi; c += 2 * LPP) {
+            const int k = IDX(c);
+            const float d0 = SERIES ? prof.at(((float)c + 0.5f - cl) * sj) : channel_derf(c, cl, sj);
+            const float d1 = SERIES ? prof.at(((float)c + 1.5f - cl) * sj) : channel_derf(c + 1, cl, sj);
+            const f32x2 dErf = pk(d0, d1);
+            const f32x2 tau_L = mul2(ac2, dErf), J_L = mul2(ec2, dErf), tau_T = add2(tau_L, td2);
+            const float2 xo = *reinterpret_cast<const float2*>(xrem + k), wv = *reinterpret_cast<const float2*>(wh + k);
+            const float2 Do = *reinterpret_cast<const float2*>(Dt + k);
+            const f32x2 xr = fma2(tau_L, pk1(-1.0f), pk(xo.x, xo.y)), w = pk(wv.x, wv.y), Dto = pk(Do.x, Do.y);
+            f32x2 ex, mx;
+            exp_and_omen2(xr, ex, mx);
+            const f32x2 Pn = mul2(w, ex), Qn = mul2(w, mx);
+            if (DUST) {
+              const float2 Qo = *reinterpret_cast<const float2*>(Q + k), Po = *reinterpret_cast<const float2*>(P + k);
+              AQo = add2(AQo, pk(Qo.x, Qo.y)); AQn = add2(AQn, Qn);
+              APo = fma2(pk(Po.x, Po.y), Dto, APo);
+            }
+            {
+              float2 t;
+              upk(xr, t.x, t.y); *reinterpret_cast<float2*>(xrem + k) = t;
+              upk(Pn, t.x, t.y); *reinterpret_cast<float2*>(P + k) = t;
+              upk(Qn, t.x, t.y); *reinterpret_cast<float2*>(Q + k) = t;
+            }
+            const f32x2 Tk = fma2(Dto, invG2, C2);
+            // 1 - exp(-tau_T) = m_d + E_d m: no second exponential, and 1 / tau_T serves w, w' and the forward step
+            f32x2 eL, m;
+            exp_and_omen2(tau_L, eL, m);
+            const f32x2 mT = fma2(Ed2, m, md2);
+            const f32x2 eT = mul2(Ed2, fma2(m, pk1(-1.0f), pk1(1.0f)));      // exp(-tau_T) itself (1 - mT is rounding noise at large tau)
+            float tt0, tt1;
+            upk(tau_T, tt0, tt1);
+            const f32x2 r = pk(rcp_approx(fabsf(tt0) < 1.0e-30f ? 1.0f : tt0), rcp_approx(fabsf(tt1) < 1.0e-30f ? 1.0f : tt1));
+            f32x2 wT, wpT;
+            w_and_wprime2(tau_T, mT, eT, r, wT, wpT);
+            const f32x2 src = add2(src0, J_L);
+            const f32x2 dIdtau = fma2(mul2(Tk, pk1(-1.0f)), eT, mul2(src, wpT));
+            Ae = fma2(mul2(Pn, wT), dErf, Ae);
+            Aa = fma2(mul2(Pn, dIdtau), dErf, Aa);
+            Ad = fma2(Pn, fma2(Sd2, wT, dIdtau), Ad);
+            AW = add2(AW, w);
+            // forward step (same cancellation-free form as transfer_window_kernel)
+            f32x2 Dn;
+            if (DUST) {
+              const f32x2 Em = mul2(Ed2, m);
+              const f32x2 t1 = add2(md2, Em);
+              const f32x2 t2 = fma2(td2, Em, mul2(mul2(tau_L, md2), pk1(-1.0f)));
+              const f32x2 num = fma2(J_L, t1, mul2(Sd2, t2));
+              Dn = fma2(mul2(add2(Dto, CG2), pk1(-1.0f)), m, Dto);
+              Dn = fma2(mul2(Gn2, r), num, Dn);
+            } else {
+              Dn = fma2(add2(sc2, mul2(Dto, pk1(-1.0f))), m, Dto);      // D + (S_L - C - D) m
+            }
+            {
+              float2 t;
+              upk(Dn, t.x, t.y); *reinterpret_cast<float2*>(Dt + k) = t;
+            }
+            if (DUST) APn = fma2(Pn, Dn, APn);
+          }
+          {
+            float lo, hi;
+            upk(Ae, lo, hi); acc_e = lo + hi;  upk(Aa, lo, hi); acc_a = lo + hi;  upk(Ad, lo, hi); acc_d = lo + hi;
+            upk(AW, lo, hi); accW = lo + hi;   upk(AQo, lo, hi); winQ_old = lo + hi;  upk(AQn, lo, hi); winQ_new = lo + hi;
+            upk(APo, lo, hi); winPD_old = lo + hi;  upk(APn, lo, hi); winPD_new = lo + hi;
+          }
+        }
+        if (!DUST) {
+          acc_e = seg_sum<LPP>(acc_e, gmask); acc_a = seg_sum<LPP>(acc_a, gmask);
+        } else {
+          if (hi >= lo) {                                        // the same for the LPP lanes of the pixel
+            float r8[8] = {acc_e, acc_a, acc_d, accW, winQ_old, winQ_new, winPD_old, winPD_new};
+            seg_sum8<LPP>(r8, gmask, gbase);
+            acc_e = r8[0]; acc_a = r8[1]; acc_d = r8[2]; accW = r8[3];
+            winQ_old = r8[4]; winQ_new = r8[5]; winPD_old = r8[6]; winPD_new = r8[7];
+          }
+          // channels outside the window: only the dust of this cell acts on them
+          accQ = SQ - winQ_old;
+          accPD = SPD - winPD_old;
+          SQ += winQ_new - winQ_old;
+          SPD += winPD_new - winPD_old;
+        }
+        if (i == 0 && valid) {
+          const float4 r5 = rec[160 + rl0 + j];
+          const float pre = r4.w;
+          float gr = pre * (acc_e * r5.x + acc_a * r5.y);
+          if (DUST) {
+            const float sub = ac.subtract ? 1.0f : 0.0f;
+            const float dSC = Sdj - Cj;
+            const float outside = fmaf(dSC, (1.0f - sub) * (Wtot - accW) - accQ, -invG * accPD);
+            const float g_d = pre * (acc_d - sub * Edj * dSC * accW + Edj * outside);
+            gr = fmaf(g_d, ac.c_d, gr);
+          }
+          grad[(int64_t)(z0 + j) * npix + pix] = gr;
+        }
+        __syncwarp();
+      }
+      // fold the accumulated dust attenuation into the stored forward state (keeps G inside the fp32 range); rare
+      if (DUST && G_run > kFoldG) {                            // the same for the LPP lanes of the pixel
+        const float inv = 1.0f / G_run;
         __syncwarp(gmask);
-        for (int c = i; c < nv; c += LPP) Dt[IDX(c)] *= inv;
+        for (int c = i; c < nvp; c += LPP) Dt[IDX(c)] *= inv;
         SPD *= inv;
-        G = 1.0f;
+        G_run = 1.0f;
       }
+      __syncwarp();
     }
-    __syncwarp();
   }
 #undef IDX
 }
@@ -534,7 +693,7 @@ march:
   const int lpp = nv <= 384 ? 16 : 32;
   const int ppw = 32 / lpp;
   const int nvp = (nv + lpp - 1) / lpp * lpp;
-  const size_t per_warp = (size_t)5 * nvp * ppw * sizeof(float);
+  const size_t per_warp = (size_t)5 * nvp * ppw * sizeof(float) + (size_t)kAdjRecFields * 32 * sizeof(float4);   // spectra + march records
   int wpc = 4;
   while (wpc > 1 && wpc * per_warp > 200 * 1024) wpc >>= 1;
   const size_t smem = wpc * per_warp;

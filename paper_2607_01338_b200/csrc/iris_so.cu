@@ -969,7 +969,7 @@ static iris_so_status observe_adjoint_impl(iris_so_ctx* ctx, const float* d_nH2,
   if (c.dust_per_channel)
     return fail(ctx, IRIS_SO_EUNSUPPORTED, "adjoint is not available with dust_per_channel = 1");
   // the adjoint march keeps five spectra per pixel in shared memory (one warp per pixel beyond 384 channels)
-  if ((size_t)5 * (((size_t)c.nv + 31) / 32 * 32) * sizeof(float) > 227u * 1024u)
+  if ((size_t)5 * (((size_t)c.nv + 31) / 32 * 32) * sizeof(float) + (size_t)iris::kAdjRecFields * 32 * sizeof(float4) > 227u * 1024u)
     return fail(ctx, IRIS_SO_EUNSUPPORTED, "adjoint: five spectra of this many channels do not fit the shared memory of an SM");
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   iris_so_status s = run_coefficients(ctx, d_nH2, d_Tgas, d_Tdust, d_vlos, nullptr, st);
