@@ -225,6 +225,20 @@ struct CentreProfile {
   }
 };
 
+// ---- packed pairs (two adjacent channels per lane; f32x2 helpers of transfer_series.cuh)
+// CentreProfile::at for the pair of channels at x and x + s
+__device__ __forceinline__ f32x2 centre_profile_pair(const CentreProfile& p, float x, float s) {
+  const f32x2 xx = pk(x, x + s);
+  const f32x2 u = mul2(xx, xx);
+  f32x2 pol = fma2(pk1(p.p4), u, pk1(p.p3));
+  pol = fma2(pol, u, pk1(p.p2));
+  pol = fma2(pol, u, pk1(p.p1));
+  pol = fma2(pol, u, pk1(p.p0));
+  float u0, u1;
+  upk(u, u0, u1);
+  return mul2(pol, pk(ex2_approx(-1.4426950408889634f * u0), ex2_approx(-1.4426950408889634f * u1)));
+}
+
 // w(tau) = (1 - exp(-tau)) / tau and w'(tau) = (exp(-tau)(1 + tau) - 1) / tau^2 from m = 1 - exp(-tau) and it = 1 / tau,
 // accurate for every tau: the closed form of w' loses a factor 2 / tau of relative accuracy to cancellation, and the
 // abundance gradient of a saturated line is itself a difference of an emission and an absorption term, so the series
@@ -294,7 +308,6 @@ __device__ __forceinline__ void seg_sum8(float (&v)[8], unsigned gmask, int gbas
   for (int j = 0; j < 8; ++j) v[j] = __shfl_sync(gmask, r, gbase + (H / 4) * j);
 }
 
-// ---- packed pairs (two adjacent channels per lane; f32x2 helpers of transfer_series.cuh)
 __device__ __forceinline__ f32x2 sel2(bool c0, bool c1, f32x2 a, f32x2 b) {      // per half: c ? a : b
   float a0, a1, b0, b1;
   upk(a, a0, a1);
@@ -420,10 +433,12 @@ adjoint_march_kernel(MarchConsts mc, AdjointConsts ac, const float* __restrict__
           // channel lies beyond |x| = X_w, both marches treat it alike)
           for (int c = (lo & ~1) + 2 * i; c <= hi; c += 2 * LPP) {
             float2* xp = reinterpret_cast<float2*>(xrem + IDX(c));
-            const float d0 = SERIES ? pa.at(((float)c + 0.5f - r0.y) * r0.x) : r0.w * channel_derf(c, r0.y, r0.x);
-            const float d1 = SERIES ? pa.at(((float)c + 1.5f - r0.y) * r0.x) : r0.w * channel_derf(c + 1, r0.y, r0.x);
+            f32x2 dd;
+            if (SERIES) dd = centre_profile_pair(pa, ((float)c + 0.5f - r0.y) * r0.x, r0.x);      // (the polynomial carries a_c)
+            else dd = pk(r0.w * channel_derf(c, r0.y, r0.x), r0.w * channel_derf(c + 1, r0.y, r0.x));
             float2 v = *xp;
-            v.x += d0; v.y += d1;                              // (the polynomial carries a_c)
+            const f32x2 nv2 = add2(pk(v.x, v.y), dd);
+            upk(nv2, v.x, v.y);
             *xp = v;
           }
         }
@@ -538,9 +553,9 @@ adjoint_march_kernel(MarchConsts mc, AdjointConsts ac, const float* __restrict__
           const f32x2 invG2 = pk1(invG), C2 = pk1(Cj), CG2 = pk1(CGj), Gn2 = pk1(Gnj), src0 = pk1(Sdj * tdj), sc2 = pk1(scj);
           for (int c = (lo & ~1) + 2 * i; c <= hi; c += 2 * LPP) {
             const int k = IDX(c);
-            const float d0 = SERIES ? prof.at(((float)c + 0.5f - cl) * sj) : channel_derf(c, cl, sj);
-            const float d1 = SERIES ? prof.at(((float)c + 1.5f - cl) * sj) : channel_derf(c + 1, cl, sj);
-            const f32x2 dErf = pk(d0, d1);
+            f32x2 dErf;
+            if (SERIES) dErf = centre_profile_pair(prof, ((float)c + 0.5f - cl) * sj, sj);
+            else dErf = pk(channel_derf(c, cl, sj), channel_derf(c + 1, cl, sj));
             const f32x2 tau_L = mul2(ac2, dErf), J_L = mul2(ec2, dErf), tau_T = add2(tau_L, td2);
             const float2 xo = *reinterpret_cast<const float2*>(xrem + k), wv = *reinterpret_cast<const float2*>(wh + k);
             const float2 Do = *reinterpret_cast<const float2*>(Dt + k);
