@@ -288,7 +288,9 @@ def bench_workload(torch, dist, name, algo, steps, warmup, rank, peaks, want_e2e
     res = dict(cfg=cfg, fields=fields, value=value, ms=ms_max, ms_per_step=ms_max / steps, launches=launches, clocks=clocks,
                stages={k: {"ms_per_step": v[0] / steps, "launches_per_step": v[1] / steps} for k, v in prof.items() if v[1]})
     # roofline of the dominant kernel (LOS transfer): the slower of HBM bytes, SFU operations and FP32 operations
-    t_k3 = prof["transfer"][0] / max(prof["transfer"][1], 1) * 1e-3          # seconds per launch
+    # seconds per step of the transfer stage (the series kernel with reachable-range spectra is two launches: the
+    # circular-buffer variant, then the whole-spectrum variant over the pixels it handed over)
+    t_k3 = prof["transfer"][0] / steps * 1e-3
     ncell = cfg.nx * cfg.ny * cfg.nz
     win_updates = it.transfer_work()
     dense_kernel = it.transfer_kernel() == "transfer_dense_kernel"

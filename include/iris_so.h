@@ -232,8 +232,12 @@ const char *iris_so_transfer_kernel(const iris_so_ctx *ctx);
  * on the dominant solution of the homogeneous BDF2 step (Eq. 4.8.10), both of which the kernel detects per
  * pixel: it lists the pixel, and the dense kernel, launched right after it and driven by that list, recomputes the
  * listed pixels.  *fell_back = the number of pixels that were handed over in the last transfer / observe call of this
- * context (for iris_so_observe_host: summed over the slabs of pixel rows of that call); 0 for every other mode.
- * Synchronises the stream. */
+ * context (for iris_so_observe_host: summed over the slabs of pixel rows of that call).
+ * The hot path hands pixels over too: its line-window kernel keeps, per pixel, a circular buffer of half the band
+ * ("reachable-range spectra": a pixel's lines only touch the channels its line-of-sight velocities reach) whenever that
+ * lets more warps stay resident, and a pixel whose lines span more than the buffer is recomputed by the same kernel with
+ * whole spectra; the count is reported here as well (the library stops using the buffers once more than 3 % of the
+ * pixels of a launch had to be recomputed).  0 for every other mode.  Synchronises the stream. */
 iris_so_status iris_so_smooth_fallback(iris_so_ctx *ctx, int32_t *fell_back, void *cuda_stream);
 
 /* Stand-alone post-processing stages (also used inside iris_so_observe). */

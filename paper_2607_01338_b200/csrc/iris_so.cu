@@ -71,6 +71,12 @@ struct iris_so_ctx {
                                   // [1] their number accumulated over the launches of one public call (slabs of the host path),
                                   // [2 ..] the list of those pixels (npix entries)
   double* d_metrics = nullptr;
+  // reachable-range spectra of the series kernel (transfer_series.cuh, CIRC): used while few pixels have to be handed over
+  bool circ_ok = true;
+  int* h_hand = nullptr;          // pinned: pixels handed over by the last launch that used them
+  cudaEvent_t ev_hand = nullptr;  // recorded after the copy into h_hand
+  bool hand_pending = false;
+  int64_t hand_npix = 0;          // pixels of that launch
   cudaStream_t s_in = nullptr, s_out = nullptr;      // copy streams of the host-buffer path
   std::vector<cudaEvent_t> slab_events;
 };
@@ -489,21 +495,57 @@ iris_so_status run_transfer(iris_so_ctx* ctx, const iris::MarchConsts& mc, float
     IRIS_CHECK_LAUNCH(ctx, "transfer_dense_kernel");
     return IRIS_SO_OK;
   }
-  cudaError_t e = algo == IRIS_SO_ALGO_WINDOW
-                      ? iris::launch_transfer_series(mc, ctx->d_coef, ctx->ncell, npix, nz, nv, dust,
-                                                     (float)(ctx->cfg.dv_cms / ctx->cfg.microturb_cms), out, out_cont, st)
-                      : iris::launch_transfer_window(mc, ctx->d_coef, ctx->ncell, npix, nz, nv, dust, ctx->sm_count, out, out_cont, st);
+  cudaError_t e;
+  if (algo == IRIS_SO_ALGO_WINDOW) {
+    // reachable-range spectra (half-size circular buffers, transfer_series.cuh) while at most 3 % of the pixels of the
+    // previous launch had to be handed over to the whole-spectrum variant
+    if (ctx->hand_pending && cudaEventQuery(ctx->ev_hand) == cudaSuccess) {
+      if ((int64_t)*ctx->h_hand * 100 > 3 * ctx->hand_npix) ctx->circ_ok = false;
+      ctx->hand_pending = false;
+    }
+    cudaGetLastError();
+    int* hand = (ctx->circ_ok && ctx->d_gate) ? ctx->d_gate : nullptr;
+    if (hand && (e = cudaMemsetAsync(hand, 0, sizeof(int), st)) != cudaSuccess) return cuda_fail(ctx, e, "cudaMemsetAsync(hand-over count)");
+    int used_circ = 0;
+    e = iris::launch_transfer_series(mc, ctx->d_coef, ctx->ncell, npix, nz, nv, dust,
+                                     (float)(ctx->cfg.dv_cms / ctx->cfg.microturb_cms), out, out_cont, st, 0, hand, &used_circ);
+    if (used_circ) {
+      ctx->launches++;
+      if (e == cudaSuccess && ctx->h_hand && !ctx->hand_pending) {
+        cudaMemcpyAsync(ctx->h_hand, hand, sizeof(int), cudaMemcpyDeviceToHost, st);
+        cudaEventRecord(ctx->ev_hand, st);
+        ctx->hand_pending = true;
+        ctx->hand_npix = npix;
+      }
+    }
+  } else {
+    e = iris::launch_transfer_window(mc, ctx->d_coef, ctx->ncell, npix, nz, nv, dust, ctx->sm_count, out, out_cont, st);
+  }
   ctx->launches++;
   if (e != cudaSuccess) return cuda_fail(ctx, e, "launch of the line-window transfer kernel");
   return IRIS_SO_OK;
 }
 
-// Start of a public call that runs the transfer: clears the accumulated fallback flag of the smooth window kernel.
+// Kernels that hand pixels over to a second launch: the smooth window kernel, and the series kernel of the hot path with
+// reachable-range spectra.
+bool uses_handover(const iris_so_config& c) {
+  return windowed_smooth_mode(c) ||
+         (hot_path_mode(c) && !c.dust_per_channel && resolved_algo(c) == IRIS_SO_ALGO_WINDOW && spectra_fit_shared(c));
+}
+
+// Start of a public call that runs the transfer: clears the accumulated hand-over count.
 iris_so_status begin_call(iris_so_ctx* ctx, cudaStream_t st) {
-  if (!windowed_smooth_mode(ctx->cfg)) return IRIS_SO_OK;
+  if (!uses_handover(ctx->cfg)) return IRIS_SO_OK;
   cudaError_t e;
-  if (!ctx->d_gate && (e = cudaMalloc(reinterpret_cast<void**>(&ctx->d_gate), (2 + (size_t)ctx->npix) * sizeof(int))) != cudaSuccess)
-    return cuda_fail(ctx, e, "cudaMalloc(gate)");
+  if (!ctx->d_gate) {
+    if ((e = cudaMalloc(reinterpret_cast<void**>(&ctx->d_gate), (2 + (size_t)ctx->npix) * sizeof(int))) != cudaSuccess)
+      return cuda_fail(ctx, e, "cudaMalloc(gate)");
+    if (cudaHostAlloc(reinterpret_cast<void**>(&ctx->h_hand), sizeof(int), cudaHostAllocDefault) != cudaSuccess ||
+        cudaEventCreateWithFlags(&ctx->ev_hand, cudaEventDisableTiming) != cudaSuccess) {
+      cudaGetLastError();
+      if (ctx->h_hand) { cudaFreeHost(ctx->h_hand); ctx->h_hand = nullptr; }      // no feedback: the choice stays as it is
+    }
+  }
   if ((e = cudaMemsetAsync(ctx->d_gate, 0, 2 * sizeof(int), st)) != cudaSuccess) return cuda_fail(ctx, e, "cudaMemsetAsync(gate)");
   return IRIS_SO_OK;
 }
@@ -725,6 +767,8 @@ iris_so_status iris_so_create(const iris_so_config* cfg, iris_so_ctx** out) {
 void iris_so_destroy(iris_so_ctx* ctx) {
   if (!ctx) return;
   cudaFree(ctx->d_coef); cudaFree(ctx->d_tmp); cudaFree(ctx->d_stage); cudaFree(ctx->d_adj); cudaFree(ctx->d_counter); cudaFree(ctx->d_gate); cudaFree(ctx->d_metrics); cudaFree(ctx->d_colltab); cudaFree(ctx->d_grid);
+  if (ctx->h_hand) cudaFreeHost(ctx->h_hand);
+  if (ctx->ev_hand) cudaEventDestroy(ctx->ev_hand);
   if (ctx->s_in) cudaStreamDestroy(ctx->s_in);
   if (ctx->s_out) cudaStreamDestroy(ctx->s_out);
   for (auto ev : ctx->slab_events) cudaEventDestroy(ev);
@@ -929,7 +973,7 @@ iris_so_status iris_so_smooth_fallback(iris_so_ctx* ctx, int32_t* fell_back, voi
   if (!ctx) return IRIS_SO_EINVAL;
   if (!fell_back) return fail(ctx, IRIS_SO_EINVAL, "iris_so_smooth_fallback: NULL output");
   *fell_back = 0;
-  if (!ctx->d_gate || !windowed_smooth_mode(ctx->cfg)) return IRIS_SO_OK;
+  if (!ctx->d_gate || !uses_handover(ctx->cfg)) return IRIS_SO_OK;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   int h = 0;
   cudaError_t e;

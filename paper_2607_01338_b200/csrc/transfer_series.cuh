@@ -182,15 +182,20 @@ struct SeriesCellOps {
 // that 2 P independent dependency chains are in flight (the SM issues in order: a lane-serial update would leave
 // the issue slot idle for the latency of every MUFU / FMA of the chain).  d: the lane's words of pair q; pairs at
 // or beyond qend are computed but neither loaded nor stored.  xx: scaled centres of the two channels of pair q.
-template <bool DUST, int DEG, int LPP, int P, int MODE = 0>
-__device__ __forceinline__ void series_passes(float* d, int q, int qend, f32x2 xx, f32x2 step2, const SeriesCellOps& o) {
+// CIRC: the spectra are circular buffers of rmask + 1 rows (see the kernel); col = the lane's column of its first row, row its
+// first row: pass k works on row (row + k) & rmask.
+template <bool DUST, int DEG, int LPP, int P, int MODE = 0, bool CIRC = false>
+__device__ __forceinline__ void series_passes(float* col, int row, int rmask, f32x2 xx, f32x2 step2, const SeriesCellOps& o) {
+  float* dk[P];
+#pragma unroll
+  for (int k = 0; k < P; ++k) dk[k] = col + (CIRC ? ((row + k) & rmask) : (row + k)) * 64;
   constexpr float L1 = 0.6931471805599453f, L2 = L1 * L1, L3 = L2 * L1, L4 = L2 * L2;
   const f32x2 ONE = pk1(1.0f), NEG1 = pk1(-1.0f);
   const f32x2 C4 = pk1(L4 / 24.0f), C3 = pk1(-L3 / 6.0f), C2 = pk1(L2 / 2.0f), C1 = pk1(-L1);   // -(1 - 2^-t) / t
   f32x2 Dt[P], u[P], pol[P], t[P], mn[P], qq[P];
 #pragma unroll
   for (int k = 0; k < P; ++k) {
-    const float2 v = *reinterpret_cast<const float2*>(d + 64 * k);
+    const float2 v = *reinterpret_cast<const float2*>(dk[k]);
     Dt[k] = pk(v.x, v.y);
     u[k] = mul2(xx, xx);
     xx = add2(xx, step2);
@@ -221,7 +226,7 @@ __device__ __forceinline__ void series_passes(float* d, int q, int qend, f32x2 x
       }
       float2 w;
       upk(Dt[k], w.x, w.y);
-      *reinterpret_cast<float2*>(d + 64 * k) = w;
+      *reinterpret_cast<float2*>(dk[k]) = w;
     }
   } else {
   float t0[P], t1[P], f0[P], f1[P];
@@ -272,19 +277,26 @@ __device__ __forceinline__ void series_passes(float* d, int q, int qend, f32x2 x
   for (int k = 0; k < P; ++k) {
     float2 v;
     upk(Dt[k], v.x, v.y);
-    *reinterpret_cast<float2*>(d + 64 * k) = v;
+    *reinterpret_cast<float2*>(dk[k]) = v;
   }
   }
-  (void)q; (void)qend;
 }
 
 // __launch_bounds__ names a minimum of 3 CTAs per SM (what the 1024-channel spectra allow): without it ptxas holds the
 // kernel to 68 registers and schedules the two pair-passes of the loop back to back; with it it takes 86 registers and
 // overlaps them (large: 6.61 -> 6.27 ms).
-template <int LPP, bool DUST, int DEG, int MODE>
+// CIRC (reachable-range spectra): a pixel's lines only ever touch the channels its line-of-sight velocities reach, a
+// fraction of the band, but whole spectra of 4 pixels per warp are what limits the resident warps (12 per SM at 1024
+// channels).  With CIRC a spectrum is a CIRCULAR buffer of rb = rmask + 1 rows of LPP pairs (a power of two, half the band or
+// less): row r of the spectrum lives in buffer row r & rmask, which is one-to-one as long as the rows a pixel has
+// touched so far span at most rb rows.  The kernel tracks that span per pixel; a pixel that exceeds it is appended to
+// the hand-over list `hand` ([0] count of this launch, [1] count since the public call began, [2..] pixel indices) and a
+// second launch of the full-size variant over that list (`plist`, `pcount`) recomputes it.  Rows never touched are zero.
+template <int LPP, bool DUST, int DEG, int MODE, bool CIRC = false>
 __global__ void __launch_bounds__(128, 3)
 transfer_series_kernel(MarchConsts mc, const float* __restrict__ coef, int64_t ncell, int npix, int nz, int nv,
-                       int nvp, float* __restrict__ out, float* __restrict__ out_cont) {
+                       int nvp, float* __restrict__ out, float* __restrict__ out_cont, int rmask, int* __restrict__ hand,
+                       const int* __restrict__ plist, const int* __restrict__ pcount) {
   extern __shared__ float4 smem4[];
   constexpr int PPW = 32 / LPP;
   constexpr int NQ = SeriesLayout<DUST, DEG>::NQ;
@@ -292,22 +304,29 @@ transfer_series_kernel(MarchConsts mc, const float* __restrict__ coef, int64_t n
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, wpc = blockDim.x >> 5;
   const int g = lane / LPP, i = lane % LPP;
   const int pix0 = (blockIdx.x * wpc + warp) * PPW;
-  const int pix = pix0 + g;
+  // list-driven launch: the warp's pixels are entries pix0 .. pix0 + PPW - 1 of the list
+  const int nlist = plist != nullptr ? *pcount : 0;
+  if (plist != nullptr && pix0 >= nlist) return;
+  auto pixel_of = [&](int slot) { return plist != nullptr ? (slot < nlist ? plist[slot] : npix) : slot; };
+  const int pix = pixel_of(pix0 + g);
   const bool valid = pix < npix;
-  const int npair = nvp / 2;                    // nvp is a multiple of 2 LPP
+  const int nvb = CIRC ? (rmask + 1) * 2 * LPP : nvp;      // points of the buffer that holds a spectrum
+  const int npair = nvb / 2;                    // nvp is a multiple of 2 LPP
   const int npts = MODE == 3 ? nv * mc.fine_m + 1 : nv;      // spectral points held per pixel
   // shared memory: records [wpc][NQ][32], then spectra [wpc][npair / LPP rows][ROW]
   float4* rec = smem4 + (size_t)warp * (NQ * 32);
   float* spec = reinterpret_cast<float*>(smem4 + (size_t)wpc * (NQ * 32));
-  float* sp = spec + (size_t)warp * nvp * PPW + g * (2 * LPP);      // pair q of this pixel: sp[(q / LPP) * ROW + (q % LPP) * 2]
+  float* sp = spec + (size_t)warp * nvb * PPW + g * (2 * LPP);      // pair q of this pixel: sp[(q / LPP) * ROW + (q % LPP) * 2]
   for (int q = i; q < npair; q += LPP) *reinterpret_cast<float2*>(sp + (q / LPP) * ROW + i * 2) = make_float2(0.0f, 0.0f);
 
   float C = mc.T_bg;      // continuum before the current cell
   float G = 1.0f;         // exp(dust optical depth accumulated so far), since the last rescale
+  int row_min = 0x3fffffff, row_max = -1;       // CIRC: rows of the spectrum pixel ga (= lane % PPW) has touched
+  bool overflow = false;                        // CIRC: they no longer fit the buffer
 
   // phase A: lane L makes record L of the chunk = (cell L / PPW, pixel L % PPW)
   const int ja = lane / PPW, ga = lane % PPW;
-  const float* p = coef + min(pix0 + ga, npix - 1) + (int64_t)ja * npix;
+  const float* p = coef + min(pixel_of(pix0 + ga), npix - 1) + (int64_t)ja * npix;
   float l_e = 0.0f, l_a = 0.0f, l_c = 0.0f, l_s = 1.0f, l_td = 0.0f, l_sd = 0.0f;
   if (ja < nz) {
     l_e = p[0]; l_a = p[ncell]; l_c = p[2 * ncell]; l_s = p[3 * ncell];
@@ -351,21 +370,22 @@ transfer_series_kernel(MarchConsts mc, const float* __restrict__ coef, int64_t n
       o.p4 = pk1(DUST ? q3.z : q2.x);
       o.tdp_or_nsc = pk1(q0.z);
       o.CG = pk1(CG); o.Pn = pk1(Pn); o.nQn = pk1(Qn); o.nRn = pk1(Rn);
-      int q = qlo + i;
-      const int qend = qlo + nq;                   // one past the last pair of the window
+      const int q = qlo + i;
       const float x = fmaf((float)(2 * i), q0.y, q0.x);
       f32x2 xx = pk(x, x + q0.y);
       const f32x2 step2 = pk1((float)(2 * LPP) * q0.y);
-      float* d = sp + (q / LPP) * ROW + (q % LPP) * 2;
+      float* col = sp + (q % LPP) * 2;             // the lane's column; pass k works on row q / LPP + k
+      int row = q / LPP;
       // (checked build) the pairs of every pass of this lane lie inside the spectra of this warp
-      IRIS_CHECK_SMEM(d, 8, spec + (size_t)warp * nvp * PPW, spec + (size_t)(warp + 1) * nvp * PPW);
-      IRIS_CHECK_SMEM(d + (npass - 1) * ROW, 8, spec + (size_t)warp * nvp * PPW, spec + (size_t)(warp + 1) * nvp * PPW);
+      IRIS_CHECK_SMEM(col + (CIRC ? (row & rmask) : row) * ROW, 8, spec + (size_t)warp * nvb * PPW, spec + (size_t)(warp + 1) * nvb * PPW);
+      IRIS_CHECK_SMEM(col + (CIRC ? ((row + npass - 1) & rmask) : row + npass - 1) * ROW, 8, spec + (size_t)warp * nvb * PPW,
+                      spec + (size_t)(warp + 1) * nvb * PPW);
       int rem = npass;
       while (rem >= 2) {
-        series_passes<DUST, DEG, LPP, 2, MODE>(d, q, qend, xx, step2, o);
-        xx = add2(xx, add2(step2, step2)); q += 2 * LPP; d += 2 * ROW; rem -= 2;
+        series_passes<DUST, DEG, LPP, 2, MODE, CIRC>(col, row, rmask, xx, step2, o);
+        xx = add2(xx, add2(step2, step2)); row += 2; rem -= 2;
       }
-      if (rem == 1) series_passes<DUST, DEG, LPP, 1, MODE>(d, q, qend, xx, step2, o);
+      if (rem == 1) series_passes<DUST, DEG, LPP, 1, MODE, CIRC>(col, row, rmask, xx, step2, o);
     }
     if (DUST && G > kFoldG) rescale_spectrum();
   };
@@ -378,6 +398,20 @@ transfer_series_kernel(MarchConsts mc, const float* __restrict__ coef, int64_t n
       if (MODE == 2 && mc.ray_simpson) wn = ray_simpson_weight(z0 + ja, nz);
       const SeriesRecord r = make_series_record<DUST, DEG, MODE>(l_e, l_a, l_c, l_s, l_td, l_sd, mc.T_bg, npts, mc.fine_m, wn);
       chunk_busy = __any_sync(0xffffffffu, ((unsigned)__float_as_int(r.q0.w) >> 16) != 0u);   // also: phase B is done
+      if (CIRC) {
+        // rows of the spectrum the chunk touches, per pixel ga (lanes ga, ga + PPW, ...): qlo / LPP .. (qlo + LPP npass - 1) / LPP
+        const int kk = __float_as_int(r.q0.w), qlo_r = kk & 0xffff, nq_r = (int)((unsigned)kk >> 16);
+        int lo = nq_r > 0 ? qlo_r / LPP : 0x3fffffff;
+        int hi = nq_r > 0 ? (qlo_r + (nq_r + LPP - 1) / LPP * LPP - 1) / LPP : -1;
+#pragma unroll
+        for (int o = PPW; o < 32; o <<= 1) {
+          lo = min(lo, __shfl_xor_sync(0xffffffffu, lo, o));
+          hi = max(hi, __shfl_xor_sync(0xffffffffu, hi, o));
+        }
+        row_min = min(row_min, lo);
+        row_max = max(row_max, hi);
+        if (row_max - row_min > rmask) overflow = true;      // (noticed after the fact: the pixel is recomputed anyway)
+      }
       rec[lane] = r.q0;
       rec[32 + lane] = r.q1;
       if (NQ > 2) rec[64 + lane] = r.q2;
@@ -425,13 +459,28 @@ transfer_series_kernel(MarchConsts mc, const float* __restrict__ coef, int64_t n
   }
   __syncwarp();
 
+  if (CIRC) {
+    // the range of THIS lane's pixel g is held by the lanes with ga = g (lane g is one of them)
+    row_min = __shfl_sync(0xffffffffu, row_min, g);
+    row_max = __shfl_sync(0xffffffffu, row_max, g);
+    overflow = __shfl_sync(0xffffffffu, (int)overflow, g) != 0;
+    // hand the pixel over when its rows did not fit the buffer (the full-size variant recomputes it)
+    if (overflow && valid && i == 0) { hand[2 + atomicAdd(hand, 1)] = pix; atomicAdd(hand + 1, 1); }
+  }
+  // buffer word of pair q (q = i + LPP row for this lane); CIRC: rows outside the touched range are zero
+  auto pair_at = [&](int q) {
+    const int row = q / LPP;
+    if (!CIRC) return *reinterpret_cast<const float2*>(sp + row * ROW + (q % LPP) * 2);
+    if (row < row_min || row > row_max) return make_float2(0.0f, 0.0f);
+    return *reinterpret_cast<const float2*>(sp + (row & rmask) * ROW + (q % LPP) * 2);
+  };
   const float invG = 1.0f / G;
   if (MODE == 3) {
     // Simpson's rule over the m + 1 points of every channel (Eq. 4.5.1), then subtraction / conversion
     if (valid && out != nullptr) {
       const int m = mc.fine_m;
       const float wgt = invG / (3.0f * (float)m);
-      auto point = [&](int k) { return sp[((k >> 1) / LPP) * ROW + ((k >> 1) % LPP) * 2 + (k & 1)]; };
+      auto point = [&](int k) { const float2 v = pair_at(k >> 1); return (k & 1) ? v.y : v.x; };
       for (int c = i; c < nv; c += LPP) {
         float acc = 0.0f;
         for (int j = 0; j < m; j += 2) acc += point(c * m + j) + 4.0f * point(c * m + j + 1) + point(c * m + j + 2);
@@ -446,7 +495,7 @@ transfer_series_kernel(MarchConsts mc, const float* __restrict__ coef, int64_t n
       float* o = out + (int64_t)pix * nv;
       const bool al = ((((int64_t)pix * nv) & 1) == 0);      // float2 stores need an even element offset
       for (int q = i; 2 * q < nv; q += LPP) {
-        const float2 v = *reinterpret_cast<const float2*>(sp + (q / LPP) * ROW + i * 2);
+        const float2 v = pair_at(q);
         const float r0 = convert_out(v.x * invG, C, mc);
         if (2 * q + 1 < nv) {
           const float r1 = convert_out(v.y * invG, C, mc);
@@ -461,9 +510,28 @@ transfer_series_kernel(MarchConsts mc, const float* __restrict__ coef, int64_t n
   }
 }
 
+// Warps per CTA that leave most warps resident for `per_warp` bytes of shared memory per warp, and that number of warps
+// (shared memory and, through the occupancy query, registers).
+template <typename Kernel>
+inline void series_residency(Kernel kernel, size_t per_warp, int& wpc, int& resident) {
+  wpc = 1; resident = 0;
+  for (int w = 4; w >= 1; w >>= 1) {
+    const size_t smem = w * per_warp;
+    if (smem + 1024 > 227 * 1024) continue;
+    if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) { cudaGetLastError(); continue; }
+    int nb = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kernel, w * 32, smem) != cudaSuccess) { cudaGetLastError(); continue; }
+    if (nb * w > resident) { resident = nb * w; wpc = w; }
+  }
+}
+
+// hand: nullptr, or the hand-over buffer of the context ([0] zeroed by the caller): the reachable-range variant (CIRC) is
+// then used when it keeps at least a quarter more warps resident than whole spectra, followed by the full-size variant
+// over the pixels it handed over.  *used_circ reports the choice.
 template <int LPP, bool DUST, int DEG, int MODE = 0>
 inline cudaError_t launch_transfer_series_t(const MarchConsts& mc, const float* coef, int64_t ncell, int npix, int nz,
-                                            int nv, float* out, float* out_cont, cudaStream_t st) {
+                                            int nv, float* out, float* out_cont, cudaStream_t st, int* hand = nullptr,
+                                            int* used_circ = nullptr) {
   constexpr int PPW = 32 / LPP;
   constexpr int NQ = SeriesLayout<DUST, DEG>::NQ;
   const int npts = MODE == 3 ? nv * mc.fine_m + 1 : nv;
@@ -472,40 +540,65 @@ inline cudaError_t launch_transfer_series_t(const MarchConsts& mc, const float* 
   const int nvp = (npts + 2 * LPP - 1) / (2 * LPP) * (2 * LPP) + 2 * LPP;
   const size_t rec_per_warp = (size_t)NQ * 32 * sizeof(float4);
   const size_t spec_per_warp = (size_t)PPW * nvp * sizeof(float);
-  // warps per CTA: the count that leaves most warps resident in the 227 KB of an SM (ties: the larger CTA)
   int wpc = 1, best = 0;
-  for (int w = 4; w >= 1; w >>= 1) {
-    const size_t per_cta = w * (rec_per_warp + spec_per_warp) + 1024;
-    const int resident = per_cta <= 227 * 1024 ? (int)((227 * 1024) / per_cta) * w : 0;
-    if (resident > best) { best = resident; wpc = w; }
-  }
+  series_residency(transfer_series_kernel<LPP, DUST, DEG, MODE, false>, rec_per_warp + spec_per_warp, wpc, best);
+  if (best == 0) return cudaErrorInvalidConfiguration;
   const size_t smem = wpc * (rec_per_warp + spec_per_warp);
-  if (smem > 227 * 1024) return cudaErrorInvalidConfiguration;
   const int ppc = wpc * PPW;
   const unsigned grid = (unsigned)((npix + ppc - 1) / ppc);
-  cudaError_t e = cudaFuncSetAttribute(transfer_series_kernel<LPP, DUST, DEG, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                       (int)smem);
+  cudaError_t e;
+  if (used_circ) *used_circ = 0;
+  if constexpr (MODE == 0) {
+    if (hand != nullptr) {
+      // circular buffers of rb rows: the largest power of two that is at most half the rows of a whole spectrum
+      const int rows_full = nvp / (2 * LPP);
+      int rb = 8;
+      while (2 * rb * 2 <= rows_full) rb <<= 1;
+      const size_t circ_per_warp = rec_per_warp + (size_t)PPW * rb * 2 * LPP * sizeof(float);
+      int wpc_c = 1, best_c = 0;
+      if (2 * rb <= rows_full) series_residency(transfer_series_kernel<LPP, DUST, DEG, 0, true>, circ_per_warp, wpc_c, best_c);
+      if (4 * best_c >= 5 * best) {
+        const size_t smem_c = wpc_c * circ_per_warp;
+        const int ppc_c = wpc_c * PPW;
+        if ((e = cudaFuncSetAttribute(transfer_series_kernel<LPP, DUST, DEG, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      (int)smem_c)) != cudaSuccess) return e;
+        transfer_series_kernel<LPP, DUST, DEG, 0, true><<<(unsigned)((npix + ppc_c - 1) / ppc_c), wpc_c * 32, smem_c, st>>>(
+            mc, coef, ncell, npix, nz, nv, nvp, out, out_cont, rb - 1, hand, nullptr, nullptr);
+        if ((e = cudaGetLastError()) != cudaSuccess) return e;
+        if (used_circ) *used_circ = 1;
+        // the pixels it handed over, with whole spectra (the warps beyond the list return at once)
+        if ((e = cudaFuncSetAttribute(transfer_series_kernel<LPP, DUST, DEG, 0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      (int)smem)) != cudaSuccess) return e;
+        transfer_series_kernel<LPP, DUST, DEG, 0, false><<<grid, wpc * 32, smem, st>>>(mc, coef, ncell, npix, nz, nv, nvp, out, out_cont, 0,
+                                                                                     nullptr, hand + 2, hand);
+        return cudaGetLastError();
+      }
+    }
+  }
+  e = cudaFuncSetAttribute(transfer_series_kernel<LPP, DUST, DEG, MODE, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
-  transfer_series_kernel<LPP, DUST, DEG, MODE><<<grid, wpc * 32, smem, st>>>(mc, coef, ncell, npix, nz, nv, nvp, out, out_cont);
+  transfer_series_kernel<LPP, DUST, DEG, MODE, false><<<grid, wpc * 32, smem, st>>>(mc, coef, ncell, npix, nz, nv, nvp, out, out_cont, 0,
+                                                                                 nullptr, nullptr, nullptr);
   return cudaGetLastError();
 }
 
 // s_max: upper bound of dv / b over all cells (dv / microturbulence); selects the polynomial degree.
 // mode: 0 optically thick, 1 selectively thin, 2 optically thin (formal integration, channel-integrated profile), 3 optically
 // thick on the fine velocity grid of mc.fine_m intervals per channel; modes 1 - 3 always run the dust instantiation
-// (tau_d = S_d = 0 planes when the dust is off).
+// (tau_d = S_d = 0 planes when the dust is off).  hand / used_circ: see launch_transfer_series_t (mode 0 only).
 inline cudaError_t launch_transfer_series(const MarchConsts& mc, const float* coef, int64_t ncell, int npix, int nz, int nv,
-                                          bool dust, float s_max, float* out, float* out_cont, cudaStream_t st, int mode = 0) {
+                                          bool dust, float s_max, float* out, float* out_cont, cudaStream_t st, int mode = 0,
+                                          int* hand = nullptr, int* used_circ = nullptr) {
   const bool deg3 = s_max <= kSeriesDeg3MaxS;
   if (mode == 1) return deg3 ? launch_transfer_series_t<8, true, 3, 1>(mc, coef, ncell, npix, nz, nv, out, out_cont, st)
                              : launch_transfer_series_t<8, true, 4, 1>(mc, coef, ncell, npix, nz, nv, out, out_cont, st);
   if (mode == 2) return deg3 ? launch_transfer_series_t<8, true, 3, 2>(mc, coef, ncell, npix, nz, nv, out, out_cont, st)
                              : launch_transfer_series_t<8, true, 4, 2>(mc, coef, ncell, npix, nz, nv, out, out_cont, st);
   if (mode == 3) return launch_transfer_series_t<8, true, 3, 3>(mc, coef, ncell, npix, nz, nv, out, out_cont, st);
-  if (dust) return deg3 ? launch_transfer_series_t<8, true, 3>(mc, coef, ncell, npix, nz, nv, out, out_cont, st)
-                        : launch_transfer_series_t<8, true, 4>(mc, coef, ncell, npix, nz, nv, out, out_cont, st);
-  return deg3 ? launch_transfer_series_t<8, false, 3>(mc, coef, ncell, npix, nz, nv, out, out_cont, st)
-              : launch_transfer_series_t<8, false, 4>(mc, coef, ncell, npix, nz, nv, out, out_cont, st);
+  if (dust) return deg3 ? launch_transfer_series_t<8, true, 3>(mc, coef, ncell, npix, nz, nv, out, out_cont, st, hand, used_circ)
+                        : launch_transfer_series_t<8, true, 4>(mc, coef, ncell, npix, nz, nv, out, out_cont, st, hand, used_circ);
+  return deg3 ? launch_transfer_series_t<8, false, 3>(mc, coef, ncell, npix, nz, nv, out, out_cont, st, hand, used_circ)
+              : launch_transfer_series_t<8, false, 4>(mc, coef, ncell, npix, nz, nv, out, out_cont, st, hand, used_circ);
 }
 
 }  // namespace iris

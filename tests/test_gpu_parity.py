@@ -578,3 +578,39 @@ def test_dust_per_channel_unsupported_combinations():
     with pytest.raises(IrisSOError) as e:
         it.transfer(*dev_fields(f), I_cont=torch.empty((cfg.ny, cfg.nx), dtype=torch.float32, device="cuda"))
     assert e.value.status == 2
+
+
+# ------------------------------------------------------------------------------------------------
+# reachable-range spectra of the series kernel (circular half-band buffers + hand-over to whole spectra)
+@pytest.mark.parametrize("wide_columns", [0, 1, 4])
+def test_reachable_range_spectra_hand_over(wide_columns):
+    """1024 channels: whole spectra of 4 pixels per warp limit the resident warps, so the hot path keeps a circular buffer
+    of half the band per pixel.  Pixels whose lines stay inside a quarter of the band are marched in the buffers; pixels
+    whose line-of-sight velocity swings across the whole band (the first `wide_columns` pixels of every row) do not fit,
+    are handed over and recomputed with whole spectra.  Either way the cube is the oracle's; once more than 3 % of the
+    pixels of a call had to be recomputed the library goes back to whole spectra."""
+    cfg, r = make_workload("small", nx=64, ny=4, nz=64, nv=1024)
+    cfg = cfg.with_(dv_cms=0.25e5, v0_cms=(0.5 - 512) * 0.25e5)
+    f = make_fields(cfg, r)
+    f["vlos"] = (0.2 * f["vlos"]).astype(np.float32)                        # lines within +-25 km/s: 200 of 1024 channels
+    rng = np.random.default_rng(3)
+    if wide_columns:
+        f["vlos"][:, :, :wide_columns] = rng.uniform(-110e5, 110e5, (cfg.nz, cfg.ny, wide_columns)).astype(np.float32)
+    ref = Oracle(cfg).observe(f)
+    it = iris(cfg)
+    assert it.transfer_kernel() == "transfer_series_kernel"
+    d = dev_fields(f)
+    cube = it.observe(*d).cpu().numpy()
+    n1 = it.smooth_fallback()
+    assert n1 == cfg.ny * wide_columns, "pixels handed over"
+    worst = assert_spectra(cube, ref, what="reachable-range spectra, %d wide columns" % wide_columns)
+    cube2 = it.observe(*d).cpu().numpy()
+    n2 = it.smooth_fallback()
+    # 4 of 64 columns = 6 % of the pixels: the second call marches whole spectra (nothing to hand over); 1 of 64 stays
+    assert n2 == (0 if wide_columns == 4 else n1)
+    assert np.array_equal(cube2, cube) or wide_columns == 4
+    assert_spectra(cube2, ref, what="second call")
+    # the dense kernel and the erfc-edge window kernel never use the buffers
+    assert iris(cfg, 1).smooth_fallback() == 0
+    print("reachable-range spectra, %d wide columns: %d / %d pixels handed over, worst pixel at %.3g of tolerance"
+          % (wide_columns, n1, n2, worst))
