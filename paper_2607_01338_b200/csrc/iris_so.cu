@@ -289,6 +289,7 @@ void fold_constants(iris_so_ctx* ctx) {
   mc.out_mode = out_mode_of(c);
   mc.fine_m = 0;
   mc.ray_simpson = 0;
+  mc.sel_thin = 0;
   mc.v0_over_c = (float)(c.v0_cms / C_LIGHT);
   mc.dv_over_c = (float)(c.dv_cms / C_LIGHT);
   mc.hnu_k_over_Tcmb = c.T_cmb > 0.0 ? (float)(H_PLANCK * nu / K_BOLTZ / c.T_cmb) : 0.0f;
@@ -427,7 +428,7 @@ bool windowed_fine_mode(const iris_so_config& c) {
 // Optically thick transfer with the smooth integrator as a line-window march (transfer_smooth.cuh), followed by the
 // dense modes kernel gated on the flag the window kernel raises when a ReLU fires where it does not look.
 bool windowed_smooth_mode(const iris_so_config& c) {
-  if (!(c.transfer_mode == 0 && c.integration == 1 && c.transfer_algo != IRIS_SO_ALGO_DENSE && c.nz >= 2)) return false;
+  if (!((c.transfer_mode == 0 || c.transfer_mode == 1) && c.integration == 1 && c.transfer_algo != IRIS_SO_ALGO_DENSE && c.nz >= 2)) return false;
   if (c.subsample == 0 && !(c.microturb_cms > 0.0 && c.dv_cms <= (double)iris::kSeriesMaxS * c.microturb_cms)) return false;
   return iris::smooth_window_smem_per_warp(c.nv, c.subsample > 0 ? c.subsample + 1 : 0) + 1024 <= 227u * 1024u;
 }
@@ -469,6 +470,7 @@ iris_so_status run_transfer(iris_so_ctx* ctx, const iris::MarchConsts& mc, float
       if (e != cudaSuccess) return cuda_fail(ctx, e, "cudaMemsetAsync(gate)");
       iris::MarchConsts mf = mc;
       mf.fine_m = md.fine_m;
+      mf.sel_thin = ctx->cfg.transfer_mode == 1;
       e = iris::launch_transfer_smooth_window(mf, ctx->d_coef, ctx->ncell, npix, nz, nv, out, out_cont, ctx->d_gate,
                                               ctx->d_gate + 2, st);
       ctx->launches++;

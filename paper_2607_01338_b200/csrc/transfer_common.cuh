@@ -63,6 +63,7 @@ struct MarchConsts {
   // dust_per_channel = 1 (dense kernel only): channel k is observed at nu_k = nu0 (1 - v_k / c)
   float v0_over_c, dv_over_c;   // v_k / c = v0_over_c + k dv_over_c
   float hnu_k_over_Tcmb;        // h nu0 / (k T_cmb); 0 = no background
+  int sel_thin;     // smooth window kernel only: 1 = selectively thin mode (the line does not absorb itself, Eq. 4.8.13)
 };
 
 // Planck function at nu = r nu0 in the units of the march (Rayleigh-Jeans Kelvin AT nu0: I c^2 / (2 k nu0^2)), for

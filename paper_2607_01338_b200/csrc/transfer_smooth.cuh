@@ -1,10 +1,11 @@
 // K3 with the SMOOTH integrator (trapezoidal first step Eq. 4.8.12, BDF2 Eq. 4.8.10, ReLU of PAPER.md:709) in the
-// optically thick mode, as a LINE-WINDOW march: the windowed counterpart of transfer_modes_kernel<0, true, *>.
+// optically thick and the selectively thin mode, as a LINE-WINDOW march: the windowed counterpart of
+// transfer_modes_kernel<0 / 1, true, *>.
 //
 // Same difference form as transfer_modes.cuh (D = I^[T] - I^[C] next to the scalar continuum C):
 //   n = 0     D_0 = 0
 //   n = 1     D_1 = [(E_0 - A_0 C_0) + (E_1 - A_1 C_1) + (2 - a_0) D_0] / (2 + a_1)
-//   n >= 2    D_n = [2 (E_n - A_n C_n) + 4 D_n-1 - D_n-2] / (3 + 2 a_n),     a_n = A_n + tau_d,n
+//   n >= 2    D_n = [2 (E_n - A_n C_n) + 4 D_n-1 - D_n-2] / (3 + 2 a_n),     a_n = A_n + tau_d,n  (thick)
 // with E = e_c p, A = a_c p for the profile weight p of the point in the cell, and the ReLU on D + C and on C.
 //
 // Why a window works.  Where a cell has no line (p = 0) the step is the homogeneous recurrence
@@ -40,9 +41,13 @@
 // record with broadcast LDS.128 and updating the points of its hull, two passes of 32 points staged together.  Cells 0
 // and 1 (initial value, trapezoidal step) are done before the chunks.
 //
-// (The selectively thin mode is NOT run this way: its absorption saturates at I^[T] = 0, i.e. the ReLU keeps acting on
-// points long after the line has left them, and the gate fires on every thick workload; measured: 3.5 + 5.8 ms against
-// 5.8 ms for the dense kernel alone on the medium cube.)
+// Selectively thin mode (MarchConsts::sel_thin, Eq. 4.8.13 - 4.8.15): a_n = tau_d, i.e. the same steps with the line
+// opacity taken out of the two denominators; nothing else changes.  Its absorption saturates at I^[T] = 0 (the ReLU
+// clamps D at -C_n) inside the hull, where every step is explicit.  A point that was clamped and then released carries
+// a = (I_m - C_m) / d_m, and a d_n + C_n = I_m d_n / d_m + (C_n - C_m d_n / d_m) is the attenuated intensity plus what the
+// dust has emitted since: not negative unless the recessive solution or rounding makes it so, which the far-point test
+// catches per pixel (8 of the medium cube's 65536 pixels; with the per-CUBE gate of the first version every thick workload
+// went to the dense kernel, which is why this mode used to stay there).
 //
 // Mapping as in transfer_window.cuh: LPP = 16 lanes per pixel, 2 pixels per warp, both spectra of a pixel in shared
 // memory, point k at word (k / LPP) * 32 + g * LPP + k % LPP of its array.  Profile: the point value of Eq. 3.3.3 on
@@ -117,6 +122,8 @@ transfer_smooth_window_kernel(MarchConsts mc, const float* __restrict__ coef, in
   const bool valid = pix_raw < npix;
   const int pix = valid ? pix_raw : npix - 1;                   // idle groups shadow the last pixel and write nothing
   const int m = mc.fine_m;
+  const float self_abs = mc.sel_thin ? 0.0f : 1.0f;   // selectively thin mode: a_n = tau_d, the line term drops out of
+                                                      // the denominators of Eq. 4.8.10 / 4.8.12 and nothing else changes
   constexpr bool point = POINT;           // fine grid with the point profile (m > 0) or channel integrals (m = 0)
   const int npts = point ? nv * m + 1 : nv;
   const size_t arr = (size_t)nvp * PPW;
@@ -171,7 +178,7 @@ transfer_smooth_window_kernel(MarchConsts mc, const float* __restrict__ coef, in
         const float pw = prof.at(xs);
         const float pw0 = prof0.at(((float)k + 0.5f - c_0) * (s_0 * SQL2E));
         const float E = e_c * pw, A = a_c * pw, E0 = e_0 * pw0, A0 = a_0 * pw0;
-        const float Du = ((E0 - A0 * mc.T_bg) + (E - A * C_unc)) * rcp_approx(2.0f + A + td);
+        const float Du = ((E0 - A0 * mc.T_bg) + (E - A * C_unc)) * rcp_approx(fmaf(self_abs, A, 2.0f + td));
         const float U = fmaxf(Du + relu_add, relu_min);                  // ReLU on D + C and on C; d_1 = 1
         IRIS_CHECK_SMEM(specB + IDX(k), 4, lo_ok, hi_ok);
         specB[IDX(k)] = U;
@@ -293,7 +300,7 @@ transfer_smooth_window_kernel(MarchConsts mc, const float* __restrict__ coef, in
       const float xb = s * SQL2E;
       const int elo = 0xffff - (int)(hull & 0xffffu), ehi = (int)(hull >> 16);
       const bool any = mine && ehi >= elo;
-      rec[lane] = make_float4(2.0f * fmaf(-a_c, C_unc, e_c), 2.0f * a_c, fmaf(2.0f, td, 3.0f), rcp_approx(d_n));
+      rec[lane] = make_float4(2.0f * fmaf(-a_c, C_unc, e_c), 2.0f * self_abs * a_c, fmaf(2.0f, td, 3.0f), rcp_approx(d_n));
       rec[32 + lane] = make_float4(4.0f * d_n1, -d_n2, C_unc >= 0.0f ? 0.0f : C_unc, C_unc >= 0.0f ? -C_unc : 0.0f);
       rec[64 + lane] = make_float4(xb, (0.5f - c_los) * xb, __int_as_float(any ? (elo | (ehi << 16)) : 0x0000ffff), d_n);
       rec[96 + lane] = make_float4(prof.p0, prof.p1, prof.p2, prof.p3);

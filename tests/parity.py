@@ -48,3 +48,25 @@ def assert_spectra(gpu, ora, floor=1e-6, rel=1e-4, extra=0.0, peak_of=None, what
     worst = float(ex.max())
     assert worst <= 1.0, "%s: worst pixel is at %.3g x the tolerance (1e-4 peak + floor)" % (what, worst)
     return worst
+
+
+def selthin_source_allowance(cfg, fields):
+    """Float32 rounding allowance [npix, nv] (Kelvin) of the selectively thin mode with the smooth integrator
+    (DESIGN.md "Tolerances").  Its step  D_n = [2 (E_n - A_n C_n) + 4 D_n-1 - D_n-2] / (3 + 2 tau_d)  has no line opacity
+    in the denominator (Eq. 4.8.13 - 4.8.15: the line does not absorb itself), so the products E_n = e p and A_n C_n
+    enter at full size whatever the optical depth, each formed by up to four float32 roundings (2^-22 relative), and the
+    root 1 of the BDF2 recurrence keeps every one of them: |error| <= 2^-22 sum_n (E_n + A_n C_n) beside the usual
+    1e-4 peak + 1e-6 K.  The sum is bounded with the oracle alone: C_n <= C_max = max(I_bg, max_n S_d,n) (a continuum never
+    exceeds its largest source), and sum_n h p (j0 + kappa0 C_max) is the optically thin formal march (Eq. 4.7.6) of the
+    column with j0 replaced by j0 + kappa0 C_max, minus its continuum.  A factor 2 covers the worst-case sign pattern."""
+    from oracle import Oracle
+    plane = cfg.nx * cfg.ny
+    c_thin = cfg.with_(transfer_mode=2, integration=0, subsample=0, subtract_continuum=False, out_unit=0)
+    o = Oracle(c_thin)
+    coef = o.coefficients(fields["nH2"], fields["Tgas"], fields["Tdust"])
+    I_bg = o.planck(cfg.nu0_Hz, cfg.T_cmb)
+    C_max = np.maximum(I_bg, coef[4].reshape(cfg.nz, plane).max(axis=0))
+    c2 = coef.copy()
+    c2[0] = coef[0] + coef[1] * np.tile(C_max, cfg.nz)
+    S, S_cont = o.march(c2, fields["vlos"])
+    return 2.0 ** -21 * krj(cfg.nu0_Hz) * (S - S_cont[:, None])

@@ -9,19 +9,20 @@ torch = pytest.importorskip("torch")
 from iris_inputs import make_fields, make_workload
 from iris_inputs.fields import KMS
 from oracle import Oracle
-from parity import assert_spectra, krj
+from parity import assert_spectra, selthin_source_allowance, krj
 
 pytestmark = pytest.mark.gpu
 
 # (transfer_mode, integration, subsample).  The formal modes (thin and selectively thin with the channel-integrated
-# profile, thick on the fine grid) run through the line-window series kernel by default and the thick smooth modes
-# through the line-window smooth kernel; the "_dense" entries force transfer_modes_kernel (transfer_algo = 1).
+# profile, thick on the fine grid) run through the line-window series kernel by default and the thick and selectively
+# thin smooth modes through the line-window smooth kernel; the "_dense" entries force transfer_modes_kernel (transfer_algo = 1).
 MODES = {"thin_formal": (2, 0, 0), "thin_smooth": (2, 1, 0), "selthin_formal": (1, 0, 0), "selthin_smooth": (1, 1, 0),
          "thick_smooth": (0, 1, 0), "thick_formal_sub1": (0, 0, 1), "thick_formal_sub3": (0, 0, 3),
          "thick_smooth_sub1": (0, 1, 1), "thick_smooth_sub7": (0, 1, 7),
          "thin_formal_dense": (2, 0, 0), "selthin_formal_dense": (1, 0, 0),
          "thick_formal_sub1_dense": (0, 0, 1), "thick_formal_sub3_dense": (0, 0, 3),
-         "thick_smooth_dense": (0, 1, 0), "thick_smooth_sub1_dense": (0, 1, 1), "thin_smooth_dense": (2, 1, 0)}
+         "thick_smooth_dense": (0, 1, 0), "thick_smooth_sub1_dense": (0, 1, 1), "thin_smooth_dense": (2, 1, 0),
+         "selthin_smooth_dense": (1, 1, 0)}
 
 
 def dev(a):
@@ -47,7 +48,7 @@ def expected_kernel(cfg, dense):
             return "transfer_series_kernel"
         if i == 1 and m == 2 and narrow:                       # Simpson's rule along the ray: a weighted thin sum
             return "transfer_series_kernel"
-        if i == 1 and m == 0 and cfg.nz >= 2 and (s > 0 or narrow):
+        if i == 1 and m in (0, 1) and cfg.nz >= 2 and (s > 0 or narrow):
             return "transfer_smooth_window_kernel"
     return "transfer_modes_kernel"
 
@@ -155,11 +156,13 @@ def test_modes_kernel_selection_and_fallbacks():
     from paper_2607_01338_b200 import IrisSO
     cfg, r = make_workload("small", nx=6, ny=2, nz=12, nv=64)
     names = {}
-    for mode in ("thin_formal", "selthin_formal", "thick_formal_sub1", "thick_formal_sub3", "thick_smooth", "thin_smooth"):
+    for mode in ("thin_formal", "selthin_formal", "thick_formal_sub1", "thick_formal_sub3", "thick_smooth", "thin_smooth",
+                 "selthin_smooth"):
         names[mode] = IrisSO(with_mode(cfg, mode)).transfer_kernel()
     assert names == {"thin_formal": "transfer_series_kernel", "selthin_formal": "transfer_series_kernel",
                      "thick_formal_sub1": "transfer_series_kernel", "thick_formal_sub3": "transfer_series_kernel",
-                     "thick_smooth": "transfer_smooth_window_kernel", "thin_smooth": "transfer_series_kernel"}
+                     "thick_smooth": "transfer_smooth_window_kernel", "thin_smooth": "transfer_series_kernel",
+                     "selthin_smooth": "transfer_smooth_window_kernel"}
     # wide channels: 1 km/s against xi = 1 km/s
     wide = cfg.with_(dv_cms=1.0 * KMS, v0_cms=-31.5 * KMS)
     f = make_fields(wide, r)
@@ -183,7 +186,7 @@ def test_modes_kernel_selection_and_fallbacks():
         assert_spectra(gpu_cube(c, fb, expect_kernel=False), Oracle(c).observe(fb), what=mode + " 4000 channels")
 
 
-@pytest.mark.parametrize("mode", ["thick_smooth_sub1", "thick_smooth", "thick_formal_sub1", "thin_smooth"])
+@pytest.mark.parametrize("mode", ["thick_smooth_sub1", "thick_smooth", "thick_formal_sub1", "thin_smooth", "selthin_smooth"])
 def test_window_kernels_agree_with_the_dense_kernel_on_every_pixel_of_medium(mode):
     """The sampled-column tests above compare 24 columns of the medium cube with the oracle; here EVERY pixel of the cube
     from the line-window kernel of a mode is compared with the dense modes kernel (itself checked against the oracle),
@@ -201,9 +204,28 @@ def test_window_kernels_agree_with_the_dense_kernel_on_every_pixel_of_medium(mod
     assert it.smooth_fallback() <= (cfg.nx * cfg.ny) // 200
     dense = IrisSO(cfg, transfer_algo=1).observe(*d, beam=False, noise=False)
     peak = dense.abs().amax(dim=-1, keepdim=True)
-    excess = ((win - dense).abs() / (0.5e-4 * peak + 0.5e-6)).max().item()
+    per_pixel = ((win - dense).abs() / (0.5e-4 * peak + 0.5e-6)).amax(dim=-1).reshape(-1)
+    excess = per_pixel.max().item()
     print("%s: window against dense kernel on all %d pixels: worst at %.3g of half the tolerance" % (mode, cfg.nx * cfg.ny, excess))
-    assert excess <= 1.0
+    if mode != "selthin_smooth":
+        assert excess <= 1.0
+        return
+    # selectively thin + smooth: two float32 evaluations of an unsaturated source differ by the rounding allowance of
+    # parity.selthin_source_allowance, which only the oracle can bound: the 32 pixels where the two kernels disagree
+    # most are marched by the oracle and BOTH kernels are held to it; elsewhere the two stay within 8 half-tolerances
+    assert excess <= 8.0
+    plane = cfg.nx * cfg.ny
+    pix = np.sort(torch.topk(per_pixel, 32).indices.cpu().numpy())
+    sub = {k: np.ascontiguousarray(f[k].reshape(cfg.nz, plane)[:, pix]).reshape(cfg.nz, 1, pix.size)
+           for k in ("nH2", "Tgas", "Tdust", "vlos")}
+    cfg_s = cfg.with_(nx=pix.size, ny=1, beam_fwhm_px=0.0, noise_sigma=0.0)
+    ref = Oracle(cfg_s).observe(sub, beam=False, noise=False).reshape(pix.size, cfg.nv)
+    extra = selthin_source_allowance(cfg_s, sub)
+    sel = torch.from_numpy(pix).cuda()
+    for what, cube in (("window kernel", win), ("dense kernel", dense)):
+        worst = assert_spectra(cube.reshape(plane, cfg.nv)[sel].cpu().numpy(), ref, extra=extra,
+                               what="selthin_smooth medium, %s on the 32 pixels of largest disagreement" % what)
+        print("selthin_smooth %s against the oracle on those pixels: worst at %.3g of tolerance" % (what, worst))
 
 
 def test_smooth_window_hands_over_when_a_relu_fires_outside_the_windows():
@@ -282,7 +304,7 @@ def test_modes_adjoint_is_refused_and_bad_modes_are_rejected():
 
 
 @pytest.mark.parametrize("mode", ["thick_smooth_sub1", "thick_smooth_sub1_dense", "thick_smooth", "thick_formal_sub1",
-                                  "selthin_formal", "thin_formal", "thin_smooth"])
+                                  "selthin_formal", "thin_formal", "thin_smooth", "selthin_smooth", "selthin_smooth_dense"])
 def test_modes_full_size_medium_sampled(mode):
     """BASELINE config "medium" at full size (256 x 256 x 288 cells, 512 channels), in the launch configuration
     bench.py times: seeded pixel columns against the oracle (columns are independent before the beam)."""
@@ -302,7 +324,9 @@ def test_modes_full_size_medium_sampled(mode):
            for k in ("nH2", "Tgas", "Tdust", "vlos")}
     cfg_s = cfg.with_(nx=n_cols, ny=1, beam_fwhm_px=0.0, noise_sigma=0.0)
     ref = Oracle(cfg_s).observe(sub, beam=False, noise=False).reshape(n_cols, cfg.nv)
-    worst = assert_spectra(got, ref, what=mode + " medium, sampled columns")
+    # (selectively thin + smooth: the unsaturated line source is rounded in float32, see selthin_source_allowance)
+    extra = selthin_source_allowance(cfg_s, sub) if mode.startswith("selthin_smooth") else 0.0
+    worst = assert_spectra(got, ref, extra=extra, what=mode + " medium, sampled columns")
     assert bool(torch.isfinite(cube).all())
     print("%s medium full size: worst sampled pixel at %.3g of tolerance" % (mode, worst))
 
