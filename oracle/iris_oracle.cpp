@@ -763,7 +763,8 @@ void orc_brute_column(const orc_config *c, const double *coef, const float *vlos
 // O10  Gradient of L = sum_voxels w * cube(noise-free, beam-convolved) with respect to n_H2.
 //
 // (a) Finite differences (the definition): central differences with relative step eps on the listed
-// cells.  Only the column holding the cell changes and the beam is linear, so L changes by
+// cells, in whatever transfer mode / integration / velocity grid the configuration names (the column goes through
+// the march of that mode).  Only the column holding the cell changes and the beam is linear, so L changes by
 // sum_v what[pixel][v] * d(cube_raw[pixel][v]) with what = G^T w (beam adjoint = same symmetric
 // zero-padded convolution, reading S20); `what` is computed by the caller with orc_beam.
 static void raw_column(const orc_config *c, const float *nH2, const float *Tgas, const float *Tdust,
@@ -774,6 +775,26 @@ static void raw_column(const orc_config *c, const float *nH2, const float *Tgas,
   const double Ibg = orc_planck(c->nu0_Hz, c->T_cmb);
   std::vector<double> It(c->nv, Ibg);
   double Ic = Ibg;
+  if (c->transfer_mode != 0 || c->integration != 0 || c->subsample != 0) {
+    // the other transfer / integration modes: the column's coefficients as a one-pixel cube through the march of O6b
+    orc_config c1 = *c;
+    c1.nx = 1; c1.ny = 1;
+    std::vector<double> coef((size_t)5 * c->nz);
+    std::vector<float> vl(c->nz);
+    for (int k = 0; k < c->nz; ++k) {
+      const int64_t cell = (int64_t)k * plane + pix;
+      const double n = cell == cell_mod ? n_mod : (double)nH2[cell];
+      double x[32], o[5];
+      orc_levelpop_cell(c, n, (double)Tgas[cell], x);
+      orc_cell_coefficients(c, n, (double)Tgas[cell], (double)Tdust[cell], x, o);
+      if (cell == cell_mod) { o[0] *= x_mod; o[1] *= x_mod; }
+      for (int q = 0; q < 5; ++q) coef[(size_t)q * c->nz + k] = o[q];
+      vl[k] = vlos[cell];
+    }
+    march_column_modes(&c1, coef.data(), vl.data(), 0, It.data(), &Ic);
+    for (int v = 0; v < c->nv; ++v) out[v] = orc_convert_voxel(c, It[v], Ic);
+    return;
+  }
   for (int k = 0; k < c->nz; ++k) {
     const int64_t cell = (int64_t)k * plane + pix;
     const double n = cell == cell_mod ? n_mod : (double)nH2[cell];
@@ -839,6 +860,102 @@ static double wprime_of_tau(double tau) {
   return (std::exp(-tau) * (1.0 + tau) - 1.0) / (tau * tau);
 }
 
+// (b') Reverse-mode derivative of total_point in the optically thick mode (transfer_mode 0), formal or smooth: one spectral
+// point with profile weights p[n], adjoint seed lam_out = dL / dI_observer.  Adds dL/dj0_n, dL/dkappa0_n, dL/dalpha_d,n
+// to gj, gk, gad.  Written as the chain rule applied to the formulas of total_point, statement by statement:
+//   formal  I_n+1 = I_n e^-tau + jT h w(tau):  as in (b)
+//   BDF2    y_n = relu(N_n / D_n),  N_n = 2 h jT_n + 4 y_n-1 - y_n-2,  D_n = 3 + 2 h aT_n           (Eq. 4.8.10)
+//           u = lam_n / D_n where N_n / D_n > 0, else 0 (ReLU):  dL/djT_n = 2 h u,  dL/daT_n = -2 h u y_n,
+//           lam_n-1 += 4 u,  lam_n-2 -= u
+//   TR      y_1 = relu(N_1 / D_1),  N_1 = h (jT_0 + jT_1) + (2 - h aT_0) y_0,  D_1 = 2 + h aT_1        (Eq. 4.8.12)
+//           u = lam_1 / D_1:  dL/djT_0 = dL/djT_1 = h u,  dL/daT_0 = -h u y_0,  dL/daT_1 = -h u y_1   (y_0 = I_bg is fixed)
+//   jT = j0 p + alpha_d S_d,  aT = kappa0 p + alpha_d  (Eq. 4.8.6 - 4.8.7)
+static void total_point_adjoint(const orc_config *c, int R, const double *p, const double *j0, const double *k0,
+                                const double *ad, const double *Sd, double Ibg, double lam_out, double *gj, double *gk,
+                                double *gad) {
+  const double h = c->cell_cm;
+  auto jT = [&](int n) { return j0[n] * p[n] + ad[n] * Sd[n]; };
+  auto aT = [&](int n) { return k0[n] * p[n] + ad[n]; };
+  auto spread = [&](int n, double dLdj, double dLda) {
+    gj[n] += dLdj * p[n];
+    gk[n] += dLda * p[n];
+    gad[n] += dLda + Sd[n] * dLdj;
+  };
+  if (c->integration == 0) {
+    std::vector<double> I(R + 1);
+    I[0] = Ibg;
+    for (int n = 0; n < R; ++n) I[n + 1] = formal_step(I[n], jT(n), aT(n), h);
+    double lam = lam_out;
+    for (int n = R - 1; n >= 0; --n) {
+      const double tau = aT(n) * h, e = std::exp(-tau);
+      spread(n, lam * h * w_of_tau(tau), lam * h * (-I[n] * e + jT(n) * h * wprime_of_tau(tau)));
+      lam *= e;
+    }
+    return;
+  }
+  if (R < 2) return;                                   // total_point returns I_bg: no dependence on the cells
+  std::vector<double> y(R), yu(R), lam(R, 0.0);
+  y[0] = yu[0] = Ibg;
+  yu[1] = (h * (jT(0) + jT(1)) + (2.0 - h * aT(0)) * y[0]) / (2.0 + h * aT(1));
+  y[1] = relu(yu[1]);
+  for (int n = 2; n < R; ++n) {
+    yu[n] = (2.0 * h * jT(n) + 4.0 * y[n - 1] - y[n - 2]) / (3.0 + 2.0 * h * aT(n));
+    y[n] = relu(yu[n]);
+  }
+  lam[R - 1] = lam_out;
+  for (int n = R - 1; n >= 2; --n) {
+    if (!(yu[n] > 0.0)) continue;                      // the ReLU passes nothing
+    const double u = lam[n] / (3.0 + 2.0 * h * aT(n));
+    spread(n, 2.0 * h * u, -2.0 * h * u * y[n]);
+    lam[n - 1] += 4.0 * u;
+    lam[n - 2] -= u;
+  }
+  if (yu[1] > 0.0) {
+    const double u = lam[1] / (2.0 + h * aT(1));
+    spread(0, h * u, -h * u * y[0]);
+    spread(1, h * u, -h * u * y[1]);
+  }
+}
+
+// dL/dj0, dL/dkappa0, dL/dalpha_d of every cell of one column in the thick mode with the smooth integrator and / or the
+// fine velocity grid (the configurations march_column_modes serves with transfer_mode = 0).  what[nv]: dL / d(cube_raw).
+// The cube is scale (I_tot[v] - I_cont) with I_tot[v] the Simpson average of the fine points (Eq. 4.5.1), so the seed of a
+// fine point is the sum over the channels it belongs to of scale what[v] (Simpson coefficient) / (3 m).
+static void column_adjoint_modes(const orc_config *c, int R, const double *j0, const double *k0, const double *b,
+                                 const double *ad, const double *Sd, const double *vl, const double *what, double scale,
+                                 double *gj, double *gk, double *gad) {
+  const double Ibg = orc_planck(c->nu0_Hz, c->T_cmb);
+  std::vector<double> p(R), zero(R, 0.0);
+  for (int n = 0; n < R; ++n) gj[n] = gk[n] = gad[n] = 0.0;
+  double lamC = 0.0;
+  for (int v = 0; v < c->nv; ++v) if (c->subtract_continuum) lamC -= scale * what[v];
+  const int f = c->subsample;
+  if (f == 0) {
+    for (int v = 0; v < c->nv; ++v) {
+      for (int n = 0; n < R; ++n) p[n] = orc_phibar(c, v, vl[n], b[n]);
+      total_point_adjoint(c, R, p.data(), j0, k0, ad, Sd, Ibg, scale * what[v], gj, gk, gad);
+    }
+  } else {
+    const int m = f + 1;
+    const double dvf = c->dv_cms / m;
+    for (int64_t q = 0; q <= (int64_t)c->nv * m; ++q) {
+      double seed = 0.0;
+      for (int64_t v = q / m - 1; v <= q / m; ++v) {     // a point on a channel edge belongs to both channels
+        if (v < 0 || v >= c->nv) continue;
+        const int64_t jq = q - v * m;                    // index of the point inside channel v: 0 .. m
+        if (jq < 0 || jq > m) continue;
+        const double simpson = (jq == 0 || jq == m) ? 1.0 : ((jq & 1) ? 4.0 : 2.0);
+        seed += scale * what[v] * simpson / (3.0 * m);
+      }
+      const double vel = c->v0_cms - 0.5 * c->dv_cms + q * dvf;
+      for (int n = 0; n < R; ++n) p[n] = orc_phi_point(c, vel, vl[n], b[n]);
+      total_point_adjoint(c, R, p.data(), j0, k0, ad, Sd, Ibg, seed, gj, gk, gad);
+    }
+  }
+  // the continuum is the same march with no line (continuum_column): p = 0
+  total_point_adjoint(c, R, zero.data(), j0, k0, ad, Sd, Ibg, lamC, gj, gk, gad);
+}
+
 static void grad_adjoint_impl(const orc_config *c, const float *nH2, const float *Tgas, const float *Tdust,
                               const float *vlos, const double *what, double *grad, bool wrt_abundance) {
   const int64_t plane = (int64_t)c->nx * c->ny;
@@ -859,9 +976,25 @@ static void grad_adjoint_impl(const orc_config *c, const float *nH2, const float
       orc_levelpop_cell(c, (double)nH2[cell], (double)Tgas[cell], &xs[k * N]);
       orc_cell_coefficients(c, (double)nH2[cell], (double)Tgas[cell], (double)Tdust[cell], &xs[k * N], &co[5 * k]);
     }
+    std::vector<double> gj(nz, 0.0), gk(nz, 0.0), gad(nz, 0.0);
+    const bool hot = c->transfer_mode == 0 && c->integration == 0 && c->subsample == 0;
+    if (!hot) {
+      // thick mode with the smooth integrator and / or the fine grid: (b').  The other transfer modes have no analytic
+      // adjoint here (finite differences (a) serve them): NaN.
+      std::vector<double> a0(nz), a1(nz), a2(nz), a3(nz), a4(nz), vl(nz);
+      for (int k = 0; k < nz; ++k) {
+        a0[k] = co[5 * k]; a1[k] = co[5 * k + 1]; a2[k] = co[5 * k + 2]; a3[k] = co[5 * k + 3]; a4[k] = co[5 * k + 4];
+        vl[k] = (double)vlos[(int64_t)k * plane + pix];
+      }
+      if (c->transfer_mode == 0)
+        column_adjoint_modes(c, nz, a0.data(), a1.data(), a2.data(), a3.data(), a4.data(), vl.data(), what + pix * nv, scale,
+                             gj.data(), gk.data(), gad.data());
+      else
+        for (int k = 0; k < nz; ++k) gj[k] = gk[k] = gad[k] = std::nan("");
+    }
     for (int v = 0; v < nv; ++v) It[v] = Ibg;
     Ic[0] = Ibg;
-    for (int k = 0; k < nz; ++k) {
+    for (int k = 0; hot && k < nz; ++k) {
       const int64_t cell = (int64_t)k * plane + pix;
       const double *o = &co[5 * k];
       for (int v = 0; v < nv; ++v) {
@@ -875,8 +1008,8 @@ static void grad_adjoint_impl(const orc_config *c, const float *nH2, const float
     for (int k = nz - 1; k >= 0; --k) {
       const int64_t cell = (int64_t)k * plane + pix;
       const double *o = &co[5 * k];
-      double g_j0 = 0.0, g_k0 = 0.0, g_ad = 0.0;
-      for (int v = 0; v < nv; ++v) {
+      double g_j0 = gj[k], g_k0 = gk[k], g_ad = gad[k];
+      for (int v = 0; hot && v < nv; ++v) {
         const double pb = orc_phibar(c, v, (double)vlos[cell], o[2]);
         const double al = o[1] * pb + o[3], j = o[0] * pb + o[3] * o[4], tau = al * h, e = std::exp(-tau);
         const double dIda = h * (-It[(int64_t)k * nv + v] * e + j * h * wprime_of_tau(tau));
@@ -886,7 +1019,7 @@ static void grad_adjoint_impl(const orc_config *c, const float *nH2, const float
         g_ad += lam[v] * (dIda + o[4] * dIdj);
         lam[v] *= e;
       }
-      {  // continuum branch
+      if (hot) {  // continuum branch
         const double tau = o[3] * h, e = std::exp(-tau), j = o[3] * o[4];
         const double dIda = h * (-Ic[k] * e + j * h * wprime_of_tau(tau));
         g_ad += lamC * (dIda + o[4] * h * w_of_tau(tau));

@@ -494,6 +494,26 @@ transfer_series_kernel(MarchConsts mc, const float* __restrict__ coef, int64_t n
     if (out != nullptr) {
       float* o = out + (int64_t)pix * nv;
       const bool al = ((((int64_t)pix * nv) & 1) == 0);      // float2 stores need an even element offset
+      if (mc.out_mode <= OUT_I_TOT && al && (nv & 1) == 0) {
+        // the units that are linear in D (Rayleigh-Jeans Kelvin or intensity, with or without the continuum): one
+        // multiply-add per value, four pairs per lane in flight (the loop is latency-bound: LDS -> FMA -> STG)
+        const float sc = mc.out_mode >= OUT_I_SUB ? mc.inv_KRJ : 1.0f;
+        const float a = invG * sc, b = (mc.out_mode & 1) ? C * sc : 0.0f;
+        float2* o2 = reinterpret_cast<float2*>(o);
+        const int nq = nv / 2;
+        int q = i;
+        for (; q + 3 * LPP < nq; q += 4 * LPP) {
+          float2 v[4];
+#pragma unroll
+          for (int k = 0; k < 4; ++k) v[k] = pair_at(q + k * LPP);
+#pragma unroll
+          for (int k = 0; k < 4; ++k) o2[q + k * LPP] = make_float2(fmaf(v[k].x, a, b), fmaf(v[k].y, a, b));
+        }
+        for (; q < nq; q += LPP) {
+          const float2 v = pair_at(q);
+          o2[q] = make_float2(fmaf(v.x, a, b), fmaf(v.y, a, b));
+        }
+      } else
       for (int q = i; 2 * q < nv; q += LPP) {
         const float2 v = pair_at(q);
         const float r0 = convert_out(v.x * invG, C, mc);

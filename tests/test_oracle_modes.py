@@ -479,3 +479,90 @@ def test_per_channel_dust_leaves_the_line_terms_alone():
     It, Ic = o.march_perchannel(coef, f["vlos"], f["Tdust"])
     It0, Ic0 = Oracle(cfg).march(coef, f["vlos"])
     assert np.all(Ic == 0.0) and np.allclose(It, It0, rtol=1e-14, atol=0.0) and It0.max() > 0
+
+
+# ------------------------------------------------------------------------------------------------
+# Gradient outside the hot-path mode (the pipeline is differentiable end to end, and its production mode
+# is thick + smooth + f = 1): the oracle's reverse-mode adjoint of the thick mode with the smooth integrator and / or the
+# fine grid, against (a) central differences of the oracle's OWN forward march of that mode, cell by cell, and (b) the
+# directional derivative of the whole observation (beam included) through observe().
+ADJ_MODES = {"thick_smooth": (1, 0), "thick_smooth_sub1": (1, 1), "thick_smooth_sub3": (1, 3), "thick_formal_sub1": (0, 1),
+             "thick_formal_sub3": (0, 3)}
+
+
+@pytest.mark.parametrize("regime", ["plain", "relu_active"])
+@pytest.mark.parametrize("mode", ADJ_MODES)
+def test_adjoint_of_the_thick_modes_matches_finite_differences(mode, regime):
+    integ, sub = ADJ_MODES[mode]
+    cfg, r = make_workload("tiny", nx=3, ny=2, nz=9, nv=24)
+    cfg = cfg.with_(integration=integ, subsample=sub, dust_on=True, kappa_gas_cm2_g=0.05, beam_fwhm_px=2.0)
+    f = make_fields(cfg, r)
+    f["vlos"] = (0.2 * f["vlos"]).astype(np.float32)
+    if regime == "relu_active":
+        if integ == 0:
+            pytest.skip("the formal thick step has no ReLU")
+        # bright background behind cold dust that turns opaque abruptly: the BDF2 continuum and the line points overshoot
+        # below zero and are clamped (the regime of test_gpu_modes.py "opaque_dust_clamp")
+        cfg = cfg.with_(T_cmb=60.0, kappa_gas_cm2_g=3.0)
+        f["Tdust"] = np.full_like(f["Tdust"], 3.0)
+        f["nH2"][: cfg.nz // 2] *= 1e-3
+        f["nH2"][cfg.nz // 2:] *= 30.0
+        # the clamp did fire: a column cut short after cell n ends in the state the full march passes through at n
+        fired = False
+        for cut in range(cfg.nz // 2 + 1, cfg.nz + 1):
+            fc = {k: np.ascontiguousarray(f[k][:cut]) for k in ("nH2", "Tgas", "Tdust", "vlos")}
+            tot = Oracle(cfg.with_(nz=cut, subtract_continuum=False, out_unit=0)).observe(fc, beam=False, noise=False)
+            fired = fired or bool((tot == 0.0).any())
+        assert fired
+    o = Oracle(cfg)
+    rng = np.random.default_rng(11)
+    w = rng.random((cfg.ny, cfg.nx, cfg.nv)) - 0.3
+    what = o.beam(w)
+    g = o.grad_adjoint(f, what)
+    assert np.all(np.isfinite(g)) and np.abs(g).max() > 0
+    cells = np.arange(cfg.n_cells)
+    # (behind the 60 K background of the clamped regime L is ~1e7 times a cell's contribution: the rounding of the
+    # difference quotient asks for a wider bracket there; measured: the gap to the adjoint falls as 1 / eps down to 4e-6 at
+    # eps = 1e-3.  A ReLU kink inside a bracket would show up as one outlier; none for this seed)
+    gfd = o.grad_fd(f, what, cells, eps=1e-3 if regime == "relu_active" else 1e-5)
+    scale = np.abs(gfd).max()
+    assert np.allclose(g.ravel(), gfd, rtol=2e-5 if regime == "relu_active" else 5e-6, atol=1e-8 * scale)
+    # whole-pipeline directional derivative through observe(), beam applied to the cube
+    d = rng.standard_normal(f["nH2"].shape) * f["nH2"] * 1e-3
+    np_ = (f["nH2"].astype(np.float64) + d).astype(np.float32)
+    nm_ = (f["nH2"].astype(np.float64) - d).astype(np.float32)
+    dd = np_.astype(np.float64) - nm_.astype(np.float64)
+
+    def L(nH2):
+        ff = dict(f)
+        ff["nH2"] = nH2
+        return float((w * o.observe(ff, beam=True, noise=False)).sum())
+    assert (L(np_) - L(nm_)) == pytest.approx(float((g * dd).sum()), rel=2e-4, abs=0.0)
+
+
+def test_adjoint_of_the_fine_grid_tends_to_the_hot_path_adjoint_for_resolved_lines():
+    """For an optically thin line the intensity is linear in the profile, so the Simpson average of the point profile over
+    a channel (Eq. 4.5.1) IS the channel-integrated profile of Eq. 4.6.3 to O((dv / (m b))^4): the gradient of the thick
+    formal mode on the fine grid tends to the hot-path gradient, which round 1 pinned on its own (test_oracle_pins.py,
+    pin 13).  (A thick line does not: averaging intensities and averaging the profile inside the exponent differ.)"""
+    cfg, r = make_workload("tiny", nx=2, ny=2, nz=8, nv=48)
+    cfg = cfg.with_(dust_on=True, kappa_gas_cm2_g=0.05, dv_cms=0.25 * cfg.dv_cms, v0_cms=0.25 * cfg.v0_cms,
+                    abundance=1e-6 * cfg.abundance)
+    f = make_fields(cfg, r)
+    f["vlos"] = (0.05 * f["vlos"]).astype(np.float32)
+    rng = np.random.default_rng(12)
+    w = rng.random((cfg.ny, cfg.nx, cfg.nv))
+    g0 = Oracle(cfg).grad_adjoint(f, w)
+    errs = []
+    for sub in (1, 3):
+        g = Oracle(cfg.with_(subsample=sub)).grad_adjoint(f, w)
+        errs.append(np.abs(g - g0).max() / np.abs(g0).max())
+    assert errs[0] < 1e-3 and errs[1] < errs[0] / 8.0, errs
+
+
+def test_adjoint_of_the_other_transfer_modes_is_not_claimed():
+    cfg, r = make_workload("tiny", nx=2, ny=1, nz=4, nv=8)
+    f = make_fields(cfg, r)
+    w = np.ones((cfg.ny, cfg.nx, cfg.nv))
+    for m in (1, 2):
+        assert np.all(np.isnan(Oracle(cfg.with_(transfer_mode=m)).grad_adjoint(f, w)))
