@@ -97,8 +97,9 @@ typedef struct {
   /* implementation choice, does not change the mathematics */
   int32_t transfer_algo;        /* IRIS_SO_ALGO_* */
   /* The paper's other transfer / integration modes (sections 4.4 - 4.8).  All three 0 = the hot
-   * path above (optically thick, formal integration, channel-integrated profile).  Any other combination runs
-   * transfer_modes_kernel; iris_so_observe_adjoint then returns IRIS_SO_EUNSUPPORTED. */
+   * path above (optically thick, formal integration, channel-integrated profile).  Any other combination runs a
+   * line-window kernel of its own or transfer_modes_kernel (iris_so_transfer_kernel names it).  The gradient entry
+   * points serve transfer_mode = 0 with every integration / subsample; transfer_mode 1 and 2: IRIS_SO_EUNSUPPORTED. */
   int32_t transfer_mode;        /* 0 optically thick (4.5), 1 selectively thin (4.6, Eq. 4.8.13-4.8.15),
                                  * 2 optically thin (4.7, Eq. 4.7.3-4.7.5) */
   int32_t integration;          /* 0 formal (Eq. 4.8.5 / 4.7.6), 1 smooth (trapezoidal first step Eq. 4.8.12 + BDF2
@@ -188,8 +189,12 @@ iris_so_status iris_so_observe_host(iris_so_ctx *ctx, const float *h_nH2, const 
                                     void *cuda_stream);
 
 /* K8 + K9.  Gradient of L = sum_{y,x,v} w * cube (noise-free cube, beam applied if configured) with
- * respect to n_H2 of every cell, by a reverse scan along every ray.  Requires subtract_space = 0 and
- * out_unit 0 or 1.  d_w [ny][nx][nv], d_grad_nH2 [nz][ny][nx]. */
+ * respect to n_H2 of every cell, by a reverse scan along every ray (the pipeline is
+ * differentiable end to end).  Requires subtract_space = 0, out_unit 0 or 1 and the optically thick transfer mode
+ * (transfer_mode = 0), with either integration and any subsample: the hot-path mode has a closed-form windowed
+ * adjoint, the smooth integrator (Eq. 4.8.10 / 4.8.12 with the ReLU) and the fine grid (Eq. 4.5.1) a stored-state
+ * reverse sweep whose scratch is sized by the resident warps, not by the cube.  Not available with coef_grid = 1 or
+ * dust_per_channel = 1 (IRIS_SO_EUNSUPPORTED).  d_w [ny][nx][nv], d_grad_nH2 [nz][ny][nx]. */
 iris_so_status iris_so_observe_adjoint(iris_so_ctx *ctx, const float *d_nH2, const float *d_Tgas,
                                        const float *d_Tdust, const float *d_vlos, const float *d_w,
                                        float *d_grad_nH2, void *cuda_stream);

@@ -676,14 +676,9 @@ inline void launch_coef_grad(const LevelConsts& lc, const AdjointConsts& ac, int
   }
 }
 
-// K9 then K8.  dcoef: scratch [2][ncell].  series: every cell has dv / b <= 0.55 (channel-centre profile expansion).  Returns the first CUDA error; *launches is advanced per kernel.
-inline cudaError_t launch_adjoint(const MarchConsts& mc, const AdjointConsts& ac, const LevelConsts& lc, int n_levels,
-                                  int band, const float* coef, float* dcoef, int64_t ncell, int npix, int nz, int nv,
-                                  bool dust, bool series, const float* nH2, const float* Tgas, const float* what, float* grad,
-                                  cudaStream_t st, uint64_t* launches, bool wrt_abundance = false) {
-  // abundance-only gradient: e_c and a_c are linear in the tracer abundance, so d e_c / d ln X = e_c, d a_c / d ln X = a_c
-  // (the first two coefficient planes take the place of dcoef) and the dust does not depend on it (ac.c_d = 0)
-  if (wrt_abundance) goto march;
+// K9 for the configured number of levels
+inline cudaError_t launch_coef_grad_levels(const LevelConsts& lc, const AdjointConsts& ac, int n_levels, int band, int64_t ncell,
+                                           const float* nH2, const float* Tgas, float* dcoef, cudaStream_t st) {
   switch (n_levels) {
     case 2: launch_coef_grad<2>(lc, ac, band, ncell, nH2, Tgas, dcoef, st); break;
     case 3: launch_coef_grad<3>(lc, ac, band, ncell, nH2, Tgas, dcoef, st); break;
@@ -695,12 +690,21 @@ inline cudaError_t launch_adjoint(const MarchConsts& mc, const AdjointConsts& ac
     case 9: launch_coef_grad<9>(lc, ac, band, ncell, nH2, Tgas, dcoef, st); break;
     default: launch_coef_grad<10>(lc, ac, band, ncell, nH2, Tgas, dcoef, st); break;
   }
-  {
-    cudaError_t e0 = cudaGetLastError();
+  return cudaGetLastError();
+}
+
+// K9 then K8.  dcoef: scratch [2][ncell].  series: every cell has dv / b <= 0.55 (channel-centre profile expansion).  Returns the first CUDA error; *launches is advanced per kernel.
+inline cudaError_t launch_adjoint(const MarchConsts& mc, const AdjointConsts& ac, const LevelConsts& lc, int n_levels,
+                                  int band, const float* coef, float* dcoef, int64_t ncell, int npix, int nz, int nv,
+                                  bool dust, bool series, const float* nH2, const float* Tgas, const float* what, float* grad,
+                                  cudaStream_t st, uint64_t* launches, bool wrt_abundance = false) {
+  // abundance-only gradient: e_c and a_c are linear in the tracer abundance, so d e_c / d ln X = e_c, d a_c / d ln X = a_c
+  // (the first two coefficient planes take the place of dcoef) and the dust does not depend on it (ac.c_d = 0)
+  if (!wrt_abundance) {
+    cudaError_t e0 = launch_coef_grad_levels(lc, ac, n_levels, band, ncell, nH2, Tgas, dcoef, st);
     if (e0 != cudaSuccess) return e0;
     ++*launches;
   }
-march:
   cudaError_t e;
   const float* dc = wrt_abundance ? coef : dcoef;
   // lanes per pixel: 16 (two pixels per warp) up to 384 channels, one warp per pixel beyond: five spectra per pixel live

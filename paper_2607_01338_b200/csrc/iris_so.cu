@@ -22,6 +22,7 @@
 #include "transfer_modes.cuh"
 #include "transfer_smooth.cuh"
 #include "adjoint_kernels.cuh"
+#include "adjoint_modes.cuh"
 #include "diagnostics.cuh"
 
 namespace {
@@ -1008,22 +1009,33 @@ static iris_so_status observe_adjoint_impl(iris_so_ctx* ctx, const float* d_nH2,
   const iris_so_config& c = ctx->cfg;
   if ((c.subtract_continuum && c.subtract_space != 0) || c.out_unit == 2)
     return fail(ctx, IRIS_SO_EUNSUPPORTED, "adjoint needs intensity-space subtraction and out_unit 0 or 1");
-  if (!hot_path_mode(c))
-    return fail(ctx, IRIS_SO_EUNSUPPORTED, "adjoint is implemented for the thick / formal / channel-integrated mode only");
+  // the hot-path mode has the windowed closed-form adjoint (adjoint_kernels.cuh); the thick mode with the smooth integrator
+  // and / or the fine grid the stored-state reverse sweep of adjoint_modes.cuh; the thin modes have none
+  const bool modes_adjoint = c.transfer_mode == 0 && !hot_path_mode(c);
+  if (c.transfer_mode != 0)
+    return fail(ctx, IRIS_SO_EUNSUPPORTED, "adjoint is implemented for the optically thick transfer mode only");
   if (c.coef_grid == 1)
     return fail(ctx, IRIS_SO_EUNSUPPORTED, "adjoint differentiates the per-cell level solve: not available with coef_grid = 1");
   if (c.dust_per_channel)
     return fail(ctx, IRIS_SO_EUNSUPPORTED, "adjoint is not available with dust_per_channel = 1");
   // the adjoint march keeps five spectra per pixel in shared memory (one warp per pixel beyond 384 channels)
-  if ((size_t)5 * (((size_t)c.nv + 31) / 32 * 32) * sizeof(float) + (size_t)iris::kAdjRecFields * 32 * sizeof(float4) > 227u * 1024u)
+  if (!modes_adjoint &&
+      (size_t)5 * (((size_t)c.nv + 31) / 32 * 32) * sizeof(float) + (size_t)iris::kAdjRecFields * 32 * sizeof(float4) > 227u * 1024u)
     return fail(ctx, IRIS_SO_EUNSUPPORTED, "adjoint: five spectra of this many channels do not fit the shared memory of an SM");
+  // the reverse sweep of the other modes stages a column's coefficients and accumulators in shared memory
+  if (modes_adjoint && iris::kAdjModesWarps * iris::adjoint_modes_smem_per_warp(c.nz) > 227u * 1024u)
+    return fail(ctx, IRIS_SO_EUNSUPPORTED, "adjoint: a column of this many cells does not fit the shared memory of an SM");
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   iris_so_status s = run_coefficients(ctx, d_nH2, d_Tgas, d_Tdust, d_vlos, nullptr, st);
   if (s != IRIS_SO_OK) return s;
   // scratch: d(e_c)/dn and d(a_c)/dn per cell, then (with a beam) what = G^T w -- the beam is symmetric and zero
   // padded, so its adjoint is the same convolution
   const size_t dcoef_floats = 2 * (size_t)ctx->ncell;
-  const size_t need = sizeof(float) * (dcoef_floats + (c.beam_fwhm_px > 0.0 ? (size_t)ctx->nvox : 0));
+  // (other modes: + the stored states of the forward sweep, one slab per resident warp)
+  const int modes_grid = modes_adjoint ? iris::adjoint_modes_grid(ctx->sm_count, c.nz) : 0;
+  const size_t states_floats =
+      modes_adjoint ? (size_t)modes_grid * iris::kAdjModesWarps * iris::adjoint_modes_scratch_per_warp(c.nz) / sizeof(float) : 0;
+  const size_t need = sizeof(float) * (dcoef_floats + (c.beam_fwhm_px > 0.0 ? (size_t)ctx->nvox : 0) + states_floats);
   if (ctx->d_adj && ctx->adj_bytes < need) { cudaFree(ctx->d_adj); ctx->d_adj = nullptr; ctx->scratch_bytes -= ctx->adj_bytes; }
   if ((s = ensure(ctx, &ctx->d_adj, need, "cudaMalloc(adjoint scratch)")) != IRIS_SO_OK) return s;
   ctx->adj_bytes = need;
@@ -1037,6 +1049,21 @@ static iris_so_status observe_adjoint_impl(iris_so_ctx* ctx, const float* d_nH2,
   ProfScope prof(ctx, IRIS_SO_STAGE_ADJOINT, st);
   iris::AdjointConsts ac = ctx->ac;
   if (wrt_abundance) ac.c_d = 0.0f;                    // the dust does not depend on the tracer abundance
+  if (modes_adjoint) {
+    cudaError_t e = cudaSuccess;
+    if (!wrt_abundance) {
+      e = iris::launch_coef_grad_levels(ctx->lc, ac, c.n_levels, ctx->band, ctx->ncell, d_nH2, d_Tgas, dcoef, st);
+      if (e != cudaSuccess) return cuda_fail(ctx, e, "launch of coef_grad_kernel");
+      ++ctx->launches;
+    }
+    float* states = ctx->d_adj + dcoef_floats + (c.beam_fwhm_px > 0.0 ? (size_t)ctx->nvox : 0);
+    e = iris::launch_adjoint_modes(ctx->mc, ac, c.integration == 1, c.subsample > 0 ? c.subsample + 1 : 0, ctx->d_coef,
+                                   wrt_abundance ? ctx->d_coef : dcoef, ctx->ncell, (int)ctx->npix, c.nz, c.nv, what, states,
+                                   d_grad, modes_grid, st);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "launch of adjoint_modes_kernel");
+    ++ctx->launches;
+    return IRIS_SO_OK;
+  }
   cudaError_t e = iris::launch_adjoint(ctx->mc, ac, ctx->lc, c.n_levels, ctx->band, ctx->d_coef, dcoef, ctx->ncell, (int)ctx->npix,
                                        c.nz, c.nv, c.dust_on != 0, resolved_algo(c) == IRIS_SO_ALGO_WINDOW, d_nH2, d_Tgas, what,
                                        d_grad, st, &ctx->launches, wrt_abundance);

@@ -33,7 +33,7 @@ def excess(g, ref, scale):
     return float(np.max(np.abs(g - ref) / (REL * np.abs(ref) + REL * FLOOR * scale)))
 
 
-def check(cfg, f, w, n_fd=48, seed=5, label="", fd_random=True):
+def check(cfg, f, w, n_fd=48, seed=5, label="", fd_random=True, eps=1e-5):
     o = Oracle(cfg)
     what = o.beam(w.astype(np.float64)) if cfg.beam_fwhm_px > 0 else w.astype(np.float64)
     ref = o.grad_adjoint(f, what)
@@ -47,7 +47,7 @@ def check(cfg, f, w, n_fd=48, seed=5, label="", fd_random=True):
     order = np.argsort(-np.abs(ref).ravel())
     rand = rng.choice(cfg.n_cells, size=n_fd // 2, replace=False) if fd_random else order[n_fd // 2: n_fd]
     cells = np.unique(np.concatenate([order[: n_fd // 2], rand]))
-    gfd = o.grad_fd(f, what, cells, eps=1e-5)
+    gfd = o.grad_fd(f, what, cells, eps=eps)
     worst_fd = excess(g.ravel()[cells], gfd, scale)
     print("adjoint %s: worst vs analytic %.3g, vs finite differences %.3g of tolerance (max|g| %.3g)" %
           (label, worst, worst_fd, scale))
@@ -218,4 +218,122 @@ def test_batch_workload_full_size_sampled():
     gfd = o.grad_fd(f, what, cells, eps=1e-5)
     worst = excess(g[cells], gfd, np.abs(g).max())
     print("batch cube at full size: gradient vs finite differences at %.3g of tolerance (max|g| %.3g)" % (worst, np.abs(g).max()))
+    assert np.all(np.isfinite(g)) and worst <= 1.0
+
+
+# ------------------------------------------------------------------------------------------------
+# Gradient outside the hot-path mode (adjoint_modes_kernel): optically thick transfer with the smooth integrator (TR + BDF2 +
+# ReLU) and / or the fine velocity grid with Simpson's rule -- thick + smooth + f = 1 is the paper's production mode
+# (PAPER.md:563).  Same bar as above: every cell against the oracle's float64 reverse-mode adjoint of that mode, sampled
+# cells against the oracle's finite differences through that mode's forward march.
+MODE_ADJ = {"thick_smooth": (1, 0), "thick_smooth_sub1": (1, 1), "thick_smooth_sub3": (1, 3), "thick_formal_sub1": (0, 1),
+            "thick_formal_sub3": (0, 3)}
+
+
+@pytest.mark.parametrize("case", ["dust_beam", "thick", "intensity_out", "no_subtraction", "heavy_dust", "no_dust", "relu_active"])
+@pytest.mark.parametrize("mode", MODE_ADJ)
+def test_adjoint_of_the_thick_modes(mode, case):
+    integ, sub = MODE_ADJ[mode]
+    cfg, r = make_workload("batch", n=16, nv=64)
+    cfg = cfg.with_(integration=integ, subsample=sub)
+    f = make_fields(cfg, r)
+    f["vlos"] = (0.2 * f["vlos"]).astype(np.float32)
+    eps = 1e-5
+    if case == "thick":
+        cfg = cfg.with_(abundance=2e-5)
+    elif case == "intensity_out":
+        cfg = cfg.with_(out_unit=0)
+    elif case == "no_subtraction":
+        cfg = cfg.with_(subtract_continuum=False)
+    elif case == "heavy_dust":
+        cfg = cfg.with_(kappa_gas_cm2_g=5.0)
+    elif case == "no_dust":
+        cfg = cfg.with_(dust_on=False)
+    elif case == "relu_active":
+        if integ == 0:
+            pytest.skip("the formal thick step has no ReLU")
+        # bright background behind cold dust that turns opaque abruptly: continuum and line points are clamped at zero for
+        # a few cells (tests/test_oracle_modes.py checks that they are).  The objective is ~1e7 times a cell's share of
+        # it there, so the finite differences take a wider bracket.
+        cfg = cfg.with_(T_cmb=60.0, kappa_gas_cm2_g=3.0)
+        f["Tdust"] = np.full_like(f["Tdust"], 3.0)
+        f["nH2"][: cfg.nz // 2] *= 1e-3
+        f["nH2"][cfg.nz // 2:] *= 30.0
+        eps = 1e-3
+    check(cfg, f, weight_cube(cfg), n_fd=32, label="%s %s" % (mode, case), fd_random=case != "relu_active", eps=eps)
+
+
+@pytest.mark.parametrize("mode", ["thick_smooth_sub1", "thick_formal_sub3", "thick_smooth"])
+def test_adjoint_of_the_thick_modes_ragged_and_degenerate(mode):
+    integ, sub = MODE_ADJ[mode]
+    cfg, r = make_workload("batch", n=8, nx=5, ny=3, nz=37, nv=45)
+    cfg = cfg.with_(integration=integ, subsample=sub)
+    f = make_fields(cfg, r)
+    f["vlos"] = (0.1 * f["vlos"]).astype(np.float32)
+    check(cfg, f, weight_cube(cfg), n_fd=20, label=mode + " ragged")
+    # more points than one block of 256 per pixel, a last block of every size class
+    cfg2, r2 = make_workload("batch", n=6, nx=3, ny=2, nz=12, nv=200)
+    cfg2 = cfg2.with_(integration=integ, subsample=sub, dv_cms=0.3 * cfg2.dv_cms, v0_cms=0.3 * cfg2.v0_cms)
+    f2 = make_fields(cfg2, r2)
+    f2["vlos"] = (0.3 * f2["vlos"]).astype(np.float32)
+    check(cfg2, f2, weight_cube(cfg2), n_fd=20, label=mode + " several blocks")
+    for nz in (1, 2, 3):
+        cfg1, r1 = make_workload("batch", n=1, nx=1, ny=1, nz=nz, nv=3)
+        cfg1 = cfg1.with_(integration=integ, subsample=sub, dv_cms=1.0e5, v0_cms=-1.0e5, beam_fwhm_px=0.0)
+        f1 = make_fields(cfg1, r1)
+        f1["vlos"] = np.zeros_like(f1["vlos"])
+        o = Oracle(cfg1)
+        ref = o.grad_adjoint(f1, np.ones((1, 1, 3)))
+        g = gpu_grad(cfg1, f1, np.ones((1, 1, 3), np.float32)).reshape(ref.shape)
+        assert excess(g, ref, max(np.abs(ref).max(), 1e-300)) <= 1.0, (mode, nz, g, ref)
+
+
+def test_adjoint_of_the_thick_modes_abundance_and_linearity():
+    cfg, r = make_workload("batch", n=12, nv=64)
+    cfg = cfg.with_(integration=1, subsample=1)
+    f = make_fields(cfg, r)
+    f["vlos"] = (0.15 * f["vlos"]).astype(np.float32)
+    from paper_2607_01338_b200 import IrisSO
+    d = [dev(f[k]) for k in ("nH2", "Tgas", "Tdust", "vlos")]
+    w1 = weight_cube(cfg, seed=2000); w2 = weight_cube(cfg, seed=2001)
+    g1, g2, g12 = gpu_grad(cfg, f, w1), gpu_grad(cfg, f, w2), gpu_grad(cfg, f, w1 + 2 * w2)
+    assert np.max(np.abs(g12 - (g1 + 2 * g2))) <= 2e-5 * np.abs(g12).max()
+    assert np.all(gpu_grad(cfg, f, np.zeros_like(w1)) == 0.0)
+    o = Oracle(cfg)
+    what = o.beam(w1.astype(np.float64))
+    ref = o.grad_adjoint(f, what, wrt="abundance")
+    g = IrisSO(cfg).observe_adjoint(*d, dev(w1.astype(np.float32)), wrt="abundance").cpu().numpy().astype(np.float64).reshape(ref.shape)
+    scale = np.abs(ref).max()
+    assert np.max(np.abs(g - ref) / (REL * np.abs(ref) + 3e-7 * scale)) <= 1.0
+
+
+def test_production_mode_gradient_at_full_size_sampled():
+    """One cube of BASELINE config 5 (128^3 cells, 256 channels, dust, beam 3 px) in the paper's production mode (thick,
+    smooth, f = 1: 513 fine points per spectrum): the gradient against the oracle's finite differences on sampled cells."""
+    from paper_2607_01338_b200 import IrisSO
+    cfg, r = make_workload("batch", seed=1003)
+    cfg = cfg.with_(integration=1, subsample=1)
+    f = make_fields(cfg, r)
+    d = [dev(f[k]) for k in ("nH2", "Tgas", "Tdust", "vlos")]
+    it = IrisSO(cfg)
+    w = weight_cube(cfg)
+    wd = dev(w)
+    g = it.observe_adjoint(*d, wd)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(3):
+        it.observe_adjoint(*d, wd)
+    e1.record()
+    torch.cuda.synchronize()
+    g = g.cpu().numpy().astype(np.float64).ravel()
+    o = Oracle(cfg)
+    what = o.beam(w.astype(np.float64))
+    rng = np.random.default_rng(78)
+    order = np.argsort(-np.abs(g))
+    cells = np.unique(np.concatenate([order[:16], rng.choice(cfg.n_cells, size=16, replace=False)]))
+    gfd = o.grad_fd(f, what, cells, eps=1e-5)
+    worst = excess(g[cells], gfd, np.abs(g).max())
+    print("production mode, 128^3 x 256 ch: gradient vs finite differences at %.3g of tolerance (max|g| %.3g), %.2f ms per call" %
+          (worst, np.abs(g).max(), e0.elapsed_time(e1) / 3))
     assert np.all(np.isfinite(g)) and worst <= 1.0
