@@ -1025,6 +1025,8 @@ static iris_so_status observe_adjoint_impl(iris_so_ctx* ctx, const float* d_nH2,
   // the reverse sweep of the other modes stages a column's coefficients and accumulators in shared memory
   if (modes_adjoint && iris::kAdjModesWarps * iris::adjoint_modes_smem_per_warp(c.nz) > 227u * 1024u)
     return fail(ctx, IRIS_SO_EUNSUPPORTED, "adjoint: a column of this many cells does not fit the shared memory of an SM");
+  if (modes_adjoint && (size_t)c.nv * (size_t)(c.subsample + 1) + 1 > 65535u)
+    return fail(ctx, IRIS_SO_EUNSUPPORTED, "adjoint: more than 65535 spectral points per pixel");
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   iris_so_status s = run_coefficients(ctx, d_nH2, d_Tgas, d_Tdust, d_vlos, nullptr, st);
   if (s != IRIS_SO_OK) return s;
