@@ -458,7 +458,14 @@ def bench_small_configs(torch, warmup):
     w = torch.from_numpy(weight_cube(cfg)).to(dev)
     grad = torch.empty((cfg.nz, cfg.ny, cfg.nx), dtype=torch.float32, device=dev)
     ms_adj = timed(lambda: it.observe_adjoint(*sets[0], w, grad=grad), 10)
+    # the same gradient in the paper's production mode (thick, smooth TR + BDF2 + ReLU, f = 1): adjoint_modes_kernel
+    it_p = IrisSO(cfg.with_(integration=1, subsample=1))
+    cube_p = torch.empty(it_p.shape_cube, dtype=torch.float32, device=dev)
+    ms_fwd_p = timed(lambda: it_p.observe(*sets[0], cube=cube_p), 10)
+    ms_adj_p = timed(lambda: it_p.observe_adjoint(*sets[0], w, grad=grad), 10)
+    it_p.close()
     out["batch"] = {"cubes": 64, "ms_per_64_cubes": ms64, "cubes_per_s": 64e3 / ms64, "adjoint_ms_per_cube": ms_adj,
+                    "production_mode_ms_per_cube": ms_fwd_p, "production_mode_adjoint_ms_per_cube": ms_adj_p,
                     "nominal_updates_per_s": 64 * cfg.nx * cfg.ny * cfg.nz * cfg.nv / (ms64 * 1e-3),
                     "what": "64 x (%dx%dx%d cells, %d channels, dust, beam %.3g px, noise %.3g K)"
                             % (cfg.nx, cfg.ny, cfg.nz, cfg.nv, cfg.beam_fwhm_px, cfg.noise_sigma)}

@@ -337,3 +337,35 @@ def test_production_mode_gradient_at_full_size_sampled():
     print("production mode, 128^3 x 256 ch: gradient vs finite differences at %.3g of tolerance (max|g| %.3g), %.2f ms per call" %
           (worst, np.abs(g).max(), e0.elapsed_time(e1) / 3))
     assert np.all(np.isfinite(g)) and worst <= 1.0
+
+
+def test_production_mode_gradient_of_the_medium_cube_sampled():
+    """BASELINE config "medium" (256 x 256 x 288 cells, 512 channels; no dust, no beam) in the production mode: 1025 fine
+    points per spectrum, several blocks of points per pixel, 288-cell columns.  Sampled cells against the oracle's finite
+    differences through that mode's forward march."""
+    from paper_2607_01338_b200 import IrisSO
+    cfg, r = make_workload("medium")
+    cfg = cfg.with_(integration=1, subsample=1)
+    f = make_fields(cfg, r)
+    d = [dev(f[k]) for k in ("nH2", "Tgas", "Tdust", "vlos")]
+    it = IrisSO(cfg)
+    w = weight_cube(cfg)
+    wd = dev(w)
+    g = it.observe_adjoint(*d, wd)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    it.observe_adjoint(*d, wd)
+    e1.record()
+    torch.cuda.synchronize()
+    g = g.cpu().numpy().astype(np.float64).ravel()
+    o = Oracle(cfg)
+    what = o.beam(w.astype(np.float64)) if cfg.beam_fwhm_px > 0 else w.astype(np.float64)
+    rng = np.random.default_rng(79)
+    order = np.argsort(-np.abs(g))
+    cells = np.unique(np.concatenate([order[:12], rng.choice(cfg.n_cells, size=12, replace=False)]))
+    gfd = o.grad_fd(f, what, cells, eps=1e-5)
+    worst = excess(g[cells], gfd, np.abs(g).max())
+    print("production mode, medium cube: gradient vs finite differences at %.3g of tolerance (max|g| %.3g), %.1f ms per call" %
+          (worst, np.abs(g).max(), e0.elapsed_time(e1)))
+    assert np.all(np.isfinite(g)) and worst <= 1.0
