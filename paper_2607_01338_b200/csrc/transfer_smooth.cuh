@@ -396,7 +396,41 @@ transfer_smooth_window_kernel(MarchConsts mc, const float* __restrict__ coef, in
     // the points are D = U d; nz = 1 leaves D = 0
     const float dfin = nz > 1 ? d_fin : 0.0f;
     const float C = C_fin;
-    if (out != nullptr) {
+    if (out != nullptr && mc.out_mode <= OUT_I_TOT) {
+      // the units that are linear in D: one multiply-add per channel, four channels per lane in flight (the loop is a
+      // chain LDS -> FMA -> STG; see the epilogue of transfer_series_kernel)
+      const float sc = mc.out_mode >= OUT_I_SUB ? mc.inv_KRJ : 1.0f;
+      const float b = (mc.out_mode & 1) ? C * sc : 0.0f;
+      float* o = out + (int64_t)pix * nv;
+      if (point) {
+        const float a = dfin / (3.0f * (float)m) * sc;
+        auto channel = [&](int c) {
+          float acc = 0.0f;
+          for (int j = 0; j < m; j += 2) acc += cur[IDX(c * m + j)] + 4.0f * cur[IDX(c * m + j + 1)] + cur[IDX(c * m + j + 2)];
+          return acc;
+        };
+        int c = i;
+        for (; c + 3 * LPP < nv; c += 4 * LPP) {
+          float v[4];
+#pragma unroll
+          for (int k = 0; k < 4; ++k) v[k] = channel(c + k * LPP);
+#pragma unroll
+          for (int k = 0; k < 4; ++k) o[c + k * LPP] = fmaf(v[k], a, b);
+        }
+        for (; c < nv; c += LPP) o[c] = fmaf(channel(c), a, b);
+      } else {
+        const float a = dfin * sc;
+        int c = i;
+        for (; c + 3 * LPP < nv; c += 4 * LPP) {
+          float v[4];
+#pragma unroll
+          for (int k = 0; k < 4; ++k) v[k] = cur[IDX(c + k * LPP)];
+#pragma unroll
+          for (int k = 0; k < 4; ++k) o[c + k * LPP] = fmaf(v[k], a, b);
+        }
+        for (; c < nv; c += LPP) o[c] = fmaf(cur[IDX(c)], a, b);
+      }
+    } else if (out != nullptr) {
       if (point) {
         const float wgt = dfin / (3.0f * (float)m);
         for (int c = i; c < nv; c += LPP) {
