@@ -83,6 +83,9 @@ __device__ __forceinline__ void adj_modes_block(float T_bg, int nz, int nv, int 
   constexpr int STR = 32 * kAdjModesNPT;       // scratch row stride (the same for every NPT)
   // does the line window of cell n reach this block of points?  (warp-uniform.)  Where it does not, every point of the
   // block takes the step without a line: no profile, one reciprocal / exponential per cell instead of per point.
+  // (checked build) every row of stored states lies inside this warp's slab of the scratch
+  const float* ys_end = ys + (size_t)nz * STR;
+  (void)ys_end;
   auto hit = [&](int n) {
     const int wv = win[n], klo = wv & 0xffff, khi = (int)((unsigned)wv >> 16);
     return khi >= klo && klo < q0 + 32 * NPT && khi >= q0;
@@ -169,6 +172,7 @@ __device__ __forceinline__ void adj_modes_block(float T_bg, int nz, int nv, int 
   // of the current one (a warp would otherwise sit out the whole latency once per cell)
   float yc[NPT], yn[NPT];
   auto load_row = [&](int n, float (&dst)[NPT]) {
+    IRIS_CHECK_SMEM(ys + (size_t)n * STR + lane, 4 * (32 * (NPT - 1) + 1), ys, ys_end);
 #pragma unroll
     for (int j = 0; j < NPT; ++j) dst[j] = ys[(size_t)n * STR + 32 * j + lane];
   };

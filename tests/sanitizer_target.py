@@ -1,6 +1,6 @@
 """Small calls of every kernel of the library, meant to be run under compute-sanitizer (tests/test_sanitizers.py):
 every LOS transfer kernel (series modes 0 - 3, window, dense, dense per-channel, modes, smooth window + hand-over list),
-the level / coefficient / grid kernels, beam, noise, diagnostics and the adjoint.  Prints one line per call."""
+the level / coefficient / grid kernels, beam, noise, diagnostics and the adjoints (hot path and the other thick modes).  Prints one line per call."""
 import os
 import sys
 
@@ -29,7 +29,8 @@ def main():
                 ("series thin simpson", dict(transfer_mode=2, integration=1), 0), ("series fine grid", dict(subsample=1), 0),
                 ("smooth window", dict(integration=1), 0), ("smooth window fine", dict(integration=1, subsample=1), 0),
                 ("smooth window hand-over", dict(integration=1, kappa_gas_cm2_g=40.0 * cfg0.kappa_gas_cm2_g), 0),
-                ("modes selectively thin smooth", dict(transfer_mode=1, integration=1), 0),
+                ("smooth window selectively thin", dict(transfer_mode=1, integration=1), 0),
+                ("modes selectively thin smooth", dict(transfer_mode=1, integration=1), 1),
                 ("modes dense thick smooth", dict(integration=1, subsample=3), 1)]
     for name, kw, algo in variants:
         it = IrisSO(cfg0.with_(**kw), transfer_algo=algo)
@@ -49,6 +50,16 @@ def main():
     torch.cuda.synchronize()
     assert bool(torch.isfinite(g).all()) and bool(torch.isfinite(ga).all())
     print("%-32s ok" % "levelpop / transfer / diagnostics / adjoint")
+    # the stored-state reverse sweep of the other thick modes (adjoint_modes_kernel): smooth / formal, coarse / fine grid
+    for name, kw in (("adjoint thick smooth", dict(integration=1)), ("adjoint production mode", dict(integration=1, subsample=1)),
+                     ("adjoint formal fine grid", dict(subsample=3))):
+        itm = IrisSO(cfg0.with_(**kw))
+        gm = itm.observe_adjoint(*d, w)
+        gma = itm.observe_adjoint(*d, w, wrt="abundance")
+        torch.cuda.synchronize()
+        assert bool(torch.isfinite(gm).all()) and bool(torch.isfinite(gma).all()), name
+        print("%-32s ok" % name)
+        itm.close()
     h = [torch.from_numpy(f[k]).pin_memory() for k in ("nH2", "Tgas", "Tdust", "vlos")]
     hc = torch.empty(it.shape_cube, dtype=torch.float32).pin_memory()
     it.observe_host(*h, hc)
