@@ -46,8 +46,8 @@ SM_COUNT, SFU_LANES_PER_SM_CLK, FP32_LANES_PER_SM_CLK = 148, 16.0, 124.9
 # from the committed `ncu --set full` capture of the named profiles/ pass, keyed by (workload, kernel).  Refreshed with
 # every profiles/ pass; `roofline.traffic_source` names the pass in the JSON line.
 NCU_TRAFFIC_BYTES = {
-    ("large", "transfer_series_kernel"): (4407247000, "profiles/r02_final.md (3.2485 + 1.0447 GB reachable-range variant, 0.1106 + 0.0034 GB list pass)"),
-    ("medium", "transfer_series_kernel"): (566557696, "profiles/r02_final.md (453.48 + 113.07 MB)"),
+    ("large", "transfer_series_kernel"): (4412700000, "profiles/r02_final.md (3.2538 + 1.0450 GB reachable-range variant, 0.1105 + 0.0034 GB list pass)"),
+    ("medium", "transfer_series_kernel"): (566200000, "profiles/r02_final.md (453.1 + 113.1 MB)"),
 }
 
 
