@@ -182,6 +182,23 @@ iris_so_status iris_so_observe_stages(iris_so_ctx *ctx, const float *d_nH2, cons
                                       const float *d_Tdust, const float *d_vlos, int32_t stage_mask,
                                       float *d_cube, void *cuda_stream);
 
+/* K1 .. K5 without any allocation, for callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid it): the raw cube of iris_so_observe_stages(..., stage_mask = 0, ...) -- no beam, no noise
+ * -- for the hot-path mode (transfer_mode = integration = subsample = 0, coef_grid = 0, dust_per_channel = 0).  The six
+ * coefficient planes K1 + K2 hand to K3 live in a file-scope `static __device__` array of the library instead of the
+ * context's cudaMalloc'ed scratch: 6 * IRIS_SO_STATIC_MAX_CELLS floats = 12 MiB, held by every GPU that loads the library
+ * until the process exits.  nx * ny * nz > IRIS_SO_STATIC_MAX_CELLS returns IRIS_SO_EUNSUPPORTED (message in
+ * iris_so_last_error).  The call makes no cudaMalloc / cudaFree / cudaHostAlloc and no allocating library call; it launches
+ * K1 + K2 and one transfer kernel on `cuda_stream` and returns without synchronising.  The array is shared by EVERY call
+ * of every context on that GPU and keeps the last call's planes: each call overwrites all 6 * ncell entries it reads
+ * before reading them (nothing has to start at zero), but two calls that overlap on the GPU (different streams, or
+ * different contexts / host threads) race on it -- serialise them.  The device of the context must be current, as for
+ * every other call.  Same layouts as iris_so_observe. */
+#define IRIS_SO_STATIC_MAX_CELLS (1 << 19)
+iris_so_status iris_so_observe_raw_static(iris_so_ctx *ctx, const float *d_nH2, const float *d_Tgas,
+                                          const float *d_Tdust, const float *d_vlos, float *d_cube,
+                                          void *cuda_stream);
+
 /* Whole path with HOST buffers (pinned or pageable): copies the four fields to the device, runs
  * iris_so_observe, copies the cube back and synchronises.  h_* fields [nz][ny][nx], h_cube [ny][nx][nv]. */
 iris_so_status iris_so_observe_host(iris_so_ctx *ctx, const float *h_nH2, const float *h_Tgas,

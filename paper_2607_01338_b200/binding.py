@@ -17,8 +17,9 @@ DECLARED_SYMBOLS = (
     "iris_so_launch_count", "iris_so_scratch_bytes", "iris_so_levelpop", "iris_so_transfer", "iris_so_observe",
     "iris_so_observe_stages", "iris_so_observe_host", "iris_so_observe_adjoint", "iris_so_beam", "iris_so_noise",
     "iris_so_profile", "iris_so_profile_read", "iris_so_transfer_work", "iris_so_transfer_kernel", "iris_so_smooth_fallback",
-    "iris_so_density_trace", "iris_so_metrics", "iris_so_observe_adjoint_abundance",
+    "iris_so_density_trace", "iris_so_metrics", "iris_so_observe_adjoint_abundance", "iris_so_observe_raw_static",
 )
+STATIC_MAX_CELLS = 1 << 19      # IRIS_SO_STATIC_MAX_CELLS of include/iris_so.h
 STAGES = {"cell": 0, "transfer": 1, "beam": 2, "noise": 3, "adjoint": 4}
 
 
@@ -95,6 +96,8 @@ def load_library():
     lib.iris_so_observe_stages.argtypes = [vp, fp, fp, fp, fp, C.c_int32, fp, vp]
     lib.iris_so_observe_host.restype = st
     lib.iris_so_observe_host.argtypes = [vp, fp, fp, fp, fp, fp, vp]
+    lib.iris_so_observe_raw_static.restype = st
+    lib.iris_so_observe_raw_static.argtypes = [vp, fp, fp, fp, fp, fp, vp]
     lib.iris_so_observe_adjoint.restype = st
     lib.iris_so_observe_adjoint.argtypes = [vp, fp, fp, fp, fp, fp, fp, vp]
     lib.iris_so_observe_adjoint_abundance.restype = st
@@ -283,6 +286,15 @@ class IrisSO:
             mask = (1 if beam else 0) | (2 if noise else 0)
             st = self.lib.iris_so_observe_stages(*args, C.c_int32(mask), self._dev(cube, self.n_vox, "cube"), self._stream())
         self._check(st)
+        return cube
+
+    def observe_raw_static(self, nH2, Tgas, Tdust, vlos, cube):
+        """iris_so_observe_raw_static: K1 - K5 (no beam, no noise) of the hot-path mode with the library's static scratch; the
+        library call allocates nothing, so the caller passes the output cube too."""
+        n = self.n_cells
+        self._check(self.lib.iris_so_observe_raw_static(
+            self._h, self._dev(nH2, n, "nH2"), self._dev(Tgas, n, "Tgas"), self._dev(Tdust, n, "Tdust"),
+            self._dev(vlos, n, "vlos"), self._dev(cube, self.n_vox, "cube"), self._stream()))
         return cube
 
     def observe_host(self, nH2, Tgas, Tdust, vlos, cube):

@@ -10,6 +10,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -24,6 +25,12 @@
 #include "adjoint_kernels.cuh"
 #include "adjoint_modes.cuh"
 #include "diagnostics.cuh"
+
+// Scratch of iris_so_observe_raw_static (the entry point that allocates nothing): the six coefficient planes of at most
+// IRIS_SO_STATIC_MAX_CELLS cells, 12 MiB on every GPU that loads the library.  In HOST code this name is a host-side
+// stand-in, not a device address: static_scratch_of_device() resolves it with cudaGetSymbolAddress once per device and
+// the kernels are given that pointer.
+static __device__ __align__(256) float g_static_coef[6 * (size_t)IRIS_SO_STATIC_MAX_CELLS];
 
 namespace {
 
@@ -78,6 +85,8 @@ struct iris_so_ctx {
   cudaEvent_t ev_hand = nullptr;  // recorded after the copy into h_hand
   bool hand_pending = false;
   int64_t hand_npix = 0;          // pixels of that launch
+  float* d_static_coef = nullptr;   // device address of g_static_coef on ctx->device (nullptr: static_err says why)
+  std::string static_err;
   cudaStream_t s_in = nullptr, s_out = nullptr;      // copy streams of the host-buffer path
   std::vector<cudaEvent_t> slab_events;
 };
@@ -108,6 +117,31 @@ iris_so_status ensure(iris_so_ctx* ctx, float** p, size_t bytes, const char* wha
   if (e != cudaSuccess) { *p = nullptr; cudaGetLastError(); return cuda_fail(ctx, e, what); }
   ctx->scratch_bytes += bytes;
   return IRIS_SO_OK;
+}
+
+// Device address of g_static_coef on device `dev`, which must be current: resolved once per device (the symbol has one
+// instance per device that loads the module).  Returns nullptr and the reason in *err when the runtime refuses.
+float* static_scratch_of_device(int dev, std::string* err) {
+  constexpr int kMaxDev = 64;
+  static std::mutex mu;
+  static float* ptr[kMaxDev] = {};
+  static bool tried[kMaxDev] = {};
+  static std::string why[kMaxDev];
+  if (dev < 0 || dev >= kMaxDev) { *err = "device index beyond the table of static scratch addresses"; return nullptr; }
+  std::lock_guard<std::mutex> lock(mu);
+  if (!tried[dev]) {
+    tried[dev] = true;
+    void* p = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&p, g_static_coef);
+    if (e != cudaSuccess) {
+      cudaGetLastError();
+      why[dev] = std::string("cudaGetSymbolAddress(static scratch): ") + cudaGetErrorString(e);
+    } else {
+      ptr[dev] = static_cast<float*>(p);
+    }
+  }
+  if (!ptr[dev]) *err = why[dev];
+  return ptr[dev];
 }
 
 // Brackets the kernels a stage launches with two events on the caller's stream when profiling is on.
@@ -763,6 +797,8 @@ iris_so_status iris_so_create(const iris_so_config* cfg, iris_so_ctx** out) {
     iris_so_status gs = build_grid(ctx);
     if (gs != IRIS_SO_OK) { iris_so_destroy(ctx); return gs; }
   }
+  // set-up for iris_so_observe_raw_static (this device is current): not fatal here, that entry point reports it
+  ctx->d_static_coef = static_scratch_of_device(dev, &ctx->static_err);
   *out = ctx;
   return IRIS_SO_OK;
 }
@@ -826,6 +862,56 @@ iris_so_status iris_so_observe_stages(iris_so_ctx* ctx, const float* d_nH2, cons
 iris_so_status iris_so_observe(iris_so_ctx* ctx, const float* d_nH2, const float* d_Tgas, const float* d_Tdust,
                                const float* d_vlos, float* d_cube, void* stream) {
   return iris_so_observe_stages(ctx, d_nH2, d_Tgas, d_Tdust, d_vlos, 3, d_cube, stream);
+}
+
+// K1 .. K5 of the hot-path mode with the coefficient planes in the library's static scratch (g_static_coef) instead of
+// ctx->d_coef: no allocation of any kind, no event, no synchronisation.  A path of its own (the other entry points are
+// untouched): K1 + K2, then the kernel resolved_algo() names -- the series kernel in its whole-spectrum variant (the
+// reachable-range variant needs a hand-over list, i.e. more scratch), the window kernel or the dense kernel.
+iris_so_status iris_so_observe_raw_static(iris_so_ctx* ctx, const float* d_nH2, const float* d_Tgas, const float* d_Tdust,
+                                          const float* d_vlos, float* d_cube, void* stream) {
+  if (!ctx) return IRIS_SO_EINVAL;
+  if (!d_nH2 || !d_Tgas || !d_Tdust || !d_vlos || !d_cube)
+    return fail(ctx, IRIS_SO_EINVAL, "iris_so_observe_raw_static: NULL pointer");
+  const iris_so_config& c = ctx->cfg;
+  if (!hot_path_mode(c) || c.coef_grid == 1 || c.dust_per_channel)
+    return fail(ctx, IRIS_SO_EUNSUPPORTED,
+                "iris_so_observe_raw_static serves the hot-path mode only (transfer_mode = integration = subsample = 0, "
+                "coef_grid = 0, dust_per_channel = 0)");
+  if (ctx->ncell > (int64_t)IRIS_SO_STATIC_MAX_CELLS) {
+    char buf[256];
+    snprintf(buf, sizeof buf, "iris_so_observe_raw_static: %lld cells exceed the static scratch of %d cells "
+             "(IRIS_SO_STATIC_MAX_CELLS); use iris_so_observe_stages", (long long)ctx->ncell, (int)IRIS_SO_STATIC_MAX_CELLS);
+    return fail(ctx, IRIS_SO_EUNSUPPORTED, buf);
+  }
+  if (!ctx->d_static_coef) return fail(ctx, IRIS_SO_ECUDA, "iris_so_observe_raw_static: " + ctx->static_err);
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  float* coef = ctx->d_static_coef;                    // planes at stride ncell, all 6 * ncell entries written by K1 + K2
+  const bool dust = c.dust_on != 0;
+  const int npix = (int)ctx->npix, nz = c.nz, nv = c.nv;
+#define CALL_(N) launch_cellcoef<N>(ctx, d_nH2, d_Tgas, d_Tdust, d_vlos, coef, st)
+  IRIS_DISPATCH_N(c.n_levels, CALL_)
+#undef CALL_
+  IRIS_CHECK_LAUNCH(ctx, "cellcoef_kernel");
+  const int algo = resolved_algo(c);
+  if (algo == IRIS_SO_ALGO_DENSE || !spectra_fit_shared(c)) {
+    constexpr int CB = 16, NW = 4;
+    const int nx = c.nx, rows = npix / nx;
+    dim3 block(32, NW), grid(((nx + 7) / 8) * ((rows + 3) / 4), (nv + CB * NW - 1) / (CB * NW));
+    if (dust) iris::transfer_dense_kernel<CB, true><<<grid, block, 0, st>>>(ctx->mc, coef, ctx->ncell, npix, nx, nz, nv, d_cube, nullptr);
+    else iris::transfer_dense_kernel<CB, false><<<grid, block, 0, st>>>(ctx->mc, coef, ctx->ncell, npix, nx, nz, nv, d_cube, nullptr);
+    IRIS_CHECK_LAUNCH(ctx, "transfer_dense_kernel");
+    return IRIS_SO_OK;
+  }
+  cudaError_t e;
+  if (algo == IRIS_SO_ALGO_WINDOW)
+    e = iris::launch_transfer_series(ctx->mc, coef, ctx->ncell, npix, nz, nv, dust, (float)(c.dv_cms / c.microturb_cms), d_cube,
+                                     nullptr, st, 0, nullptr, nullptr);
+  else
+    e = iris::launch_transfer_window(ctx->mc, coef, ctx->ncell, npix, nz, nv, dust, ctx->sm_count, d_cube, nullptr, st);
+  ctx->launches++;
+  if (e != cudaSuccess) return cuda_fail(ctx, e, "launch of the line-window transfer kernel (static scratch)");
+  return IRIS_SO_OK;
 }
 
 // Host-buffer path.  Pixel columns are independent up to the beam, so the sky plane is cut into slabs of rows and
