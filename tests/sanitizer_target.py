@@ -60,6 +60,13 @@ def main():
         assert bool(torch.isfinite(gm).all()) and bool(torch.isfinite(gma).all()), name
         print("%-32s ok" % name)
         itm.close()
+    # the entry point that allocates nothing (coefficient planes in the library's static scratch), twice in a row
+    raw = torch.empty(it.shape_cube, dtype=torch.float32, device=dev)
+    for _ in range(2):
+        it.observe_raw_static(*d, raw)
+    torch.cuda.synchronize()
+    assert bool(torch.isfinite(raw).all())
+    print("%-32s ok" % "static-scratch entry point")
     h = [torch.from_numpy(f[k]).pin_memory() for k in ("nH2", "Tgas", "Tdust", "vlos")]
     hc = torch.empty(it.shape_cube, dtype=torch.float32).pin_memory()
     it.observe_host(*h, hc)
