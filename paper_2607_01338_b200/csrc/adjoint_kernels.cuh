@@ -44,7 +44,7 @@ __device__ __forceinline__ void level_fractions_grad(const LevelConsts& lc, floa
   float kf = n, wt = 0.0f;
   int t0 = 0;
   if (TABLE) locate_temperature(tb, T, t0, wt);
-  else kf = n * exp2f(lc.Texp * log2f(T * lc.inv_Tref));
+  else kf = n * pow_approx(T * lc.inv_Tref, lc.Texp);
   float q[N];
   boltzmann_adjacent<N>(lc, T, q);
   // collisional de-excitation rates of the band (per unit kf), and the same times g_u / g_l

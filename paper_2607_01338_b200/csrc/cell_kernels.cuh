@@ -108,7 +108,7 @@ __device__ __forceinline__ void level_fractions(const LevelConsts& lc, float n, 
   float kf = n, wt = 0.0f;
   int t0 = 0;
   if (TABLE) locate_temperature(*tb, T, t0, wt);
-  else kf = n * exp2f(lc.Texp * log2f(T * lc.inv_Tref));
+  else kf = n * pow_approx(T * lc.inv_Tref, lc.Texp);
   float q[N];      // Boltzmann factors of adjacent levels, exp(-(E_i - E_{i-1}) / T)
   boltzmann_adjacent<N>(lc, T, q);
 #pragma unroll
@@ -176,7 +176,7 @@ __device__ __forceinline__ void cell_coefficients(const CoefConsts& cc, float n,
   o[2] = fmaf(vlos - cc.v0, cc.inv_dv, 0.5f);
   o[3] = cc.dv * rsqrtf(fmaf(cc.c_b, T, cc.xi2));
   o[4] = cc.c_d * n;
-  o[5] = cc.dust_on ? cc.hnu_k * rcp_approx(expm1f(cc.hnu_k * rcp_approx(Td))) : 0.0f;
+  o[5] = cc.dust_on ? cc.hnu_k * rcp_approx(expm1_pos(cc.hnu_k * rcp_approx(Td))) : 0.0f;
 }
 
 // K1: pop[N][ncell]
@@ -215,6 +215,109 @@ __global__ void __launch_bounds__(128) cellcoef_kernel(LevelConsts lc, CoefConst
   cell_coefficients(cc, n, T, Tdust[i], vlos[i], xu, xl, o);
 #pragma unroll
   for (int q = 0; q < 6; ++q) coef[(int64_t)q * ncell + i] = o[q];
+}
+
+// ---- K1 + K2 for TWO cells per thread (cells 2 t and 2 t + 1) with packed fp32 arithmetic ------------------------------
+// cellcoef_kernel is bound by instruction issue (86 % of the issue slots, FMA pipe half idle), and 60 % of its
+// instructions are scalar FFMA / FMUL / FADD of the rate matrix, the elimination and the back substitution.  Here both
+// cells of a thread go through those steps in the two halves of f32x2 registers (fma / mul / add.rn.f32x2: one issue slot
+// for two cells); the operations and their order are those of level_fractions / cell_coefficients, element by element, so
+// the results are bit-identical.  MUFU operations (reciprocals, the power law, exp(x) - 1, rsqrt) stay scalar.  The fields
+// are read and the planes written as 8-byte accesses.  Power-law collision rates only (TABLE variants keep the scalar kernel).
+template <int N, int BW>
+__device__ __forceinline__ void level_fractions2(const LevelConsts& lc, float n0, float n1, float T0, float T1, f32x2 (&x)[N],
+                                                 f32x2& inv_tot) {
+  f32x2 R[N][N];
+  const f32x2 kf = pk(n0 * pow_approx(T0 * lc.inv_Tref, lc.Texp), n1 * pow_approx(T1 * lc.inv_Tref, lc.Texp));
+  f32x2 q[N];
+  {
+    const float i0 = 1.0f / T0, i1 = 1.0f / T1;
+    const f32x2 invT = pk(i0, i1), ninvT = pk(-i0, -i1);
+#pragma unroll
+    for (int i = 1; i < N; ++i) {
+      const f32x2 c = pk1(lc.ndE2[i]);
+      const f32x2 nt = mul2(c, ninvT);                    // -t exactly (there is no packed negation)
+      const f32x2 r = fma2(c, invT, nt);
+      float ta, tb;
+      upk(nt, ta, tb);
+      const f32x2 e = pk(ex2_approx(-ta), ex2_approx(-tb));
+      q[i] = fma2(mul2(e, pk1(0.6931471805599453f)), r, e);
+    }
+  }
+#pragma unroll
+  for (int u = 1; u < N; ++u) {
+    f32x2 bz = pk1(1.0f);
+#pragma unroll
+    for (int l = u - 1; l >= 0; --l) {
+      if (u - l > BW) continue;
+      bz = mul2(bz, q[l + 1]);
+      const float4 pr = lc.pr[pair_index(u, l)];
+      R[u][l] = fma2(kf, pk1(pr.x), pk1(pr.y));
+      R[l][u] = fma2(mul2(kf, bz), pk1(pr.z), pk1(pr.w));
+    }
+  }
+#pragma unroll
+  for (int m = N - 1; m >= 1; --m) {
+    const int lo = m - BW > 0 ? m - BW : 0;
+    f32x2 sum = pk1(0.0f);
+#pragma unroll
+    for (int j = 0; j < m; ++j)
+      if (j >= lo) sum = add2(sum, R[m][j]);
+    float sa, sb;
+    upk(sum, sa, sb);
+    const f32x2 inv = pk(rcp_approx(sa), rcp_approx(sb));
+#pragma unroll
+    for (int i = 0; i < m; ++i)
+      if (i >= lo) R[i][m] = mul2(R[i][m], inv);
+#pragma unroll
+    for (int i = 0; i < m; ++i)
+#pragma unroll
+      for (int j = 0; j < m; ++j)
+        if (i != j && i >= lo && j >= lo) R[i][j] = fma2(R[i][m], R[m][j], R[i][j]);
+  }
+  x[0] = pk1(1.0f);
+  f32x2 tot = pk1(1.0f);
+#pragma unroll
+  for (int j = 1; j < N; ++j) {
+    f32x2 sum = pk1(0.0f);
+#pragma unroll
+    for (int i = 0; i < j; ++i)
+      if (j - i <= BW) sum = fma2(x[i], R[i][j], sum);
+    x[j] = sum;
+    tot = add2(tot, sum);
+  }
+  float ta, tb;
+  upk(tot, ta, tb);
+  inv_tot = pk(rcp_approx(ta), rcp_approx(tb));
+}
+
+template <int N, int BW>
+__global__ void __launch_bounds__(128) cellcoef2_kernel(LevelConsts lc, CoefConsts cc, int64_t ncell,
+                                                        const float* __restrict__ nH2, const float* __restrict__ Tgas,
+                                                        const float* __restrict__ Tdust, const float* __restrict__ vlos,
+                                                        float* __restrict__ coef) {
+  // ncell is even and every pointer 8-byte aligned (the host checks)
+  const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (2 * t >= ncell) return;
+  const float2 n = reinterpret_cast<const float2*>(nH2)[t], T = reinterpret_cast<const float2*>(Tgas)[t];
+  const float2 Td = reinterpret_cast<const float2*>(Tdust)[t], v = reinterpret_cast<const float2*>(vlos)[t];
+  f32x2 x[N], inv;
+  level_fractions2<N, BW>(lc, n.x, n.y, T.x, T.y, x, inv);
+  f32x2 xu2 = pk1(0.0f), xl2 = pk1(0.0f);
+#pragma unroll
+  for (int l = 0; l < N; ++l) {
+    xu2 = fma2(x[l], pk1(cc.pick_upper[l]), xu2);
+    xl2 = fma2(x[l], pk1(cc.pick_lower[l]), xl2);
+  }
+  xu2 = mul2(xu2, inv); xl2 = mul2(xl2, inv);
+  float xu0, xu1, xl0, xl1;
+  upk(xu2, xu0, xu1);
+  upk(xl2, xl0, xl1);
+  float o0[6], o1[6];
+  cell_coefficients(cc, n.x, T.x, Td.x, v.x, xu0, xl0, o0);
+  cell_coefficients(cc, n.y, T.y, Td.y, v.y, xu1, xl1, o1);
+#pragma unroll
+  for (int q = 0; q < 6; ++q) reinterpret_cast<float2*>(coef + (int64_t)q * ncell)[t] = make_float2(o0[q], o1[q]);
 }
 
 // ---- Grid precomputation and lookup (section 4.2, and section 4.3) -------------

@@ -19,6 +19,56 @@ __device__ __forceinline__ float rcp_approx(float x) {
   return y;
 }
 
+__device__ __forceinline__ float lg2_approx(float x) {
+  float y;
+  asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+
+// x^p for x > 0 with the SFU: 2^(p log2 x).  MUFU.LG2 has an absolute error of 2^-22 on (0.5, 2) and a relative one of 2^-22
+// elsewhere, so |log2 x| <= 10 and |p| <= 2 keep the result within 2e-6 relative.
+__device__ __forceinline__ float pow_approx(float x, float p) { return ex2_approx(p * lg2_approx(x)); }
+
+// exp(x) - 1 for x >= 0 to ~2e-7 relative: series through x^6 / 720 below 0.25 (truncation 5e-8), 2^(x log2 e) - 1 above
+// (cancellation <= 6e-8 / 0.28, argument rounding 6e-8 x); both evaluated and selected.  12 instructions against ~35 of expm1f.
+__device__ __forceinline__ float expm1_pos(float x) {
+  const float big = ex2_approx(x * 1.4426950408889634f) - 1.0f;
+  float p = fmaf(x, 1.0f / 720.0f, 1.0f / 120.0f);
+  p = fmaf(p, x, 1.0f / 24.0f);
+  p = fmaf(p, x, 1.0f / 6.0f);
+  p = fmaf(p, x, 0.5f);
+  p = fmaf(p, x, 1.0f);
+  return x < 0.25f ? p * x : big;
+}
+
+// ---- packed fp32 pairs (sm_100: FFMA2 / FMUL2 / FADD2), carried in 64-bit registers
+typedef unsigned long long f32x2;
+
+__device__ __forceinline__ f32x2 pk(float lo, float hi) {
+  f32x2 r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ f32x2 pk1(float v) { return pk(v, v); }
+__device__ __forceinline__ void upk(f32x2 v, float& lo, float& hi) {
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) {
+  f32x2 r;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+  return r;
+}
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) {
+  f32x2 r;
+  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+  return r;
+}
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) {
+  f32x2 r;
+  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+  return r;
+}
+
 // "Signed complementary error function"  G(x) = sign(x) * erfc(|x|)   (so erf(x) = sign(x) - G(x)).
 // erfc(t) = 2^(t Q(t)) with a degree-10 polynomial (erfc_poly.inc): absolute error ~5e-8 near the line
 // centre and RELATIVE error ~2e-6 in the wings, which a plain erf cannot give in fp32 (erf -> 1).

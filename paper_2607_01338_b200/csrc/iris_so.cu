@@ -381,6 +381,14 @@ void launch_cellcoef(iris_so_ctx* ctx, const float* n, const float* T, const flo
   const unsigned grid = (unsigned)((nc + 127) / 128);
   constexpr int BN = iris::kBandNarrow < N - 1 ? iris::kBandNarrow : N - 1;
   const bool table = ctx->lc.tb.K != nullptr;
+  // two cells per thread with packed arithmetic (bit-identical results, cell_kernels.cuh) where the 8-byte accesses line up
+  const bool pairs = !table && ctx->band <= BN && nc % 2 == 0 &&
+                     ((reinterpret_cast<uintptr_t>(n) | reinterpret_cast<uintptr_t>(T) | reinterpret_cast<uintptr_t>(Td) |
+                       reinterpret_cast<uintptr_t>(v) | reinterpret_cast<uintptr_t>(coef)) % 8 == 0);
+  if (pairs) {
+    iris::cellcoef2_kernel<N, BN><<<(unsigned)((nc / 2 + 127) / 128), 128, 0, st>>>(ctx->lc, ctx->cc, nc, n, T, Td, v, coef);
+    return;
+  }
   if (ctx->band <= BN) {
     if (table) iris::cellcoef_kernel<N, BN, true><<<grid, 128, 0, st>>>(ctx->lc, ctx->cc, nc, n, T, Td, v, coef);
     else iris::cellcoef_kernel<N, BN, false><<<grid, 128, 0, st>>>(ctx->lc, ctx->cc, nc, n, T, Td, v, coef);

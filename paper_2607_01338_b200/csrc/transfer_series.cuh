@@ -143,33 +143,7 @@ __device__ __forceinline__ SeriesRecord make_series_record(float e_c, float a_c,
   return r;
 }
 
-// ---- packed fp32 pairs (sm_100: FFMA2 / FMUL2 / FADD2), carried in 64-bit registers
-typedef unsigned long long f32x2;
-
-__device__ __forceinline__ f32x2 pk(float lo, float hi) {
-  f32x2 r;
-  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
-  return r;
-}
-__device__ __forceinline__ f32x2 pk1(float v) { return pk(v, v); }
-__device__ __forceinline__ void upk(f32x2 v, float& lo, float& hi) {
-  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
-}
-__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) {
-  f32x2 r;
-  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
-  return r;
-}
-__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) {
-  f32x2 r;
-  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
-  return r;
-}
-__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) {
-  f32x2 r;
-  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
-  return r;
-}
+// (packed fp32 pairs -- f32x2, pk, pk1, upk, fma2, mul2, add2 -- are in iris_math.cuh)
 
 // Per-cell operands of the update, duplicated into both halves of a packed register.
 struct SeriesCellOps {

@@ -614,3 +614,38 @@ def test_reachable_range_spectra_hand_over(wide_columns):
     assert iris(cfg, 1).smooth_fallback() == 0
     print("reachable-range spectra, %d wide columns: %d / %d pixels handed over, worst pixel at %.3g of tolerance"
           % (wide_columns, n1, n2, worst))
+
+
+def test_packed_cell_kernel_is_bit_identical_to_the_scalar_one():
+    """K1 + K2 run two cells per thread with packed f32x2 arithmetic (cellcoef2_kernel) when the cell count is even and the
+    field pointers are 8-byte aligned, and one cell per thread otherwise (cellcoef_kernel): the same operations in the same
+    order, so the cubes must agree bit for bit.  Fields at a 4-byte offset force the scalar kernel."""
+    from paper_2607_01338_b200 import IrisSO
+    cfg, r = make_workload("small", n=40, nv=64)
+    cfg = cfg.with_(beam_fwhm_px=0.0, noise_sigma=0.0)
+    f = make_fields(cfg, r)
+    f["vlos"] = (0.25 * f["vlos"]).astype(np.float32)
+    assert cfg.n_cells % 2 == 0
+    it = IrisSO(cfg)
+    d = [torch.from_numpy(np.ascontiguousarray(f[k])).cuda() for k in ("nH2", "Tgas", "Tdust", "vlos")]
+    shifted = []
+    for t in d:
+        buf = torch.empty(t.numel() + 1, dtype=torch.float32, device="cuda")
+        buf[1:] = t.flatten()
+        shifted.append(buf[1:].view(t.shape))
+        assert shifted[-1].data_ptr() % 8 == 4 and t.data_ptr() % 8 == 0
+    It_a, Ic_a = it.transfer(*d)
+    It_b, Ic_b = it.transfer(*shifted)
+    assert torch.equal(It_a, It_b) and torch.equal(Ic_a, Ic_b)
+    # and both against the oracle on the cube
+    cube = it.observe(*d, beam=False, noise=False).cpu().numpy()
+    assert_spectra(cube, Oracle(cfg).observe(f, beam=False, noise=False), what="packed cell kernel")
+    # an odd number of cells takes the scalar kernel too
+    cfg_o, r_o = make_workload("small", nx=7, ny=5, nz=9, nv=32)
+    cfg_o = cfg_o.with_(beam_fwhm_px=0.0, noise_sigma=0.0)
+    f_o = make_fields(cfg_o, r_o)
+    f_o["vlos"] = (0.1 * f_o["vlos"]).astype(np.float32)
+    d_o = [torch.from_numpy(np.ascontiguousarray(f_o[k])).cuda() for k in ("nH2", "Tgas", "Tdust", "vlos")]
+    assert cfg_o.n_cells % 2 == 1
+    assert_spectra(IrisSO(cfg_o).observe(*d_o, beam=False, noise=False).cpu().numpy(),
+                   Oracle(cfg_o).observe(f_o, beam=False, noise=False), what="odd cell count")
