@@ -248,16 +248,20 @@ transfer_modes_kernel(MarchConsts mc, ModeConsts md, const float* __restrict__ c
   }
 
   // ---- channel values of this thread -> convert and store
+  // (modes with the ReLU keep I_T = D + C >= 0 point by point, hence for a Simpson average too; the clamp below only
+  // removes the rounding of the average)
+  constexpr bool RELU = MODE != 2 && (SMOOTH || MODE == 1);
+  auto conv = [&](float D) { return convert_out(RELU ? fmaxf(D, -Cfin) : D, Cfin, mc); };
   constexpr int NRES = PROF == 0 ? kModesCh0 : 8;
   float res[NRES];
   int nch = min(cpb, nv - v0);
   if constexpr (PROF == 0) {
 #pragma unroll
-    for (int k = 0; k < NRES; ++k) res[k] = convert_out(Dfin[k], Cfin, mc);
+    for (int k = 0; k < NRES; ++k) res[k] = conv(Dfin[k]);
   } else if constexpr (PROF == 3) {
 #pragma unroll
     for (int c = 0; c < 8; ++c)
-      res[c] = convert_out((Dfin[2 * c] + 4.0f * Dfin[2 * c + 1] + Dfin[2 * c + 2]) * (1.0f / 6.0f), Cfin, mc);
+      res[c] = conv((Dfin[2 * c] + 4.0f * Dfin[2 * c + 1] + Dfin[2 * c + 2]) * (1.0f / 6.0f));
   } else if constexpr (PROF == 1) {
 #pragma unroll
     for (int c = 0; c < 4; ++c) {                     // at most 2 channels (m = 4)
@@ -276,10 +280,10 @@ transfer_modes_kernel(MarchConsts mc, ModeConsts md, const float* __restrict__ c
           acc += d0 + 4.0f * d1 + d2;
         }
       }
-      res[c] = convert_out(acc * (inv_m * (1.0f / 3.0f)), Cfin, mc);
+      res[c] = conv(acc * (inv_m * (1.0f / 3.0f)));
     }
   } else {
-    res[0] = convert_out(Dacc, Cfin, mc);
+    res[0] = conv(Dacc);
   }
   if (out != nullptr) {
     float* o = out + (int64_t)pix * nv + v0;

@@ -468,7 +468,7 @@ transfer_series_kernel(MarchConsts mc, const float* __restrict__ coef, int64_t n
     if (out != nullptr) {
       float* o = out + (int64_t)pix * nv;
       const bool al = ((((int64_t)pix * nv) & 1) == 0);      // float2 stores need an even element offset
-      if (mc.out_mode <= OUT_I_TOT && al && (nv & 1) == 0) {
+      if (MODE != 1 && mc.out_mode <= OUT_I_TOT && al && (nv & 1) == 0) {
         // the units that are linear in D (Rayleigh-Jeans Kelvin or intensity, with or without the continuum): one
         // multiply-add per value, four pairs per lane in flight (the loop is latency-bound: LDS -> FMA -> STG)
         const float sc = mc.out_mode >= OUT_I_SUB ? mc.inv_KRJ : 1.0f;
@@ -490,9 +490,12 @@ transfer_series_kernel(MarchConsts mc, const float* __restrict__ coef, int64_t n
       } else
       for (int q = i; 2 * q < nv; q += LPP) {
         const float2 v = pair_at(q);
-        const float r0 = convert_out(v.x * invG, C, mc);
+        // (selectively thin: the ReLU keeps I_T = D + C >= 0; the clamp was applied to the dust-scaled spectrum, and
+        // unscaling it can leave D one rounding below -C)
+        const float d0 = MODE == 1 ? fmaxf(v.x * invG, -C) : v.x * invG, d1 = MODE == 1 ? fmaxf(v.y * invG, -C) : v.y * invG;
+        const float r0 = convert_out(d0, C, mc);
         if (2 * q + 1 < nv) {
-          const float r1 = convert_out(v.y * invG, C, mc);
+          const float r1 = convert_out(d1, C, mc);
           if (al) *reinterpret_cast<float2*>(o + 2 * q) = make_float2(r0, r1);
           else { o[2 * q] = r0; o[2 * q + 1] = r1; }
         } else {

@@ -400,10 +400,11 @@ transfer_smooth_window_kernel(MarchConsts mc, const float* __restrict__ coef, in
       // the units that are linear in D: one multiply-add per channel, four channels per lane in flight (the loop is a
       // chain LDS -> FMA -> STG; see the epilogue of transfer_series_kernel)
       const float sc = mc.out_mode >= OUT_I_SUB ? mc.inv_KRJ : 1.0f;
-      const float b = (mc.out_mode & 1) ? C * sc : 0.0f;
+      const float cadd = (mc.out_mode & 1) ? C : 0.0f;      // total = (D + C) sc is exactly 0 where the ReLU holds D at -C
       float* o = out + (int64_t)pix * nv;
+      // (the ReLU keeps I_T = D + C >= 0 at every step; D = U d_fin can come out one rounding below -C: clamp)
       if (point) {
-        const float a = dfin / (3.0f * (float)m) * sc;
+        const float a = dfin / (3.0f * (float)m);
         auto channel = [&](int c) {
           float acc = 0.0f;
           for (int j = 0; j < m; j += 2) acc += cur[IDX(c * m + j)] + 4.0f * cur[IDX(c * m + j + 1)] + cur[IDX(c * m + j + 2)];
@@ -415,20 +416,20 @@ transfer_smooth_window_kernel(MarchConsts mc, const float* __restrict__ coef, in
 #pragma unroll
           for (int k = 0; k < 4; ++k) v[k] = channel(c + k * LPP);
 #pragma unroll
-          for (int k = 0; k < 4; ++k) o[c + k * LPP] = fmaf(v[k], a, b);
+          for (int k = 0; k < 4; ++k) o[c + k * LPP] = (fmaxf(v[k] * a, -C) + cadd) * sc;
         }
-        for (; c < nv; c += LPP) o[c] = fmaf(channel(c), a, b);
+        for (; c < nv; c += LPP) o[c] = (fmaxf(channel(c) * a, -C) + cadd) * sc;
       } else {
-        const float a = dfin * sc;
+        const float a = dfin;
         int c = i;
         for (; c + 3 * LPP < nv; c += 4 * LPP) {
           float v[4];
 #pragma unroll
           for (int k = 0; k < 4; ++k) v[k] = cur[IDX(c + k * LPP)];
 #pragma unroll
-          for (int k = 0; k < 4; ++k) o[c + k * LPP] = fmaf(v[k], a, b);
+          for (int k = 0; k < 4; ++k) o[c + k * LPP] = (fmaxf(v[k] * a, -C) + cadd) * sc;
         }
-        for (; c < nv; c += LPP) o[c] = fmaf(cur[IDX(c)], a, b);
+        for (; c < nv; c += LPP) o[c] = (fmaxf(cur[IDX(c)] * a, -C) + cadd) * sc;
       }
     } else if (out != nullptr) {
       if (point) {
@@ -436,10 +437,10 @@ transfer_smooth_window_kernel(MarchConsts mc, const float* __restrict__ coef, in
         for (int c = i; c < nv; c += LPP) {
           float acc = 0.0f;
           for (int j = 0; j < m; j += 2) acc += cur[IDX(c * m + j)] + 4.0f * cur[IDX(c * m + j + 1)] + cur[IDX(c * m + j + 2)];
-          out[(int64_t)pix * nv + c] = convert_out(acc * wgt, C, mc);
+          out[(int64_t)pix * nv + c] = convert_out(fmaxf(acc * wgt, -C), C, mc);
         }
       } else {
-        for (int c = i; c < nv; c += LPP) out[(int64_t)pix * nv + c] = convert_out(cur[IDX(c)] * dfin, C, mc);
+        for (int c = i; c < nv; c += LPP) out[(int64_t)pix * nv + c] = convert_out(fmaxf(cur[IDX(c)] * dfin, -C), C, mc);
       }
     }
     if (out_cont != nullptr && i == 0) out_cont[pix] = C * mc.inv_KRJ;

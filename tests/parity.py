@@ -51,8 +51,9 @@ def assert_spectra(gpu, ora, floor=1e-6, rel=1e-4, extra=0.0, peak_of=None, what
 
 
 def selthin_source_allowance(cfg, fields):
-    """Float32 rounding allowance [npix, nv] (Kelvin) of the selectively thin mode with the smooth integrator
-    (DESIGN.md "Tolerances").  Its step  D_n = [2 (E_n - A_n C_n) + 4 D_n-1 - D_n-2] / (3 + 2 tau_d)  has no line opacity
+    """Float32 rounding allowance [npix, nv] (Kelvin) of the selectively thin mode (derived for
+    the smooth integrator, the formal step D' = E_d D + (E - A C') w(tau_d) is unsaturated in the same way).
+    The step  D_n = [2 (E_n - A_n C_n) + 4 D_n-1 - D_n-2] / (3 + 2 tau_d)  has no line opacity
     in the denominator (Eq. 4.8.13 - 4.8.15: the line does not absorb itself), so the products E_n = e p and A_n C_n
     enter at full size whatever the optical depth, each formed by up to four float32 roundings (2^-22 relative), and the
     root 1 of the BDF2 recurrence keeps every one of them: |error| <= 2^-22 sum_n (E_n + A_n C_n) beside the usual
@@ -70,3 +71,42 @@ def selthin_source_allowance(cfg, fields):
     c2[0] = coef[0] + coef[1] * np.tile(C_max, cfg.nz)
     S, S_cont = o.march(c2, fields["vlos"])
     return 2.0 ** -21 * krj(cfg.nu0_Hz) * (S - S_cont[:, None])
+
+
+# ---- allowances of the randomised campaign (tests/test_gpu_random.py; DESIGN.md "Tolerances") -------------------------------
+def total_allowance(ora_total, ora_subtracted):
+    """[..., 1] Kelvin.  The CUDA path marches D = I_T - I_C next to the continuum C, so a value that is printed as a
+    total (or a line seen in absorption against a bright continuum) carries the float32 rounding of max(|total|, C):
+    3e-7 of it (storage rounding of both, and of their sum)."""
+    cont = np.abs(np.asarray(ora_total) - np.asarray(ora_subtracted)).max(axis=-1, keepdims=True)
+    return 3e-7 * np.maximum(np.abs(ora_total).max(axis=-1, keepdims=True), cont)
+
+
+def line_centre_allowance(cfg, ora_subtracted):
+    """[..., 1] Kelvin.  The line-centre plane c_los = (v_los - v0) / dv + 1/2 is a float32 in channel units: its rounding
+    (6e-8 nv channels) times the channel width in Doppler widths (<= dv / xi) moves the profile of a cell by that much of a
+    Doppler width; negligible for resolved lines (dv < b), 1e-4 of the peak for 200 channels 6 Doppler widths wide."""
+    return 1.2e-7 * cfg.nv * (cfg.dv_cms / cfg.microturb_cms) * np.abs(ora_subtracted).max(axis=-1, keepdims=True)
+
+
+def cancellation_allowance(cfg, fields, delta=2.0e-6):
+    """[npix, nv] Kelvin.  K1's level fractions are within 1.2e-6 relative of the oracle's (north_star asks 1e-5), so the
+    emission and the absorption of every cell carry ~2e-6 relative each.  Where the line source function S_L is close to
+    the continuum the line is seen against (excitation temperature ~ background temperature), D = sum_n (S_L,n - C)
+    (1 - e^-tau_n) e^-tau_beyond is a small difference of terms that do not share that error: the bound is delta times the
+    same sum with S_L,n + C_max, i.e. the formal thick solution (oracle, hot-path mode) of the column with j0 replaced by
+    j0 + kappa0 C_max, no dust and no background."""
+    from oracle import Oracle
+    plane = cfg.nx * cfg.ny
+    c0 = cfg.with_(transfer_mode=0, integration=0, subsample=0, subtract_continuum=False, out_unit=0, T_cmb=0.0, coef_grid=0,
+                   dust_per_channel=0)
+    coef = Oracle(cfg.with_(coef_grid=0)).coefficients(fields["nH2"], fields["Tgas"], fields["Tdust"])
+    I_bg = Oracle(cfg).planck(cfg.nu0_Hz, cfg.T_cmb) if cfg.T_cmb > 0 else 0.0
+    C_max = np.maximum(I_bg, coef[4].reshape(cfg.nz, plane).max(axis=0))
+    c2 = coef.copy()
+    c2[0] = coef[0] + np.abs(coef[1]) * np.tile(C_max, cfg.nz)
+    c2[1] = np.abs(coef[1])
+    c2[3] = 0.0
+    c2[4] = 0.0
+    I, _ = Oracle(c0).march(c2, fields["vlos"])
+    return delta * krj(cfg.nu0_Hz) * I
