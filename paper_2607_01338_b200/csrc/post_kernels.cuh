@@ -20,11 +20,19 @@ struct NoiseConsts {
 // z ~ N(0,1) per voxel (reading S10): one Philox4x32-10(key, counter = voxel / 4) call serves four
 // consecutive voxels; words (r0, r1) the voxels 4c, 4c+1, words (r2, r3) the voxels 4c+2, 4c+3; a word pair gives
 // u1, u2 and the two Box-Muller deviates sqrt(-2 ln u1) cos(2 pi u2) (even voxel), sqrt(-2 ln u1) sin(2 pi u2) (odd).
-// The uniforms use the top 24 bits, so they are exact in fp32 and identical to the float64 definition.
+// The uniforms use the top 24 bits: k + 1/2 is exact in fp32 for k < 2^23 only; above, it rounds to k or k + 1.  For the
+// radius that matters where u1 is close to 1 (ln u1 = -(1 - u1): a rounding of 2^-25 in u1 is an absolute error of 3e-8 in
+// ln u1, i.e. 1e-5 in a deviate of 1e-3, and u1 = 1 - 2^-25 rounds to 1, R = 0), so the known residual
+// (k + 1/2) - fl(k + 1/2) in {0, +-1/2} is put back to first order: ln u1 = ln(u~) + (u1 - u~) / u~ (the next term is 1e-15).
+// For the angle the rounding of u2 moves a deviate by 2e-7 R.
 __device__ __forceinline__ void box_muller_pair(uint32_t ra, uint32_t rb, float& z_even, float& z_odd) {
-  const float u1 = ((float)(ra >> 8) + 0.5f) * (1.0f / 16777216.0f);
+  const float kf = (float)(ra >> 8);                      // exact
+  const float t = kf + 0.5f;                              // rounded above 2^23
+  const float resid = (kf - t) + 0.5f;                    // exact: 0 below 2^23, +-1/2 above
+  const float u1 = t * (1.0f / 16777216.0f);
+  const float ln_u1 = fmaf(resid * (1.0f / 16777216.0f), rcp_approx(u1), logf(u1));
   const float u2 = ((float)(rb >> 8) + 0.5f) * (1.0f / 16777216.0f);
-  const float R = sqrtf(-2.0f * logf(u1));
+  const float R = sqrtf(-2.0f * ln_u1);
   float sn, cs;
   sincospif(2.0f * u2, &sn, &cs);
   z_even = R * cs;
