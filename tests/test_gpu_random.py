@@ -147,3 +147,45 @@ def test_random_gradients_match_the_oracle(seed):
         it.close()
     print("seed %d: %d random gradients, worst cell at %.3g of the bound" % (seed, ran, worst))
     assert ran >= 40
+
+
+@pytest.mark.parametrize("seed", range(1, 4))
+def test_random_molecules_match_the_oracle_populations(seed):
+    """K1 on random molecules: 2 - 10 levels, random rate-matrix bandwidths (banded and dense elimination), analytic power-law
+    rates with random exponents and a random radiation temperature or random tables (1 - 13 temperatures, 1 - 4 partners),
+    densities 1e-2 .. 1e9 cm^-3 and temperatures 5 .. 3000 K drawn log-uniformly per cell; component-wise relative error of
+    every level fraction <= 1e-5 (north_star)."""
+    from paper_2607_01338_b200 import IrisSO
+    from parity import pop_errors
+    worst = 0.0
+    for case in range(100):
+        rng = np.random.default_rng(9000000 + 100000 * seed + case)
+        N = int(rng.integers(2, 11))
+        max_dj = int(rng.integers(1, N)) if N > 2 else 1
+        cfg, _ = make_workload("small", nx=int(rng.integers(1, 50)), ny=int(rng.integers(1, 20)), nz=int(rng.integers(1, 9)), nv=8,
+                               n_levels=N, seed=int(rng.integers(1 << 30)))
+        if rng.integers(2):
+            grid = np.unique(np.round(np.sort(10 ** rng.uniform(0.7, 3.3, int(rng.integers(1, 14)))), 3))
+            nP = int(rng.integers(1, 5))
+            tab = np.zeros((nP, grid.size, N, N))
+            for p in range(nP):
+                for u in range(1, N):
+                    for l in range(max(0, u - max_dj), u):
+                        tab[p, :, u, l] = rng.uniform(0.3, 3.0) * 1e-11 * (grid / 100.0) ** rng.uniform(-0.5, 1.0) / (u - l)
+            cfg = cfg.with_(coll_T_grid=grid, coll_table=tab, coll_partner_frac=rng.uniform(0.05, 1.0, nP))
+        else:
+            Kd = np.array(cfg.coll_down_ref, dtype=np.float64, copy=True)
+            for u in range(1, N):
+                for l in range(u):
+                    Kd[u, l] = (10 ** rng.uniform(-12, -10)) / (u - l) if u - l <= max_dj else 0.0
+            cfg = cfg.with_(coll_down_ref=Kd, coll_T_exp=float(rng.uniform(-0.5, 1.5)), T_bar=float(rng.choice([0.0, 2.725, 20.0])))
+        n = (10 ** rng.uniform(-2, 9, (cfg.nz, cfg.ny, cfg.nx))).astype(np.float32)
+        T = (10 ** rng.uniform(np.log10(5), np.log10(3000), n.shape)).astype(np.float32)
+        it = IrisSO(cfg)
+        pop = it.levelpop(torch.from_numpy(n).cuda(), torch.from_numpy(T).cuda()).cpu().numpy().reshape(N, -1)
+        rel, absmax = pop_errors(pop, np.asarray(Oracle(cfg).levelpop(n, T)).reshape(N, -1))
+        assert rel <= 1e-5 and absmax <= 1e-35, "seed %d case %d (%d levels, dJ <= %d, tables %s): rel %.3g" % (
+            seed, case, N, max_dj, cfg.coll_table is not None, rel)
+        worst = max(worst, rel)
+        it.close()
+    print("seed %d: 100 random molecules, worst level fraction at %.3g relative" % (seed, worst))
