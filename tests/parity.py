@@ -82,20 +82,23 @@ def total_allowance(ora_total, ora_subtracted):
     return 3e-7 * np.maximum(np.abs(ora_total).max(axis=-1, keepdims=True), cont)
 
 
-def line_centre_allowance(cfg, ora_subtracted):
+def line_centre_allowance(cfg, ora_subtracted, saturated=None):
     """[..., 1] Kelvin.  The line-centre plane c_los = (v_los - v0) / dv + 1/2 is a float32 in channel units: its rounding
     (6e-8 nv channels) times the channel width in Doppler widths (<= dv / xi) moves the profile of a cell by that much of a
-    Doppler width; negligible for resolved lines (dv < b), 1e-4 of the peak for 200 channels 6 Doppler widths wide."""
-    return 1.2e-7 * cfg.nv * (cfg.dv_cms / cfg.microturb_cms) * np.abs(ora_subtracted).max(axis=-1, keepdims=True)
+    Doppler width; negligible for resolved lines (dv < b), 1e-4 of the peak for 200 channels 6 Doppler widths wide.
+    `saturated` (saturated_source of the same configuration, thick modes): a pixel that shows only the WINGS of opaque cells
+    (a 1 K spectrum out of cells with S_L = 26 K at 2 - 3 Doppler widths, where d ln(profile) / dx = -2 x) answers to the
+    shift with the source function of those cells, not with its own peak: the scale is then the larger of the two."""
+    scale = np.abs(ora_subtracted).max(axis=-1, keepdims=True)
+    if saturated is not None:
+        scale = np.maximum(scale, np.asarray(saturated).reshape(ora_subtracted.shape).max(axis=-1, keepdims=True))
+    return 1.2e-7 * cfg.nv * (cfg.dv_cms / cfg.microturb_cms) * scale
 
 
-def cancellation_allowance(cfg, fields, delta=2.0e-6):
-    """[npix, nv] Kelvin.  K1's level fractions are within 1.2e-6 relative of the oracle's (north_star asks 1e-5), so the
-    emission and the absorption of every cell carry ~2e-6 relative each.  Where the line source function S_L is close to
-    the continuum the line is seen against (excitation temperature ~ background temperature), D = sum_n (S_L,n - C)
-    (1 - e^-tau_n) e^-tau_beyond is a small difference of terms that do not share that error: the bound is delta times the
-    same sum with S_L,n + C_max, i.e. the formal thick solution (oracle, hot-path mode) of the column with j0 replaced by
-    j0 + kappa0 C_max, no dust and no background."""
+def saturated_source(cfg, fields):
+    """[npix, nv] Kelvin: sum_n (S_L,n + C_max) (1 - e^-tau_n) e^-tau_beyond, the formal thick solution (oracle, hot-path
+    mode) of the column with j0 replaced by j0 + kappa0 C_max, no dust and no background -- what every cell can put into a
+    channel at most, the scale the allowances below are proportional to."""
     from oracle import Oracle
     plane = cfg.nx * cfg.ny
     c0 = cfg.with_(transfer_mode=0, integration=0, subsample=0, subtract_continuum=False, out_unit=0, T_cmb=0.0, coef_grid=0,
@@ -109,4 +112,13 @@ def cancellation_allowance(cfg, fields, delta=2.0e-6):
     c2[3] = 0.0
     c2[4] = 0.0
     I, _ = Oracle(c0).march(c2, fields["vlos"])
-    return delta * krj(cfg.nu0_Hz) * I
+    return krj(cfg.nu0_Hz) * I
+
+
+def cancellation_allowance(cfg, fields, delta=2.0e-6, saturated=None):
+    """[npix, nv] Kelvin.  K1's level fractions are within 1.2e-6 relative of the oracle's (north_star asks 1e-5), so the
+    emission and the absorption of every cell carry ~2e-6 relative each.  Where the line source function S_L is close to
+    the continuum the line is seen against (excitation temperature ~ background temperature), D = sum_n (S_L,n - C)
+    (1 - e^-tau_n) e^-tau_beyond is a small difference of terms that do not share that error: the bound is delta times the
+    same sum with S_L,n + C_max (saturated_source)."""
+    return delta * (saturated_source(cfg, fields) if saturated is None else saturated)

@@ -15,8 +15,8 @@ torch = pytest.importorskip("torch")
 
 from iris_inputs import make_fields, make_workload
 from oracle import Oracle
-from parity import (cancellation_allowance, line_centre_allowance, selthin_source_allowance, spectrum_excess,
-                    total_allowance)
+from parity import (cancellation_allowance, line_centre_allowance, saturated_source, selthin_source_allowance,
+                    spectrum_excess, total_allowance)
 
 pytestmark = pytest.mark.gpu
 
@@ -57,11 +57,12 @@ def allowance(cfg, f, ref):
     o_sub = ref if cfg.subtract_continuum else Oracle(cfg.with_(subtract_continuum=True)).observe(f)
     o_tot = ref if not cfg.subtract_continuum else Oracle(cfg.with_(subtract_continuum=False)).observe(f)
     plain = 3e-7 * np.abs(o_tot).max(axis=-1, keepdims=True)
-    extra = total_allowance(o_tot, o_sub) + line_centre_allowance(cfg, o_sub)
+    sat = saturated_source(cfg, f) if cfg.transfer_mode == 0 else None
+    extra = total_allowance(o_tot, o_sub) + line_centre_allowance(cfg, o_sub, sat)
     if cfg.transfer_mode == 1:
         extra = extra + selthin_source_allowance(cfg, f).reshape(ref.shape)
     if cfg.transfer_mode == 0:
-        extra = extra + cancellation_allowance(cfg, f).reshape(ref.shape)
+        extra = extra + cancellation_allowance(cfg, f, saturated=sat).reshape(ref.shape)
     return plain, extra
 
 
