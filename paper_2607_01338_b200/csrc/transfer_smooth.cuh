@@ -332,12 +332,13 @@ transfer_smooth_window_kernel(MarchConsts mc, const float* __restrict__ coef, in
         // NP passes of a lane written stage by stage (loads, profile, step, stores): the passes are independent, but
         // the compiler cannot move a load of the next pass above a store of this one, and a pass alone is one
         // dependent chain LDS -> MUFU -> FMA -> MUFU -> STS that the few resident warps do not cover
-        auto passes = [&](auto np_tag, int k) {
+        int wk = IDX(k0);                            // word of the lane's pair in the pass at hand
+        auto passes = [&](auto np_tag, int) {
           constexpr int NP = decltype(np_tag)::value;
           f32x2 Uv[NP], Vv[NP], pw[NP];
 #pragma unroll
           for (int q = 0; q < NP; ++q) {
-            const int w = IDX(k + 2 * LPP * q);
+            const int w = wk + 64 * q;               // = IDX(k + 2 LPP q): a pass is two rows of the pixel further
             IRIS_CHECK_SMEM(cur + w, 8, lo_ok, hi_ok);
             IRIS_CHECK_SMEM(prv + w, 8, lo_ok, hi_ok);
             const float2 Uo = *reinterpret_cast<const float2*>(cur + w), Vo = *reinterpret_cast<const float2*>(prv + w);
@@ -363,13 +364,14 @@ transfer_smooth_window_kernel(MarchConsts mc, const float* __restrict__ coef, in
           }
 #pragma unroll
           for (int q = 0; q < NP; ++q) {
-            const int kq = k + 2 * LPP * q;
             float2 Un;
             upk(Uv[q], Un.x, Un.y);
-            if (kq + 1 >= npts) Un.y = 0.0f;                                           // padding, not a point
-            *reinterpret_cast<float2*>(prv + IDX(kq)) = Un;
+            // (a pair may end on the padding point npts of the last row: it gets the value the step gives there, nobody
+            // reads it as a point, and through u_min it can only make the hand-over test more careful)
+            *reinterpret_cast<float2*>(prv + wk + 64 * q) = Un;
             u_min = fminf(u_min, fminf(Un.x, Un.y));
           }
+          wk += 64 * NP;
         };
         int k = k0;
         for (; k + 2 * LPP <= ehi; k += 4 * LPP) passes(std::integral_constant<int, 2>{}, k);
