@@ -99,7 +99,7 @@ struct SmoothProfile {
 };
 
 // Records of phase A (one per lane = (pixel g, cell j of the chunk)), field-major in shared memory: rec[f * 32 + lane]
-//   f0 = { g2 = 2 (e_c - a_c C_n), a2 = 2 a_c, den0 = 3 + 2 tau_d, 1 / d_n }
+//   f0 = { g2 = 2 (e_c - a_c C_n), a2 = 2 a_c, den0 = 3 + 2 tau_d, 1 / d_n }   (point profile: g2, a2 times its amplitude p0)
 //   f1 = { 4 d_n-1, -d_n-2, relu_add, relu_min }
 //   f2 = { xb = s sqrt(log2 e) per point, (1/2 - c_los) xb, bits(elo | ehi << 16) of the hull, d_n }
 //   f3 = { p0, p1, p2, p3 }   profile polynomial (point profile: p0 only)
@@ -300,7 +300,9 @@ transfer_smooth_window_kernel(MarchConsts mc, const float* __restrict__ coef, in
       const float xb = s * SQL2E;
       const int elo = 0xffff - (int)(hull & 0xffffu), ehi = (int)(hull >> 16);
       const bool any = mine && ehi >= elo;
-      rec[lane] = make_float4(2.0f * fmaf(-a_c, C_unc, e_c), 2.0f * self_abs * a_c, fmaf(2.0f, td, 3.0f), rcp_approx(d_n));
+      // (point profile: its constant amplitude p0 is folded into the two line coefficients here, once per cell)
+      const float amp2 = POINT ? 2.0f * prof.p0 : 2.0f;
+      rec[lane] = make_float4(amp2 * fmaf(-a_c, C_unc, e_c), amp2 * self_abs * a_c, fmaf(2.0f, td, 3.0f), rcp_approx(d_n));
       rec[32 + lane] = make_float4(4.0f * d_n1, -d_n2, C_unc >= 0.0f ? 0.0f : C_unc, C_unc >= 0.0f ? -C_unc : 0.0f);
       rec[64 + lane] = make_float4(xb, (0.5f - c_los) * xb, __int_as_float(any ? (elo | (ehi << 16)) : 0x0000ffff), d_n);
       rec[96 + lane] = make_float4(prof.p0, prof.p1, prof.p2, prof.p3);
@@ -348,8 +350,7 @@ transfer_smooth_window_kernel(MarchConsts mc, const float* __restrict__ coef, in
             float u0, u1;
             upk(u, u0, u1);
             pw[q] = pk(ex2_approx(-u0), ex2_approx(-u1));
-            if (POINT) pw[q] = mul2(pw[q], pp0);
-            else pw[q] = mul2(pw[q], fma2(fma2(fma2(fma2(pp4, u, pp3), u, pp2), u, pp1), u, pp0));
+            if (!POINT) pw[q] = mul2(pw[q], fma2(fma2(fma2(fma2(pp4, u, pp3), u, pp2), u, pp1), u, pp0));
           }
 #pragma unroll
           for (int q = 0; q < NP; ++q) {
