@@ -943,12 +943,26 @@ iris_so_status iris_so_observe_host(iris_so_ctx* ctx, const float* h_nH2, const 
   cudaError_t e;
   // slab height: 128 MB of field data per slab (a sixth of the fields for smaller cubes), at least 3 slabs, else one shot
   const size_t row_bytes = (size_t)cfg0.nz * cfg0.nx * sizeof(float) * 4;
-  // (measured on the 512^3 cube, 2.1 GB of fields: 16 MB slabs 49.3 ms, 48 MB 48.5, 128 MB 43.3, 256 MB 44.8, 512 MB 47.4)
+  // (measured on the 512^3 cube, 2.1 GB of fields: 16 MB slabs 49.3 ms, 48 MB 48.5, 128 MB 43.3, 256 MB 44.8, 512 MB 47.4;
+  // with the last slab tapered as below: 44.6 -> 43.6 ms)
   const size_t slab_bytes = std::min<size_t>((size_t)128 << 20, std::max<size_t>((size_t)16 << 20, 4 * fb / 6));
   int rows = (int)std::max<size_t>(1, slab_bytes / std::max<size_t>(row_bytes, 1));
   rows = std::min(rows, cfg0.ny);
-  const int nslab = (cfg0.ny + rows - 1) / rows;
-  if (nslab < 3) {
+  // the slabs: equal heights, the last one cut into a half, a quarter and two eighths -- what follows the last H2D (K1-K5 and
+  // the D2H of that slab) is the part of the pipeline nothing overlaps with
+  std::vector<int> slab_y0, slab_ny;
+  for (int y = 0; y < cfg0.ny; y += rows) {
+    const int h = std::min(rows, cfg0.ny - y);
+    if (y + rows >= cfg0.ny && h >= 8) {
+      const int parts[4] = {h / 2, h / 4, h / 8, h - h / 2 - h / 4 - h / 8};
+      int yy = y;
+      for (int q = 0; q < 4; ++q) { slab_y0.push_back(yy); slab_ny.push_back(parts[q]); yy += parts[q]; }
+    } else {
+      slab_y0.push_back(y); slab_ny.push_back(h);
+    }
+  }
+  const int nslab = (int)slab_y0.size();
+  if ((cfg0.ny + rows - 1) / rows < 3) {
     for (int i = 0; i < 4; ++i)
       if ((e = cudaMemcpyAsync(f[i], h[i], fb, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_fail(ctx, e, "H2D copy");
     if ((s = iris_so_observe(ctx, f[0], f[1], f[2], f[3], d_cube, stream)) != IRIS_SO_OK) return s;
@@ -977,7 +991,7 @@ iris_so_status iris_so_observe_host(iris_so_ctx* ctx, const float* h_nH2, const 
   HOSTPATH_CU(cudaStreamWaitEvent(ctx->s_in, ev_start, 0), "cudaStreamWaitEvent");      // staging may still be in use on st
   HOSTPATH_CU(cudaStreamWaitEvent(ctx->s_out, ev_start, 0), "cudaStreamWaitEvent");
   for (int k = 0; k < nslab; ++k) {
-    const int y0 = k * rows, ny_k = std::min(rows, cfg0.ny - y0);
+    const int y0 = slab_y0[k], ny_k = slab_ny[k];
     const int64_t cells_before = (int64_t)cfg0.nz * y0 * cfg0.nx;         // compact slabs are stored back to back
     const size_t width = (size_t)ny_k * cfg0.nx * sizeof(float), spitch = (size_t)cfg0.ny * cfg0.nx * sizeof(float);
     for (int i = 0; i < 4; ++i)
